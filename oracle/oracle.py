@@ -1,0 +1,211 @@
+"""ctypes binding of the CPU oracle (oracle/otoo_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this.  It imports nothing from the product package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle.so")
+_SRC = os.path.join(_HERE, "otoo_oracle.c")
+
+CELL_DTYPE = np.dtype([("prefix", "<u8"), ("first", "<u4"), ("count", "<u4"), ("child_first", "<u4"),
+                       ("level", "u1"), ("child_count", "u1")], align=True)
+assert CELL_DTYPE.itemsize == 24
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so (gcc, -ffp-contract=off) if missing or stale."""
+    hdr = os.path.join(_HERE, "otoo_oracle.h")
+    if (not force and os.path.exists(_SO)
+            and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
+        return _SO
+    cmd = ["gcc", "-O2", "-std=c99", "-D_GNU_SOURCE", "-fopenmp", "-ffp-contract=off", "-fPIC",
+           "-shared", "-o", _SO, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        L = _lib
+        vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+        L.orc_build.restype = vp
+        L.orc_build.argtypes = [i64, vp, i32]
+        L.orc_free.argtypes = [vp]
+        L.orc_ncell.restype = i64
+        L.orc_ncell.argtypes = [vp]
+        L.orc_nleaf.restype = i64
+        L.orc_nleaf.argtypes = [vp]
+        L.orc_depth.restype = i32
+        L.orc_depth.argtypes = [vp]
+        L.orc_root.argtypes = [vp, vp, vp]
+        L.orc_export.argtypes = [vp] * 7
+        L.orc_key.restype = C.c_uint64
+        L.orc_key.argtypes = [vp, vp]
+        L.orc_rb2.argtypes = [vp, dbl, i32, vp]
+        L.orc_direct_sum.argtypes = [i64, vp, dbl, i64, vp, vp]
+        L.orc_gravity.restype = C.c_uint64
+        L.orc_gravity.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, vp, vp, vp]
+        L.orc_group_lists.argtypes = [vp, dbl, i32, i32, i64, vp, vp]
+        L.orc_sph_cell_radii.argtypes = [vp, vp, vp, vp]
+        L.orc_sph_density.restype = C.c_uint64
+        L.orc_sph_density.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+        L.orc_sph_group_list.argtypes = [vp, vp, i32, i64, vp]
+        L.orc_sph_force.restype = C.c_uint64
+        L.orc_sph_force.argtypes = [vp, vp, vp, vp, vp, i32, vp]
+        L.orc_W.restype = dbl
+        L.orc_W.argtypes = [dbl, dbl]
+        L.orc_dWdr.restype = dbl
+        L.orc_dWdr.argtypes = [dbl, dbl]
+        L.orc_max_threads.restype = i32
+        L.orc_set_threads.argtypes = [i32]
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if shape is not None:
+        assert a.shape == shape, (a.shape, shape)
+    return a
+
+
+def max_threads() -> int:
+    return lib().orc_max_threads()
+
+
+def set_threads(n: int) -> None:
+    lib().orc_set_threads(int(n))
+
+
+def direct_sum(pos_mass, eps, targets=None):
+    pm = _f32(pos_mass)
+    n = pm.shape[0]
+    if targets is None:
+        out = np.empty((n, 4), dtype=np.float64)
+        lib().orc_direct_sum(n, _p(pm), float(eps), 0, None, _p(out))
+    else:
+        tg = np.ascontiguousarray(targets, dtype=np.int64)
+        out = np.empty((len(tg), 4), dtype=np.float64)
+        lib().orc_direct_sum(n, _p(pm), float(eps), len(tg), _p(tg), _p(out))
+    return out
+
+
+def W(r, h):
+    return lib().orc_W(float(r), float(h))
+
+
+def dWdr(r, h):
+    return lib().orc_dWdr(float(r), float(h))
+
+
+class Tree:
+    """Oracle tree: PAPER.md III-B (build) + III-C (cell properties)."""
+
+    def __init__(self, pos_mass, n_crit=16):
+        self.pm = _f32(pos_mass)
+        assert self.pm.ndim == 2 and self.pm.shape[1] == 4
+        self.N = self.pm.shape[0]
+        self.n_crit = int(n_crit)
+        self._h = lib().orc_build(self.N, _p(self.pm), self.n_crit)
+        self.ncell = lib().orc_ncell(self._h)
+        self.nleaf = lib().orc_nleaf(self._h)
+        self.depth = lib().orc_depth(self._h)
+        lo = np.empty(3, dtype=np.float32)
+        S = np.empty(1, dtype=np.float32)
+        lib().orc_root(self._h, _p(lo), _p(S))
+        self.lo, self.S = lo, float(S[0])
+
+    def __del__(self):
+        try:
+            if self._h:
+                lib().orc_free(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    def export(self):
+        perm = np.empty(self.N, dtype=np.uint32)
+        keys = np.empty(self.N, dtype=np.uint64)
+        cells = np.zeros(self.ncell, dtype=CELL_DTYPE)
+        com_m = np.empty((self.ncell, 4), dtype=np.float32)
+        s = np.empty(self.ncell, dtype=np.float64)
+        MP = np.empty((self.ncell, 4), dtype=np.float64)
+        lib().orc_export(self._h, _p(perm), _p(keys), _p(cells), _p(com_m), _p(s), _p(MP))
+        return dict(perm=perm, keys=keys, cells=cells, com_m=com_m, s=s, MP=MP)
+
+    def key(self, xyz):
+        a = _f32(xyz, (3,))
+        return int(lib().orc_key(self._h, _p(a)))
+
+    def rb2(self, theta, mac_kind=0):
+        out = np.empty(self.ncell, dtype=np.float32)
+        lib().orc_rb2(self._h, float(theta), int(mac_kind), _p(out))
+        return out
+
+    def n_groups(self, G):
+        return (self.N + G - 1) // G
+
+    def gravity(self, eps, theta, group_size, mac_kind=0, walk_kind=0, forces=True):
+        ng = self.n_groups(group_size)
+        acc = np.zeros((self.N, 4), dtype=np.float64) if forces else None
+        nt = np.zeros(ng, dtype=np.uint32)
+        nc = np.zeros(ng, dtype=np.uint32)
+        npart = np.zeros(ng, dtype=np.uint32)
+        tot = lib().orc_gravity(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
+                                int(walk_kind), _p(acc), _p(nt), _p(nc), _p(npart))
+        return dict(acc_pot=acc, n_tests=nt, n_cells=nc, n_parts=npart, interactions=int(tot))
+
+    def group_lists(self, theta, group_size, g, n_cells, n_parts, mac_kind=0):
+        cells = np.empty(max(int(n_cells), 1), dtype=np.uint32)
+        parts = np.empty(max(int(n_parts), 1), dtype=np.uint32)
+        lib().orc_group_lists(self._h, float(theta), int(group_size), int(mac_kind), int(g),
+                              _p(cells), _p(parts))
+        return cells[:int(n_cells)], parts[:int(n_parts)]
+
+    def sph_cell_radii(self, h):
+        h = _f32(h, (self.N,))
+        b = np.empty(self.ncell, dtype=np.float32)
+        r = np.empty(self.ncell, dtype=np.float32)
+        lib().orc_sph_cell_radii(self._h, _p(h), _p(b), _p(r))
+        return b, r
+
+    def sph_density(self, h, group_size, sums=True):
+        h = _f32(h, (self.N,))
+        ng = self.n_groups(group_size)
+        rho = np.zeros(self.N, dtype=np.float64) if sums else None
+        nngb = np.zeros(self.N, dtype=np.uint32)
+        nt = np.zeros(ng, dtype=np.uint32)
+        npart = np.zeros(ng, dtype=np.uint32)
+        tot = lib().orc_sph_density(self._h, _p(h), int(group_size), _p(rho), _p(nngb), _p(nt), _p(npart))
+        return dict(rho=rho, nngb=nngb, n_tests=nt, n_parts=npart, candidates=int(tot))
+
+    def sph_group_list(self, h, group_size, g, n_parts):
+        h = _f32(h, (self.N,))
+        parts = np.empty(max(int(n_parts), 1), dtype=np.uint32)
+        lib().orc_sph_group_list(self._h, _p(h), int(group_size), int(g), _p(parts))
+        return parts[:int(n_parts)]
+
+    def sph_force(self, h, rho, P, group_size, vel=None):
+        h = _f32(h, (self.N,))
+        rho = np.ascontiguousarray(rho, dtype=np.float64)
+        P = np.ascontiguousarray(P, dtype=np.float64)
+        v = None if vel is None else _f32(vel, (self.N, 4))
+        out = np.zeros((self.N, 4), dtype=np.float64)
+        tot = lib().orc_sph_force(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(out))
+        return dict(acc_dudt=out, candidates=int(tot))

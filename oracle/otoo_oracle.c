@@ -1,0 +1,600 @@
+/* otoo_oracle.c -- see otoo_oracle.h.  TEST INFRASTRUCTURE ONLY; plain C99 + OpenMP.
+ * Compile with -ffp-contract=off so that no a*b+c is fused behind our back; fmaf() is used
+ * where DESIGN.md's readings state a fused operation.
+ * Citations are PAPER.md line numbers (L..) and DESIGN.md readings (R..). */
+#include "otoo_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define MAXLEV 21
+
+struct orc_tree {
+  int64_t N;
+  int n_crit;
+  float lo[3], S;
+  uint64_t* key;  /* sorted keys */
+  uint32_t* perm; /* perm[s] = original index of sorted slot s */
+  float* spos;    /* sorted (x,y,z,m) */
+  int64_t ncell, cap, nleaf;
+  int depth;
+  orc_cell* cell; /* canonical order after build */
+  double* MP;     /* 4*ncell: M, Px, Py, Pz (unnormalised first moment), R6 */
+  double* cm;     /* 3*ncell fp64 centre of mass */
+  float* com_m;   /* 4*ncell fp32 (cm, m) as the walk sees them */
+  double* s;      /* distance CM - geometric centre, R7 */
+  /* paper-style linked list (L49-L57, L135): node < N particle slot, node >= N cell N+id */
+  int64_t* next;
+  int64_t* more;
+};
+
+/* ---------------- R1-R4: root cube, keys, sort (PAPER III-B steps 1-3, L121-L133) --------- */
+static uint64_t key_of(const float lo[3], float scale, const float* p) {
+  uint32_t q[3];
+  for (int k = 0; k < 3; k++) {
+    float d = p[k] - lo[k];         /* one fp32 subtract */
+    float t = d * scale;            /* one fp32 multiply */
+    uint32_t v = (t >= 2097151.0f) ? 2097151u : (t > 0.0f ? (uint32_t)t : 0u);
+    q[k] = v;
+  }
+  uint64_t key = 0;
+  for (int lev = 1; lev <= MAXLEV; lev++) { /* L129: concatenation of the octant index per level */
+    int b = MAXLEV - lev;
+    uint64_t oct = (((q[0] >> b) & 1u) << 2) | (((q[1] >> b) & 1u) << 1) | ((q[2] >> b) & 1u);
+    key |= oct << (3 * b);
+  }
+  return key;
+}
+
+typedef struct { uint64_t key; uint32_t id; } kv_t;
+static int kv_cmp(const void* a, const void* b) {
+  const kv_t* x = (const kv_t*)a; const kv_t* y = (const kv_t*)b;
+  if (x->key != y->key) return x->key < y->key ? -1 : 1;
+  if (x->id != y->id) return x->id < y->id ? -1 : 1;   /* R4: ties by original index */
+  return 0;
+}
+
+static int64_t new_cell(orc_tree* t) {
+  if (t->ncell == t->cap) {
+    t->cap = t->cap ? 2 * t->cap : 1024;
+    t->cell = (orc_cell*)realloc(t->cell, sizeof(orc_cell) * t->cap);
+  }
+  return t->ncell++;
+}
+
+/* R5 / L135: slice the sorted keys by octant index, recursively; leaf iff count <= n_crit or
+ * level 21.  Cells are created in depth-first order here and renumbered afterwards. */
+static void split(orc_tree* t, int64_t id) {
+  orc_cell c = t->cell[id];
+  if (c.count <= (uint32_t)t->n_crit || c.level == MAXLEV) { t->nleaf++; return; }
+  int shift = 3 * (MAXLEV - (c.level + 1));
+  int64_t kids[8]; int nk = 0;
+  uint32_t s = c.first, end = c.first + c.count;
+  while (s < end) {
+    uint64_t oct = (t->key[s] >> shift) & 7u;
+    uint32_t e = s;
+    while (e < end && ((t->key[e] >> shift) & 7u) == oct) e++;
+    int64_t k = new_cell(t);
+    t->cell[k].prefix = t->key[s] >> shift;
+    t->cell[k].first = s; t->cell[k].count = e - s;
+    t->cell[k].level = (uint8_t)(c.level + 1);
+    t->cell[k].child_first = 0; t->cell[k].child_count = 0;
+    kids[nk++] = k;
+    s = e;
+  }
+  t->cell[id].child_first = (uint32_t)kids[0];   /* the nk children were created consecutively */
+  t->cell[id].child_count = (uint8_t)nk;
+  for (int i = 0; i < nk; i++) split(t, kids[i]);
+}
+
+typedef struct { orc_cell c; int64_t old; } cs_t;
+static int cs_cmp(const void* a, const void* b) {
+  const cs_t* x = (const cs_t*)a; const cs_t* y = (const cs_t*)b;
+  if (x->c.level != y->c.level) return x->c.level < y->c.level ? -1 : 1;
+  if (x->c.first != y->c.first) return x->c.first < y->c.first ? -1 : 1;
+  return 0;
+}
+
+static void cell_coord(uint64_t prefix, int level, uint32_t c[3]) {
+  c[0] = c[1] = c[2] = 0;
+  for (int i = 0; i < level; i++) {
+    uint64_t oct = (prefix >> (3 * i)) & 7u;
+    c[0] |= (uint32_t)((oct >> 2) & 1u) << i;
+    c[1] |= (uint32_t)((oct >> 1) & 1u) << i;
+    c[2] |= (uint32_t)(oct & 1u) << i;
+  }
+}
+
+/* R6 / L155: recursive depth-first mass and first moment, fp64, fixed order. */
+static void moments(orc_tree* t, int64_t id) {
+  orc_cell* c = &t->cell[id];
+  double M = 0, Px = 0, Py = 0, Pz = 0;
+  if (c->child_count == 0) {
+    for (uint32_t s = c->first; s < c->first + c->count; s++) {
+      const float* p = t->spos + 4 * (int64_t)s;
+      double m = p[3];
+      M = M + m;
+      Px = Px + m * (double)p[0];
+      Py = Py + m * (double)p[1];
+      Pz = Pz + m * (double)p[2];
+    }
+  } else {
+    for (int k = 0; k < c->child_count; k++) {
+      int64_t ch = (int64_t)c->child_first + k;
+      moments(t, ch);
+      M = M + t->MP[4 * ch];
+      Px = Px + t->MP[4 * ch + 1];
+      Py = Py + t->MP[4 * ch + 2];
+      Pz = Pz + t->MP[4 * ch + 3];
+    }
+  }
+  t->MP[4 * id] = M; t->MP[4 * id + 1] = Px; t->MP[4 * id + 2] = Py; t->MP[4 * id + 3] = Pz;
+  /* geometric centre and s (R7) */
+  uint32_t cc[3]; cell_coord(c->prefix, c->level, cc);
+  double l = ldexp((double)t->S, -(int)c->level);
+  double g[3];
+  for (int k = 0; k < 3; k++) g[k] = (double)t->lo[k] + ((double)cc[k] + 0.5) * l;
+  double cm[3];
+  if (M != 0.0) { cm[0] = Px / M; cm[1] = Py / M; cm[2] = Pz / M; }
+  else { cm[0] = g[0]; cm[1] = g[1]; cm[2] = g[2]; }
+  for (int k = 0; k < 3; k++) { t->cm[3 * id + k] = cm[k]; t->com_m[4 * id + k] = (float)cm[k]; }
+  t->com_m[4 * id + 3] = (float)M;
+  double dx = cm[0] - g[0], dy = cm[1] - g[1], dz = cm[2] - g[2];
+  t->s[id] = sqrt((dx * dx + dy * dy) + dz * dz);
+}
+
+orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit) {
+  orc_tree* t = (orc_tree*)calloc(1, sizeof(orc_tree));
+  t->N = N; t->n_crit = n_crit;
+  /* R1 / L121,L127: cube enclosing all particles, anchored at the lo corner */
+  float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+  for (int64_t i = 0; i < N; i++)
+    for (int k = 0; k < 3; k++) {
+      float v = pos_mass[4 * i + k];
+      if (i == 0 || v < lo[k]) lo[k] = v;
+      if (i == 0 || v > hi[k]) hi[k] = v;
+    }
+  float S = 0.0f;
+  for (int k = 0; k < 3; k++) { float d = hi[k] - lo[k]; if (d > S) S = d; t->lo[k] = lo[k]; }
+  if (!(S > 0.0f)) S = 1.0f;
+  t->S = S;
+  float scale = 2097152.0f / S;   /* R2: IEEE fp32 division */
+  kv_t* kv = (kv_t*)malloc(sizeof(kv_t) * (N > 0 ? N : 1));
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < N; i++) { kv[i].key = key_of(lo, scale, pos_mass + 4 * i); kv[i].id = (uint32_t)i; }
+  qsort(kv, (size_t)N, sizeof(kv_t), kv_cmp);   /* L133 */
+  t->key = (uint64_t*)malloc(8 * (N > 0 ? N : 1));
+  t->perm = (uint32_t*)malloc(4 * (N > 0 ? N : 1));
+  t->spos = (float*)malloc(16 * (N > 0 ? N : 1));
+  for (int64_t s = 0; s < N; s++) {
+    t->key[s] = kv[s].key; t->perm[s] = kv[s].id;
+    memcpy(t->spos + 4 * s, pos_mass + 4 * (int64_t)kv[s].id, 16);
+  }
+  free(kv);
+  /* R5: topology */
+  int64_t root = new_cell(t);
+  t->cell[root].prefix = 0; t->cell[root].first = 0; t->cell[root].count = (uint32_t)N;
+  t->cell[root].level = 0; t->cell[root].child_first = 0; t->cell[root].child_count = 0;
+  split(t, root);
+  /* canonical renumbering: level ascending, then first ascending */
+  cs_t* cs = (cs_t*)malloc(sizeof(cs_t) * t->ncell);
+  for (int64_t i = 0; i < t->ncell; i++) { cs[i].c = t->cell[i]; cs[i].old = i; }
+  qsort(cs, (size_t)t->ncell, sizeof(cs_t), cs_cmp);
+  int64_t* newid = (int64_t*)malloc(8 * t->ncell);
+  for (int64_t i = 0; i < t->ncell; i++) newid[cs[i].old] = i;
+  t->depth = 0;
+  for (int64_t i = 0; i < t->ncell; i++) {
+    t->cell[i] = cs[i].c;
+    if (t->cell[i].child_count) t->cell[i].child_first = (uint32_t)newid[cs[i].c.child_first];
+    if (t->cell[i].level > t->depth) t->depth = t->cell[i].level;
+  }
+  free(cs); free(newid);
+  /* R6, R7 */
+  t->MP = (double*)malloc(32 * t->ncell);
+  t->cm = (double*)malloc(24 * t->ncell);
+  t->com_m = (float*)malloc(16 * t->ncell);
+  t->s = (double*)malloc(8 * t->ncell);
+  moments(t, 0);
+  /* L49-L57, L135: next/more linked list, particles 0..N-1, cells N.. */
+  t->next = (int64_t*)malloc(8 * (N + t->ncell));
+  t->more = (int64_t*)malloc(8 * (N + t->ncell));
+  for (int64_t i = 0; i < N; i++) t->more[i] = -1;
+  t->next[N + 0] = -1;
+  for (int64_t id = 0; id < t->ncell; id++) {   /* parents precede children in canonical order */
+    orc_cell* c = &t->cell[id];
+    int64_t after = t->next[N + id];
+    if (c->child_count == 0) {
+      if (c->count == 0) { t->more[N + id] = after; continue; }
+      t->more[N + id] = c->first;
+      for (uint32_t s = c->first; s < c->first + c->count; s++)
+        t->next[s] = (s + 1 < c->first + c->count) ? (int64_t)(s + 1) : after;
+    } else {
+      t->more[N + id] = N + c->child_first;
+      for (int k = 0; k < c->child_count; k++)
+        t->next[N + c->child_first + k] = (k + 1 < c->child_count) ? N + c->child_first + k + 1 : after;
+    }
+  }
+  return t;
+}
+
+void orc_free(orc_tree* t) {
+  if (!t) return;
+  free(t->key); free(t->perm); free(t->spos); free(t->cell); free(t->MP); free(t->cm);
+  free(t->com_m); free(t->s); free(t->next); free(t->more); free(t);
+}
+int64_t orc_ncell(const orc_tree* t) { return t->ncell; }
+int64_t orc_nleaf(const orc_tree* t) { return t->nleaf; }
+int orc_depth(const orc_tree* t) { return t->depth; }
+void orc_root(const orc_tree* t, float lo[3], float* S) { memcpy(lo, t->lo, 12); *S = t->S; }
+uint64_t orc_key(const orc_tree* t, const float xyz[3]) { return key_of(t->lo, 2097152.0f / t->S, xyz); }
+
+void orc_export(const orc_tree* t, uint32_t* perm, uint64_t* keys, orc_cell* cells, float* com_m,
+                double* s, double* MP) {
+  if (perm) memcpy(perm, t->perm, 4 * t->N);
+  if (keys) memcpy(keys, t->key, 8 * t->N);
+  if (cells) memcpy(cells, t->cell, sizeof(orc_cell) * t->ncell);
+  if (com_m) memcpy(com_m, t->com_m, 16 * t->ncell);
+  if (s) memcpy(s, t->s, 8 * t->ncell);
+  if (MP) memcpy(MP, t->MP, 32 * t->ncell);
+}
+
+/* ---------------- direct sum: the plain O(N^2) definition (L43 "O(N^2) ... brute force") ----- */
+void orc_direct_sum(int64_t N, const float* pm, double eps, int64_t nt, const int64_t* targets,
+                    double* out) {
+  int64_t T = targets ? nt : N;
+  double e2 = eps * eps;
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t t = 0; t < T; t++) {
+    int64_t i = targets ? targets[t] : t;
+    double xi = pm[4 * i], yi = pm[4 * i + 1], zi = pm[4 * i + 2];
+    double ax = 0, ay = 0, az = 0, ph = 0;
+    for (int64_t j = 0; j < N; j++) {
+      if (j == i) continue;
+      double dx = (double)pm[4 * j] - xi, dy = (double)pm[4 * j + 1] - yi, dz = (double)pm[4 * j + 2] - zi;
+      double r2 = dx * dx + dy * dy + dz * dz + e2;
+      if (r2 == 0.0) continue;
+      double ri = 1.0 / sqrt(r2);
+      double m = pm[4 * j + 3];
+      double mr3 = m * ri * ri * ri;
+      ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= m * ri;
+    }
+    out[4 * t] = ax; out[4 * t + 1] = ay; out[4 * t + 2] = az; out[4 * t + 3] = ph;
+  }
+}
+
+/* ---------------- R7: theta-MAC bounding radius (the paper's r_b abstraction, L61) ---------- */
+void orc_rb2(const orc_tree* t, double theta, int mac_kind, float* rb2) {
+  for (int64_t id = 0; id < t->ncell; id++) {
+    if (theta <= 0.0) { rb2[id] = INFINITY; continue; }
+    double l = ldexp((double)t->S, -(int)t->cell[id].level);
+    double rb = l / theta;
+    if (mac_kind == 0) rb = rb + t->s[id];
+    rb2[id] = (float)(rb * rb);
+  }
+}
+
+/* ---------------- R8: group AABB and group-cell distance (L163, Barnes 1990 form) ----------- */
+typedef struct { float lo[3], hi[3]; float hmax; } gbox_t;
+static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs /*sorted h or NULL*/) {
+  gbox_t g; g.hmax = 0.0f;
+  for (int k = 0; k < 3; k++) { g.lo[k] = t->spos[4 * a + k]; g.hi[k] = g.lo[k]; }
+  for (int64_t s = a; s < b; s++) {
+    for (int k = 0; k < 3; k++) {
+      float v = t->spos[4 * s + k];
+      if (v < g.lo[k]) g.lo[k] = v;
+      if (v > g.hi[k]) g.hi[k] = v;
+    }
+    if (hs && hs[s] > g.hmax) g.hmax = hs[s];
+  }
+  return g;
+}
+static float box_d2(const gbox_t* g, const float* cm) {
+  float e[3];
+  for (int k = 0; k < 3; k++) {
+    float a = g->lo[k] - cm[k], b = cm[k] - g->hi[k];
+    float m = a > b ? a : b;
+    e[k] = m > 0.0f ? m : 0.0f;
+  }
+  return fmaf(e[2], e[2], fmaf(e[1], e[1], e[0] * e[0]));
+}
+
+typedef struct {
+  uint32_t *cells, *parts; int64_t nc, np, capc, capp; uint32_t ntests;
+} lists_t;
+static void push_u32(uint32_t** a, int64_t* n, int64_t* cap, uint32_t v) {
+  if (*n == *cap) { *cap = *cap ? 2 * *cap : 4096; *a = (uint32_t*)realloc(*a, 4 * *cap); }
+  (*a)[(*n)++] = v;
+}
+
+/* R9 / L57 rules as a recursion: accepted -> cell list; not accepted leaf -> its particles;
+ * otherwise descend.  Particles are never MAC-tested (rule 3). */
+static void walk_rec(const orc_tree* t, const float* rb2, const gbox_t* g, int64_t id, lists_t* L) {
+  const orc_cell* c = &t->cell[id];
+  L->ntests++;
+  float d2 = box_d2(g, t->com_m + 4 * id);
+  if (d2 > rb2[id]) { push_u32(&L->cells, &L->nc, &L->capc, (uint32_t)id); return; }
+  if (c->child_count == 0) {
+    for (uint32_t s = c->first; s < c->first + c->count; s++) push_u32(&L->parts, &L->np, &L->capp, s);
+    return;
+  }
+  for (int k = 0; k < c->child_count; k++) walk_rec(t, rb2, g, (int64_t)c->child_first + k, L);
+}
+/* The paper's own iterative traversal, literally (L57 rules 1-4). */
+static void walk_stackless(const orc_tree* t, const float* rb2, const gbox_t* g, lists_t* L) {
+  int64_t N = t->N, node = N;                       /* start from the root cell */
+  while (node != -1) {                              /* (4) null pointer: stop */
+    if (node < N) {                                 /* (3) particle: interact, follow next */
+      push_u32(&L->parts, &L->np, &L->capp, (uint32_t)node);
+      node = t->next[node];
+    } else {
+      int64_t id = node - N;
+      L->ntests++;
+      float d2 = box_d2(g, t->com_m + 4 * id);
+      if (d2 > rb2[id]) {                           /* (2) accepted: interact, follow next */
+        push_u32(&L->cells, &L->nc, &L->capc, (uint32_t)id);
+        node = t->next[node];
+      } else node = t->more[node];                  /* (1) not accepted: follow more */
+    }
+  }
+}
+
+/* R10: softened Plummer sums, fp64, with the fp32-rounded cell data the walk uses. */
+static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double e2, double* out) {
+  const float* p = t->spos + 4 * slot;
+  double xi = p[0], yi = p[1], zi = p[2];
+  double ax = 0, ay = 0, az = 0, ph = 0;
+  for (int64_t k = 0; k < L->nc; k++) {
+    const float* c = t->com_m + 4 * (int64_t)L->cells[k];
+    double dx = (double)c[0] - xi, dy = (double)c[1] - yi, dz = (double)c[2] - zi;
+    double r2 = dx * dx + dy * dy + dz * dz + e2;
+    if (r2 == 0.0) continue;
+    double ri = 1.0 / sqrt(r2), m = c[3];
+    double mr3 = m * ri * ri * ri;
+    ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= m * ri;
+  }
+  for (int64_t k = 0; k < L->np; k++) {
+    int64_t j = L->parts[k];
+    if (j == slot) continue;                        /* self term excluded by index */
+    const float* q = t->spos + 4 * j;
+    double dx = (double)q[0] - xi, dy = (double)q[1] - yi, dz = (double)q[2] - zi;
+    double r2 = dx * dx + dy * dy + dz * dz + e2;
+    if (r2 == 0.0) continue;
+    double ri = 1.0 / sqrt(r2), m = q[3];
+    double mr3 = m * ri * ri * ri;
+    ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= m * ri;
+  }
+  out[0] = ax; out[1] = ay; out[2] = az; out[3] = ph;
+}
+
+uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
+                     double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts) {
+  int64_t N = t->N, ng = (N + G - 1) / G;
+  float* rb2 = (float*)malloc(4 * t->ncell);
+  orc_rb2(t, theta, mac_kind, rb2);
+  double e2 = eps * eps;
+  uint64_t total = 0;
+#pragma omp parallel reduction(+ : total)
+  {
+    lists_t L; memset(&L, 0, sizeof L);
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t g = 0; g < ng; g++) {
+      int64_t a = g * G, b = a + G < N ? a + G : N;
+      gbox_t box = group_box(t, a, b, NULL);
+      L.nc = L.np = 0; L.ntests = 0;
+      if (walk_kind == 0) walk_rec(t, rb2, &box, 0, &L); else walk_stackless(t, rb2, &box, &L);
+      if (n_tests) n_tests[g] = L.ntests;
+      if (n_cells) n_cells[g] = (uint32_t)L.nc;
+      if (n_parts) n_parts[g] = (uint32_t)L.np;
+      total += (uint64_t)(b - a) * (uint64_t)(L.nc + L.np);   /* R11 */
+      if (acc_pot)
+        for (int64_t s = a; s < b; s++) grav_sums(t, &L, s, e2, acc_pot + 4 * (int64_t)t->perm[s]);
+    }
+    free(L.cells); free(L.parts);
+  }
+  free(rb2);
+  return total;
+}
+
+void orc_group_lists(const orc_tree* t, double theta, int G, int mac_kind, int64_t g,
+                     uint32_t* cell_ids, uint32_t* part_slots) {
+  float* rb2 = (float*)malloc(4 * t->ncell);
+  orc_rb2(t, theta, mac_kind, rb2);
+  int64_t a = g * G, b = a + G < t->N ? a + G : t->N;
+  gbox_t box = group_box(t, a, b, NULL);
+  lists_t L; memset(&L, 0, sizeof L);
+  walk_rec(t, rb2, &box, 0, &L);
+  if (cell_ids) memcpy(cell_ids, L.cells, 4 * L.nc);
+  if (part_slots) memcpy(part_slots, L.parts, 4 * L.np);
+  free(L.cells); free(L.parts); free(rb2);
+}
+
+/* ---------------- SPH (PAPER II-C, L85-L105; readings R13-R17) ------------------------------ */
+/* R13: cubic spline, h = support radius (L89: W "is zero outside of a given neighbor radius h") */
+double orc_W(double r, double h) {
+  double q = r / h, sig = 8.0 / (M_PI * h * h * h);
+  if (q <= 0.5) return sig * (1.0 - 6.0 * q * q + 6.0 * q * q * q);
+  if (q < 1.0) { double u = 1.0 - q; return sig * 2.0 * u * u * u; }
+  return 0.0;
+}
+double orc_dWdr(double r, double h) {
+  double q = r / h, sig = 8.0 / (M_PI * h * h * h * h);
+  if (q <= 0.5) return sig * (-12.0 * q + 18.0 * q * q);
+  if (q < 1.0) { double u = 1.0 - q; return sig * (-6.0 * u * u); }
+  return 0.0;
+}
+
+static float* sorted_h(const orc_tree* t, const float* h) {
+  float* hs = (float*)malloc(4 * (t->N > 0 ? t->N : 1));
+  for (int64_t s = 0; s < t->N; s++) hs[s] = h[t->perm[s]];
+  return hs;
+}
+static float up32(double v) { /* fp32 rounded up (R14) */
+  float f = (float)v;
+  if ((double)f < v) f = nextafterf(f, INFINITY);
+  return f;
+}
+/* R14 / Eq. 5 (L101-L105): per cell, over ALL particles of the cell, from the fp64 CM. */
+static void sph_radii_sorted(const orc_tree* t, const float* hs, float* bmax, float* rsph) {
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t id = 0; id < t->ncell; id++) {
+    const orc_cell* c = &t->cell[id];
+    double b = 0.0, r = 0.0;
+    for (uint32_t s = c->first; s < c->first + c->count; s++) {
+      const float* p = t->spos + 4 * (int64_t)s;
+      double dx = (double)p[0] - t->cm[3 * id], dy = (double)p[1] - t->cm[3 * id + 1], dz = (double)p[2] - t->cm[3 * id + 2];
+      double d = sqrt((dx * dx + dy * dy) + dz * dz);
+      if (d > b) b = d;
+      double dh = d + (double)hs[s];
+      if (dh > r) r = dh;
+    }
+    bmax[id] = up32(b); rsph[id] = up32(r);
+  }
+}
+void orc_sph_cell_radii(const orc_tree* t, const float* h, float* bmax, float* rsph) {
+  float* hs = sorted_h(t, h);
+  sph_radii_sorted(t, hs, bmax, rsph);
+  free(hs);
+}
+
+/* R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); no cell list (L105). */
+static void walk_sph(const orc_tree* t, const float* bmax, const float* rsph, const gbox_t* g,
+                     int64_t id, lists_t* L) {
+  const orc_cell* c = &t->cell[id];
+  L->ntests++;
+  float d2 = box_d2(g, t->com_m + 4 * id);
+  float R = fmaxf(rsph[id], bmax[id] + g->hmax);
+  float R2 = R * R;
+  if (!(d2 <= R2)) return;
+  if (c->child_count == 0) {
+    for (uint32_t s = c->first; s < c->first + c->count; s++) push_u32(&L->parts, &L->np, &L->capp, s);
+    return;
+  }
+  for (int k = 0; k < c->child_count; k++) walk_sph(t, bmax, rsph, g, (int64_t)c->child_first + k, L);
+}
+static float r2_f32(const float* a, const float* b) { /* R16: the fp32 neighbour distance */
+  float dx = b[0] - a[0], dy = b[1] - a[1], dz = b[2] - a[2];
+  return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+}
+
+uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, uint32_t* nngb,
+                         uint32_t* n_tests, uint32_t* n_parts) {
+  int64_t N = t->N, ng = (N + G - 1) / G;
+  float* hs = sorted_h(t, h);
+  float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
+  sph_radii_sorted(t, hs, bmax, rsph);
+  uint64_t total = 0;
+#pragma omp parallel reduction(+ : total)
+  {
+    lists_t L; memset(&L, 0, sizeof L);
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t g = 0; g < ng; g++) {
+      int64_t a = g * G, b = a + G < N ? a + G : N;
+      gbox_t box = group_box(t, a, b, hs);
+      L.np = 0; L.ntests = 0;
+      walk_sph(t, bmax, rsph, &box, 0, &L);
+      if (n_tests) n_tests[g] = L.ntests;
+      if (n_parts) n_parts[g] = (uint32_t)L.np;
+      total += (uint64_t)(b - a) * (uint64_t)L.np;
+      for (int64_t s = a; s < b && rho; s++) {
+        const float* pi = t->spos + 4 * s;
+        float hi = hs[s], h2 = hi * hi;
+        double sum = 0.0; uint32_t cnt = 0;
+        for (int64_t k = 0; k < L.np; k++) {
+          const float* pj = t->spos + 4 * (int64_t)L.parts[k];
+          if (!(r2_f32(pi, pj) < h2)) continue;      /* R16: decision in fp32 */
+          double dx = (double)pj[0] - pi[0], dy = (double)pj[1] - pi[1], dz = (double)pj[2] - pi[2];
+          double r = sqrt(dx * dx + dy * dy + dz * dz);
+          sum += (double)pj[3] * orc_W(r, (double)hi);   /* Eq. 4 (L87) with A = m */
+          cnt++;
+        }
+        rho[t->perm[s]] = sum;
+        if (nngb) nngb[t->perm[s]] = cnt;
+      }
+    }
+    free(L.parts); free(L.cells);
+  }
+  free(hs); free(bmax); free(rsph);
+  return total;
+}
+
+void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uint32_t* part_slots) {
+  float* hs = sorted_h(t, h);
+  float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
+  sph_radii_sorted(t, hs, bmax, rsph);
+  int64_t a = g * G, b = a + G < t->N ? a + G : t->N;
+  gbox_t box = group_box(t, a, b, hs);
+  lists_t L; memset(&L, 0, sizeof L);
+  walk_sph(t, bmax, rsph, &box, 0, &L);
+  memcpy(part_slots, L.parts, 4 * L.np);
+  free(L.parts); free(L.cells); free(hs); free(bmax); free(rsph);
+}
+
+/* R17: symmetric pressure force (TREESPH/GADGET form) and optional du/dt. */
+uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, const double* P,
+                       const float* vel, int G, double* out) {
+  int64_t N = t->N, ng = (N + G - 1) / G;
+  float* hs = sorted_h(t, h);
+  float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
+  sph_radii_sorted(t, hs, bmax, rsph);
+  uint64_t total = 0;
+#pragma omp parallel reduction(+ : total)
+  {
+    lists_t L; memset(&L, 0, sizeof L);
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t g = 0; g < ng; g++) {
+      int64_t a = g * G, b = a + G < N ? a + G : N;
+      gbox_t box = group_box(t, a, b, hs);
+      L.np = 0; L.ntests = 0;
+      walk_sph(t, bmax, rsph, &box, 0, &L);
+      total += (uint64_t)(b - a) * (uint64_t)L.np;
+      for (int64_t s = a; s < b; s++) {
+        const float* pi = t->spos + 4 * s;
+        int64_t io = t->perm[s];
+        float hi = hs[s];
+        double pri = P[io] / (rho[io] * rho[io]);
+        double ax = 0, ay = 0, az = 0, du = 0;
+        for (int64_t k = 0; k < L.np; k++) {
+          int64_t j = L.parts[k];
+          if (j == s) continue;
+          const float* pj = t->spos + 4 * j;
+          float hj = hs[j], hm = hi > hj ? hi : hj;
+          if (!(r2_f32(pi, pj) < hm * hm)) continue;   /* decision in fp32 */
+          int64_t jo = t->perm[j];
+          double dx = (double)pi[0] - pj[0], dy = (double)pi[1] - pj[1], dz = (double)pi[2] - pj[2];
+          double r = sqrt(dx * dx + dy * dy + dz * dz);
+          if (r == 0.0) continue;
+          double gw = 0.5 * (orc_dWdr(r, (double)hi) + orc_dWdr(r, (double)hj)) / r;  /* grad_i W = gw * (xi-xj) */
+          double f = (double)pj[3] * (pri + P[jo] / (rho[jo] * rho[jo])) * gw;
+          ax -= f * dx; ay -= f * dy; az -= f * dz;
+          if (vel) {
+            double vx = (double)vel[4 * io] - vel[4 * jo], vy = (double)vel[4 * io + 1] - vel[4 * jo + 1],
+                   vz = (double)vel[4 * io + 2] - vel[4 * jo + 2];
+            du += 0.5 * f * (vx * dx + vy * dy + vz * dz);
+          }
+        }
+        out[4 * io] = ax; out[4 * io + 1] = ay; out[4 * io + 2] = az; out[4 * io + 3] = du;
+      }
+    }
+    free(L.parts); free(L.cells);
+  }
+  free(hs); free(bmax); free(rsph);
+  return total;
+}
+
+int orc_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+  omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}

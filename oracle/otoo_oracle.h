@@ -1,0 +1,91 @@
+/* otoo_oracle.h -- plain, slow, fp64 CPU oracle for the OTOO force path (arxiv 1206.1199).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_1206_1199_b200/, include/)
+ * may include, link or call this; only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs do.  It shares no code with the CUDA path.
+ *
+ * The method is an approximation (a tree code), so the oracle follows the algorithm step by
+ * step in the paper's order (section II, III-B, III-C, III-D), with the readings
+ * R1..R17 listed in DESIGN.md.  The O(N^2) definition (orc_direct_sum) is its truth check.
+ * All host pointers.  Positions/masses come in as fp32 (single precision),
+ * every sum is fp64; the quantities that decide an integer (key quantisation, the MAC compare,
+ * the SPH neighbour compare) are evaluated in fp32 exactly as DESIGN.md states.
+ *
+ * Pins (tests/test_oracle_*.py): brute-force octants, stable sort, tree invariants, two-particle
+ * cell, tiling invariant of the lists, stackless walk == recursive walk,
+ * theta=0 == direct sum, Newton's third law, two-body closed form, Plummer potential, kernel
+ * normalisation, lattice density, brute-force SPH neighbour sets.
+ * parity unpinned: the absolute accuracy level of the theta-MAC (the paper's error plot, Fig. 5,
+ * is for its Delta-MAC and is missing from PAPER.md).
+ */
+#ifndef OTOO_ORACLE_H
+#define OTOO_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_tree orc_tree;
+
+typedef struct {
+  uint64_t prefix;      /* key >> 3*(21-level) */
+  uint32_t first;       /* first sorted slot */
+  uint32_t count;       /* particles in the cell */
+  uint32_t child_first; /* canonical id of first child, 0 if leaf */
+  uint8_t level;        /* 0 = root */
+  uint8_t child_count;  /* 0 if leaf */
+} orc_cell;
+
+/* O(N^2) softened Plummer direct sum (fp64).  acc_pot[4*t..] = (ax,ay,az,phi) of target
+ * index targets[t] (targets==NULL: all N in order, n_targets ignored). */
+void orc_direct_sum(int64_t N, const float* pos_mass, double eps, int64_t n_targets,
+                    const int64_t* targets, double* acc_pot);
+
+/* Tree build: PAPER.md III-B steps 1-4 + III-C (mass, centre of mass). */
+orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit);
+void orc_free(orc_tree*);
+int64_t orc_ncell(const orc_tree*);
+int64_t orc_nleaf(const orc_tree*);
+int orc_depth(const orc_tree*);
+void orc_root(const orc_tree*, float lo[3], float* S);
+/* canonical order (level asc, first asc). Any pointer may be NULL. */
+void orc_export(const orc_tree*, uint32_t* perm, uint64_t* keys, orc_cell* cells,
+                float* cell_com_m /*4*ncell*/, double* cell_s /*ncell*/,
+                double* cell_M_P /*4*ncell: M, Px, Py, Pz*/);
+/* key of a single point for the tree's root cube (R2, R3). */
+uint64_t orc_key(const orc_tree*, const float xyz[3]);
+
+/* rb^2 (fp32) for each cell under the theta-MAC.  mac_kind 0: r_b = l/theta + s (default),
+ * 1: r_b = l/theta. */
+void orc_rb2(const orc_tree*, double theta, int mac_kind, float* rb2 /*ncell*/);
+
+/* Group walk + gravity sums.  Outputs in the CALLER's original particle order.
+ * walk_kind 0: recursive (R9); 1: stackless next/more exactly as PAPER.md L57.
+ * group counters are per group g = sorted slots [gG, min((g+1)G, N)). Pointers may be NULL
+ * (acc_pot NULL = count only). Returns total interactions (R11). */
+uint64_t orc_gravity(const orc_tree*, double eps, double theta, int group_size, int mac_kind,
+                     int walk_kind, double* acc_pot /*4N*/, uint32_t* n_tests, uint32_t* n_cells,
+                     uint32_t* n_parts);
+/* the lists of one group (sizes from orc_gravity counters) */
+void orc_group_lists(const orc_tree*, double theta, int group_size, int mac_kind, int64_t g,
+                     uint32_t* cell_ids, uint32_t* part_slots);
+
+/* SPH.  h = support radius per particle (original order).  */
+void orc_sph_cell_radii(const orc_tree*, const float* h, float* bmax, float* rsph /*ncell each*/);
+uint64_t orc_sph_density(const orc_tree*, const float* h, int group_size, double* rho,
+                         uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
+/* candidate list of one SPH group (sorted slots) */
+void orc_sph_group_list(const orc_tree*, const float* h, int group_size, int64_t g,
+                        uint32_t* part_slots);
+uint64_t orc_sph_force(const orc_tree*, const float* h, const double* rho, const double* P,
+                       const float* vel /*4N or NULL*/, int group_size, double* acc_dudt /*4N*/);
+/* cubic spline with support h (R13) */
+double orc_W(double r, double h);
+double orc_dWdr(double r, double h);
+
+int orc_max_threads(void);
+void orc_set_threads(int n);
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,133 @@
+"""Pins for the oracle's walk and gravity sums (PAPER.md II, III-D; readings R7-R11).
+Expected values come from closed forms, numpy brute force and invariants, never from oracle/."""
+import numpy as np
+import pytest
+
+from workloads import generators as gen
+
+
+def np_direct(pm, eps):
+    x = pm[:, :3].astype(np.float64)
+    m = pm[:, 3].astype(np.float64)
+    d = x[None, :, :] - x[:, None, :]
+    r2 = (d ** 2).sum(-1) + eps * eps
+    np.fill_diagonal(r2, np.inf)
+    ri = 1.0 / np.sqrt(r2)
+    acc = (m[None, :, None] * d * ri[:, :, None] ** 3).sum(1)
+    pot = -(m[None, :] * ri).sum(1)
+    return np.concatenate([acc, pot[:, None]], axis=1)
+
+
+def test_direct_sum_two_body_closed_form(orc):
+    pm = np.array([[0, 0, 0, 2.0], [3.0, 4.0, 0, 5.0]], np.float32)
+    eps = 0.5
+    out = orc.direct_sum(pm, eps)
+    r2 = 25.0 + 0.25
+    a0 = 5.0 / r2 ** 1.5
+    assert out[0] == pytest.approx([a0 * 3, a0 * 4, 0, -5.0 / np.sqrt(r2)], rel=1e-14)
+    a1 = 2.0 / r2 ** 1.5
+    assert out[1] == pytest.approx([-a1 * 3, -a1 * 4, 0, -2.0 / np.sqrt(r2)], rel=1e-14)
+
+
+def test_direct_sum_vs_numpy_and_newton3(orc):
+    pm = gen.plummer(700, 11)
+    pm[:, 3] *= (1 + np.arange(700) % 3).astype(np.float32)
+    out = orc.direct_sum(pm, 0.01)
+    ref = np_direct(pm, 0.01)
+    assert np.allclose(out, ref, rtol=1e-12, atol=1e-14)
+    m = pm[:, 3].astype(np.float64)
+    mom = (m[:, None] * out[:, :3]).sum(0)
+    scale = (m[:, None] * np.abs(out[:, :3])).sum()
+    assert np.all(np.abs(mom) < 1e-13 * scale)            # Newton's third law
+    sub = orc.direct_sum(pm, 0.01, targets=[5, 699, 0])
+    assert np.array_equal(sub, out[[5, 699, 0]])
+
+
+@pytest.mark.parametrize("G", [32, 64])
+def test_theta0_is_direct_sum(orc, G):
+    pm = gen.plummer(1500, 3)
+    t = orc.Tree(pm, 16)
+    r = t.gravity(0.01, 0.0, G)
+    assert np.all(r["n_cells"] == 0) and np.all(r["n_parts"] == 1500)   # L43: no cell accepted
+    ref = np_direct(pm, 0.01)
+    assert np.allclose(r["acc_pot"], ref, rtol=1e-11, atol=1e-13)
+    assert r["interactions"] == 1500 * 1500
+
+
+@pytest.mark.parametrize("theta,mac", [(0.5, 0), (0.8, 0), (1.0, 0), (0.6, 1)])
+def test_lists_tile_the_system(orc, theta, mac):
+    """Every particle is covered exactly once by (accepted cells' ranges) U (particle list);
+    with the default MAC (R7) each group member sits in its own particle list."""
+    n, G = 6000, 64
+    pm = gen.plummer(n, 21)
+    t = orc.Tree(pm, 8)
+    ex = t.export()
+    r = t.gravity(0.01, theta, G, mac_kind=mac, forces=False)
+    for g in range(0, t.n_groups(G), 5):
+        cells, parts = t.group_lists(theta, G, g, r["n_cells"][g], r["n_parts"][g], mac_kind=mac)
+        cover = np.zeros(n, np.int32)
+        for c in cells:
+            f, k = ex["cells"]["first"][c], ex["cells"]["count"][c]
+            cover[f:f + k] += 1
+        np.add.at(cover, parts, 1)
+        assert np.all(cover == 1)
+        if mac == 0:
+            members = np.arange(g * G, min((g + 1) * G, n))
+            assert np.isin(members, parts).all()
+
+
+def test_stackless_equals_recursive(orc):
+    """PAPER L57 rules (1)-(4) on the next/more list visit exactly what the recursion visits."""
+    pm = gen.hernquist(5000, 2)
+    t = orc.Tree(pm, 16)
+    for theta in (0.0, 0.4, 0.8):
+        a = t.gravity(0.01, theta, 64, walk_kind=0)
+        b = t.gravity(0.01, theta, 64, walk_kind=1)
+        for k in ("n_tests", "n_cells", "n_parts"):
+            assert np.array_equal(a[k], b[k])
+        assert a["interactions"] == b["interactions"]
+        assert np.allclose(a["acc_pot"], b["acc_pot"], rtol=1e-12, atol=1e-15)
+
+
+def test_error_decreases_with_theta_and_lists_shrink(orc):
+    pm = gen.plummer(8192, 1206)
+    t = orc.Tree(pm, 16)
+    ref = orc.direct_sum(pm, 0.01)
+    an = np.linalg.norm(ref[:, :3], axis=1)
+    errs, inter = [], []
+    for theta in (0.8, 0.6, 0.4, 0.2):
+        r = t.gravity(0.01, theta, 64)
+        e = np.linalg.norm(r["acc_pot"][:, :3] - ref[:, :3], axis=1) / an
+        errs.append(np.sqrt((e ** 2).mean()))
+        inter.append(r["interactions"])
+    assert errs[0] > errs[1] > errs[2] > errs[3]
+    assert errs[3] < 2e-4 and errs[0] < 3e-2
+    assert inter[0] < inter[1] < inter[2] < inter[3]
+
+
+def test_plummer_potential_profile(orc):
+    """Analytic Plummer potential phi(r) = -1/sqrt(r^2+1) (G=M=a=1), PAPER L193 workload."""
+    n = 16384
+    pm = gen.plummer(n, 1199)
+    t = orc.Tree(pm, 16)
+    r = t.gravity(0.01, 0.5, 64)
+    rad = np.linalg.norm(pm[:, :3].astype(np.float64), axis=1)
+    for lo, hi in [(0.0, 0.5), (0.5, 1.0), (1.0, 2.0), (2.0, 5.0)]:
+        sel = (rad >= lo) & (rad < hi)
+        got = r["acc_pot"][sel, 3].mean()
+        want = (-1.0 / np.sqrt(rad[sel] ** 2 + 1.0)).mean()
+        assert got == pytest.approx(want, rel=0.02)
+    # radial acceleration: a_r = -r/(r^2+1)^1.5
+    ar = (r["acc_pot"][:, :3] * pm[:, :3]).sum(1) / rad
+    sel = (rad > 0.5) & (rad < 2.0)
+    assert ar[sel].mean() == pytest.approx((-rad[sel] / (rad[sel] ** 2 + 1) ** 1.5).mean(), rel=0.03)
+
+
+def test_interaction_count_definition(orc):
+    n, G = 3000, 64
+    pm = gen.uniform_cube(n, 4)
+    t = orc.Tree(pm, 16)
+    r = t.gravity(0.001, 0.5, G, forces=False)
+    sizes = np.minimum(G, n - np.arange(t.n_groups(G)) * G)
+    assert r["interactions"] == int((sizes * (r["n_cells"].astype(np.int64) + r["n_parts"])).sum())
+    assert r["acc_pot"] is None

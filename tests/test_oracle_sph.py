@@ -1,0 +1,123 @@
+"""Pins for the oracle's SPH path (PAPER.md II-C Eq. 4-5; readings R13-R17)."""
+import numpy as np
+import pytest
+
+from workloads import generators as gen
+
+
+def W_np(r, h):
+    q = r / h
+    s = 8.0 / (np.pi * h ** 3)
+    return s * np.where(q <= 0.5, 1 - 6 * q ** 2 + 6 * q ** 3, np.where(q < 1, 2 * (1 - q) ** 3, 0.0))
+
+
+def test_kernel_normalisation_continuity_derivative(orc):
+    h = 0.7
+    r = np.linspace(0, h, 200001)
+    w = np.array([orc.W(x, h) for x in r[::100]])
+    rr = r[::100]
+    integral = np.trapezoid(4 * np.pi * rr ** 2 * w, rr)
+    assert integral == pytest.approx(1.0, rel=1e-6)            # int W d^3r = 1
+    assert orc.W(h, h) == 0.0 and orc.W(1.5 * h, h) == 0.0      # L89: zero outside h
+    assert orc.W(0.0, h) == pytest.approx(8 / (np.pi * h ** 3))
+    e = 1e-9
+    assert orc.W(0.5 * h - e, h) == pytest.approx(orc.W(0.5 * h + e, h), rel=1e-7)
+    assert orc.dWdr(0.5 * h - e, h) == pytest.approx(orc.dWdr(0.5 * h + e, h), rel=1e-7)
+    assert abs(orc.dWdr(h - e, h)) < 1e-12
+    for x in (0.1, 0.3, 0.45, 0.55, 0.8, 0.95):
+        d = 1e-6
+        num = (orc.W(x * h + d, h) - orc.W(x * h - d, h)) / (2 * d)
+        assert orc.dWdr(x * h, h) == pytest.approx(num, rel=1e-6)
+
+
+def test_candidate_lists_are_supersets(orc):
+    """Eq. 5 guarantee (L105): the walk's candidate list of a group contains every j with
+    r_ij < max(h_i, h_j) for some member i."""
+    n, G = 3000, 32
+    w = gen.wd_pair(n, 5)
+    pm, h = w["pos_mass"], w["h"]
+    t = orc.Tree(pm, 8)
+    ex = t.export()
+    r = t.sph_density(h, G, sums=False)
+    sp = pm[ex["perm"]].astype(np.float64)
+    sh = h[ex["perm"]].astype(np.float64)
+    for g in range(0, t.n_groups(G), 3):
+        parts = t.sph_group_list(h, G, g, r["n_parts"][g])
+        assert len(np.unique(parts)) == len(parts)
+        mem = np.arange(g * G, min((g + 1) * G, n))
+        d = np.linalg.norm(sp[mem, None, :3] - sp[None, :, :3], axis=2)
+        need = (d < np.maximum(sh[mem, None], sh[None, :])).any(0)
+        assert np.isin(np.nonzero(need)[0], parts).all()
+
+
+def test_density_bruteforce_and_lattice(orc):
+    n = 2500
+    w = gen.wd_pair(n, 8)
+    pm, h = w["pos_mass"], w["h"]
+    t = orc.Tree(pm, 16)
+    r = t.sph_density(h, 64)
+    x = pm[:, :3].astype(np.float64)
+    d = np.linalg.norm(x[:, None] - x[None, :], axis=2)
+    rho = (pm[None, :, 3] * W_np(d, h[:, None].astype(np.float64))).sum(1)
+    assert np.allclose(r["rho"], rho, rtol=1e-10)
+    cnt = (d < h[:, None]).sum(1)
+    assert np.abs(r["nngb"].astype(int) - cnt).max() <= 1          # fp32 vs fp64 edge decisions
+    # simple cubic lattice: interior density equals the finite lattice sum, and ~ m/a^3
+    k, a, m = 12, 0.5, 0.25
+    lat = gen.lattice(k, a, m)
+    hh = np.full(k ** 3, 2.3 * a, np.float32)
+    tl = orc.Tree(lat, 16)
+    rl = tl.sph_density(hh, 64)
+    g = np.arange(-3, 4)
+    gx, gy, gz = np.meshgrid(g, g, g, indexing="ij")
+    rr = a * np.sqrt(gx ** 2 + gy ** 2 + gz ** 2).ravel()
+    want = m * W_np(rr, float(hh[0])).sum()
+    idx = np.arange(k ** 3).reshape(k, k, k)[4:8, 4:8, 4:8].ravel()
+    assert np.allclose(rl["rho"][idx], want, rtol=1e-12)
+    assert want == pytest.approx(m / a ** 3, rel=0.01)
+    assert np.all(rl["nngb"][idx] == (rr < float(hh[0])).sum())
+
+
+def test_pressure_force(orc):
+    # (i) brute force + antisymmetry on a WD pair
+    n = 2000
+    w = gen.wd_pair(n, 3)
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    t = orc.Tree(pm, 16)
+    rho = t.sph_density(h, 64)["rho"]
+    P = (2.0 / 3.0) * rho * u
+    out = t.sph_force(h, rho, P, 64, vel=w["vel"])["acc_dudt"]
+    x = pm[:, :3].astype(np.float64)
+    hd = h.astype(np.float64)
+    dvec = x[:, None] - x[None, :]
+    d = np.linalg.norm(dvec, axis=2)
+    np.fill_diagonal(d, 1.0)
+
+    def dW(r, hh):
+        q = r / hh
+        s = 8.0 / (np.pi * hh ** 4)
+        return s * np.where(q <= 0.5, -12 * q + 18 * q * q, np.where(q < 1, -6 * (1 - q) ** 2, 0.0))
+    gw = 0.5 * (dW(d, hd[:, None]) + dW(d, hd[None, :])) / d
+    np.fill_diagonal(gw, 0.0)
+    pr = P / rho ** 2
+    f = pm[None, :, 3] * (pr[:, None] + pr[None, :]) * gw
+    acc = -(f[:, :, None] * dvec).sum(1)
+    assert np.allclose(out[:, :3], acc, rtol=1e-9, atol=1e-12 * np.abs(acc).max())
+    v = w["vel"][:, :3].astype(np.float64)
+    du = 0.5 * (f * ((v[:, None] - v[None, :]) * dvec).sum(2)).sum(1)
+    assert np.allclose(out[:, 3], du, rtol=1e-8, atol=1e-11 * np.abs(du).max())
+    mom = (pm[:, 3:4] * out[:, :3]).sum(0)
+    assert np.all(np.abs(mom) < 1e-12 * (pm[:, 3:4] * np.abs(out[:, :3])).sum())
+    # (ii) lattice, uniform P: zero force in the interior; linear P: a ~ -grad P / rho
+    k, a, m = 14, 1.0, 1.0
+    lat = gen.lattice(k, a, m)
+    hh = np.full(k ** 3, 2.3, np.float32)
+    tl = orc.Tree(lat, 16)
+    rhol = tl.sph_density(hh, 64)["rho"]
+    idx = np.arange(k ** 3).reshape(k, k, k)[5:9, 5:9, 5:9].ravel()
+    o = tl.sph_force(hh, rhol, np.full(k ** 3, 3.0), 64)["acc_dudt"]
+    assert np.abs(o[idx, :3]).max() < 1e-12
+    Plin = 10.0 + 0.1 * lat[:, 0].astype(np.float64)
+    o = tl.sph_force(hh, rhol, Plin, 64)["acc_dudt"]
+    assert np.allclose(o[idx, 0], -0.1 / rhol[idx], rtol=0.05)
+    assert np.abs(o[idx, 1:3]).max() < 1e-12
