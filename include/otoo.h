@@ -1,0 +1,131 @@
+/* otoo.h -- C-ABI boundary of the B200-native OTOO force path (arxiv 1206.1199).
+ *
+ * One library, libotoo.so (sm_100a), one opaque context per GPU.  Citations are PAPER.md line
+ * numbers (L..) and DESIGN.md readings (R..).
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE memory owned by the caller (the Python binding passes
+ *    torch tensors' data_ptr()).  Pointers named h_* / *_out are HOST memory.  The library never
+ *    frees or reallocates caller memory and keeps no caller pointer after a call returns;
+ *    otoo_build_tree copies what it needs into context-owned sorted arrays.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work
+ *    on it and return without synchronising unless stated.
+ *  - Inputs and outputs are in the CALLER's original particle order; the Morton sort is internal.
+ *  - Units: G = 1.  Everything the path computes is fp32 (L161) except the cell moments,
+ *    which are accumulated in fp64 in a fixed order (R6) so that the tree is reproducible.
+ *  - Every function returns otoo_status; nothing aborts, prints or throws.
+ *    otoo_last_error(ctx) gives a context-owned message for the last non-OK status.
+ *  - The *_host entry points are the end-to-end form: host buffers in, host buffers out, the
+ *    copies inside the call (used for bench.py's `e2e`).
+ */
+#ifndef OTOO_H
+#define OTOO_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct otoo_ctx otoo_ctx;
+
+typedef enum {
+  OTOO_OK = 0,
+  OTOO_ERR_INVALID_ARG = 1,
+  OTOO_ERR_OOM = 2,
+  OTOO_ERR_CUDA = 3,
+  OTOO_ERR_NOT_BUILT = 4,
+  OTOO_ERR_CAPACITY = 5
+} otoo_status;
+
+/* One tree cell in canonical order: level ascending, then `first` ascending (R5).
+ * prefix = key >> 3*(21-level); [first, first+count) = its range of sorted particle slots;
+ * children are the cells child_first .. child_first+child_count-1 (0,0 for a leaf). */
+typedef struct {
+  uint64_t prefix;
+  uint32_t first, count, child_first;
+  uint8_t level, child_count;
+} otoo_cell_t;
+
+typedef struct {
+  int64_t N, N_cell, N_leaf;
+  int32_t depth;        /* deepest level that holds a cell, 0..21 */
+  float lo[3], S;       /* root cube [lo, lo+S]^3 (R1) */
+} otoo_tree_info_t;
+
+typedef struct {
+  uint64_t sum_tests;        /* MAC tests of the last walk, all groups */
+  uint64_t sum_interactions; /* R11: sum_g |g| (n_cells,g + n_parts,g) of the last walk */
+  uint64_t sum_cells, sum_parts;
+  int64_t n_groups;
+  int32_t group_size;
+  int32_t launches;          /* kernels launched by the last call */
+} otoo_stats_t;
+
+/* Lifecycle.  `device` is a CUDA ordinal; max_particles bounds N of every later build
+ * (1 <= max_particles <= 2^31-1).  Allocates context-owned scratch. */
+otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles);
+void otoo_destroy(otoo_ctx* ctx);
+const char* otoo_last_error(const otoo_ctx* ctx);
+/* ABI version of this header (1). */
+int otoo_version(void);
+
+/* PAPER III-B steps 1-4 + III-C, all on the device: root cube (L121,L127; R1), Morton keys
+ * (L129; R2,R3), key sort (L133; R4), cells from the sorted keys (L135; R5), mass and centre of
+ * mass bottom-up (L155; R6).  d_pos_mass: N x float4 (x,y,z,m), original order.  n_crit >= 1 is
+ * the largest number of particles a leaf may hold (L41).  N = 0 is a no-op that leaves the
+ * context "not built".  Synchronises `stream` once (to size the cell arrays). */
+otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit,
+                            void* stream);
+
+/* PAPER III-D: group walk (L57, L163; R7-R9) fused with the softened Plummer monopole/particle
+ * sums (L43; R10).  eps >= 0 scalar softening; theta >= 0 opening angle (0 opens every cell =
+ * direct sum); group_size in {32, 64, 128, 256} consecutive Morton-sorted targets share one
+ * interaction list.  d_acc_pot: N x float4 (ax, ay, az, phi), original order. Asynchronous. */
+otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, float* d_acc_pot,
+                         void* stream);
+
+/* PAPER II-C (Eq. 4, Eq. 5) SPH stage 1: density by direct summation during the walk (L99-L105;
+ * R13-R16).  d_h: N floats, kernel SUPPORT radius (W = 0 for r >= h, L89), original order.
+ * d_rho: N floats out.  d_nngb: N uint32 out (neighbours with r < h_i, self included) or NULL. */
+otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho,
+                             uint32_t* d_nngb, void* stream);
+
+/* SPH stage 2 (L252 step 6; R17): symmetric pressure force.  d_rho, d_P: N floats (P from the
+ * caller's EOS).  d_vel: N x float4 or NULL.  d_acc_sph: N x float4 (ax, ay, az, w), w = du/dt
+ * if d_vel != NULL else 0. */
+otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,
+                           const float* d_vel, int group_size, float* d_acc_sph, void* stream);
+
+/* Ideal-gas EOS of BASELINE config 4 (replaces the paper's host Helmholtz step 5, L248):
+ * P_i = (gamma-1) rho_i u_i, element-wise. */
+otoo_status otoo_eos_ideal(otoo_ctx* ctx, const float* d_rho, const float* d_u, float gamma,
+                           int64_t N, float* d_P, void* stream);
+
+/* Introspection for parity tests and the metric.  All synchronise the context's last stream. */
+otoo_status otoo_tree_info(otoo_ctx* ctx, otoo_tree_info_t* host_out);
+/* Any pointer may be NULL.  d_perm[s] = original index of sorted slot s (N); d_sorted_keys (N);
+ * d_cells (N_cell, canonical order); d_cell_com_m (N_cell x 4: cm, m as the walk sees them);
+ * d_cell_rb2 (N_cell: r_b^2 of the last otoo_gravity, R7; zeros before any). */
+otoo_status otoo_export_tree(otoo_ctx* ctx, uint32_t* d_perm, uint64_t* d_sorted_keys,
+                             otoo_cell_t* d_cells, float* d_cell_com_m, float* d_cell_rb2);
+/* SPH cell radii of the last SPH call (R14): b_max, r_SPH, each N_cell floats, canonical order. */
+otoo_status otoo_export_sph_radii(otoo_ctx* ctx, float* d_bmax, float* d_rsph);
+/* Per-group counters of the last walk (gravity or SPH), each ceil(N/G) uint32; any may be NULL.
+ * OTOO_ERR_NOT_BUILT before any walk. */
+otoo_status otoo_export_group_stats(otoo_ctx* ctx, uint32_t* d_ntests, uint32_t* d_ncells,
+                                    uint32_t* d_nparts);
+otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
+
+/* Tuning/debug knobs.  "walk_stack" = shared-memory walk stack entries per warp before the
+ * global-memory spill is used (test hook; 64..OTOO_WALK_STACK_MAX). Unknown names:
+ * OTOO_ERR_INVALID_ARG. */
+otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value);
+
+/* End-to-end form with HOST buffers (pageable or pinned): copies h_pos_mass to the device,
+ * builds the tree, runs otoo_gravity, copies N x float4 back into h_acc_pot, synchronises. */
+otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit,
+                              float eps, float theta, int group_size, float* h_acc_pot);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,296 @@
+// api.cu -- the C-ABI of include/otoo.h: argument checks, context lifecycle, exports.
+#include <string.h>
+#include <new>
+#include "common.cuh"
+
+namespace {
+
+template <typename T>
+otoo_status dalloc(otoo_ctx* ctx, T** p, size_t count) {
+  *p = nullptr;
+  OTOO_CUDA(ctx, cudaMalloc((void**)p, (count ? count : 1) * sizeof(T)));
+  return OTOO_OK;
+}
+
+__global__ void __launch_bounds__(256) export_cells_kernel(int64_t ncell, const uint32_t* __restrict__ c_first,
+                                                           const uint32_t* __restrict__ c_count,
+                                                           const uint32_t* __restrict__ c_child_first,
+                                                           const uint8_t* __restrict__ c_level,
+                                                           const uint8_t* __restrict__ c_child_count,
+                                                           const uint64_t* __restrict__ key, otoo_cell_t* __restrict__ out) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  otoo_cell_t o;
+  memset(&o, 0, sizeof o);
+  o.level = c_level[c]; o.first = c_first[c]; o.count = c_count[c];
+  o.child_first = c_child_first[c]; o.child_count = c_child_count[c];
+  o.prefix = (o.level > 0 && o.count > 0) ? key[o.first] >> (3 * (OTOO_MAXLEV - o.level)) : 0ull;
+  out[c] = o;
+}
+__global__ void __launch_bounds__(256) export_rb2_kernel(int64_t ncell, const cellb_t* __restrict__ cell_b, float* __restrict__ out) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < ncell) out[c] = __uint_as_float(cell_b[c].x);
+}
+__global__ void __launch_bounds__(256) export_sph_kernel(int64_t ncell, const float2* __restrict__ in, float* __restrict__ b, float* __restrict__ r) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < ncell) { float2 v = in[c]; if (b) b[c] = v.x; if (r) r[c] = v.y; }
+}
+__global__ void __launch_bounds__(256) eos_ideal_kernel(const float* __restrict__ rho, const float* __restrict__ u, float gm1,
+                                                        int64_t n, float* __restrict__ P) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) P[i] = __fmul_rn(__fmul_rn(gm1, rho[i]), u[i]);
+}
+
+bool valid_group(int G) { return G == 32 || G == 64 || G == 128 || G == 256; }
+
+}  // namespace
+
+otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups) {
+  if (ngroups <= ctx->groupCap) return OTOO_OK;
+  if (ctx->g_ntests) cudaFree(ctx->g_ntests);
+  if (ctx->g_ncells) cudaFree(ctx->g_ncells);
+  if (ctx->g_nparts) cudaFree(ctx->g_nparts);
+  ctx->groupCap = 0;
+  OTOO_TRY(dalloc(ctx, &ctx->g_ntests, ngroups));
+  OTOO_TRY(dalloc(ctx, &ctx->g_ncells, ngroups));
+  OTOO_TRY(dalloc(ctx, &ctx->g_nparts, ngroups));
+  ctx->groupCap = ngroups;
+  return OTOO_OK;
+}
+otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps) {
+  if (warps <= ctx->spill_warps) return OTOO_OK;
+  if (ctx->walk_spill) cudaFree(ctx->walk_spill);
+  ctx->spill_warps = 0;
+  OTOO_TRY(dalloc(ctx, &ctx->walk_spill, (size_t)warps * OTOO_WALK_SPILL));
+  ctx->spill_warps = warps;
+  return OTOO_OK;
+}
+
+extern "C" {
+
+int otoo_version(void) { return 1; }
+
+otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
+  if (!out) return OTOO_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (max_particles < 1 || max_particles > 2147483647LL) return OTOO_ERR_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return OTOO_ERR_CUDA;
+  otoo_ctx* ctx = new (std::nothrow) otoo_ctx;
+  if (!ctx) return OTOO_ERR_OOM;
+  memset(ctx, 0, sizeof *ctx);
+  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX;
+  otoo_status s = OTOO_OK;
+  auto body = [&]() -> otoo_status {
+    OTOO_CUDA(ctx, cudaSetDevice(device));
+    cudaDeviceProp prop;
+    OTOO_CUDA(ctx, cudaGetDeviceProperties(&prop, device));
+    ctx->sm_count = prop.multiProcessorCount;
+    const size_t n = (size_t)max_particles;
+    for (int b = 0; b < 2; b++) { OTOO_TRY(dalloc(ctx, &ctx->key[b], n)); OTOO_TRY(dalloc(ctx, &ctx->val[b], n)); }
+    OTOO_TRY(dalloc(ctx, &ctx->spos, n));
+    OTOO_TRY(dalloc(ctx, &ctx->slot_nc, n));
+    ctx->hist_cap = (size_t)cdiv(max_particles, 4096) * 256 + 256;
+    OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
+    OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));
+    OTOO_TRY(dalloc(ctx, &ctx->d_bbox, 16));
+    OTOO_TRY(dalloc(ctx, &ctx->d_counters, 64));
+    OTOO_TRY(dalloc(ctx, &ctx->d_sums, 4));
+    OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, 4 * sizeof(unsigned long long)));
+    OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
+    OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
+    return OTOO_OK;
+  };
+  s = body();
+  if (s != OTOO_OK) { otoo_destroy(ctx); return s; }
+  *out = ctx;
+  return OTOO_OK;
+}
+
+void otoo_destroy(otoo_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  void* ptrs[] = {ctx->key[0], ctx->key[1], ctx->val[0], ctx->val[1], ctx->spos, ctx->slot_nc, ctx->scan_tmp, ctx->hist,
+                  ctx->sorted_h, ctx->sorted_aux, ctx->sorted_vel, ctx->cell_cm, ctx->cell_b, ctx->c_first, ctx->c_count,
+                  ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_sph,
+                  ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
+                  ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
+  if (ctx->h_root) cudaFreeHost(ctx->h_root);
+  delete ctx;
+}
+
+const char* otoo_last_error(const otoo_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (N < 0 || n_crit < 1) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "N >= 0 and n_crit >= 1 required");
+  if (N > ctx->maxN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "N exceeds max_particles of otoo_create");
+  ctx->launches = 0;
+  ctx->last_stream = (cudaStream_t)stream;
+  if (N == 0) { ctx->built = false; ctx->walked = false; ctx->N = 0; return OTOO_OK; }
+  if (!d_pos_mass) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_pos_mass is NULL");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  return otoo_build_impl(ctx, d_pos_mass, N, n_crit, (cudaStream_t)stream);
+}
+
+otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, float* d_acc_pot, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!(eps >= 0.0f) || !(theta >= 0.0f)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "eps >= 0 and theta >= 0 required");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_acc_pot is NULL");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_gravity_impl(ctx, eps, theta, group_size, d_acc_pot, (cudaStream_t)stream);
+}
+
+static otoo_status sph_scratch(otoo_ctx* ctx) {
+  if (!ctx->sorted_h) {
+    OTOO_TRY(dalloc(ctx, &ctx->sorted_h, (size_t)ctx->maxN));
+    OTOO_TRY(dalloc(ctx, &ctx->sorted_aux, (size_t)ctx->maxN));
+    OTOO_TRY(dalloc(ctx, &ctx->sorted_vel, (size_t)ctx->maxN));
+  }
+  return OTOO_OK;
+}
+
+otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho, uint32_t* d_nngb, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_h || !d_rho) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_h and d_rho must not be NULL");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_TRY(sph_scratch(ctx));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_sph_density_impl(ctx, d_h, group_size, d_rho, d_nngb, (cudaStream_t)stream);
+}
+
+otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
+                           int group_size, float* d_acc_sph, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_h || !d_rho || !d_P || !d_acc_sph) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL argument");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_TRY(sph_scratch(ctx));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_sph_force_impl(ctx, d_h, d_rho, d_P, d_vel, group_size, d_acc_sph, (cudaStream_t)stream);
+}
+
+otoo_status otoo_eos_ideal(otoo_ctx* ctx, const float* d_rho, const float* d_u, float gamma, int64_t N, float* d_P, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (N < 0 || !(gamma > 1.0f)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "N >= 0 and gamma > 1 required");
+  if (N == 0) return OTOO_OK;
+  if (!d_rho || !d_u || !d_P) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL argument");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  eos_ideal_kernel<<<(unsigned)cdiv(N, 256), 256, 0, (cudaStream_t)stream>>>(d_rho, d_u, gamma - 1.0f, N, d_P);
+  ctx->launches = 1;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  return OTOO_OK;
+}
+
+otoo_status otoo_tree_info(otoo_ctx* ctx, otoo_tree_info_t* o) {
+  if (!ctx || !o) return OTOO_ERR_INVALID_ARG;
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+  ctx->N_leaf = ctx->h_counters[32];
+  o->N = ctx->N; o->N_cell = ctx->N_cell; o->N_leaf = ctx->N_leaf; o->depth = ctx->depth;
+  for (int k = 0; k < 3; k++) o->lo[k] = ctx->lo[k];
+  o->S = ctx->S;
+  return OTOO_OK;
+}
+
+otoo_status otoo_export_tree(otoo_ctx* ctx, uint32_t* d_perm, uint64_t* d_keys, otoo_cell_t* d_cells, float* d_com_m, float* d_rb2) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->last_stream;
+  const unsigned nbC = (unsigned)cdiv(ctx->N_cell, 256);
+  if (d_perm) OTOO_CUDA(ctx, cudaMemcpyAsync(d_perm, ctx->val[0], 4 * (size_t)ctx->N, cudaMemcpyDeviceToDevice, st));
+  if (d_keys) OTOO_CUDA(ctx, cudaMemcpyAsync(d_keys, ctx->key[0], 8 * (size_t)ctx->N, cudaMemcpyDeviceToDevice, st));
+  if (d_cells)
+    export_cells_kernel<<<nbC, 256, 0, st>>>(ctx->N_cell, ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
+                                             ctx->c_child_count, ctx->key[0], d_cells);
+  if (d_com_m) OTOO_CUDA(ctx, cudaMemcpyAsync(d_com_m, ctx->cell_cm, 16 * (size_t)ctx->N_cell, cudaMemcpyDeviceToDevice, st));
+  if (d_rb2) export_rb2_kernel<<<nbC, 256, 0, st>>>(ctx->N_cell, ctx->cell_b, d_rb2);
+  OTOO_CUDA(ctx, cudaGetLastError());
+  OTOO_CUDA(ctx, cudaStreamSynchronize(st));
+  return OTOO_OK;
+}
+
+otoo_status otoo_export_sph_radii(otoo_ctx* ctx, float* d_bmax, float* d_rsph) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!ctx->built || !ctx->sph_radii_valid) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "no SPH call since the last build");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  export_sph_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, ctx->last_stream>>>(ctx->N_cell, ctx->c_sph, d_bmax, d_rsph);
+  OTOO_CUDA(ctx, cudaGetLastError());
+  OTOO_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+  return OTOO_OK;
+}
+
+otoo_status otoo_export_group_stats(otoo_ctx* ctx, uint32_t* d_ntests, uint32_t* d_ncells, uint32_t* d_nparts) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!ctx->built || !ctx->walked) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "no walk since the last build");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->last_stream;
+  size_t b = 4 * (size_t)ctx->last_ngroups;
+  if (d_ntests) OTOO_CUDA(ctx, cudaMemcpyAsync(d_ntests, ctx->g_ntests, b, cudaMemcpyDeviceToDevice, st));
+  if (d_ncells) OTOO_CUDA(ctx, cudaMemcpyAsync(d_ncells, ctx->g_ncells, b, cudaMemcpyDeviceToDevice, st));
+  if (d_nparts) OTOO_CUDA(ctx, cudaMemcpyAsync(d_nparts, ctx->g_nparts, b, cudaMemcpyDeviceToDevice, st));
+  OTOO_CUDA(ctx, cudaStreamSynchronize(st));
+  return OTOO_OK;
+}
+
+otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
+  if (!ctx || !o) return OTOO_ERR_INVALID_ARG;
+  memset(o, 0, sizeof *o);
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+  if (ctx->walked) {
+    unsigned long long h[4];
+    OTOO_CUDA(ctx, cudaMemcpy(h, ctx->d_sums, sizeof h, cudaMemcpyDeviceToHost));
+    o->sum_tests = h[0]; o->sum_interactions = h[1]; o->sum_cells = h[2]; o->sum_parts = h[3];
+    o->n_groups = ctx->last_ngroups; o->group_size = ctx->last_group_size;
+  }
+  o->launches = ctx->launches;
+  return OTOO_OK;
+}
+
+otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
+  if (!ctx || !name) return OTOO_ERR_INVALID_ARG;
+  if (strcmp(name, "walk_stack") == 0) {
+    if (value < 512 || value > OTOO_WALK_STACK_MAX) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "walk_stack must be in [512, 1024]");
+    ctx->walk_stack = (int)value;
+    return OTOO_OK;
+  }
+  return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");
+}
+
+otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit, float eps, float theta,
+                              int group_size, float* h_acc_pot) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (N < 0 || !h_pos_mass || !h_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL host buffer or N < 0");
+  if (N > ctx->maxN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "N exceeds max_particles of otoo_create");
+  if (N == 0) return OTOO_OK;
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  // staging: key[1] (8 B/particle) + val[1] are free before the sort; use dedicated buffers instead
+  float4 *d_in = nullptr, *d_out = nullptr;
+  OTOO_CUDA(ctx, cudaMalloc((void**)&d_in, 16 * (size_t)N));
+  cudaError_t e = cudaMalloc((void**)&d_out, 16 * (size_t)N);
+  if (e != cudaSuccess) { cudaFree(d_in); return otoo_fail(ctx, OTOO_ERR_OOM, "staging allocation failed"); }
+  otoo_status s = OTOO_OK;
+  cudaStream_t st = 0;
+  if (cudaMemcpyAsync(d_in, h_pos_mass, 16 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "H2D copy failed");
+  if (s == OTOO_OK) s = otoo_build_tree(ctx, reinterpret_cast<const float*>(d_in), N, n_crit, st);
+  int l1 = ctx->launches;
+  if (s == OTOO_OK) s = otoo_gravity(ctx, eps, theta, group_size, reinterpret_cast<float*>(d_out), st);
+  ctx->launches += l1;
+  if (s == OTOO_OK && cudaMemcpyAsync(h_acc_pot, d_out, 16 * (size_t)N, cudaMemcpyDeviceToHost, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "D2H copy failed");
+  if (s == OTOO_OK && cudaStreamSynchronize(st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "synchronize failed");
+  cudaFree(d_in); cudaFree(d_out);
+  return s;
+}
+
+}  // extern "C"

@@ -1,0 +1,322 @@
+// build.cu -- device-side tree construction (PAPER.md III-B steps 1-4, III-C), readings R1-R7.
+// The paper builds the tree on the host and calls the pointer set-up "difficult to parallelize"
+// (L135, L151); here every step is a data-parallel kernel over the sorted keys:
+//   a cell (level l, first slot s) exists  <=>  s starts a level-l prefix range AND the level-(l-1)
+//   range holding s has more than n_crit particles  <=>  cpl(s) < l <= min(D(s)+1, 21), where
+//   cpl(s) = common prefix levels of key[s-1], key[s] and D(s) = max over windows of n_crit+1
+//   consecutive slots containing s of their common prefix levels.
+#include "common.cuh"
+
+namespace {
+
+__device__ __forceinline__ unsigned f2ord(float f) {
+  unsigned u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(unsigned u) {
+  return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u);
+}
+
+// H1 (L121, L127; R1): per-axis min/max.  d_bbox[0..2] = min (ordered uint), [3..5] = max.
+__global__ void __launch_bounds__(256) bbox_kernel(const float4* __restrict__ pos, int64_t n, unsigned* bbox) {
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    float4 p = pos[i];
+    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+  }
+#pragma unroll
+  for (int k = 0; k < 3; k++)
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      lo[k] = fminf(lo[k], __shfl_xor_sync(0xFFFFFFFFu, lo[k], o));
+      hi[k] = fmaxf(hi[k], __shfl_xor_sync(0xFFFFFFFFu, hi[k], o));
+    }
+  if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) { atomicMin(&bbox[k], f2ord(lo[k])); atomicMax(&bbox[3 + k], f2ord(hi[k])); }
+  }
+}
+// root cube: floats at bbox[8..12] = lo.xyz, S, scale
+__global__ void root_kernel(unsigned* bbox) {
+  float* out = reinterpret_cast<float*>(bbox) + 8;
+  float S = 0.0f;
+  for (int k = 0; k < 3; k++) {
+    float lo = ord2f(bbox[k]), hi = ord2f(bbox[3 + k]);
+    float d = __fsub_rn(hi, lo);
+    if (d > S) S = d;
+    out[k] = lo;
+  }
+  if (!(S > 0.0f)) S = 1.0f;
+  out[3] = S;
+  out[4] = __fdiv_rn(2097152.0f, S);  // R2: IEEE division
+}
+
+__device__ __forceinline__ uint64_t dilate3(uint32_t v) {
+  uint64_t x = v & 0x1FFFFFu;
+  x = (x | x << 32) & 0x001F00000000FFFFull;
+  x = (x | x << 16) & 0x001F0000FF0000FFull;
+  x = (x | x << 8) & 0x100F00F00F00F00Full;
+  x = (x | x << 4) & 0x10C30C30C30C30C3ull;
+  x = (x | x << 2) & 0x1249249249249249ull;
+  return x;
+}
+__device__ __forceinline__ uint32_t compact3(uint64_t x) {
+  x &= 0x1249249249249249ull;
+  x = (x | x >> 2) & 0x10C30C30C30C30C3ull;
+  x = (x | x >> 4) & 0x100F00F00F00F00Full;
+  x = (x | x >> 8) & 0x001F0000FF0000FFull;
+  x = (x | x >> 16) & 0x001F00000000FFFFull;
+  x = (x | x >> 32) & 0x1FFFFFull;
+  return (uint32_t)x;
+}
+__device__ __forceinline__ uint32_t quant(float x, float lo, float scale) {
+  float t = __fmul_rn(__fsub_rn(x, lo), scale);
+  return (t >= 2097151.0f) ? 2097151u : (t > 0.0f ? __float2uint_rz(t) : 0u);
+}
+// H2 (L129; R2, R3): 63-bit Morton key by bit dilation, x most significant in each octant.
+__global__ void __launch_bounds__(256) key_kernel(const float4* __restrict__ pos, int64_t n,
+                                                  const unsigned* __restrict__ bbox, uint64_t* __restrict__ key,
+                                                  uint32_t* __restrict__ id) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float* r = reinterpret_cast<const float*>(bbox) + 8;
+  float scale = r[4];
+  float4 p = pos[i];
+  key[i] = (dilate3(quant(p.x, r[0], scale)) << 2) | (dilate3(quant(p.y, r[1], scale)) << 1) |
+           dilate3(quant(p.z, r[2], scale));
+  id[i] = (uint32_t)i;
+}
+// H4: positions into sorted order
+__global__ void __launch_bounds__(256) gather4_kernel(const float4* __restrict__ src, const uint32_t* __restrict__ perm,
+                                                      int64_t n, float4* __restrict__ dst) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) dst[s] = src[perm[s]];
+}
+
+__device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leading levels, 0..21
+  uint64_t x = a ^ b;
+  if (x == 0) return OTOO_MAXLEV;
+  return 20 - (63 - __clzll((long long)x)) / 3;
+}
+// H5a: number of cells that start at each sorted slot, and the per-level cell counts.
+//   info[s] = (cpl+1) | LL << 8
+__global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
+                                                         uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
+                                                         uint32_t* __restrict__ level_count) {
+  __shared__ uint32_t lc[OTOO_NLEV];
+  if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
+  __syncthreads();
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) {
+    int cpl = (s == 0) ? -1 : cplev(key[s - 1], key[s]);
+    int D = -1;
+    int64_t tlo = s - n_crit; if (tlo < 0) tlo = 0;
+    int64_t thi = n - n_crit - 1; if (thi > s) thi = s;
+    for (int64_t t = tlo; t <= thi; t++) { int c = cplev(key[t], key[t + n_crit]); if (c > D) D = c; }
+    int LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
+    int nc = LL - cpl; if (nc < 0) nc = 0;
+    slot_nc[s] = (uint32_t)nc;
+    info[s] = (uint32_t)(cpl + 1) | ((uint32_t)LL << 8);
+    for (int l = cpl + 1; l <= LL; l++) atomicAdd(&lc[l], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x < OTOO_NLEV && lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+}
+// H5b: emit (level, first) for every cell, in slot order
+__global__ void __launch_bounds__(256) emit_cells_kernel(const uint32_t* __restrict__ slot_off,
+                                                         const uint32_t* __restrict__ info, int64_t n,
+                                                         uint64_t* __restrict__ lev, uint32_t* __restrict__ first) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  uint32_t inf = info[s];
+  int l0 = inf & 0xFF, LL = inf >> 8;
+  uint32_t off = slot_off[s];
+  for (int l = l0; l <= LL; l++, off++) { lev[off] = (uint64_t)l; first[off] = (uint32_t)s; }
+}
+
+struct LevelOff { uint32_t v[OTOO_NLEV + 1]; };
+
+__device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* __restrict__ a, uint32_t lo, uint32_t hi, uint32_t x) {
+  while (lo < hi) { uint32_t mid = lo + ((hi - lo) >> 1); if (a[mid] < x) lo = mid + 1; else hi = mid; }
+  return lo;
+}
+// H5c: per canonical cell: count, leaf flag, children (L135: "slicing the keys"; R5)
+__global__ void __launch_bounds__(256) cell_topology_kernel(const uint64_t* __restrict__ lev, const uint32_t* __restrict__ first,
+                                                            int64_t ncell, const uint64_t* __restrict__ key, int64_t n,
+                                                            int n_crit, LevelOff off, uint32_t* __restrict__ c_first,
+                                                            uint32_t* __restrict__ c_count, uint32_t* __restrict__ c_child_first,
+                                                            uint8_t* __restrict__ c_level, uint8_t* __restrict__ c_child_count,
+                                                            cellb_t* __restrict__ cell_b, uint32_t* __restrict__ n_leaf) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  int level = (int)lev[c];
+  uint32_t s = first[c];
+  uint32_t count;
+  if (level == 0) count = (uint32_t)n;
+  else {
+    int sh = 3 * (OTOO_MAXLEV - level);
+    uint64_t prefix = key[s] >> sh;
+    // gallop then bisect for the end of the prefix range
+    uint64_t step = 1, lo = s;  // key[lo] has the prefix
+    while (s + step < (uint64_t)n && (key[s + step] >> sh) == prefix) { lo = s + step; step <<= 1; }
+    uint64_t hi = s + step < (uint64_t)n ? s + step : (uint64_t)n;  // key[hi] lacks it (or hi == n)
+    while (lo + 1 < hi) { uint64_t mid = (lo + hi) >> 1; if ((key[mid] >> sh) == prefix) lo = mid; else hi = mid; }
+    count = (uint32_t)(hi - s);
+  }
+  bool leaf = count <= (uint32_t)n_crit || level == OTOO_MAXLEV;
+  uint32_t cf = 0, cc = 0;
+  if (!leaf) {
+    uint32_t a = off.v[level + 1], b = off.v[level + 2];
+    cf = lower_bound_u32(first, a, b, s);
+    cc = lower_bound_u32(first, cf, b, s + count) - cf;
+  }
+  c_first[c] = s; c_count[c] = count; c_child_first[c] = cf;
+  c_level[c] = (uint8_t)level; c_child_count[c] = (uint8_t)cc;
+  cell_b[c] = leaf ? make_uint4(0u, s, count, 1u | ((uint32_t)level << 8))
+                   : make_uint4(0u, cf, cc, ((uint32_t)level << 8));
+  if (leaf) atomicAdd(n_leaf, 1u);
+}
+
+// H6 (L155; R6, R7): one level of the bottom-up pass; fp64, fixed summation order.
+__global__ void __launch_bounds__(128) moments_kernel(uint32_t c0, uint32_t c1, int level, const float4* __restrict__ spos,
+                                                      const uint64_t* __restrict__ key, const uint32_t* __restrict__ c_first,
+                                                      const uint32_t* __restrict__ c_count,
+                                                      const uint32_t* __restrict__ c_child_first,
+                                                      const uint8_t* __restrict__ c_child_count, const unsigned* __restrict__ bbox,
+                                                      double* __restrict__ MP, double* __restrict__ cm64,
+                                                      float4* __restrict__ cell_cm, double* __restrict__ c_s) {
+  uint32_t c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= c1) return;
+  uint32_t first = c_first[c], count = c_count[c];
+  int nch = c_child_count[c];
+  double M = 0.0, Px = 0.0, Py = 0.0, Pz = 0.0;
+  if (nch == 0) {
+    for (uint32_t s = first; s < first + count; s++) {
+      float4 p = spos[s];
+      double m = (double)p.w;
+      M = __dadd_rn(M, m);
+      Px = __dadd_rn(Px, __dmul_rn(m, (double)p.x));
+      Py = __dadd_rn(Py, __dmul_rn(m, (double)p.y));
+      Pz = __dadd_rn(Pz, __dmul_rn(m, (double)p.z));
+    }
+  } else {
+    uint32_t ch = c_child_first[c];
+    for (int k = 0; k < nch; k++) {
+      const double* q = MP + 4 * (size_t)(ch + k);
+      M = __dadd_rn(M, q[0]); Px = __dadd_rn(Px, q[1]); Py = __dadd_rn(Py, q[2]); Pz = __dadd_rn(Pz, q[3]);
+    }
+  }
+  double* o = MP + 4 * (size_t)c;
+  o[0] = M; o[1] = Px; o[2] = Py; o[3] = Pz;
+  const float* r = reinterpret_cast<const float*>(bbox) + 8;
+  double l = ldexp((double)r[3], -level);
+  uint64_t prefix = (count > 0 && level > 0) ? (key[first] >> (3 * (OTOO_MAXLEV - level))) : 0ull;
+  double g[3];
+  g[0] = __dadd_rn((double)r[0], __dmul_rn((double)compact3(prefix >> 2) + 0.5, l));
+  g[1] = __dadd_rn((double)r[1], __dmul_rn((double)compact3(prefix >> 1) + 0.5, l));
+  g[2] = __dadd_rn((double)r[2], __dmul_rn((double)compact3(prefix) + 0.5, l));
+  double cx, cy, cz;
+  if (M != 0.0) { cx = __ddiv_rn(Px, M); cy = __ddiv_rn(Py, M); cz = __ddiv_rn(Pz, M); }
+  else { cx = g[0]; cy = g[1]; cz = g[2]; }
+  cm64[3 * (size_t)c] = cx; cm64[3 * (size_t)c + 1] = cy; cm64[3 * (size_t)c + 2] = cz;
+  cell_cm[c] = make_float4(__double2float_rn(cx), __double2float_rn(cy), __double2float_rn(cz), __double2float_rn(M));
+  double dx = __dsub_rn(cx, g[0]), dy = __dsub_rn(cy, g[1]), dz = __dsub_rn(cz, g[2]);
+  c_s[c] = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+}
+
+template <typename T>
+otoo_status grow(otoo_ctx* ctx, T** p, size_t count) {
+  if (*p) cudaFree(*p);
+  *p = nullptr;
+  OTOO_CUDA(ctx, cudaMalloc((void**)p, count * sizeof(T)));
+  return OTOO_OK;
+}
+
+otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
+  if (ncell <= ctx->cellCap) return OTOO_OK;
+  int64_t cap = ncell + ncell / 8 + 1024;
+  ctx->cellCap = 0;
+  OTOO_TRY(grow(ctx, &ctx->cell_cm, cap));
+  OTOO_TRY(grow(ctx, &ctx->cell_b, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_first, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_count, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_child_first, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_level, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_child_count, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_MP, 4 * cap));
+  OTOO_TRY(grow(ctx, &ctx->c_cm64, 3 * cap));
+  OTOO_TRY(grow(ctx, &ctx->c_s, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
+  OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
+  for (int b = 0; b < 2; b++) { OTOO_TRY(grow(ctx, &ctx->tmp_key[b], cap)); OTOO_TRY(grow(ctx, &ctx->tmp_val[b], cap)); }
+  size_t need = (size_t)cdiv(cap, 4096) * 256 + 256;
+  if (need > ctx->hist_cap) { OTOO_TRY(grow(ctx, &ctx->hist, need)); ctx->hist_cap = need; }
+  ctx->cellCap = cap;
+  return OTOO_OK;
+}
+
+}  // namespace
+
+otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st) {
+  ctx->built = false; ctx->walked = false; ctx->sph_radii_valid = false;
+  const float4* pos = reinterpret_cast<const float4*>(d_pos_mass);
+  unsigned* bbox = reinterpret_cast<unsigned*>(ctx->d_bbox);
+  const unsigned nbN = (unsigned)cdiv(N, 256);
+  // H1
+  OTOO_CUDA(ctx, cudaMemsetAsync(bbox, 0xFF, 12, st));      // min = 0xFFFFFFFF
+  OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 12, st));  // max = 0
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 64 * sizeof(uint32_t), st));
+  int gb = ctx->sm_count * 8; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
+  bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
+  root_kernel<<<1, 1, 0, st>>>(bbox);
+  // H2, H3, H4
+  key_kernel<<<nbN, 256, 0, st>>>(pos, N, bbox, ctx->key[0], ctx->val[0]);
+  ctx->launches += 3;
+  int res = 0;
+  OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res));
+  if (res != 0) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: sort result buffer");
+  gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
+  // H5a
+  uint32_t* info = ctx->val[1];
+  slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
+  ctx->launches += 2;
+  OTOO_TRY(otoo_exclusive_scan_u32(ctx, ctx->slot_nc, N, ctx->d_counters + 40, st));
+  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, 64 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_root, ctx->d_bbox + 8, 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
+  OTOO_CUDA(ctx, cudaStreamSynchronize(st));
+  int64_t ncell = ctx->h_counters[40];
+  LevelOff off;
+  uint32_t run = 0; int depth = 0;
+  for (int l = 0; l < OTOO_NLEV; l++) { off.v[l] = run; run += ctx->h_counters[l]; if (ctx->h_counters[l]) depth = l; }
+  off.v[OTOO_NLEV] = run;
+  if ((int64_t)run != ncell || ncell < 1) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: level counts disagree with cell count");
+  OTOO_TRY(ensure_cells(ctx, ncell));
+  const unsigned nbC = (unsigned)cdiv(ncell, 256);
+  // H5b, canonical order (level, first), H5c
+  emit_cells_kernel<<<nbN, 256, 0, st>>>(ctx->slot_nc, info, N, ctx->tmp_key[0], ctx->tmp_val[0]);
+  ctx->launches += 1;
+  OTOO_TRY(otoo_sort_pairs(ctx, ctx->tmp_key, ctx->tmp_val, ncell, 0, 8, st, &res));
+  cell_topology_kernel<<<nbC, 256, 0, st>>>(ctx->tmp_key[res], ctx->tmp_val[res], ncell, ctx->key[0], N, n_crit, off,
+                                            ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
+                                            ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);
+  ctx->launches += 1;
+  // H6 deepest level first
+  for (int l = depth; l >= 0; l--) {
+    uint32_t c0 = off.v[l], c1 = off.v[l + 1];
+    if (c1 == c0) continue;
+    moments_kernel<<<(unsigned)cdiv(c1 - c0, 128), 128, 0, st>>>(c0, c1, l, ctx->spos, ctx->key[0], ctx->c_first,
+                                                                 ctx->c_count, ctx->c_child_first, ctx->c_child_count,
+                                                                 bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s);
+    ctx->launches += 1;
+  }
+  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 32, ctx->d_counters + 32, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  OTOO_CUDA(ctx, cudaGetLastError());
+  ctx->N = N; ctx->N_cell = ncell; ctx->n_crit = n_crit; ctx->depth = depth;
+  for (int k = 0; k < 3; k++) ctx->lo[k] = ctx->h_root[k];
+  ctx->S = ctx->h_root[3];
+  for (int l = 0; l <= OTOO_NLEV; l++) ctx->level_off[l] = off.v[l];
+  ctx->built = true;
+  return OTOO_OK;
+}

@@ -1,0 +1,122 @@
+// common.cuh -- context layout and helpers shared by the kernels of libotoo.so (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/otoo.h"
+
+#define OTOO_MAXLEV 21
+#define OTOO_NLEV 22                 // levels 0..21
+#define OTOO_WALK_STACK_MAX 1024     // smem walk-stack entries per warp
+#define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
+#define OTOO_LIST_CAP 512            // smem interaction-list entries per warp (float4 each)
+#define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
+
+// Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).
+//   x = rb^2 bits (gravity MAC, R7), y = first child id (internal) or first sorted slot (leaf),
+//   z = child count (internal) or particle count (leaf), w = bit0 leaf flag | level << 8.
+typedef uint4 cellb_t;
+
+struct otoo_ctx {
+  int device;
+  int sm_count;
+  int64_t maxN;
+  char err[256];
+  cudaStream_t last_stream;
+
+  // ---- per-particle arrays, capacity maxN
+  uint64_t* key[2];      // key double buffer for the LSD sort; key[0] holds the sorted keys after build
+  uint32_t* val[2];      // id double buffer; val[0] = perm after build
+  float4* spos;          // positions+mass in sorted order
+  uint32_t* slot_nc;     // cells starting at slot s, then its exclusive scan
+  uint32_t* scan_tmp;    // block sums for the scan
+  uint32_t* hist;        // radix histograms [256][nblocks]
+  size_t hist_cap;
+  float* sorted_h;       // SPH: h in sorted order
+  float4* sorted_aux;    // SPH force: (rho-independent) per-particle packed inputs in sorted order
+  float4* sorted_vel;
+
+  // ---- per-cell arrays, capacity cellCap (grow-only)
+  int64_t cellCap;
+  float4* cell_cm;       // (cm.xyz, m) fp32 -- what the walk reads
+  cellb_t* cell_b;
+  uint32_t* c_first;
+  uint32_t* c_count;
+  uint32_t* c_child_first;
+  uint8_t* c_level;
+  uint8_t* c_child_count;
+  double* c_MP;          // 4 per cell: M, Px, Py, Pz (R6)
+  double* c_cm64;        // 3 per cell: fp64 centre of mass (needed for Eq. 5)
+  double* c_s;           // |CM - geometric centre| (R7)
+  float2* c_sph;         // (b_max, r_SPH) (R14)
+  unsigned long long* sph_acc;  // 2 per cell: fp64 maxima as ordered bits
+  uint64_t* tmp_key[2];  // (level) keys for the canonical ordering pass
+  uint32_t* tmp_val[2];
+
+  // ---- small device scalars
+  float* d_bbox;         // 6 floats lo/hi as ordered ints, then lo[3], S, scale
+  uint32_t* d_counters;  // [0..21] cells per level, [32] n_leaf, [33] work-queue counter, [34] error flag
+  // pinned host mirror
+  uint32_t* h_counters;
+  float* h_root;         // lo[3], S
+
+  // ---- walk outputs
+  int64_t groupCap;
+  uint32_t* g_ntests;
+  uint32_t* g_ncells;
+  uint32_t* g_nparts;
+  uint32_t* walk_spill;  // OTOO_WALK_SPILL entries per resident warp
+  int64_t spill_warps;
+  unsigned long long* d_sums; // [0] tests [1] interactions [2] cells [3] parts
+
+  // ---- state
+  bool built;
+  bool walked;
+  bool sph_radii_valid;
+  int64_t N, N_cell, N_leaf;
+  int n_crit, depth;
+  float lo[3], S;
+  uint32_t level_off[OTOO_NLEV + 1];
+  int walk_stack;        // option "walk_stack"
+  int last_group_size;
+  int64_t last_ngroups;
+  int launches;          // kernels launched by the current/last API call
+};
+
+#define OTOO_CUDA(ctx, call)                                                                   \
+  do {                                                                                         \
+    cudaError_t e_ = (call);                                                                   \
+    if (e_ != cudaSuccess) {                                                                   \
+      snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call,     \
+               cudaGetErrorString(e_));                                                        \
+      return (e_ == cudaErrorMemoryAllocation) ? OTOO_ERR_OOM : OTOO_ERR_CUDA;                 \
+    }                                                                                          \
+  } while (0)
+
+#define OTOO_TRY(call)                    \
+  do {                                    \
+    otoo_status s_ = (call);              \
+    if (s_ != OTOO_OK) return s_;         \
+  } while (0)
+
+static inline otoo_status otoo_fail(otoo_ctx* ctx, otoo_status s, const char* msg) {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", msg);
+  return s;
+}
+static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// ---- internal entry points (one per .cu file)
+otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n,
+                            int first_bit, int end_bit, cudaStream_t st, int* result_buf);
+otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, uint32_t* total_out_dev,
+                                    cudaStream_t st);
+otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st);
+otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, float* d_acc_pot, cudaStream_t st);
+otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb,
+                                  cudaStream_t st);
+otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,
+                                const float* d_vel, int G, float* d_acc, cudaStream_t st);
+otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups);
+otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps);
+size_t otoo_walk_smem_bytes();

@@ -1,0 +1,364 @@
+// sph.cu -- SPH cell radii (Eq. 5; R14), SPH group walk (R15) fused with the
+// density sum (Eq. 4; R13, R16) and the symmetric pressure force (L252 step 6; R17).
+// "There is no particle-cell interaction in SPH" (L105): the walk only produces a particle list.
+#include "walk.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256) gather_h_kernel(const float* __restrict__ h, const uint32_t* __restrict__ perm,
+                                                       int64_t n, float* __restrict__ hs) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) hs[s] = h[perm[s]];
+}
+// per sorted slot: (h, P/rho^2) and velocity
+__global__ void __launch_bounds__(256) gather_force_inputs_kernel(const float* __restrict__ h, const float* __restrict__ rho,
+                                                                  const float* __restrict__ P, const float4* __restrict__ vel,
+                                                                  const uint32_t* __restrict__ perm, int64_t n,
+                                                                  float4* __restrict__ aux, float4* __restrict__ svel) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  uint32_t i = perm[s];
+  float r = rho[i];
+  aux[s] = make_float4(h[i], __fdiv_rn(P[i], __fmul_rn(r, r)), 0.0f, 0.0f);
+  if (vel) svel[s] = vel[i];
+}
+
+// ---- R14: b_max and r_SPH over ALL particles of every cell, from the fp64 centre of mass.
+// Each particle walks down its own root-to-leaf path; consecutive slots share cells, so a warp
+// first reduces runs of equal cell id with shuffles and only run heads touch memory.
+__global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict__ spos, const float* __restrict__ hs, int64_t n,
+                                                        const uint32_t* __restrict__ c_first, const uint32_t* __restrict__ c_count,
+                                                        const uint32_t* __restrict__ c_child_first,
+                                                        const uint8_t* __restrict__ c_child_count, const double* __restrict__ cm64,
+                                                        unsigned long long* __restrict__ acc /* 2 per cell */) {
+  const int lane = threadIdx.x & 31;
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = s < n;
+  float4 p = valid ? spos[s] : make_float4(0, 0, 0, 0);
+  double h = valid ? (double)hs[s] : 0.0;
+  uint32_t cell = valid ? 0u : 0xFFFFFFFFu;
+  while (__any_sync(0xFFFFFFFFu, cell != 0xFFFFFFFFu)) {
+    double b = 0.0, r = 0.0;
+    if (cell != 0xFFFFFFFFu) {
+      double dx = __dsub_rn((double)p.x, cm64[3 * (size_t)cell]), dy = __dsub_rn((double)p.y, cm64[3 * (size_t)cell + 1]),
+             dz = __dsub_rn((double)p.z, cm64[3 * (size_t)cell + 2]);
+      b = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+      r = __dadd_rn(b, h);
+    }
+    // segmented max over runs of equal cell id (runs are contiguous in slot order)
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
+      double ob = __shfl_down_sync(0xFFFFFFFFu, b, o), orr = __shfl_down_sync(0xFFFFFFFFu, r, o);
+      if (lane + o < 32 && oc == cell) { b = fmax(b, ob); r = fmax(r, orr); }
+    }
+    uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
+    bool head = (lane == 0) || (pc != cell);
+    if (head && cell != 0xFFFFFFFFu) {
+      atomicMax(acc + 2 * (size_t)cell, (unsigned long long)__double_as_longlong(b));
+      atomicMax(acc + 2 * (size_t)cell + 1, (unsigned long long)__double_as_longlong(r));
+    }
+    // descend
+    if (cell != 0xFFFFFFFFu) {
+      int nch = c_child_count[cell];
+      if (nch == 0) cell = 0xFFFFFFFFu;
+      else {
+        uint32_t ch = c_child_first[cell], next = 0xFFFFFFFFu;
+        for (int k = 0; k < nch; k++) {
+          uint32_t f = c_first[ch + k];
+          if ((uint32_t)s - f < c_count[ch + k]) { next = ch + k; break; }
+        }
+        cell = next;
+      }
+    }
+  }
+}
+__global__ void __launch_bounds__(256) sph_radii_finish_kernel(const unsigned long long* __restrict__ acc, int64_t ncell,
+                                                               float2* __restrict__ out) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  double b = __longlong_as_double((long long)acc[2 * c]), r = __longlong_as_double((long long)acc[2 * c + 1]);
+  out[c] = make_float2(__double2float_ru(b), __double2float_ru(r));  // rounded up: supersets survive rounding
+}
+
+struct SphParams {
+  const float4* spos;
+  const float* hs;
+  const float4* aux;    // (h, P/rho^2, -, -) sorted
+  const float4* svel;   // sorted velocities or NULL
+  const float4* cell_cm;
+  const cellb_t* cell_b;
+  const float2* c_sph;
+  const uint32_t* perm;
+  int64_t N, ngroups;
+  float* rho; uint32_t* nngb;   // density outputs
+  float4* acc;                  // force output
+  uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;
+  uint32_t* queue; uint32_t* spill; unsigned long long* sums;
+  int stack_cap;
+};
+
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// MODE 0: density.  MODE 1: pressure force.  MODE 2: pressure force + du/dt.
+template <int T, int MODE>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(SphParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int G = 32 * T;
+  constexpr int E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);   // float4 per list entry
+  constexpr int CAP = OTOO_LIST_CAP / E;                   // entries
+  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
+  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
+                  warp * OTOO_WALK_STACK_MAX;
+  const int64_t gwarp = (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp;
+  WarpStack st;
+  unsigned long long tot_tests = 0, tot_inter = 0, tot_parts = 0;
+  const float PI_F = 3.14159265358979323846f;
+
+  for (;;) {
+    uint32_t g = 0;
+    if (lane == 0) g = atomicAdd(p.queue, 1u);
+    g = __shfl_sync(0xFFFFFFFFu, g, 0);
+    if ((int64_t)g >= p.ngroups) break;
+    const int64_t g0 = (int64_t)g * G;
+    const int gcount = (int)((p.N - g0) < G ? (p.N - g0) : G);
+    float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
+    float glo[3], ghi[3], hmax = 0.0f;
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      int64_t s = g0 + t * 32 + lane;
+      s = s < p.N ? s : g0;
+      float4 v = p.spos[s];
+      px[t] = v.x; py[t] = v.y; pz[t] = v.z;
+      if (MODE == 0) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
+      else { float4 a = p.aux[s]; ph[t] = a.x; ppr[t] = a.y; }
+      if (MODE == 2) { float4 w = p.svel[s]; vx[t] = w.x; vy[t] = w.y; vz[t] = w.z; } else { vx[t] = vy[t] = vz[t] = 0.0f; }
+      hmax = fmaxf(hmax, ph[t]);
+      if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
+      else {
+        glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
+        glo[1] = fminf(glo[1], v.y); ghi[1] = fmaxf(ghi[1], v.y);
+        glo[2] = fminf(glo[2], v.z); ghi[2] = fmaxf(ghi[2], v.z);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
+        ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
+      }
+      hmax = fmaxf(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, o));
+    }
+    float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T];
+    uint32_t cnt_ngb[T];
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      h2[t] = __fmul_rn(ph[t], ph[t]); hinv[t] = 1.0f / ph[t];
+      o0[t] = o1[t] = o2[t] = o3[t] = 0.0f; cnt_ngb[t] = 0;
+    }
+
+    st.init(stk, p.spill + gwarp * OTOO_WALK_SPILL, p.stack_cap);
+    if (lane == 0) stk[0] = 0u;
+    __syncwarp();
+    st.sp = 1;
+    int nlist = 0;
+    uint32_t ntests = 0, nparts = 0;
+
+    auto flush = [&]() {
+      __syncwarp();
+      for (int j = 0; j < nlist; j++) {
+        const float4 a = list[E * j];
+        float4 b = make_float4(0, 0, 0, 0), c = make_float4(0, 0, 0, 0);
+        if (E >= 2) b = list[E * j + 1];
+        if (E >= 3) c = list[E * j + 2];
+#pragma unroll
+        for (int t = 0; t < T; t++) {
+          if (MODE == 0) {
+            // R16: the neighbour decision in fp32, exactly this chain
+            float dx = __fsub_rn(a.x, px[t]), dy = __fsub_rn(a.y, py[t]), dz = __fsub_rn(a.z, pz[t]);
+            float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            bool in = r2 < h2[t];
+            float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
+            float u = 1.0f - q;
+            float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
+            float w2 = 2.0f * u * u * u;
+            float w = q <= 0.5f ? w1 : w2;
+            o0[t] = fmaf(in ? a.w : 0.0f, w, o0[t]);
+            cnt_ngb[t] += in ? 1u : 0u;
+          } else {
+            // R17: d = x_i - x_j; decision r2 < max(h_i,h_j)^2 in fp32, same r2 chain on (x_j - x_i)
+            float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
+            float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
+            float hj = b.x, hm = fmaxf(ph[t], hj);
+            bool in = (r2 < __fmul_rn(hm, hm)) && (r2 > 0.0f);
+            float rinv = rsqrt_approx(fmaxf(r2, 1e-37f));
+            float r = r2 * rinv;
+            float hjinv = __fdividef(1.0f, hj);
+            float qi = r * hinv[t], qj = r * hjinv;
+            float ui = 1.0f - qi, uj = 1.0f - qj;
+            float di = qi <= 0.5f ? fmaf(18.0f * qi, qi, -12.0f * qi) : (qi < 1.0f ? -6.0f * ui * ui : 0.0f);
+            float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
+            float hi2 = hinv[t] * hinv[t], hj2 = hjinv * hjinv;
+            float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2 * hj2) * rinv;   // (dW_i + dW_j)/(2r)
+            float f = in ? a.w * (ppr[t] + b.y) * gw : 0.0f;
+            // a_i -= f * (x_i - x_j) = += f * e
+            o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
+            if (MODE == 2) {
+              float vd = fmaf(vx[t] - c.x, -ex, fmaf(vy[t] - c.y, -ey, (vz[t] - c.z) * -ez));  // (v_i - v_j).(x_i - x_j)
+              o3[t] = fmaf(0.5f * f, vd, o3[t]);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      nlist = 0;
+    };
+
+    while (!st.empty()) {
+      if (st.sp == 0) st.refill(lane);
+      const int k = st.sp < 32 ? st.sp : 32;
+      const bool have = lane < k;
+      uint32_t cell = 0;
+      if (have) cell = stk[st.sp - k + lane];
+      __syncwarp();
+      st.sp -= k;
+      cellb_t B = make_uint4(0u, 0u, 0u, 0u);
+      bool open = false;
+      if (have) {
+        float4 A = __ldg(p.cell_cm + cell);
+        B = __ldg(p.cell_b + cell);
+        float2 rr = __ldg(p.c_sph + cell);
+        float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
+        float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));     // R15
+        open = d2 <= __fmul_rn(R, R);
+      }
+      ntests += (uint32_t)k;
+      const bool leaf = (B.w & 1u) != 0u;
+      const bool open_leaf = open && leaf, open_int = open && !leaf;
+      {
+        const int nch = open_int ? (int)B.z : 0;
+        const int inc = warp_inclusive_scan(nch, lane);
+        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        if (total) {
+          st.reserve(total, lane);
+          const int o = st.sp + inc - nch;
+          for (int i = 0; i < nch; i++) stk[o + i] = B.y + (uint32_t)i;
+          __syncwarp();
+          st.sp += total;
+        }
+      }
+      unsigned m = __ballot_sync(0xFFFFFFFFu, open_leaf);
+      while (m) {   // one leaf at a time, 32 particles a chunk
+        const int src = __ffs(m) - 1; m &= m - 1;
+        const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), c = __shfl_sync(0xFFFFFFFFu, B.z, src);
+        for (uint32_t i = 0; i < c; i += 32) {
+          if (nlist + 32 > CAP) flush();
+          if (i + lane < c) {
+            const uint32_t s = f + i + lane;
+            list[E * (nlist + lane)] = p.spos[s];
+            if (E >= 2) list[E * (nlist + lane) + 1] = p.aux[s];
+            if (E >= 3) list[E * (nlist + lane) + 2] = p.svel[s];
+          }
+          nlist += (int)((c - i) < 32u ? (c - i) : 32u);
+        }
+        nparts += c;
+      }
+    }
+    if (nlist) flush();
+
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      const int64_t s = g0 + t * 32 + lane;
+      if (s < p.N) {
+        const uint32_t i = p.perm[s];
+        if (MODE == 0) {
+          float hi3 = hinv[t] * hinv[t] * hinv[t];
+          p.rho[i] = o0[t] * (8.0f / PI_F) * hi3;
+          if (p.nngb) p.nngb[i] = cnt_ngb[t];
+        } else p.acc[i] = make_float4(o0[t], o1[t], o2[t], o3[t]);
+      }
+    }
+    if (lane == 0) { p.g_ntests[g] = ntests; p.g_ncells[g] = 0u; p.g_nparts[g] = nparts; }
+    tot_tests += ntests; tot_parts += nparts;
+    tot_inter += (unsigned long long)gcount * nparts;
+  }
+  if (lane == 0 && tot_tests) {
+    atomicAdd(p.sums + 0, tot_tests); atomicAdd(p.sums + 1, tot_inter); atomicAdd(p.sums + 3, tot_parts);
+  }
+}
+
+template <int MODE>
+otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_t smem, cudaStream_t st) {
+#define OTOO_SPH_CASE(TT)                                                                                              \
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_kernel<TT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+  walk_sph_kernel<TT, MODE><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
+  switch (G) {
+    case 32: OTOO_SPH_CASE(1) break;
+    case 64: OTOO_SPH_CASE(2) break;
+    case 128: OTOO_SPH_CASE(4) break;
+    case 256: OTOO_SPH_CASE(8) break;
+    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  }
+#undef OTOO_SPH_CASE
+  return OTOO_OK;
+}
+
+otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, int* grid, size_t* smem, cudaStream_t st) {
+  if (G != 32 && G != 64 && G != 128 && G != 256)
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  const int64_t ngroups = cdiv(ctx->N, G);
+  OTOO_TRY(otoo_ensure_groups(ctx, ngroups));
+  *smem = otoo_walk_smem_bytes();
+  int per_sm = (int)((227 * 1024) / (*smem + 1024));
+  if (per_sm < 1) per_sm = 1;
+  *grid = ctx->sm_count * per_sm;
+  if ((int64_t)*grid * OTOO_WALK_WARPS > ngroups) *grid = (int)cdiv(ngroups, OTOO_WALK_WARPS);
+  OTOO_TRY(otoo_ensure_spill(ctx, (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS));
+  const unsigned nbN = (unsigned)cdiv(ctx->N, 256), nbC = (unsigned)cdiv(ctx->N_cell, 256);
+  // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3)
+  gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
+  sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->c_first, ctx->c_count, ctx->c_child_first,
+                                        ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
+  sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
+  ctx->launches += 3;
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters + 33, 0, sizeof(uint32_t), st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 4 * sizeof(unsigned long long), st));
+  p->spos = ctx->spos; p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr;
+  p->cell_cm = ctx->cell_cm; p->cell_b = ctx->cell_b; p->c_sph = ctx->c_sph; p->perm = ctx->val[0];
+  p->N = ctx->N; p->ngroups = ngroups; p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
+  p->g_ntests = ctx->g_ntests; p->g_ncells = ctx->g_ncells; p->g_nparts = ctx->g_nparts;
+  p->queue = ctx->d_counters + 33; p->spill = ctx->walk_spill; p->sums = ctx->d_sums; p->stack_cap = ctx->walk_stack;
+  ctx->sph_radii_valid = true;
+  return OTOO_OK;
+}
+
+}  // namespace
+
+otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb, cudaStream_t st) {
+  SphParams p; int grid; size_t smem;
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  p.rho = d_rho; p.nngb = d_nngb;
+  OTOO_TRY(launch_sph<0>(ctx, p, G, grid, smem, st));
+  ctx->launches += 1;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  ctx->walked = true; ctx->last_group_size = G; ctx->last_ngroups = p.ngroups;
+  return OTOO_OK;
+}
+
+otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
+                                int G, float* d_acc, cudaStream_t st) {
+  SphParams p; int grid; size_t smem;
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  gather_force_inputs_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_h, d_rho, d_P, reinterpret_cast<const float4*>(d_vel),
+                                                                          ctx->val[0], ctx->N, ctx->sorted_aux, ctx->sorted_vel);
+  p.acc = reinterpret_cast<float4*>(d_acc);
+  if (d_vel) { p.svel = ctx->sorted_vel; OTOO_TRY(launch_sph<2>(ctx, p, G, grid, smem, st)); }
+  else OTOO_TRY(launch_sph<1>(ctx, p, G, grid, smem, st));
+  ctx->launches += 2;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  ctx->walked = true; ctx->last_group_size = G; ctx->last_ngroups = p.ngroups;
+  return OTOO_OK;
+}

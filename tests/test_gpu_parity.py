@@ -1,0 +1,178 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded
+inputs.  Integer work (keys, permutation, cells, per-group counters) must match bit for bit;
+floating point within the tolerances of DESIGN.md (R12, north_star: 1e-5)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from workloads import generators as gen  # noqa: E402
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def otoo():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    o = binding.Otoo(max_particles=1 << 21, device=0)
+    yield o
+    o.close()
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def acc_err(got, want):
+    """R12: per-particle relative error with the 1e-2 a_rms floor; also the un-floored maximum."""
+    d = np.linalg.norm(got[:, :3].astype(np.float64) - want[:, :3], axis=1)
+    an = np.linalg.norm(want[:, :3], axis=1)
+    arms = np.sqrt((an ** 2).mean())
+    return d / np.maximum(an, 1e-2 * arms), d / np.maximum(an, 1e-300)
+
+
+def check_tree(otoo, orc, pm, n_crit):
+    t = orc.Tree(pm, n_crit)
+    otoo.otoo_build_tree(dev(pm), n_crit)
+    ex = otoo.otoo_export_tree()
+    eo = t.export()
+    assert ex["N"] == t.N and ex["N_cell"] == t.ncell and ex["N_leaf"] == t.nleaf and ex["depth"] == t.depth
+    assert np.array_equal(ex["lo"], t.lo) and ex["S"] == t.S
+    assert np.array_equal(ex["keys"], eo["keys"])
+    assert np.array_equal(ex["perm"], eo["perm"])
+    for f in ("level", "prefix", "first", "count", "child_first", "child_count"):
+        assert np.array_equal(ex["cells"][f], eo["cells"][f]), f
+    assert np.array_equal(ex["com_m"].view(np.uint32), eo["com_m"].view(np.uint32))   # bit-exact cm, m (R6)
+    return t
+
+
+@pytest.mark.parametrize("kind,n,n_crit,seed", [("plummer", 16384, 16, 1206), ("plummer", 5000, 1, 1199),
+                                                ("uniform_cube", 3001, 8, 2012), ("hernquist", 40000, 16, 3),
+                                                ("plummer", 1, 16, 1), ("plummer", 7, 16, 2), ("uniform_sphere", 4097, 2, 5)])
+def test_tree_parity(otoo, orc, kind, n, n_crit, seed):
+    check_tree(otoo, orc, gen.make(kind, n, seed), n_crit)
+
+
+def test_tree_degenerate_inputs(otoo, orc):
+    pm = np.zeros((300, 4), np.float32)
+    pm[:, :3] = 2.5
+    pm[:, 3] = 1.0
+    check_tree(otoo, orc, pm, 4)            # all coincident: chain to level 21, leaf of 300
+    pm2 = gen.plummer(2000, 4)
+    pm2[100:140] = pm2[100]                 # a clump of duplicates inside a normal tree
+    pm2[:, 3] = (1 + np.arange(2000) % 5) / 2000.0
+    check_tree(otoo, orc, pm2, 8)
+    pm3 = gen.uniform_cube(1000, 9)
+    pm3[:, 2] = 0.25                        # planar: S from x/y only
+    check_tree(otoo, orc, pm3, 16)
+
+
+@pytest.mark.parametrize("kind,n,G,theta,eps", [("plummer", 16384, 64, 0.5, 0.01), ("plummer", 16384 + 37, 128, 0.6, 0.01),
+                                                ("plummer", 20000, 256, 0.8, 0.004), ("hernquist", 30000, 32, 0.4, 0.002),
+                                                ("uniform_cube", 50000, 128, 0.5, 0.001), ("plummer", 3000, 64, 0.0, 0.01),
+                                                ("plummer", 3000, 128, 0.5, 0.0), ("uniform_sphere", 2500, 256, 0.0, 0.0),
+                                                ("plummer", 40, 64, 0.5, 0.01)])
+def test_gravity_parity(otoo, orc, kind, n, G, theta, eps):
+    pm = gen.make(kind, n, 1206)
+    t = check_tree(otoo, orc, pm, 16)
+    theta32, eps32 = float(np.float32(theta)), float(np.float32(eps))
+    ref = t.gravity(eps32, theta32, G)
+    out = otoo.otoo_gravity(eps32, theta32, G).cpu().numpy()
+    assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta32).view(np.uint32))
+    nt, nc, npart = otoo.otoo_export_group_stats()
+    assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+    st = otoo.otoo_last_stats()
+    assert st["sum_interactions"] == ref["interactions"] and st["sum_tests"] == int(ref["n_tests"].sum())
+    e, raw = acc_err(out, ref["acc_pot"])
+    assert e.max() <= TOL, (e.max(), np.median(e), raw.max())
+    pe = np.abs(out[:, 3] - ref["acc_pot"][:, 3]) / np.abs(ref["acc_pot"][:, 3])
+    assert pe.max() <= TOL, pe.max()
+
+
+def test_walk_stack_spill(otoo, orc):
+    """theta = 0 on a deep tree overflows a 512-entry shared stack: the global spill path must
+    give the same lists."""
+    pm = gen.plummer(30000, 77)
+    t = check_tree(otoo, orc, pm, 1)
+    otoo.otoo_set_option("walk_stack", 512)
+    try:
+        for theta in (0.0, 0.3):
+            ref = t.gravity(0.01, theta, 32)
+            out = otoo.otoo_gravity(0.01, theta, 32).cpu().numpy()
+            nt, nc, npart = otoo.otoo_export_group_stats()
+            assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+            e, _ = acc_err(out, ref["acc_pot"])
+            assert e.max() <= TOL
+    finally:
+        otoo.otoo_set_option("walk_stack", 1024)
+
+
+@pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
+def test_sph_parity(otoo, orc, n, G):
+    w = gen.wd_pair(n, 1206)
+    pm, h, u, vel = w["pos_mass"], w["h"], w["u"], w["vel"]
+    t = check_tree(otoo, orc, pm, 16)
+    ref = t.sph_density(h, G)
+    rho, nngb = otoo.otoo_sph_density(dev(h), G)
+    b, r = otoo.otoo_export_sph_radii()
+    bo, ro = t.sph_cell_radii(h)
+    assert np.array_equal(b.view(np.uint32), bo.view(np.uint32)) and np.array_equal(r.view(np.uint32), ro.view(np.uint32))
+    nt, _, npart = otoo.otoo_export_group_stats()
+    assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(npart, ref["n_parts"])
+    assert otoo.otoo_last_stats()["sum_interactions"] == ref["candidates"]
+    assert np.array_equal(nngb.cpu().numpy().view(np.uint32), ref["nngb"])
+    rg = rho.cpu().numpy()
+    assert (np.abs(rg - ref["rho"]) / ref["rho"]).max() <= TOL
+    # stage 2 from the GPU's own density (R17): EOS on the device, oracle fed the same fp32 rho, P
+    P = otoo.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
+    Pg = P.cpu().numpy()
+    assert np.array_equal(Pg, (np.float32(5.0 / 3.0) - np.float32(1.0)) * rg * u)
+    for v in (None, vel):
+        reff = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=v)["acc_dudt"]
+        out = otoo.otoo_sph_force(dev(h), rho, P, G, vel=None if v is None else dev(v)).cpu().numpy()
+        e, _ = acc_err(out, reff)
+        assert e.max() <= TOL, e.max()
+        if v is not None:
+            du_rms = np.sqrt((reff[:, 3] ** 2).mean())
+            de = np.abs(out[:, 3] - reff[:, 3]) / np.maximum(np.abs(reff[:, 3]), 1e-2 * du_rms)
+            assert de.max() <= TOL, de.max()
+        else:
+            assert np.all(out[:, 3] == 0)
+
+
+def test_status_codes(otoo):
+    from paper_1206_1199_b200 import binding
+    fresh = binding.Otoo(max_particles=1000)
+    out = torch.empty((10, 4), device="cuda")
+    with pytest.raises(binding.OtooError) as e:
+        fresh.otoo_gravity(0.01, 0.5, 64, out=out)
+    assert e.value.status == binding.OTOO_ERR_NOT_BUILT
+    pm = dev(gen.plummer(2000, 1))
+    with pytest.raises(binding.OtooError) as e:
+        fresh.otoo_build_tree(pm, 16)
+    assert e.value.status == binding.OTOO_ERR_CAPACITY
+    fresh.otoo_build_tree(pm[:500].contiguous(), 16)
+    for bad in (dict(eps=-1.0, theta=0.5, group_size=64), dict(eps=0.01, theta=-0.5, group_size=64),
+                dict(eps=0.01, theta=0.5, group_size=48)):
+        with pytest.raises(binding.OtooError) as e:
+            fresh.otoo_gravity(**bad)
+        assert e.value.status == binding.OTOO_ERR_INVALID_ARG
+    with pytest.raises(binding.OtooError) as e:
+        fresh.otoo_build_tree(pm[:500].contiguous(), 0)
+    assert e.value.status == binding.OTOO_ERR_INVALID_ARG
+    fresh.otoo_build_tree(None, 16)          # N = 0: no-op, context not built
+    with pytest.raises(binding.OtooError) as e:
+        fresh.otoo_tree_info()
+    assert e.value.status == binding.OTOO_ERR_NOT_BUILT
+    fresh.close()
+
+
+def test_host_entry_point(otoo, orc):
+    pm = gen.plummer(10000, 5)
+    out = otoo.otoo_gravity_host(pm, 16, 0.01, 0.5, 64)
+    ref = orc.Tree(pm, 16).gravity(float(np.float32(0.01)), 0.5, 64)
+    e, _ = acc_err(out, ref["acc_pot"])
+    assert e.max() <= TOL
