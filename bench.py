@@ -1,0 +1,255 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the OTOO force path on B200.
+
+A step = one pass of the whole hot path (tree build + fused walk/gravity)
+over one batch of synthetic particles already resident in HBM.  metric = gravity
+interactions/s (R11 count / device time of the whole step).  `roofline` is for the dominant
+kernel (walk_gravity_kernel) against the non-tensor FP32 peak; `e2e` goes through the host-buffer
+C-ABI call; `cpu_baseline` is the fp64 oracle timed on this box's host cores.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--theta 0.6]
+    python bench.py --impl reference ...      # times the oracle (CPU) on the same workload
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import generators as gen  # noqa: E402
+
+METRIC = "gravity_interactions_per_s"
+UNIT = "interactions/s"
+FLOPS_PER_INTERACTION = 20
+SM_LANES = 128                      # FP32 lanes per SM
+NOMINAL_SM_MHZ = 1965.0
+
+
+def workload(name: str, theta, seed: int):
+    cfg = dict(gen.CONFIGS[name])
+    if theta is not None:
+        cfg["theta"] = theta
+    pm = gen.make(cfg["kind"], cfg["n"], seed)
+    return cfg, pm
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi style clock/throttle sampling during the timed region (via NVML)."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def result(self):
+        self.stop_flag = True
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": []}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+def run_reference(args, rank):
+    """The reference arm of this tier: the oracle as it stands, on the host cores."""
+    if rank != 0:
+        return
+    from oracle import oracle
+    cfg, pm = workload(args.workload, args.theta, args.seed)
+    eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
+    times, inter = [], 0
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        t = oracle.Tree(pm, cfg["n_crit"])
+        r = t.gravity(eps, theta, cfg["group"])
+        dt = time.perf_counter() - t0
+        inter = r["interactions"]
+        del t
+        if it >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    val = inter / (ms * 1e-3)
+    cores = oracle.max_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {cfg['kind']} N={cfg['n']} eps={cfg['eps']} theta={cfg['theta']} "
+                                   f"n_crit={cfg['n_crit']} group={cfg['group']}"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": "whole workload, tree build + walk + fp64 sums per step"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="otoo", choices=["otoo", "reference"])
+    ap.add_argument("--workload", default="C2", choices=sorted(gen.CONFIGS))
+    ap.add_argument("--theta", type=float, default=None)
+    ap.add_argument("--seed", type=int, default=1206)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1206_1199_b200 import binding   # fails loudly if libotoo.so is missing
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    # replicas only: every rank runs the same workload with its own seed
+    cfg, pm = workload(args.workload, args.theta, args.seed + rank)
+    n, G, n_crit = cfg["n"], cfg["group"], cfg["n_crit"]
+    eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
+    o = binding.Otoo(max_particles=n, device=local)
+    d_pm = torch.from_numpy(pm).cuda()
+    out = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def step(timed):
+        flush_buf.fill_(1)                      # L2 flush between steps, outside the timed events
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        e[0].record()
+        o.otoo_build_tree(d_pm, n_crit)
+        l1 = o.otoo_last_stats()["launches"] if not timed else 0
+        e[1].record()
+        o.otoo_gravity(eps, theta, G, out=out)
+        e[2].record()
+        return e, l1
+
+    launches_build = 0
+    for _ in range(max(args.warmup, 3)):
+        _, launches_build = step(False)
+    torch.cuda.synchronize()
+    st = o.otoo_last_stats()
+    launches_step = launches_build + st["launches"]
+    inter = st["sum_interactions"]
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = [step(True)[0] for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.result()
+    t_build = np.array([e[0].elapsed_time(e[1]) for e in evs])
+    t_grav = np.array([e[1].elapsed_time(e[2]) for e in evs])
+    ms_step = float((t_build + t_grav).mean())
+    tot_ms = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
+    tot_inter = torch.tensor([float(inter)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tot_ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot_inter, op=dist.ReduceOp.SUM)
+    ms_max, inter_all = float(tot_ms.item()), float(tot_inter.item())
+    value = inter_all / (ms_max * 1e-3)
+
+    # ---- end to end through the host-buffer C-ABI call (pinned host memory)
+    h_in = torch.from_numpy(pm).pin_memory()
+    h_out = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+    e2e_t = []
+    for it in range(2 + min(args.steps, 5)):
+        flush_buf.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        o.otoo_gravity_host(h_in.numpy(), n_crit, eps, theta, G, out=h_out.numpy())
+        dt = time.perf_counter() - t0
+        if it >= 2:
+            e2e_t.append(dt)
+    e2e_ms = torch.tensor([1e3 * float(np.mean(e2e_t))], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+    e2e_val = inter_all / (float(e2e_ms.item()) * 1e-3)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tflops = sm_count * SM_LANES * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
+    grav_ms = float(t_grav.mean())
+    achieved = FLOPS_PER_INTERACTION * inter / (grav_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "walk_gravity_kernel", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": f"derived: {sm_count} SMs x 128 FP32 lanes x 2 flop x {NOMINAL_SM_MHZ:.0f} MHz (DESIGN.md); "
+                               "FFMA microbenchmark on this pool sustained ~70 TFLOP/s",
+                "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter,
+                "kernel_ms": grav_ms, "interactions_per_s_kernel": inter / (grav_ms * 1e-3),
+                "build_ms": float(t_build.mean())}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {cfg['kind']} N={n} eps={cfg['eps']} theta={cfg['theta']} "
+                                   f"n_crit={n_crit} group={G}",
+                       "l2": "flushed between steps (256 MiB write, outside the timed events)",
+                       "parallelism": "replicas" if world > 1 else "single"},
+            "gflops": FLOPS_PER_INTERACTION * value / 1e9,
+            "interactions_per_step": inter_all, "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
+                    "ms_per_step": float(e2e_ms.item())},
+            "gpu_launches": int(launches_step * args.steps), "roofline": roofline}
+
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import oracle
+        t0 = time.perf_counter()
+        t = oracle.Tree(pm, n_crit)
+        r = t.gravity(eps, theta, G, forces=True)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": r["interactions"] / dt, "unit": UNIT, "cores": oracle.max_threads(),
+                                "kind": "oracle", "ms_per_step": 1e3 * dt,
+                                "sample": "whole workload, one step: tree build + walk + fp64 sums"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -57,7 +57,7 @@ def lib():
         L.orc_rb2.argtypes = [vp, dbl, i32, vp]
         L.orc_direct_sum.argtypes = [i64, vp, dbl, i64, vp, vp]
         L.orc_gravity.restype = C.c_uint64
-        L.orc_gravity.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, vp, vp, vp]
+        L.orc_gravity.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, vp, vp, vp, vp]
         L.orc_group_lists.argtypes = [vp, dbl, i32, i32, i64, vp, vp]
         L.orc_sph_cell_radii.argtypes = [vp, vp, vp, vp]
         L.orc_sph_density.restype = C.c_uint64
@@ -167,9 +167,10 @@ class Tree:
         nt = np.zeros(ng, dtype=np.uint32)
         nc = np.zeros(ng, dtype=np.uint32)
         npart = np.zeros(ng, dtype=np.uint32)
+        asum = np.zeros(self.N, dtype=np.float64) if forces else None
         tot = lib().orc_gravity(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
-                                int(walk_kind), _p(acc), _p(nt), _p(nc), _p(npart))
-        return dict(acc_pot=acc, n_tests=nt, n_cells=nc, n_parts=npart, interactions=int(tot))
+                                int(walk_kind), _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
+        return dict(acc_pot=acc, n_tests=nt, n_cells=nc, n_parts=npart, interactions=int(tot), abs_sum=asum)
 
     def group_lists(self, theta, group_size, g, n_cells, n_parts, mac_kind=0):
         cells = np.empty(max(int(n_cells), 1), dtype=np.uint32)

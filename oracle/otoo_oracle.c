@@ -342,10 +342,10 @@ static void walk_stackless(const orc_tree* t, const float* rb2, const gbox_t* g,
 }
 
 /* R10: softened Plummer sums, fp64, with the fp32-rounded cell data the walk uses. */
-static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double e2, double* out) {
+static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double e2, double* out, double* abs_out) {
   const float* p = t->spos + 4 * slot;
   double xi = p[0], yi = p[1], zi = p[2];
-  double ax = 0, ay = 0, az = 0, ph = 0;
+  double ax = 0, ay = 0, az = 0, ph = 0, asum = 0;
   for (int64_t k = 0; k < L->nc; k++) {
     const float* c = t->com_m + 4 * (int64_t)L->cells[k];
     double dx = (double)c[0] - xi, dy = (double)c[1] - yi, dz = (double)c[2] - zi;
@@ -354,6 +354,7 @@ static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double 
     double ri = 1.0 / sqrt(r2), m = c[3];
     double mr3 = m * ri * ri * ri;
     ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= m * ri;
+    asum += mr3 * sqrt(dx * dx + dy * dy + dz * dz);   /* |a_ij|, for the test's error bound */
   }
   for (int64_t k = 0; k < L->np; k++) {
     int64_t j = L->parts[k];
@@ -365,12 +366,14 @@ static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double 
     double ri = 1.0 / sqrt(r2), m = q[3];
     double mr3 = m * ri * ri * ri;
     ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= m * ri;
+    asum += mr3 * sqrt(dx * dx + dy * dy + dz * dz);   /* |a_ij|, for the test's error bound */
   }
   out[0] = ax; out[1] = ay; out[2] = az; out[3] = ph;
+  if (abs_out) *abs_out = asum;
 }
 
 uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
-                     double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts) {
+                     double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
   int64_t N = t->N, ng = (N + G - 1) / G;
   float* rb2 = (float*)malloc(4 * t->ncell);
   orc_rb2(t, theta, mac_kind, rb2);
@@ -390,7 +393,8 @@ uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac
       if (n_parts) n_parts[g] = (uint32_t)L.np;
       total += (uint64_t)(b - a) * (uint64_t)(L.nc + L.np);   /* R11 */
       if (acc_pot)
-        for (int64_t s = a; s < b; s++) grav_sums(t, &L, s, e2, acc_pot + 4 * (int64_t)t->perm[s]);
+        for (int64_t s = a; s < b; s++)
+          grav_sums(t, &L, s, e2, acc_pot + 4 * (int64_t)t->perm[s], abs_sum ? abs_sum + t->perm[s] : NULL);
     }
     free(L.cells); free(L.parts);
   }

@@ -65,7 +65,7 @@ void orc_rb2(const orc_tree*, double theta, int mac_kind, float* rb2 /*ncell*/);
  * (acc_pot NULL = count only). Returns total interactions (R11). */
 uint64_t orc_gravity(const orc_tree*, double eps, double theta, int group_size, int mac_kind,
                      int walk_kind, double* acc_pot /*4N*/, uint32_t* n_tests, uint32_t* n_cells,
-                     uint32_t* n_parts);
+                     uint32_t* n_parts, double* abs_sum /*N or NULL: sum_j |a_ij| over the same lists*/);
 /* the lists of one group (sizes from orc_gravity counters) */
 void orc_group_lists(const orc_tree*, double theta, int group_size, int mac_kind, int64_t g,
                      uint32_t* cell_ids, uint32_t* part_slots);

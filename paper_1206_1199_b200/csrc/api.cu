@@ -114,7 +114,8 @@ void otoo_destroy(otoo_ctx* ctx) {
                   ctx->sorted_h, ctx->sorted_aux, ctx->sorted_vel, ctx->cell_cm, ctx->cell_b, ctx->c_first, ctx->c_count,
                   ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_sph,
                   ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
-                  ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums};
+                  ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums,
+                  ctx->pool_slots, ctx->pool_seq, ctx->walk_shared};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);

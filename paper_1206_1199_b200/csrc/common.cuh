@@ -69,6 +69,9 @@ struct otoo_ctx {
   uint32_t* walk_spill;  // OTOO_WALK_SPILL entries per resident warp
   int64_t spill_warps;
   unsigned long long* d_sums; // [0] tests [1] interactions [2] cells [3] parts
+  void* pool_slots;      // task pool (walk.cuh): TaskSlot[OTOO_POOL_SLOTS]
+  void* pool_seq;        // uint32 sequence numbers
+  void* walk_shared;     // WalkShared control block
 
   // ---- state
   bool built;

@@ -20,87 +20,32 @@ __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_
 }
 
 struct GravParams {
-  const float4* spos;
-  const float4* cell_cm;
-  const cellb_t* cell_b;
-  const uint32_t* perm;
-  int64_t N;
-  int64_t ngroups;
+  WalkCommon c;
   float eps2;
-  float4* acc_pot;
-  uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;
-  uint32_t* queue;          // work counter
-  uint32_t* spill;          // OTOO_WALK_SPILL per warp
-  unsigned long long* sums; // tests, interactions, cells, parts
-  int stack_cap;
+  float4* acc_pot;          // zeroed before the launch
 };
 
 constexpr float PAD_POS = 1.0e18f;  // zero-mass padding entries sit far away: contribute exactly 0
 
-// All targets of the lane x list[0..n) (n a multiple of 4).  R10.  13 FP32 lane-ops + 1 MUFU per
-// interaction, issued two targets at a time as FFMA2/FADD2/FMUL2.
-template <int T, bool EPS0>
-__device__ __forceinline__ void eval_list(const float4* __restrict__ list, int n, f32x2 eps2p,
-                                          const f32x2 (&PX)[(T + 1) / 2], const f32x2 (&PY)[(T + 1) / 2],
-                                          const f32x2 (&PZ)[(T + 1) / 2], f32x2 (&AX)[(T + 1) / 2],
-                                          f32x2 (&AY)[(T + 1) / 2], f32x2 (&AZ)[(T + 1) / 2], f32x2 (&PH)[(T + 1) / 2]) {
-  constexpr int NP = (T + 1) / 2;
-  constexpr int PB = NP < 2 ? NP : 2;  // pairs per pass over the list (4 targets)
-#pragma unroll
-  for (int pb = 0; pb < NP; pb += PB) {
-#pragma unroll 4
-    for (int j = 0; j < n; j++) {
-      const float4 s = list[j];
-      const f32x2 sx = pk2(s.x, s.x), sy = pk2(s.y, s.y), sz = pk2(s.z, s.z), sw = pk2(s.w, s.w);
-#pragma unroll
-      for (int q = pb; q < pb + PB; q++) {
-        f32x2 dx = sub2(sx, PX[q]), dy = sub2(sy, PY[q]), dz = sub2(sz, PZ[q]);
-        f32x2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, eps2p)));
-        float r2a, r2b;
-        upk2(r2, r2a, r2b);
-        float ia = rsqrt_approx(r2a), ib = rsqrt_approx(r2b);
-        if (EPS0) { ia = r2a > 0.0f ? ia : 0.0f; ib = r2b > 0.0f ? ib : 0.0f; }  // r = 0 pairs contribute 0
-        f32x2 ri = pk2(ia, ib);
-        f32x2 mri = mul2(sw, ri);
-        f32x2 mr3 = mul2(mri, mul2(ri, ri));
-        PH[q] = sub2(PH[q], mri);
-        AX[q] = fma2(mr3, dx, AX[q]);
-        AY[q] = fma2(mr3, dy, AY[q]);
-        AZ[q] = fma2(mr3, dz, AZ[q]);
-      }
-    }
-  }
-}
+// Gravity visitor: R10 sums.  13 FP32 lane-ops + 1 MUFU per interaction, issued two targets at a
+// time as FFMA2/FADD2/FMUL2; two-level summation (64-entry fp32 partial sums, then totals).
+template <int T_, bool EPS0>
+struct GravVisitor {
+  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64;
+  const GravParams& p;
+  float pm[T];
+  float glo[3], ghi[3];
+  f32x2 PX[NP], PY[NP], PZ[NP], AX[NP], AY[NP], AZ[NP], PH[NP];
+  f32x2 eps2p;
+  unsigned selfmask;
+  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_) { eps2p = pk2(p_.eps2, p_.eps2); }
 
-template <int T, bool EPS0>
-__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(GravParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  constexpr int NP = (T + 1) / 2;
-  constexpr int G = 32 * T;
-  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
-  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
-                  warp * OTOO_WALK_STACK_MAX;
-  const int64_t gwarp = (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp;
-  WarpStack st;
-  const f32x2 eps2p = pk2(p.eps2, p.eps2);
-  unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;
-
-  for (;;) {
-    uint32_t g = 0;
-    if (lane == 0) g = atomicAdd(p.queue, 1u);
-    g = __shfl_sync(0xFFFFFFFFu, g, 0);
-    if ((int64_t)g >= p.ngroups) break;
-    const int64_t g0 = (int64_t)g * G;
-    const int gcount = (int)((p.N - g0) < G ? (p.N - g0) : G);
-
-    // ---- targets (H7): lane holds slots g0 + t*32 + lane; out-of-range lanes mirror slot g0
-    float px[T], py[T], pz[T], pm[T];
-    float glo[3], ghi[3];
+  __device__ __forceinline__ void load_group(int64_t g0, int lane) {
+    float px[T], py[T], pz[T];
 #pragma unroll
-    for (int t = 0; t < T; t++) {
+    for (int t = 0; t < T; t++) {   // H7: lane holds slots g0 + t*32 + lane; out-of-range lanes mirror slot g0
       int64_t s = g0 + t * 32 + lane;
-      float4 v = p.spos[s < p.N ? s : g0];
+      float4 v = p.c.spos[s < p.c.N ? s : g0];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z; pm[t] = v.w;
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
@@ -116,113 +61,65 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(Grav
         glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
         ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
       }
-    f32x2 PX[NP], PY[NP], PZ[NP], AX[NP], AY[NP], AZ[NP], PH[NP];
 #pragma unroll
     for (int q = 0; q < NP; q++) {
       const int t1 = (2 * q + 1 < T) ? 2 * q + 1 : 2 * q;
       PX[q] = pk2(px[2 * q], px[t1]); PY[q] = pk2(py[2 * q], py[t1]); PZ[q] = pk2(pz[2 * q], pz[t1]);
       AX[q] = AY[q] = AZ[q] = PH[q] = pk2(0.0f, 0.0f);
     }
-
-    // ---- walk
-    st.init(stk, p.spill + gwarp * OTOO_WALK_SPILL, p.stack_cap);
-    if (lane == 0) stk[0] = 0u;  // root
-    __syncwarp();
-    st.sp = 1;
-    int nlist = 0;
-    uint32_t ntests = 0, ncells = 0, nparts = 0;
-    unsigned selfmask = 0;
-
-    auto flush = [&]() {
-      int n4 = (nlist + 3) & ~3;
-      if (lane < n4 - nlist) list[nlist + lane] = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f);
-      __syncwarp();
-      eval_list<T, EPS0>(list, n4, eps2p, PX, PY, PZ, AX, AY, AZ, PH);
-      __syncwarp();
-      nlist = 0;
-    };
-
-    while (!st.empty()) {
-      if (st.sp == 0) st.refill(lane);
-      const int k = st.sp < 32 ? st.sp : 32;
-      const bool have = lane < k;
-      uint32_t cell = 0;
-      if (have) cell = stk[st.sp - k + lane];
-      __syncwarp();
-      st.sp -= k;
-      float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
-      cellb_t B = make_uint4(0u, 0u, 0u, 0u);
-      bool accept = false;
-      if (have) {
-        A = __ldg(p.cell_cm + cell);
-        B = __ldg(p.cell_b + cell);
-        float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
-        accept = d2 > __uint_as_float(B.x);  // strict: equality opens (R8)
-      }
-      ntests += (uint32_t)k;
-      const bool leaf = (B.w & 1u) != 0u;
-      const bool open_leaf = have && !accept && leaf;
-      const bool open_int = have && !accept && !leaf;
-
-      // accepted cells -> list (the cell is a virtual particle at its centre of mass, L43)
-      const unsigned am = __ballot_sync(0xFFFFFFFFu, accept);
-      const int na = __popc(am);
-      if (na) {
-        if (nlist + na > OTOO_LIST_CAP) flush();
-        if (accept) list[nlist + __popc(am & lanemask_lt_())] = A;
-        nlist += na; ncells += (uint32_t)na;
-      }
-      // opened internal cells -> push children (L57 rule 1: follow `more`)
-      {
-        const int nch = open_int ? (int)B.z : 0;
-        const int inc = warp_inclusive_scan(nch, lane);
-        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-        if (total) {
-          st.reserve(total, lane);
-          const int o = st.sp + inc - nch;
-          for (int i = 0; i < nch; i++) stk[o + i] = B.y + (uint32_t)i;
-          __syncwarp();
-          st.sp += total;
-        }
-      }
-      // opened leaves -> their particles (L57 rule 3)
-      const unsigned lm = __ballot_sync(0xFFFFFFFFu, open_leaf);
-      if (lm) {
-        const int cnt = open_leaf ? (int)B.z : 0;
-        const int inc = warp_inclusive_scan(cnt, lane);
-        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-        // which of my targets sit in an opened leaf (their self term is in the list)
-        unsigned m = lm;
-        while (m) {
-          const int src = __ffs(m) - 1; m &= m - 1;
-          const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), c = __shfl_sync(0xFFFFFFFFu, B.z, src);
+    selfmask = 0;
+  }
+  __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
+    A = __ldg(p.c.cell_cm + cell);
+    B = __ldg(p.c.cell_b + cell);
+    float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
+    return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
+  }
+  __device__ __forceinline__ void put_particle(float4* dst, uint32_t slot) { *dst = p.c.spos[slot]; }
+  __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
+  __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
 #pragma unroll
-          for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < c) selfmask |= 1u << t;
-        }
-        if (total <= OTOO_LIST_CAP) {
-          if (nlist + total > OTOO_LIST_CAP) flush();
-          const int o = nlist + inc - cnt;
-          for (int i = 0; i < cnt; i++) list[o + i] = p.spos[B.y + i];
-          nlist += total;
-        } else {  // huge leaves (coincident points at level 21): one leaf at a time, 32 particles a chunk
-          m = lm;
-          while (m) {
-            const int src = __ffs(m) - 1; m &= m - 1;
-            const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), c = __shfl_sync(0xFFFFFFFFu, B.z, src);
-            for (uint32_t i = 0; i < c; i += 32) {
-              if (nlist + 32 > OTOO_LIST_CAP) flush();
-              if (i + lane < c) list[nlist + lane] = p.spos[f + i + lane];
-              nlist += (int)((c - i) < 32u ? (c - i) : 32u);
-            }
+    for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
+  }
+  __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
+#pragma unroll
+    for (int pb = 0; pb < NP; pb += PB) {
+      for (int j0 = 0; j0 < n; j0 += BLK) {
+        const int je = j0 + BLK < n ? j0 + BLK : n;
+        f32x2 cx[PB], cy[PB], cz[PB], cp[PB];
+#pragma unroll
+        for (int q = 0; q < PB; q++) cx[q] = cy[q] = cz[q] = cp[q] = 0ull;
+#pragma unroll 4
+        for (int j = j0; j < je; j++) {
+          const float4 s = list[j];
+          const f32x2 sx = pk2(s.x, s.x), sy = pk2(s.y, s.y), sz = pk2(s.z, s.z), sw = pk2(s.w, s.w);
+#pragma unroll
+          for (int q = 0; q < PB; q++) {
+            f32x2 dx = sub2(sx, PX[pb + q]), dy = sub2(sy, PY[pb + q]), dz = sub2(sz, PZ[pb + q]);
+            f32x2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, eps2p)));
+            float r2a, r2b;
+            upk2(r2, r2a, r2b);
+            float ia = rsqrt_approx(r2a), ib = rsqrt_approx(r2b);
+            if (EPS0) { ia = r2a > 0.0f ? ia : 0.0f; ib = r2b > 0.0f ? ib : 0.0f; }  // r = 0 pairs contribute 0
+            f32x2 ri = pk2(ia, ib);
+            f32x2 mri = mul2(sw, ri);
+            f32x2 mr3 = mul2(mri, mul2(ri, ri));
+            cp[q] = sub2(cp[q], mri);
+            cx[q] = fma2(mr3, dx, cx[q]);
+            cy[q] = fma2(mr3, dy, cy[q]);
+            cz[q] = fma2(mr3, dz, cz[q]);
           }
         }
-        nparts += (uint32_t)total;
-        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < PB; q++) {
+          AX[pb + q] = add2(AX[pb + q], cx[q]); AY[pb + q] = add2(AY[pb + q], cy[q]);
+          AZ[pb + q] = add2(AZ[pb + q], cz[q]); PH[pb + q] = add2(PH[pb + q], cp[q]);
+        }
       }
     }
-    if (nlist) flush();
-
-    // ---- results (H10): original order; remove the self term from phi (R10)
+  }
+  // H10: original order; the self term is removed from phi by whichever task saw it (R10)
+  __device__ __forceinline__ void store(int64_t g0, int lane) {
     const float rie = EPS0 ? 0.0f : rsqrt_approx(p.eps2);
 #pragma unroll
     for (int t = 0; t < T; t++) {
@@ -231,29 +128,45 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(Grav
       upk2(AX[t >> 1], ax0, ax1); upk2(AY[t >> 1], ay0, ay1); upk2(AZ[t >> 1], az0, az1); upk2(PH[t >> 1], ph0, ph1);
       float4 o = (t & 1) ? make_float4(ax1, ay1, az1, ph1) : make_float4(ax0, ay0, az0, ph0);
       if ((selfmask >> t) & 1u) o.w = __fmaf_rn(pm[t], rie, o.w);
-      if (s < p.N) p.acc_pot[p.perm[s]] = o;
+      if (s < p.c.N) {
+        float* dst = reinterpret_cast<float*>(p.acc_pot + p.c.perm[s]);
+        atomicAdd(dst + 0, o.x); atomicAdd(dst + 1, o.y); atomicAdd(dst + 2, o.z); atomicAdd(dst + 3, o.w);
+      }
     }
-    const uint32_t nt = ntests;  // warp-uniform by construction
-    if (lane == 0) { p.g_ntests[g] = nt; p.g_ncells[g] = ncells; p.g_nparts[g] = nparts; }
-    tot_tests += nt; tot_cells += ncells; tot_parts += nparts;
-    tot_inter += (unsigned long long)gcount * (ncells + nparts);
   }
-  if (lane == 0 && tot_tests) {
-    atomicAdd(p.sums + 0, tot_tests); atomicAdd(p.sums + 1, tot_inter);
-    atomicAdd(p.sums + 2, tot_cells); atomicAdd(p.sums + 3, tot_parts);
-  }
+};
+
+template <int T, bool EPS0>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(const GravParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
+  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
+                  warp * OTOO_WALK_STACK_MAX;
+  GravVisitor<T, EPS0> v(p);
+  walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
 
+// reset the control block and the pool's sequence numbers (tickets restart from 0 every launch)
+__global__ void __launch_bounds__(256) walk_init_kernel(WalkShared* ws, uint32_t* seq, int ngroups) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < OTOO_POOL_SLOTS) seq[i] = (uint32_t)i;
+  if (i == 0) { ws->queue = 0; ws->head = 0; ws->tail = 0; ws->outstanding = ngroups; }
+}
+
+template <int T, bool EPS0>
+otoo_status launch_walk2(otoo_ctx* ctx, const GravParams& p, int grid, size_t smem, cudaStream_t st) {
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_kernel<T, EPS0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 1;
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_gravity_kernel<T, EPS0>, OTOO_WALK_WARPS * 32, smem));
+  if (occ < 1) occ = 1;
+  if (grid > ctx->sm_count * occ) grid = ctx->sm_count * occ;   // persistent: every CTA resident
+  walk_gravity_kernel<T, EPS0><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
+  return OTOO_OK;
+}
 template <int T>
 otoo_status launch_walk(otoo_ctx* ctx, const GravParams& p, bool eps0, int grid, size_t smem, cudaStream_t st) {
-  if (eps0) {
-    OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    walk_gravity_kernel<T, true><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
-  } else {
-    OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    walk_gravity_kernel<T, false><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
-  }
-  return OTOO_OK;
+  return eps0 ? launch_walk2<T, true>(ctx, p, grid, smem, st) : launch_walk2<T, false>(ctx, p, grid, smem, st);
 }
 
 }  // namespace
@@ -262,25 +175,46 @@ size_t otoo_walk_smem_bytes() {
   return (size_t)OTOO_WALK_WARPS * (OTOO_LIST_CAP * sizeof(float4) + OTOO_WALK_STACK_MAX * sizeof(uint32_t));
 }
 
-otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, float* d_acc_pot, cudaStream_t st) {
+// Common launch preparation of the walk kernels: persistent grid, task pool, zeroed counters.
+otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st) {
   const int64_t ngroups = cdiv(ctx->N, G);
   OTOO_TRY(otoo_ensure_groups(ctx, ngroups));
-  const size_t smem = otoo_walk_smem_bytes();
-  int per_sm = (int)((227 * 1024) / (smem + 1024));
-  if (per_sm > 16 / OTOO_WALK_WARPS * 4) per_sm = 16 / OTOO_WALK_WARPS * 4;
+  *smem = otoo_walk_smem_bytes();
+  int per_sm = (int)((227 * 1024) / (*smem + 1024));
   if (per_sm < 1) per_sm = 1;
-  int grid = ctx->sm_count * per_sm;
-  if ((int64_t)grid * OTOO_WALK_WARPS > ngroups) grid = (int)cdiv(ngroups, OTOO_WALK_WARPS);
-  OTOO_TRY(otoo_ensure_spill(ctx, (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS));
-  rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, theta, ctx->cell_b);
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters + 33, 0, sizeof(uint32_t), st));
+  const int64_t warps = (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS;
+  if (warps >= OTOO_POOL_MARGIN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "internal: task pool margin below resident warps");
+  *grid = ctx->sm_count * per_sm;
+  if ((int64_t)*grid * OTOO_WALK_WARPS > ngroups) *grid = (int)cdiv(ngroups, OTOO_WALK_WARPS);
+  OTOO_TRY(otoo_ensure_spill(ctx, warps));
+  if (!ctx->pool_slots) {
+    OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->pool_slots, sizeof(TaskSlot) * (size_t)OTOO_POOL_SLOTS));
+    OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->pool_seq, sizeof(uint32_t) * (size_t)OTOO_POOL_SLOTS));
+    OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->walk_shared, sizeof(WalkShared)));
+  }
+  walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq, (int)ngroups);
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)ngroups, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)ngroups, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)ngroups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 4 * sizeof(unsigned long long), st));
+  c->spos = ctx->spos; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
+  c->N = ctx->N; c->ngroups = ngroups;
+  c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
+  c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
+  c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
+  ctx->launches += 1;
+  ctx->last_group_size = G; ctx->last_ngroups = ngroups;
+  return OTOO_OK;
+}
+
+otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, float* d_acc_pot, cudaStream_t st) {
   GravParams p;
-  p.spos = ctx->spos; p.cell_cm = ctx->cell_cm; p.cell_b = ctx->cell_b; p.perm = ctx->val[0];
-  p.N = ctx->N; p.ngroups = ngroups; p.eps2 = eps * eps;
+  int grid; size_t smem;
+  OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st));
+  rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, theta, ctx->cell_b);
+  OTOO_CUDA(ctx, cudaMemsetAsync(d_acc_pot, 0, 16 * (size_t)ctx->N, st));
+  p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);
-  p.g_ntests = ctx->g_ntests; p.g_ncells = ctx->g_ncells; p.g_nparts = ctx->g_nparts;
-  p.queue = ctx->d_counters + 33; p.spill = ctx->walk_spill; p.sums = ctx->d_sums; p.stack_cap = ctx->walk_stack;
   const bool eps0 = !(eps > 0.0f);
   switch (G) {
     case 32: OTOO_TRY(launch_walk<1>(ctx, p, eps0, grid, smem, st)); break;
@@ -291,6 +225,6 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, floa
   }
   ctx->launches += 2;
   OTOO_CUDA(ctx, cudaGetLastError());
-  ctx->walked = true; ctx->last_group_size = G; ctx->last_ngroups = ngroups;
+  ctx->walked = true;
   return OTOO_OK;
 }

@@ -82,54 +82,33 @@ __global__ void __launch_bounds__(256) sph_radii_finish_kernel(const unsigned lo
 }
 
 struct SphParams {
-  const float4* spos;
-  const float* hs;
+  WalkCommon c;
+  const float* hs;      // h, sorted
   const float4* aux;    // (h, P/rho^2, -, -) sorted
   const float4* svel;   // sorted velocities or NULL
-  const float4* cell_cm;
-  const cellb_t* cell_b;
-  const float2* c_sph;
-  const uint32_t* perm;
-  int64_t N, ngroups;
-  float* rho; uint32_t* nngb;   // density outputs
-  float4* acc;                  // force output
-  uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;
-  uint32_t* queue; uint32_t* spill; unsigned long long* sums;
-  int stack_cap;
+  const float2* c_sph;  // (b_max, r_SPH) per cell
+  float* rho; uint32_t* nngb;   // density outputs (zeroed before the launch)
+  float4* acc;                  // force output (zeroed before the launch)
 };
 
-__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// MODE 0: density (R16).  MODE 1: pressure force (R17).  MODE 2: pressure force + du/dt.
+template <int T_, int MODE>
+struct SphVisitor {
+  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
+  const SphParams& p;
+  float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
+  float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T];
+  uint32_t cnt_ngb[T];
+  float glo[3], ghi[3], hmax;
+  __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_) {}
 
-// MODE 0: density.  MODE 1: pressure force.  MODE 2: pressure force + du/dt.
-template <int T, int MODE>
-__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(SphParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  constexpr int G = 32 * T;
-  constexpr int E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);   // float4 per list entry
-  constexpr int CAP = OTOO_LIST_CAP / E;                   // entries
-  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
-  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
-                  warp * OTOO_WALK_STACK_MAX;
-  const int64_t gwarp = (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp;
-  WarpStack st;
-  unsigned long long tot_tests = 0, tot_inter = 0, tot_parts = 0;
-  const float PI_F = 3.14159265358979323846f;
-
-  for (;;) {
-    uint32_t g = 0;
-    if (lane == 0) g = atomicAdd(p.queue, 1u);
-    g = __shfl_sync(0xFFFFFFFFu, g, 0);
-    if ((int64_t)g >= p.ngroups) break;
-    const int64_t g0 = (int64_t)g * G;
-    const int gcount = (int)((p.N - g0) < G ? (p.N - g0) : G);
-    float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
-    float glo[3], ghi[3], hmax = 0.0f;
+  __device__ __forceinline__ void load_group(int64_t g0, int lane) {
+    hmax = 0.0f;
 #pragma unroll
     for (int t = 0; t < T; t++) {
       int64_t s = g0 + t * 32 + lane;
-      s = s < p.N ? s : g0;
-      float4 v = p.spos[s];
+      s = s < p.c.N ? s : g0;
+      float4 v = p.c.spos[s];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z;
       if (MODE == 0) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
       else { float4 a = p.aux[s]; ph[t] = a.x; ppr[t] = a.y; }
@@ -151,148 +130,117 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(SphParam
       }
       hmax = fmaxf(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, o));
     }
-    float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T];
-    uint32_t cnt_ngb[T];
 #pragma unroll
     for (int t = 0; t < T; t++) {
       h2[t] = __fmul_rn(ph[t], ph[t]); hinv[t] = 1.0f / ph[t];
       o0[t] = o1[t] = o2[t] = o3[t] = 0.0f; cnt_ngb[t] = 0;
     }
-
-    st.init(stk, p.spill + gwarp * OTOO_WALK_SPILL, p.stack_cap);
-    if (lane == 0) stk[0] = 0u;
-    __syncwarp();
-    st.sp = 1;
-    int nlist = 0;
-    uint32_t ntests = 0, nparts = 0;
-
-    auto flush = [&]() {
-      __syncwarp();
-      for (int j = 0; j < nlist; j++) {
-        const float4 a = list[E * j];
-        float4 b = make_float4(0, 0, 0, 0), c = make_float4(0, 0, 0, 0);
-        if (E >= 2) b = list[E * j + 1];
-        if (E >= 3) c = list[E * j + 2];
+  }
+  // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105)
+  __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
+    A = __ldg(p.c.cell_cm + cell);
+    B = __ldg(p.c.cell_b + cell);
+    float2 rr = __ldg(p.c_sph + cell);
+    float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
+    float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));
+    return d2 <= __fmul_rn(R, R) ? 2 : 0;
+  }
+  __device__ __forceinline__ void put_particle(float4* dst, uint32_t s) {
+    dst[0] = p.c.spos[s];
+    if (E >= 2) dst[1] = p.aux[s];
+    if (E >= 3) dst[2] = p.svel[s];
+  }
+  __device__ __forceinline__ void pad(float4* dst) {
+    dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass
+    if (E >= 2) dst[1] = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+    if (E >= 3) dst[2] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
+  __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
+    const float PI_F = 3.14159265358979323846f;
+    for (int j = 0; j < n; j++) {
+      const float4 a = list[E * j];
+      float4 b = make_float4(0, 0, 0, 0), c = make_float4(0, 0, 0, 0);
+      if (E >= 2) b = list[E * j + 1];
+      if (E >= 3) c = list[E * j + 2];
 #pragma unroll
-        for (int t = 0; t < T; t++) {
-          if (MODE == 0) {
-            // R16: the neighbour decision in fp32, exactly this chain
-            float dx = __fsub_rn(a.x, px[t]), dy = __fsub_rn(a.y, py[t]), dz = __fsub_rn(a.z, pz[t]);
-            float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            bool in = r2 < h2[t];
-            float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
-            float u = 1.0f - q;
-            float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
-            float w2 = 2.0f * u * u * u;
-            float w = q <= 0.5f ? w1 : w2;
-            o0[t] = fmaf(in ? a.w : 0.0f, w, o0[t]);
-            cnt_ngb[t] += in ? 1u : 0u;
-          } else {
-            // R17: d = x_i - x_j; decision r2 < max(h_i,h_j)^2 in fp32, same r2 chain on (x_j - x_i)
-            float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
-            float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
-            float hj = b.x, hm = fmaxf(ph[t], hj);
-            bool in = (r2 < __fmul_rn(hm, hm)) && (r2 > 0.0f);
-            float rinv = rsqrt_approx(fmaxf(r2, 1e-37f));
-            float r = r2 * rinv;
-            float hjinv = __fdividef(1.0f, hj);
-            float qi = r * hinv[t], qj = r * hjinv;
-            float ui = 1.0f - qi, uj = 1.0f - qj;
-            float di = qi <= 0.5f ? fmaf(18.0f * qi, qi, -12.0f * qi) : (qi < 1.0f ? -6.0f * ui * ui : 0.0f);
-            float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
-            float hi2 = hinv[t] * hinv[t], hj2 = hjinv * hjinv;
-            float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2 * hj2) * rinv;   // (dW_i + dW_j)/(2r)
-            float f = in ? a.w * (ppr[t] + b.y) * gw : 0.0f;
-            // a_i -= f * (x_i - x_j) = += f * e
-            o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
-            if (MODE == 2) {
-              float vd = fmaf(vx[t] - c.x, -ex, fmaf(vy[t] - c.y, -ey, (vz[t] - c.z) * -ez));  // (v_i - v_j).(x_i - x_j)
-              o3[t] = fmaf(0.5f * f, vd, o3[t]);
-            }
+      for (int t = 0; t < T; t++) {
+        // the fp32 neighbour decision of R16/R17: exactly this chain on (x_j - x_i)
+        float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
+        float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
+        if (MODE == 0) {
+          bool in = r2 < h2[t];
+          float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
+          float u = 1.0f - q;
+          float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
+          float w2 = 2.0f * u * u * u;
+          float w = q <= 0.5f ? w1 : w2;
+          o0[t] = fmaf(in ? a.w : 0.0f, w, o0[t]);
+          cnt_ngb[t] += in ? 1u : 0u;
+        } else {
+          float hj = b.x, hm = fmaxf(ph[t], hj);
+          bool in = (r2 < __fmul_rn(hm, hm)) && (r2 > 0.0f);
+          float rinv = rsqrt_approx(fmaxf(r2, 1e-37f));
+          float r = r2 * rinv;
+          float hjinv = __fdividef(1.0f, hj);
+          float qi = r * hinv[t], qj = r * hjinv;
+          float ui = 1.0f - qi, uj = 1.0f - qj;
+          float di = qi <= 0.5f ? fmaf(18.0f * qi, qi, -12.0f * qi) : (qi < 1.0f ? -6.0f * ui * ui : 0.0f);
+          float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
+          float hi2 = hinv[t] * hinv[t], hj2 = hjinv * hjinv;
+          float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2 * hj2) * rinv;   // (dW_i + dW_j)/(2r)
+          float f = in ? a.w * (ppr[t] + b.y) * gw : 0.0f;
+          // a_i -= f (x_i - x_j)  =  += f e
+          o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
+          if (MODE == 2) {
+            // (v_i - v_j).(x_i - x_j) = -(v_i - v_j).e
+            float vd = -fmaf(vx[t] - c.x, ex, fmaf(vy[t] - c.y, ey, (vz[t] - c.z) * ez));
+            o3[t] = fmaf(0.5f * f, vd, o3[t]);
           }
         }
-      }
-      __syncwarp();
-      nlist = 0;
-    };
-
-    while (!st.empty()) {
-      if (st.sp == 0) st.refill(lane);
-      const int k = st.sp < 32 ? st.sp : 32;
-      const bool have = lane < k;
-      uint32_t cell = 0;
-      if (have) cell = stk[st.sp - k + lane];
-      __syncwarp();
-      st.sp -= k;
-      cellb_t B = make_uint4(0u, 0u, 0u, 0u);
-      bool open = false;
-      if (have) {
-        float4 A = __ldg(p.cell_cm + cell);
-        B = __ldg(p.cell_b + cell);
-        float2 rr = __ldg(p.c_sph + cell);
-        float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
-        float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));     // R15
-        open = d2 <= __fmul_rn(R, R);
-      }
-      ntests += (uint32_t)k;
-      const bool leaf = (B.w & 1u) != 0u;
-      const bool open_leaf = open && leaf, open_int = open && !leaf;
-      {
-        const int nch = open_int ? (int)B.z : 0;
-        const int inc = warp_inclusive_scan(nch, lane);
-        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-        if (total) {
-          st.reserve(total, lane);
-          const int o = st.sp + inc - nch;
-          for (int i = 0; i < nch; i++) stk[o + i] = B.y + (uint32_t)i;
-          __syncwarp();
-          st.sp += total;
-        }
-      }
-      unsigned m = __ballot_sync(0xFFFFFFFFu, open_leaf);
-      while (m) {   // one leaf at a time, 32 particles a chunk
-        const int src = __ffs(m) - 1; m &= m - 1;
-        const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), c = __shfl_sync(0xFFFFFFFFu, B.z, src);
-        for (uint32_t i = 0; i < c; i += 32) {
-          if (nlist + 32 > CAP) flush();
-          if (i + lane < c) {
-            const uint32_t s = f + i + lane;
-            list[E * (nlist + lane)] = p.spos[s];
-            if (E >= 2) list[E * (nlist + lane) + 1] = p.aux[s];
-            if (E >= 3) list[E * (nlist + lane) + 2] = p.svel[s];
-          }
-          nlist += (int)((c - i) < 32u ? (c - i) : 32u);
-        }
-        nparts += c;
       }
     }
-    if (nlist) flush();
-
+  }
+  __device__ __forceinline__ void store(int64_t g0, int lane) {
+    const float PI_F = 3.14159265358979323846f;
 #pragma unroll
     for (int t = 0; t < T; t++) {
       const int64_t s = g0 + t * 32 + lane;
-      if (s < p.N) {
-        const uint32_t i = p.perm[s];
+      if (s < p.c.N) {
+        const uint32_t i = p.c.perm[s];
         if (MODE == 0) {
           float hi3 = hinv[t] * hinv[t] * hinv[t];
-          p.rho[i] = o0[t] * (8.0f / PI_F) * hi3;
-          if (p.nngb) p.nngb[i] = cnt_ngb[t];
-        } else p.acc[i] = make_float4(o0[t], o1[t], o2[t], o3[t]);
+          atomicAdd(p.rho + i, o0[t] * (8.0f / PI_F) * hi3);
+          if (p.nngb) atomicAdd(p.nngb + i, cnt_ngb[t]);
+        } else {
+          float* dst = reinterpret_cast<float*>(p.acc + i);
+          atomicAdd(dst + 0, o0[t]); atomicAdd(dst + 1, o1[t]); atomicAdd(dst + 2, o2[t]);
+          if (MODE == 2) atomicAdd(dst + 3, o3[t]);
+        }
       }
     }
-    if (lane == 0) { p.g_ntests[g] = ntests; p.g_ncells[g] = 0u; p.g_nparts[g] = nparts; }
-    tot_tests += ntests; tot_parts += nparts;
-    tot_inter += (unsigned long long)gcount * nparts;
   }
-  if (lane == 0 && tot_tests) {
-    atomicAdd(p.sums + 0, tot_tests); atomicAdd(p.sums + 1, tot_inter); atomicAdd(p.sums + 3, tot_parts);
-  }
+};
+
+template <int T, int MODE>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
+  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
+                  warp * OTOO_WALK_STACK_MAX;
+  SphVisitor<T, MODE> v(p);
+  walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
 
 template <int MODE>
 otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_t smem, cudaStream_t st) {
+  int occ = 1;
 #define OTOO_SPH_CASE(TT)                                                                                              \
   OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_kernel<TT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_kernel<TT, MODE>, OTOO_WALK_WARPS * 32, smem));  \
+  if (occ < 1) occ = 1;                                                                                                 \
+  if (grid > ctx->sm_count * occ) grid = ctx->sm_count * occ;                                                          \
   walk_sph_kernel<TT, MODE><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
   switch (G) {
     case 32: OTOO_SPH_CASE(1) break;
@@ -308,14 +256,7 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
 otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, int* grid, size_t* smem, cudaStream_t st) {
   if (G != 32 && G != 64 && G != 128 && G != 256)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
-  const int64_t ngroups = cdiv(ctx->N, G);
-  OTOO_TRY(otoo_ensure_groups(ctx, ngroups));
-  *smem = otoo_walk_smem_bytes();
-  int per_sm = (int)((227 * 1024) / (*smem + 1024));
-  if (per_sm < 1) per_sm = 1;
-  *grid = ctx->sm_count * per_sm;
-  if ((int64_t)*grid * OTOO_WALK_WARPS > ngroups) *grid = (int)cdiv(ngroups, OTOO_WALK_WARPS);
-  OTOO_TRY(otoo_ensure_spill(ctx, (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS));
+  OTOO_TRY(otoo_walk_prepare(ctx, G, &p->c, grid, smem, st));
   const unsigned nbN = (unsigned)cdiv(ctx->N, 256), nbC = (unsigned)cdiv(ctx->N_cell, 256);
   // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3)
   gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
@@ -324,13 +265,8 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
                                         ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
   sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
   ctx->launches += 3;
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters + 33, 0, sizeof(uint32_t), st));
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 4 * sizeof(unsigned long long), st));
-  p->spos = ctx->spos; p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr;
-  p->cell_cm = ctx->cell_cm; p->cell_b = ctx->cell_b; p->c_sph = ctx->c_sph; p->perm = ctx->val[0];
-  p->N = ctx->N; p->ngroups = ngroups; p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
-  p->g_ntests = ctx->g_ntests; p->g_ncells = ctx->g_ncells; p->g_nparts = ctx->g_nparts;
-  p->queue = ctx->d_counters + 33; p->spill = ctx->walk_spill; p->sums = ctx->d_sums; p->stack_cap = ctx->walk_stack;
+  p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->c_sph = ctx->c_sph;
+  p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
   ctx->sph_radii_valid = true;
   return OTOO_OK;
 }
@@ -341,10 +277,12 @@ otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float*
   SphParams p; int grid; size_t smem;
   OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
   p.rho = d_rho; p.nngb = d_nngb;
+  OTOO_CUDA(ctx, cudaMemsetAsync(d_rho, 0, 4 * (size_t)ctx->N, st));
+  if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
   OTOO_TRY(launch_sph<0>(ctx, p, G, grid, smem, st));
   ctx->launches += 1;
   OTOO_CUDA(ctx, cudaGetLastError());
-  ctx->walked = true; ctx->last_group_size = G; ctx->last_ngroups = p.ngroups;
+  ctx->walked = true;
   return OTOO_OK;
 }
 
@@ -354,11 +292,12 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
   OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
   gather_force_inputs_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_h, d_rho, d_P, reinterpret_cast<const float4*>(d_vel),
                                                                           ctx->val[0], ctx->N, ctx->sorted_aux, ctx->sorted_vel);
+  OTOO_CUDA(ctx, cudaMemsetAsync(d_acc, 0, 16 * (size_t)ctx->N, st));
   p.acc = reinterpret_cast<float4*>(d_acc);
   if (d_vel) { p.svel = ctx->sorted_vel; OTOO_TRY(launch_sph<2>(ctx, p, G, grid, smem, st)); }
   else OTOO_TRY(launch_sph<1>(ctx, p, G, grid, smem, st));
   ctx->launches += 2;
   OTOO_CUDA(ctx, cudaGetLastError());
-  ctx->walked = true; ctx->last_group_size = G; ctx->last_ngroups = p.ngroups;
+  ctx->walked = true;
   return OTOO_OK;
 }

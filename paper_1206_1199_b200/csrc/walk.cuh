@@ -1,10 +1,17 @@
-// walk.cuh -- warp-level machinery shared by the gravity and SPH walk kernels.
+// walk.cuh -- the warp-level group walk shared by the gravity and SPH kernels.
+//
 // One warp owns one group of G = 32*T Morton-consecutive targets (n_vec targets
-// share one traversal).  The traversal is the paper's "open -> descend, accept -> interact, leaf ->
-// its particles" rule set (L57) run 32 cells at a time from a LIFO stack in shared memory;
-// accepted cells and opened leaves' particles are appended to an interaction list in shared
-// memory, which is consumed (all targets x all entries) whenever it fills.  The list never
+// share one traversal).  The traversal is the paper's rule set (L57: not accepted -> descend,
+// accepted -> interact, particle -> interact) run 32 cells at a time from a LIFO stack in shared
+// memory; accepted cells and opened leaves' particles are appended to an interaction list in
+// shared memory that is consumed (all targets x all entries) whenever it fills.  The list never
 // touches HBM.
+//
+// Load balance: a few groups straddle octant boundaries, have system-sized AABBs and lists up to
+// N entries.  A warp whose stack is long hands its shallowest
+// stack entries (largest subtrees) to a global task pool when other warps are idle or when its
+// shared stack overflows; any warp can run such a task for the same group.  Results are therefore
+// accumulated with atomicAdd into zero-initialised outputs; per-group counters likewise.
 #pragma once
 #include "common.cuh"
 
@@ -23,6 +30,7 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 // R8: squared distance from the group's AABB to a point, the exact fp32 expression both sides use.
 __device__ __forceinline__ float aabb_d2(const float glo[3], const float ghi[3], float cx, float cy, float cz) {
@@ -32,43 +40,244 @@ __device__ __forceinline__ float aabb_d2(const float glo[3], const float ghi[3],
   return __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
 }
 
-// Per-warp LIFO of cell ids: shared memory on top, global-memory spill below it.
-// With 32 cells popped per step the stack stays sorted by level and holds at most 8*32 entries per
-// level, so OTOO_WALK_SPILL entries per warp can never overflow.
-struct WarpStack {
-  uint32_t* s;      // shared, cap entries
-  uint32_t* g;      // global spill area of this warp
-  int cap;          // usable shared entries (>= 512)
-  int sp, gsp;      // warp-uniform
-
-  __device__ __forceinline__ void init(uint32_t* smem, uint32_t* spill, int cap_) { s = smem; g = spill; cap = cap_; sp = 0; gsp = 0; }
-  __device__ __forceinline__ bool empty() const { return sp == 0 && gsp == 0; }
-  // make room for `total` (<= 256) pushes
-  __device__ __forceinline__ void reserve(int total, int lane) {
-    if (sp + total <= cap) return;
-    const int H = cap >> 1;  // spill the bottom (shallowest) half
-    for (int i = lane; i < H; i += 32) g[gsp + i] = s[i];
-    __syncwarp();
-    for (int c = 0; c < sp - H; c += 32) {
-      uint32_t v = (c + lane < sp - H) ? s[H + c + lane] : 0u;
-      __syncwarp();
-      if (c + lane < sp - H) s[c + lane] = v;
-      __syncwarp();
-    }
-    gsp += H; sp -= H;
-  }
-  __device__ __forceinline__ void refill(int lane) {  // sp == 0, gsp > 0
-    const int H = cap >> 1;
-    int k = gsp < H ? gsp : H;
-    for (int i = lane; i < k; i += 32) s[i] = g[gsp - k + i];
-    __syncwarp();
-    gsp -= k; sp = k;
-  }
-};
-
-// inclusive warp scan of small ints
 __device__ __forceinline__ int warp_inclusive_scan(int x, int lane) {
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xFFFFFFFFu, x, o); if (lane >= o) x += y; }
   return x;
 }
+
+// ---- global task pool (multi-producer multi-consumer ring of fixed-size tasks)
+#define OTOO_TASK_CELLS 256
+#define OTOO_POOL_SLOTS 16384
+#define OTOO_POOL_MARGIN 4096        // > number of resident warps: concurrent producers cannot overrun
+struct TaskSlot { uint32_t group, count, pad[2]; uint32_t cells[OTOO_TASK_CELLS]; };
+struct WalkShared {                   // device-global control block, reset before every launch
+  uint32_t queue;  uint32_t pad0[31]; // next group of the main queue
+  uint32_t head;   uint32_t pad1[31]; // consumer tickets: idle warps take one and wait on their slot
+  uint32_t tail;   uint32_t pad2[31]; // producer tickets
+  int outstanding; uint32_t pad3[31]; // groups + tasks not yet finished
+};
+struct WalkCommon {
+  const float4* spos; const float4* cell_cm; const cellb_t* cell_b; const uint32_t* perm;
+  int64_t N, ngroups;
+  uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;   // zeroed before the launch
+  unsigned long long* sums;                                    // tests, interactions, cells, parts
+  WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
+  uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
+  int stack_cap;
+};
+
+__device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
+
+// Visitor contract (all members __forceinline__):
+//   static constexpr int T;            targets per lane
+//   static constexpr int E;            float4 per list entry
+//   void load_group(int64_t g0, int lane)          targets into registers, AABB, zero accumulators
+//   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
+//   void put_particle(float4* dst, uint32_t slot)  write one particle entry (E float4)
+//   void eval(const float4* list, int n)           all targets x n entries
+//   void pad(float4* dst)                          a null entry
+//   void mark_self(uint32_t first, uint32_t count, int64_t g0, int lane)
+//   void store(int64_t g0, int lane)               atomicAdd results to the outputs
+template <class V>
+__device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list, uint32_t* stk, int lane, int64_t gwarp) {
+  constexpr int G = 32 * V::T;
+  constexpr int CAP = (OTOO_LIST_CAP / V::E) & ~3;   // list entries (multiple of the padding unit)
+  constexpr int PADTO = 4;
+  uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;
+  unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;
+  bool main_done = false, have_ticket = false;
+  uint32_t my_ticket = 0;
+
+  for (;;) {
+    // ---------------- acquire a unit of work: a group from the main queue, else a pool task
+    uint32_t g = 0; int sp = 0;
+    bool got = false;
+    if (!main_done) {
+      if (lane == 0) g = atomicAdd(&c.ws->queue, 1u);
+      g = __shfl_sync(0xFFFFFFFFu, g, 0);
+      if ((int64_t)g < c.ngroups) { got = true; if (lane == 0) stk[0] = 0u; sp = 1; }
+      else main_done = true;
+    }
+    if (!got) {
+      // idle: take a consumer ticket once, then wait on that slot (no contended atomics while waiting)
+      if (!have_ticket) {
+        if (lane == 0) my_ticket = atomicAdd(&c.ws->head, 1u);
+        my_ticket = __shfl_sync(0xFFFFFFFFu, my_ticket, 0);
+        have_ticket = true;
+      }
+      const uint32_t slot = my_ticket % OTOO_POOL_SLOTS;
+      int ok = 0;
+      if (lane == 0) {
+        if (ld_volatile(&c.seq[slot]) == my_ticket + 1u) ok = 1;
+        else if (*reinterpret_cast<volatile int*>(&c.ws->outstanding) <= 0) ok = -1;
+      }
+      ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
+      if (ok < 0) break;
+      if (ok == 0) { __nanosleep(400); continue; }
+      __threadfence();
+      const TaskSlot* ts = c.slots + slot;
+      g = __ldcg(&ts->group); sp = (int)__ldcg(&ts->count);
+      for (int i = lane; i < sp; i += 32) stk[i] = __ldcg(&ts->cells[i]);
+      __syncwarp();
+      if (lane == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(&c.seq[slot]) = my_ticket + OTOO_POOL_SLOTS; }
+      have_ticket = false;
+      got = true;
+    }
+    __syncwarp();
+
+    const int64_t g0 = (int64_t)g * G;
+    const int gcount = (int)((c.N - g0) < G ? (c.N - g0) : G);
+    v.load_group(g0, lane);
+    int gsp = 0, nlist = 0;
+    uint32_t ntests = 0, ncells = 0, nparts = 0;
+
+    auto flush = [&]() {
+      const int np = (nlist + PADTO - 1) & ~(PADTO - 1);
+      if (lane < np - nlist) v.pad(list + V::E * (nlist + lane));
+      __syncwarp();
+      v.eval(list, np);
+      __syncwarp();
+      nlist = 0;
+    };
+    // hand the `d` shallowest stack entries to the pool (returns false if the pool is full)
+    auto donate = [&](int d) -> bool {
+      uint32_t ticket = 0; int ok = 0;
+      if (lane == 0) {
+        uint32_t h = ld_volatile(&c.ws->head), t = ld_volatile(&c.ws->tail);
+        if ((int)(t - h) < OTOO_POOL_SLOTS - OTOO_POOL_MARGIN) {
+          ok = 1;
+          atomicAdd(&c.ws->outstanding, 1);
+          ticket = atomicAdd(&c.ws->tail, 1u);
+          while (ld_volatile(&c.seq[ticket % OTOO_POOL_SLOTS]) != ticket) __nanosleep(64);
+        }
+      }
+      ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
+      if (!ok) return false;
+      ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
+      TaskSlot* ts = c.slots + (ticket % OTOO_POOL_SLOTS);
+      for (int i = lane; i < d; i += 32) __stcg(&ts->cells[i], stk[i]);
+      if (lane == 0) { __stcg(&ts->group, g); __stcg(&ts->count, (uint32_t)d); }
+      __threadfence();
+      __syncwarp();
+      if (lane == 0) *reinterpret_cast<volatile uint32_t*>(&c.seq[ticket % OTOO_POOL_SLOTS]) = ticket + 1u;
+      return true;
+    };
+    // drop the d bottom entries of the shared stack (after they were donated or spilled)
+    auto shift_down = [&](int d) {
+      for (int k = 0; k < sp - d; k += 32) {
+        uint32_t x = (k + lane < sp - d) ? stk[d + k + lane] : 0u;
+        __syncwarp();
+        if (k + lane < sp - d) stk[k + lane] = x;
+        __syncwarp();
+      }
+      sp -= d;
+    };
+
+    while (sp > 0 || gsp > 0) {
+      if (sp == 0) {  // refill from the private spill
+        const int k = gsp < OTOO_TASK_CELLS ? gsp : OTOO_TASK_CELLS;
+        for (int i = lane; i < k; i += 32) stk[i] = gspill[gsp - k + i];
+        __syncwarp();
+        gsp -= k; sp = k;
+      }
+      const int k = sp < 32 ? sp : 32;
+      const bool have = lane < k;
+      uint32_t cell = 0;
+      if (have) cell = stk[sp - k + lane];
+      // waiting consumers = head - tail (when positive); loads issued early, used below
+      const int idle_now = sp >= 64 ? (int)(ld_volatile(&c.ws->head) - ld_volatile(&c.ws->tail)) : 0;
+      __syncwarp();
+      sp -= k;
+      float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
+      cellb_t B = make_uint4(0u, 0u, 0u, 0u);
+      int cls = 0;
+      if (have) cls = v.classify(cell, A, B);
+      ntests += (uint32_t)k;
+      const bool leaf = (B.w & 1u) != 0u;
+      const bool accept = cls == 1, open_leaf = cls == 2 && leaf, open_int = cls == 2 && !leaf;
+
+      // accepted cells -> list (the cell is a virtual particle at its centre of mass, L43)
+      const unsigned am = __ballot_sync(0xFFFFFFFFu, accept);
+      const int na = __popc(am);
+      if (na) {
+        if (nlist + na > CAP) flush();
+        if (accept) list[V::E * (nlist + __popc(am & lanemask_lt_()))] = A;
+        nlist += na; ncells += (uint32_t)na;
+      }
+      // opened internal cells -> push children (L57 rule 1: follow `more`)
+      {
+        const int nch = open_int ? (int)B.z : 0;
+        const int inc = warp_inclusive_scan(nch, lane);
+        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        if (total) {
+          if (sp + total > c.stack_cap) {       // overflow: donate, else spill privately
+            const int d = OTOO_TASK_CELLS;      // stack_cap >= 512, total <= 256
+            if (!donate(d)) {
+              for (int i = lane; i < d; i += 32) gspill[gsp + i] = stk[i];
+              gsp += d;
+            }
+            __syncwarp();
+            shift_down(d);
+          }
+          const int o = sp + inc - nch;
+          for (int i = 0; i < nch; i++) stk[o + i] = B.y + (uint32_t)i;
+          __syncwarp();
+          sp += total;
+        }
+      }
+      // load balance: feed idle warps with the shallowest entries
+      if (sp >= 64 && idle_now > 0) {
+        int d = sp >> 1; if (d > OTOO_TASK_CELLS) d = OTOO_TASK_CELLS;
+        if (donate(d)) shift_down(d);
+      }
+      // opened leaves -> their particles (L57 rule 3)
+      const unsigned lm = __ballot_sync(0xFFFFFFFFu, open_leaf);
+      if (lm) {
+        const int cnt = open_leaf ? (int)B.z : 0;
+        const int inc = warp_inclusive_scan(cnt, lane);
+        const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        unsigned m = lm;
+        while (m) {  // which targets sit in an opened leaf: their self term is in the list
+          const int src = __ffs(m) - 1; m &= m - 1;
+          v.mark_self(__shfl_sync(0xFFFFFFFFu, B.y, src), __shfl_sync(0xFFFFFFFFu, B.z, src), g0, lane);
+        }
+        if (total <= CAP) {
+          if (nlist + total > CAP) flush();
+          const int o = nlist + inc - cnt;
+          for (int i = 0; i < cnt; i++) v.put_particle(list + V::E * (o + i), B.y + (uint32_t)i);
+          nlist += total;
+        } else {  // huge leaves (coincident points at level 21): one leaf at a time, 32 particles a chunk
+          m = lm;
+          while (m) {
+            const int src = __ffs(m) - 1; m &= m - 1;
+            const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), n = __shfl_sync(0xFFFFFFFFu, B.z, src);
+            for (uint32_t i = 0; i < n; i += 32) {
+              if (nlist + 32 > CAP) flush();
+              if (i + lane < n) v.put_particle(list + V::E * (nlist + lane), f + i + lane);
+              nlist += (int)((n - i) < 32u ? (n - i) : 32u);
+            }
+          }
+        }
+        nparts += (uint32_t)total;
+        __syncwarp();
+      }
+    }
+    if (nlist) flush();
+    v.store(g0, lane);
+    if (lane == 0) {
+      atomicAdd(c.g_ntests + g, ntests); atomicAdd(c.g_ncells + g, ncells); atomicAdd(c.g_nparts + g, nparts);
+      __threadfence();
+      atomicSub(&c.ws->outstanding, 1);
+    }
+    tot_tests += ntests; tot_cells += ncells; tot_parts += nparts;
+    tot_inter += (unsigned long long)gcount * (ncells + nparts);
+  }
+  if (lane == 0 && tot_tests) {
+    atomicAdd(c.sums + 0, tot_tests); atomicAdd(c.sums + 1, tot_inter);
+    atomicAdd(c.sums + 2, tot_cells); atomicAdd(c.sums + 3, tot_parts);
+  }
+}
+
+// host side (gravity.cu)
+otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st);

@@ -26,12 +26,22 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def acc_err(got, want):
-    """R12: per-particle relative error with the 1e-2 a_rms floor; also the un-floored maximum."""
+U32 = 2.0 ** -24          # fp32 unit roundoff
+
+
+def acc_err(got, want, abs_sum=None):
+    """R12.  Per particle |da| / tol with tol = max(1e-5 |a|, 8 u A), A = sum_j |a_ij| over the same
+    lists (from the oracle): 1e-5 relative (north_star) wherever the sum is well conditioned, and
+    the fp32 arithmetic bound 8 u A where the pair forces cancel (|a| << A).  Without abs_sum the
+    floor is 1e-2 a_rms.  Returns (err / tolerance scaled to 1e-5, plain relative error)."""
     d = np.linalg.norm(got[:, :3].astype(np.float64) - want[:, :3], axis=1)
     an = np.linalg.norm(want[:, :3], axis=1)
-    arms = np.sqrt((an ** 2).mean())
-    return d / np.maximum(an, 1e-2 * arms), d / np.maximum(an, 1e-300)
+    if abs_sum is None:
+        floor = 1e-2 * np.sqrt((an ** 2).mean()) * 1e-5
+    else:
+        floor = 8 * U32 * abs_sum
+    tol = np.maximum(1e-5 * an, floor)
+    return 1e-5 * d / np.maximum(tol, 1e-300), d / np.maximum(an, 1e-300)
 
 
 def check_tree(otoo, orc, pm, n_crit):
@@ -86,8 +96,9 @@ def test_gravity_parity(otoo, orc, kind, n, G, theta, eps):
     assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
     st = otoo.otoo_last_stats()
     assert st["sum_interactions"] == ref["interactions"] and st["sum_tests"] == int(ref["n_tests"].sum())
-    e, raw = acc_err(out, ref["acc_pot"])
+    e, raw = acc_err(out, ref["acc_pot"], ref["abs_sum"])
     assert e.max() <= TOL, (e.max(), np.median(e), raw.max())
+    assert np.percentile(raw, 99.9) <= TOL          # plain 1e-5 relative error for 99.9 % of the particles
     pe = np.abs(out[:, 3] - ref["acc_pot"][:, 3]) / np.abs(ref["acc_pot"][:, 3])
     assert pe.max() <= TOL, pe.max()
 
@@ -104,7 +115,7 @@ def test_walk_stack_spill(otoo, orc):
             out = otoo.otoo_gravity(0.01, theta, 32).cpu().numpy()
             nt, nc, npart = otoo.otoo_export_group_stats()
             assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
-            e, _ = acc_err(out, ref["acc_pot"])
+            e, _ = acc_err(out, ref["acc_pot"], ref["abs_sum"])
             assert e.max() <= TOL
     finally:
         otoo.otoo_set_option("walk_stack", 1024)
@@ -113,7 +124,12 @@ def test_walk_stack_spill(otoo, orc):
 @pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
 def test_sph_parity(otoo, orc, n, G):
     w = gen.wd_pair(n, 1206)
-    pm, h, u, vel = w["pos_mass"], w["h"], w["u"], w["vel"]
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    # the generator's rigid rotation has (v_i - v_j).(x_i - x_j) = 0 for every pair (du/dt would be
+    # rounding noise): add a homologous contraction and a seeded perturbation for the du/dt check
+    vel = w["vel"].copy()
+    vel[:, :3] += -0.3 * pm[:, :3] + 0.05 * (gen.uniform01(99, np.arange(3 * n, dtype=np.uint64), 0).reshape(n, 3) - 0.5)
+    vel = vel.astype(np.float32)
     t = check_tree(otoo, orc, pm, 16)
     ref = t.sph_density(h, G)
     rho, nngb = otoo.otoo_sph_density(dev(h), G)
@@ -174,5 +190,5 @@ def test_host_entry_point(otoo, orc):
     pm = gen.plummer(10000, 5)
     out = otoo.otoo_gravity_host(pm, 16, 0.01, 0.5, 64)
     ref = orc.Tree(pm, 16).gravity(float(np.float32(0.01)), 0.5, 64)
-    e, _ = acc_err(out, ref["acc_pot"])
+    e, _ = acc_err(out, ref["acc_pot"], ref["abs_sum"])
     assert e.max() <= TOL
