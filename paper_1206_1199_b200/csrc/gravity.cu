@@ -29,18 +29,22 @@ constexpr float PAD_POS = 1.0e18f;  // zero-mass padding entries sit far away: c
 
 // Gravity visitor: R10 sums.  13 FP32 lane-ops + 1 MUFU per interaction, issued two targets at a
 // time as FFMA2/FADD2/FMUL2; two-level summation (64-entry fp32 partial sums, then totals).
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
+
 template <int T_, bool EPS0>
 struct GravVisitor {
   static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64;
   const GravParams& p;
   float pm[T];
   float glo[3], ghi[3];
-  f32x2 PX[NP], PY[NP], PZ[NP], AX[NP], AY[NP], AZ[NP], PH[NP];
-  f32x2 eps2p;
+  f32x2 PX[NP], PY[NP], PZ[NP];                       // two targets per aligned register pair (kept as b64)
+  float2 AX[NP], AY[NP], AZ[NP], PH[NP];
   unsigned selfmask;
-  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_) { eps2p = pk2(p_.eps2, p_.eps2); }
+  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_) {}
 
-  __device__ __forceinline__ void load_group(int64_t g0, int lane) {
+  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4* scratch) {
     float px[T], py[T], pz[T];
 #pragma unroll
     for (int t = 0; t < T; t++) {   // H7: lane holds slots g0 + t*32 + lane; out-of-range lanes mirror slot g0
@@ -64,8 +68,17 @@ struct GravVisitor {
 #pragma unroll
     for (int q = 0; q < NP; q++) {
       const int t1 = (2 * q + 1 < T) ? 2 * q + 1 : 2 * q;
-      PX[q] = pk2(px[2 * q], px[t1]); PY[q] = pk2(py[2 * q], py[t1]); PZ[q] = pk2(pz[2 * q], pz[t1]);
-      AX[q] = AY[q] = AZ[q] = PH[q] = pk2(0.0f, 0.0f);
+      // Round trip through (idle) list memory: the pairs are born as 64-bit values in aligned register
+      // pairs.  Without it ptxas keeps the LDG.128 quads and re-pairs x/y/z with 6 MOVs per target pair
+      // and list entry inside the hot loop (measured: 25 % of all issued instructions).
+      const unsigned sa = (unsigned)__cvta_generic_to_shared(scratch) + (unsigned)(lane * NP * 3 + q * 3) * 8u;
+      asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(sa), "f"(px[2 * q]), "f"(px[t1]) : "memory");
+      asm volatile("st.shared.v2.f32 [%0+8], {%1,%2};" ::"r"(sa), "f"(py[2 * q]), "f"(py[t1]) : "memory");
+      asm volatile("st.shared.v2.f32 [%0+16], {%1,%2};" ::"r"(sa), "f"(pz[2 * q]), "f"(pz[t1]) : "memory");
+      asm volatile("ld.shared.b64 %0, [%1];" : "=l"(PX[q]) : "r"(sa) : "memory");
+      asm volatile("ld.shared.b64 %0, [%1+8];" : "=l"(PY[q]) : "r"(sa) : "memory");
+      asm volatile("ld.shared.b64 %0, [%1+16];" : "=l"(PZ[q]) : "r"(sa) : "memory");
+      AX[q] = AY[q] = AZ[q] = PH[q] = make_float2(0.0f, 0.0f);
     }
     selfmask = 0;
   }
@@ -81,39 +94,40 @@ struct GravVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
+  // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
+  // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
+    const float2 e2 = bc2(p.eps2);
 #pragma unroll
     for (int pb = 0; pb < NP; pb += PB) {
       for (int j0 = 0; j0 < n; j0 += BLK) {
         const int je = j0 + BLK < n ? j0 + BLK : n;
-        f32x2 cx[PB], cy[PB], cz[PB], cp[PB];
+        float2 cx[PB], cy[PB], cz[PB], cp[PB];
 #pragma unroll
-        for (int q = 0; q < PB; q++) cx[q] = cy[q] = cz[q] = cp[q] = 0ull;
+        for (int q = 0; q < PB; q++) cx[q] = cy[q] = cz[q] = cp[q] = make_float2(0.0f, 0.0f);
 #pragma unroll 4
         for (int j = j0; j < je; j++) {
           const float4 s = list[j];
-          const f32x2 sx = pk2(s.x, s.x), sy = pk2(s.y, s.y), sz = pk2(s.z, s.z), sw = pk2(s.w, s.w);
 #pragma unroll
           for (int q = 0; q < PB; q++) {
-            f32x2 dx = sub2(sx, PX[pb + q]), dy = sub2(sy, PY[pb + q]), dz = sub2(sz, PZ[pb + q]);
-            f32x2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, eps2p)));
-            float r2a, r2b;
-            upk2(r2, r2a, r2b);
-            float ia = rsqrt_approx(r2a), ib = rsqrt_approx(r2b);
-            if (EPS0) { ia = r2a > 0.0f ? ia : 0.0f; ib = r2b > 0.0f ? ib : 0.0f; }  // r = 0 pairs contribute 0
-            f32x2 ri = pk2(ia, ib);
-            f32x2 mri = mul2(sw, ri);
-            f32x2 mr3 = mul2(mri, mul2(ri, ri));
-            cp[q] = sub2(cp[q], mri);
-            cx[q] = fma2(mr3, dx, cx[q]);
-            cy[q] = fma2(mr3, dy, cy[q]);
-            cz[q] = fma2(mr3, dz, cz[q]);
+            const float2 dx = __fadd2_rn(bc2(s.x), neg2(as2(PX[pb + q])));
+            const float2 dy = __fadd2_rn(bc2(s.y), neg2(as2(PY[pb + q])));
+            const float2 dz = __fadd2_rn(bc2(s.z), neg2(as2(PZ[pb + q])));
+            const float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __ffma2_rn(dz, dz, e2)));
+            float2 ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
+            if (EPS0) { ri.x = r2.x > 0.0f ? ri.x : 0.0f; ri.y = r2.y > 0.0f ? ri.y : 0.0f; }  // r = 0 pairs contribute 0
+            const float2 mri = __fmul2_rn(bc2(s.w), ri);
+            const float2 mr3 = __fmul2_rn(mri, __fmul2_rn(ri, ri));
+            cp[q] = __fadd2_rn(cp[q], neg2(mri));
+            cx[q] = __ffma2_rn(mr3, dx, cx[q]);
+            cy[q] = __ffma2_rn(mr3, dy, cy[q]);
+            cz[q] = __ffma2_rn(mr3, dz, cz[q]);
           }
         }
 #pragma unroll
         for (int q = 0; q < PB; q++) {
-          AX[pb + q] = add2(AX[pb + q], cx[q]); AY[pb + q] = add2(AY[pb + q], cy[q]);
-          AZ[pb + q] = add2(AZ[pb + q], cz[q]); PH[pb + q] = add2(PH[pb + q], cp[q]);
+          AX[pb + q] = __fadd2_rn(AX[pb + q], cx[q]); AY[pb + q] = __fadd2_rn(AY[pb + q], cy[q]);
+          AZ[pb + q] = __fadd2_rn(AZ[pb + q], cz[q]); PH[pb + q] = __fadd2_rn(PH[pb + q], cp[q]);
         }
       }
     }
@@ -124,9 +138,8 @@ struct GravVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) {
       const int64_t s = g0 + t * 32 + lane;
-      float ax0, ax1, ay0, ay1, az0, az1, ph0, ph1;
-      upk2(AX[t >> 1], ax0, ax1); upk2(AY[t >> 1], ay0, ay1); upk2(AZ[t >> 1], az0, az1); upk2(PH[t >> 1], ph0, ph1);
-      float4 o = (t & 1) ? make_float4(ax1, ay1, az1, ph1) : make_float4(ax0, ay0, az0, ph0);
+      const int q = t >> 1;
+      float4 o = (t & 1) ? make_float4(AX[q].y, AY[q].y, AZ[q].y, PH[q].y) : make_float4(AX[q].x, AY[q].x, AZ[q].x, PH[q].x);
       if ((selfmask >> t) & 1u) o.w = __fmaf_rn(pm[t], rie, o.w);
       if (s < p.c.N) {
         float* dst = reinterpret_cast<float*>(p.acc_pot + p.c.perm[s]);

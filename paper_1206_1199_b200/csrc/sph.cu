@@ -102,7 +102,7 @@ struct SphVisitor {
   float glo[3], ghi[3], hmax;
   __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_) {}
 
-  __device__ __forceinline__ void load_group(int64_t g0, int lane) {
+  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4*) {
     hmax = 0.0f;
 #pragma unroll
     for (int t = 0; t < T; t++) {

@@ -72,7 +72,7 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 // Visitor contract (all members __forceinline__):
 //   static constexpr int T;            targets per lane
 //   static constexpr int E;            float4 per list entry
-//   void load_group(int64_t g0, int lane)          targets into registers, AABB, zero accumulators
+//   void load_group(int64_t g0, int lane, float4* scratch)   targets into registers, AABB, zero accumulators
 //   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
 //   void put_particle(float4* dst, uint32_t slot)  write one particle entry (E float4)
 //   void eval(const float4* list, int n)           all targets x n entries
@@ -128,7 +128,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
 
     const int64_t g0 = (int64_t)g * G;
     const int gcount = (int)((c.N - g0) < G ? (c.N - g0) : G);
-    v.load_group(g0, lane);
+    v.load_group(g0, lane, list);   // the list is empty here: usable as scratch
     int gsp = 0, nlist = 0;
     uint32_t ntests = 0, ncells = 0, nparts = 0;
 
