@@ -115,9 +115,10 @@ otoo_status otoo_export_group_stats(otoo_ctx* ctx, uint32_t* d_ntests, uint32_t*
                                     uint32_t* d_nparts);
 otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
 
-/* Tuning/debug knobs.  "walk_stack" = shared-memory walk stack entries per warp before the
- * global-memory spill is used (test hook; 64..OTOO_WALK_STACK_MAX). Unknown names:
- * OTOO_ERR_INVALID_ARG. */
+/* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
+ * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
+ * 0: it only spills to its private global area (test hook for that path).
+ * Unknown names: OTOO_ERR_INVALID_ARG. */
 otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value);
 
 /* End-to-end form with HOST buffers (pageable or pinned): copies h_pos_mass to the device,

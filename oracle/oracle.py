@@ -64,7 +64,7 @@ def lib():
         L.orc_sph_density.argtypes = [vp, vp, i32, vp, vp, vp, vp]
         L.orc_sph_group_list.argtypes = [vp, vp, i32, i64, vp]
         L.orc_sph_force.restype = C.c_uint64
-        L.orc_sph_force.argtypes = [vp, vp, vp, vp, vp, i32, vp]
+        L.orc_sph_force.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
         L.orc_W.restype = dbl
         L.orc_W.argtypes = [dbl, dbl]
         L.orc_dWdr.restype = dbl
@@ -208,5 +208,6 @@ class Tree:
         P = np.ascontiguousarray(P, dtype=np.float64)
         v = None if vel is None else _f32(vel, (self.N, 4))
         out = np.zeros((self.N, 4), dtype=np.float64)
-        tot = lib().orc_sph_force(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(out))
-        return dict(acc_dudt=out, candidates=int(tot))
+        asum = np.zeros((self.N, 2), dtype=np.float64)
+        tot = lib().orc_sph_force(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(out), _p(asum))
+        return dict(acc_dudt=out, candidates=int(tot), abs_sum=asum)

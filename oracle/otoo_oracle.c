@@ -538,7 +538,7 @@ void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uin
 
 /* R17: symmetric pressure force (TREESPH/GADGET form) and optional du/dt. */
 uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, const double* P,
-                       const float* vel, int G, double* out) {
+                       const float* vel, int G, double* out, double* abs_sum) {
   int64_t N = t->N, ng = (N + G - 1) / G;
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
@@ -559,7 +559,7 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
         int64_t io = t->perm[s];
         float hi = hs[s];
         double pri = P[io] / (rho[io] * rho[io]);
-        double ax = 0, ay = 0, az = 0, du = 0;
+        double ax = 0, ay = 0, az = 0, du = 0, asum = 0, dsum = 0;
         for (int64_t k = 0; k < L.np; k++) {
           int64_t j = L.parts[k];
           if (j == s) continue;
@@ -573,13 +573,16 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
           double gw = 0.5 * (orc_dWdr(r, (double)hi) + orc_dWdr(r, (double)hj)) / r;  /* grad_i W = gw * (xi-xj) */
           double f = (double)pj[3] * (pri + P[jo] / (rho[jo] * rho[jo])) * gw;
           ax -= f * dx; ay -= f * dy; az -= f * dz;
+          asum += fabs(f) * r;                       /* |a_ij|, for the test's error bound */
           if (vel) {
             double vx = (double)vel[4 * io] - vel[4 * jo], vy = (double)vel[4 * io + 1] - vel[4 * jo + 1],
                    vz = (double)vel[4 * io + 2] - vel[4 * jo + 2];
             du += 0.5 * f * (vx * dx + vy * dy + vz * dz);
+            dsum += fabs(0.5 * f * (vx * dx + vy * dy + vz * dz));
           }
         }
         out[4 * io] = ax; out[4 * io + 1] = ay; out[4 * io + 2] = az; out[4 * io + 3] = du;
+        if (abs_sum) { abs_sum[2 * io] = asum; abs_sum[2 * io + 1] = dsum; }
       }
     }
     free(L.parts); free(L.cells);

@@ -78,7 +78,8 @@ uint64_t orc_sph_density(const orc_tree*, const float* h, int group_size, double
 void orc_sph_group_list(const orc_tree*, const float* h, int group_size, int64_t g,
                         uint32_t* part_slots);
 uint64_t orc_sph_force(const orc_tree*, const float* h, const double* rho, const double* P,
-                       const float* vel /*4N or NULL*/, int group_size, double* acc_dudt /*4N*/);
+                       const float* vel /*4N or NULL*/, int group_size, double* acc_dudt /*4N*/,
+                       double* abs_sum /*2N or NULL: sum_j |a_ij|, sum_j |du_ij|*/);
 /* cubic spline with support h (R13) */
 double orc_W(double r, double h);
 double orc_dWdr(double r, double h);

@@ -8,9 +8,9 @@
 
 #define OTOO_MAXLEV 21
 #define OTOO_NLEV 22                 // levels 0..21
-#define OTOO_WALK_STACK_MAX 1024     // smem walk-stack entries per warp
+#define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
-#define OTOO_LIST_CAP 512            // smem interaction-list entries per warp (float4 each)
+#define OTOO_LIST_CAP 256            // smem interaction-list float4 per warp (small: leaves the SM's L1 for the tree)
 #define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
 
 // Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).
@@ -82,6 +82,7 @@ struct otoo_ctx {
   float lo[3], S;
   uint32_t level_off[OTOO_NLEV + 1];
   int walk_stack;        // option "walk_stack"
+  int use_pool;          // option "task_pool"
   int last_group_size;
   int64_t last_ngroups;
   int launches;          // kernels launched by the current/last API call

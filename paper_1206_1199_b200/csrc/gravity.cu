@@ -88,7 +88,9 @@ struct GravVisitor {
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
     return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
   }
-  __device__ __forceinline__ void put_particle(float4* dst, uint32_t slot) { *dst = p.c.spos[slot]; }
+  struct Entry { float4 a; };
+  __device__ __forceinline__ Entry get(uint32_t slot) const { Entry e; e.a = p.c.spos[slot]; return e; }
+  __device__ __forceinline__ void put(float4* dst, const Entry& e) const { *dst = e.a; }
   __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
   __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
 #pragma unroll
@@ -195,6 +197,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   *smem = otoo_walk_smem_bytes();
   int per_sm = (int)((227 * 1024) / (*smem + 1024));
   if (per_sm < 1) per_sm = 1;
+  if (per_sm > 6) per_sm = 6;   // 24 warps per SM at most (registers allow 4-6 CTAs)
   const int64_t warps = (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS;
   if (warps >= OTOO_POOL_MARGIN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "internal: task pool margin below resident warps");
   *grid = ctx->sm_count * per_sm;
@@ -215,6 +218,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
+  c->use_pool = ctx->use_pool;
   ctx->launches += 1;
   ctx->last_group_size = G; ctx->last_ngroups = ngroups;
   return OTOO_OK;

@@ -145,10 +145,17 @@ struct SphVisitor {
     float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));
     return d2 <= __fmul_rn(R, R) ? 2 : 0;
   }
-  __device__ __forceinline__ void put_particle(float4* dst, uint32_t s) {
-    dst[0] = p.c.spos[s];
-    if (E >= 2) dst[1] = p.aux[s];
-    if (E >= 3) dst[2] = p.svel[s];
+  struct Entry { float4 v[E]; };
+  __device__ __forceinline__ Entry get(uint32_t s) const {
+    Entry e;
+    e.v[0] = p.c.spos[s];
+    if (E >= 2) e.v[1] = p.aux[s];
+    if (E >= 3) e.v[2] = p.svel[s];
+    return e;
+  }
+  __device__ __forceinline__ void put(float4* dst, const Entry& e) const {
+#pragma unroll
+    for (int k = 0; k < E; k++) dst[k] = e.v[k];
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass

@@ -65,6 +65,7 @@ struct WalkCommon {
   WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
   uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
   int stack_cap;
+  int use_pool;                                                 // 0: never donate (test hook: private spill only)
 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
@@ -74,7 +75,7 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 //   static constexpr int E;            float4 per list entry
 //   void load_group(int64_t g0, int lane, float4* scratch)   targets into registers, AABB, zero accumulators
 //   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
-//   void put_particle(float4* dst, uint32_t slot)  write one particle entry (E float4)
+//   struct Entry; Entry get(uint32_t slot); void put(float4* dst, const Entry&)   one particle entry (E float4)
 //   void eval(const float4* list, int n)           all targets x n entries
 //   void pad(float4* dst)                          a null entry
 //   void mark_self(uint32_t first, uint32_t count, int64_t g0, int lane)
@@ -143,6 +144,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     // hand the `d` shallowest stack entries to the pool (returns false if the pool is full)
     auto donate = [&](int d) -> bool {
       uint32_t ticket = 0; int ok = 0;
+      if (!c.use_pool) return false;
       if (lane == 0) {
         uint32_t h = ld_volatile(&c.ws->head), t = ld_volatile(&c.ws->tail);
         if ((int)(t - h) < OTOO_POOL_SLOTS - OTOO_POOL_MARGIN) {
@@ -186,7 +188,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       uint32_t cell = 0;
       if (have) cell = stk[sp - k + lane];
       // waiting consumers = head - tail (when positive); loads issued early, used below
-      const int idle_now = sp >= 64 ? (int)(ld_volatile(&c.ws->head) - ld_volatile(&c.ws->tail)) : 0;
+      const int idle_now = sp >= 16 ? (int)(ld_volatile(&c.ws->head) - ld_volatile(&c.ws->tail)) : 0;
       __syncwarp();
       sp -= k;
       float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -227,7 +229,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
         }
       }
       // load balance: feed idle warps with the shallowest entries
-      if (sp >= 64 && idle_now > 0) {
+      if (sp >= 16 && idle_now > 0) {
         int d = sp >> 1; if (d > OTOO_TASK_CELLS) d = OTOO_TASK_CELLS;
         if (donate(d)) shift_down(d);
       }
@@ -242,21 +244,36 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
           const int src = __ffs(m) - 1; m &= m - 1;
           v.mark_self(__shfl_sync(0xFFFFFFFFu, B.y, src), __shfl_sync(0xFFFFFFFFu, B.z, src), g0, lane);
         }
-        if (total <= CAP) {
-          if (nlist + total > CAP) flush();
-          const int o = nlist + inc - cnt;
-          for (int i = 0; i < cnt; i++) v.put_particle(list + V::E * (o + i), B.y + (uint32_t)i);
-          nlist += total;
-        } else {  // huge leaves (coincident points at level 21): one leaf at a time, 32 particles a chunk
-          m = lm;
-          while (m) {
-            const int src = __ffs(m) - 1; m &= m - 1;
-            const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, src), n = __shfl_sync(0xFFFFFFFFu, B.z, src);
-            for (uint32_t i = 0; i < n; i += 32) {
-              if (nlist + 32 > CAP) flush();
-              if (i + lane < n) v.put_particle(list + V::E * (nlist + lane), f + i + lane);
-              nlist += (int)((n - i) < 32u ? (n - i) : 32u);
-            }
+        // cooperative expansion: output position j -> (leaf, offset) by a shuffle binary search over the
+        // inclusive counts; every lane loads one particle per chunk, loads of two chunks are in flight.
+        const int startv = inc - cnt;
+        auto locate = [&](int j) -> uint32_t {
+          int L = 0;
+#pragma unroll
+          for (int st = 16; st; st >>= 1) { const int x = __shfl_sync(0xFFFFFFFFu, inc, L + st - 1); if (x <= j) L += st; }
+          const uint32_t f = __shfl_sync(0xFFFFFFFFu, B.y, L);
+          const int s0 = __shfl_sync(0xFFFFFFFFu, startv, L);
+          return f + (uint32_t)(j - s0);
+        };
+        for (int j0 = 0; j0 < total;) {
+          if (nlist + 32 > CAP) flush();
+          const int room = (CAP - nlist) >> 5, need = (total - j0 + 31) >> 5;
+          int nb = room < need ? room : need;
+          for (; nb >= 2; nb -= 2, j0 += 64) {
+            const int ja = j0 + lane, jb = j0 + 32 + lane;
+            const uint32_t sa = locate(ja < total ? ja : total - 1), sb = locate(jb < total ? jb : total - 1);
+            typename V::Entry ea = v.get(sa), eb = v.get(sb);
+            if (ja < total) v.put(list + V::E * (nlist + lane), ea);
+            if (jb < total) v.put(list + V::E * (nlist + 32 + lane), eb);
+            nlist += (total - j0) < 64 ? (total - j0) : 64;
+          }
+          if (nb == 1) {
+            const int ja = j0 + lane;
+            const uint32_t sa = locate(ja < total ? ja : total - 1);
+            typename V::Entry ea = v.get(sa);
+            if (ja < total) v.put(list + V::E * (nlist + lane), ea);
+            nlist += (total - j0) < 32 ? (total - j0) : 32;
+            j0 += 32;
           }
         }
         nparts += (uint32_t)total;
