@@ -58,6 +58,9 @@ typedef struct {
   int64_t n_groups;
   int32_t group_size;
   int32_t launches;          /* kernels launched by the last call */
+  uint64_t sum_steps;        /* walk steps (batches of <= 32 MAC tests) of the last walk */
+  uint64_t sum_tasks;        /* units of work run: groups + task-pool tasks */
+  uint64_t sum_flushes;      /* evaluations of a (full or final) shared-memory list */
 } otoo_stats_t;
 
 /* Lifecycle.  `device` is a CUDA ordinal; max_particles bounds N of every later build
@@ -118,6 +121,8 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).
+ * "walk_only" = 1: the walks build and count their lists but skip the pair sums (outputs are
+ * meaningless; counters exact) -- measures the walk's share of the fused kernel; default 0.
  * Unknown names: OTOO_ERR_INVALID_ARG. */
 otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value);
 

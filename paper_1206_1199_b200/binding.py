@@ -37,7 +37,8 @@ class TreeInfo(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("sum_tests", C.c_uint64), ("sum_interactions", C.c_uint64), ("sum_cells", C.c_uint64),
                 ("sum_parts", C.c_uint64), ("n_groups", C.c_int64), ("group_size", C.c_int32),
-                ("launches", C.c_int32)]
+                ("launches", C.c_int32), ("sum_steps", C.c_uint64), ("sum_tasks", C.c_uint64),
+                ("sum_flushes", C.c_uint64)]
 
 
 CELL_DTYPE = np.dtype([("prefix", "<u8"), ("first", "<u4"), ("count", "<u4"), ("child_first", "<u4"),

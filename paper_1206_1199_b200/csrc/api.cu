@@ -95,8 +95,8 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));
     OTOO_TRY(dalloc(ctx, &ctx->d_bbox, 16));
     OTOO_TRY(dalloc(ctx, &ctx->d_counters, 64));
-    OTOO_TRY(dalloc(ctx, &ctx->d_sums, 4));
-    OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, 4 * sizeof(unsigned long long)));
+    OTOO_TRY(dalloc(ctx, &ctx->d_sums, 8));
+    OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, 8 * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
     return OTOO_OK;
@@ -250,9 +250,10 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
   OTOO_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
   if (ctx->walked) {
-    unsigned long long h[4];
+    unsigned long long h[8];
     OTOO_CUDA(ctx, cudaMemcpy(h, ctx->d_sums, sizeof h, cudaMemcpyDeviceToHost));
     o->sum_tests = h[0]; o->sum_interactions = h[1]; o->sum_cells = h[2]; o->sum_parts = h[3];
+    o->sum_steps = h[4]; o->sum_tasks = h[5]; o->sum_flushes = h[6];
     o->n_groups = ctx->last_ngroups; o->group_size = ctx->last_group_size;
   }
   o->launches = ctx->launches;
@@ -267,6 +268,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     return OTOO_OK;
   }
   if (strcmp(name, "task_pool") == 0) { ctx->use_pool = value != 0; return OTOO_OK; }
+  if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");
 }
 

@@ -83,6 +83,7 @@ struct otoo_ctx {
   uint32_t level_off[OTOO_NLEV + 1];
   int walk_stack;        // option "walk_stack"
   int use_pool;          // option "task_pool"
+  int walk_only;         // option "walk_only" (diagnostic)
   int last_group_size;
   int64_t last_ngroups;
   int launches;          // kernels launched by the current/last API call

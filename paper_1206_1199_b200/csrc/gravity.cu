@@ -212,13 +212,14 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)ngroups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)ngroups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)ngroups, st));
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 4 * sizeof(unsigned long long), st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 8 * sizeof(unsigned long long), st));
   c->spos = ctx->spos; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
   c->N = ctx->N; c->ngroups = ngroups;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
   c->use_pool = ctx->use_pool;
+  c->walk_only = ctx->walk_only;
   ctx->launches += 1;
   ctx->last_group_size = G; ctx->last_ngroups = ngroups;
   return OTOO_OK;

@@ -66,6 +66,7 @@ struct WalkCommon {
   uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
   int stack_cap;
   int use_pool;                                                 // 0: never donate (test hook: private spill only)
+  int walk_only;                                                // 1: lists are built and counted but not evaluated (measures the walk)
 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
@@ -87,6 +88,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   constexpr int PADTO = 4;
   uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;
   unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;
+  unsigned long long tot_steps = 0, tot_tasks = 0, tot_flushes = 0;
   bool main_done = false, have_ticket = false;
   uint32_t my_ticket = 0;
 
@@ -131,15 +133,15 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     const int gcount = (int)((c.N - g0) < G ? (c.N - g0) : G);
     v.load_group(g0, lane, list);   // the list is empty here: usable as scratch
     int gsp = 0, nlist = 0;
-    uint32_t ntests = 0, ncells = 0, nparts = 0;
+    uint32_t ntests = 0, ncells = 0, nparts = 0, iter = 0, nflush = 0;
 
     auto flush = [&]() {
       const int np = (nlist + PADTO - 1) & ~(PADTO - 1);
       if (lane < np - nlist) v.pad(list + V::E * (nlist + lane));
       __syncwarp();
-      v.eval(list, np);
+      if (!c.walk_only) v.eval(list, np);
       __syncwarp();
-      nlist = 0;
+      nlist = 0; nflush++;
     };
     // hand the `d` shallowest stack entries to the pool (returns false if the pool is full)
     auto donate = [&](int d) -> bool {
@@ -189,6 +191,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       if (have) cell = stk[sp - k + lane];
       // waiting consumers = head - tail (when positive); loads issued early, used below
       const int idle_now = sp >= 16 ? (int)(ld_volatile(&c.ws->head) - ld_volatile(&c.ws->tail)) : 0;
+      iter++;
       __syncwarp();
       sp -= k;
       float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -288,11 +291,13 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       atomicSub(&c.ws->outstanding, 1);
     }
     tot_tests += ntests; tot_cells += ncells; tot_parts += nparts;
+    tot_steps += iter; tot_tasks += 1; tot_flushes += nflush;
     tot_inter += (unsigned long long)gcount * (ncells + nparts);
   }
   if (lane == 0 && tot_tests) {
     atomicAdd(c.sums + 0, tot_tests); atomicAdd(c.sums + 1, tot_inter);
     atomicAdd(c.sums + 2, tot_cells); atomicAdd(c.sums + 3, tot_parts);
+    atomicAdd(c.sums + 4, tot_steps); atomicAdd(c.sums + 5, tot_tasks); atomicAdd(c.sums + 6, tot_flushes);
   }
 }
 
