@@ -216,7 +216,7 @@ def main():
     peak_tflops = sm_count * SM_LANES * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
     grav_ms = float(t_grav.mean())
     achieved = FLOPS_PER_INTERACTION * inter / (grav_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "walk_gravity_kernel", "achieved": achieved, "peak": peak_tflops,
+    roofline = {"bound": "alu", "kernel": "walk_gravity_ws_kernel", "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
                 # profiles/r1_walk_gravity_full.md (C2, theta=0.6 only); the kernel is ALU-bound, DRAM < 1 %

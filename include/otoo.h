@@ -121,6 +121,9 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).
+ * "warp_specialized" = 1 (default): otoo_gravity runs walker/evaluator warp pairs (walker warps build
+ * the lists in shared memory, evaluator warps hold the targets and sum), 0: one warp does both in turn.
+ * Same lists, same counters; sums differ in rounding order only.
  * "walk_only" = 1: the walks build and count their lists but skip the pair sums (outputs are
  * meaningless; counters exact) -- measures the walk's share of the fused kernel; default 0.
  * Unknown names: OTOO_ERR_INVALID_ARG. */

@@ -79,7 +79,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
   otoo_ctx* ctx = new (std::nothrow) otoo_ctx;
   if (!ctx) return OTOO_ERR_OOM;
   memset(ctx, 0, sizeof *ctx);
-  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->use_pool = 1;
+  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->use_pool = 1; ctx->use_ws = 1;
   otoo_status s = OTOO_OK;
   auto body = [&]() -> otoo_status {
     OTOO_CUDA(ctx, cudaSetDevice(device));
@@ -269,6 +269,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   }
   if (strcmp(name, "task_pool") == 0) { ctx->use_pool = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
+  if (strcmp(name, "warp_specialized") == 0) { ctx->use_ws = value != 0; return OTOO_OK; }
   return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");
 }
 

@@ -11,6 +11,7 @@
 #define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
 #define OTOO_LIST_CAP 256            // smem interaction-list float4 per warp (small: leaves the SM's L1 for the tree)
+#define OTOO_LIST_STRIDE (OTOO_LIST_CAP + 4)  // per-warp list buffer incl. slack (gravity's pipelined loop reads one entry ahead)
 #define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
 
 // Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).
@@ -84,6 +85,7 @@ struct otoo_ctx {
   int walk_stack;        // option "walk_stack"
   int use_pool;          // option "task_pool"
   int walk_only;         // option "walk_only" (diagnostic)
+  int use_ws;            // option "warp_specialized": gravity walk with walker/evaluator warp pairs
   int last_group_size;
   int64_t last_ngroups;
   int launches;          // kernels launched by the current/last API call

@@ -1,6 +1,15 @@
 // gravity.cu -- theta-MAC radii (R7) and the fused group walk + softened Plummer sums
 // (PAPER.md III-D L159-L167, L43, L57; readings R7-R11).
-#include "walk.cuh"
+#include "walk_ws.cuh"
+
+#ifndef OTOO_EVAL_UNR
+#define OTOO_EVAL_UNR 4
+#endif
+#ifndef OTOO_WS_MINB
+#define OTOO_WS_MINB 3
+#define OTOO_WS_EVAL_REGS 112
+#define OTOO_WS_WALK_REGS 48
+#endif
 
 namespace {
 
@@ -35,7 +44,7 @@ __device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); re
 
 template <int T_, bool EPS0>
 struct GravVisitor {
-  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64;
+  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64, UNR = OTOO_EVAL_UNR;
   const GravParams& p;
   float pm[T];
   float glo[3], ghi[3];
@@ -96,6 +105,13 @@ struct GravVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
+  static constexpr bool SUBMIT_LAST = false;
+  __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
+    if (!p.c.walk_only) eval(list, n);
+    return list;
+  }
+  // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
+  // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
   // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
   // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
@@ -107,7 +123,7 @@ struct GravVisitor {
         float2 cx[PB], cy[PB], cz[PB], cp[PB];
 #pragma unroll
         for (int q = 0; q < PB; q++) cx[q] = cy[q] = cz[q] = cp[q] = make_float2(0.0f, 0.0f);
-#pragma unroll 4
+#pragma unroll UNR
         for (int j = j0; j < je; j++) {
           const float4 s = list[j];
 #pragma unroll
@@ -155,11 +171,145 @@ template <int T, bool EPS0>
 __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(const GravParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
-  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
+  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_STRIDE;
+  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
   GravVisitor<T, EPS0> v(p);
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
+}
+
+
+// ---------------------------------------------------------------- warp-specialised form (walk_ws.cuh)
+// Walker-side visitor: the MAC, the list entries and the self marks of GravVisitor without targets or
+// sums; submit() publishes the filled buffer to the pair's evaluator warp and returns the next one.
+template <int T_>
+struct GravWalker {
+  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2;
+  static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
+  typedef WsPair<32 * NP * 3> Pair;
+  const GravParams& p;
+  Pair& sm;
+  float glo[3], ghi[3];
+  unsigned selfmask;
+  uint32_t group, buf, eparity, first;
+  int lane_;
+  __device__ __forceinline__ GravWalker(const GravParams& p_, Pair& sm_, int lane) : p(p_), sm(sm_), buf(0), eparity(~0u), first(0), lane_(lane) {}
+
+  __device__ __forceinline__ float4* acquire() {     // wait until the evaluator has released buffer `buf`
+    mbar_wait<500>(&sm.empty[buf], (eparity >> buf) & 1u);   // walkers run ahead: wait without stealing issue slots
+    eparity ^= 1u << buf;
+    return sm.list[buf];
+  }
+  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4*) {
+#pragma unroll
+    for (int t = 0; t < T; t++) {   // H7: the group's tight AABB
+      int64_t s = g0 + t * 32 + lane;
+      float4 v = p.c.spos[s < p.c.N ? s : g0];
+      if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
+      else {
+        glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
+        glo[1] = fminf(glo[1], v.y); ghi[1] = fmaxf(ghi[1], v.y);
+        glo[2] = fminf(glo[2], v.z); ghi[2] = fmaxf(ghi[2], v.z);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; k++)
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
+        ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
+      }
+    selfmask = 0; first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+  }
+  __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
+    A = __ldg(p.c.cell_cm + cell);
+    B = __ldg(p.c.cell_b + cell);
+    float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
+    return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
+  }
+  struct Entry { float4 a; };
+  __device__ __forceinline__ Entry get(uint32_t slot) const { Entry e; e.a = p.c.spos[slot]; return e; }
+  __device__ __forceinline__ void put(float4* dst, const Entry& e) const { *dst = e.a; }
+  __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
+  __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
+#pragma unroll
+    for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
+  }
+  __device__ __forceinline__ float4* submit(float4*, int n, bool last) {
+    if (lane_ == 0) sm.meta[buf] = WsMeta{(uint32_t)n, first | (last ? WS_LAST : 0u), group, 0u};
+    if (last) sm.self[buf][lane_] = selfmask;
+    first = 0;
+    mbar_arrive(&sm.full[buf]);
+    buf = (buf + 1) % OTOO_WS_NBUF;
+    return acquire();
+  }
+  __device__ __forceinline__ void store(int64_t, int) {}
+  __device__ __forceinline__ void finish() {          // tell the evaluator to exit
+    if (lane_ == 0) sm.meta[buf] = WsMeta{0u, WS_EXIT, 0u, 0u};
+    mbar_arrive(&sm.full[buf]);
+  }
+};
+
+template <int T> struct WsRegs { static constexpr int MINB = OTOO_WS_MINB, EVAL = OTOO_WS_EVAL_REGS, WALK = OTOO_WS_WALK_REGS; };
+template <> struct WsRegs<8> { static constexpr int MINB = 2, EVAL = 176, WALK = 80; };
+
+template <int T, bool EPS0>
+__global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_gravity_ws_kernel(const GravParams p) {
+  typedef typename GravWalker<T>::Pair Pair;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  Pair* pairs = reinterpret_cast<Pair*>(smem_raw);
+  if (threadIdx.x < OTOO_WS_PAIRS) {
+    Pair& s = pairs[threadIdx.x];
+#pragma unroll
+    for (int b = 0; b < OTOO_WS_NBUF; b++) { mbar_init(&s.full[b], 32); mbar_init(&s.empty[b], 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp >= OTOO_WS_PAIRS) {
+    // ---- walker: L57 rules through walk_driver, lists into the pair's buffers
+    if (WsRegs<T>::WALK) setmaxnreg_dec<WsRegs<T>::WALK>();
+    Pair& sm = pairs[warp - OTOO_WS_PAIRS];
+    GravWalker<T> w(p, sm, lane);
+    float4* list = w.acquire();
+    walk_driver(p.c, w, list, sm.stk, lane, (int64_t)blockIdx.x * OTOO_WS_PAIRS + (warp - OTOO_WS_PAIRS));
+    w.finish();
+  } else {
+    // ---- evaluator: targets and sums in registers, consumes the buffers in order
+    if (WsRegs<T>::EVAL) setmaxnreg_inc<WsRegs<T>::EVAL>();
+    Pair& sm = pairs[warp];
+    GravVisitor<T, EPS0> v(p);
+    uint32_t buf = 0, fparity = 0;
+    for (;;) {
+      mbar_wait(&sm.full[buf], (fparity >> buf) & 1u);
+      fparity ^= 1u << buf;
+      const WsMeta m = sm.meta[buf];
+      if (m.flags & WS_EXIT) break;
+      const int64_t g0 = (int64_t)m.group * (32 * T);
+      if (m.flags & WS_FIRST) { v.load_group(g0, lane, reinterpret_cast<float4*>(sm.tgt)); __syncwarp(); }
+      if (!p.c.walk_only && m.count) v.eval(sm.list[buf], (int)m.count);
+      if (m.flags & WS_LAST) { v.selfmask = sm.self[buf][lane]; v.store(g0, lane); }
+      mbar_arrive(&sm.empty[buf]);
+      buf = (buf + 1) % OTOO_WS_NBUF;
+    }
+  }
+}
+
+template <int T, bool EPS0>
+otoo_status launch_walk_ws2(otoo_ctx* ctx, const GravParams& p, cudaStream_t st) {
+  const size_t smem = OTOO_WS_PAIRS * sizeof(typename GravWalker<T>::Pair);
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_ws_kernel<T, EPS0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 1;
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_gravity_ws_kernel<T, EPS0>, OTOO_WS_PAIRS * 64, smem));
+  if (occ < 1) occ = 1;
+  int64_t grid = (int64_t)ctx->sm_count * occ;                       // persistent: every CTA resident
+  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups, OTOO_WS_PAIRS);
+  walk_gravity_ws_kernel<T, EPS0><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
+  return OTOO_OK;
+}
+template <int T>
+otoo_status launch_walk_ws(otoo_ctx* ctx, const GravParams& p, bool eps0, cudaStream_t st) {
+  return eps0 ? launch_walk_ws2<T, true>(ctx, p, st) : launch_walk_ws2<T, false>(ctx, p, st);
 }
 
 // reset the control block and the pool's sequence numbers (tickets restart from 0 every launch)
@@ -187,7 +337,7 @@ otoo_status launch_walk(otoo_ctx* ctx, const GravParams& p, bool eps0, int grid,
 }  // namespace
 
 size_t otoo_walk_smem_bytes() {
-  return (size_t)OTOO_WALK_WARPS * (OTOO_LIST_CAP * sizeof(float4) + OTOO_WALK_STACK_MAX * sizeof(uint32_t));
+  return (size_t)OTOO_WALK_WARPS * (OTOO_LIST_STRIDE * sizeof(float4) + OTOO_WALK_STACK_MAX * sizeof(uint32_t));
 }
 
 // Common launch preparation of the walk kernels: persistent grid, task pool, zeroed counters.
@@ -234,6 +384,15 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, floa
   p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);
   const bool eps0 = !(eps > 0.0f);
+  if (ctx->use_ws) {
+    switch (G) {
+      case 32: OTOO_TRY(launch_walk_ws<1>(ctx, p, eps0, st)); break;
+      case 64: OTOO_TRY(launch_walk_ws<2>(ctx, p, eps0, st)); break;
+      case 128: OTOO_TRY(launch_walk_ws<4>(ctx, p, eps0, st)); break;
+      case 256: OTOO_TRY(launch_walk_ws<8>(ctx, p, eps0, st)); break;
+      default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+    }
+  } else
   switch (G) {
     case 32: OTOO_TRY(launch_walk<1>(ctx, p, eps0, grid, smem, st)); break;
     case 64: OTOO_TRY(launch_walk<2>(ctx, p, eps0, grid, smem, st)); break;

@@ -163,6 +163,11 @@ struct SphVisitor {
     if (E >= 3) dst[2] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
+  static constexpr bool SUBMIT_LAST = false;
+  __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
+    if (!p.c.walk_only) eval(list, n);
+    return list;
+  }
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
     const float PI_F = 3.14159265358979323846f;
     for (int j = 0; j < n; j++) {
@@ -233,8 +238,8 @@ template <int T, int MODE>
 __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_CAP;
-  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_CAP * sizeof(float4)) +
+  float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_STRIDE;
+  uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
   SphVisitor<T, MODE> v(p);
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);

@@ -49,6 +49,9 @@ __device__ __forceinline__ int warp_inclusive_scan(int x, int lane) {
 // ---- global task pool (multi-producer multi-consumer ring of fixed-size tasks)
 #define OTOO_TASK_CELLS 256
 #define OTOO_POOL_SLOTS 16384
+#ifndef OTOO_MULTI_DONATE
+#define OTOO_MULTI_DONATE 4
+#endif
 #define OTOO_POOL_MARGIN 4096        // > number of resident warps: concurrent producers cannot overrun
 struct TaskSlot { uint32_t group, count, pad[2]; uint32_t cells[OTOO_TASK_CELLS]; };
 struct WalkShared {                   // device-global control block, reset before every launch
@@ -77,12 +80,15 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 //   void load_group(int64_t g0, int lane, float4* scratch)   targets into registers, AABB, zero accumulators
 //   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
 //   struct Entry; Entry get(uint32_t slot); void put(float4* dst, const Entry&)   one particle entry (E float4)
-//   void eval(const float4* list, int n)           all targets x n entries
+//   static constexpr bool SUBMIT_LAST;  true: the last list of a unit of work is submitted even if empty
+//   float4* submit(float4* list, int n, bool last)   consume n entries (fused visitors: all targets x n
+//                                                  entries, same buffer back; the warp-specialised walker:
+//                                                  hand the buffer to its evaluator warp, next buffer back)
 //   void pad(float4* dst)                          a null entry
 //   void mark_self(uint32_t first, uint32_t count, int64_t g0, int lane)
 //   void store(int64_t g0, int lane)               atomicAdd results to the outputs
 template <class V>
-__device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list, uint32_t* stk, int lane, int64_t gwarp) {
+__device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list0, uint32_t* stk, int lane, int64_t gwarp) {
   constexpr int G = 32 * V::T;
   constexpr int CAP = (OTOO_LIST_CAP / V::E) & ~3;   // list entries (multiple of the padding unit)
   constexpr int PADTO = 4;
@@ -91,12 +97,24 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   unsigned long long tot_steps = 0, tot_tasks = 0, tot_flushes = 0;
   bool main_done = false, have_ticket = false;
   uint32_t my_ticket = 0;
+  float4* list = list0;
 
   for (;;) {
-    // ---------------- acquire a unit of work: a group from the main queue, else a pool task
+    // ---------------- acquire a unit of work: the next group of the main queue, else a pool task
+    // (polling the pool before the queue was tried: 1776 warps contending for the head word with CAS
+    // cost more than it gained)
     uint32_t g = 0; int sp = 0;
     bool got = false;
-    if (!main_done) {
+    auto take = [&](uint32_t ticket) {   // copy task `ticket` (already published) to the shared stack
+      const uint32_t slot = ticket % OTOO_POOL_SLOTS;
+      __threadfence();
+      const TaskSlot* ts = c.slots + slot;
+      g = __ldcg(&ts->group); sp = (int)__ldcg(&ts->count);
+      for (int i = lane; i < sp; i += 32) stk[i] = __ldcg(&ts->cells[i]);
+      __syncwarp();
+      if (lane == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(&c.seq[slot]) = ticket + OTOO_POOL_SLOTS; }
+    };
+    if (!got && !main_done) {
       if (lane == 0) g = atomicAdd(&c.ws->queue, 1u);
       g = __shfl_sync(0xFFFFFFFFu, g, 0);
       if ((int64_t)g < c.ngroups) { got = true; if (lane == 0) stk[0] = 0u; sp = 1; }
@@ -109,21 +127,15 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
         my_ticket = __shfl_sync(0xFFFFFFFFu, my_ticket, 0);
         have_ticket = true;
       }
-      const uint32_t slot = my_ticket % OTOO_POOL_SLOTS;
       int ok = 0;
       if (lane == 0) {
-        if (ld_volatile(&c.seq[slot]) == my_ticket + 1u) ok = 1;
+        if (ld_volatile(&c.seq[my_ticket % OTOO_POOL_SLOTS]) == my_ticket + 1u) ok = 1;
         else if (*reinterpret_cast<volatile int*>(&c.ws->outstanding) <= 0) ok = -1;
       }
       ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
       if (ok < 0) break;
       if (ok == 0) { __nanosleep(400); continue; }
-      __threadfence();
-      const TaskSlot* ts = c.slots + slot;
-      g = __ldcg(&ts->group); sp = (int)__ldcg(&ts->count);
-      for (int i = lane; i < sp; i += 32) stk[i] = __ldcg(&ts->cells[i]);
-      __syncwarp();
-      if (lane == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(&c.seq[slot]) = my_ticket + OTOO_POOL_SLOTS; }
+      take(my_ticket);
       have_ticket = false;
       got = true;
     }
@@ -135,36 +147,46 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     int gsp = 0, nlist = 0;
     uint32_t ntests = 0, ncells = 0, nparts = 0, iter = 0, nflush = 0;
 
-    auto flush = [&]() {
+    auto flush = [&](bool last = false) {
       const int np = (nlist + PADTO - 1) & ~(PADTO - 1);
       if (lane < np - nlist) v.pad(list + V::E * (nlist + lane));
       __syncwarp();
-      if (!c.walk_only) v.eval(list, np);
+      list = v.submit(list, np, last);
       __syncwarp();
       nlist = 0; nflush++;
     };
-    // hand the `d` shallowest stack entries to the pool (returns false if the pool is full)
-    auto donate = [&](int d) -> bool {
-      uint32_t ticket = 0; int ok = 0;
-      if (!c.use_pool) return false;
+    // task pool, producer side: pool_begin reserves a slot (NULL if the pool is full), the caller writes
+    // `d` cell ids into it, pool_end publishes it
+    uint32_t pticket = 0;
+    auto pool_begin = [&]() -> TaskSlot* {
+      int ok = 0;
+      if (!c.use_pool) return nullptr;
       if (lane == 0) {
         uint32_t h = ld_volatile(&c.ws->head), t = ld_volatile(&c.ws->tail);
         if ((int)(t - h) < OTOO_POOL_SLOTS - OTOO_POOL_MARGIN) {
           ok = 1;
           atomicAdd(&c.ws->outstanding, 1);
-          ticket = atomicAdd(&c.ws->tail, 1u);
-          while (ld_volatile(&c.seq[ticket % OTOO_POOL_SLOTS]) != ticket) __nanosleep(64);
+          pticket = atomicAdd(&c.ws->tail, 1u);
+          while (ld_volatile(&c.seq[pticket % OTOO_POOL_SLOTS]) != pticket) __nanosleep(64);
         }
       }
       ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
-      if (!ok) return false;
-      ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
-      TaskSlot* ts = c.slots + (ticket % OTOO_POOL_SLOTS);
-      for (int i = lane; i < d; i += 32) __stcg(&ts->cells[i], stk[i]);
+      if (!ok) return nullptr;
+      pticket = __shfl_sync(0xFFFFFFFFu, pticket, 0);
+      return c.slots + (pticket % OTOO_POOL_SLOTS);
+    };
+    auto pool_end = [&](TaskSlot* ts, int d) {
       if (lane == 0) { __stcg(&ts->group, g); __stcg(&ts->count, (uint32_t)d); }
       __threadfence();
       __syncwarp();
-      if (lane == 0) *reinterpret_cast<volatile uint32_t*>(&c.seq[ticket % OTOO_POOL_SLOTS]) = ticket + 1u;
+      if (lane == 0) *reinterpret_cast<volatile uint32_t*>(&c.seq[pticket % OTOO_POOL_SLOTS]) = pticket + 1u;
+    };
+    // hand the `d` shallowest stack entries to the pool (returns false if the pool is full)
+    auto donate = [&](int d) -> bool {
+      TaskSlot* ts = pool_begin();
+      if (!ts) return false;
+      for (int i = lane; i < d; i += 32) __stcg(&ts->cells[i], stk[i]);
+      pool_end(ts, d);
       return true;
     };
     // drop the d bottom entries of the shared stack (after they were donated or spilled)
@@ -216,25 +238,43 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
         const int inc = warp_inclusive_scan(nch, lane);
         const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
         if (total) {
-          if (sp + total > c.stack_cap) {       // overflow: donate, else spill privately
-            const int d = OTOO_TASK_CELLS;      // stack_cap >= 512, total <= 256
-            if (!donate(d)) {
+          bool pushed = false;
+          if (sp + total > c.stack_cap) {
+            // overflow (a group with a system-sized box): the new children become a pool task of their own
+            // -- deep cells, small subtrees: the task is finished by whoever takes it and nothing circulates;
+            // this warp keeps generating such tasks from its shallow backlog.  Pool full: spill privately.
+            TaskSlot* ts = pool_begin();
+            if (ts) {
+              const int o = inc - nch;
+              for (int i = 0; i < nch; i++) __stcg(&ts->cells[o + i], B.y + (uint32_t)i);
+              pool_end(ts, total);
+              pushed = true;
+            } else {
+              const int d = OTOO_TASK_CELLS;      // stack_cap >= 512, total <= 256
               for (int i = lane; i < d; i += 32) gspill[gsp + i] = stk[i];
               gsp += d;
+              __syncwarp();
+              shift_down(d);
             }
-            __syncwarp();
-            shift_down(d);
           }
+          if (!pushed) {
           const int o = sp + inc - nch;
           for (int i = 0; i < nch; i++) stk[o + i] = B.y + (uint32_t)i;
           __syncwarp();
           sp += total;
+          }
         }
       }
       // load balance: feed idle warps with the shallowest entries
       if (sp >= 16 && idle_now > 0) {
-        int d = sp >> 1; if (d > OTOO_TASK_CELLS) d = OTOO_TASK_CELLS;
-        if (donate(d)) shift_down(d);
+        // several idle warps and a long stack: several smaller tasks at once (the shallowest entries first)
+        int nt = idle_now < OTOO_MULTI_DONATE ? idle_now : OTOO_MULTI_DONATE;
+        if (nt > (sp >> 4)) nt = sp >> 4;
+        int d = (sp >> 1) / nt; if (d > OTOO_TASK_CELLS) d = OTOO_TASK_CELLS;
+        for (int k = 0; k < nt; k++) {
+          if (!donate(d)) break;
+          shift_down(d);
+        }
       }
       // opened leaves -> their particles (L57 rule 3)
       const unsigned lm = __ballot_sync(0xFFFFFFFFu, open_leaf);
@@ -283,7 +323,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
         __syncwarp();
       }
     }
-    if (nlist) flush();
+    if (nlist || V::SUBMIT_LAST) flush(true);
     v.store(g0, lane);
     if (lane == 0) {
       atomicAdd(c.g_ntests + g, ntests); atomicAdd(c.g_ncells + g, ncells); atomicAdd(c.g_nparts + g, nparts);
@@ -296,8 +336,10 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   }
   if (lane == 0 && tot_tests) {
     atomicAdd(c.sums + 0, tot_tests); atomicAdd(c.sums + 1, tot_inter);
-    atomicAdd(c.sums + 2, tot_cells); atomicAdd(c.sums + 3, tot_parts);
-    atomicAdd(c.sums + 4, tot_steps); atomicAdd(c.sums + 5, tot_tasks); atomicAdd(c.sums + 6, tot_flushes);
+    atomicAdd(c.sums + 2, tot_cells);
+    atomicAdd(c.sums + 3, tot_parts);
+    atomicAdd(c.sums + 4, tot_steps); atomicAdd(c.sums + 5, tot_tasks);
+    atomicAdd(c.sums + 6, tot_flushes);
   }
 }
 

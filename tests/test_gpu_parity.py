@@ -85,12 +85,18 @@ def test_tree_degenerate_inputs(otoo, orc):
                                                 ("uniform_cube", 50000, 128, 0.5, 0.001), ("plummer", 3000, 64, 0.0, 0.01),
                                                 ("plummer", 3000, 128, 0.5, 0.0), ("uniform_sphere", 2500, 256, 0.0, 0.0),
                                                 ("plummer", 40, 64, 0.5, 0.01)])
-def test_gravity_parity(otoo, orc, kind, n, G, theta, eps):
+@pytest.mark.parametrize("ws", [1, 0])
+def test_gravity_parity(otoo, orc, kind, n, G, theta, eps, ws):
+    """ws = 1: walker/evaluator warp pairs (default); ws = 0: the fused one-warp-does-both kernel."""
     pm = gen.make(kind, n, 1206)
     t = check_tree(otoo, orc, pm, 16)
     theta32, eps32 = float(np.float32(theta)), float(np.float32(eps))
     ref = t.gravity(eps32, theta32, G)
-    out = otoo.otoo_gravity(eps32, theta32, G).cpu().numpy()
+    otoo.otoo_set_option("warp_specialized", ws)
+    try:
+        out = otoo.otoo_gravity(eps32, theta32, G).cpu().numpy()
+    finally:
+        otoo.otoo_set_option("warp_specialized", 1)
     assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta32).view(np.uint32))
     nt, nc, npart = otoo.otoo_export_group_stats()
     assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
@@ -109,8 +115,9 @@ def test_walk_stack_spill(otoo, orc):
     pm = gen.plummer(30000, 77)
     t = check_tree(otoo, orc, pm, 1)
     try:
-        for theta, pool in ((0.0, 0), (0.0, 1), (0.3, 0)):
+        for theta, pool, ws in ((0.0, 0, 1), (0.0, 1, 1), (0.3, 0, 1), (0.0, 0, 0), (0.0, 1, 0)):
             otoo.otoo_set_option("task_pool", pool)
+            otoo.otoo_set_option("warp_specialized", ws)
             ref = t.gravity(0.01, theta, 32)
             out = otoo.otoo_gravity(0.01, theta, 32).cpu().numpy()
             nt, nc, npart = otoo.otoo_export_group_stats()
@@ -119,6 +126,7 @@ def test_walk_stack_spill(otoo, orc):
             assert e.max() <= TOL
     finally:
         otoo.otoo_set_option("task_pool", 1)
+        otoo.otoo_set_option("warp_specialized", 1)
 
 
 @pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
