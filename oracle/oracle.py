@@ -58,6 +58,12 @@ def lib():
         L.orc_direct_sum.argtypes = [i64, vp, dbl, i64, vp, vp]
         L.orc_gravity.restype = C.c_uint64
         L.orc_gravity.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, vp, vp, vp, vp]
+        L.orc_gravity_sel.restype = C.c_uint64
+        L.orc_gravity_sel.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, i64, vp, vp, vp, vp, vp]
+        L.orc_sph_density_sel.restype = C.c_uint64
+        L.orc_sph_density_sel.argtypes = [vp, vp, i32, vp, i64, vp, vp, vp, vp]
+        L.orc_sph_force_sel.restype = C.c_uint64
+        L.orc_sph_force_sel.argtypes = [vp, vp, vp, vp, vp, i32, vp, i64, vp, vp]
         L.orc_group_lists.argtypes = [vp, dbl, i32, i32, i64, vp, vp]
         L.orc_sph_cell_radii.argtypes = [vp, vp, vp, vp]
         L.orc_sph_density.restype = C.c_uint64
@@ -161,16 +167,29 @@ class Tree:
     def n_groups(self, G):
         return (self.N + G - 1) // G
 
-    def gravity(self, eps, theta, group_size, mac_kind=0, walk_kind=0, forces=True):
-        ng = self.n_groups(group_size)
+    def gravity(self, eps, theta, group_size, mac_kind=0, walk_kind=0, forces=True, groups=None):
+        """groups: optional array of group indices; then only those are walked, the counters are indexed
+        by position in `groups`, and acc_pot / abs_sum (still N rows) are filled for their targets only."""
+        sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
+        ng = self.n_groups(group_size) if sel is None else len(sel)
         acc = np.zeros((self.N, 4), dtype=np.float64) if forces else None
         nt = np.zeros(ng, dtype=np.uint32)
         nc = np.zeros(ng, dtype=np.uint32)
         npart = np.zeros(ng, dtype=np.uint32)
         asum = np.zeros(self.N, dtype=np.float64) if forces else None
-        tot = lib().orc_gravity(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
-                                int(walk_kind), _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
+        tot = lib().orc_gravity_sel(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
+                                    int(walk_kind), _p(sel), 0 if sel is None else len(sel),
+                                    _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
         return dict(acc_pot=acc, n_tests=nt, n_cells=nc, n_parts=npart, interactions=int(tot), abs_sum=asum)
+
+    def group_targets(self, group_size, groups):
+        """original particle indices of the members of the given groups (sorted slots -> perm)"""
+        perm = self.export()["perm"] if not hasattr(self, "_perm") else self._perm
+        self._perm = perm
+        out = []
+        for g in np.asarray(groups, dtype=np.int64):
+            out.append(perm[g * group_size:min((g + 1) * group_size, self.N)])
+        return np.concatenate(out).astype(np.int64)
 
     def group_lists(self, theta, group_size, g, n_cells, n_parts, mac_kind=0):
         cells = np.empty(max(int(n_cells), 1), dtype=np.uint32)
@@ -186,14 +205,16 @@ class Tree:
         lib().orc_sph_cell_radii(self._h, _p(h), _p(b), _p(r))
         return b, r
 
-    def sph_density(self, h, group_size, sums=True):
+    def sph_density(self, h, group_size, sums=True, groups=None):
         h = _f32(h, (self.N,))
-        ng = self.n_groups(group_size)
+        sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
+        ng = self.n_groups(group_size) if sel is None else len(sel)
         rho = np.zeros(self.N, dtype=np.float64) if sums else None
         nngb = np.zeros(self.N, dtype=np.uint32)
         nt = np.zeros(ng, dtype=np.uint32)
         npart = np.zeros(ng, dtype=np.uint32)
-        tot = lib().orc_sph_density(self._h, _p(h), int(group_size), _p(rho), _p(nngb), _p(nt), _p(npart))
+        tot = lib().orc_sph_density_sel(self._h, _p(h), int(group_size), _p(sel), 0 if sel is None else len(sel),
+                                        _p(rho), _p(nngb), _p(nt), _p(npart))
         return dict(rho=rho, nngb=nngb, n_tests=nt, n_parts=npart, candidates=int(tot))
 
     def sph_group_list(self, h, group_size, g, n_parts):
@@ -202,12 +223,14 @@ class Tree:
         lib().orc_sph_group_list(self._h, _p(h), int(group_size), int(g), _p(parts))
         return parts[:int(n_parts)]
 
-    def sph_force(self, h, rho, P, group_size, vel=None):
+    def sph_force(self, h, rho, P, group_size, vel=None, groups=None):
         h = _f32(h, (self.N,))
         rho = np.ascontiguousarray(rho, dtype=np.float64)
         P = np.ascontiguousarray(P, dtype=np.float64)
         v = None if vel is None else _f32(vel, (self.N, 4))
         out = np.zeros((self.N, 4), dtype=np.float64)
         asum = np.zeros((self.N, 2), dtype=np.float64)
-        tot = lib().orc_sph_force(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(out), _p(asum))
+        sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
+        tot = lib().orc_sph_force_sel(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(sel),
+                                      0 if sel is None else len(sel), _p(out), _p(asum))
         return dict(acc_dudt=out, candidates=int(tot), abs_sum=asum)

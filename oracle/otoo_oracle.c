@@ -372,34 +372,45 @@ static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double 
   if (abs_out) *abs_out = asum;
 }
 
-uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
-                     double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
-  int64_t N = t->N, ng = (N + G - 1) / G;
+/* sel != NULL: only the groups sel[0..nsel) are walked (counters indexed by position in sel, sums written
+ * for their targets only); the loop over groups is then serial and the targets of a group run in parallel,
+ * so that one system-sized group does not serialise the run.  Same arithmetic either way. */
+uint64_t orc_gravity_sel(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
+                         const int64_t* sel, int64_t nsel,
+                         double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
+  int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
   float* rb2 = (float*)malloc(4 * t->ncell);
   orc_rb2(t, theta, mac_kind, rb2);
   double e2 = eps * eps;
   uint64_t total = 0;
-#pragma omp parallel reduction(+ : total)
+#pragma omp parallel reduction(+ : total) if (sel == NULL)
   {
     lists_t L; memset(&L, 0, sizeof L);
 #pragma omp for schedule(dynamic, 1)
-    for (int64_t g = 0; g < ng; g++) {
+    for (int64_t gi = 0; gi < ng; gi++) {
+      int64_t g = sel ? sel[gi] : gi;
       int64_t a = g * G, b = a + G < N ? a + G : N;
       gbox_t box = group_box(t, a, b, NULL);
       L.nc = L.np = 0; L.ntests = 0;
       if (walk_kind == 0) walk_rec(t, rb2, &box, 0, &L); else walk_stackless(t, rb2, &box, &L);
-      if (n_tests) n_tests[g] = L.ntests;
-      if (n_cells) n_cells[g] = (uint32_t)L.nc;
-      if (n_parts) n_parts[g] = (uint32_t)L.np;
+      if (n_tests) n_tests[gi] = L.ntests;
+      if (n_cells) n_cells[gi] = (uint32_t)L.nc;
+      if (n_parts) n_parts[gi] = (uint32_t)L.np;
       total += (uint64_t)(b - a) * (uint64_t)(L.nc + L.np);   /* R11 */
-      if (acc_pot)
+      if (acc_pot) {
+#pragma omp parallel for schedule(dynamic, 1) if (sel != NULL)
         for (int64_t s = a; s < b; s++)
           grav_sums(t, &L, s, e2, acc_pot + 4 * (int64_t)t->perm[s], abs_sum ? abs_sum + t->perm[s] : NULL);
+      }
     }
     free(L.cells); free(L.parts);
   }
   free(rb2);
   return total;
+}
+uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
+                     double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
+  return orc_gravity_sel(t, eps, theta, G, mac_kind, walk_kind, NULL, 0, acc_pot, n_tests, n_cells, n_parts, abs_sum);
 }
 
 void orc_group_lists(const orc_tree* t, double theta, int G, int mac_kind, int64_t g,
@@ -483,9 +494,9 @@ static float r2_f32(const float* a, const float* b) { /* R16: the fp32 neighbour
   return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
 }
 
-uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, uint32_t* nngb,
-                         uint32_t* n_tests, uint32_t* n_parts) {
-  int64_t N = t->N, ng = (N + G - 1) / G;
+uint64_t orc_sph_density_sel(const orc_tree* t, const float* h, int G, const int64_t* sel, int64_t nsel,
+                             double* rho, uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts) {
+  int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
   sph_radii_sorted(t, hs, bmax, rsph);
@@ -494,13 +505,14 @@ uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, 
   {
     lists_t L; memset(&L, 0, sizeof L);
 #pragma omp for schedule(dynamic, 1)
-    for (int64_t g = 0; g < ng; g++) {
+    for (int64_t gi = 0; gi < ng; gi++) {
+      int64_t g = sel ? sel[gi] : gi;
       int64_t a = g * G, b = a + G < N ? a + G : N;
       gbox_t box = group_box(t, a, b, hs);
       L.np = 0; L.ntests = 0;
       walk_sph(t, bmax, rsph, &box, 0, &L);
-      if (n_tests) n_tests[g] = L.ntests;
-      if (n_parts) n_parts[g] = (uint32_t)L.np;
+      if (n_tests) n_tests[gi] = L.ntests;
+      if (n_parts) n_parts[gi] = (uint32_t)L.np;
       total += (uint64_t)(b - a) * (uint64_t)L.np;
       for (int64_t s = a; s < b && rho; s++) {
         const float* pi = t->spos + 4 * s;
@@ -524,6 +536,10 @@ uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, 
   return total;
 }
 
+uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, uint32_t* nngb,
+                         uint32_t* n_tests, uint32_t* n_parts) {
+  return orc_sph_density_sel(t, h, G, NULL, 0, rho, nngb, n_tests, n_parts);
+}
 void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uint32_t* part_slots) {
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
@@ -537,9 +553,9 @@ void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uin
 }
 
 /* R17: symmetric pressure force (TREESPH/GADGET form) and optional du/dt. */
-uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, const double* P,
-                       const float* vel, int G, double* out, double* abs_sum) {
-  int64_t N = t->N, ng = (N + G - 1) / G;
+uint64_t orc_sph_force_sel(const orc_tree* t, const float* h, const double* rho, const double* P,
+                           const float* vel, int G, const int64_t* sel, int64_t nsel, double* out, double* abs_sum) {
+  int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
   sph_radii_sorted(t, hs, bmax, rsph);
@@ -548,7 +564,8 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
   {
     lists_t L; memset(&L, 0, sizeof L);
 #pragma omp for schedule(dynamic, 1)
-    for (int64_t g = 0; g < ng; g++) {
+    for (int64_t gi = 0; gi < ng; gi++) {
+      int64_t g = sel ? sel[gi] : gi;
       int64_t a = g * G, b = a + G < N ? a + G : N;
       gbox_t box = group_box(t, a, b, hs);
       L.np = 0; L.ntests = 0;
@@ -589,6 +606,10 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
   }
   free(hs); free(bmax); free(rsph);
   return total;
+}
+uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, const double* P,
+                       const float* vel, int G, double* out, double* abs_sum) {
+  return orc_sph_force_sel(t, h, rho, P, vel, G, NULL, 0, out, abs_sum);
 }
 
 int orc_max_threads(void) {

@@ -66,6 +66,11 @@ void orc_rb2(const orc_tree*, double theta, int mac_kind, float* rb2 /*ncell*/);
 uint64_t orc_gravity(const orc_tree*, double eps, double theta, int group_size, int mac_kind,
                      int walk_kind, double* acc_pot /*4N*/, uint32_t* n_tests, uint32_t* n_cells,
                      uint32_t* n_parts, double* abs_sum /*N or NULL: sum_j |a_ij| over the same lists*/);
+/* The same for a selection of groups only (sel[0..nsel) group indices; counters indexed by position
+ * in sel; acc_pot/abs_sum still 4N/N, written for the selected groups' targets only). */
+uint64_t orc_gravity_sel(const orc_tree*, double eps, double theta, int group_size, int mac_kind,
+                         int walk_kind, const int64_t* sel, int64_t nsel, double* acc_pot,
+                         uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum);
 /* the lists of one group (sizes from orc_gravity counters) */
 void orc_group_lists(const orc_tree*, double theta, int group_size, int mac_kind, int64_t g,
                      uint32_t* cell_ids, uint32_t* part_slots);
@@ -74,12 +79,17 @@ void orc_group_lists(const orc_tree*, double theta, int group_size, int mac_kind
 void orc_sph_cell_radii(const orc_tree*, const float* h, float* bmax, float* rsph /*ncell each*/);
 uint64_t orc_sph_density(const orc_tree*, const float* h, int group_size, double* rho,
                          uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
+uint64_t orc_sph_density_sel(const orc_tree*, const float* h, int group_size, const int64_t* sel,
+                             int64_t nsel, double* rho, uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
 /* candidate list of one SPH group (sorted slots) */
 void orc_sph_group_list(const orc_tree*, const float* h, int group_size, int64_t g,
                         uint32_t* part_slots);
 uint64_t orc_sph_force(const orc_tree*, const float* h, const double* rho, const double* P,
                        const float* vel /*4N or NULL*/, int group_size, double* acc_dudt /*4N*/,
                        double* abs_sum /*2N or NULL: sum_j |a_ij|, sum_j |du_ij|*/);
+uint64_t orc_sph_force_sel(const orc_tree*, const float* h, const double* rho, const double* P,
+                           const float* vel, int group_size, const int64_t* sel, int64_t nsel,
+                           double* acc_dudt, double* abs_sum);
 /* cubic spline with support h (R13) */
 double orc_W(double r, double h);
 double orc_dWdr(double r, double h);

@@ -1,0 +1,134 @@
+"""GPU parity at BASELINE.json's full sizes (configs 2-5), in the launch configuration bench.py times.
+
+At these sizes the oracle still builds the whole tree and walks every group in seconds, so all the
+integer work is compared in full and bit for bit: keys, permutation, every cell tuple, fp32 (cm, M),
+per-group (n_tests, n_cells, n_parts) of EVERY group, total interactions.  The fp64 sums are computed
+by the oracle one group at a time for a seeded sample of groups plus the group with the longest list,
+and compared per particle with the tolerances of DESIGN.md section 7.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from workloads import generators as gen  # noqa: E402
+
+TOL = 1e-5
+U32 = 2.0 ** -24
+N_SAMPLE = 48
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def check_tree_full(o, t):
+    ex, eo = o.otoo_export_tree(), t.export()
+    assert ex["N"] == t.N and ex["N_cell"] == t.ncell and ex["N_leaf"] == t.nleaf and ex["depth"] == t.depth
+    assert np.array_equal(ex["lo"], t.lo) and ex["S"] == t.S
+    assert np.array_equal(ex["keys"], eo["keys"]) and np.array_equal(ex["perm"], eo["perm"])
+    for f in ("level", "prefix", "first", "count", "child_first", "child_count"):
+        assert np.array_equal(ex["cells"][f], eo["cells"][f]), f
+    assert np.array_equal(ex["com_m"].view(np.uint32), eo["com_m"].view(np.uint32))
+    return eo["perm"]
+
+
+def sample_groups(ng, lengths, seed, max_list):
+    """seeded sample of groups + the group with the longest list the oracle can sum in seconds"""
+    rng = np.random.default_rng(seed)
+    sel = set(rng.choice(ng, size=min(N_SAMPLE, ng), replace=False).tolist())
+    ok = np.where(lengths <= max_list)[0]
+    sel.add(int(ok[np.argmax(lengths[ok])]))
+    sel.add(ng - 1)                                   # the ragged last group
+    return np.array(sorted(sel), dtype=np.int64)
+
+
+def vec_check(got, want, abs_sum, pct):
+    d = np.linalg.norm(got[:, :3].astype(np.float64) - want[:, :3], axis=1)
+    an = np.linalg.norm(want[:, :3], axis=1)
+    tol = np.maximum(TOL * an, 8 * U32 * abs_sum)
+    assert np.all(d <= tol), float((d / np.maximum(tol, 1e-300)).max())
+    assert np.percentile(d / np.maximum(an, 1e-300), pct) <= TOL
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_fullsize_gravity(orc, name):
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    cfg = gen.CONFIGS[name]
+    n, G = cfg["n"], cfg["group"]
+    pm = gen.make(cfg["kind"], n, 1206)
+    eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        d_pm = dev(pm)
+        o.otoo_build_tree(d_pm, cfg["n_crit"])
+        t = orc.Tree(pm, cfg["n_crit"])
+        perm = check_tree_full(o, t).astype(np.int64)
+        out = o.otoo_gravity(eps, theta, G).cpu().numpy()
+        assert np.array_equal(o.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta).view(np.uint32))
+        # every group's counters, bit for bit
+        ref = t.gravity(eps, theta, G, forces=False)
+        nt, nc, npart = o.otoo_export_group_stats()
+        assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+        st = o.otoo_last_stats()
+        assert st["sum_interactions"] == ref["interactions"] and st["sum_tests"] == int(ref["n_tests"].sum())
+        # fp64 sums for a sample of groups
+        ng = t.n_groups(G)
+        lengths = nc.astype(np.int64) + npart
+        sel = sample_groups(ng, lengths, 1206, max_list=4_000_000)
+        rs = t.gravity(eps, theta, G, groups=sel)
+        assert np.array_equal(rs["n_tests"], nt[sel])
+        idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
+        vec_check(out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9)
+        pe = np.abs(out[idx, 3] - rs["acc_pot"][idx, 3]) / np.abs(rs["acc_pot"][idx, 3])
+        assert pe.max() <= TOL, pe.max()
+        assert np.isfinite(out).all()
+    finally:
+        o.close()
+
+
+def test_fullsize_sph(orc):
+    """BASELINE config 4: SPH density and pressure force (+du/dt) on the 2M-particle white-dwarf pair."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    cfg = gen.CONFIGS["C4"]
+    n, G = cfg["n"], cfg["group_sph"]
+    w = gen.wd_pair(n, 1206)
+    pm, h, u, vel = w["pos_mass"], w["h"], w["u"], w["vel"]
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        o.otoo_build_tree(dev(pm), cfg["n_crit"])
+        t = orc.Tree(pm, cfg["n_crit"])
+        perm = check_tree_full(o, t).astype(np.int64)
+        d_h = dev(h)
+        rho, nngb = o.otoo_sph_density(d_h, G)
+        b, r = o.otoo_export_sph_radii()
+        bo, ro = t.sph_cell_radii(h)
+        assert np.array_equal(b.view(np.uint32), bo.view(np.uint32)) and np.array_equal(r.view(np.uint32), ro.view(np.uint32))
+        ref = t.sph_density(h, G, sums=False)                      # every group's counters
+        nt, _, npart = o.otoo_export_group_stats()
+        assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(npart, ref["n_parts"])
+        assert o.otoo_last_stats()["sum_interactions"] == ref["candidates"]
+        ng = t.n_groups(G)
+        sel = sample_groups(ng, npart.astype(np.int64), 1199, max_list=1 << 30)
+        idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
+        rs = t.sph_density(h, G, groups=sel)
+        rg = rho.cpu().numpy()
+        assert np.array_equal(nngb.cpu().numpy().view(np.uint32)[idx], rs["nngb"][idx])
+        assert (np.abs(rg[idx] - rs["rho"][idx]) / rs["rho"][idx]).max() <= TOL
+        assert np.isfinite(rg).all() and (rg > 0).all()
+        P = o.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
+        Pg = P.cpu().numpy()
+        vel2 = vel.copy()
+        vel2[:, :3] += (-0.3 * pm[:, :3]).astype(np.float32)          # a contraction: du/dt is not rounding noise
+        out = o.otoo_sph_force(d_h, rho, P, G, vel=dev(vel2)).cpu().numpy()
+        rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel2, groups=sel)
+        vec_check(out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
+        tol = np.maximum(TOL * np.abs(rf["acc_dudt"][idx, 3]), 8 * U32 * rf["abs_sum"][idx, 1])
+        assert np.all(np.abs(out[idx, 3] - rf["acc_dudt"][idx, 3]) <= tol)
+    finally:
+        o.close()

@@ -131,3 +131,32 @@ def test_interaction_count_definition(orc):
     sizes = np.minimum(G, n - np.arange(t.n_groups(G)) * G)
     assert r["interactions"] == int((sizes * (r["n_cells"].astype(np.int64) + r["n_parts"])).sum())
     assert r["acc_pot"] is None
+
+
+def test_group_selection_equals_full_run(orc):
+    """orc_gravity_sel / orc_sph_*_sel (used by the full-size GPU parity tests) give, for the selected
+    groups, exactly what the all-groups run gives."""
+    pm = gen.plummer(6000, 11)
+    t = orc.Tree(pm, 8)
+    full = t.gravity(0.01, 0.6, 64)
+    sel = np.array([0, 3, 17, 50, t.n_groups(64) - 1], dtype=np.int64)
+    part = t.gravity(0.01, 0.6, 64, groups=sel)
+    for k in ("n_tests", "n_cells", "n_parts"):
+        assert np.array_equal(part[k], full[k][sel])
+    idx = t.group_targets(64, sel)
+    assert np.array_equal(part["acc_pot"][idx], full["acc_pot"][idx])
+    assert np.array_equal(part["abs_sum"][idx], full["abs_sum"][idx])
+    rest = np.setdiff1d(np.arange(6000), idx)
+    assert not part["acc_pot"][rest].any()
+    w = gen.wd_pair(5000, 3)
+    ts = orc.Tree(w["pos_mass"], 16)
+    fd = ts.sph_density(w["h"], 32)
+    sel = np.array([1, 2, 40, ts.n_groups(32) - 1], dtype=np.int64)
+    pd = ts.sph_density(w["h"], 32, groups=sel)
+    idx = ts.group_targets(32, sel)
+    assert np.array_equal(pd["n_parts"], fd["n_parts"][sel]) and np.array_equal(pd["rho"][idx], fd["rho"][idx])
+    assert np.array_equal(pd["nngb"][idx], fd["nngb"][idx])
+    P = (2.0 / 3.0) * fd["rho"] * w["u"]
+    ff = ts.sph_force(w["h"], fd["rho"], P, 32, vel=w["vel"])
+    pf = ts.sph_force(w["h"], fd["rho"], P, 32, vel=w["vel"], groups=sel)
+    assert np.array_equal(pf["acc_dudt"][idx], ff["acc_dudt"][idx])
