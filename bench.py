@@ -136,14 +136,14 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1206_1199_b200 import binding   # fails loudly if libotoo.so is missing
+    from paper_1206_1199_b200 import binding, replicas   # fails loudly if libotoo.so is missing
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     # replicas only: every rank runs the same workload with its own seed
-    cfg, pm = workload(args.workload, args.theta, args.seed + rank)
+    cfg, pm = workload(args.workload, args.theta, replicas.replica_seed(args.seed, rank))
     n, G, n_crit = cfg["n"], cfg["group"], cfg["n_crit"]
     eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
     o = binding.Otoo(max_particles=n, device=local)
@@ -182,12 +182,7 @@ def main():
     t_build = np.array([e[0].elapsed_time(e[1]) for e in evs])
     t_grav = np.array([e[1].elapsed_time(e[2]) for e in evs])
     ms_step = float((t_build + t_grav).mean())
-    tot_ms = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
-    tot_inter = torch.tensor([float(inter)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tot_ms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot_inter, op=dist.ReduceOp.SUM)
-    ms_max, inter_all = float(tot_ms.item()), float(tot_inter.item())
+    ms_max, inter_all = replicas.aggregate(ms_step, float(inter), device="cuda")   # max over ranks, sum over ranks
     value = inter_all / (ms_max * 1e-3)
 
     # ---- end to end through the host-buffer C-ABI call (pinned host memory)
@@ -202,10 +197,8 @@ def main():
         dt = time.perf_counter() - t0
         if it >= 2:
             e2e_t.append(dt)
-    e2e_ms = torch.tensor([1e3 * float(np.mean(e2e_t))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
-    e2e_val = inter_all / (float(e2e_ms.item()) * 1e-3)
+    e2e_ms, _ = replicas.aggregate(1e3 * float(np.mean(e2e_t)), float(inter), device="cuda")
+    e2e_val = inter_all / (e2e_ms * 1e-3)
 
     if rank != 0:
         if world > 1:
@@ -237,7 +230,7 @@ def main():
             "gflops": FLOPS_PER_INTERACTION * value / 1e9,
             "interactions_per_step": inter_all, "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
-                    "ms_per_step": float(e2e_ms.item())},
+                    "ms_per_step": e2e_ms},
             "gpu_launches": int(launches_step * args.steps), "roofline": roofline}
 
     if not args.no_cpu_baseline and world == 1:

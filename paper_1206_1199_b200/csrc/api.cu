@@ -90,8 +90,9 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     for (int b = 0; b < 2; b++) { OTOO_TRY(dalloc(ctx, &ctx->key[b], n)); OTOO_TRY(dalloc(ctx, &ctx->val[b], n)); }
     OTOO_TRY(dalloc(ctx, &ctx->spos, n));
     OTOO_TRY(dalloc(ctx, &ctx->slot_nc, n));
-    ctx->hist_cap = (size_t)cdiv(max_particles, 4096) * 256 + 256;
+    ctx->hist_cap = (size_t)cdiv(max_particles, 4096) * 512 + 4096;   // look-back status (u64 per tile and digit) + histograms
     OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
+    OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t)));
     OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));
     OTOO_TRY(dalloc(ctx, &ctx->d_bbox, 16));
     OTOO_TRY(dalloc(ctx, &ctx->d_counters, 64));
@@ -115,7 +116,7 @@ void otoo_destroy(otoo_ctx* ctx) {
                   ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_sph,
                   ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
                   ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums,
-                  ctx->pool_slots, ctx->pool_seq, ctx->walk_shared};
+                  ctx->pool_slots, ctx->pool_seq, ctx->walk_shared, ctx->stage_in, ctx->stage_out};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);
@@ -280,11 +281,21 @@ otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N,
   if (N > ctx->maxN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "N exceeds max_particles of otoo_create");
   if (N == 0) return OTOO_OK;
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
-  // staging: key[1] (8 B/particle) + val[1] are free before the sort; use dedicated buffers instead
-  float4 *d_in = nullptr, *d_out = nullptr;
-  OTOO_CUDA(ctx, cudaMalloc((void**)&d_in, 16 * (size_t)N));
-  cudaError_t e = cudaMalloc((void**)&d_out, 16 * (size_t)N);
-  if (e != cudaSuccess) { cudaFree(d_in); return otoo_fail(ctx, OTOO_ERR_OOM, "staging allocation failed"); }
+  // context-owned staging buffers (grow-only: no allocation on the repeated call of a time-step loop)
+  if (N > ctx->stage_cap) {
+    if (ctx->stage_in) cudaFree(ctx->stage_in);
+    if (ctx->stage_out) cudaFree(ctx->stage_out);
+    ctx->stage_in = ctx->stage_out = nullptr; ctx->stage_cap = 0;
+    if (cudaMalloc((void**)&ctx->stage_in, 16 * (size_t)N) != cudaSuccess ||
+        cudaMalloc((void**)&ctx->stage_out, 16 * (size_t)N) != cudaSuccess) {
+      if (ctx->stage_in) cudaFree(ctx->stage_in);
+      ctx->stage_in = nullptr;
+      cudaGetLastError();
+      return otoo_fail(ctx, OTOO_ERR_OOM, "staging allocation failed");
+    }
+    ctx->stage_cap = N;
+  }
+  float4 *d_in = ctx->stage_in, *d_out = ctx->stage_out;
   otoo_status s = OTOO_OK;
   cudaStream_t st = 0;
   if (cudaMemcpyAsync(d_in, h_pos_mass, 16 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "H2D copy failed");
@@ -294,7 +305,6 @@ otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N,
   ctx->launches += l1;
   if (s == OTOO_OK && cudaMemcpyAsync(h_acc_pot, d_out, 16 * (size_t)N, cudaMemcpyDeviceToHost, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "D2H copy failed");
   if (s == OTOO_OK && cudaStreamSynchronize(st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "synchronize failed");
-  cudaFree(d_in); cudaFree(d_out);
   return s;
 }
 

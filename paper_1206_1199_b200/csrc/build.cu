@@ -251,8 +251,13 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
   OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
   for (int b = 0; b < 2; b++) { OTOO_TRY(grow(ctx, &ctx->tmp_key[b], cap)); OTOO_TRY(grow(ctx, &ctx->tmp_val[b], cap)); }
-  size_t need = (size_t)cdiv(cap, 4096) * 256 + 256;
-  if (need > ctx->hist_cap) { OTOO_TRY(grow(ctx, &ctx->hist, need)); ctx->hist_cap = need; }
+  size_t need = (size_t)cdiv(cap, 4096) * 512 + 4096;
+  if (need > ctx->hist_cap) {
+    OTOO_TRY(grow(ctx, &ctx->hist, need));
+    ctx->hist_cap = need;
+    OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, need * sizeof(uint32_t)));   // status epochs restart
+    ctx->sort_epoch = 0;
+  }
   ctx->cellCap = cap;
   return OTOO_OK;
 }

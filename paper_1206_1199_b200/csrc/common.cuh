@@ -32,7 +32,9 @@ struct otoo_ctx {
   float4* spos;          // positions+mass in sorted order
   uint32_t* slot_nc;     // cells starting at slot s, then its exclusive scan
   uint32_t* scan_tmp;    // block sums for the scan
-  uint32_t* hist;        // radix histograms [256][nblocks]
+  uint32_t* hist;        // sort scratch: digit histograms, tile tickets, look-back status words
+  uint32_t sort_epoch;   // one epoch per radix pass: stale status words never match
+  bool sort_attr_set;
   size_t hist_cap;
   float* sorted_h;       // SPH: h in sorted order
   float4* sorted_aux;    // SPH force: (rho-independent) per-particle packed inputs in sorted order
@@ -73,6 +75,9 @@ struct otoo_ctx {
   void* pool_slots;      // task pool (walk.cuh): TaskSlot[OTOO_POOL_SLOTS]
   void* pool_seq;        // uint32 sequence numbers
   void* walk_shared;     // WalkShared control block
+
+  // ---- otoo_gravity_host staging (grow-only)
+  float4* stage_in; float4* stage_out; int64_t stage_cap;
 
   // ---- state
   bool built;

@@ -1,7 +1,7 @@
 // sort.cu -- device LSD radix sort of (u64 key, u32 value) pairs and a u32 exclusive scan.
 // PAPER.md L133 (III-B step 3): "we sort an array of the pair of a key and a particle's id".
-// The paper used a host parallel quicksort; here it is an 8-bit-digit stable LSD radix sort
-// (stable + ids initially ascending = ties broken by original index, reading R4).
+// The paper used a host parallel quicksort; here it is an 8-bit-digit stable LSD radix sort in the
+// one-sweep form (stable + ids initially ascending = ties broken by original index, reading R4).
 #include "common.cuh"
 
 namespace {
@@ -17,41 +17,78 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   return m;
 }
 
-// per-CTA digit histogram -> hist[d * nb + b]
-__global__ void __launch_bounds__(SORT_THREADS) radix_hist_kernel(const uint64_t* __restrict__ keys, int64_t n,
-                                                                  int shift, uint32_t* __restrict__ hist, int nb) {
-  __shared__ uint32_t sh[256];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  sh[tid] = 0;
+// ---------------- one-sweep passes: global digit histograms up front, then one kernel per digit whose
+// tiles find their global offsets by decoupled look-back (no per-pass histogram/scan kernels, 12 B read
+// + 12 B written per pair and pass), keys ranked in the tile and staged through shared memory so that the
+// global writes are runs of consecutive addresses.
+constexpr int OS_MAXPASS = 8;
+constexpr uint32_t OS_GHIST = 0;                       // u32 offsets into ctx->hist
+constexpr uint32_t OS_TICKET = OS_MAXPASS * 256;       // one tile ticket counter per pass
+constexpr uint32_t OS_STATUS = OS_TICKET + 256;        // u64 status words [tile][digit] from here (8 B aligned)
+constexpr size_t OS_SMEM = SORT_TILE * 12 + SORT_WARPS * 256 * 4 + 2 * 256 * 4 + 16;
+
+// all digit histograms of the key bits [first_bit, first_bit + 8 * npass) in one read of the keys
+__global__ void __launch_bounds__(SORT_THREADS) radix_hist_all_kernel(const uint64_t* __restrict__ keys, int64_t n,
+                                                                      int first_bit, int npass,
+                                                                      uint32_t* __restrict__ ghist) {
+  __shared__ uint32_t sh[OS_MAXPASS][256];
+  const int tid = threadIdx.x;
+  for (int p = 0; p < npass; p++) sh[p][tid] = 0;
   __syncthreads();
-  const int64_t base = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS);
-#pragma unroll 4
-  for (int i = 0; i < SORT_ITEMS; i++) {
-    int64_t idx = base + i * 32 + lane;
-    unsigned d = 0xFFFFFFFFu;
-    if (idx < n) d = (unsigned)((keys[idx] >> shift) & 0xFF);
-    unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-    if (d != 0xFFFFFFFFu && (peers & lanemask_lt()) == 0) atomicAdd(&sh[d], __popc(peers));
+  for (int64_t i = (int64_t)blockIdx.x * SORT_THREADS + tid; i < n; i += (int64_t)gridDim.x * SORT_THREADS) {
+    const uint64_t k = keys[i] >> first_bit;
+    for (int p = 0; p < npass; p++) atomicAdd(&sh[p][(unsigned)(k >> (8 * p)) & 0xFF], 1u);
   }
   __syncthreads();
-  hist[(size_t)tid * nb + blockIdx.x] = sh[tid];
+  for (int p = 0; p < npass; p++) if (sh[p][tid]) atomicAdd(&ghist[p * 256 + tid], sh[p][tid]);
+}
+// counts -> exclusive digit offsets, one block per pass
+__global__ void __launch_bounds__(256) radix_hist_scan_kernel(uint32_t* __restrict__ ghist) {
+  __shared__ uint32_t sh[256];
+  uint32_t* h = ghist + blockIdx.x * 256;
+  const int tid = threadIdx.x;
+  const uint32_t c = h[tid];
+  sh[tid] = c;
+  __syncthreads();
+  for (int o = 1; o < 256; o <<= 1) {
+    uint32_t y = tid >= o ? sh[tid - o] : 0;
+    __syncthreads();
+    sh[tid] += y;
+    __syncthreads();
+  }
+  h[tid] = sh[tid] - c;
 }
 
-// stable scatter of one digit
-__global__ void __launch_bounds__(SORT_THREADS) radix_scatter_kernel(const uint64_t* __restrict__ kin,
+// status word: [63:34] epoch of the pass, [33:32] 1 = tile aggregate, 2 = inclusive prefix, [31:0] count
+__device__ __forceinline__ unsigned long long os_pack(uint32_t epoch, uint32_t state, uint32_t v) {
+  return ((unsigned long long)((epoch << 2) | state) << 32) | v;
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const uint64_t* __restrict__ kin,
                                                                      const uint32_t* __restrict__ vin,
                                                                      uint64_t* __restrict__ kout,
                                                                      uint32_t* __restrict__ vout, int64_t n, int shift,
-                                                                     const uint32_t* __restrict__ offs, int nb) {
-  __shared__ uint32_t whist[SORT_WARPS][256];
+                                                                     const uint32_t* __restrict__ gbase,
+                                                                     unsigned long long* status, uint32_t* ticket,
+                                                                     uint32_t epoch) {
+  extern __shared__ __align__(16) unsigned char os_smem[];
+  uint64_t* skey = reinterpret_cast<uint64_t*>(os_smem);
+  uint32_t* sval = reinterpret_cast<uint32_t*>(os_smem + SORT_TILE * 8);
+  uint32_t(*whist)[256] = reinterpret_cast<uint32_t(*)[256]>(os_smem + SORT_TILE * 12);
+  uint32_t* dstart = reinterpret_cast<uint32_t*>(os_smem + SORT_TILE * 12 + SORT_WARPS * 256 * 4);
+  uint32_t* goff = dstart + 256;
+  uint32_t* stile = goff + 256;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) *stile = atomicAdd(ticket, 1u);      // tiles are numbered in starting order: look-back cannot hang
 #pragma unroll
   for (int w = 0; w < SORT_WARPS; w++) whist[w][tid] = 0;
   __syncthreads();
-  const int64_t base = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS);
+  const uint32_t tile = *stile;
+  const int64_t tbase = (int64_t)tile * SORT_TILE;
+  const int64_t base = tbase + warp * (32 * SORT_ITEMS);
   uint64_t k[SORT_ITEMS];
   uint32_t v[SORT_ITEMS];
-  uint32_t rk[SORT_ITEMS];  // rank within the warp's chunk among equal digits
+  uint32_t rk[SORT_ITEMS];  // rank among equal digits within the warp's chunk, in index order (stable)
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; i++) {
     int64_t idx = base + i * 32 + lane;
@@ -60,11 +97,10 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_scatter_kernel(const uint6
   }
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; i++) {
-    int64_t idx = base + i * 32 + lane;
-    bool valid = idx < n;
-    unsigned d = valid ? (unsigned)((k[i] >> shift) & 0xFF) : 0xFFFFFFFFu;
-    unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-    int leader = __ffs(peers) - 1;
+    const bool valid = base + i * 32 + lane < n;
+    const unsigned d = valid ? (unsigned)((k[i] >> shift) & 0xFF) : 0xFFFFFFFFu;
+    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+    const int leader = __ffs(peers) - 1;
     uint32_t b = 0;
     if (valid && lane == leader) { b = whist[warp][d]; whist[warp][d] = b + __popc(peers); }
     b = __shfl_sync(0xFFFFFFFFu, b, leader);
@@ -72,21 +108,52 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_scatter_kernel(const uint6
     __syncwarp();
   }
   __syncthreads();
-  {  // digit `tid`: global offset of this CTA, then exclusive prefix over the warps
-    uint32_t run = offs[(size_t)tid * nb + blockIdx.x];
+  // digit `tid`: exclusive prefix over the warps, tile count, look-back over the preceding tiles
+  uint32_t cnt = 0;
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; w++) { uint32_t c = whist[w][tid]; whist[w][tid] = run; run += c; }
+  for (int w = 0; w < SORT_WARPS; w++) { uint32_t c = whist[w][tid]; whist[w][tid] = cnt; cnt += c; }
+  volatile unsigned long long* st = status + (size_t)tile * 256 + tid;
+  *st = os_pack(epoch, tile == 0 ? 2u : 1u, cnt);
+  dstart[tid] = cnt;
+  __syncthreads();
+  for (int o = 1; o < 256; o <<= 1) {                 // inclusive scan of the tile's digit counts
+    uint32_t y = tid >= o ? dstart[tid - o] : 0;
+    __syncthreads();
+    dstart[tid] += y;
+    __syncthreads();
   }
+  const uint32_t my_start = dstart[tid] - cnt;
+  uint32_t excl = 0;
+  if (tile > 0) {
+    for (int64_t t = (int64_t)tile - 1; t >= 0; t--) {
+      const volatile unsigned long long* ps = status + (size_t)t * 256 + tid;
+      unsigned long long w;
+      do { w = *ps; } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0u);
+      excl += (uint32_t)w;
+      if (((w >> 32) & 3u) == 2u) break;
+    }
+    *st = os_pack(epoch, 2u, excl + cnt);
+  }
+  __syncthreads();
+  dstart[tid] = my_start;
+  goff[tid] = gbase[tid] + excl - my_start;           // global slot = goff[digit] + position in the sorted tile
   __syncthreads();
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; i++) {
-    int64_t idx = base + i * 32 + lane;
-    if (idx < n) {
-      unsigned d = (unsigned)((k[i] >> shift) & 0xFF);
-      uint32_t dst = whist[warp][d] + rk[i];
-      kout[dst] = k[i];
-      vout[dst] = v[i];
+    if (base + i * 32 + lane < n) {
+      const unsigned d = (unsigned)((k[i] >> shift) & 0xFF);
+      const uint32_t pos = dstart[d] + whist[warp][d] + rk[i];
+      skey[pos] = k[i];
+      sval[pos] = v[i];
     }
+  }
+  __syncthreads();
+  const int cnt_tile = (int)((n - tbase) < SORT_TILE ? (n - tbase) : SORT_TILE);
+  for (int j = tid; j < cnt_tile; j += SORT_THREADS) {
+    const uint64_t key = skey[j];
+    const uint32_t dst = goff[(unsigned)((key >> shift) & 0xFF)] + (uint32_t)j;
+    kout[dst] = key;
+    vout[dst] = sval[j];
   }
 }
 
@@ -169,20 +236,34 @@ otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, ui
   return OTOO_OK;
 }
 
-// Sort n pairs on bits [first_bit, end_bit) in 8-bit digits. Input in buffer 0; *result_buf tells
-// which buffer holds the result.  Uses ctx->hist and ctx->scan_tmp.
+// Sort n pairs on bits [first_bit, end_bit) in 8-bit digits (stable).  Input in buffer 0; *result_buf
+// tells which buffer holds the result.  Uses ctx->hist (digit histograms, tile tickets, look-back status).
 otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n, int first_bit,
                             int end_bit, cudaStream_t st, int* result_buf) {
   int cur = 0;
   if (n > 0) {
-    int nb = (int)cdiv(n, SORT_TILE);
-    if ((size_t)nb * 256 > ctx->hist_cap) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "sort histogram scratch too small");
-    for (int shift = first_bit; shift < end_bit; shift += 8) {
-      radix_hist_kernel<<<nb, SORT_THREADS, 0, st>>>(key[cur], n, shift, ctx->hist, nb);
-      ctx->launches += 1;
-      OTOO_TRY(otoo_exclusive_scan_u32(ctx, ctx->hist, (int64_t)nb * 256, nullptr, st));
-      radix_scatter_kernel<<<nb, SORT_THREADS, 0, st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, shift,
-                                                        ctx->hist, nb);
+    const int nb = (int)cdiv(n, SORT_TILE);
+    const int npass = (end_bit - first_bit + 7) / 8;
+    if (npass > OS_MAXPASS || OS_STATUS + (size_t)nb * 512 > ctx->hist_cap)
+      return otoo_fail(ctx, OTOO_ERR_CAPACITY, "sort scratch too small");
+    if (!ctx->sort_attr_set) {
+      OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_SMEM));
+      ctx->sort_attr_set = true;
+    }
+    if (ctx->sort_epoch + (uint32_t)npass >= (1u << 30)) {      // epochs exhausted: clear the status words, restart
+      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t), st));
+      ctx->sort_epoch = 0;
+    }
+    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
+    int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
+    radix_hist_all_kernel<<<gh, SORT_THREADS, 0, st>>>(key[0], n, first_bit, npass, ctx->hist + OS_GHIST);
+    radix_hist_scan_kernel<<<npass, 256, 0, st>>>(ctx->hist + OS_GHIST);
+    ctx->launches += 2;
+    unsigned long long* status = reinterpret_cast<unsigned long long*>(ctx->hist + OS_STATUS);
+    for (int p = 0; p < npass; p++) {
+      onesweep_pass_kernel<<<nb, SORT_THREADS, OS_SMEM, st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n,
+                                                              first_bit + 8 * p, ctx->hist + OS_GHIST + p * 256, status,
+                                                              ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
       ctx->launches += 1;
       cur ^= 1;
     }

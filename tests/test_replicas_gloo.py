@@ -1,0 +1,63 @@
+"""The N>1 path of bench.py on CPU: world_size 2 over gloo.  Replicas only:
+the exchange is max-over-ranks time and sum-over-ranks interactions, nothing on the data path."""
+import importlib.util
+import os
+import socket
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist  # noqa: E402
+import torch.multiprocessing as mp  # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _load_replicas():
+    # by path: importing the package would load libotoo.so, which this test does not need
+    spec = importlib.util.spec_from_file_location("replicas", os.path.join(ROOT, "paper_1206_1199_b200", "replicas.py"))
+    m = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(m)
+    return m
+
+
+def _worker(rank, world, port, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    rep = _load_replicas()
+    ms_local = [4.0, 5.5][rank]           # rank 1 is the slow one
+    units_local = [7.0e9, 7.5e9][rank]
+    ms, units = rep.aggregate(ms_local, units_local)
+    val = rep.throughput(ms_local, units_local)
+    dist.barrier()
+    q.put((rank, ms, units, val, rep.replica_seed(1206, rank)))
+    dist.destroy_process_group()
+
+
+def test_replica_aggregation_world2():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, units, val, seed in res:
+        assert ms == 5.5 and units == 14.5e9
+        assert val == pytest.approx(14.5e9 / 5.5e-3)
+        assert seed == 1206 + rank
+    assert res[0][4] != res[1][4]
+
+
+def test_aggregate_without_process_group():
+    rep = _load_replicas()
+    assert rep.aggregate(3.0, 10.0) == (3.0, 10.0)
+    assert rep.throughput(2.0, 10.0) == pytest.approx(5000.0)
