@@ -90,7 +90,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     for (int b = 0; b < 2; b++) { OTOO_TRY(dalloc(ctx, &ctx->key[b], n)); OTOO_TRY(dalloc(ctx, &ctx->val[b], n)); }
     OTOO_TRY(dalloc(ctx, &ctx->spos, n));
     OTOO_TRY(dalloc(ctx, &ctx->slot_nc, n));
-    ctx->hist_cap = (size_t)cdiv(max_particles, 4096) * 512 + 4096;   // look-back status (u64 per tile and digit) + histograms
+    ctx->hist_cap = OTOO_SORT_SCRATCH(max_particles);   // look-back status (u64 per tile and digit) + histograms
     OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
     OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t)));
     OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));

@@ -6,6 +6,8 @@
 //   cpl(s) = common prefix levels of key[s-1], key[s] and D(s) = max over windows of n_crit+1
 //   consecutive slots containing s of their common prefix levels.
 #include "common.cuh"
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -33,11 +35,17 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4* __restrict__ po
       lo[k] = fminf(lo[k], __shfl_xor_sync(0xFFFFFFFFu, lo[k], o));
       hi[k] = fmaxf(hi[k], __shfl_xor_sync(0xFFFFFFFFu, hi[k], o));
     }
-  if ((threadIdx.x & 31) == 0) {
-#pragma unroll
-    for (int k = 0; k < 3; k++) { atomicMin(&bbox[k], f2ord(lo[k])); atomicMax(&bbox[3 + k], f2ord(hi[k])); }
+  __shared__ float sh[8][6];                          // one partial per warp, then 6 atomics per CTA
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { for (int k = 0; k < 3; k++) { sh[warp][k] = lo[k]; sh[warp][3 + k] = hi[k]; } }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    float v = sh[0][threadIdx.x];
+    for (int w = 1; w < 8; w++) v = threadIdx.x < 3 ? fminf(v, sh[w][threadIdx.x]) : fmaxf(v, sh[w][threadIdx.x]);
+    if (threadIdx.x < 3) atomicMin(&bbox[threadIdx.x], f2ord(v)); else atomicMax(&bbox[threadIdx.x], f2ord(v));
   }
 }
+
 // root cube: floats at bbox[8..12] = lo.xyz, S, scale
 __global__ void root_kernel(unsigned* bbox) {
   float* out = reinterpret_cast<float*>(bbox) + 8;
@@ -180,26 +188,34 @@ __global__ void __launch_bounds__(256) cell_topology_kernel(const uint64_t* __re
 }
 
 // H6 (L155; R6, R7): one level of the bottom-up pass; fp64, fixed summation order.
-__global__ void __launch_bounds__(128) moments_kernel(uint32_t c0, uint32_t c1, int level, const float4* __restrict__ spos,
-                                                      const uint64_t* __restrict__ key, const uint32_t* __restrict__ c_first,
-                                                      const uint32_t* __restrict__ c_count,
-                                                      const uint32_t* __restrict__ c_child_first,
-                                                      const uint8_t* __restrict__ c_child_count, const unsigned* __restrict__ bbox,
-                                                      double* __restrict__ MP, double* __restrict__ cm64,
-                                                      float4* __restrict__ cell_cm, double* __restrict__ c_s) {
-  uint32_t c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= c1) return;
+struct MomentArgs {
+  const float4* spos; const uint64_t* key; const uint32_t* c_first; const uint32_t* c_count;
+  const uint32_t* c_child_first; const uint8_t* c_child_count; const unsigned* bbox;
+  double* MP; double* cm64; float4* cell_cm; double* c_s;
+};
+__device__ __forceinline__ void moments_cell(uint32_t c, int level, const MomentArgs& a) {
+  const float4* __restrict__ spos = a.spos; const uint64_t* __restrict__ key = a.key;
+  const uint32_t* __restrict__ c_first = a.c_first; const uint32_t* __restrict__ c_count = a.c_count;
+  const uint32_t* __restrict__ c_child_first = a.c_child_first; const uint8_t* __restrict__ c_child_count = a.c_child_count;
+  const unsigned* __restrict__ bbox = a.bbox;
+  double* MP = a.MP; double* cm64 = a.cm64; float4* cell_cm = a.cell_cm; double* c_s = a.c_s;
   uint32_t first = c_first[c], count = c_count[c];
   int nch = c_child_count[c];
   double M = 0.0, Px = 0.0, Py = 0.0, Pz = 0.0;
   if (nch == 0) {
-    for (uint32_t s = first; s < first + count; s++) {
-      float4 p = spos[s];
-      double m = (double)p.w;
-      M = __dadd_rn(M, m);
-      Px = __dadd_rn(Px, __dmul_rn(m, (double)p.x));
-      Py = __dadd_rn(Py, __dmul_rn(m, (double)p.y));
-      Pz = __dadd_rn(Pz, __dmul_rn(m, (double)p.z));
+    for (uint32_t s0 = first; s0 < first + count; s0 += 8) {   // 8 loads in flight, sums in slot order (R6)
+      float4 p[8];
+      const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) p[j] = spos[s0 + j];
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) {
+        double m = (double)p[j].w;
+        M = __dadd_rn(M, m);
+        Px = __dadd_rn(Px, __dmul_rn(m, (double)p[j].x));
+        Py = __dadd_rn(Py, __dmul_rn(m, (double)p[j].y));
+        Pz = __dadd_rn(Pz, __dmul_rn(m, (double)p[j].z));
+      }
     }
   } else {
     uint32_t ch = c_child_first[c];
@@ -224,6 +240,16 @@ __global__ void __launch_bounds__(128) moments_kernel(uint32_t c0, uint32_t c1, 
   cell_cm[c] = make_float4(__double2float_rn(cx), __double2float_rn(cy), __double2float_rn(cz), __double2float_rn(M));
   double dx = __dsub_rn(cx, g[0]), dy = __dsub_rn(cy, g[1]), dz = __dsub_rn(cz, g[2]);
   c_s[c] = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+}
+// the whole bottom-up pass in ONE cooperative launch: every level deepest first, a grid-wide barrier
+// between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
+__global__ void __launch_bounds__(256) moments_all_kernel(const LevelOff off, const int depth, const MomentArgs a) {
+  cg::grid_group grid = cg::this_grid();
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+  for (int l = depth; l >= 0; l--) {
+    for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) moments_cell(c, l, a);
+    if (l > 0) grid.sync();
+  }
 }
 
 template <typename T>
@@ -251,7 +277,7 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
   OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
   for (int b = 0; b < 2; b++) { OTOO_TRY(grow(ctx, &ctx->tmp_key[b], cap)); OTOO_TRY(grow(ctx, &ctx->tmp_val[b], cap)); }
-  size_t need = (size_t)cdiv(cap, 4096) * 512 + 4096;
+  size_t need = OTOO_SORT_SCRATCH(cap);
   if (need > ctx->hist_cap) {
     OTOO_TRY(grow(ctx, &ctx->hist, need));
     ctx->hist_cap = need;
@@ -273,7 +299,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_CUDA(ctx, cudaMemsetAsync(bbox, 0xFF, 12, st));      // min = 0xFFFFFFFF
   OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 12, st));  // max = 0
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 64 * sizeof(uint32_t), st));
-  int gb = ctx->sm_count * 8; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
+  int gb = ctx->sm_count * 4; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
   root_kernel<<<1, 1, 0, st>>>(bbox);
   // H2, H3, H4
@@ -308,12 +334,19 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
                                             ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);
   ctx->launches += 1;
   // H6 deepest level first
-  for (int l = depth; l >= 0; l--) {
-    uint32_t c0 = off.v[l], c1 = off.v[l + 1];
-    if (c1 == c0) continue;
-    moments_kernel<<<(unsigned)cdiv(c1 - c0, 128), 128, 0, st>>>(c0, c1, l, ctx->spos, ctx->key[0], ctx->c_first,
-                                                                 ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                                                                 bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s);
+  const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s};
+  {
+    int occ = 1;
+    OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));
+    if (occ > 4) occ = 4;
+    int64_t grid = (int64_t)ctx->sm_count * (occ < 1 ? 1 : occ);
+    uint32_t widest = 1;
+    for (int l = 0; l <= depth; l++) if (off.v[l + 1] - off.v[l] > widest) widest = off.v[l + 1] - off.v[l];
+    if (grid > cdiv(widest, 256)) grid = cdiv(widest, 256);
+    int depth_arg = depth;
+    void* args[] = {(void*)&off, (void*)&depth_arg, (void*)&ma};
+    OTOO_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)moments_all_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
     ctx->launches += 1;
   }
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 32, ctx->d_counters + 32, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));

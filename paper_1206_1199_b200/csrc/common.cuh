@@ -12,6 +12,11 @@
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
 #define OTOO_LIST_CAP 256            // smem interaction-list float4 per warp (small: leaves the SM's L1 for the tree)
 #define OTOO_LIST_STRIDE (OTOO_LIST_CAP + 4)  // per-warp list buffer incl. slack (gravity's pipelined loop reads one entry ahead)
+#ifndef OTOO_SORT_TILE
+#define OTOO_SORT_TILE 4096            // pairs per CTA of a radix pass (256 threads x 16; 1024 and 2048 measured slower)
+#endif
+// u32 words of sort scratch for n pairs: digit histograms + tickets (4096) + one u64 status word per tile and digit
+#define OTOO_SORT_SCRATCH(n) ((size_t)(((n) + OTOO_SORT_TILE - 1) / OTOO_SORT_TILE) * 512 + 4096)
 #define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
 
 // Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).

@@ -7,8 +7,8 @@
 namespace {
 
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS = 16;
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;  // 4096 keys per CTA
+constexpr int SORT_TILE = OTOO_SORT_TILE;             // pairs per CTA
+constexpr int SORT_ITEMS = SORT_TILE / SORT_THREADS;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 
 __device__ __forceinline__ unsigned lanemask_lt() {
@@ -112,6 +112,7 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const uint6
   uint32_t cnt = 0;
 #pragma unroll
   for (int w = 0; w < SORT_WARPS; w++) { uint32_t c = whist[w][tid]; whist[w][tid] = cnt; cnt += c; }
+  const volatile unsigned long long* status_v = status;
   volatile unsigned long long* st = status + (size_t)tile * 256 + tid;
   *st = os_pack(epoch, tile == 0 ? 2u : 1u, cnt);
   dstart[tid] = cnt;
@@ -125,12 +126,28 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const uint6
   const uint32_t my_start = dstart[tid] - cnt;
   uint32_t excl = 0;
   if (tile > 0) {
-    for (int64_t t = (int64_t)tile - 1; t >= 0; t--) {
-      const volatile unsigned long long* ps = status + (size_t)t * 256 + tid;
-      unsigned long long w;
-      do { w = *ps; } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0u);
-      excl += (uint32_t)w;
-      if (((w >> 32) & 3u) == 2u) break;
+    // look back over the preceding tiles, 8 status words in flight at a time (when all tiles of a small
+    // sort run in one wave the walk is long, and one L2 round trip per tile would dominate the pass)
+    int64_t t = (int64_t)tile - 1;
+    bool done = false;
+    while (!done) {
+      unsigned long long w[8];
+#pragma unroll
+      for (int j = 0; j < 8; j++)
+        w[j] = t - j >= 0 ? *(status_v + (size_t)(t - j) * 256 + tid) : os_pack(epoch, 2u, 0u);
+      int used = 0;
+#pragma unroll
+      for (int j = 0; j < 8; j++) {
+        if (!done && used == j) {
+          const uint32_t state = (uint32_t)(w[j] >> 32) & 3u;
+          if ((uint32_t)(w[j] >> 34) == epoch && state != 0u) {
+            excl += (uint32_t)w[j];
+            used = j + 1;
+            done = state == 2u;
+          }
+        }
+      }
+      t -= used;
     }
     *st = os_pack(epoch, 2u, excl + cnt);
   }
@@ -244,7 +261,7 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
   if (n > 0) {
     const int nb = (int)cdiv(n, SORT_TILE);
     const int npass = (end_bit - first_bit + 7) / 8;
-    if (npass > OS_MAXPASS || OS_STATUS + (size_t)nb * 512 > ctx->hist_cap)
+    if (npass > OS_MAXPASS || OTOO_SORT_SCRATCH(n) > ctx->hist_cap)
       return otoo_fail(ctx, OTOO_ERR_CAPACITY, "sort scratch too small");
     if (!ctx->sort_attr_set) {
       OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_SMEM));
