@@ -11,7 +11,7 @@
 #define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
 #define OTOO_LIST_CAP 256            // smem interaction-list float4 per warp (small: leaves the SM's L1 for the tree)
-#define OTOO_LIST_STRIDE (OTOO_LIST_CAP + 4)  // per-warp list buffer incl. slack (gravity's pipelined loop reads one entry ahead)
+#define OTOO_LIST_STRIDE (OTOO_LIST_CAP + 4)  // per-warp list buffer (+4: consecutive warps start on different banks)
 #ifndef OTOO_SORT_TILE
 #define OTOO_SORT_TILE 4096            // pairs per CTA of a radix pass (256 threads x 16; 1024 and 2048 measured slower)
 #endif

@@ -100,9 +100,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   float4* list = list0;
 
   for (;;) {
-    // ---------------- acquire a unit of work: the next group of the main queue, else a pool task
-    // (polling the pool before the queue was tried: 1776 warps contending for the head word with CAS
-    // cost more than it gained)
+    // ---------------- acquire a unit of work
     uint32_t g = 0; int sp = 0;
     bool got = false;
     auto take = [&](uint32_t ticket) {   // copy task `ticket` (already published) to the shared stack
@@ -114,6 +112,8 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       __syncwarp();
       if (lane == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(&c.seq[slot]) = ticket + OTOO_POOL_SLOTS; }
     };
+    // (taking pending pool tasks before new groups was tried twice -- CAS claims: every warp retrying on
+    // one word; unconditional claims: overshooting warps wait -- and lost 3-5 %: the pool is drained at the end)
     if (!got && !main_done) {
       if (lane == 0) g = atomicAdd(&c.ws->queue, 1u);
       g = __shfl_sync(0xFFFFFFFFu, g, 0);

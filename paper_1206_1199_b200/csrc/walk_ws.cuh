@@ -23,7 +23,7 @@ struct WsMeta { uint32_t count, flags, group, pad; };
 // shared memory of one pair; NT = float2 words of target staging (32 lanes x NP x 3)
 template <int NT>
 struct __align__(16) WsPair {
-  float4 list[OTOO_WS_NBUF][OTOO_WS_LCAP + 4];   // + slack: the pipelined sum loop reads one entry ahead
+  float4 list[OTOO_WS_NBUF][OTOO_WS_LCAP + 4];   // +4 entries: consecutive buffers start on different banks
   float2 tgt[NT];
   uint32_t stk[OTOO_WALK_STACK_MAX];
   uint32_t self[OTOO_WS_NBUF][32];
