@@ -58,6 +58,12 @@ def lib():
         L.orc_direct_sum.argtypes = [i64, vp, dbl, i64, vp, vp]
         L.orc_gravity.restype = C.c_uint64
         L.orc_gravity.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, vp, vp, vp, vp]
+        L.orc_delta_cell_props.argtypes = [vp, vp, vp]
+        L.orc_B2_direct.restype = dbl
+        L.orc_B2_direct.argtypes = [vp, i64]
+        L.orc_rb2_delta.argtypes = [vp, dbl, dbl, vp]
+        L.orc_gravity_rb2.restype = C.c_uint64
+        L.orc_gravity_rb2.argtypes = [vp, dbl, vp, i32, i32, vp, i64, vp, vp, vp, vp, vp]
         L.orc_gravity_sel.restype = C.c_uint64
         L.orc_gravity_sel.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, i64, vp, vp, vp, vp, vp]
         L.orc_sph_density_sel.restype = C.c_uint64
@@ -65,6 +71,7 @@ def lib():
         L.orc_sph_force_sel.restype = C.c_uint64
         L.orc_sph_force_sel.argtypes = [vp, vp, vp, vp, vp, i32, vp, i64, vp, vp]
         L.orc_group_lists.argtypes = [vp, dbl, i32, i32, i64, vp, vp]
+        L.orc_group_lists_rb2.argtypes = [vp, vp, i32, i64, vp, vp]
         L.orc_sph_cell_radii.argtypes = [vp, vp, vp, vp]
         L.orc_sph_density.restype = C.c_uint64
         L.orc_sph_density.argtypes = [vp, vp, i32, vp, vp, vp, vp]
@@ -164,10 +171,26 @@ class Tree:
         lib().orc_rb2(self._h, float(theta), int(mac_kind), _p(out))
         return out
 
+    def delta_cell_props(self):
+        """(B2, b_max) per cell in fp64: PAPER.md Eq. 2 (bottom-up, reading R19) and L63."""
+        B2 = np.empty(self.ncell, dtype=np.float64)
+        bm = np.empty(self.ncell, dtype=np.float64)
+        lib().orc_delta_cell_props(self._h, _p(B2), _p(bm))
+        return B2, bm
+
+    def B2_direct(self, cell):
+        return lib().orc_B2_direct(self._h, int(cell))
+
+    def rb2_delta(self, delta, m_limit=np.inf):
+        """rb^2 (fp32) of the paper's absolute-error MAC, Eq. 1, with the m_limit rule of L157."""
+        out = np.empty(self.ncell, dtype=np.float32)
+        lib().orc_rb2_delta(self._h, float(delta), float(m_limit), _p(out))
+        return out
+
     def n_groups(self, G):
         return (self.N + G - 1) // G
 
-    def gravity(self, eps, theta, group_size, mac_kind=0, walk_kind=0, forces=True, groups=None):
+    def gravity(self, eps, theta, group_size, mac_kind=0, walk_kind=0, forces=True, groups=None, rb2=None):
         """groups: optional array of group indices; then only those are walked, the counters are indexed
         by position in `groups`, and acc_pot / abs_sum (still N rows) are filled for their targets only."""
         sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
@@ -177,9 +200,15 @@ class Tree:
         nc = np.zeros(ng, dtype=np.uint32)
         npart = np.zeros(ng, dtype=np.uint32)
         asum = np.zeros(self.N, dtype=np.float64) if forces else None
-        tot = lib().orc_gravity_sel(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
-                                    int(walk_kind), _p(sel), 0 if sel is None else len(sel),
-                                    _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
+        if rb2 is not None:       # any MAC of the form "accept iff d > r_b": theta is ignored
+            rb2 = np.ascontiguousarray(rb2, dtype=np.float32)
+            assert rb2.shape == (self.ncell,)
+            tot = lib().orc_gravity_rb2(self._h, float(eps), _p(rb2), int(group_size), int(walk_kind), _p(sel),
+                                        0 if sel is None else len(sel), _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
+        else:
+            tot = lib().orc_gravity_sel(self._h, float(eps), float(theta), int(group_size), int(mac_kind),
+                                        int(walk_kind), _p(sel), 0 if sel is None else len(sel),
+                                        _p(acc), _p(nt), _p(nc), _p(npart), _p(asum))
         return dict(acc_pot=acc, n_tests=nt, n_cells=nc, n_parts=npart, interactions=int(tot), abs_sum=asum)
 
     def group_targets(self, group_size, groups):
@@ -192,10 +221,18 @@ class Tree:
         return np.concatenate(out).astype(np.int64)
 
     def group_lists(self, theta, group_size, g, n_cells, n_parts, mac_kind=0):
+        """theta-MAC lists of one group (for other MACs use group_lists_rb2)"""
         cells = np.empty(max(int(n_cells), 1), dtype=np.uint32)
         parts = np.empty(max(int(n_parts), 1), dtype=np.uint32)
         lib().orc_group_lists(self._h, float(theta), int(group_size), int(mac_kind), int(g),
                               _p(cells), _p(parts))
+        return cells[:int(n_cells)], parts[:int(n_parts)]
+
+    def group_lists_rb2(self, rb2, group_size, g, n_cells, n_parts):
+        rb2 = np.ascontiguousarray(rb2, dtype=np.float32)
+        cells = np.empty(max(int(n_cells), 1), dtype=np.uint32)
+        parts = np.empty(max(int(n_parts), 1), dtype=np.uint32)
+        lib().orc_group_lists_rb2(self._h, _p(rb2), int(group_size), int(g), _p(cells), _p(parts))
         return cells[:int(n_cells)], parts[:int(n_parts)]
 
     def sph_cell_radii(self, h):

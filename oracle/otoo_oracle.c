@@ -276,6 +276,78 @@ void orc_rb2(const orc_tree* t, double theta, int mac_kind, float* rb2) {
   }
 }
 
+/* ---------------- the paper's own MAC: absolute-error criterion (PAPER II-B Eq. 1-2; III-C L157)
+ * B2 (Eq. 2) = sum over the cell's particles of m |r_CM - r|^2.  Reading R19: like mass and
+ * centre of mass (R6) it is accumulated bottom-up in a fixed order so that it is reproducible bit for bit:
+ * leaf: sequentially over its particles in sorted order; internal cell: over its children in octant order
+ * with the parallel-axis theorem, B2 += B2_child, then B2 += M_child |CM_child - CM|^2.  orc_B2_direct is
+ * Eq. 2 written out (the pin).  b_max = max over ALL particles of the cell of |r - CM| (fp64, L63). */
+void orc_delta_cell_props(const orc_tree* t, double* B2, double* bmax) {
+  for (int64_t id = t->ncell - 1; id >= 0; id--) {   /* canonical ids: children come after their parent */
+    const orc_cell* c = &t->cell[id];
+    const double* cm = t->cm + 3 * id;
+    double b2 = 0.0;
+    if (c->child_count == 0) {
+      for (uint32_t s = c->first; s < c->first + c->count; s++) {
+        const float* p = t->spos + 4 * (int64_t)s;
+        double dx = (double)p[0] - cm[0], dy = (double)p[1] - cm[1], dz = (double)p[2] - cm[2];
+        double r2 = (dx * dx + dy * dy) + dz * dz;
+        b2 = b2 + (double)p[3] * r2;
+      }
+    } else {
+      for (int k = 0; k < c->child_count; k++) {
+        int64_t ch = (int64_t)c->child_first + k;
+        const double* cc = t->cm + 3 * ch;
+        double dx = cc[0] - cm[0], dy = cc[1] - cm[1], dz = cc[2] - cm[2];
+        double r2 = (dx * dx + dy * dy) + dz * dz;
+        b2 = b2 + B2[ch];
+        b2 = b2 + t->MP[4 * ch] * r2;
+      }
+    }
+    B2[id] = b2;
+    if (bmax) {
+      double b = 0.0;
+      for (uint32_t s = c->first; s < c->first + c->count; s++) {
+        const float* p = t->spos + 4 * (int64_t)s;
+        double dx = (double)p[0] - cm[0], dy = (double)p[1] - cm[1], dz = (double)p[2] - cm[2];
+        double r = sqrt((dx * dx + dy * dy) + dz * dz);
+        if (r > b) b = r;
+      }
+      bmax[id] = b;
+    }
+  }
+}
+double orc_B2_direct(const orc_tree* t, int64_t id) {   /* Eq. 2 as printed */
+  const orc_cell* c = &t->cell[id];
+  const double* cm = t->cm + 3 * id;
+  double b2 = 0.0;
+  for (uint32_t s = c->first; s < c->first + c->count; s++) {
+    const float* p = t->spos + 4 * (int64_t)s;
+    double dx = cm[0] - (double)p[0], dy = cm[1] - (double)p[1], dz = cm[2] - (double)p[2];
+    b2 += (double)p[3] * (dx * dx + dy * dy + dz * dz);
+  }
+  return b2;
+}
+/* Eq. 1: r_b = b/2 + sqrt(b^2/4 + sqrt(3 B2 / Delta)); cells heavier than m_limit: r_b = 2 S_root (L157);
+ * Delta <= 0: open everything.  rb^2 rounded once to fp32, as for the theta-MAC (R7). */
+void orc_rb2_delta(const orc_tree* t, double delta, double m_limit, float* rb2) {
+  double* B2 = (double*)malloc(8 * t->ncell);
+  double* bm = (double*)malloc(8 * t->ncell);
+  orc_delta_cell_props(t, B2, bm);
+  for (int64_t id = 0; id < t->ncell; id++) {
+    double rb;
+    if (!(delta > 0.0)) { rb2[id] = INFINITY; continue; }
+    if (t->MP[4 * id] > m_limit) rb = 2.0 * (double)t->S;
+    else {
+      double h = 0.5 * bm[id];
+      double q = sqrt((3.0 * B2[id]) / delta);
+      rb = h + sqrt(h * h + q);
+    }
+    rb2[id] = (float)(rb * rb);
+  }
+  free(B2); free(bm);
+}
+
 /* ---------------- R8: group AABB and group-cell distance (L163, Barnes 1990 form) ----------- */
 typedef struct { float lo[3], hi[3]; float hmax; } gbox_t;
 static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs /*sorted h or NULL*/) {
@@ -375,12 +447,10 @@ static void grav_sums(const orc_tree* t, const lists_t* L, int64_t slot, double 
 /* sel != NULL: only the groups sel[0..nsel) are walked (counters indexed by position in sel, sums written
  * for their targets only); the loop over groups is then serial and the targets of a group run in parallel,
  * so that one system-sized group does not serialise the run.  Same arithmetic either way. */
-uint64_t orc_gravity_sel(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
+uint64_t orc_gravity_rb2(const orc_tree* t, double eps, const float* rb2, int G, int walk_kind,
                          const int64_t* sel, int64_t nsel,
                          double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
   int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
-  float* rb2 = (float*)malloc(4 * t->ncell);
-  orc_rb2(t, theta, mac_kind, rb2);
   double e2 = eps * eps;
   uint64_t total = 0;
 #pragma omp parallel reduction(+ : total) if (sel == NULL)
@@ -405,6 +475,14 @@ uint64_t orc_gravity_sel(const orc_tree* t, double eps, double theta, int G, int
     }
     free(L.cells); free(L.parts);
   }
+  return total;
+}
+uint64_t orc_gravity_sel(const orc_tree* t, double eps, double theta, int G, int mac_kind, int walk_kind,
+                         const int64_t* sel, int64_t nsel,
+                         double* acc_pot, uint32_t* n_tests, uint32_t* n_cells, uint32_t* n_parts, double* abs_sum) {
+  float* rb2 = (float*)malloc(4 * t->ncell);
+  orc_rb2(t, theta, mac_kind, rb2);
+  uint64_t total = orc_gravity_rb2(t, eps, rb2, G, walk_kind, sel, nsel, acc_pot, n_tests, n_cells, n_parts, abs_sum);
   free(rb2);
   return total;
 }
@@ -413,17 +491,22 @@ uint64_t orc_gravity(const orc_tree* t, double eps, double theta, int G, int mac
   return orc_gravity_sel(t, eps, theta, G, mac_kind, walk_kind, NULL, 0, acc_pot, n_tests, n_cells, n_parts, abs_sum);
 }
 
-void orc_group_lists(const orc_tree* t, double theta, int G, int mac_kind, int64_t g,
-                     uint32_t* cell_ids, uint32_t* part_slots) {
-  float* rb2 = (float*)malloc(4 * t->ncell);
-  orc_rb2(t, theta, mac_kind, rb2);
+void orc_group_lists_rb2(const orc_tree* t, const float* rb2, int G, int64_t g,
+                         uint32_t* cell_ids, uint32_t* part_slots) {
   int64_t a = g * G, b = a + G < t->N ? a + G : t->N;
   gbox_t box = group_box(t, a, b, NULL);
   lists_t L; memset(&L, 0, sizeof L);
   walk_rec(t, rb2, &box, 0, &L);
   if (cell_ids) memcpy(cell_ids, L.cells, 4 * L.nc);
   if (part_slots) memcpy(part_slots, L.parts, 4 * L.np);
-  free(L.cells); free(L.parts); free(rb2);
+  free(L.cells); free(L.parts);
+}
+void orc_group_lists(const orc_tree* t, double theta, int G, int mac_kind, int64_t g,
+                     uint32_t* cell_ids, uint32_t* part_slots) {
+  float* rb2 = (float*)malloc(4 * t->ncell);
+  orc_rb2(t, theta, mac_kind, rb2);
+  orc_group_lists_rb2(t, rb2, G, g, cell_ids, part_slots);
+  free(rb2);
 }
 
 /* ---------------- SPH (PAPER II-C, L85-L105; readings R13-R17) ------------------------------ */

@@ -14,7 +14,8 @@
  * Pins (tests/test_oracle_*.py): brute-force octants, stable sort, tree invariants, two-particle
  * cell, tiling invariant of the lists, stackless walk == recursive walk,
  * theta=0 == direct sum, Newton's third law, two-body closed form, Plummer potential, kernel
- * normalisation, lattice density, brute-force SPH neighbour sets.
+ * normalisation, lattice density, brute-force SPH neighbour sets; Delta-MAC: two-particle cell and
+ * Eq. 3, B2 bottom-up == Eq. 2 direct, per-cell error <= Delta, r_b limits (L81).
  * parity unpinned: the absolute accuracy level of the theta-MAC (the paper's error plot, Fig. 5,
  * is for its Delta-MAC and is missing from PAPER.md).
  */
@@ -59,6 +60,16 @@ uint64_t orc_key(const orc_tree*, const float xyz[3]);
  * 1: r_b = l/theta. */
 void orc_rb2(const orc_tree*, double theta, int mac_kind, float* rb2 /*ncell*/);
 
+/* The paper's absolute-error MAC (Eq. 1-2; reading R19 for the summation order of B2).
+ * B2, bmax: ncell doubles each (bmax may be NULL). */
+void orc_delta_cell_props(const orc_tree*, double* B2, double* bmax);
+double orc_B2_direct(const orc_tree*, int64_t cell);      /* Eq. 2 written out, for the pin */
+void orc_rb2_delta(const orc_tree*, double delta, double m_limit, float* rb2 /*ncell*/);
+/* Group walk + gravity sums with a given rb^2 per cell (any MAC of the form "accept iff d > r_b", L61). */
+uint64_t orc_gravity_rb2(const orc_tree*, double eps, const float* rb2, int group_size, int walk_kind,
+                         const int64_t* sel, int64_t nsel, double* acc_pot, uint32_t* n_tests,
+                         uint32_t* n_cells, uint32_t* n_parts, double* abs_sum);
+
 /* Group walk + gravity sums.  Outputs in the CALLER's original particle order.
  * walk_kind 0: recursive (R9); 1: stackless next/more exactly as PAPER.md L57.
  * group counters are per group g = sorted slots [gG, min((g+1)G, N)). Pointers may be NULL
@@ -74,6 +85,9 @@ uint64_t orc_gravity_sel(const orc_tree*, double eps, double theta, int group_si
 /* the lists of one group (sizes from orc_gravity counters) */
 void orc_group_lists(const orc_tree*, double theta, int group_size, int mac_kind, int64_t g,
                      uint32_t* cell_ids, uint32_t* part_slots);
+
+void orc_group_lists_rb2(const orc_tree*, const float* rb2, int group_size, int64_t g,
+                         uint32_t* cell_ids, uint32_t* part_slots);
 
 /* SPH.  h = support radius per particle (original order).  */
 void orc_sph_cell_radii(const orc_tree*, const float* h, float* bmax, float* rsph /*ncell each*/);
