@@ -86,6 +86,17 @@ otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
 otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, float* d_acc_pot,
                          void* stream);
 
+/* The same walk and sums under the paper's own acceptance criterion, the absolute-error MAC
+ * (PAPER.md II-B Eq. 1-2): a cell is accepted iff the group-cell distance exceeds
+ *   r_b = b_max/2 + sqrt(b_max^2/4 + sqrt(3 B2 / delta)),  B2 = sum_i m_i |r_CM - r_i|^2  (Eq. 2),
+ * delta = accuracy parameter with the dimension of an acceleration (each accepted cell's monopole is within
+ * delta of the sum over its particles); delta = 0 opens everything (direct sum).  Cells heavier than
+ * m_limit get r_b = 2 S_root and are never accepted (III-C, L157); pass INFINITY for no limit.
+ * B2 is accumulated bottom-up in a fixed order (R19).  Group distance, lists, counters, sums
+ * and output exactly as otoo_gravity.  OTOO_ERR_INVALID_ARG: eps < 0, delta < 0, m_limit <= 0, NaN. */
+otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_limit, int group_size,
+                               float* d_acc_pot, void* stream);
+
 /* PAPER II-C (Eq. 4, Eq. 5) SPH stage 1: density by direct summation during the walk (L99-L105;
  * R13-R16).  d_h: N floats, kernel SUPPORT radius (W = 0 for r >= h, L89), original order.
  * d_rho: N floats out.  d_nngb: N uint32 out (neighbours with r < h_i, self included) or NULL. */

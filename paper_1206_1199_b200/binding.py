@@ -26,7 +26,7 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host"]
+           "otoo_gravity_host", "otoo_gravity_delta"]
 
 
 class TreeInfo(C.Structure):
@@ -53,6 +53,7 @@ _lib.otoo_last_error.argtypes = [_vp]
 _lib.otoo_last_error.restype = C.c_char_p
 _lib.otoo_build_tree.argtypes = [_vp, _vp, _i64, _i32, _vp]
 _lib.otoo_gravity.argtypes = [_vp, _f, _f, _i32, _vp, _vp]
+_lib.otoo_gravity_delta.argtypes = [_vp, _f, _f, _f, _i32, _vp, _vp]
 _lib.otoo_sph_density.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp]
 _lib.otoo_sph_force.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp]
 _lib.otoo_eos_ideal.argtypes = [_vp, _vp, _vp, _f, _i64, _vp, _vp]
@@ -130,6 +131,13 @@ class Otoo:
             out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
         self._check(_lib.otoo_gravity(self._h, float(eps), float(theta), int(group_size),
                                       _ptr(out, torch.float32, 4), _stream(stream)))
+        return out
+
+    def otoo_gravity_delta(self, eps, delta, m_limit, group_size, out=None, stream=None):
+        if out is None:
+            out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
+        self._check(_lib.otoo_gravity_delta(self._h, float(eps), float(delta), float(m_limit), int(group_size),
+                                            _ptr(out, torch.float32, 4), _stream(stream)))
         return out
 
     def otoo_sph_density(self, h, group_size, want_nngb=True, stream=None):

@@ -113,7 +113,7 @@ void otoo_destroy(otoo_ctx* ctx) {
   cudaSetDevice(ctx->device);
   void* ptrs[] = {ctx->key[0], ctx->key[1], ctx->val[0], ctx->val[1], ctx->spos, ctx->slot_nc, ctx->scan_tmp, ctx->hist,
                   ctx->sorted_h, ctx->sorted_aux, ctx->sorted_vel, ctx->cell_cm, ctx->cell_b, ctx->c_first, ctx->c_count,
-                  ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_sph,
+                  ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_B2, ctx->c_sph,
                   ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
                   ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums,
                   ctx->pool_slots, ctx->pool_seq, ctx->walk_shared, ctx->stage_in, ctx->stage_out};
@@ -145,7 +145,20 @@ otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, 
   if (!d_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_acc_pot is NULL");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
   ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
-  return otoo_gravity_impl(ctx, eps, theta, group_size, d_acc_pot, (cudaStream_t)stream);
+  return otoo_gravity_impl(ctx, eps, 0, theta, 0.0f, group_size, d_acc_pot, (cudaStream_t)stream);
+}
+
+otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_limit, int group_size, float* d_acc_pot,
+                               void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!(eps >= 0.0f) || !(delta >= 0.0f) || !(m_limit > 0.0f))
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "eps >= 0, delta >= 0 and m_limit > 0 required");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_acc_pot is NULL");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_gravity_impl(ctx, eps, 1, delta, m_limit, group_size, d_acc_pot, (cudaStream_t)stream);
 }
 
 static otoo_status sph_scratch(otoo_ctx* ctx) {

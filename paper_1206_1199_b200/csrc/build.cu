@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(256) cell_topology_kernel(const uint64_t* __re
 struct MomentArgs {
   const float4* spos; const uint64_t* key; const uint32_t* c_first; const uint32_t* c_count;
   const uint32_t* c_child_first; const uint8_t* c_child_count; const unsigned* bbox;
-  double* MP; double* cm64; float4* cell_cm; double* c_s;
+  double* MP; double* cm64; float4* cell_cm; double* c_s; double* c_B2;
 };
 __device__ __forceinline__ void moments_cell(uint32_t c, int level, const MomentArgs& a) {
   const float4* __restrict__ spos = a.spos; const uint64_t* __restrict__ key = a.key;
@@ -240,6 +240,33 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, const Moment
   cell_cm[c] = make_float4(__double2float_rn(cx), __double2float_rn(cy), __double2float_rn(cz), __double2float_rn(M));
   double dx = __dsub_rn(cx, g[0]), dy = __dsub_rn(cy, g[1]), dz = __dsub_rn(cz, g[2]);
   c_s[c] = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+  // PAPER Eq. 2, B2 = sum m |r_CM - r|^2, accumulated bottom-up in a fixed order (R19): leaf: its particles in
+  // slot order; internal: children in octant order, B2 += B2_child, then B2 += M_child |CM_child - CM|^2
+  double b2 = 0.0;
+  if (nch == 0) {
+    for (uint32_t s0 = first; s0 < first + count; s0 += 8) {
+      float4 p[8];
+      const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) p[j] = spos[s0 + j];
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) {
+        const double ex = __dsub_rn((double)p[j].x, cx), ey = __dsub_rn((double)p[j].y, cy), ez = __dsub_rn((double)p[j].z, cz);
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        b2 = __dadd_rn(b2, __dmul_rn((double)p[j].w, r2));
+      }
+    }
+  } else {
+    const uint32_t ch = c_child_first[c];
+    for (int k = 0; k < nch; k++) {
+      const double* q = cm64 + 3 * (size_t)(ch + k);
+      const double ex = __dsub_rn(q[0], cx), ey = __dsub_rn(q[1], cy), ez = __dsub_rn(q[2], cz);
+      const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+      b2 = __dadd_rn(b2, a.c_B2[ch + k]);
+      b2 = __dadd_rn(b2, __dmul_rn(MP[4 * (size_t)(ch + k)], r2));
+    }
+  }
+  a.c_B2[c] = b2;
 }
 // the whole bottom-up pass in ONE cooperative launch: every level deepest first, a grid-wide barrier
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
@@ -274,6 +301,7 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   OTOO_TRY(grow(ctx, &ctx->c_MP, 4 * cap));
   OTOO_TRY(grow(ctx, &ctx->c_cm64, 3 * cap));
   OTOO_TRY(grow(ctx, &ctx->c_s, cap));
+  OTOO_TRY(grow(ctx, &ctx->c_B2, cap));
   OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
   OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
   for (int b = 0; b < 2; b++) { OTOO_TRY(grow(ctx, &ctx->tmp_key[b], cap)); OTOO_TRY(grow(ctx, &ctx->tmp_val[b], cap)); }
@@ -335,7 +363,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   ctx->launches += 1;
   // H6 deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s};
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2};
   {
     int occ = 1;
     OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));

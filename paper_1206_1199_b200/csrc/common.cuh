@@ -57,6 +57,7 @@ struct otoo_ctx {
   double* c_MP;          // 4 per cell: M, Px, Py, Pz (R6)
   double* c_cm64;        // 3 per cell: fp64 centre of mass (needed for Eq. 5)
   double* c_s;           // |CM - geometric centre| (R7)
+  double* c_B2;          // trace of the quadrupole tensor about the CM (PAPER Eq. 2; R19)
   float2* c_sph;         // (b_max, r_SPH) (R14)
   unsigned long long* sph_acc;  // 2 per cell: fp64 maxima as ordered bits
   uint64_t* tmp_key[2];  // (level) keys for the canonical ordering pass
@@ -129,7 +130,9 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
 otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, uint32_t* total_out_dev,
                                     cudaStream_t st);
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st);
-otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, float* d_acc_pot, cudaStream_t st);
+// mac 0: theta criterion (p0 = theta); mac 1: the paper's absolute-error criterion (p0 = Delta, p1 = m_limit)
+otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float p1, int G, float* d_acc_pot, cudaStream_t st);
+otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st);   // fp64 b_max of every cell into sph_acc[2c] (sph.cu)
 otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb,
                                   cudaStream_t st);
 otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,

@@ -28,6 +28,28 @@ __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_
   reinterpret_cast<uint32_t*>(cell_b + c)[0] = __float_as_uint(rb2);
 }
 
+// PAPER Eq. 1: r_b = b/2 + sqrt(b^2/4 + sqrt(3 B2 / Delta)), b = b_max (fp64, from the radii pass); cells heavier
+// than m_limit: r_b = 2 S_root (L157); Delta = 0: open everything.  Same fp64 operation order as the oracle.
+__global__ void __launch_bounds__(256) rb2_delta_kernel(const double* __restrict__ c_B2, const double* __restrict__ c_MP,
+                                                        const unsigned long long* __restrict__ bmax_bits, int64_t ncell,
+                                                        float S, float delta, float m_limit, cellb_t* __restrict__ cell_b) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  float rb2;
+  if (!(delta > 0.0f)) rb2 = INFINITY;
+  else {
+    double rb;
+    if (c_MP[4 * c] > (double)m_limit) rb = __dmul_rn(2.0, (double)S);
+    else {
+      const double h = __dmul_rn(0.5, __longlong_as_double((long long)bmax_bits[2 * c]));
+      const double q = __dsqrt_rn(__ddiv_rn(__dmul_rn(3.0, c_B2[c]), (double)delta));
+      rb = __dadd_rn(h, __dsqrt_rn(__dadd_rn(__dmul_rn(h, h), q)));
+    }
+    rb2 = __double2float_rn(__dmul_rn(rb, rb));
+  }
+  reinterpret_cast<uint32_t*>(cell_b + c)[0] = __float_as_uint(rb2);
+}
+
 struct GravParams {
   WalkCommon c;
   float eps2;
@@ -375,11 +397,17 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   return OTOO_OK;
 }
 
-otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, float theta, int G, float* d_acc_pot, cudaStream_t st) {
+otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float p1, int G, float* d_acc_pot, cudaStream_t st) {
   GravParams p;
   int grid; size_t smem;
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st));
-  rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, theta, ctx->cell_b);
+  if (mac == 0) {
+    rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b);
+  } else {
+    OTOO_TRY(otoo_bmax_impl(ctx, st));
+    rb2_delta_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_B2, ctx->c_MP, ctx->sph_acc, ctx->N_cell, ctx->S,
+                                                                         p0, p1, ctx->cell_b);
+  }
   OTOO_CUDA(ctx, cudaMemsetAsync(d_acc_pot, 0, 16 * (size_t)ctx->N, st));
   p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);

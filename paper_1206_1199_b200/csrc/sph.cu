@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = s < n;
   float4 p = valid ? spos[s] : make_float4(0, 0, 0, 0);
-  double h = valid ? (double)hs[s] : 0.0;
+  double h = (valid && hs) ? (double)hs[s] : 0.0;     // hs == NULL: b_max only (the Delta-MAC of gravity)
   uint32_t cell = valid ? 0u : 0xFFFFFFFFu;
   while (__any_sync(0xFFFFFFFFu, cell != 0xFFFFFFFFu)) {
     double b = 0.0, r = 0.0;
@@ -284,6 +284,17 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
 }
 
 }  // namespace
+
+// fp64 b_max (L63) of every cell for the absolute-error MAC: the Eq. 5 pass with h = 0; leaves the maxima as
+// ordered bits in sph_acc[2c].  The fp32 SPH radii are recomputed by every SPH call anyway.
+otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st) {
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
+  sph_radii_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->c_first, ctx->c_count,
+                                                                ctx->c_child_first, ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
+  ctx->launches += 1;
+  ctx->sph_radii_valid = false;
+  return OTOO_OK;
+}
 
 otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb, cudaStream_t st) {
   SphParams p; int grid; size_t smem;

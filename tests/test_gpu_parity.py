@@ -109,6 +109,37 @@ def test_gravity_parity(otoo, orc, kind, n, G, theta, eps, ws):
     assert pe.max() <= TOL, pe.max()
 
 
+@pytest.mark.parametrize("kind,n,G,delta,m_limit,eps", [("plummer", 16384, 64, 0.01, 0.05, 0.01), ("plummer", 20000 + 5, 128, 0.1, np.inf, 0.004),
+                                                        ("uniform_sphere", 30000, 32, 0.001, 0.025, 0.0), ("hernquist", 25000, 256, 1.0, 0.05, 0.002),
+                                                        ("plummer", 3000, 64, 0.0, np.inf, 0.01)])
+def test_gravity_delta_mac_parity(otoo, orc, kind, n, G, delta, m_limit, eps):
+    """The paper's absolute-error MAC (Eq. 1-2, m_limit rule L157): rb^2 of every cell bit-exact,
+    hence lists and counters exact; sums within the tolerances of the theta path."""
+    pm = gen.make(kind, n, 1199)
+    pm[:, 3] = ((1 + np.arange(n) % 3) / (2.0 * n)).astype(np.float32)        # unequal masses
+    t = check_tree(otoo, orc, pm, 16)
+    d32, ml32, eps32 = float(np.float32(delta)), float(np.float32(m_limit)), float(np.float32(eps))
+    rb2 = t.rb2_delta(d32, ml32)
+    ref = t.gravity(eps32, 0.0, G, rb2=rb2)
+    out = otoo.otoo_gravity_delta(eps32, d32, ml32, G).cpu().numpy()
+    assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), rb2.view(np.uint32))
+    nt, nc, npart = otoo.otoo_export_group_stats()
+    assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+    assert otoo.otoo_last_stats()["sum_interactions"] == ref["interactions"]
+    e, raw = acc_err(out, ref["acc_pot"], ref["abs_sum"])
+    assert e.max() <= TOL, (e.max(), raw.max())
+    assert np.percentile(raw, 99.9) <= TOL
+    pe = np.abs(out[:, 3] - ref["acc_pot"][:, 3]) / np.abs(ref["acc_pot"][:, 3])
+    assert pe.max() <= TOL
+    # an SPH call after it must not see the h = 0 radii of the Delta pass
+    if n == 16384:
+        h = np.full(n, 0.3, np.float32)
+        rho, _ = otoo.otoo_sph_density(dev(h), 64)
+        rref = t.sph_density(h, 64, groups=np.arange(4))
+        idx = t.group_targets(64, np.arange(4))
+        assert (np.abs(rho.cpu().numpy()[idx] - rref["rho"][idx]) / rref["rho"][idx]).max() <= TOL
+
+
 def test_walk_stack_spill(otoo, orc):
     """theta = 0 on a deep tree overflows the 512-entry shared stack: both overflow paths (task pool,
     private global spill) must give the same lists."""
@@ -181,6 +212,11 @@ def test_status_codes(otoo):
         fresh.otoo_build_tree(pm, 16)
     assert e.value.status == binding.OTOO_ERR_CAPACITY
     fresh.otoo_build_tree(pm[:500].contiguous(), 16)
+    for bad in (dict(eps=0.01, delta=-1.0, m_limit=1.0, group_size=64), dict(eps=0.01, delta=0.1, m_limit=0.0, group_size=64),
+                dict(eps=0.01, delta=float("nan"), m_limit=1.0, group_size=64)):
+        with pytest.raises(binding.OtooError) as e:
+            fresh.otoo_gravity_delta(**bad)
+        assert e.value.status == binding.OTOO_ERR_INVALID_ARG
     for bad in (dict(eps=-1.0, theta=0.5, group_size=64), dict(eps=0.01, theta=-0.5, group_size=64),
                 dict(eps=0.01, theta=0.5, group_size=48)):
         with pytest.raises(binding.OtooError) as e:
