@@ -95,7 +95,11 @@ def run_reference(args, rank):
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         t = oracle.Tree(pm, cfg["n_crit"])
-        r = t.gravity(eps, theta, cfg["group"])
+        rb2 = None
+        if args.mac == "delta":
+            rb2 = t.rb2_delta(float(np.float32(args.delta if args.delta is not None else cfg.get("delta", 0.01))),
+                              float(np.float32(args.m_limit if args.m_limit is not None else cfg.get("m_limit", 0.05))))
+        r = t.gravity(eps, theta, cfg["group"], rb2=rb2)
         dt = time.perf_counter() - t0
         inter = r["interactions"]
         del t
@@ -124,6 +128,10 @@ def main():
     ap.add_argument("--impl", default="otoo", choices=["otoo", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(gen.CONFIGS))
     ap.add_argument("--theta", type=float, default=None)
+    ap.add_argument("--mac", default="theta", choices=["theta", "delta"],
+                    help="delta: the paper's absolute-error MAC (otoo_gravity_delta) instead of BASELINE's theta criterion")
+    ap.add_argument("--delta", type=float, default=None)
+    ap.add_argument("--m-limit", type=float, default=None)
     ap.add_argument("--seed", type=int, default=1206)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -146,6 +154,8 @@ def main():
     cfg, pm = workload(args.workload, args.theta, replicas.replica_seed(args.seed, rank))
     n, G, n_crit = cfg["n"], cfg["group"], cfg["n_crit"]
     eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
+    delta = float(np.float32(args.delta if args.delta is not None else cfg.get("delta", 0.01)))
+    m_limit = float(np.float32(args.m_limit if args.m_limit is not None else cfg.get("m_limit", 0.05)))
     o = binding.Otoo(max_particles=n, device=local)
     d_pm = torch.from_numpy(pm).cuda()
     out = torch.empty((n, 4), dtype=torch.float32, device="cuda")
@@ -158,7 +168,10 @@ def main():
         o.otoo_build_tree(d_pm, n_crit)
         l1 = o.otoo_last_stats()["launches"] if not timed else 0
         e[1].record()
-        o.otoo_gravity(eps, theta, G, out=out)
+        if args.mac == "delta":
+            o.otoo_gravity_delta(eps, delta, m_limit, G, out=out)
+        else:
+            o.otoo_gravity(eps, theta, G, out=out)
         e[2].record()
         return e, l1
 
@@ -193,7 +206,13 @@ def main():
         flush_buf.fill_(1)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        o.otoo_gravity_host(h_in.numpy(), n_crit, eps, theta, G, out=h_out.numpy())
+        if args.mac == "delta":      # same public calls on pinned host buffers (there is no host form of the Delta entry point)
+            d_in = h_in.cuda(non_blocking=True)
+            o.otoo_build_tree(d_in, n_crit)
+            h_out.copy_(o.otoo_gravity_delta(eps, delta, m_limit, G, out=out), non_blocking=True)
+            torch.cuda.synchronize()
+        else:
+            o.otoo_gravity_host(h_in.numpy(), n_crit, eps, theta, G, out=h_out.numpy())
         dt = time.perf_counter() - t0
         if it >= 2:
             e2e_t.append(dt)
@@ -220,10 +239,11 @@ def main():
                 "kernel_ms": grav_ms, "interactions_per_s_kernel": inter / (grav_ms * 1e-3),
                 "build_ms": float(t_build.mean())}
 
+    mac_txt = f"theta={cfg['theta']}" if args.mac == "theta" else f"Delta-MAC delta={delta:g} m_limit={m_limit:g}"
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {cfg['kind']} N={n} eps={cfg['eps']} theta={cfg['theta']} "
+            "config": {"workload": f"{args.workload}: {cfg['kind']} N={n} eps={cfg['eps']} {mac_txt} "
                                    f"n_crit={n_crit} group={G}",
                        "l2": "flushed between steps (256 MiB write, outside the timed events)",
                        "parallelism": "replicas" if world > 1 else "single"},
@@ -237,7 +257,7 @@ def main():
         from oracle import oracle
         t0 = time.perf_counter()
         t = oracle.Tree(pm, n_crit)
-        r = t.gravity(eps, theta, G, forces=True)
+        r = t.gravity(eps, theta, G, forces=True, rb2=t.rb2_delta(delta, m_limit) if args.mac == "delta" else None)
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": r["interactions"] / dt, "unit": UNIT, "cores": oracle.max_threads(),
                                 "kind": "oracle", "ms_per_step": 1e3 * dt,

@@ -189,6 +189,9 @@ CONFIGS = {
     "C3": dict(kind="hernquist", n=8388608, eps=0.002, theta=0.6, n_crit=16, group=128),
     "C4": dict(kind="wd_pair", n=2097152, eps=0.005, theta=0.5, n_crit=16, group=128, group_sph=64),
     "C5": dict(kind="uniform_cube", n=33554432, eps=0.001, theta=0.5, n_crit=16, group=256),
+    # not a BASELINE config: the paper's own gravity benchmark (uniform sphere, r = 1, M = 1,
+    # N = 8000 x 1024, Delta = 0.01, n_crit = 16, m_limit = 0.05), run with otoo_gravity_delta (bench.py --mac delta)
+    "F4": dict(kind="uniform_sphere", n=8192000, eps=0.002, theta=0.6, n_crit=16, group=128, delta=0.01, m_limit=0.05),
 }
 
 
