@@ -43,6 +43,11 @@ def lib():
         vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
         L.orc_build.restype = vp
         L.orc_build.argtypes = [i64, vp, i32]
+        L.orc_build_ord.restype = vp
+        L.orc_build_ord.argtypes = [i64, vp, i32, i32]
+        L.orc_hilbert_key.restype = C.c_uint64
+        L.orc_hilbert_key.argtypes = [vp]
+        L.orc_hilbert_coords.argtypes = [C.c_uint64, vp]
         L.orc_free.argtypes = [vp]
         L.orc_ncell.restype = i64
         L.orc_ncell.argtypes = [vp]
@@ -127,15 +132,30 @@ def dWdr(r, h):
     return lib().orc_dWdr(float(r), float(h))
 
 
+def hilbert_key(q):
+    """63-bit Hilbert key of 21-bit integer coordinates (x, y, z)"""
+    a = np.ascontiguousarray(q, dtype=np.uint32)
+    assert a.shape == (3,)
+    return int(lib().orc_hilbert_key(_p(a)))
+
+
+def hilbert_coords(key):
+    out = np.zeros(3, dtype=np.uint32)
+    lib().orc_hilbert_coords(C.c_uint64(int(key)), _p(out))
+    return out
+
+
 class Tree:
     """Oracle tree: PAPER.md III-B (build) + III-C (cell properties)."""
 
-    def __init__(self, pos_mass, n_crit=16):
+    def __init__(self, pos_mass, n_crit=16, key_order=0):
+        """key_order 0: Morton keys (R3); 1: Hilbert keys (reading R20)"""
         self.pm = _f32(pos_mass)
         assert self.pm.ndim == 2 and self.pm.shape[1] == 4
         self.N = self.pm.shape[0]
         self.n_crit = int(n_crit)
-        self._h = lib().orc_build(self.N, _p(self.pm), self.n_crit)
+        self.key_order = int(key_order)
+        self._h = lib().orc_build_ord(self.N, _p(self.pm), self.n_crit, self.key_order)
         self.ncell = lib().orc_ncell(self._h)
         self.nleaf = lib().orc_nleaf(self._h)
         self.depth = lib().orc_depth(self._h)

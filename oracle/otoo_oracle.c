@@ -15,6 +15,7 @@
 struct orc_tree {
   int64_t N;
   int n_crit;
+  int key_order;  /* 0 Morton (R3), 1 Hilbert (R20) */
   float lo[3], S;
   uint64_t* key;  /* sorted keys */
   uint32_t* perm; /* perm[s] = original index of sorted slot s */
@@ -31,8 +32,60 @@ struct orc_tree {
   int64_t* more;
 };
 
+/* ---------------- Hilbert order (PAPER III-B step 2, L131: "we convert the Morton key into the Hilbert key")
+ * The paper gives no algorithm; reading R20: the 3-D Hilbert curve in Skilling's transpose
+ * form ("Programming the Hilbert curve", 2004), b = 21 bits per axis, x the most significant axis.  The
+ * key is the bit interleave of the transformed coordinates, so its top 3l bits still name the level-l
+ * octree cell: the tree holds the same cells as with Morton keys, visited in Hilbert order. */
+static void hilbert_axes_to_transpose(uint32_t X[3], int b) {
+  uint32_t M = 1u << (b - 1), P, Q, t;
+  for (Q = M; Q > 1; Q >>= 1) {
+    P = Q - 1;
+    for (int i = 0; i < 3; i++) {
+      if (X[i] & Q) X[0] ^= P;                                       /* invert the low bits of x */
+      else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }          /* exchange the low bits of x and axis i */
+    }
+  }
+  for (int i = 1; i < 3; i++) X[i] ^= X[i - 1];                      /* Gray encode */
+  t = 0;
+  for (Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+  for (int i = 0; i < 3; i++) X[i] ^= t;
+}
+static void hilbert_transpose_to_axes(uint32_t X[3], int b) {
+  uint32_t N = 2u << (b - 1), P, Q, t;
+  t = X[2] >> 1;                                                     /* Gray decode */
+  for (int i = 2; i > 0; i--) X[i] ^= X[i - 1];
+  X[0] ^= t;
+  for (Q = 2; Q != N; Q <<= 1) {
+    P = Q - 1;
+    for (int i = 2; i >= 0; i--) {
+      if (X[i] & Q) X[0] ^= P;
+      else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+    }
+  }
+}
+static uint64_t interleave3(const uint32_t q[3]) {
+  uint64_t key = 0;
+  for (int b = 0; b < MAXLEV; b++)
+    key |= (uint64_t)((((q[0] >> b) & 1u) << 2) | (((q[1] >> b) & 1u) << 1) | ((q[2] >> b) & 1u)) << (3 * b);
+  return key;
+}
+uint64_t orc_hilbert_key(const uint32_t q_in[3]) {   /* quantised coordinates (21 bits each) -> 63-bit Hilbert key */
+  uint32_t X[3] = {q_in[0], q_in[1], q_in[2]};
+  hilbert_axes_to_transpose(X, MAXLEV);
+  return interleave3(X);
+}
+void orc_hilbert_coords(uint64_t key, uint32_t q[3]) {   /* the inverse */
+  q[0] = q[1] = q[2] = 0;
+  for (int b = 0; b < MAXLEV; b++) {
+    uint64_t oct = (key >> (3 * b)) & 7u;
+    q[0] |= (uint32_t)((oct >> 2) & 1u) << b; q[1] |= (uint32_t)((oct >> 1) & 1u) << b; q[2] |= (uint32_t)(oct & 1u) << b;
+  }
+  hilbert_transpose_to_axes(q, MAXLEV);
+}
+
 /* ---------------- R1-R4: root cube, keys, sort (PAPER III-B steps 1-3, L121-L133) --------- */
-static uint64_t key_of(const float lo[3], float scale, const float* p) {
+static uint64_t key_of_ord(const float lo[3], float scale, const float* p, int key_order) {
   uint32_t q[3];
   for (int k = 0; k < 3; k++) {
     float d = p[k] - lo[k];         /* one fp32 subtract */
@@ -40,6 +93,7 @@ static uint64_t key_of(const float lo[3], float scale, const float* p) {
     uint32_t v = (t >= 2097151.0f) ? 2097151u : (t > 0.0f ? (uint32_t)t : 0u);
     q[k] = v;
   }
+  if (key_order == 1) return orc_hilbert_key(q);
   uint64_t key = 0;
   for (int lev = 1; lev <= MAXLEV; lev++) { /* L129: concatenation of the octant index per level */
     int b = MAXLEV - lev;
@@ -98,7 +152,14 @@ static int cs_cmp(const void* a, const void* b) {
   return 0;
 }
 
-static void cell_coord(uint64_t prefix, int level, uint32_t c[3]) {
+static void cell_coord_ord(uint64_t prefix, int level, uint32_t c[3], int key_order) {
+  if (key_order == 1) {   /* Hilbert prefix -> any key of the cell -> coordinates -> their top `level` bits */
+    uint32_t q[3];
+    if (level == 0) { c[0] = c[1] = c[2] = 0; return; }
+    orc_hilbert_coords(prefix << (3 * (MAXLEV - level)), q);
+    for (int k = 0; k < 3; k++) c[k] = q[k] >> (MAXLEV - level);
+    return;
+  }
   c[0] = c[1] = c[2] = 0;
   for (int i = 0; i < level; i++) {
     uint64_t oct = (prefix >> (3 * i)) & 7u;
@@ -133,7 +194,7 @@ static void moments(orc_tree* t, int64_t id) {
   }
   t->MP[4 * id] = M; t->MP[4 * id + 1] = Px; t->MP[4 * id + 2] = Py; t->MP[4 * id + 3] = Pz;
   /* geometric centre and s (R7) */
-  uint32_t cc[3]; cell_coord(c->prefix, c->level, cc);
+  uint32_t cc[3]; cell_coord_ord(c->prefix, c->level, cc, t->key_order);
   double l = ldexp((double)t->S, -(int)c->level);
   double g[3];
   for (int k = 0; k < 3; k++) g[k] = (double)t->lo[k] + ((double)cc[k] + 0.5) * l;
@@ -146,9 +207,10 @@ static void moments(orc_tree* t, int64_t id) {
   t->s[id] = sqrt((dx * dx + dy * dy) + dz * dz);
 }
 
-orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit) {
+orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit) { return orc_build_ord(N, pos_mass, n_crit, 0); }
+orc_tree* orc_build_ord(int64_t N, const float* pos_mass, int n_crit, int key_order) {
   orc_tree* t = (orc_tree*)calloc(1, sizeof(orc_tree));
-  t->N = N; t->n_crit = n_crit;
+  t->N = N; t->n_crit = n_crit; t->key_order = key_order;
   /* R1 / L121,L127: cube enclosing all particles, anchored at the lo corner */
   float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
   for (int64_t i = 0; i < N; i++)
@@ -164,7 +226,7 @@ orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit) {
   float scale = 2097152.0f / S;   /* R2: IEEE fp32 division */
   kv_t* kv = (kv_t*)malloc(sizeof(kv_t) * (N > 0 ? N : 1));
 #pragma omp parallel for schedule(static)
-  for (int64_t i = 0; i < N; i++) { kv[i].key = key_of(lo, scale, pos_mass + 4 * i); kv[i].id = (uint32_t)i; }
+  for (int64_t i = 0; i < N; i++) { kv[i].key = key_of_ord(lo, scale, pos_mass + 4 * i, key_order); kv[i].id = (uint32_t)i; }
   qsort(kv, (size_t)N, sizeof(kv_t), kv_cmp);   /* L133 */
   t->key = (uint64_t*)malloc(8 * (N > 0 ? N : 1));
   t->perm = (uint32_t*)malloc(4 * (N > 0 ? N : 1));
@@ -229,7 +291,7 @@ int64_t orc_ncell(const orc_tree* t) { return t->ncell; }
 int64_t orc_nleaf(const orc_tree* t) { return t->nleaf; }
 int orc_depth(const orc_tree* t) { return t->depth; }
 void orc_root(const orc_tree* t, float lo[3], float* S) { memcpy(lo, t->lo, 12); *S = t->S; }
-uint64_t orc_key(const orc_tree* t, const float xyz[3]) { return key_of(t->lo, 2097152.0f / t->S, xyz); }
+uint64_t orc_key(const orc_tree* t, const float xyz[3]) { return key_of_ord(t->lo, 2097152.0f / t->S, xyz, t->key_order); }
 
 void orc_export(const orc_tree* t, uint32_t* perm, uint64_t* keys, orc_cell* cells, float* com_m,
                 double* s, double* MP) {

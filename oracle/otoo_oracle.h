@@ -44,6 +44,10 @@ void orc_direct_sum(int64_t N, const float* pos_mass, double eps, int64_t n_targ
 
 /* Tree build: PAPER.md III-B steps 1-4 + III-C (mass, centre of mass). */
 orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit);
+/* key_order 0: Morton keys (R3); 1: Hilbert keys (reading R20: Skilling's transpose form) */
+orc_tree* orc_build_ord(int64_t N, const float* pos_mass, int n_crit, int key_order);
+uint64_t orc_hilbert_key(const uint32_t q[3]);           /* 21-bit coordinates -> 63-bit Hilbert key */
+void orc_hilbert_coords(uint64_t key, uint32_t q[3]);    /* and back */
 void orc_free(orc_tree*);
 int64_t orc_ncell(const orc_tree*);
 int64_t orc_nleaf(const orc_tree*);
