@@ -132,6 +132,10 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).
+ * "key_order" = 0 (default): particles, groups and cells in Morton order (R3); 1: in Hilbert
+ * order (the paper's own ordering; R20) -- same cells, other order: no group straddles an
+ * octant boundary with a system-sized box, fewer interactions at the same theta.  Read by the next
+ * otoo_build_tree; otoo_cell_t.prefix is then a Hilbert-key prefix.
  * "warp_specialized" = 1 (default): otoo_gravity runs walker/evaluator warp pairs (walker warps build
  * the lists in shared memory, evaluator warps hold the targets and sum), 0: one warp does both in turn.
  * Same lists, same counters; sums differ in rounding order only.

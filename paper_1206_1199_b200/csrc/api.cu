@@ -282,6 +282,11 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     return OTOO_OK;
   }
   if (strcmp(name, "task_pool") == 0) { ctx->use_pool = value != 0; return OTOO_OK; }
+  if (strcmp(name, "key_order") == 0) {
+    if (value != 0 && value != 1) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "key_order must be 0 (Morton) or 1 (Hilbert)");
+    ctx->key_order = (int)value;
+    return OTOO_OK;
+  }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "warp_specialized") == 0) { ctx->use_ws = value != 0; return OTOO_OK; }
   return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");

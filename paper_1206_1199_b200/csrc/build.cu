@@ -79,6 +79,38 @@ __device__ __forceinline__ uint32_t compact3(uint64_t x) {
   x = (x | x >> 32) & 0x1FFFFFull;
   return (uint32_t)x;
 }
+// Hilbert order (reading R20): Skilling's transpose form of the 3-D Hilbert curve on the 21-bit
+// quantised coordinates, x the most significant axis.  The key is the interleave of the transformed
+// coordinates, so its top 3l bits still name the level-l octree cell.
+__device__ __forceinline__ void hilbert_axes_to_transpose(uint32_t& x, uint32_t& y, uint32_t& z) {
+  uint32_t X[3] = {x, y, z};
+  for (uint32_t Q = 1u << (OTOO_MAXLEV - 1); Q > 1; Q >>= 1) {
+    const uint32_t P = Q - 1;
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+      if (X[i] & Q) X[0] ^= P;
+      else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+    }
+  }
+  X[1] ^= X[0]; X[2] ^= X[1];
+  uint32_t t = 0;
+  for (uint32_t Q = 1u << (OTOO_MAXLEV - 1); Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+  x = X[0] ^ t; y = X[1] ^ t; z = X[2] ^ t;
+}
+__device__ __forceinline__ void hilbert_transpose_to_axes(uint32_t& x, uint32_t& y, uint32_t& z) {
+  uint32_t X[3] = {x, y, z};
+  uint32_t t = X[2] >> 1;
+  X[2] ^= X[1]; X[1] ^= X[0]; X[0] ^= t;
+  for (uint32_t Q = 2; Q != (2u << (OTOO_MAXLEV - 1)); Q <<= 1) {
+    const uint32_t P = Q - 1;
+#pragma unroll
+    for (int i = 2; i >= 0; i--) {
+      if (X[i] & Q) X[0] ^= P;
+      else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+    }
+  }
+  x = X[0]; y = X[1]; z = X[2];
+}
 __device__ __forceinline__ uint32_t quant(float x, float lo, float scale) {
   float t = __fmul_rn(__fsub_rn(x, lo), scale);
   return (t >= 2097151.0f) ? 2097151u : (t > 0.0f ? __float2uint_rz(t) : 0u);
@@ -86,14 +118,15 @@ __device__ __forceinline__ uint32_t quant(float x, float lo, float scale) {
 // H2 (L129; R2, R3): 63-bit Morton key by bit dilation, x most significant in each octant.
 __global__ void __launch_bounds__(256) key_kernel(const float4* __restrict__ pos, int64_t n,
                                                   const unsigned* __restrict__ bbox, uint64_t* __restrict__ key,
-                                                  uint32_t* __restrict__ id) {
+                                                  uint32_t* __restrict__ id, int hilbert) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const float* r = reinterpret_cast<const float*>(bbox) + 8;
   float scale = r[4];
   float4 p = pos[i];
-  key[i] = (dilate3(quant(p.x, r[0], scale)) << 2) | (dilate3(quant(p.y, r[1], scale)) << 1) |
-           dilate3(quant(p.z, r[2], scale));
+  uint32_t qx = quant(p.x, r[0], scale), qy = quant(p.y, r[1], scale), qz = quant(p.z, r[2], scale);
+  if (hilbert) hilbert_axes_to_transpose(qx, qy, qz);
+  key[i] = (dilate3(qx) << 2) | (dilate3(qy) << 1) | dilate3(qz);
   id[i] = (uint32_t)i;
 }
 // H4: positions into sorted order
@@ -192,6 +225,7 @@ struct MomentArgs {
   const float4* spos; const uint64_t* key; const uint32_t* c_first; const uint32_t* c_count;
   const uint32_t* c_child_first; const uint8_t* c_child_count; const unsigned* bbox;
   double* MP; double* cm64; float4* cell_cm; double* c_s; double* c_B2;
+  int hilbert;
 };
 __device__ __forceinline__ void moments_cell(uint32_t c, int level, const MomentArgs& a) {
   const float4* __restrict__ spos = a.spos; const uint64_t* __restrict__ key = a.key;
@@ -228,11 +262,18 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, const Moment
   o[0] = M; o[1] = Px; o[2] = Py; o[3] = Pz;
   const float* r = reinterpret_cast<const float*>(bbox) + 8;
   double l = ldexp((double)r[3], -level);
-  uint64_t prefix = (count > 0 && level > 0) ? (key[first] >> (3 * (OTOO_MAXLEV - level))) : 0ull;
+  // integer cell coordinates = top `level` bits of the quantised coordinates of any particle of the cell
+  uint32_t qx = 0, qy = 0, qz = 0;
+  if (count > 0 && level > 0) {
+    const uint64_t k0 = key[first];
+    qx = compact3(k0 >> 2); qy = compact3(k0 >> 1); qz = compact3(k0);
+    if (a.hilbert) hilbert_transpose_to_axes(qx, qy, qz);
+    qx >>= OTOO_MAXLEV - level; qy >>= OTOO_MAXLEV - level; qz >>= OTOO_MAXLEV - level;
+  }
   double g[3];
-  g[0] = __dadd_rn((double)r[0], __dmul_rn((double)compact3(prefix >> 2) + 0.5, l));
-  g[1] = __dadd_rn((double)r[1], __dmul_rn((double)compact3(prefix >> 1) + 0.5, l));
-  g[2] = __dadd_rn((double)r[2], __dmul_rn((double)compact3(prefix) + 0.5, l));
+  g[0] = __dadd_rn((double)r[0], __dmul_rn((double)qx + 0.5, l));
+  g[1] = __dadd_rn((double)r[1], __dmul_rn((double)qy + 0.5, l));
+  g[2] = __dadd_rn((double)r[2], __dmul_rn((double)qz + 0.5, l));
   double cx, cy, cz;
   if (M != 0.0) { cx = __ddiv_rn(Px, M); cy = __ddiv_rn(Py, M); cz = __ddiv_rn(Pz, M); }
   else { cx = g[0]; cy = g[1]; cz = g[2]; }
@@ -331,7 +372,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
   root_kernel<<<1, 1, 0, st>>>(bbox);
   // H2, H3, H4
-  key_kernel<<<nbN, 256, 0, st>>>(pos, N, bbox, ctx->key[0], ctx->val[0]);
+  key_kernel<<<nbN, 256, 0, st>>>(pos, N, bbox, ctx->key[0], ctx->val[0], ctx->key_order);
   ctx->launches += 3;
   int res = 0;
   OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res));
@@ -363,7 +404,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   ctx->launches += 1;
   // H6 deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2};
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order};
   {
     int occ = 1;
     OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));

@@ -95,6 +95,7 @@ struct otoo_ctx {
   uint32_t level_off[OTOO_NLEV + 1];
   int walk_stack;        // option "walk_stack"
   int use_pool;          // option "task_pool"
+  int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int walk_only;         // option "walk_only" (diagnostic)
   int use_ws;            // option "warp_specialized": gravity walk with walker/evaluator warp pairs
   int last_group_size;

@@ -44,9 +44,13 @@ def acc_err(got, want, abs_sum=None):
     return 1e-5 * d / np.maximum(tol, 1e-300), d / np.maximum(an, 1e-300)
 
 
-def check_tree(otoo, orc, pm, n_crit):
-    t = orc.Tree(pm, n_crit)
-    otoo.otoo_build_tree(dev(pm), n_crit)
+def check_tree(otoo, orc, pm, n_crit, key_order=0):
+    t = orc.Tree(pm, n_crit, key_order=key_order)
+    otoo.otoo_set_option("key_order", key_order)
+    try:
+        otoo.otoo_build_tree(dev(pm), n_crit)
+    finally:
+        otoo.otoo_set_option("key_order", 0)
     ex = otoo.otoo_export_tree()
     eo = t.export()
     assert ex["N"] == t.N and ex["N_cell"] == t.ncell and ex["N_leaf"] == t.nleaf and ex["depth"] == t.depth
@@ -138,6 +142,35 @@ def test_gravity_delta_mac_parity(otoo, orc, kind, n, G, delta, m_limit, eps):
         rref = t.sph_density(h, 64, groups=np.arange(4))
         idx = t.group_targets(64, np.arange(4))
         assert (np.abs(rho.cpu().numpy()[idx] - rref["rho"][idx]) / rref["rho"][idx]).max() <= TOL
+
+
+@pytest.mark.parametrize("kind,n,n_crit,G", [("plummer", 16384, 16, 64), ("hernquist", 30000 + 7, 8, 128), ("uniform_cube", 40000, 16, 256),
+                                             ("plummer", 9, 16, 32), ("uniform_sphere", 5000, 1, 32)])
+def test_hilbert_order_parity(otoo, orc, kind, n, n_crit, G):
+    """key_order = 1 (reading R20): keys, permutation, cells, moments bit-exact against the oracle's
+    Hilbert tree; theta- and Delta-MAC walks exact; SPH density on the same tree."""
+    pm = gen.make(kind, n, 2012)
+    t = check_tree(otoo, orc, pm, n_crit, key_order=1)
+    ref = t.gravity(0.01, float(np.float32(0.6)), G)
+    out = otoo.otoo_gravity(0.01, float(np.float32(0.6)), G).cpu().numpy()
+    nt, nc, npart = otoo.otoo_export_group_stats()
+    assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+    e, raw = acc_err(out, ref["acc_pot"], ref["abs_sum"])
+    assert e.max() <= TOL
+    rb2 = t.rb2_delta(float(np.float32(0.01)), float(np.float32(0.05)))
+    refd = t.gravity(0.01, 0.0, G, rb2=rb2)
+    outd = otoo.otoo_gravity_delta(0.01, 0.01, 0.05, G).cpu().numpy()
+    assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), rb2.view(np.uint32))
+    nt, nc, npart = otoo.otoo_export_group_stats()
+    assert np.array_equal(nt, refd["n_tests"]) and np.array_equal(nc, refd["n_cells"]) and np.array_equal(npart, refd["n_parts"])
+    e, _ = acc_err(outd, refd["acc_pot"], refd["abs_sum"])
+    assert e.max() <= TOL
+    if n >= 1000:
+        h = np.full(n, 0.1 * t.S / n ** (1 / 3) * 4, np.float32)
+        rs = t.sph_density(h, G if G <= 128 else 128)
+        rho, nngb = otoo.otoo_sph_density(dev(h), G if G <= 128 else 128)
+        assert np.array_equal(nngb.cpu().numpy().view(np.uint32), rs["nngb"])
+        assert (np.abs(rho.cpu().numpy() - rs["rho"]) / rs["rho"]).max() <= TOL
 
 
 def test_walk_stack_spill(otoo, orc):
