@@ -227,6 +227,7 @@ def main():
             dist.destroy_process_group()
         return
 
+    peak_measured = o.otoo_measure_fp32_peak()      # FFMA2-only kernel on this GPU, at the clock it holds
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tflops = sm_count * SM_LANES * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
     grav_ms = float(t_grav.mean())
@@ -236,8 +237,8 @@ def main():
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
                 # profiles/r1_walk_gravity_full.md (C2, theta=0.6 only); the kernel is ALU-bound, DRAM < 1 %
                 "traffic": 51.11e6 if (args.workload == "C2" and args.theta is None) else None,
-                "peak_source": f"derived: {sm_count} SMs x 128 FP32 lanes x 2 flop x {NOMINAL_SM_MHZ:.0f} MHz (DESIGN.md); "
-                               "FFMA microbenchmark on this pool sustained ~70 TFLOP/s",
+                "peak_source": f"derived: {sm_count} SMs x 128 FP32 lanes x 2 flop x {NOMINAL_SM_MHZ:.0f} MHz (DESIGN.md)",
+                "peak_measured_ffma": peak_measured, "frac_of_measured": achieved / peak_measured,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter,
                 "kernel_ms": grav_ms, "interactions_per_s_kernel": inter / (grav_ms * 1e-3),
                 "build_ms": float(t_build.mean())}

@@ -129,6 +129,11 @@ otoo_status otoo_export_group_stats(otoo_ctx* ctx, uint32_t* d_ntests, uint32_t*
                                     uint32_t* d_nparts);
 otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
 
+/* Measurement aid: the FP32 rate the FMA pipe of this GPU sustains (FFMA2-only kernel, 16 independent
+ * chains per thread, ~20 ms), in TFLOP/s, counted 2 flop per lane FMA -- the measured denominator of the
+ * force kernel's roofline next to the nominal SMs x 128 x 2 x clock.  Synchronises. */
+otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* stream);
+
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).

@@ -26,7 +26,7 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host", "otoo_gravity_delta"]
+           "otoo_gravity_host", "otoo_gravity_delta", "otoo_measure_fp32_peak"]
 
 
 class TreeInfo(C.Structure):
@@ -63,6 +63,7 @@ _lib.otoo_export_sph_radii.argtypes = [_vp, _vp, _vp]
 _lib.otoo_export_group_stats.argtypes = [_vp, _vp, _vp, _vp]
 _lib.otoo_last_stats.argtypes = [_vp, C.POINTER(Stats)]
 _lib.otoo_set_option.argtypes = [_vp, C.c_char_p, _i64]
+_lib.otoo_measure_fp32_peak.argtypes = [_vp, C.POINTER(C.c_double), _vp]
 _lib.otoo_gravity_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _i32, _vp]
 
 
@@ -209,6 +210,11 @@ class Otoo:
         s = Stats()
         self._check(_lib.otoo_last_stats(self._h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def otoo_measure_fp32_peak(self, stream=None) -> float:
+        v = C.c_double(0.0)
+        self._check(_lib.otoo_measure_fp32_peak(self._h, C.byref(v), _stream(stream)))
+        return float(v.value)
 
     def otoo_set_option(self, name: str, value: int):
         self._check(_lib.otoo_set_option(self._h, name.encode(), int(value)))

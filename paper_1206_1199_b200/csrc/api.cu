@@ -274,6 +274,12 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
   return OTOO_OK;
 }
 
+otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* stream) {
+  if (!ctx || !host_tflops) return OTOO_ERR_INVALID_ARG;
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  return otoo_measure_fp32_peak_impl(ctx, host_tflops, (cudaStream_t)stream);
+}
+
 otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   if (!ctx || !name) return OTOO_ERR_INVALID_ARG;
   if (strcmp(name, "walk_stack") == 0) {

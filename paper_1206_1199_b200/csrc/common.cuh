@@ -141,3 +141,4 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
 otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups);
 otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps);
 size_t otoo_walk_smem_bytes();
+otoo_status otoo_measure_fp32_peak_impl(otoo_ctx* ctx, double* tflops, cudaStream_t st);

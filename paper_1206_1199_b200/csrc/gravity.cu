@@ -433,3 +433,47 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   ctx->walked = true;
   return OTOO_OK;
 }
+
+// ---------------------------------------------------------------- the FP32 roofline denominator, measured
+// 16 independent FFMA2 chains per thread, 8 warps per scheduler: what the FMA pipe of this GPU sustains at
+// the clock it holds (bench.py reports the kernel against the nominal peak AND against this number).
+namespace {
+__global__ void __launch_bounds__(256) fp32_peak_kernel(float2* out, int iters, float2 a) {
+  float2 acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = make_float2((float)(threadIdx.x + i), (float)i);
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc[i] = __ffma2_rn(acc[i], a, acc[i]);   // one register pair + one uniform operand:
+                                                                          // three distinct pairs lose 15-25 % to the register banks
+  }
+  float2 s = make_float2(0.0f, 0.0f);
+#pragma unroll
+  for (int i = 0; i < 16; i++) { s.x += acc[i].x; s.y += acc[i].y; }
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+otoo_status otoo_measure_fp32_peak_impl(otoo_ctx* ctx, double* tflops, cudaStream_t st) {
+  const int grid = ctx->sm_count * 8, iters = 20000;
+  float2* out = reinterpret_cast<float2*>(ctx->key[1]);          // scratch: 8 B x grid x 256 <= capacity of key[1]?
+  float2* tmp = nullptr;
+  if ((int64_t)grid * 256 > ctx->maxN) { OTOO_CUDA(ctx, cudaMalloc((void**)&tmp, sizeof(float2) * (size_t)grid * 256)); out = tmp; }
+  cudaEvent_t e0, e1;
+  OTOO_CUDA(ctx, cudaEventCreate(&e0)); OTOO_CUDA(ctx, cudaEventCreate(&e1));
+  fp32_peak_kernel<<<grid, 256, 0, st>>>(out, 200, make_float2(-1e-6f, -1e-6f));
+  float best = 1e30f;
+  for (int r = 0; r < 3; r++) {
+    cudaEventRecord(e0, st);
+    fp32_peak_kernel<<<grid, 256, 0, st>>>(out, iters, make_float2(-1e-6f, -1e-6f));
+    cudaEventRecord(e1, st);
+    cudaEventSynchronize(e1);
+    float ms = 0.0f; cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (tmp) cudaFree(tmp);
+  OTOO_CUDA(ctx, cudaGetLastError());
+  *tflops = (double)grid * 256.0 * 16.0 * 2.0 * 2.0 * (double)iters / ((double)best * 1e-3) / 1e12;
+  return OTOO_OK;
+}
