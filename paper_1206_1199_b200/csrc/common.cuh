@@ -141,4 +141,7 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
 otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups);
 otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps);
 size_t otoo_walk_smem_bytes();
+__host__ __device__ constexpr size_t otoo_walk_smem_bytes_dev() {   // lists + stacks of the one-warp-does-both walk kernels
+  return (size_t)OTOO_WALK_WARPS * (OTOO_LIST_STRIDE * 16 + OTOO_WALK_STACK_MAX * 4);
+}
 otoo_status otoo_measure_fp32_peak_impl(otoo_ctx* ctx, double* tflops, cudaStream_t st);

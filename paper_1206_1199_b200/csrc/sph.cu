@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(256) gather_force_inputs_kernel(const float* _
   if (s >= n) return;
   uint32_t i = perm[s];
   float r = rho[i];
-  aux[s] = make_float4(h[i], __fdiv_rn(P[i], __fmul_rn(r, r)), 0.0f, 0.0f);
+  aux[s] = make_float4(h[i], __fdiv_rn(P[i], __fmul_rn(r, r)), __fmul_rn(h[i], h[i]), 0.0f);   // (h, P/rho^2, h^2, -)
   if (vel) svel[s] = vel[i];
 }
 
@@ -159,7 +159,7 @@ struct SphVisitor {
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass
-    if (E >= 2) dst[1] = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+    if (E >= 2) dst[1] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);
     if (E >= 3) dst[2] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
@@ -168,48 +168,103 @@ struct SphVisitor {
     if (!p.c.walk_only) eval(list, n);
     return list;
   }
+  // Only ~2 % of the (target, candidate) pairs are neighbours (C4: 5.6e9 candidates, 1.1e8 true pairs), so the
+  // list is consumed in two passes.  Pass 1: the fp32 neighbour decision of R16/R17 alone (6 FP32 operations
+  // + compare per pair), one result bit per pair, 32 candidates per mask word and target, words parked in
+  // shared memory.  Pass 2: every lane walks the set bits of its own targets and evaluates the kernel for
+  // those pairs only; the warp runs as many rounds as its busiest lane has hits.
+  static constexpr int CAPE = (OTOO_LIST_CAP / E) & ~3, W = (CAPE + 31) / 32;
+  uint32_t* msk;      // this warp's mask words in shared memory: [W][T][32 lanes]
+  int lane_;
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
-    const float PI_F = 3.14159265358979323846f;
-    for (int j = 0; j < n; j++) {
-      const float4 a = list[E * j];
-      float4 b = make_float4(0, 0, 0, 0), c = make_float4(0, 0, 0, 0);
-      if (E >= 2) b = list[E * j + 1];
-      if (E >= 3) c = list[E * j + 2];
+    int w = 0;
+    for (int jb = 0; jb < n; jb += 32, w++) {
+      uint32_t mk[T];
+#pragma unroll
+      for (int t = 0; t < T; t++) mk[t] = 0u;
+      const int nb = n - jb < 32 ? n - jb : 32;
+#pragma unroll 4
+      for (int k = 0; k < nb; k++) {
+        const float4 a = list[E * (jb + k)];
+        float hj2 = 0.0f;
+        if (MODE != 0) hj2 = list[E * (jb + k) + 1].z;
+        // exactly this chain on (x_j - x_i): both sides take the neighbour decision in fp32 (R16, R17);
+        // two targets per packed instruction (FADD2 / FMUL2 / FFMA2 round each half like the scalar forms)
+#pragma unroll
+        for (int q = 0; q < T / 2; q++) {
+          const float2 ex = __fadd2_rn(make_float2(a.x, a.x), make_float2(-px[2 * q], -px[2 * q + 1]));
+          const float2 ey = __fadd2_rn(make_float2(a.y, a.y), make_float2(-py[2 * q], -py[2 * q + 1]));
+          const float2 ez = __fadd2_rn(make_float2(a.z, a.z), make_float2(-pz[2 * q], -pz[2 * q + 1]));
+          const float2 r2 = __ffma2_rn(ez, ez, __ffma2_rn(ey, ey, __fmul2_rn(ex, ex)));
+          // r2 < lim  <=>  the sign bit of fl32(r2 - lim) (exact: the difference of two floats is negative iff
+          // the first is smaller); one funnel shift appends it to the mask word
+          const float l0 = MODE == 0 ? h2[2 * q] : fmaxf(h2[2 * q], hj2), l1 = MODE == 0 ? h2[2 * q + 1] : fmaxf(h2[2 * q + 1], hj2);
+          const float2 d = __fadd2_rn(r2, make_float2(-l0, -l1));
+          mk[2 * q] = __funnelshift_l(__float_as_uint(d.x), mk[2 * q], 1);
+          mk[2 * q + 1] = __funnelshift_l(__float_as_uint(d.y), mk[2 * q + 1], 1);
+        }
+        if (T & 1) {
+          const int t = T - 1;
+          const float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
+          const float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
+          const float lim = MODE == 0 ? h2[t] : fmaxf(h2[t], hj2);
+          mk[t] = __funnelshift_l(__float_as_uint(__fsub_rn(r2, lim)), mk[t], 1);
+        }
+      }
 #pragma unroll
       for (int t = 0; t < T; t++) {
-        // the fp32 neighbour decision of R16/R17: exactly this chain on (x_j - x_i)
-        float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
-        float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
-        if (MODE == 0) {
-          bool in = r2 < h2[t];
-          float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
-          float u = 1.0f - q;
-          float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
-          float w2 = 2.0f * u * u * u;
-          float w = q <= 0.5f ? w1 : w2;
-          o0[t] = fmaf(in ? a.w : 0.0f, w, o0[t]);
-          cnt_ngb[t] += in ? 1u : 0u;
-        } else {
-          float hj = b.x, hm = fmaxf(ph[t], hj);
-          bool in = (r2 < __fmul_rn(hm, hm)) && (r2 > 0.0f);
-          float rinv = rsqrt_approx(fmaxf(r2, 1e-37f));
-          float r = r2 * rinv;
-          float hjinv = __fdividef(1.0f, hj);
-          float qi = r * hinv[t], qj = r * hjinv;
-          float ui = 1.0f - qi, uj = 1.0f - qj;
-          float di = qi <= 0.5f ? fmaf(18.0f * qi, qi, -12.0f * qi) : (qi < 1.0f ? -6.0f * ui * ui : 0.0f);
-          float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
-          float hi2 = hinv[t] * hinv[t], hj2 = hjinv * hjinv;
-          float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2 * hj2) * rinv;   // (dW_i + dW_j)/(2r)
-          float f = in ? a.w * (ppr[t] + b.y) * gw : 0.0f;
-          // a_i -= f (x_i - x_j)  =  += f e
-          o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
-          if (MODE == 2) {
-            // (v_i - v_j).(x_i - x_j) = -(v_i - v_j).e
-            float vd = -fmaf(vx[t] - c.x, ex, fmaf(vy[t] - c.y, ey, (vz[t] - c.z) * ez));
-            o3[t] = fmaf(0.5f * f, vd, o3[t]);
-          }
-        }
+        mk[t] <<= 32 - nb;                       // candidate k of the word sits at bit 31 - k
+        if (MODE == 0) cnt_ngb[t] += (uint32_t)__popc(mk[t]);
+        msk[(w * T + t) * 32 + lane_] = mk[t];
+      }
+    }
+    const int nw = w;
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      int ww = 0;
+      uint32_t m = msk[t * 32 + lane_];
+      for (;;) {
+        while (m == 0u && ++ww < nw) m = msk[(ww * T + t) * 32 + lane_];
+        if (m == 0u) break;
+        const int k = __clz(m);
+        m &= ~(0x80000000u >> k);
+        hit(list, (ww << 5) + k, t);
+      }
+    }
+  }
+  // one neighbour pair: cubic spline (R13), density term (R16) or symmetric pressure term (R17)
+  __device__ __forceinline__ void hit(const float4* __restrict__ list, int j, int t) {
+    const float PI_F = 3.14159265358979323846f;
+    const float4 a = list[E * j];
+    const float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
+    const float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
+    if (MODE == 0) {
+      float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
+      float u = 1.0f - q;
+      float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
+      float w2 = 2.0f * u * u * u;
+      o0[t] = fmaf(a.w, q <= 0.5f ? w1 : w2, o0[t]);
+    } else {
+      const float4 b = list[E * j + 1];
+      if (!(r2 > 0.0f)) return;                  // the target itself / coincident points: no force (R17)
+      float hj = b.x;
+      float rinv = rsqrt_approx(r2);
+      float r = r2 * rinv;
+      float hjinv = __fdividef(1.0f, hj);
+      float qi = r * hinv[t], qj = r * hjinv;
+      float ui = 1.0f - qi, uj = 1.0f - qj;
+      float di = qi <= 0.5f ? fmaf(18.0f * qi, qi, -12.0f * qi) : (qi < 1.0f ? -6.0f * ui * ui : 0.0f);
+      float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
+      float hi2 = hinv[t] * hinv[t], hj2i = hjinv * hjinv;
+      float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2i * hj2i) * rinv;   // (dW_i + dW_j)/(2r)
+      float f = a.w * (ppr[t] + b.y) * gw;
+      // a_i -= f (x_i - x_j)  =  += f e
+      o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
+      if (MODE == 2) {
+        const float4 c = list[E * j + 2];
+        // (v_i - v_j).(x_i - x_j) = -(v_i - v_j).e
+        float vd = -fmaf(vx[t] - c.x, ex, fmaf(vy[t] - c.y, ey, (vz[t] - c.z) * ez));
+        o3[t] = fmaf(0.5f * f, vd, o3[t]);
       }
     }
   }
@@ -242,13 +297,17 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const Sp
   uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
   SphVisitor<T, MODE> v(p);
+  v.msk = reinterpret_cast<uint32_t*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (SphVisitor<T, MODE>::W * T * 32);
+  v.lane_ = lane;
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
 
 template <int MODE>
 otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_t smem, cudaStream_t st) {
   int occ = 1;
+  const size_t smem0 = smem;
 #define OTOO_SPH_CASE(TT)                                                                                              \
+  smem = smem0 + (size_t)OTOO_WALK_WARPS * SphVisitor<TT, MODE>::W * TT * 32 * sizeof(uint32_t);   /* + the mask words */   \
   OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_kernel<TT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_kernel<TT, MODE>, OTOO_WALK_WARPS * 32, smem));  \
   if (occ < 1) occ = 1;                                                                                                 \
