@@ -29,6 +29,16 @@ from workloads import generators as gen  # noqa: E402
 METRIC = "gravity_interactions_per_s"
 UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 20
+BUILD_BYTES_PER_PARTICLE = 390      # algorithmic HBM bytes of the tree build per particle
+
+
+def hbm_peak_gbs():
+    """measured HBM copy bandwidth of this pool (driver-written MEASURED_PEAKS.json), else the guide's fallback"""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except Exception:
+        return 6650.0, "fallback of B200_PROFILING.md"
 SM_LANES = 128                      # FP32 lanes per SM
 NOMINAL_SM_MHZ = 1965.0
 
@@ -244,6 +254,34 @@ def main():
                 "build_ms": float(t_build.mean())}
 
     mac_txt = f"theta={cfg['theta']}" if args.mac == "theta" else f"Delta-MAC delta={delta:g} m_limit={m_limit:g}"
+    hbm, hbm_src = hbm_peak_gbs()
+    build_ms = float(t_build.mean())
+    build_gbs = BUILD_BYTES_PER_PARTICLE * n / (build_ms * 1e-3) / 1e9
+    build_info = {"ms": build_ms, "bound": "hbm", "algorithmic_bytes": BUILD_BYTES_PER_PARTICLE * n, "achieved_gbs": build_gbs,
+                  "peak_gbs": hbm, "frac": build_gbs / hbm, "peak_source": hbm_src}
+    sph_info = None
+    if cfg["kind"] == "wd_pair" and world == 1:
+        # BASELINE config 4: the SPH rows (H11-H13) on the same tree, timed like the gravity step
+        w = gen.wd_pair(n, replicas.replica_seed(args.seed, rank))
+        d_h, d_u, d_v = (torch.from_numpy(w[k]).cuda() for k in ("h", "u", "vel"))
+        Gs = cfg.get("group_sph", 64)
+        ts = []
+        for it in range(3 + args.steps):
+            flush_buf.fill_(1)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            ev[0].record()
+            rho, nn = o.otoo_sph_density(d_h, Gs)
+            P = o.otoo_eos_ideal(rho, d_u, 5.0 / 3.0)
+            ev[1].record()
+            o.otoo_sph_force(d_h, rho, P, Gs, vel=d_v)
+            ev[2].record()
+            torch.cuda.synchronize()
+            if it >= 3:
+                ts.append((ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])))
+        cand = o.otoo_last_stats()["sum_interactions"]
+        td, tf = float(np.mean([x[0] for x in ts])), float(np.mean([x[1] for x in ts]))
+        sph_info = {"group": Gs, "density_eos_ms": td, "force_dudt_ms": tf, "candidate_pairs_per_pass": cand,
+                    "neighbour_pairs": int(nn.sum().item()), "candidate_pairs_per_s": 2 * cand / ((td + tf) * 1e-3)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -255,7 +293,9 @@ def main():
             "interactions_per_step": inter_all, "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
                     "ms_per_step": e2e_ms},
-            "gpu_launches": int(launches_step * args.steps), "roofline": roofline}
+            "gpu_launches": int(launches_step * args.steps), "roofline": roofline, "build": build_info}
+    if sph_info:
+        line["sph"] = sph_info
 
     if not args.no_cpu_baseline and world == 1:
         from oracle import oracle
