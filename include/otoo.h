@@ -144,6 +144,9 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
  * "warp_specialized" = 1 (default): otoo_gravity runs walker/evaluator warp pairs (walker warps build
  * the lists in shared memory, evaluator warps hold the targets and sum), 0: one warp does both in turn.
  * Same lists, same counters; sums differ in rounding order only.
+ * "warp_specialized_sph" = 0 (default): the SPH kernels let one warp walk and sum in turn; 1: walker/evaluator
+ * pairs as for gravity (SPH lists are short, the walkers become the bottleneck: faster only for
+ * group_size >= 128).
  * "walk_only" = 1: the walks build and count their lists but skip the pair sums (outputs are
  * meaningless; counters exact) -- measures the walk's share of the fused kernel; default 0.
  * Unknown names: OTOO_ERR_INVALID_ARG. */

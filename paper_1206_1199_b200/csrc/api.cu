@@ -295,6 +295,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "warp_specialized") == 0) { ctx->use_ws = value != 0; return OTOO_OK; }
+  if (strcmp(name, "warp_specialized_sph") == 0) { ctx->use_ws_sph = value != 0; return OTOO_OK; }
   return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");
 }
 

@@ -98,6 +98,7 @@ struct otoo_ctx {
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int walk_only;         // option "walk_only" (diagnostic)
   int use_ws;            // option "warp_specialized": gravity walk with walker/evaluator warp pairs
+  int use_ws_sph;        // option "warp_specialized_sph": the same split for the SPH kernels (default off)
   int last_group_size;
   int64_t last_ngroups;
   int launches;          // kernels launched by the current/last API call

@@ -1,7 +1,7 @@
 // sph.cu -- SPH cell radii (Eq. 5; R14), SPH group walk (R15) fused with the
 // density sum (Eq. 4; R13, R16) and the symmetric pressure force (L252 step 6; R17).
 // "There is no particle-cell interaction in SPH" (L105): the walk only produces a particle list.
-#include "walk.cuh"
+#include "walk_ws.cuh"
 
 namespace {
 
@@ -302,6 +302,160 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const Sp
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
 
+
+// ---------------------------------------------------------------- warp-specialised form (walk_ws.cuh)
+// Walker-side visitor: the SPH MAC (R15) and the list entries of SphVisitor without targets or sums;
+// submit() publishes the filled buffer to the pair's evaluator warp and returns the next one.
+template <int T_, int MODE>
+struct SphWalker {
+  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
+  static constexpr bool SUBMIT_LAST = true;
+  typedef WsPair<2> Pair;
+  const SphParams& p;
+  Pair& sm;
+  float glo[3], ghi[3], hmax;
+  uint32_t group, buf, eparity, first;
+  int lane_;
+  __device__ __forceinline__ SphWalker(const SphParams& p_, Pair& sm_, int lane) : p(p_), sm(sm_), buf(0), eparity(~0u), first(0), lane_(lane) {}
+  __device__ __forceinline__ float4* acquire() {
+    mbar_wait<500>(&sm.empty[buf], (eparity >> buf) & 1u);
+    eparity ^= 1u << buf;
+    return sm.list[buf];
+  }
+  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4*) {
+    hmax = 0.0f;
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      int64_t s = g0 + t * 32 + lane;
+      s = s < p.c.N ? s : g0;
+      float4 v = p.c.spos[s];
+      hmax = fmaxf(hmax, MODE == 0 ? p.hs[s] : p.aux[s].x);
+      if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
+      else {
+        glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
+        glo[1] = fminf(glo[1], v.y); ghi[1] = fmaxf(ghi[1], v.y);
+        glo[2] = fminf(glo[2], v.z); ghi[2] = fmaxf(ghi[2], v.z);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
+        ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
+      }
+      hmax = fmaxf(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, o));
+    }
+    first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+  }
+  __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
+    A = __ldg(p.c.cell_cm + cell);
+    B = __ldg(p.c.cell_b + cell);
+    float2 rr = __ldg(p.c_sph + cell);
+    float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
+    float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));
+    return d2 <= __fmul_rn(R, R) ? 2 : 0;
+  }
+  struct Entry { float4 v[E]; };
+  __device__ __forceinline__ Entry get(uint32_t s) const {
+    Entry e;
+    e.v[0] = p.c.spos[s];
+    if (E >= 2) e.v[1] = p.aux[s];
+    if (E >= 3) e.v[2] = p.svel[s];
+    return e;
+  }
+  __device__ __forceinline__ void put(float4* dst, const Entry& e) const {
+#pragma unroll
+    for (int k = 0; k < E; k++) dst[k] = e.v[k];
+  }
+  __device__ __forceinline__ void pad(float4* dst) {
+    dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);
+    if (E >= 2) dst[1] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);
+    if (E >= 3) dst[2] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
+  __device__ __forceinline__ float4* submit(float4*, int n, bool last) {
+    if (lane_ == 0) sm.meta[buf] = WsMeta{(uint32_t)n, first | (last ? WS_LAST : 0u), group, 0u};
+    first = 0;
+    mbar_arrive(&sm.full[buf]);
+    buf = (buf + 1) % OTOO_WS_NBUF;
+    return acquire();
+  }
+  __device__ __forceinline__ void store(int64_t, int) {}
+  __device__ __forceinline__ void finish() {
+    if (lane_ == 0) sm.meta[buf] = WsMeta{0u, WS_EXIT, 0u, 0u};
+    mbar_arrive(&sm.full[buf]);
+  }
+};
+
+template <int T, int MODE>
+__global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, T >= 8 ? 2 : 3) walk_sph_ws_kernel(const SphParams p) {
+  typedef typename SphWalker<T, MODE>::Pair Pair;
+  typedef SphVisitor<T, MODE> Eval;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  Pair* pairs = reinterpret_cast<Pair*>(smem_raw);
+  uint32_t* masks = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WS_PAIRS * sizeof(Pair));
+  if (threadIdx.x < OTOO_WS_PAIRS) {
+    Pair& s = pairs[threadIdx.x];
+#pragma unroll
+    for (int b = 0; b < OTOO_WS_NBUF; b++) { mbar_init(&s.full[b], 32); mbar_init(&s.empty[b], 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp >= OTOO_WS_PAIRS) {
+    if (T >= 8) setmaxnreg_dec<80>(); else setmaxnreg_dec<48>();
+    Pair& sm = pairs[warp - OTOO_WS_PAIRS];
+    SphWalker<T, MODE> w(p, sm, lane);
+    float4* list = w.acquire();
+    walk_driver(p.c, w, list, sm.stk, lane, (int64_t)blockIdx.x * OTOO_WS_PAIRS + (warp - OTOO_WS_PAIRS));
+    w.finish();
+  } else {
+    if (T >= 8) setmaxnreg_inc<176>(); else setmaxnreg_inc<112>();
+    Pair& sm = pairs[warp];
+    Eval v(p);
+    v.msk = masks + warp * (Eval::W * T * 32);
+    v.lane_ = lane;
+    uint32_t buf = 0, fparity = 0;
+    for (;;) {
+      mbar_wait(&sm.full[buf], (fparity >> buf) & 1u);
+      fparity ^= 1u << buf;
+      const WsMeta m = sm.meta[buf];
+      if (m.flags & WS_EXIT) break;
+      const int64_t g0 = (int64_t)m.group * (32 * T);
+      if (m.flags & WS_FIRST) v.load_group(g0, lane, nullptr);
+      if (!p.c.walk_only && m.count) v.eval(sm.list[buf], (int)m.count);
+      __syncwarp();
+      if (m.flags & WS_LAST) v.store(g0, lane);
+      mbar_arrive(&sm.empty[buf]);
+      buf = (buf + 1) % OTOO_WS_NBUF;
+    }
+  }
+}
+
+template <int T, int MODE>
+otoo_status launch_sph_ws2(otoo_ctx* ctx, const SphParams& p, cudaStream_t st) {
+  const size_t smem = OTOO_WS_PAIRS * (sizeof(typename SphWalker<T, MODE>::Pair) + (size_t)SphVisitor<T, MODE>::W * T * 32 * sizeof(uint32_t));
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_ws_kernel<T, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 1;
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_ws_kernel<T, MODE>, OTOO_WS_PAIRS * 64, smem));
+  if (occ < 1) occ = 1;
+  int64_t grid = (int64_t)ctx->sm_count * occ;
+  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups, OTOO_WS_PAIRS);
+  walk_sph_ws_kernel<T, MODE><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
+  return OTOO_OK;
+}
+template <int MODE>
+otoo_status launch_sph_ws(otoo_ctx* ctx, const SphParams& p, int G, cudaStream_t st) {
+  switch (G) {
+    case 32: return launch_sph_ws2<1, MODE>(ctx, p, st);
+    case 64: return launch_sph_ws2<2, MODE>(ctx, p, st);
+    case 128: return launch_sph_ws2<4, MODE>(ctx, p, st);
+    case 256: return launch_sph_ws2<8, MODE>(ctx, p, st);
+    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  }
+}
+
 template <int MODE>
 otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_t smem, cudaStream_t st) {
   int occ = 1;
@@ -361,7 +515,7 @@ otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float*
   p.rho = d_rho; p.nngb = d_nngb;
   OTOO_CUDA(ctx, cudaMemsetAsync(d_rho, 0, 4 * (size_t)ctx->N, st));
   if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
-  OTOO_TRY(launch_sph<0>(ctx, p, G, grid, smem, st));
+  if (ctx->use_ws_sph) OTOO_TRY(launch_sph_ws<0>(ctx, p, G, st)); else OTOO_TRY(launch_sph<0>(ctx, p, G, grid, smem, st));
   ctx->launches += 1;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;
@@ -376,8 +530,9 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
                                                                           ctx->val[0], ctx->N, ctx->sorted_aux, ctx->sorted_vel);
   OTOO_CUDA(ctx, cudaMemsetAsync(d_acc, 0, 16 * (size_t)ctx->N, st));
   p.acc = reinterpret_cast<float4*>(d_acc);
-  if (d_vel) { p.svel = ctx->sorted_vel; OTOO_TRY(launch_sph<2>(ctx, p, G, grid, smem, st)); }
-  else OTOO_TRY(launch_sph<1>(ctx, p, G, grid, smem, st));
+  if (d_vel) p.svel = ctx->sorted_vel;
+  if (ctx->use_ws_sph) { if (d_vel) OTOO_TRY(launch_sph_ws<2>(ctx, p, G, st)); else OTOO_TRY(launch_sph_ws<1>(ctx, p, G, st)); }
+  else { if (d_vel) OTOO_TRY(launch_sph<2>(ctx, p, G, grid, smem, st)); else OTOO_TRY(launch_sph<1>(ctx, p, G, grid, smem, st)); }
   ctx->launches += 2;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;

@@ -193,8 +193,18 @@ def test_walk_stack_spill(otoo, orc):
         otoo.otoo_set_option("warp_specialized", 1)
 
 
+@pytest.mark.parametrize("ws", [1, 0])
 @pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
-def test_sph_parity(otoo, orc, n, G):
+def test_sph_parity(otoo, orc, n, G, ws):
+    """ws = 0: one warp walks and sums in turn (default); ws = 1: walker/evaluator warp pairs."""
+    otoo.otoo_set_option("warp_specialized_sph", ws)
+    try:
+        _sph_parity(otoo, orc, n, G)
+    finally:
+        otoo.otoo_set_option("warp_specialized_sph", 0)
+
+
+def _sph_parity(otoo, orc, n, G):
     w = gen.wd_pair(n, 1206)
     pm, h, u = w["pos_mass"], w["h"], w["u"]
     # the generator's rigid rotation has (v_i - v_j).(x_i - x_j) = 0 for every pair (du/dt would be
