@@ -81,6 +81,8 @@ def lib():
         L.orc_sph_density.restype = C.c_uint64
         L.orc_sph_density.argtypes = [vp, vp, i32, vp, vp, vp, vp]
         L.orc_sph_group_list.argtypes = [vp, vp, i32, i64, vp]
+        L.orc_sph_adapt_h.restype = i32
+        L.orc_sph_adapt_h.argtypes = [vp, vp, dbl, dbl, i32, i32, vp]
         L.orc_sph_force.restype = C.c_uint64
         L.orc_sph_force.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
         L.orc_W.restype = dbl
@@ -273,6 +275,13 @@ class Tree:
         tot = lib().orc_sph_density_sel(self._h, _p(h), int(group_size), _p(sel), 0 if sel is None else len(sel),
                                         _p(rho), _p(nngb), _p(nt), _p(npart))
         return dict(rho=rho, nngb=nngb, n_tests=nt, n_parts=npart, candidates=int(tot))
+
+    def sph_adapt_h(self, h, n_target, tol, max_iter, group_size):
+        """reading R21: returns (h after the iteration, neighbour counts of that h, iterations done)"""
+        h = _f32(h, (self.N,)).copy()
+        nngb = np.zeros(self.N, dtype=np.uint32)
+        it = lib().orc_sph_adapt_h(self._h, _p(h), float(n_target), float(tol), int(max_iter), int(group_size), _p(nngb))
+        return h, nngb, int(it)
 
     def sph_group_list(self, h, group_size, g, n_parts):
         h = _f32(h, (self.N,))

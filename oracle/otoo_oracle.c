@@ -685,6 +685,54 @@ uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, 
                          uint32_t* n_tests, uint32_t* n_parts) {
   return orc_sph_density_sel(t, h, G, NULL, 0, rho, nngb, n_tests, n_parts);
 }
+/* ---------------- adaptive smoothing length ("h for each particle variable", L246; BASELINE config 4
+ * "adaptive to ~50 neighbours"; no rule in the paper).  Reading R21: per-particle root search on the
+ * neighbour count n_i(h_i) of R16 (self included; a monotone step function of h_i alone).  Every iteration
+ * counts neighbours with the current h; a particle with |n_i - n_target| <= tol is settled; otherwise its
+ * bracket is updated (n_i < n_target: lo_i = h_i, else hi_i = h_i) and
+ *   both ends known:  h_i <- fl32(0.5f * fl32(lo_i + hi_i))   (bisection; if that equals an end, settled)
+ *   else:             h_i <- fl32( h_i * clamp(1 + (n_target - n_i) / (3 n_i), 0.7, 1.3) )   in fp64
+ * (the first-order form of (n_target/n_i)^(1/3); only IEEE + - * /, so both sides get the same bits).
+ * Stops when every particle is settled or after max_iter updates.  The tree is not rebuilt; radii (Eq. 5)
+ * and lists are recomputed every iteration.  Returns the number of updates; nngb_out = counts of the final h. */
+int orc_sph_adapt_h(const orc_tree* t, float* h, double n_target, double tol, int max_iter, int G, uint32_t* nngb_out) {
+  int64_t N = t->N;
+  uint32_t* n = (uint32_t*)malloc(4 * (N > 0 ? N : 1));
+  double* rho = (double*)malloc(8 * (N > 0 ? N : 1));
+  float* lo = (float*)calloc(N > 0 ? N : 1, 4);
+  float* hi = (float*)malloc(4 * (N > 0 ? N : 1));
+  unsigned char* settled = (unsigned char*)calloc(N > 0 ? N : 1, 1);
+  for (int64_t i = 0; i < N; i++) hi[i] = INFINITY;
+  int it = 0;
+  for (;;) {
+    orc_sph_density(t, h, G, rho, n, NULL, NULL);
+    int64_t bad = 0;
+    for (int64_t i = 0; i < N; i++) {
+      if (!(fabs((double)n[i] - n_target) > tol)) settled[i] = 1;     /* also re-settles nothing: h_i is frozen once settled */
+      if (!settled[i]) bad++;
+    }
+    if (bad == 0 || it >= max_iter) break;
+    for (int64_t i = 0; i < N; i++) {
+      if (settled[i]) continue;
+      double ni = (double)n[i];
+      if (ni < n_target) lo[i] = h[i]; else hi[i] = h[i];
+      if (lo[i] > 0.0f && hi[i] < INFINITY) {
+        float mid = 0.5f * (lo[i] + hi[i]);
+        if (mid == lo[i] || mid == hi[i]) settled[i] = 1;             /* the step jumps over the band */
+        else h[i] = mid;
+      } else {
+        double f = 1.0 + (n_target - ni) / (3.0 * ni);                  /* n_i >= 1: the particle itself */
+        if (f < 0.7) f = 0.7;
+        if (f > 1.3) f = 1.3;
+        h[i] = (float)((double)h[i] * f);
+      }
+    }
+    it++;
+  }
+  if (nngb_out) memcpy(nngb_out, n, 4 * N);
+  free(n); free(rho); free(lo); free(hi); free(settled);
+  return it;
+}
 void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uint32_t* part_slots) {
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);

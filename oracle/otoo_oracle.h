@@ -99,6 +99,9 @@ uint64_t orc_sph_density(const orc_tree*, const float* h, int group_size, double
                          uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
 uint64_t orc_sph_density_sel(const orc_tree*, const float* h, int group_size, const int64_t* sel,
                              int64_t nsel, double* rho, uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
+/* adaptive h (reading R21): iterate h in place towards n_target neighbours (+- tol); returns iterations */
+int orc_sph_adapt_h(const orc_tree*, float* h, double n_target, double tol, int max_iter, int group_size,
+                    uint32_t* nngb_out);
 /* candidate list of one SPH group (sorted slots) */
 void orc_sph_group_list(const orc_tree*, const float* h, int group_size, int64_t g,
                         uint32_t* part_slots);

@@ -121,3 +121,30 @@ def test_pressure_force(orc):
     o = tl.sph_force(hh, rhol, Plin, 64)["acc_dudt"]
     assert np.allclose(o[idx, 0], -0.1 / rhol[idx], rtol=0.05)
     assert np.abs(o[idx, 1:3]).max() < 1e-12
+
+
+def test_adaptive_h_iteration(orc):
+    """Reading R21 (h adapted to a neighbour count, BASELINE config 4 "~50 neighbours").
+    Pins: on random points every particle ends within the tolerance from starts 2x too small and too large;
+    a converged input is a fixed point (0 updates, h untouched); the returned counts are those of the
+    density pass; on a lattice, where the count is a known step function of h (27 for sqrt(3) < h <= 2,
+    33 for 2 < h <= sqrt(5)), interior particles end on the right step; max_iter caps the updates."""
+    pm = gen.uniform_cube(5000, 5)
+    n = len(pm)
+    t = orc.Tree(pm, 16)
+    for h0 in (0.07, 0.3):
+        h, nn, it = t.sph_adapt_h(np.full(n, h0, np.float32), 40.0, 2.0, 60, 32)
+        assert 0 < it < 40 and np.all(np.abs(nn.astype(float) - 40.0) <= 2.0)
+        assert np.array_equal(nn, t.sph_density(h, 32)["nngb"])
+        h2, nn2, it2 = t.sph_adapt_h(h, 40.0, 2.0, 60, 32)
+        assert it2 == 0 and np.array_equal(h2, h) and np.array_equal(nn2, nn)
+    h3, _, it3 = t.sph_adapt_h(np.full(n, 0.07, np.float32), 40.0, 2.0, 3, 32)
+    assert it3 == 3
+    k, a = 12, 1.0
+    lat = gen.lattice(k, a, 1.0)
+    tl = orc.Tree(lat, 8)
+    for h0 in (1.3, 3.2):
+        h, nn, it = tl.sph_adapt_h(np.full(len(lat), h0, np.float32), 33.0, 2.0, 80, 32)
+        inner = np.all((lat[:, :3] >= 3 * a) & (lat[:, :3] <= (k - 4) * a), axis=1)
+        assert it < 80 and np.all(nn[inner] == 33)
+        assert np.all((h[inner] > 2.0) & (h[inner] <= np.sqrt(5.0)))
