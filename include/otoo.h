@@ -103,6 +103,15 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
 otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho,
                              uint32_t* d_nngb, void* stream);
 
+/* Adaptive smoothing length (h is variable per particle; BASELINE config 4: "~50 neighbours";
+ * rule: DESIGN.md R21).  Iterates d_h (N floats, caller's order, IN/OUT) by a per-particle bracketed root
+ * search on the neighbour count of otoo_sph_density (self included) until every particle has
+ * |n_i - n_target| <= tol, its bracket has collapsed, or max_iter updates were made.  The tree is not
+ * rebuilt.  d_nngb (may be NULL): counts of the final h.  host_iters (may be NULL): updates made.
+ * Synchronises once per iteration (one 4-byte read). */
+otoo_status otoo_sph_adapt_h(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter,
+                             int group_size, uint32_t* d_nngb, int* host_iters, void* stream);
+
 /* SPH stage 2 (L252 step 6; R17): symmetric pressure force.  d_rho, d_P: N floats (P from the
  * caller's EOS).  d_vel: N x float4 or NULL.  d_acc_sph: N x float4 (ax, ay, az, w), w = du/dt
  * if d_vel != NULL else 0. */

@@ -538,3 +538,79 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
   ctx->walked = true;
   return OTOO_OK;
 }
+
+// ---------------------------------------------------------------- adaptive smoothing length (reading R21)
+namespace {
+// settle the particles whose count is within the tolerance, count the others
+__global__ void __launch_bounds__(256) adapt_check_kernel(const uint32_t* __restrict__ nngb, int64_t n, double n_target, double tol,
+                                                          const float* __restrict__ h, float* __restrict__ lo, float* __restrict__ hi,
+                                                          uint32_t* __restrict__ bad) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool unsettled = false;
+  if (i < n) {
+    if (lo[i] != hi[i]) {                                           // lo == hi marks a settled particle
+      if (!(fabs((double)nngb[i] - n_target) > tol)) lo[i] = hi[i] = h[i];
+      else unsettled = true;
+    }
+  }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, unsettled);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(bad, (uint32_t)__popc(m));
+}
+// one update of the bracketed root search, same operations as the oracle
+__global__ void __launch_bounds__(256) adapt_update_kernel(const uint32_t* __restrict__ nngb, int64_t n, double n_target,
+                                                           float* __restrict__ h, float* __restrict__ lo, float* __restrict__ hi) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || lo[i] == hi[i]) return;
+  const double ni = (double)nngb[i];
+  float l = lo[i], u = hi[i];
+  const float hc = h[i];
+  if (ni < n_target) l = hc; else u = hc;
+  if (l > 0.0f && u < INFINITY) {
+    const float mid = __fmul_rn(0.5f, __fadd_rn(l, u));
+    if (mid == l || mid == u) l = u = hc;                            // the count steps over the band: settled
+    else h[i] = mid;
+  } else {
+    double f = __dadd_rn(1.0, __ddiv_rn(__dsub_rn(n_target, ni), __dmul_rn(3.0, ni)));
+    if (f < 0.7) f = 0.7;
+    if (f > 1.3) f = 1.3;
+    h[i] = __double2float_rn(__dmul_rn((double)hc, f));
+  }
+  lo[i] = l; hi[i] = u;
+}
+__global__ void __launch_bounds__(256) adapt_init_kernel(int64_t n, float* __restrict__ lo, float* __restrict__ hi) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { lo[i] = 0.0f; hi[i] = INFINITY; }
+}
+}  // namespace
+
+otoo_status otoo_sph_adapt_h_impl(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter, int G, uint32_t* d_nngb,
+                                  int* host_iters, cudaStream_t st) {
+  const int64_t N = ctx->N;
+  // scratch inside sorted_aux (4 floats per particle, unused by the density pass): lo, hi, rho, counts
+  float* lo = reinterpret_cast<float*>(ctx->sorted_aux);
+  float* hi = lo + N;
+  float* rho = lo + 2 * N;
+  uint32_t* cnt = reinterpret_cast<uint32_t*>(lo + 3 * N);
+  uint32_t* bad = ctx->d_counters + 48;
+  const unsigned nb = (unsigned)cdiv(N, 256);
+  adapt_init_kernel<<<nb, 256, 0, st>>>(N, lo, hi);
+  int it = 0, launches = 1;
+  for (;;) {
+    OTOO_TRY(otoo_sph_density_impl(ctx, d_h, G, rho, cnt, st));
+    launches += ctx->launches; ctx->launches = 0;
+    OTOO_CUDA(ctx, cudaMemsetAsync(bad, 0, sizeof(uint32_t), st));
+    adapt_check_kernel<<<nb, 256, 0, st>>>(cnt, N, (double)n_target, (double)tol, d_h, lo, hi, bad);
+    OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 48, bad, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    OTOO_CUDA(ctx, cudaStreamSynchronize(st));
+    launches += 1;
+    if (ctx->h_counters[48] == 0 || it >= max_iter) break;
+    adapt_update_kernel<<<nb, 256, 0, st>>>(cnt, N, (double)n_target, d_h, lo, hi);
+    launches += 1;
+    it++;
+  }
+  if (d_nngb) OTOO_CUDA(ctx, cudaMemcpyAsync(d_nngb, cnt, 4 * (size_t)N, cudaMemcpyDeviceToDevice, st));
+  OTOO_CUDA(ctx, cudaGetLastError());
+  ctx->launches = launches;
+  if (host_iters) *host_iters = it;
+  return OTOO_OK;
+}

@@ -243,6 +243,27 @@ def _sph_parity(otoo, orc, n, G):
             assert np.all(out[:, 3] == 0)
 
 
+@pytest.mark.parametrize("kind,n,G,target,tol,h0", [("uniform_cube", 20000, 64, 40.0, 2.0, 0.03), ("wd", 16384 + 3, 32, 50.0, 3.0, None),
+                                                      ("uniform_cube", 5000, 128, 32.0, 0.0, 0.2)])
+def test_adaptive_h_parity(otoo, orc, kind, n, G, target, tol, h0):
+    """otoo_sph_adapt_h (reading R21): the same number of updates, the same h bit for bit, the same counts."""
+    if kind == "wd":
+        w = gen.wd_pair(n, 77)
+        pm, h = w["pos_mass"], (w["h"] * np.float32(0.6)).astype(np.float32)
+    else:
+        pm, h = gen.make(kind, n, 77), np.full(n, h0, np.float32)
+    t = check_tree(otoo, orc, pm, 16)
+    for max_iter in (2, 40):
+        href, nref, itref = t.sph_adapt_h(h, target, tol, max_iter, G)
+        d_h = dev(h.copy())
+        nn, it = otoo.otoo_sph_adapt_h(d_h, target, tol, max_iter, G)
+        assert it == itref
+        assert np.array_equal(d_h.cpu().numpy().view(np.uint32), href.view(np.uint32))
+        assert np.array_equal(nn.cpu().numpy().view(np.uint32), nref)
+    if tol > 0:
+        assert np.all(np.abs(nref.astype(float) - target) <= tol)
+
+
 def test_status_codes(otoo):
     from paper_1206_1199_b200 import binding
     fresh = binding.Otoo(max_particles=1000)
