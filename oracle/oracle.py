@@ -81,6 +81,8 @@ def lib():
         L.orc_sph_density.restype = C.c_uint64
         L.orc_sph_density.argtypes = [vp, vp, i32, vp, vp, vp, vp]
         L.orc_sph_group_list.argtypes = [vp, vp, i32, i64, vp]
+        L.orc_sph_divrot_sel.restype = C.c_uint64
+        L.orc_sph_divrot_sel.argtypes = [vp, vp, vp, i32, vp, i64, vp, vp, vp]
         L.orc_sph_adapt_h.restype = i32
         L.orc_sph_adapt_h.argtypes = [vp, vp, dbl, dbl, i32, i32, vp]
         L.orc_sph_force.restype = C.c_uint64
@@ -275,6 +277,18 @@ class Tree:
         tot = lib().orc_sph_density_sel(self._h, _p(h), int(group_size), _p(sel), 0 if sel is None else len(sel),
                                         _p(rho), _p(nngb), _p(nt), _p(npart))
         return dict(rho=rho, nngb=nngb, n_tests=nt, n_parts=npart, candidates=int(tot))
+
+    def sph_divrot(self, h, vel, group_size, groups=None):
+        """SPH stage 1 with velocity derivatives (reading R22): rho, (div v, rot v) per particle, caller's order"""
+        h = _f32(h, (self.N,))
+        v = _f32(vel, (self.N, 4))
+        sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
+        rho = np.zeros(self.N, dtype=np.float64)
+        out = np.zeros((self.N, 4), dtype=np.float64)
+        asum = np.zeros(self.N, dtype=np.float64)
+        tot = lib().orc_sph_divrot_sel(self._h, _p(h), _p(v), int(group_size), _p(sel), 0 if sel is None else len(sel),
+                                       _p(rho), _p(out), _p(asum))
+        return dict(rho=rho, divrot=out, abs_sum=asum, candidates=int(tot))
 
     def sph_adapt_h(self, h, n_target, tol, max_iter, group_size):
         """reading R21: returns (h after the iteration, neighbour counts of that h, iterations done)"""

@@ -685,6 +685,65 @@ uint64_t orc_sph_density(const orc_tree* t, const float* h, int G, double* rho, 
                          uint32_t* n_tests, uint32_t* n_parts) {
   return orc_sph_density_sel(t, h, G, NULL, 0, rho, nngb, n_tests, n_parts);
 }
+/* ---------------- SPH stage 1 with velocity derivatives (PAPER L252 step 4: "density, div v, rot v").  The paper
+ * prints no formula; reading R22: the standard gather estimates with the particle's own h,
+ *   div v_i = (1/rho_i) sum_j m_j (v_j - v_i) . grad_i W(r_ij, h_i)
+ *   rot v_i = (1/rho_i) sum_j m_j (v_i - v_j) x grad_i W(r_ij, h_i),   grad_i W = dW/dr (x_i - x_j)/r,
+ * over the neighbours of R16 (fp32 decision r^2 < h_i^2), r > 0, with rho_i of R16 (from the same pass).
+ * out: 4N doubles (div, rot_x, rot_y, rot_z), caller's order; abs_sum (N or NULL): sum_j m_j |v_j - v_i| |dW/dr| / rho_i. */
+uint64_t orc_sph_divrot_sel(const orc_tree* t, const float* h, const float* vel, int G, const int64_t* sel, int64_t nsel,
+                            double* rho, double* out, double* abs_sum) {
+  int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
+  float* hs = sorted_h(t, h);
+  float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
+  sph_radii_sorted(t, hs, bmax, rsph);
+  uint64_t total = 0;
+#pragma omp parallel reduction(+ : total)
+  {
+    lists_t L; memset(&L, 0, sizeof L);
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t gi = 0; gi < ng; gi++) {
+      int64_t g = sel ? sel[gi] : gi;
+      int64_t a = g * G, b = a + G < N ? a + G : N;
+      gbox_t box = group_box(t, a, b, hs);
+      L.np = 0; L.ntests = 0;
+      walk_sph(t, bmax, rsph, &box, 0, &L);
+      total += (uint64_t)(b - a) * (uint64_t)L.np;
+      for (int64_t s = a; s < b; s++) {
+        const float* pi = t->spos + 4 * s;
+        int64_t io = t->perm[s];
+        float hi = hs[s], h2 = hi * hi;
+        double r0 = 0, dv = 0, rx = 0, ry = 0, rz = 0, as = 0;
+        for (int64_t k = 0; k < L.np; k++) {
+          int64_t j = L.parts[k];
+          const float* pj = t->spos + 4 * j;
+          if (!(r2_f32(pi, pj) < h2)) continue;
+          double ex = (double)pi[0] - pj[0], ey = (double)pi[1] - pj[1], ez = (double)pi[2] - pj[2];   /* x_i - x_j */
+          double r = sqrt(ex * ex + ey * ey + ez * ez);
+          r0 += (double)pj[3] * orc_W(r, (double)hi);
+          if (r == 0.0) continue;
+          int64_t jo = t->perm[j];
+          double gw = orc_dWdr(r, (double)hi) / r;                                                   /* grad_i W = gw (x_i - x_j) */
+          double ux = (double)vel[4 * jo] - vel[4 * io], uy = (double)vel[4 * jo + 1] - vel[4 * io + 1],
+                 uz = (double)vel[4 * jo + 2] - vel[4 * io + 2];                                     /* v_j - v_i */
+          double m = pj[3];
+          dv += m * gw * (ux * ex + uy * ey + uz * ez);
+          /* (v_i - v_j) x grad W = -u x (gw e) = gw (e x u) */
+          rx += m * gw * (ey * uz - ez * uy);
+          ry += m * gw * (ez * ux - ex * uz);
+          rz += m * gw * (ex * uy - ey * ux);
+          as += m * fabs(gw) * r * sqrt(ux * ux + uy * uy + uz * uz);
+        }
+        if (rho) rho[io] = r0;
+        out[4 * io] = dv / r0; out[4 * io + 1] = rx / r0; out[4 * io + 2] = ry / r0; out[4 * io + 3] = rz / r0;
+        if (abs_sum) abs_sum[io] = as / r0;
+      }
+    }
+    free(L.parts); free(L.cells);
+  }
+  free(hs); free(bmax); free(rsph);
+  return total;
+}
 /* ---------------- adaptive smoothing length ("h for each particle variable", L246; BASELINE config 4
  * "adaptive to ~50 neighbours"; no rule in the paper).  Reading R21: per-particle root search on the
  * neighbour count n_i(h_i) of R16 (self included; a monotone step function of h_i alone).  Every iteration

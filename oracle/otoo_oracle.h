@@ -99,6 +99,9 @@ uint64_t orc_sph_density(const orc_tree*, const float* h, int group_size, double
                          uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
 uint64_t orc_sph_density_sel(const orc_tree*, const float* h, int group_size, const int64_t* sel,
                              int64_t nsel, double* rho, uint32_t* nngb, uint32_t* n_tests, uint32_t* n_parts);
+/* SPH stage 1 with velocity derivatives (PAPER L252 step 4; reading R22): out = 4N (div v, rot v), rho = N or NULL */
+uint64_t orc_sph_divrot_sel(const orc_tree*, const float* h, const float* vel /*4N*/, int group_size,
+                            const int64_t* sel, int64_t nsel, double* rho, double* out, double* abs_sum);
 /* adaptive h (reading R21): iterate h in place towards n_target neighbours (+- tol); returns iterations */
 int orc_sph_adapt_h(const orc_tree*, float* h, double n_target, double tol, int max_iter, int group_size,
                     uint32_t* nngb_out);

@@ -148,3 +148,35 @@ def test_adaptive_h_iteration(orc):
         inner = np.all((lat[:, :3] >= 3 * a) & (lat[:, :3] <= (k - 4) * a), axis=1)
         assert it < 80 and np.all(nn[inner] == 33)
         assert np.all((h[inner] > 2.0) & (h[inner] <= np.sqrt(5.0)))
+
+
+def test_div_and_rot_of_linear_velocity_fields(orc):
+    """Reading R22 (PAPER L252 step 4: "density, div v, rot v").  Pins: for v = A x the estimates are exactly
+    linear in A with one common factor c = -(1/(3 rho)) sum_j m_j r dW/dr (-> 1 as the sum -> integral, since
+    -int r W' d^3r = 3 int W = 3): on a lattice interior div v = c tr(A), rot v = c (A32-A23, A13-A31, A21-A12),
+    with c within a few per cent of 1; a uniform translation has div = rot = 0; the density is R16's."""
+    k, a = 12, 1.0
+    pm = gen.lattice(k, a, 1.0)
+    n = len(pm)
+    x = pm[:, :3].astype(np.float64)
+    h = np.full(n, 2.3 * a, np.float32)
+    t = orc.Tree(pm, 8)
+    inner = np.all((x >= 3 * a) & (x <= (k - 4) * a), axis=1)
+    A = np.array([[0.3, -0.7, 0.2], [0.5, -0.1, 0.9], [-0.4, 0.25, 0.6]])
+    vel = np.zeros((n, 4), np.float32)
+    vel[:, :3] = x @ A.T + np.array([5.0, -3.0, 1.0])              # + a uniform translation
+    r = t.sph_divrot(h, vel, 32)
+    assert np.allclose(r["rho"], t.sph_density(h, 32)["rho"], rtol=1e-14)
+    d = r["divrot"][inner]
+    c = d[:, 0] / np.trace(A)
+    assert np.allclose(c, c[0], rtol=1e-6) and abs(c[0] - 1.0) < 0.05
+    curl = np.array([A[2, 1] - A[1, 2], A[0, 2] - A[2, 0], A[1, 0] - A[0, 1]])
+    assert np.allclose(d[:, 1:], c[0] * curl, rtol=1e-5, atol=1e-7)
+    vel[:, :3] = np.array([5.0, -3.0, 1.0])
+    r0 = t.sph_divrot(h, vel, 32)
+    assert np.abs(r0["divrot"]).max() == 0.0
+    # rigid rotation: div = 0, rot = 2 Omega (times c)
+    Om = np.array([0.2, -0.5, 0.9])
+    vel[:, :3] = np.cross(Om, x)
+    rr = t.sph_divrot(h, vel, 32)["divrot"][inner]
+    assert np.abs(rr[:, 0]).max() < 1e-6 and np.allclose(rr[:, 1:], 2 * c[0] * Om, rtol=1e-5, atol=1e-7)
