@@ -103,6 +103,14 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
 otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho,
                              uint32_t* d_nngb, void* stream);
 
+/* SPH stage 1 as the paper runs it (PAPER.md L252 step 4: "density, div v, rot v"): the density pass of
+ * otoo_sph_density plus the gather estimates (R22)
+ *   div v_i = (1/rho_i) sum_j m_j (v_j - v_i) . grad_i W(r_ij, h_i),
+ *   rot v_i = (1/rho_i) sum_j m_j (v_i - v_j) x grad_i W(r_ij, h_i)
+ * over the same neighbours.  d_vel: N x float4 (vx, vy, vz, -).  d_divrot: N x float4 (div v, rot v). */
+otoo_status otoo_sph_stage1(otoo_ctx* ctx, const float* d_h, const float* d_vel, int group_size,
+                            float* d_rho, uint32_t* d_nngb, float* d_divrot, void* stream);
+
 /* Adaptive smoothing length (h is variable per particle; BASELINE config 4: "~50 neighbours";
  * rule: DESIGN.md R21).  Iterates d_h (N floats, caller's order, IN/OUT) by a per-particle bracketed root
  * search on the neighbour count of otoo_sph_density (self included) until every particle has

@@ -181,6 +181,18 @@ otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, fl
   return otoo_sph_density_impl(ctx, d_h, group_size, d_rho, d_nngb, (cudaStream_t)stream);
 }
 
+otoo_status otoo_sph_stage1(otoo_ctx* ctx, const float* d_h, const float* d_vel, int group_size, float* d_rho, uint32_t* d_nngb,
+                            float* d_divrot, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_h || !d_vel || !d_rho || !d_divrot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_h, d_vel, d_rho, d_divrot must not be NULL");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_TRY(sph_scratch(ctx));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_sph_stage1_impl(ctx, d_h, d_vel, group_size, d_rho, d_nngb, d_divrot, (cudaStream_t)stream);
+}
+
 otoo_status otoo_sph_adapt_h(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter, int group_size,
                              uint32_t* d_nngb, int* host_iters, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;

@@ -139,6 +139,8 @@ otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float*
                                   cudaStream_t st);
 otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,
                                 const float* d_vel, int G, float* d_acc, cudaStream_t st);
+otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d_vel, int G, float* d_rho, uint32_t* d_nngb,
+                                 float* d_divrot, cudaStream_t st);
 otoo_status otoo_sph_adapt_h_impl(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter, int G, uint32_t* d_nngb,
                                   int* host_iters, cudaStream_t st);
 otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups);

@@ -23,6 +23,19 @@ __global__ void __launch_bounds__(256) gather_force_inputs_kernel(const float* _
   if (vel) svel[s] = vel[i];
 }
 
+__global__ void __launch_bounds__(256) gather_vel_kernel(const float4* __restrict__ vel, const uint32_t* __restrict__ perm, int64_t n,
+                                                         float4* __restrict__ svel) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) svel[s] = vel[perm[s]];
+}
+// (div v, rot v) sums -> estimates: divide by the particle's density (R22)
+__global__ void __launch_bounds__(256) divrot_finish_kernel(const float* __restrict__ rho, int64_t n, float4* __restrict__ dr) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float r = rho[i];
+  float4 v = dr[i];
+  dr[i] = make_float4(__fdiv_rn(v.x, r), __fdiv_rn(v.y, r), __fdiv_rn(v.z, r), __fdiv_rn(v.w, r));
+}
 // ---- R14: b_max and r_SPH over ALL particles of every cell, from the fp64 centre of mass.
 // Each particle walks down its own root-to-leaf path; consecutive slots share cells, so a warp
 // first reduces runs of equal cell id with shuffles and only run heads touch memory.
@@ -92,12 +105,14 @@ struct SphParams {
 };
 
 // MODE 0: density (R16).  MODE 1: pressure force (R17).  MODE 2: pressure force + du/dt.
+// MODE 3: density + div v + rot v (SPH stage 1 of PAPER L252; R22).
 template <int T_, int MODE>
 struct SphVisitor {
-  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
+  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : 3);
+  static constexpr bool GATHER = MODE == 0 || MODE == 3;     // neighbours by the target's own h only (R16)
   const SphParams& p;
   float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
-  float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T];
+  float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T], o4[T];
   uint32_t cnt_ngb[T];
   float glo[3], ghi[3], hmax;
   __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_) {}
@@ -110,9 +125,9 @@ struct SphVisitor {
       s = s < p.c.N ? s : g0;
       float4 v = p.c.spos[s];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z;
-      if (MODE == 0) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
+      if (GATHER) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
       else { float4 a = p.aux[s]; ph[t] = a.x; ppr[t] = a.y; }
-      if (MODE == 2) { float4 w = p.svel[s]; vx[t] = w.x; vy[t] = w.y; vz[t] = w.z; } else { vx[t] = vy[t] = vz[t] = 0.0f; }
+      if (MODE >= 2) { float4 w = p.svel[s]; vx[t] = w.x; vy[t] = w.y; vz[t] = w.z; } else { vx[t] = vy[t] = vz[t] = 0.0f; }
       hmax = fmaxf(hmax, ph[t]);
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
@@ -133,7 +148,7 @@ struct SphVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) {
       h2[t] = __fmul_rn(ph[t], ph[t]); hinv[t] = 1.0f / ph[t];
-      o0[t] = o1[t] = o2[t] = o3[t] = 0.0f; cnt_ngb[t] = 0;
+      o0[t] = o1[t] = o2[t] = o3[t] = o4[t] = 0.0f; cnt_ngb[t] = 0;
     }
   }
   // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105)
@@ -149,7 +164,7 @@ struct SphVisitor {
   __device__ __forceinline__ Entry get(uint32_t s) const {
     Entry e;
     e.v[0] = p.c.spos[s];
-    if (E >= 2) e.v[1] = p.aux[s];
+    if (E >= 2) e.v[1] = MODE == 3 ? p.svel[s] : p.aux[s];
     if (E >= 3) e.v[2] = p.svel[s];
     return e;
   }
@@ -187,7 +202,7 @@ struct SphVisitor {
       for (int k = 0; k < nb; k++) {
         const float4 a = list[E * (jb + k)];
         float hj2 = 0.0f;
-        if (MODE != 0) hj2 = list[E * (jb + k) + 1].z;
+        if (!GATHER) hj2 = list[E * (jb + k) + 1].z;
         // exactly this chain on (x_j - x_i): both sides take the neighbour decision in fp32 (R16, R17);
         // two targets per packed instruction (FADD2 / FMUL2 / FFMA2 round each half like the scalar forms)
 #pragma unroll
@@ -198,7 +213,7 @@ struct SphVisitor {
           const float2 r2 = __ffma2_rn(ez, ez, __ffma2_rn(ey, ey, __fmul2_rn(ex, ex)));
           // r2 < lim  <=>  the sign bit of fl32(r2 - lim) (exact: the difference of two floats is negative iff
           // the first is smaller); one funnel shift appends it to the mask word
-          const float l0 = MODE == 0 ? h2[2 * q] : fmaxf(h2[2 * q], hj2), l1 = MODE == 0 ? h2[2 * q + 1] : fmaxf(h2[2 * q + 1], hj2);
+          const float l0 = GATHER ? h2[2 * q] : fmaxf(h2[2 * q], hj2), l1 = GATHER ? h2[2 * q + 1] : fmaxf(h2[2 * q + 1], hj2);
           const float2 d = __fadd2_rn(r2, make_float2(-l0, -l1));
           mk[2 * q] = __funnelshift_l(__float_as_uint(d.x), mk[2 * q], 1);
           mk[2 * q + 1] = __funnelshift_l(__float_as_uint(d.y), mk[2 * q + 1], 1);
@@ -207,14 +222,14 @@ struct SphVisitor {
           const int t = T - 1;
           const float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
           const float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
-          const float lim = MODE == 0 ? h2[t] : fmaxf(h2[t], hj2);
+          const float lim = GATHER ? h2[t] : fmaxf(h2[t], hj2);
           mk[t] = __funnelshift_l(__float_as_uint(__fsub_rn(r2, lim)), mk[t], 1);
         }
       }
 #pragma unroll
       for (int t = 0; t < T; t++) {
         mk[t] <<= 32 - nb;                       // candidate k of the word sits at bit 31 - k
-        if (MODE == 0) cnt_ngb[t] += (uint32_t)__popc(mk[t]);
+        if (GATHER) cnt_ngb[t] += (uint32_t)__popc(mk[t]);
         msk[(w * T + t) * 32 + lane_] = mk[t];
       }
     }
@@ -238,7 +253,21 @@ struct SphVisitor {
     const float4 a = list[E * j];
     const float ex = __fsub_rn(a.x, px[t]), ey = __fsub_rn(a.y, py[t]), ez = __fsub_rn(a.z, pz[t]);
     const float r2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
-    if (MODE == 0) {
+    if (MODE == 3) {
+      // R22: density term + the gather estimates of div v and rot v with the target's own h
+      const float4 c = list[E * j + 1];                      // v_j
+      const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
+      const float q = fminf(r2 * rinv * hinv[t], 2.0f);
+      const float u = 1.0f - q;
+      o0[t] = fmaf(a.w, q <= 0.5f ? fmaf(-6.0f * q * q, u, 1.0f) : 2.0f * u * u * u, o0[t]);
+      const float dq = q <= 0.5f ? fmaf(18.0f * q, q, -12.0f * q) : -6.0f * u * u;       // dW/dr in units of 8/(pi h^4)
+      const float g = a.w * dq * rinv;                       // m_j (dW/dr)/r; e = x_j - x_i, grad_i W = -(..) e
+      const float ux = c.x - vx[t], uy = c.y - vy[t], uz = c.z - vz[t];                  // v_j - v_i
+      o1[t] = fmaf(-g, fmaf(ux, ex, fmaf(uy, ey, uz * ez)), o1[t]);                      // div:  m gw u.(x_i - x_j)
+      o2[t] = fmaf(-g, ey * uz - ez * uy, o2[t]);                                        // rot:  m gw (x_i - x_j) x u = -g (e x u)
+      o3[t] = fmaf(-g, ez * ux - ex * uz, o3[t]);
+      o4[t] = fmaf(-g, ex * uy - ey * ux, o4[t]);
+    } else if (MODE == 0) {
       float q = fminf(sqrt_approx(r2) * hinv[t], 2.0f);
       float u = 1.0f - q;
       float w1 = fmaf(-6.0f * q * q, u, 1.0f);   // 1 - 6q^2 + 6q^3
@@ -275,10 +304,15 @@ struct SphVisitor {
       const int64_t s = g0 + t * 32 + lane;
       if (s < p.c.N) {
         const uint32_t i = p.c.perm[s];
-        if (MODE == 0) {
+        if (GATHER) {
           float hi3 = hinv[t] * hinv[t] * hinv[t];
           atomicAdd(p.rho + i, o0[t] * (8.0f / PI_F) * hi3);
           if (p.nngb) atomicAdd(p.nngb + i, cnt_ngb[t]);
+          if (MODE == 3) {                                   // unnormalised: divided by rho after the walk
+            const float k4 = (8.0f / PI_F) * hi3 * hinv[t];
+            float* dst = reinterpret_cast<float*>(p.acc + i);
+            atomicAdd(dst + 0, o1[t] * k4); atomicAdd(dst + 1, o2[t] * k4); atomicAdd(dst + 2, o3[t] * k4); atomicAdd(dst + 3, o4[t] * k4);
+          }
         } else {
           float* dst = reinterpret_cast<float*>(p.acc + i);
           atomicAdd(dst + 0, o0[t]); atomicAdd(dst + 1, o1[t]); atomicAdd(dst + 2, o2[t]);
@@ -517,6 +551,23 @@ otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float*
   if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
   if (ctx->use_ws_sph) OTOO_TRY(launch_sph_ws<0>(ctx, p, G, st)); else OTOO_TRY(launch_sph<0>(ctx, p, G, grid, smem, st));
   ctx->launches += 1;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  ctx->walked = true;
+  return OTOO_OK;
+}
+
+otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d_vel, int G, float* d_rho, uint32_t* d_nngb,
+                                 float* d_divrot, cudaStream_t st) {
+  SphParams p; int grid; size_t smem;
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  gather_vel_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(reinterpret_cast<const float4*>(d_vel), ctx->val[0], ctx->N, ctx->sorted_vel);
+  p.svel = ctx->sorted_vel; p.rho = d_rho; p.nngb = d_nngb; p.acc = reinterpret_cast<float4*>(d_divrot);
+  OTOO_CUDA(ctx, cudaMemsetAsync(d_rho, 0, 4 * (size_t)ctx->N, st));
+  if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(d_divrot, 0, 16 * (size_t)ctx->N, st));
+  OTOO_TRY(launch_sph<3>(ctx, p, G, grid, smem, st));
+  divrot_finish_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_rho, ctx->N, reinterpret_cast<float4*>(d_divrot));
+  ctx->launches += 3;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;
   return OTOO_OK;

@@ -264,6 +264,30 @@ def test_adaptive_h_parity(otoo, orc, kind, n, G, target, tol, h0):
         assert np.all(np.abs(nref.astype(float) - target) <= tol)
 
 
+@pytest.mark.parametrize("n,G", [(20000, 64), (9000 + 5, 32), (6000, 128)])
+def test_sph_stage1_divrot_parity(otoo, orc, n, G):
+    """otoo_sph_stage1 (PAPER L252 step 4; reading R22): density and counts as otoo_sph_density, div v and rot v
+    within max(1e-5 |x|, 8 u sum_j |x_ij|) (the velocity differences cancel like the pressure terms)."""
+    w = gen.wd_pair(n, 31)
+    pm, h = w["pos_mass"], w["h"]
+    vel = w["vel"].copy()
+    vel[:, :3] += -0.3 * pm[:, :3] + 0.05 * (gen.uniform01(5, np.arange(3 * n, dtype=np.uint64), 0).reshape(n, 3) - 0.5)
+    vel = vel.astype(np.float32)
+    t = check_tree(otoo, orc, pm, 16)
+    ref = t.sph_divrot(h, vel, G)
+    rho, nngb, dr = otoo.otoo_sph_stage1(dev(h), dev(vel), G)
+    rho0, nn0 = otoo.otoo_sph_density(dev(h), G)
+    assert np.array_equal(nngb.cpu().numpy(), nn0.cpu().numpy())
+    rg = rho.cpu().numpy()
+    assert (np.abs(rg - ref["rho"]) / ref["rho"]).max() <= TOL
+    assert (np.abs(rg - rho0.cpu().numpy()) / rg).max() <= 4 * U32 * 8
+    got = dr.cpu().numpy().astype(np.float64)
+    tol = 8 * U32 * ref["abs_sum"]
+    assert np.all(np.abs(got[:, 0] - ref["divrot"][:, 0]) <= np.maximum(TOL * np.abs(ref["divrot"][:, 0]), tol))
+    d = np.linalg.norm(got[:, 1:] - ref["divrot"][:, 1:], axis=1)
+    assert np.all(d <= np.maximum(TOL * np.linalg.norm(ref["divrot"][:, 1:], axis=1), tol))
+
+
 def test_status_codes(otoo):
     from paper_1206_1199_b200 import binding
     fresh = binding.Otoo(max_particles=1000)
