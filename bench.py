@@ -105,6 +105,7 @@ def run_reference(args, rank):
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         t = oracle.Tree(pm, cfg["n_crit"], key_order=1 if args.key_order == "hilbert" else 0)
+        t.set_dist_kind(1 if args.group_distance == "exact" else 0)
         rb2 = None
         if args.mac == "delta":
             rb2 = t.rb2_delta(float(np.float32(args.delta if args.delta is not None else cfg.get("delta", 0.01))),
@@ -142,6 +143,8 @@ def main():
                     help="delta: the paper's absolute-error MAC (otoo_gravity_delta) instead of BASELINE's theta criterion")
     ap.add_argument("--key-order", default="morton", choices=["morton", "hilbert"],
                     help="hilbert: the paper's ordering (L131) instead of BASELINE's Morton-contiguous groups")
+    ap.add_argument("--group-distance", default="box", choices=["box", "exact"],
+                    help="exact: the paper's minimum over the members' distances (L163) instead of the group box distance")
     ap.add_argument("--delta", type=float, default=None)
     ap.add_argument("--m-limit", type=float, default=None)
     ap.add_argument("--seed", type=int, default=1206)
@@ -170,6 +173,7 @@ def main():
     m_limit = float(np.float32(args.m_limit if args.m_limit is not None else cfg.get("m_limit", 0.05)))
     o = binding.Otoo(max_particles=n, device=local)
     o.otoo_set_option("key_order", 1 if args.key_order == "hilbert" else 0)
+    o.otoo_set_option("group_distance", 1 if args.group_distance == "exact" else 0)
     d_pm = torch.from_numpy(pm).cuda()
     out = torch.empty((n, 4), dtype=torch.float32, device="cuda")
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -286,7 +290,7 @@ def main():
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{args.workload}: {cfg['kind']} N={n} eps={cfg['eps']} {mac_txt} "
-                                   f"n_crit={n_crit} group={G} order={args.key_order}",
+                                   f"n_crit={n_crit} group={G} order={args.key_order} distance={args.group_distance}",
                        "l2": "flushed between steps (256 MiB write, outside the timed events)",
                        "parallelism": "replicas" if world > 1 else "single"},
             "gflops": FLOPS_PER_INTERACTION * value / 1e9,
@@ -301,6 +305,7 @@ def main():
         from oracle import oracle
         t0 = time.perf_counter()
         t = oracle.Tree(pm, n_crit, key_order=1 if args.key_order == "hilbert" else 0)
+        t.set_dist_kind(1 if args.group_distance == "exact" else 0)
         r = t.gravity(eps, theta, G, forces=True, rb2=t.rb2_delta(delta, m_limit) if args.mac == "delta" else None)
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": r["interactions"] / dt, "unit": UNIT, "cores": oracle.max_threads(),

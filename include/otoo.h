@@ -158,6 +158,9 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
  * order (the paper's own ordering; R20) -- same cells, other order: no group straddles an
  * octant boundary with a system-sized box, fewer interactions at the same theta.  Read by the next
  * otoo_build_tree; otoo_cell_t.prefix is then a Hilbert-key prefix.
+ * "group_distance" = 0 (default): the gravity MAC compares r_b with the distance from the group's bounding box
+ * (R8); 1: with the actual minimum of the members' distances, as the paper does (R23):
+ * shorter lists (no system-sized boxes), costlier tests.  Gravity only; needs "warp_specialized" = 1.
  * "warp_specialized" = 1 (default): otoo_gravity runs walker/evaluator warp pairs (walker warps build
  * the lists in shared memory, evaluator warps hold the targets and sum), 0: one warp does both in turn.
  * Same lists, same counters; sums differ in rounding order only.

@@ -91,6 +91,7 @@ def lib():
         L.orc_W.argtypes = [dbl, dbl]
         L.orc_dWdr.restype = dbl
         L.orc_dWdr.argtypes = [dbl, dbl]
+        L.orc_set_dist_kind.argtypes = [vp, i32]
         L.orc_max_threads.restype = i32
         L.orc_set_threads.argtypes = [i32]
     return _lib
@@ -194,6 +195,10 @@ class Tree:
         out = np.empty(self.ncell, dtype=np.float32)
         lib().orc_rb2(self._h, float(theta), int(mac_kind), _p(out))
         return out
+
+    def set_dist_kind(self, kind):
+        """0: group AABB distance (R8); 1: exact minimum over the group's members (R23)"""
+        lib().orc_set_dist_kind(self._h, int(kind))
 
     def delta_cell_props(self):
         """(B2, b_max) per cell in fp64: PAPER.md Eq. 2 (bottom-up, reading R19) and L63."""

@@ -16,6 +16,7 @@ struct orc_tree {
   int64_t N;
   int n_crit;
   int key_order;  /* 0 Morton (R3), 1 Hilbert (R20) */
+  int dist_kind;  /* 0 group AABB distance (R8), 1 the paper's exact minimum over the members (L163; R23) */
   float lo[3], S;
   uint64_t* key;  /* sorted keys */
   uint32_t* perm; /* perm[s] = original index of sorted slot s */
@@ -411,9 +412,10 @@ void orc_rb2_delta(const orc_tree* t, double delta, double m_limit, float* rb2) 
 }
 
 /* ---------------- R8: group AABB and group-cell distance (L163, Barnes 1990 form) ----------- */
-typedef struct { float lo[3], hi[3]; float hmax; } gbox_t;
+typedef struct { float lo[3], hi[3]; float hmax; const float* mem; int nmem; } gbox_t;   /* mem: the members' (x,y,z,m), set for dist_kind 1 */
 static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs /*sorted h or NULL*/) {
   gbox_t g; g.hmax = 0.0f;
+  g.mem = (t->dist_kind == 1 && !hs) ? t->spos + 4 * a : NULL; g.nmem = (int)(b - a);   /* SPH walks (hs given): AABB only */
   for (int k = 0; k < 3; k++) { g.lo[k] = t->spos[4 * a + k]; g.hi[k] = g.lo[k]; }
   for (int64_t s = a; s < b; s++) {
     for (int k = 0; k < 3; k++) {
@@ -426,6 +428,17 @@ static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs
   return g;
 }
 static float box_d2(const gbox_t* g, const float* cm) {
+  if (g->mem) {
+    /* "compute n_vec distances for each pair and then select the actual minimum distance";
+     * reading R23: d_i^2 = fma(dz,dz, fma(dy,dy, dx*dx)), d = fl32(x_i - cm), in fp32; the minimum is exact */
+    float best = INFINITY;
+    for (int i = 0; i < g->nmem; i++) {
+      float dx = g->mem[4 * i] - cm[0], dy = g->mem[4 * i + 1] - cm[1], dz = g->mem[4 * i + 2] - cm[2];
+      float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+      if (d2 < best) best = d2;
+    }
+    return best;
+  }
   float e[3];
   for (int k = 0; k < 3; k++) {
     float a = g->lo[k] - cm[k], b = cm[k] - g->hi[k];
@@ -864,6 +877,7 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
   return orc_sph_force_sel(t, h, rho, P, vel, G, NULL, 0, out, abs_sum);
 }
 
+void orc_set_dist_kind(orc_tree* t, int kind) { t->dist_kind = kind; }
 int orc_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

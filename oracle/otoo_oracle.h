@@ -118,6 +118,9 @@ uint64_t orc_sph_force_sel(const orc_tree*, const float* h, const double* rho, c
 double orc_W(double r, double h);
 double orc_dWdr(double r, double h);
 
+/* group-cell distance of the gravity walks: 0 = from the group's AABB (R8, default), 1 = the paper's exact
+ * minimum over the group's members (R23).  SPH walks always use the AABB. */
+void orc_set_dist_kind(orc_tree*, int kind);
 int orc_max_threads(void);
 void orc_set_threads(int n);
 #ifdef __cplusplus

@@ -319,6 +319,11 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     ctx->key_order = (int)value;
     return OTOO_OK;
   }
+  if (strcmp(name, "group_distance") == 0) {
+    if (value != 0 && value != 1) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance must be 0 (AABB) or 1 (exact minimum)");
+    ctx->dist_kind = (int)value;
+    return OTOO_OK;
+  }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "warp_specialized") == 0) { ctx->use_ws = value != 0; return OTOO_OK; }
   if (strcmp(name, "warp_specialized_sph") == 0) { ctx->use_ws_sph = value != 0; return OTOO_OK; }

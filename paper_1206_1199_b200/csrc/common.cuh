@@ -97,6 +97,7 @@ struct otoo_ctx {
   int use_pool;          // option "task_pool"
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int walk_only;         // option "walk_only" (diagnostic)
+  int dist_kind;         // option "group_distance": 0 AABB (R8), 1 exact minimum over the group's members (R23)
   int use_ws;            // option "warp_specialized": gravity walk with walker/evaluator warp pairs
   int use_ws_sph;        // option "warp_specialized_sph": the same split for the SPH kernels (default off)
   int last_group_size;

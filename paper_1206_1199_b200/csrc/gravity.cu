@@ -208,13 +208,13 @@ template <int T_>
 struct GravWalker {
   static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2;
   static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
-  typedef WsPair<32 * NP * 3> Pair;
+  typedef WsPair<32 * NP * 3, 32 * T_> Pair;
   const GravParams& p;
   Pair& sm;
   float glo[3], ghi[3];
   unsigned selfmask;
   uint32_t group, buf, eparity, first;
-  int lane_;
+  int lane_, nmem;
   __device__ __forceinline__ GravWalker(const GravParams& p_, Pair& sm_, int lane) : p(p_), sm(sm_), buf(0), eparity(~0u), first(0), lane_(lane) {}
 
   __device__ __forceinline__ float4* acquire() {     // wait until the evaluator has released buffer `buf`
@@ -227,6 +227,7 @@ struct GravWalker {
     for (int t = 0; t < T; t++) {   // H7: the group's tight AABB
       int64_t s = g0 + t * 32 + lane;
       float4 v = p.c.spos[s < p.c.N ? s : g0];
+      if (p.c.dist_kind) sm.mem[t * 32 + lane] = v;      // out-of-range slots mirror slot g0: harmless duplicates
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
         glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
@@ -242,12 +243,45 @@ struct GravWalker {
         ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
       }
     selfmask = 0; first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+    nmem = 32 * T;
+    __syncwarp();
+    if (p.c.dist_kind) {
+      // tight boxes of 8 consecutive members (neighbours on the key curve): a box farther than r_b settles its
+      // 8 members at once -- in fp32 too: rounding is monotone, so the box distance never exceeds a member's
+      for (int b = lane; b < 4 * T; b += 32) {
+        float4 lo = sm.mem[8 * b], hi = lo;
+#pragma unroll
+        for (int i = 1; i < 8; i++) {
+          const float4 m = sm.mem[8 * b + i];
+          lo.x = fminf(lo.x, m.x); lo.y = fminf(lo.y, m.y); lo.z = fminf(lo.z, m.z);
+          hi.x = fmaxf(hi.x, m.x); hi.y = fmaxf(hi.y, m.y); hi.z = fmaxf(hi.z, m.z);
+        }
+        sm.sub[2 * b] = lo; sm.sub[2 * b + 1] = hi;
+      }
+      __syncwarp();
+    }
   }
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
     A = __ldg(p.c.cell_cm + cell);
     B = __ldg(p.c.cell_b + cell);
+    const float rb2 = __uint_as_float(B.x);
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
-    return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
+    if (d2 > rb2) return 1;                      // strict: equality opens (R8); the box distance bounds every member's from below
+    if (!p.c.dist_kind) return 2;
+    // PAPER L163 (R23): the actual minimum of the members' distances decides: accept iff every member is
+    // farther than r_b.  d_i^2 = fma(dz,dz, fma(dy,dy, dx*dx)), d = fl32(x_i - cm), as the oracle computes it.
+    for (int b = 0; b < 4 * T; b++) {
+      const float4 lo = sm.sub[2 * b], hi = sm.sub[2 * b + 1];
+      const float blo[3] = {lo.x, lo.y, lo.z}, bhi[3] = {hi.x, hi.y, hi.z};
+      if (aabb_d2(blo, bhi, A.x, A.y, A.z) > rb2) continue;
+#pragma unroll
+      for (int i = 0; i < 8; i++) {
+        const float4 m = sm.mem[8 * b + i];
+        const float dx = __fsub_rn(m.x, A.x), dy = __fsub_rn(m.y, A.y), dz = __fsub_rn(m.z, A.z);
+        if (!(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))) > rb2)) return 2;
+      }
+    }
+    return 1;
   }
   struct Entry { float4 a; };
   __device__ __forceinline__ Entry get(uint32_t slot) const { Entry e; e.a = p.c.spos[slot]; return e; }
@@ -392,6 +426,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
   c->use_pool = ctx->use_pool;
   c->walk_only = ctx->walk_only;
+  c->dist_kind = 0;
   ctx->launches += 1;
   ctx->last_group_size = G; ctx->last_ngroups = ngroups;
   return OTOO_OK;
@@ -412,6 +447,9 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);
   const bool eps0 = !(eps > 0.0f);
+  if (ctx->dist_kind && !ctx->use_ws)
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance = 1 needs warp_specialized = 1");
+  p.c.dist_kind = ctx->dist_kind;
   if (ctx->use_ws) {
     switch (G) {
       case 32: OTOO_TRY(launch_walk_ws<1>(ctx, p, eps0, st)); break;

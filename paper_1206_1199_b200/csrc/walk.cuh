@@ -70,6 +70,7 @@ struct WalkCommon {
   int stack_cap;
   int use_pool;                                                 // 0: never donate (test hook: private spill only)
   int walk_only;                                                // 1: lists are built and counted but not evaluated (measures the walk)
+  int dist_kind;                                                // gravity: 0 group AABB distance (R8), 1 exact minimum over the members (R23)
 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }

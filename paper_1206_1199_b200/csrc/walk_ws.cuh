@@ -21,9 +21,12 @@ enum : uint32_t { WS_FIRST = 1u, WS_LAST = 2u, WS_EXIT = 4u };
 struct WsMeta { uint32_t count, flags, group, pad; };
 
 // shared memory of one pair; NT = float2 words of target staging (32 lanes x NP x 3)
-template <int NT>
+// NM = float4 slots for the group's members (exact-minimum group distance of the gravity walker)
+template <int NT, int NM = 1>
 struct __align__(16) WsPair {
   float4 list[OTOO_WS_NBUF][OTOO_WS_LCAP + 4];   // +4 entries: consecutive buffers start on different banks
+  float4 mem[NM];
+  float4 sub[(NM + 7) / 8 * 2];                  // tight boxes of 8 consecutive members: (lo.xyz, -), (hi.xyz, -)
   float2 tgt[NT];
   uint32_t stk[OTOO_WALK_STACK_MAX];
   uint32_t self[OTOO_WS_NBUF][32];

@@ -173,6 +173,41 @@ def test_hilbert_order_parity(otoo, orc, kind, n, n_crit, G):
         assert (np.abs(rho.cpu().numpy() - rs["rho"]) / rs["rho"]).max() <= TOL
 
 
+@pytest.mark.parametrize("kind,n,G,theta,key_order", [("plummer", 16384, 64, 0.5, 0), ("plummer", 20000 + 9, 128, 0.6, 0), ("hernquist", 30000, 32, 0.4, 1),
+                                                       ("uniform_cube", 40000, 256, 0.5, 0), ("plummer", 3000, 128, 0.0, 0)])
+def test_exact_min_group_distance_parity(otoo, orc, kind, n, G, theta, key_order):
+    """group_distance = 1: the paper's vector walk (reading R23) -- the MAC compares r_b with the
+    actual minimum of the members' distances.  Lists (counters) exact, sums within tolerance, for both MACs."""
+    pm = gen.make(kind, n, 1206)
+    t = check_tree(otoo, orc, pm, 16, key_order=key_order)
+    theta32 = float(np.float32(theta))
+    aabb = t.gravity(0.01, theta32, G, forces=False)
+    t.set_dist_kind(1)
+    otoo.otoo_set_option("group_distance", 1)
+    try:
+        ref = t.gravity(0.01, theta32, G)
+        out = otoo.otoo_gravity(0.01, theta32, G).cpu().numpy()
+        nt, nc, npart = otoo.otoo_export_group_stats()
+        assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+        assert otoo.otoo_last_stats()["sum_interactions"] == ref["interactions"] <= aabb["interactions"]
+        e, raw = acc_err(out, ref["acc_pot"], ref["abs_sum"])
+        assert e.max() <= TOL and np.percentile(raw, 99.9) <= TOL
+        rb2 = t.rb2_delta(float(np.float32(0.01)), float(np.float32(0.05)))
+        refd = t.gravity(0.01, 0.0, G, rb2=rb2)
+        outd = otoo.otoo_gravity_delta(0.01, 0.01, 0.05, G).cpu().numpy()
+        nt, nc, npart = otoo.otoo_export_group_stats()
+        assert np.array_equal(nt, refd["n_tests"]) and np.array_equal(nc, refd["n_cells"]) and np.array_equal(npart, refd["n_parts"])
+        e, _ = acc_err(outd, refd["acc_pot"], refd["abs_sum"])
+        assert e.max() <= TOL
+        otoo.otoo_set_option("warp_specialized", 0)          # the one-warp kernel has no exact-minimum form: refused
+        from paper_1206_1199_b200 import binding
+        with pytest.raises(binding.OtooError):
+            otoo.otoo_gravity(0.01, theta32, G)
+    finally:
+        otoo.otoo_set_option("warp_specialized", 1)
+        otoo.otoo_set_option("group_distance", 0)
+
+
 def test_walk_stack_spill(otoo, orc):
     """theta = 0 on a deep tree overflows the 512-entry shared stack: both overflow paths (task pool,
     private global spill) must give the same lists."""

@@ -160,3 +160,46 @@ def test_group_selection_equals_full_run(orc):
     ff = ts.sph_force(w["h"], fd["rho"], P, 32, vel=w["vel"])
     pf = ts.sph_force(w["h"], fd["rho"], P, 32, vel=w["vel"], groups=sel)
     assert np.array_equal(pf["acc_dudt"][idx], ff["acc_dudt"][idx])
+
+
+def test_exact_minimum_group_distance(orc):
+    """dist_kind = 1 ("compute n_vec distances ... select the actual minimum"; reading R23).
+    Pins by brute force on a small system: every accepted cell is farther than r_b from EVERY member of the
+    group (fp32 distances recomputed here with numpy), every cell that was opened has some member within
+    r_b, the lists still tile the system, they are never longer than the bounding-box lists, and theta = 0
+    is the direct sum."""
+    n, G, theta = 3000, 32, np.float32(0.7)
+    pm = gen.plummer(n, 17)
+    t = orc.Tree(pm, 8)
+    e = t.export()
+    spos = pm[e["perm"]]
+    rb2 = t.rb2(float(theta))
+    aabb = t.gravity(0.01, float(theta), G, forces=False)
+    t.set_dist_kind(1)
+    ex = t.gravity(0.01, float(theta), G, forces=False)
+    assert np.all(ex["n_cells"].astype(int) + ex["n_parts"] <= aabb["n_cells"].astype(int) + aabb["n_parts"])
+    assert ex["interactions"] < aabb["interactions"]
+    cm = e["com_m"][:, :3]
+    first, count, cf, cc = (e["cells"][k].astype(np.int64) for k in ("first", "count", "child_first", "child_count"))
+
+    for g in range(0, t.n_groups(G), 9):
+        cells, parts = t.group_lists_rb2(rb2, G, g, ex["n_cells"][g], ex["n_parts"][g])
+        mem = spos[g * G:min((g + 1) * G, n), :3]
+        cover = np.zeros(n, np.int32)
+        cover[parts] += 1
+        for c in cells:
+            cover[first[c]:first[c] + count[c]] += 1
+            d = (mem - cm[c]).astype(np.float32).astype(np.float64)
+            assert ((d ** 2).sum(axis=1).min()) > float(rb2[c]) * (1 - 1e-6)       # every member outside r_b
+            par = np.where((cf <= c) & (c < cf + cc) & (cc > 0))[0]                 # its parent was opened:
+            if len(par):
+                dp = (mem - cm[par[0]]).astype(np.float32).astype(np.float64)
+                assert ((dp ** 2).sum(axis=1).min()) <= float(rb2[par[0]]) * (1 + 1e-6)   # some member inside the parent's r_b
+        assert np.all(cover == 1)
+    d = orc.direct_sum(pm, 0.01)
+    assert np.allclose(t.gravity(0.01, 0.0, G)["acc_pot"], d, rtol=1e-12, atol=1e-14)
+    # the accuracy is that of a per-particle MAC: no worse than a few times the box lists' error
+    t2 = orc.Tree(pm, 8)
+    eb = np.linalg.norm(t2.gravity(0.01, float(theta), G)["acc_pot"][:, :3] - d[:, :3], axis=1).mean()
+    ee = np.linalg.norm(t.gravity(0.01, float(theta), G)["acc_pot"][:, :3] - d[:, :3], axis=1).mean()
+    assert eb <= ee <= 3 * eb
