@@ -73,6 +73,8 @@ def lib():
         L.orc_gravity_sel.argtypes = [vp, dbl, dbl, i32, i32, i32, vp, i64, vp, vp, vp, vp, vp]
         L.orc_sph_density_sel.restype = C.c_uint64
         L.orc_sph_density_sel.argtypes = [vp, vp, i32, vp, i64, vp, vp, vp, vp]
+        L.orc_sph_force_visc_sel.restype = C.c_uint64
+        L.orc_sph_force_visc_sel.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, i64, vp, vp]
         L.orc_sph_force_sel.restype = C.c_uint64
         L.orc_sph_force_sel.argtypes = [vp, vp, vp, vp, vp, i32, vp, i64, vp, vp]
         L.orc_group_lists.argtypes = [vp, dbl, i32, i32, i64, vp, vp]
@@ -308,7 +310,8 @@ class Tree:
         lib().orc_sph_group_list(self._h, _p(h), int(group_size), int(g), _p(parts))
         return parts[:int(n_parts)]
 
-    def sph_force(self, h, rho, P, group_size, vel=None, groups=None):
+    def sph_force(self, h, rho, P, group_size, vel=None, groups=None, visc=None):
+        """visc: optional (N,4) fp32 (sound speed c, alpha, Balsara f, -): artificial viscosity, reading R24 (needs vel)"""
         h = _f32(h, (self.N,))
         rho = np.ascontiguousarray(rho, dtype=np.float64)
         P = np.ascontiguousarray(P, dtype=np.float64)
@@ -316,6 +319,12 @@ class Tree:
         out = np.zeros((self.N, 4), dtype=np.float64)
         asum = np.zeros((self.N, 2), dtype=np.float64)
         sel = None if groups is None else np.ascontiguousarray(groups, dtype=np.int64)
-        tot = lib().orc_sph_force_sel(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(sel),
-                                      0 if sel is None else len(sel), _p(out), _p(asum))
+        if visc is not None:
+            assert v is not None
+            q = _f32(visc, (self.N, 4))
+            tot = lib().orc_sph_force_visc_sel(self._h, _p(h), _p(rho), _p(P), _p(v), _p(q), int(group_size), _p(sel),
+                                               0 if sel is None else len(sel), _p(out), _p(asum))
+        else:
+            tot = lib().orc_sph_force_sel(self._h, _p(h), _p(rho), _p(P), _p(v), int(group_size), _p(sel),
+                                          0 if sel is None else len(sel), _p(out), _p(asum))
         return dict(acc_dudt=out, candidates=int(tot), abs_sum=asum)

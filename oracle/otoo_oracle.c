@@ -818,8 +818,15 @@ void orc_sph_group_list(const orc_tree* t, const float* h, int G, int64_t g, uin
 }
 
 /* R17: symmetric pressure force (TREESPH/GADGET form) and optional du/dt. */
-uint64_t orc_sph_force_sel(const orc_tree* t, const float* h, const double* rho, const double* P,
-                           const float* vel, int G, const int64_t* sel, int64_t nsel, double* out, double* abs_sum) {
+/* visc != NULL (needs vel): artificial viscosity ("a hybrid of [53] and [54]", i.e. the standard
+ * pair viscosity with the Balsara shear switch and a per-particle alpha; the paper prints no formula).
+ * Reading R24: visc = 4N floats (c_i sound speed, alpha_i, f_i Balsara factor, -); for a pair with
+ * w = (v_i - v_j).(x_i - x_j) < 0:  l = (h_i + h_j)/4,  mu = l w / (r^2 + 0.01 l^2),
+ *   Pi_ij = fbar (-abar cbar mu + 2 abar mu^2) / rhobar   (bars: arithmetic means of the two particles),
+ * else Pi_ij = 0; Pi_ij is added to (P_i/rho_i^2 + P_j/rho_j^2) in both the force and du/dt of R17. */
+static uint64_t sph_force_impl(const orc_tree* t, const float* h, const double* rho, const double* P,
+                               const float* vel, const float* visc, int G, const int64_t* sel, int64_t nsel,
+                               double* out, double* abs_sum) {
   int64_t N = t->N, ng = sel ? nsel : (N + G - 1) / G;
   float* hs = sorted_h(t, h);
   float* bmax = (float*)malloc(4 * t->ncell); float* rsph = (float*)malloc(4 * t->ncell);
@@ -853,7 +860,20 @@ uint64_t orc_sph_force_sel(const orc_tree* t, const float* h, const double* rho,
           double r = sqrt(dx * dx + dy * dy + dz * dz);
           if (r == 0.0) continue;
           double gw = 0.5 * (orc_dWdr(r, (double)hi) + orc_dWdr(r, (double)hj)) / r;  /* grad_i W = gw * (xi-xj) */
-          double f = (double)pj[3] * (pri + P[jo] / (rho[jo] * rho[jo])) * gw;
+          double Pi = 0.0;
+          if (visc && vel) {
+            double wx = (double)vel[4 * io] - vel[4 * jo], wy = (double)vel[4 * io + 1] - vel[4 * jo + 1],
+                   wz = (double)vel[4 * io + 2] - vel[4 * jo + 2];
+            double w = wx * dx + wy * dy + wz * dz;
+            if (w < 0.0) {
+              double l = 0.25 * ((double)hi + (double)hj);
+              double mu = l * w / (r * r + 0.01 * l * l);
+              double ab = 0.5 * ((double)visc[4 * io + 1] + visc[4 * jo + 1]), cb = 0.5 * ((double)visc[4 * io] + visc[4 * jo]);
+              double fb = 0.5 * ((double)visc[4 * io + 2] + visc[4 * jo + 2]), rb = 0.5 * (rho[io] + rho[jo]);
+              Pi = fb * (-ab * cb * mu + 2.0 * ab * mu * mu) / rb;
+            }
+          }
+          double f = (double)pj[3] * (pri + P[jo] / (rho[jo] * rho[jo]) + Pi) * gw;
           ax -= f * dx; ay -= f * dy; az -= f * dz;
           asum += fabs(f) * r;                       /* |a_ij|, for the test's error bound */
           if (vel) {
@@ -871,6 +891,15 @@ uint64_t orc_sph_force_sel(const orc_tree* t, const float* h, const double* rho,
   }
   free(hs); free(bmax); free(rsph);
   return total;
+}
+uint64_t orc_sph_force_sel(const orc_tree* t, const float* h, const double* rho, const double* P,
+                           const float* vel, int G, const int64_t* sel, int64_t nsel, double* out, double* abs_sum) {
+  return sph_force_impl(t, h, rho, P, vel, NULL, G, sel, nsel, out, abs_sum);
+}
+uint64_t orc_sph_force_visc_sel(const orc_tree* t, const float* h, const double* rho, const double* P,
+                                const float* vel, const float* visc, int G, const int64_t* sel, int64_t nsel,
+                                double* out, double* abs_sum) {
+  return sph_force_impl(t, h, rho, P, vel, visc, G, sel, nsel, out, abs_sum);
 }
 uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, const double* P,
                        const float* vel, int G, double* out, double* abs_sum) {

@@ -114,6 +114,10 @@ uint64_t orc_sph_force(const orc_tree*, const float* h, const double* rho, const
 uint64_t orc_sph_force_sel(const orc_tree*, const float* h, const double* rho, const double* P,
                            const float* vel, int group_size, const int64_t* sel, int64_t nsel,
                            double* acc_dudt, double* abs_sum);
+/* the same with artificial viscosity (reading R24): visc = 4N floats (c, alpha, Balsara f, -), vel required */
+uint64_t orc_sph_force_visc_sel(const orc_tree*, const float* h, const double* rho, const double* P,
+                                const float* vel, const float* visc, int group_size, const int64_t* sel,
+                                int64_t nsel, double* acc_dudt, double* abs_sum);
 /* cubic spline with support h (R13) */
 double orc_W(double r, double h);
 double orc_dWdr(double r, double h);

@@ -180,3 +180,54 @@ def test_div_and_rot_of_linear_velocity_fields(orc):
     vel[:, :3] = np.cross(Om, x)
     rr = t.sph_divrot(h, vel, 32)["divrot"][inner]
     assert np.abs(rr[:, 0]).max() < 1e-6 and np.allclose(rr[:, 1:], 2 * c[0] * Om, rtol=1e-5, atol=1e-7)
+
+
+def test_artificial_viscosity(orc):
+    """Reading R24 (PAPER L246 names the scheme, prints no formula).  What the pair form fixes: with alpha = 0 or
+    Balsara f = 0 the result is R17's; a receding (expanding) flow feels no viscosity; the viscous pair forces
+    are antisymmetric (momentum conserved), the viscous heating is non-negative for every particle and equals
+    the kinetic energy it removes (total energy conserved)."""
+    n = 3000
+    w = gen.wd_pair(n, 11)
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    m = pm[:, 3].astype(np.float64)
+    t = orc.Tree(pm, 16)
+    rho = t.sph_density(h, 32)["rho"]
+    P = (2.0 / 3.0) * rho * u
+    cs = np.sqrt((5.0 / 3.0) * P / rho)
+    x = pm[:, :3].astype(np.float64)
+    visc = np.zeros((n, 4), np.float32)
+    visc[:, 0], visc[:, 1], visc[:, 2] = cs, 1.0, 0.8
+    vel = np.zeros((n, 4), np.float32)
+    vel[:, :3] = -0.4 * x + 0.1 * np.sin(7 * x[:, [1, 2, 0]])          # compression + some shear
+    base = t.sph_force(h, rho, P, 32, vel=vel)["acc_dudt"]
+    full = t.sph_force(h, rho, P, 32, vel=vel, visc=visc)["acc_dudt"]
+    for k, val in ((1, 0.0), (2, 0.0)):                                 # alpha = 0, f = 0: R17
+        v0 = visc.copy()
+        v0[:, k] = val
+        assert np.array_equal(t.sph_force(h, rho, P, 32, vel=vel, visc=v0)["acc_dudt"], base)
+    dv = full - base                                                    # the viscous part
+    assert np.abs(dv[:, :3]).max() > 1e-3 * np.abs(base[:, :3]).max()
+    assert np.all(dv[:, 3] >= -1e-12 * np.abs(base[:, 3]).max())        # heating only
+    mom = (m[:, None] * dv[:, :3]).sum(axis=0)
+    assert np.abs(mom).max() <= 1e-12 * (m[:, None] * np.abs(dv[:, :3])).sum()
+    e_kin = (m * (vel[:, :3].astype(np.float64) * dv[:, :3]).sum(axis=1)).sum()
+    e_int = (m * dv[:, 3]).sum()
+    assert abs(e_kin + e_int) <= 1e-10 * abs(e_int) and e_int > 0
+    vel[:, :3] = 0.4 * x                                                # homologous expansion: every pair recedes
+    assert np.array_equal(t.sph_force(h, rho, P, 32, vel=vel, visc=visc)["acc_dudt"], t.sph_force(h, rho, P, 32, vel=vel)["acc_dudt"])
+    # two particles approaching head-on: the closed form of the pair term
+    pm2 = np.array([[0, 0, 0, 1.0], [0.5, 0, 0, 1.0]], np.float32)
+    t2 = orc.Tree(pm2, 16)
+    h2 = np.array([1.0, 1.0], np.float32)
+    v2 = np.array([[0.25, 0, 0, 0], [-0.25, 0, 0, 0]], np.float32)
+    q2 = np.array([[2.0, 1.5, 1.0, 0], [2.0, 1.5, 1.0, 0]], np.float32)
+    r2 = np.array([1.0, 1.0])
+    a = t2.sph_force(h2, r2, np.zeros(2), 32, vel=v2, visc=q2)["acc_dudt"]
+    r, wdot, l = 0.5, 0.5 * (-0.5), 0.5
+    mu = l * wdot / (r * r + 0.01 * l * l)
+    Pi = (-1.5 * 2.0 * mu + 2 * 1.5 * mu * mu) / 1.0
+    gw = orc.dWdr(r, 1.0)                                               # (dW_i + dW_j)/2 with equal h
+    assert a[0, 0] == pytest.approx(-1.0 * Pi * gw * (0 - 0.5) / r, rel=1e-12)     # pushed apart: a_0x < 0
+    assert a[0, 0] < 0 and a[1, 0] == pytest.approx(-a[0, 0], rel=1e-12)
+    assert a[0, 3] == pytest.approx(0.5 * Pi * gw * wdot / r, rel=1e-12) and a[0, 3] > 0
