@@ -103,6 +103,15 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
 otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho,
                              uint32_t* d_nngb, void* stream);
 
+/* otoo_sph_force with artificial viscosity (PAPER.md L246 names the scheme: Balsara switch + per-particle
+ * alpha; formula: DESIGN.md R24).  d_visc: N x float4 (sound speed c_i, alpha_i, Balsara factor f_i, -);
+ * d_vel is required.  For a pair with w = (v_i - v_j).(x_i - x_j) < 0:
+ *   Pi_ij = fbar (-abar cbar mu + 2 abar mu^2) / rhobar,  mu = l w / (r^2 + 0.01 l^2),  l = (h_i + h_j)/4,
+ * added to (P_i/rho_i^2 + P_j/rho_j^2) in the force and in du/dt.  Output as otoo_sph_force (w = du/dt). */
+otoo_status otoo_sph_force_visc(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,
+                                const float* d_vel, const float* d_visc, int group_size, float* d_acc_sph,
+                                void* stream);
+
 /* SPH stage 1 as the paper runs it (PAPER.md L252 step 4: "density, div v, rot v"): the density pass of
  * otoo_sph_density plus the gather estimates (R22)
  *   div v_i = (1/rho_i) sum_j m_j (v_j - v_i) . grad_i W(r_ij, h_i),

@@ -26,7 +26,7 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_sph_adapt_h", "otoo_sph_stage1"]
+           "otoo_gravity_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
 
 
 class TreeInfo(C.Structure):
@@ -55,6 +55,7 @@ _lib.otoo_build_tree.argtypes = [_vp, _vp, _i64, _i32, _vp]
 _lib.otoo_gravity.argtypes = [_vp, _f, _f, _i32, _vp, _vp]
 _lib.otoo_gravity_delta.argtypes = [_vp, _f, _f, _f, _i32, _vp, _vp]
 _lib.otoo_sph_density.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp]
+_lib.otoo_sph_force_visc.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp]
 _lib.otoo_sph_stage1.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.otoo_sph_adapt_h.argtypes = [_vp, _vp, _f, _f, _i32, _i32, _vp, C.POINTER(C.c_int), _vp]
 _lib.otoo_sph_force.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp]
@@ -149,6 +150,14 @@ class Otoo:
         self._check(_lib.otoo_sph_density(self._h, _ptr(h, torch.float32), int(group_size), _ptr(rho),
                                           _ptr(nngb), _stream(stream)))
         return rho, nngb
+
+    def otoo_sph_force_visc(self, h, rho, P, vel, visc, group_size, stream=None):
+        """pressure force + artificial viscosity + du/dt; visc = (N,4) fp32 (c, alpha, Balsara f, -)"""
+        out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
+        self._check(_lib.otoo_sph_force_visc(self._h, _ptr(h, torch.float32), _ptr(rho, torch.float32), _ptr(P, torch.float32),
+                                             _ptr(vel, torch.float32, 4), _ptr(visc, torch.float32, 4), int(group_size),
+                                             out.data_ptr(), _stream(stream)))
+        return out
 
     def otoo_sph_stage1(self, h, vel, group_size, stream=None):
         """density, neighbour counts and (div v, rot v): returns (rho, nngb, divrot)"""

@@ -112,7 +112,7 @@ void otoo_destroy(otoo_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   void* ptrs[] = {ctx->key[0], ctx->key[1], ctx->val[0], ctx->val[1], ctx->spos, ctx->slot_nc, ctx->scan_tmp, ctx->hist,
-                  ctx->sorted_h, ctx->sorted_aux, ctx->sorted_vel, ctx->cell_cm, ctx->cell_b, ctx->c_first, ctx->c_count,
+                  ctx->sorted_h, ctx->sorted_aux, ctx->sorted_vel, ctx->sorted_vis, ctx->cell_cm, ctx->cell_b, ctx->c_first, ctx->c_count,
                   ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_B2, ctx->c_sph,
                   ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
                   ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums,
@@ -166,6 +166,7 @@ static otoo_status sph_scratch(otoo_ctx* ctx) {
     OTOO_TRY(dalloc(ctx, &ctx->sorted_h, (size_t)ctx->maxN));
     OTOO_TRY(dalloc(ctx, &ctx->sorted_aux, (size_t)ctx->maxN));
     OTOO_TRY(dalloc(ctx, &ctx->sorted_vel, (size_t)ctx->maxN));
+    OTOO_TRY(dalloc(ctx, &ctx->sorted_vis, (size_t)ctx->maxN));
   }
   return OTOO_OK;
 }
@@ -216,7 +217,19 @@ otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, 
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
   OTOO_TRY(sph_scratch(ctx));
   ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
-  return otoo_sph_force_impl(ctx, d_h, d_rho, d_P, d_vel, group_size, d_acc_sph, (cudaStream_t)stream);
+  return otoo_sph_force_impl(ctx, d_h, d_rho, d_P, d_vel, nullptr, group_size, d_acc_sph, (cudaStream_t)stream);
+}
+
+otoo_status otoo_sph_force_visc(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
+                                const float* d_visc, int group_size, float* d_acc_sph, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_h || !d_rho || !d_P || !d_vel || !d_visc || !d_acc_sph) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL argument");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  OTOO_TRY(sph_scratch(ctx));
+  ctx->launches = 0; ctx->last_stream = (cudaStream_t)stream;
+  return otoo_sph_force_impl(ctx, d_h, d_rho, d_P, d_vel, d_visc, group_size, d_acc_sph, (cudaStream_t)stream);
 }
 
 otoo_status otoo_eos_ideal(otoo_ctx* ctx, const float* d_rho, const float* d_u, float gamma, int64_t N, float* d_P, void* stream) {

@@ -44,6 +44,7 @@ struct otoo_ctx {
   float* sorted_h;       // SPH: h in sorted order
   float4* sorted_aux;    // SPH force: (rho-independent) per-particle packed inputs in sorted order
   float4* sorted_vel;
+  float4* sorted_vis;    // SPH viscosity: (alpha, Balsara f, -, -) in sorted order
 
   // ---- per-cell arrays, capacity cellCap (grow-only)
   int64_t cellCap;
@@ -139,7 +140,7 @@ otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st);   // fp64 b_max of e
 otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb,
                                   cudaStream_t st);
 otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P,
-                                const float* d_vel, int G, float* d_acc, cudaStream_t st);
+                                const float* d_vel, const float* d_visc, int G, float* d_acc, cudaStream_t st);
 otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d_vel, int G, float* d_rho, uint32_t* d_nngb,
                                  float* d_divrot, cudaStream_t st);
 otoo_status otoo_sph_adapt_h_impl(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter, int G, uint32_t* d_nngb,

@@ -13,14 +13,17 @@ __global__ void __launch_bounds__(256) gather_h_kernel(const float* __restrict__
 // per sorted slot: (h, P/rho^2) and velocity
 __global__ void __launch_bounds__(256) gather_force_inputs_kernel(const float* __restrict__ h, const float* __restrict__ rho,
                                                                   const float* __restrict__ P, const float4* __restrict__ vel,
+                                                                  const float4* __restrict__ visc,
                                                                   const uint32_t* __restrict__ perm, int64_t n,
-                                                                  float4* __restrict__ aux, float4* __restrict__ svel) {
+                                                                  float4* __restrict__ aux, float4* __restrict__ svel,
+                                                                  float4* __restrict__ svis) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t i = perm[s];
   float r = rho[i];
-  aux[s] = make_float4(h[i], __fdiv_rn(P[i], __fmul_rn(r, r)), __fmul_rn(h[i], h[i]), 0.0f);   // (h, P/rho^2, h^2, -)
-  if (vel) svel[s] = vel[i];
+  aux[s] = make_float4(h[i], __fdiv_rn(P[i], __fmul_rn(r, r)), __fmul_rn(h[i], h[i]), r);   // (h, P/rho^2, h^2, rho)
+  if (vel) { float4 v = vel[i]; if (visc) v.w = visc[i].x; svel[s] = v; }                        // (v, c)
+  if (visc) svis[s] = make_float4(visc[i].y, visc[i].z, 0.0f, 0.0f);                            // (alpha, f)
 }
 
 __global__ void __launch_bounds__(256) gather_vel_kernel(const float4* __restrict__ vel, const uint32_t* __restrict__ perm, int64_t n,
@@ -98,20 +101,22 @@ struct SphParams {
   WalkCommon c;
   const float* hs;      // h, sorted
   const float4* aux;    // (h, P/rho^2, -, -) sorted
-  const float4* svel;   // sorted velocities or NULL
+  const float4* svel;   // sorted velocities (w: sound speed for the viscosity) or NULL
+  const float4* svis;   // sorted (alpha, Balsara f, -, -) or NULL
   const float2* c_sph;  // (b_max, r_SPH) per cell
   float* rho; uint32_t* nngb;   // density outputs (zeroed before the launch)
   float4* acc;                  // force output (zeroed before the launch)
 };
 
 // MODE 0: density (R16).  MODE 1: pressure force (R17).  MODE 2: pressure force + du/dt.
-// MODE 3: density + div v + rot v (SPH stage 1 of PAPER L252; R22).
+// MODE 3: density + div v + rot v (SPH stage 1 of PAPER L252; R22).  MODE 4: MODE 2 + artificial viscosity (R24).
 template <int T_, int MODE>
 struct SphVisitor {
-  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : 3);
+  static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : (MODE == 4 ? 4 : 3));
   static constexpr bool GATHER = MODE == 0 || MODE == 3;     // neighbours by the target's own h only (R16)
   const SphParams& p;
   float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
+  float prho[MODE == 4 ? T : 1], pc[MODE == 4 ? T : 1], pal[MODE == 4 ? T : 1], pf[MODE == 4 ? T : 1];   // viscosity inputs of the targets
   float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T], o4[T];
   uint32_t cnt_ngb[T];
   float glo[3], ghi[3], hmax;
@@ -126,8 +131,9 @@ struct SphVisitor {
       float4 v = p.c.spos[s];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z;
       if (GATHER) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
-      else { float4 a = p.aux[s]; ph[t] = a.x; ppr[t] = a.y; }
-      if (MODE >= 2) { float4 w = p.svel[s]; vx[t] = w.x; vy[t] = w.y; vz[t] = w.z; } else { vx[t] = vy[t] = vz[t] = 0.0f; }
+      else { float4 a = p.aux[s]; ph[t] = a.x; ppr[t] = a.y; if (MODE == 4) prho[t] = a.w; }
+      if (MODE >= 2) { float4 w = p.svel[s]; vx[t] = w.x; vy[t] = w.y; vz[t] = w.z; if (MODE == 4) pc[t] = w.w; } else { vx[t] = vy[t] = vz[t] = 0.0f; }
+      if (MODE == 4) { float4 q = p.svis[s]; pal[t] = q.x; pf[t] = q.y; }
       hmax = fmaxf(hmax, ph[t]);
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
@@ -166,6 +172,7 @@ struct SphVisitor {
     e.v[0] = p.c.spos[s];
     if (E >= 2) e.v[1] = MODE == 3 ? p.svel[s] : p.aux[s];
     if (E >= 3) e.v[2] = p.svel[s];
+    if (E >= 4) e.v[3] = p.svis[s];
     return e;
   }
   __device__ __forceinline__ void put(float4* dst, const Entry& e) const {
@@ -176,6 +183,7 @@ struct SphVisitor {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass
     if (E >= 2) dst[1] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);
     if (E >= 3) dst[2] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (E >= 4) dst[3] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
   static constexpr bool SUBMIT_LAST = false;
@@ -286,15 +294,24 @@ struct SphVisitor {
       float dj = qj <= 0.5f ? fmaf(18.0f * qj, qj, -12.0f * qj) : (qj < 1.0f ? -6.0f * uj * uj : 0.0f);
       float hi2 = hinv[t] * hinv[t], hj2i = hjinv * hjinv;
       float gw = (8.0f / PI_F) * 0.5f * fmaf(di, hi2 * hi2, dj * hj2i * hj2i) * rinv;   // (dW_i + dW_j)/(2r)
-      float f = a.w * (ppr[t] + b.y) * gw;
-      // a_i -= f (x_i - x_j)  =  += f e
-      o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
-      if (MODE == 2) {
+      float vd = 0.0f, Pi = 0.0f;
+      if (MODE == 2 || MODE == 4) {
         const float4 c = list[E * j + 2];
         // (v_i - v_j).(x_i - x_j) = -(v_i - v_j).e
-        float vd = -fmaf(vx[t] - c.x, ex, fmaf(vy[t] - c.y, ey, (vz[t] - c.z) * ez));
-        o3[t] = fmaf(0.5f * f, vd, o3[t]);
+        vd = -fmaf(vx[t] - c.x, ex, fmaf(vy[t] - c.y, ey, (vz[t] - c.z) * ez));
+        if (MODE == 4 && vd < 0.0f) {
+          // R24: approaching pair: Pi = fbar (-abar cbar mu + 2 abar mu^2) / rhobar, mu = l w / (r^2 + 0.01 l^2), l = (h_i + h_j)/4
+          const float4 q = list[E * j + 3];
+          const float l = 0.25f * (ph[t] + hj);
+          const float mu = l * vd * __fdividef(1.0f, fmaf(0.01f * l, l, r2));
+          const float ab = 0.5f * (pal[t] + q.x), cb = 0.5f * (pc[t] + c.w), fb = 0.5f * (pf[t] + q.y), rb = 0.5f * (prho[t] + b.w);
+          Pi = fb * ab * mu * fmaf(2.0f, mu, -cb) * __fdividef(1.0f, rb);
+        }
       }
+      float f = a.w * (ppr[t] + b.y + Pi) * gw;
+      // a_i -= f (x_i - x_j)  =  += f e
+      o0[t] = fmaf(f, ex, o0[t]); o1[t] = fmaf(f, ey, o1[t]); o2[t] = fmaf(f, ez, o2[t]);
+      if (MODE == 2 || MODE == 4) o3[t] = fmaf(0.5f * f, vd, o3[t]);
     }
   }
   __device__ __forceinline__ void store(int64_t g0, int lane) {
@@ -316,7 +333,7 @@ struct SphVisitor {
         } else {
           float* dst = reinterpret_cast<float*>(p.acc + i);
           atomicAdd(dst + 0, o0[t]); atomicAdd(dst + 1, o1[t]); atomicAdd(dst + 2, o2[t]);
-          if (MODE == 2) atomicAdd(dst + 3, o3[t]);
+          if (MODE == 2 || MODE == 4) atomicAdd(dst + 3, o3[t]);
         }
       }
     }
@@ -524,7 +541,7 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
                                         ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
   sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
   ctx->launches += 3;
-  p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->c_sph = ctx->c_sph;
+  p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->svis = nullptr; p->c_sph = ctx->c_sph;
   p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
   ctx->sph_radii_valid = true;
   return OTOO_OK;
@@ -574,11 +591,22 @@ otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d
 }
 
 otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
-                                int G, float* d_acc, cudaStream_t st) {
+                                const float* d_visc, int G, float* d_acc, cudaStream_t st) {
   SphParams p; int grid; size_t smem;
   OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
   gather_force_inputs_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_h, d_rho, d_P, reinterpret_cast<const float4*>(d_vel),
-                                                                          ctx->val[0], ctx->N, ctx->sorted_aux, ctx->sorted_vel);
+                                                                          reinterpret_cast<const float4*>(d_visc), ctx->val[0],
+                                                                          ctx->N, ctx->sorted_aux, ctx->sorted_vel, ctx->sorted_vis);
+  if (d_visc) {
+    p.svel = ctx->sorted_vel; p.svis = ctx->sorted_vis;
+    OTOO_CUDA(ctx, cudaMemsetAsync(d_acc, 0, 16 * (size_t)ctx->N, st));
+    p.acc = reinterpret_cast<float4*>(d_acc);
+    OTOO_TRY(launch_sph<4>(ctx, p, G, grid, smem, st));
+    ctx->launches += 2;
+    OTOO_CUDA(ctx, cudaGetLastError());
+    ctx->walked = true;
+    return OTOO_OK;
+  }
   OTOO_CUDA(ctx, cudaMemsetAsync(d_acc, 0, 16 * (size_t)ctx->N, st));
   p.acc = reinterpret_cast<float4*>(d_acc);
   if (d_vel) p.svel = ctx->sorted_vel;

@@ -323,6 +323,37 @@ def test_sph_stage1_divrot_parity(otoo, orc, n, G):
     assert np.all(d <= np.maximum(TOL * np.linalg.norm(ref["divrot"][:, 1:], axis=1), tol))
 
 
+@pytest.mark.parametrize("n,G", [(20000, 64), (7000 + 3, 32), (6000, 128)])
+def test_sph_force_viscosity_parity(otoo, orc, n, G):
+    """otoo_sph_force_visc (reading R24): the oracle fed the GPU's own fp32 rho, P; tolerance as the pressure force."""
+    w = gen.wd_pair(n, 5)
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    vel = np.zeros((n, 4), np.float32)
+    vel[:, :3] = -0.4 * pm[:, :3] + 0.1 * np.sin(7 * pm[:, [1, 2, 0]])
+    t = check_tree(otoo, orc, pm, 16)
+    rho, _ = otoo.otoo_sph_density(dev(h), G)
+    P = otoo.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
+    rg, Pg = rho.cpu().numpy(), P.cpu().numpy()
+    visc = np.zeros((n, 4), np.float32)
+    visc[:, 0] = np.sqrt((5.0 / 3.0) * Pg / rg)
+    visc[:, 1] = 0.5 + 0.5 * gen.uniform01(3, np.arange(n, dtype=np.uint64), 0)
+    visc[:, 2] = gen.uniform01(4, np.arange(n, dtype=np.uint64), 0)
+    ref = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel, visc=visc)
+    base = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel)
+    assert np.abs(ref["acc_dudt"] - base["acc_dudt"]).max() > 1e-3 * np.abs(base["acc_dudt"]).max()   # the term is there
+    out = otoo.otoo_sph_force_visc(dev(h), rho, P, dev(vel), dev(visc), G).cpu().numpy()
+    e, raw = acc_err(out, ref["acc_dudt"], ref["abs_sum"][:, 0])
+    assert e.max() <= TOL, e.max()
+    assert np.percentile(raw, 99) <= TOL
+    tol = np.maximum(1e-5 * np.abs(ref["acc_dudt"][:, 3]), 8 * U32 * ref["abs_sum"][:, 1])
+    assert np.all(np.abs(out[:, 3] - ref["acc_dudt"][:, 3]) <= tol)
+    v0 = visc.copy()
+    v0[:, 1] = 0.0                                                                                   # alpha = 0: the plain force
+    out0 = otoo.otoo_sph_force_visc(dev(h), rho, P, dev(vel), dev(v0), G).cpu().numpy()
+    plain = otoo.otoo_sph_force(dev(h), rho, P, G, vel=dev(vel)).cpu().numpy()
+    assert np.allclose(out0, plain, rtol=1e-5, atol=1e-6 * np.abs(plain).max())
+
+
 def test_status_codes(otoo):
     from paper_1206_1199_b200 import binding
     fresh = binding.Otoo(max_particles=1000)
