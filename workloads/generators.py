@@ -95,6 +95,21 @@ def uniform_sphere(n: int, seed: int) -> np.ndarray:
     return _pack(r * ux, r * uy, r * uz, np.full(n, 1.0 / n))
 
 
+def cold_sphere(n: int, seed: int, u0: float = 0.05):
+    """The paper's gravity+SPH test ("Cold Collapse Test" [50],[51]): an isothermal sphere,
+    rho ~ r^-2 (M(<r) ~ r: the radius is uniform in [0,1)), M = R = G = 1, at rest, cold (specific internal
+    energy u0 << |W|/M = 1).  Returns dict pos_mass (n,4), vel (n,4) zeros, u (n,), h (n,) support radius for
+    ~50 neighbours from the model density rho(r) = 1/(4 pi r^2)."""
+    idx = np.arange(n, dtype=np.uint64)
+    r = np.maximum(uniform01(seed, idx, 2), 1e-6)
+    ux, uy, uz = _isotropic(seed, idx, 0)
+    m = 1.0 / n
+    rho = 1.0 / (4.0 * np.pi * r * r)
+    h = np.minimum((3.0 * 50.0 * m / (4.0 * np.pi * rho)) ** (1.0 / 3.0), 0.3)
+    return dict(pos_mass=_pack(r * ux, r * uy, r * uz, np.full(n, m)), vel=np.zeros((n, 4), np.float32),
+                u=np.full(n, u0, np.float32), h=h.astype(np.float32))
+
+
 def lattice(k: int, spacing: float = 1.0, mass: float = 1.0) -> np.ndarray:
     """k^3 simple cubic lattice, first point at the origin."""
     g = np.arange(k, dtype=np.float64) * spacing
