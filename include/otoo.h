@@ -167,6 +167,11 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
  * order (the paper's own ordering; R20) -- same cells, other order: no group straddles an
  * octant boundary with a system-sized box, fewer interactions at the same theta.  Read by the next
  * otoo_build_tree; otoo_cell_t.prefix is then a Hilbert-key prefix.
+ * "group_begin" = b, "group_count" = c (defaults 0, -1 = to the end): the walks (gravity and SPH) cover only the
+ * target groups [b, b + c) of the group_size they are called with; outputs of other targets stay zero and
+ * the counters cover the range.  This is the paper's multi-device scheme (PAPER.md III-E, L179): every device
+ * builds the same tree and takes a contiguous range of targets in key order; the ranges' outputs add up to
+ * the whole.  A range outside the groups of a call: OTOO_ERR_INVALID_ARG.
  * "group_distance" = 0 (default): the gravity MAC compares r_b with the distance from the group's bounding box
  * (R8); 1: with the actual minimum of the members' distances, as the paper does (R23):
  * shorter lists (no system-sized boxes), costlier tests.  Gravity only; needs "warp_specialized" = 1.

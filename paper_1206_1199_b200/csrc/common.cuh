@@ -96,6 +96,7 @@ struct otoo_ctx {
   uint32_t level_off[OTOO_NLEV + 1];
   int walk_stack;        // option "walk_stack"
   int use_pool;          // option "task_pool"
+  int64_t group_begin, group_count;   // options: the walks cover groups [begin, begin + count) only (count < 0: to the end)
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int walk_only;         // option "walk_only" (diagnostic)
   int dist_kind;         // option "group_distance": 0 AABB (R8), 1 exact minimum over the group's members (R23)

@@ -359,7 +359,7 @@ otoo_status launch_walk_ws2(otoo_ctx* ctx, const GravParams& p, cudaStream_t st)
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_gravity_ws_kernel<T, EPS0>, OTOO_WS_PAIRS * 64, smem));
   if (occ < 1) occ = 1;
   int64_t grid = (int64_t)ctx->sm_count * occ;                       // persistent: every CTA resident
-  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups, OTOO_WS_PAIRS);
+  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups > 0 ? p.c.ngroups : 1, OTOO_WS_PAIRS);
   walk_gravity_ws_kernel<T, EPS0><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
   return OTOO_OK;
 }
@@ -398,8 +398,13 @@ size_t otoo_walk_smem_bytes() {
 
 // Common launch preparation of the walk kernels: persistent grid, task pool, zeroed counters.
 otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st) {
-  const int64_t ngroups = cdiv(ctx->N, G);
-  OTOO_TRY(otoo_ensure_groups(ctx, ngroups));
+  const int64_t total_groups = cdiv(ctx->N, G);
+  // target sharding (PAPER III-E, L179: every device holds the whole tree and walks a contiguous range of targets)
+  const int64_t g_begin = ctx->group_begin;
+  const int64_t ngroups = ctx->group_count < 0 ? total_groups - g_begin : ctx->group_count;
+  if (g_begin < 0 || ngroups < 0 || g_begin + ngroups > total_groups)
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_begin / group_count outside the groups of this group_size");
+  OTOO_TRY(otoo_ensure_groups(ctx, total_groups));
   *smem = otoo_walk_smem_bytes();
   int per_sm = (int)((227 * 1024) / (*smem + 1024));
   if (per_sm < 1) per_sm = 1;
@@ -407,7 +412,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   const int64_t warps = (int64_t)ctx->sm_count * per_sm * OTOO_WALK_WARPS;
   if (warps >= OTOO_POOL_MARGIN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "internal: task pool margin below resident warps");
   *grid = ctx->sm_count * per_sm;
-  if ((int64_t)*grid * OTOO_WALK_WARPS > ngroups) *grid = (int)cdiv(ngroups, OTOO_WALK_WARPS);
+  if ((int64_t)*grid * OTOO_WALK_WARPS > ngroups) *grid = (int)cdiv(ngroups > 0 ? ngroups : 1, OTOO_WALK_WARPS);
   OTOO_TRY(otoo_ensure_spill(ctx, warps));
   if (!ctx->pool_slots) {
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->pool_slots, sizeof(TaskSlot) * (size_t)OTOO_POOL_SLOTS));
@@ -415,12 +420,12 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->walk_shared, sizeof(WalkShared)));
   }
   walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq, (int)ngroups);
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)ngroups, st));
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)ngroups, st));
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)ngroups, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)total_groups, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)total_groups, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 8 * sizeof(unsigned long long), st));
   c->spos = ctx->spos; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
-  c->N = ctx->N; c->ngroups = ngroups;
+  c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
@@ -428,7 +433,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->walk_only = ctx->walk_only;
   c->dist_kind = 0;
   ctx->launches += 1;
-  ctx->last_group_size = G; ctx->last_ngroups = ngroups;
+  ctx->last_group_size = G; ctx->last_ngroups = total_groups;
   return OTOO_OK;
 }
 

@@ -492,7 +492,7 @@ otoo_status launch_sph_ws2(otoo_ctx* ctx, const SphParams& p, cudaStream_t st) {
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_ws_kernel<T, MODE>, OTOO_WS_PAIRS * 64, smem));
   if (occ < 1) occ = 1;
   int64_t grid = (int64_t)ctx->sm_count * occ;
-  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups, OTOO_WS_PAIRS);
+  if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups > 0 ? p.c.ngroups : 1, OTOO_WS_PAIRS);
   walk_sph_ws_kernel<T, MODE><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
   return OTOO_OK;
 }

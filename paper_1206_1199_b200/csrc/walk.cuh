@@ -62,7 +62,8 @@ struct WalkShared {                   // device-global control block, reset befo
 };
 struct WalkCommon {
   const float4* spos; const float4* cell_cm; const cellb_t* cell_b; const uint32_t* perm;
-  int64_t N, ngroups;
+  int64_t N, ngroups;                                           // ngroups: groups of THIS launch, starting at g_begin
+  uint32_t g_begin;                                             // (target sharding over devices)
   uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;   // zeroed before the launch
   unsigned long long* sums;                                    // tests, interactions, cells, parts
   WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
@@ -118,7 +119,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     if (!got && !main_done) {
       if (lane == 0) g = atomicAdd(&c.ws->queue, 1u);
       g = __shfl_sync(0xFFFFFFFFu, g, 0);
-      if ((int64_t)g < c.ngroups) { got = true; if (lane == 0) stk[0] = 0u; sp = 1; }
+      if ((int64_t)g < c.ngroups) { got = true; g += c.g_begin; if (lane == 0) stk[0] = 0u; sp = 1; }
       else main_done = true;
     }
     if (!got) {

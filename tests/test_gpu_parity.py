@@ -354,6 +354,54 @@ def test_sph_force_viscosity_parity(otoo, orc, n, G):
     assert np.allclose(out0, plain, rtol=1e-5, atol=1e-6 * np.abs(plain).max())
 
 
+@pytest.mark.parametrize("world,by_cost", [(3, False), (4, True)])
+def test_target_sharding_ranges_add_up(otoo, orc, world, by_cost):
+    """The paper's multi-device scheme (PAPER.md III-E, L179) on one GPU: the ranks' ranges are run one after the
+    other on the same tree (no rank waits for another); every group's counters are those of the oracle, each
+    target is written by exactly one range, and the ranges' outputs add up to the single-call result."""
+    from paper_1206_1199_b200 import sharded
+    n, G = 40000, 64
+    pm = gen.plummer(n, 8)
+    t = check_tree(otoo, orc, pm, 16)
+    ref = t.gravity(0.01, 0.5, G)
+    whole = otoo.otoo_gravity(0.01, 0.5, G).cpu().numpy()
+    ng = t.n_groups(G)
+    cost = (ref["n_cells"].astype(np.int64) + ref["n_parts"]) if by_cost else None
+    ranges = sharded.group_ranges(ng, world, cost)
+    total = np.zeros((n, 4), np.float64)
+    written = np.zeros(n, np.int32)
+    perm = t.export()["perm"].astype(np.int64)
+    inter = 0
+    try:
+        for b, c in ranges:
+            otoo.otoo_set_option("group_begin", b)
+            otoo.otoo_set_option("group_count", c)
+            part = otoo.otoo_gravity(0.01, 0.5, G).cpu().numpy()
+            nt, nc, npart = otoo.otoo_export_group_stats()
+            assert np.array_equal(nt[b:b + c], ref["n_tests"][b:b + c]) and np.array_equal(nc[b:b + c], ref["n_cells"][b:b + c])
+            assert not nt[:b].any() and not nt[b + c:].any()
+            inter += otoo.otoo_last_stats()["sum_interactions"]
+            mine = perm[b * G:min((b + c) * G, n)]
+            written[mine] += 1
+            rest = np.setdiff1d(np.arange(n), mine)
+            assert not part[rest].any()
+            total += part
+        otoo.otoo_set_option("group_begin", ng)                    # an empty range at the end is legal, one past it is not
+        otoo.otoo_set_option("group_count", 0)
+        assert not otoo.otoo_gravity(0.01, 0.5, G).cpu().numpy().any()
+        otoo.otoo_set_option("group_count", 1)
+        from paper_1206_1199_b200 import binding
+        with pytest.raises(binding.OtooError):
+            otoo.otoo_gravity(0.01, 0.5, G)
+    finally:
+        otoo.otoo_set_option("group_begin", 0)
+        otoo.otoo_set_option("group_count", -1)
+    assert np.all(written == 1) and inter == ref["interactions"]
+    assert np.allclose(total, whole, rtol=2e-6, atol=1e-6 * np.abs(whole).max())
+    e, _ = acc_err(total.astype(np.float32), ref["acc_pot"], ref["abs_sum"])
+    assert e.max() <= TOL
+
+
 def test_status_codes(otoo):
     from paper_1206_1199_b200 import binding
     fresh = binding.Otoo(max_particles=1000)
