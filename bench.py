@@ -43,10 +43,12 @@ SM_LANES = 128                      # FP32 lanes per SM
 NOMINAL_SM_MHZ = 1965.0
 
 
-def workload(name: str, theta, seed: int):
+def workload(name: str, theta, seed: int, n=None):
     cfg = dict(gen.CONFIGS[name])
     if theta is not None:
         cfg["theta"] = theta
+    if n is not None:
+        cfg["n"] = int(n)
     pm = gen.make(cfg["kind"], cfg["n"], seed)
     return cfg, pm
 
@@ -99,7 +101,7 @@ def run_reference(args, rank):
     if rank != 0:
         return
     from oracle import oracle
-    cfg, pm = workload(args.workload, args.theta, args.seed)
+    cfg, pm = workload(args.workload, args.theta, args.seed, args.n)
     eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
     times, inter = [], 0
     for it in range(args.warmup + args.steps):
@@ -148,6 +150,7 @@ def main():
     ap.add_argument("--delta", type=float, default=None)
     ap.add_argument("--m-limit", type=float, default=None)
     ap.add_argument("--seed", type=int, default=1206)
+    ap.add_argument("--n", type=int, default=None, help="override the workload's particle count (scaling runs, e.g. Fig. 9)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -166,7 +169,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     # replicas only: every rank runs the same workload with its own seed
-    cfg, pm = workload(args.workload, args.theta, replicas.replica_seed(args.seed, rank))
+    cfg, pm = workload(args.workload, args.theta, replicas.replica_seed(args.seed, rank), args.n)
     n, G, n_crit = cfg["n"], cfg["group"], cfg["n_crit"]
     eps, theta = float(np.float32(cfg["eps"])), float(np.float32(cfg["theta"]))
     delta = float(np.float32(args.delta if args.delta is not None else cfg.get("delta", 0.01)))
@@ -264,9 +267,9 @@ def main():
     build_info = {"ms": build_ms, "bound": "hbm", "algorithmic_bytes": BUILD_BYTES_PER_PARTICLE * n, "achieved_gbs": build_gbs,
                   "peak_gbs": hbm, "frac": build_gbs / hbm, "peak_source": hbm_src}
     sph_info = None
-    if cfg["kind"] == "wd_pair" and world == 1:
-        # BASELINE config 4: the SPH rows (H11-H13) on the same tree, timed like the gravity step
-        w = gen.wd_pair(n, replicas.replica_seed(args.seed, rank))
+    if cfg["kind"] in ("wd_pair", "cold_sphere") and world == 1:
+        # BASELINE config 4 / the paper's cold collapse: the SPH rows (H11-H13) on the same tree, timed like the gravity step
+        w = (gen.wd_pair if cfg["kind"] == "wd_pair" else gen.cold_sphere)(n, replicas.replica_seed(args.seed, rank))
         d_h, d_u, d_v = (torch.from_numpy(w[k]).cuda() for k in ("h", "u", "vel"))
         Gs = cfg.get("group_sph", 64)
         ts = []

@@ -206,6 +206,9 @@ CONFIGS = {
     "C5": dict(kind="uniform_cube", n=33554432, eps=0.001, theta=0.5, n_crit=16, group=256),
     # not a BASELINE config: the paper's own gravity benchmark (uniform sphere, r = 1, M = 1,
     # N = 8000 x 1024, Delta = 0.01, n_crit = 16, m_limit = 0.05), run with otoo_gravity_delta (bench.py --mac delta)
+    # the paper's gravity+SPH benchmark (Fig. 9: cold collapse, Delta = 0.01, n_crit = 16, m_limit = 0.05;
+    # N = 2 M is the size its text quotes, L242); bench.py --workload COLD --mac delta [--n N]
+    "COLD": dict(kind="cold_sphere", n=2097152, eps=0.005, theta=0.5, n_crit=16, group=128, group_sph=64, delta=0.01, m_limit=0.05),
     "F4": dict(kind="uniform_sphere", n=8192000, eps=0.002, theta=0.6, n_crit=16, group=128, delta=0.01, m_limit=0.05),
 }
 
@@ -221,4 +224,6 @@ def make(kind: str, n: int, seed: int):
         return uniform_sphere(n, seed)
     if kind == "wd_pair":
         return wd_pair(n, seed)["pos_mass"]
+    if kind == "cold_sphere":
+        return cold_sphere(n, seed)["pos_mass"]
     raise ValueError(kind)
