@@ -281,33 +281,6 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, const Moment
   cell_cm[c] = make_float4(__double2float_rn(cx), __double2float_rn(cy), __double2float_rn(cz), __double2float_rn(M));
   double dx = __dsub_rn(cx, g[0]), dy = __dsub_rn(cy, g[1]), dz = __dsub_rn(cz, g[2]);
   c_s[c] = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
-  // PAPER Eq. 2, B2 = sum m |r_CM - r|^2, accumulated bottom-up in a fixed order (R19): leaf: its particles in
-  // slot order; internal: children in octant order, B2 += B2_child, then B2 += M_child |CM_child - CM|^2
-  double b2 = 0.0;
-  if (nch == 0) {
-    for (uint32_t s0 = first; s0 < first + count; s0 += 8) {
-      float4 p[8];
-      const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
-#pragma unroll
-      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) p[j] = spos[s0 + j];
-#pragma unroll
-      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) {
-        const double ex = __dsub_rn((double)p[j].x, cx), ey = __dsub_rn((double)p[j].y, cy), ez = __dsub_rn((double)p[j].z, cz);
-        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-        b2 = __dadd_rn(b2, __dmul_rn((double)p[j].w, r2));
-      }
-    }
-  } else {
-    const uint32_t ch = c_child_first[c];
-    for (int k = 0; k < nch; k++) {
-      const double* q = cm64 + 3 * (size_t)(ch + k);
-      const double ex = __dsub_rn(q[0], cx), ey = __dsub_rn(q[1], cy), ez = __dsub_rn(q[2], cz);
-      const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-      b2 = __dadd_rn(b2, a.c_B2[ch + k]);
-      b2 = __dadd_rn(b2, __dmul_rn(MP[4 * (size_t)(ch + k)], r2));
-    }
-  }
-  a.c_B2[c] = b2;
 }
 // the whole bottom-up pass in ONE cooperative launch: every level deepest first, a grid-wide barrier
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
@@ -357,10 +330,55 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   return OTOO_OK;
 }
 
+
+// PAPER Eq. 2 for the absolute-error MAC, computed on demand (otoo_gravity_delta) after the moments pass
+__device__ __forceinline__ void b2_cell(uint32_t c, const MomentArgs& a) {
+  const float4* __restrict__ spos = a.spos;
+  const uint32_t first = a.c_first[c], count = a.c_count[c];
+  const int nch = a.c_child_count[c];
+  const uint32_t* __restrict__ c_child_first = a.c_child_first;
+  const double* cm64 = a.cm64; const double* MP = a.MP;
+  const double cx = cm64[3 * (size_t)c], cy = cm64[3 * (size_t)c + 1], cz = cm64[3 * (size_t)c + 2];
+  // PAPER Eq. 2, B2 = sum m |r_CM - r|^2, accumulated bottom-up in a fixed order (R19): leaf: its particles in
+  // slot order; internal: children in octant order, B2 += B2_child, then B2 += M_child |CM_child - CM|^2
+  double b2 = 0.0;
+  if (nch == 0) {
+    for (uint32_t s0 = first; s0 < first + count; s0 += 8) {
+      float4 p[8];
+      const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) p[j] = spos[s0 + j];
+#pragma unroll
+      for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) {
+        const double ex = __dsub_rn((double)p[j].x, cx), ey = __dsub_rn((double)p[j].y, cy), ez = __dsub_rn((double)p[j].z, cz);
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        b2 = __dadd_rn(b2, __dmul_rn((double)p[j].w, r2));
+      }
+    }
+  } else {
+    const uint32_t ch = c_child_first[c];
+    for (int k = 0; k < nch; k++) {
+      const double* q = cm64 + 3 * (size_t)(ch + k);
+      const double ex = __dsub_rn(q[0], cx), ey = __dsub_rn(q[1], cy), ez = __dsub_rn(q[2], cz);
+      const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+      b2 = __dadd_rn(b2, a.c_B2[ch + k]);
+      b2 = __dadd_rn(b2, __dmul_rn(MP[4 * (size_t)(ch + k)], r2));
+    }
+  }
+  a.c_B2[c] = b2;
+}
+__global__ void __launch_bounds__(256) b2_all_kernel(const LevelOff off, const int depth, const MomentArgs a) {
+  cg::grid_group grid = cg::this_grid();
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+  for (int l = depth; l >= 0; l--) {
+    for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) b2_cell(c, a);
+    if (l > 0) grid.sync();
+  }
+}
 }  // namespace
 
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st) {
-  ctx->built = false; ctx->walked = false; ctx->sph_radii_valid = false;
+  ctx->built = false; ctx->walked = false; ctx->sph_radii_valid = false; ctx->b2_valid = false;
   const float4* pos = reinterpret_cast<const float4*>(d_pos_mass);
   unsigned* bbox = reinterpret_cast<unsigned*>(ctx->d_bbox);
   const unsigned nbN = (unsigned)cdiv(N, 256);
@@ -424,6 +442,29 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   for (int k = 0; k < 3; k++) ctx->lo[k] = ctx->h_root[k];
   ctx->S = ctx->h_root[3];
   for (int l = 0; l <= OTOO_NLEV; l++) ctx->level_off[l] = off.v[l];
+  ctx->key_order_built = ctx->key_order;
   ctx->built = true;
+  return OTOO_OK;
+}
+
+// B2 of every cell (PAPER Eq. 2; R19) for the absolute-error MAC: one cooperative bottom-up pass, once per build
+otoo_status otoo_b2_impl(otoo_ctx* ctx, cudaStream_t st) {
+  if (ctx->b2_valid) return OTOO_OK;
+  LevelOff off;
+  for (int l = 0; l <= OTOO_NLEV; l++) off.v[l] = ctx->level_off[l];
+  const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
+                      reinterpret_cast<const unsigned*>(ctx->d_bbox), ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order_built};
+  int occ = 1;
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, b2_all_kernel, 256, 0));
+  if (occ > 4) occ = 4;
+  int64_t grid = (int64_t)ctx->sm_count * (occ < 1 ? 1 : occ);
+  uint32_t widest = 1;
+  for (int l = 0; l <= ctx->depth; l++) if (off.v[l + 1] - off.v[l] > widest) widest = off.v[l + 1] - off.v[l];
+  if (grid > cdiv(widest, 256)) grid = cdiv(widest, 256);
+  int depth_arg = ctx->depth;
+  void* args[] = {(void*)&off, (void*)&depth_arg, (void*)&ma};
+  OTOO_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)b2_all_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
+  ctx->launches += 1;
+  ctx->b2_valid = true;
   return OTOO_OK;
 }

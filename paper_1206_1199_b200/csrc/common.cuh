@@ -90,6 +90,8 @@ struct otoo_ctx {
   bool built;
   bool walked;
   bool sph_radii_valid;
+  bool b2_valid;         // c_B2 computed for the current tree (on demand, by otoo_gravity_delta)
+  int key_order_built;   // key order of the current tree
   int64_t N, N_cell, N_leaf;
   int n_crit, depth;
   float lo[3], S;
@@ -137,6 +139,7 @@ otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, ui
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st);
 // mac 0: theta criterion (p0 = theta); mac 1: the paper's absolute-error criterion (p0 = Delta, p1 = m_limit)
 otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float p1, int G, float* d_acc_pot, cudaStream_t st);
+otoo_status otoo_b2_impl(otoo_ctx* ctx, cudaStream_t st);     // B2 of every cell into c_B2 (build.cu), once per build
 otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st);   // fp64 b_max of every cell into sph_acc[2c] (sph.cu)
 otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb,
                                   cudaStream_t st);

@@ -66,7 +66,7 @@ __device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); re
 
 template <int T_, bool EPS0>
 struct GravVisitor {
-  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64, UNR = OTOO_EVAL_UNR;
+  static constexpr int T = T_, E = 1, LCAP = OTOO_LIST_CAP, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64, UNR = OTOO_EVAL_UNR;
   const GravParams& p;
   float pm[T];
   float glo[3], ghi[3];
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(cons
 // sums; submit() publishes the filled buffer to the pair's evaluator warp and returns the next one.
 template <int T_>
 struct GravWalker {
-  static constexpr int T = T_, E = 1, NP = (T_ + 1) / 2;
+  static constexpr int T = T_, E = 1, LCAP = OTOO_WS_LCAP, NP = (T_ + 1) / 2;
   static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
   typedef WsPair<32 * NP * 3, 32 * T_> Pair;
   const GravParams& p;
@@ -444,6 +444,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   if (mac == 0) {
     rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b);
   } else {
+    OTOO_TRY(otoo_b2_impl(ctx, st));
     OTOO_TRY(otoo_bmax_impl(ctx, st));
     rb2_delta_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_B2, ctx->c_MP, ctx->sph_acc, ctx->N_cell, ctx->S,
                                                                          p0, p1, ctx->cell_b);

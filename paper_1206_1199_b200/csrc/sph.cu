@@ -113,6 +113,7 @@ struct SphParams {
 template <int T_, int MODE>
 struct SphVisitor {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : (MODE == 4 ? 4 : 3));
+  static constexpr int LCAP = OTOO_LIST_CAP;
   static constexpr bool GATHER = MODE == 0 || MODE == 3;     // neighbours by the target's own h only (R16)
   const SphParams& p;
   float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
@@ -360,6 +361,7 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const Sp
 template <int T_, int MODE>
 struct SphWalker {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
+  static constexpr int LCAP = OTOO_WS_LCAP;
   static constexpr bool SUBMIT_LAST = true;
   typedef WsPair<2> Pair;
   const SphParams& p;

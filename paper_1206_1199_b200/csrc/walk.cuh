@@ -79,6 +79,7 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 // Visitor contract (all members __forceinline__):
 //   static constexpr int T;            targets per lane
 //   static constexpr int E;            float4 per list entry
+//   static constexpr int LCAP;         float4 per list buffer
 //   void load_group(int64_t g0, int lane, float4* scratch)   targets into registers, AABB, zero accumulators
 //   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
 //   struct Entry; Entry get(uint32_t slot); void put(float4* dst, const Entry&)   one particle entry (E float4)
@@ -92,7 +93,7 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 template <class V>
 __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list0, uint32_t* stk, int lane, int64_t gwarp) {
   constexpr int G = 32 * V::T;
-  constexpr int CAP = (OTOO_LIST_CAP / V::E) & ~3;   // list entries (multiple of the padding unit)
+  constexpr int CAP = (V::LCAP / V::E) & ~3;         // list entries per buffer (multiple of the padding unit)
   constexpr int PADTO = 4;
   uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;
   unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;

@@ -15,7 +15,9 @@
 #ifndef OTOO_WS_NBUF
 #define OTOO_WS_NBUF 2      // list buffers per pair
 #endif
+#ifndef OTOO_WS_LCAP
 #define OTOO_WS_LCAP 256    // float4 entries per buffer
+#endif
 
 enum : uint32_t { WS_FIRST = 1u, WS_LAST = 2u, WS_EXIT = 4u };
 struct WsMeta { uint32_t count, flags, group, pad; };
