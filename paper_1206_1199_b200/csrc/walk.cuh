@@ -285,7 +285,9 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
         const int cnt = open_leaf ? (int)B.z : 0;
         const int inc = warp_inclusive_scan(cnt, lane);
         const int total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-        unsigned m = lm;
+        // only the few leaves that overlap the group's own slots can hold a target (one ballot instead of a
+        // shuffle round per opened leaf: ~450 leaves are opened per group, ~10 of them overlap it)
+        unsigned m = __ballot_sync(0xFFFFFFFFu, open_leaf && (int64_t)B.y < g0 + G && (int64_t)B.y + (int64_t)B.z > g0);
         while (m) {  // which targets sit in an opened leaf: their self term is in the list
           const int src = __ffs(m) - 1; m &= m - 1;
           v.mark_self(__shfl_sync(0xFFFFFFFFu, B.y, src), __shfl_sync(0xFFFFFFFFu, B.z, src), g0, lane);
