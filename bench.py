@@ -253,7 +253,7 @@ def main():
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
                 # profiles/r1_walk_gravity_full.md (C2, theta=0.6 only); the kernel is ALU-bound, DRAM < 1 %
-                "traffic": 53.09e6 if (args.workload == "C2" and args.theta is None and args.n is None and args.mac == "theta"
+                "traffic": 53.70e6 if (args.workload == "C2" and args.theta is None and args.n is None and args.mac == "theta"
                                        and args.key_order == "morton" and args.group_distance == "box") else None,
                 "peak_source": f"derived: {sm_count} SMs x 128 FP32 lanes x 2 flop x {NOMINAL_SM_MHZ:.0f} MHz (DESIGN.md)",
                 "peak_measured_ffma": peak_measured, "frac_of_measured": achieved / peak_measured,
