@@ -6,7 +6,7 @@
  *
  * The method is an approximation (a tree code), so the oracle follows the algorithm step by
  * step in the paper's order (section II, III-B, III-C, III-D), with the readings
- * R1..R17 listed in DESIGN.md.  The O(N^2) definition (orc_direct_sum) is its truth check.
+ * R1..R24 listed in DESIGN.md.  The O(N^2) definition (orc_direct_sum) is its truth check.
  * All host pointers.  Positions/masses come in as fp32 (single precision),
  * every sum is fp64; the quantities that decide an integer (key quantisation, the MAC compare,
  * the SPH neighbour compare) are evaluated in fp32 exactly as DESIGN.md states.
@@ -15,7 +15,12 @@
  * cell, tiling invariant of the lists, stackless walk == recursive walk,
  * theta=0 == direct sum, Newton's third law, two-body closed form, Plummer potential, kernel
  * normalisation, lattice density, brute-force SPH neighbour sets; Delta-MAC: two-particle cell and
- * Eq. 3, B2 bottom-up == Eq. 2 direct, per-cell error <= Delta, r_b limits (L81).
+ * Eq. 3, B2 bottom-up == Eq. 2 direct, per-cell error <= Delta, r_b limits (L81);
+ * exact-minimum group distance (L163): brute force over members, lists never longer than the box lists;
+ * Hilbert keys (L131): bijection, face adjacency of consecutive keys, hierarchy, inverse, same cells as
+ * the Morton tree; adaptive h: fixed point, lattice count steps; div v / rot v: linear fields, rigid
+ * rotation; artificial viscosity: alpha = 0 / f = 0 limits, receding flow, momentum and energy balance,
+ * two-particle closed form.
  * parity unpinned: the absolute accuracy level of the theta-MAC (the paper's error plot, Fig. 5,
  * is for its Delta-MAC and is missing from PAPER.md).
  */
