@@ -52,10 +52,11 @@ def vec_check(got, want, abs_sum, pct):
     assert np.percentile(d / np.maximum(an, 1e-300), pct) <= TOL
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5", "C2:hilbert", "C3:hilbert"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5", "C2:hilbert", "C3:hilbert", "C2:exact", "C3:hilbert+exact"])
 def test_fullsize_gravity(orc, name):
     name, _, order = name.partition(":")
-    key_order = 1 if order == "hilbert" else 0
+    key_order = 1 if "hilbert" in order else 0
+    dist_kind = 1 if "exact" in order else 0
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from paper_1206_1199_b200 import binding
@@ -67,8 +68,10 @@ def test_fullsize_gravity(orc, name):
     try:
         d_pm = dev(pm)
         o.otoo_set_option("key_order", key_order)
+        o.otoo_set_option("group_distance", dist_kind)
         o.otoo_build_tree(d_pm, cfg["n_crit"])
         t = orc.Tree(pm, cfg["n_crit"], key_order=key_order)
+        t.set_dist_kind(dist_kind)
         perm = check_tree_full(o, t).astype(np.int64)
         out = o.otoo_gravity(eps, theta, G).cpu().numpy()
         assert np.array_equal(o.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta).view(np.uint32))
