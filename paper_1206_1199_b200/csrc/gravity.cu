@@ -127,7 +127,8 @@ struct GravVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
-  static constexpr bool SUBMIT_LAST = false;
+  static constexpr bool SUBMIT_LAST = false, CULL = false;
+  template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
   __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
     if (!p.c.walk_only) eval(list, n);
     return list;
@@ -208,6 +209,8 @@ template <int T_>
 struct GravWalker {
   static constexpr int T = T_, E = 1, LCAP = OTOO_WS_LCAP, NP = (T_ + 1) / 2;
   static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
+  static constexpr bool CULL = false;
+  template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
   typedef WsPair<32 * NP * 3, 32 * T_> Pair;
   const GravParams& p;
   Pair& sm;

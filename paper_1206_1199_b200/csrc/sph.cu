@@ -110,6 +110,9 @@ struct SphParams {
 
 // MODE 0: density (R16).  MODE 1: pressure force (R17).  MODE 2: pressure force + du/dt.
 // MODE 3: density + div v + rot v (SPH stage 1 of PAPER L252; R22).  MODE 4: MODE 2 + artificial viscosity (R24).
+#ifndef OTOO_SPH_CULL
+#define OTOO_SPH_CULL 1    // walk-time cull of particles out of reach of the group's box (keep())
+#endif
 template <int T_, int MODE>
 struct SphVisitor {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : (MODE == 4 ? 4 : 3));
@@ -179,6 +182,20 @@ struct SphVisitor {
   __device__ __forceinline__ void put(float4* dst, const Entry& e) const {
 #pragma unroll
     for (int k = 0; k < E; k++) dst[k] = e.v[k];
+  }
+  // Walk-time cull: a particle of an opened leaf enters the list only if it can be a neighbour of some member.
+  // Its distance to the group's box, taken with the operations and the order of pass 1's r^2 chain, is never
+  // above the fp32 r^2 to any member (every step is monotone in |component|), and the limit is the largest
+  // one a member can have, so "box d^2 >= limit" implies that every pair test of this entry fails.
+  static constexpr bool CULL = OTOO_SPH_CULL != 0;
+  __device__ __forceinline__ bool keep(const Entry& e) const {
+    const float4 a = e.v[0];
+    const float bx = fmaxf(fmaxf(__fsub_rn(glo[0], a.x), __fsub_rn(a.x, ghi[0])), 0.0f);
+    const float by = fmaxf(fmaxf(__fsub_rn(glo[1], a.y), __fsub_rn(a.y, ghi[1])), 0.0f);
+    const float bz = fmaxf(fmaxf(__fsub_rn(glo[2], a.z), __fsub_rn(a.z, ghi[2])), 0.0f);
+    const float d2 = __fmaf_rn(bz, bz, __fmaf_rn(by, by, __fmul_rn(bx, bx)));
+    const float hm2 = __fmul_rn(hmax, hmax);
+    return d2 < (GATHER ? hm2 : fmaxf(hm2, e.v[E >= 2 ? 1 : 0].z));
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass
@@ -420,6 +437,20 @@ struct SphWalker {
   __device__ __forceinline__ void put(float4* dst, const Entry& e) const {
 #pragma unroll
     for (int k = 0; k < E; k++) dst[k] = e.v[k];
+  }
+  // Walk-time cull: a particle of an opened leaf enters the list only if it can be a neighbour of some member.
+  // Its distance to the group's box, taken with the operations and the order of pass 1's r^2 chain, is never
+  // above the fp32 r^2 to any member (every step is monotone in |component|), and the limit is the largest
+  // one a member can have, so "box d^2 >= limit" implies that every pair test of this entry fails.
+  static constexpr bool CULL = OTOO_SPH_CULL != 0;
+  __device__ __forceinline__ bool keep(const Entry& e) const {
+    const float4 a = e.v[0];
+    const float bx = fmaxf(fmaxf(__fsub_rn(glo[0], a.x), __fsub_rn(a.x, ghi[0])), 0.0f);
+    const float by = fmaxf(fmaxf(__fsub_rn(glo[1], a.y), __fsub_rn(a.y, ghi[1])), 0.0f);
+    const float bz = fmaxf(fmaxf(__fsub_rn(glo[2], a.z), __fsub_rn(a.z, ghi[2])), 0.0f);
+    const float d2 = __fmaf_rn(bz, bz, __fmaf_rn(by, by, __fmul_rn(bx, bx)));
+    const float hm2 = __fmul_rn(hmax, hmax);
+    return d2 < (MODE == 0 ? hm2 : fmaxf(hm2, e.v[E >= 2 ? 1 : 0].z));
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);

@@ -83,6 +83,8 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 //   void load_group(int64_t g0, int lane, float4* scratch)   targets into registers, AABB, zero accumulators
 //   int  classify(uint32_t cell, float4& A, cellb_t& B)   0 = drop, 1 = accept (A goes to the list), 2 = open
 //   struct Entry; Entry get(uint32_t slot); void put(float4* dst, const Entry&)   one particle entry (E float4)
+//   static constexpr bool CULL;  true: keep(entry) decides per particle of an opened leaf whether it enters the
+//                                list at all (the counters still count the paper's list: every particle)
 //   static constexpr bool SUBMIT_LAST;  true: the last list of a unit of work is submitted even if empty
 //   float4* submit(float4* list, int n, bool last)   consume n entries (fused visitors: all targets x n
 //                                                  entries, same buffer back; the warp-specialised walker:
@@ -311,16 +313,32 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
             const int ja = j0 + lane, jb = j0 + 32 + lane;
             const uint32_t sa = locate(ja < total ? ja : total - 1), sb = locate(jb < total ? jb : total - 1);
             typename V::Entry ea = v.get(sa), eb = v.get(sb);
-            if (ja < total) v.put(list + V::E * (nlist + lane), ea);
-            if (jb < total) v.put(list + V::E * (nlist + 32 + lane), eb);
-            nlist += (total - j0) < 64 ? (total - j0) : 64;
+            if (V::CULL) {   // entries that cannot interact with any member of the group stay out of the list
+              const bool ka = ja < total && v.keep(ea), kb = jb < total && v.keep(eb);
+              const unsigned ma = __ballot_sync(0xFFFFFFFFu, ka), mb = __ballot_sync(0xFFFFFFFFu, kb);
+              const int na = __popc(ma);
+              if (ka) v.put(list + V::E * (nlist + __popc(ma & lanemask_lt_())), ea);
+              if (kb) v.put(list + V::E * (nlist + na + __popc(mb & lanemask_lt_())), eb);
+              nlist += na + __popc(mb);
+            } else {
+              if (ja < total) v.put(list + V::E * (nlist + lane), ea);
+              if (jb < total) v.put(list + V::E * (nlist + 32 + lane), eb);
+              nlist += (total - j0) < 64 ? (total - j0) : 64;
+            }
           }
           if (nb == 1) {
             const int ja = j0 + lane;
             const uint32_t sa = locate(ja < total ? ja : total - 1);
             typename V::Entry ea = v.get(sa);
-            if (ja < total) v.put(list + V::E * (nlist + lane), ea);
-            nlist += (total - j0) < 32 ? (total - j0) : 32;
+            if (V::CULL) {
+              const bool ka = ja < total && v.keep(ea);
+              const unsigned ma = __ballot_sync(0xFFFFFFFFu, ka);
+              if (ka) v.put(list + V::E * (nlist + __popc(ma & lanemask_lt_())), ea);
+              nlist += __popc(ma);
+            } else {
+              if (ja < total) v.put(list + V::E * (nlist + lane), ea);
+              nlist += (total - j0) < 32 ? (total - j0) : 32;
+            }
             j0 += 32;
           }
         }
