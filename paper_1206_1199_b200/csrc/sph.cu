@@ -110,23 +110,36 @@ struct SphParams {
 
 // MODE 0: density (R16).  MODE 1: pressure force (R17).  MODE 2: pressure force + du/dt.
 // MODE 3: density + div v + rot v (SPH stage 1 of PAPER L252; R22).  MODE 4: MODE 2 + artificial viscosity (R24).
+#ifndef OTOO_SPH_NZ
+#define OTOO_SPH_NZ 1
+#endif
+#ifndef OTOO_SPH_PAIRS
+#define OTOO_SPH_PAIRS 1    // pass-1 targets as 64-bit register pairs (2: in every mode)
+#endif
 #ifndef OTOO_SPH_CULL
 #define OTOO_SPH_CULL 1    // walk-time cull of particles out of reach of the group's box (keep())
 #endif
+// volatile: the pair is built once per group, not rematerialised from its halves inside the pass-1 loop
+__device__ __forceinline__ f32x2 pk2v(float a, float b) { f32x2 r; asm volatile("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
 template <int T_, int MODE>
 struct SphVisitor {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : (MODE == 4 ? 4 : 3));
   static constexpr int LCAP = OTOO_LIST_CAP;
+  // measured at C4, G = 64: density 3.02 -> 2.83 ms, force + du/dt 4.33 -> 4.21 ms, plain force 3.78 -> 3.84 ms (kept scalar)
+  static constexpr bool PAIRS = OTOO_SPH_PAIRS == 2 || (OTOO_SPH_PAIRS == 1 && MODE != 1);
   static constexpr bool GATHER = MODE == 0 || MODE == 3;     // neighbours by the target's own h only (R16)
   const SphParams& p;
   float px[T], py[T], pz[T], ph[T], ppr[T], vx[T], vy[T], vz[T];
   float prho[MODE == 4 ? T : 1], pc[MODE == 4 ? T : 1], pal[MODE == 4 ? T : 1], pf[MODE == 4 ? T : 1];   // viscosity inputs of the targets
   float h2[T], hinv[T], o0[T], o1[T], o2[T], o3[T], o4[T];
+  f32x2 PX[(T + 1) / 2], PY[(T + 1) / 2], PZ[(T + 1) / 2], H2[(T + 1) / 2];   // pass 1: two targets per aligned register pair
   uint32_t cnt_ngb[T];
   float glo[3], ghi[3], hmax;
   __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_) {}
 
-  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4*) {
+  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4* scratch) {
     hmax = 0.0f;
 #pragma unroll
     for (int t = 0; t < T; t++) {
@@ -160,6 +173,22 @@ struct SphVisitor {
       h2[t] = __fmul_rn(ph[t], ph[t]); hinv[t] = 1.0f / ph[t];
       o0[t] = o1[t] = o2[t] = o3[t] = o4[t] = 0.0f; cnt_ngb[t] = 0;
     }
+    // Pairs for pass 1.  Built from their halves, ptxas keeps the halves and re-pairs them with two MOVs per
+    // operand inside the loop (6 of 16 instructions per entry); read back from shared memory as 64-bit words
+    // they are register pairs from the start (the empty list buffer is the scratch: 4 float2 x T/2 per lane).
+#pragma unroll
+    for (int q = 0; q < (PAIRS ? T / 2 : 0); q++) {
+      if (scratch) {
+        volatile unsigned long long* sc = reinterpret_cast<volatile unsigned long long*>(scratch) + (q * 4) * 32 + lane;
+        sc[0] = pk2(px[2 * q], px[2 * q + 1]); sc[32] = pk2(py[2 * q], py[2 * q + 1]);
+        sc[64] = pk2(pz[2 * q], pz[2 * q + 1]); sc[96] = pk2(h2[2 * q], h2[2 * q + 1]);
+        PX[q] = sc[0]; PY[q] = sc[32]; PZ[q] = sc[64]; H2[q] = sc[96];
+      } else {
+        PX[q] = pk2v(px[2 * q], px[2 * q + 1]); PY[q] = pk2v(py[2 * q], py[2 * q + 1]); PZ[q] = pk2v(pz[2 * q], pz[2 * q + 1]);
+        H2[q] = pk2v(h2[2 * q], h2[2 * q + 1]);
+      }
+    }
+    if (scratch) __syncwarp();
   }
   // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105)
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
@@ -219,6 +248,9 @@ struct SphVisitor {
   int lane_;
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
     int w = 0;
+    uint32_t nz[T];
+#pragma unroll
+    for (int t = 0; t < T; t++) nz[t] = 0u;
     for (int jb = 0; jb < n; jb += 32, w++) {
       uint32_t mk[T];
 #pragma unroll
@@ -233,14 +265,14 @@ struct SphVisitor {
         // two targets per packed instruction (FADD2 / FMUL2 / FFMA2 round each half like the scalar forms)
 #pragma unroll
         for (int q = 0; q < T / 2; q++) {
-          const float2 ex = __fadd2_rn(make_float2(a.x, a.x), make_float2(-px[2 * q], -px[2 * q + 1]));
-          const float2 ey = __fadd2_rn(make_float2(a.y, a.y), make_float2(-py[2 * q], -py[2 * q + 1]));
-          const float2 ez = __fadd2_rn(make_float2(a.z, a.z), make_float2(-pz[2 * q], -pz[2 * q + 1]));
+          const float2 ex = __fadd2_rn(make_float2(a.x, a.x), PAIRS ? neg2(as2(PX[q])) : make_float2(-px[2 * q], -px[2 * q + 1]));
+          const float2 ey = __fadd2_rn(make_float2(a.y, a.y), PAIRS ? neg2(as2(PY[q])) : make_float2(-py[2 * q], -py[2 * q + 1]));
+          const float2 ez = __fadd2_rn(make_float2(a.z, a.z), PAIRS ? neg2(as2(PZ[q])) : make_float2(-pz[2 * q], -pz[2 * q + 1]));
           const float2 r2 = __ffma2_rn(ez, ez, __ffma2_rn(ey, ey, __fmul2_rn(ex, ex)));
           // r2 < lim  <=>  the sign bit of fl32(r2 - lim) (exact: the difference of two floats is negative iff
           // the first is smaller); one funnel shift appends it to the mask word
-          const float l0 = GATHER ? h2[2 * q] : fmaxf(h2[2 * q], hj2), l1 = GATHER ? h2[2 * q + 1] : fmaxf(h2[2 * q + 1], hj2);
-          const float2 d = __fadd2_rn(r2, make_float2(-l0, -l1));
+          const float2 hq = PAIRS ? as2(H2[q]) : make_float2(h2[2 * q], h2[2 * q + 1]);
+          const float2 d = __fadd2_rn(r2, GATHER ? neg2(hq) : make_float2(-fmaxf(hq.x, hj2), -fmaxf(hq.y, hj2)));
           mk[2 * q] = __funnelshift_l(__float_as_uint(d.x), mk[2 * q], 1);
           mk[2 * q + 1] = __funnelshift_l(__float_as_uint(d.y), mk[2 * q + 1], 1);
         }
@@ -257,16 +289,26 @@ struct SphVisitor {
         mk[t] <<= 32 - nb;                       // candidate k of the word sits at bit 31 - k
         if (GATHER) cnt_ngb[t] += (uint32_t)__popc(mk[t]);
         msk[(w * T + t) * 32 + lane_] = mk[t];
+        nz[t] |= (mk[t] != 0u ? 1u : 0u) << w;   // most words are empty: pass 2 visits the others only
       }
     }
-    const int nw = w;
 #pragma unroll
     for (int t = 0; t < T; t++) {
       int ww = 0;
+#if OTOO_SPH_NZ
+      uint32_t m = 0u, z = nz[t];
+      for (;;) {
+        if (m == 0u) {
+          if (z == 0u) break;
+          ww = __ffs(z) - 1; z &= z - 1u;
+          m = msk[(ww * T + t) * 32 + lane_];
+        }
+#else
       uint32_t m = msk[t * 32 + lane_];
       for (;;) {
-        while (m == 0u && ++ww < nw) m = msk[(ww * T + t) * 32 + lane_];
+        while (m == 0u && ++ww < w) m = msk[(ww * T + t) * 32 + lane_];
         if (m == 0u) break;
+#endif
         const int k = __clz(m);
         m &= ~(0x80000000u >> k);
         hit(list, (ww << 5) + k, t);
