@@ -143,9 +143,47 @@ __device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leadin
 }
 // H5a: number of cells that start at each sorted slot, and the per-level cell counts.
 //   info[s] = (cpl+1) | LL << 8
+// A level-l range starting at s is a cell iff some window of n_crit+1 slots containing s shares l-1 levels:
+// c[t] = cplev(key[t], key[t + n_crit]) is computed once per t into shared memory (every thread of the
+// plain form recomputed its n_crit+1 windows from global memory: 480 GB/s at 32 M particles), the per-level
+// counts are warp-aggregated (one ballot per level instead of contended shared-memory atomics).
+#define OTOO_SLOT_NCRIT_MAX 256
 __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
                                                          uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
                                                          uint32_t* __restrict__ level_count) {
+  __shared__ uint32_t lc[OTOO_NLEV];
+  __shared__ signed char cw[256 + OTOO_SLOT_NCRIT_MAX];
+  const int64_t s0 = (int64_t)blockIdx.x * 256;
+  if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
+  for (int i = threadIdx.x; i < 256 + n_crit; i += 256) {
+    const int64_t t = s0 - n_crit + i;
+    cw[i] = (t >= 0 && t <= n - n_crit - 1) ? (signed char)cplev(key[t], key[t + n_crit]) : (signed char)-1;
+  }
+  __syncthreads();
+  const int64_t s = s0 + threadIdx.x;
+  int lo = 1, LL = 0;   // empty level range for threads past the end
+  if (s < n) {
+    const int cpl = (s == 0) ? -1 : cplev(key[s - 1], key[s]);
+    int D = -1;
+    for (int i = 0; i <= n_crit; i++) { const int c = cw[threadIdx.x + i]; D = c > D ? c : D; }
+    LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
+    lo = cpl + 1;
+    int nc = LL - cpl; if (nc < 0) nc = 0;
+    slot_nc[s] = (uint32_t)nc;
+    info[s] = (uint32_t)lo | ((uint32_t)LL << 8);
+  }
+#pragma unroll
+  for (int l = 0; l < OTOO_NLEV; l++) {
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
+    if (b && (threadIdx.x & 31) == 0) atomicAdd(&lc[l], (uint32_t)__popc(b));
+  }
+  __syncthreads();
+  if (threadIdx.x < OTOO_NLEV && lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+}
+// the same for n_crit > OTOO_SLOT_NCRIT_MAX (every thread scans its own windows)
+__global__ void __launch_bounds__(256) slot_cells_wide_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
+                                                              uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
+                                                              uint32_t* __restrict__ level_count) {
   __shared__ uint32_t lc[OTOO_NLEV];
   if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
   __syncthreads();
@@ -398,7 +436,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
   // H5a
   uint32_t* info = ctx->val[1];
-  slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
+  if (n_crit <= OTOO_SLOT_NCRIT_MAX) slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
+  else slot_cells_wide_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
   ctx->launches += 2;
   OTOO_TRY(otoo_exclusive_scan_u32(ctx, ctx->slot_nc, N, ctx->d_counters + 40, st));
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, 64 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));

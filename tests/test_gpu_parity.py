@@ -65,7 +65,8 @@ def check_tree(otoo, orc, pm, n_crit, key_order=0):
 
 @pytest.mark.parametrize("kind,n,n_crit,seed", [("plummer", 16384, 16, 1206), ("plummer", 5000, 1, 1199),
                                                 ("uniform_cube", 3001, 8, 2012), ("hernquist", 40000, 16, 3),
-                                                ("plummer", 1, 16, 1), ("plummer", 7, 16, 2), ("uniform_sphere", 4097, 2, 5)])
+                                                ("plummer", 1, 16, 1), ("plummer", 7, 16, 2), ("uniform_sphere", 4097, 2, 5),
+                                                ("plummer", 9000, 256, 6), ("plummer", 9000, 300, 7), ("plummer", 200, 256, 8)])
 def test_tree_parity(otoo, orc, kind, n, n_crit, seed):
     check_tree(otoo, orc, gen.make(kind, n, seed), n_crit)
 
