@@ -138,3 +138,54 @@ def test_fullsize_sph(orc):
         assert np.all(np.abs(out[idx, 3] - rf["acc_dudt"][idx, 3]) <= tol)
     finally:
         o.close()
+
+
+def test_fullsize_sph_stage1_and_viscosity(orc):
+    """BASELINE config 4 at full size, Hilbert order: SPH stage 1 (density, div v, rot v; R22) and stage 2 with
+    artificial viscosity (R24) against the oracle on a seeded sample of groups; counters of every group."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    cfg = gen.CONFIGS["C4"]
+    n, G = cfg["n"], cfg["group_sph"]
+    w = gen.wd_pair(n, 1199)
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    vel = np.zeros((n, 4), np.float32)
+    vel[:, :3] = -0.4 * pm[:, :3] + 0.1 * np.sin(7 * pm[:, [1, 2, 0]])
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        o.otoo_set_option("key_order", 1)
+        o.otoo_build_tree(dev(pm), cfg["n_crit"])
+        t = orc.Tree(pm, cfg["n_crit"], key_order=1)
+        perm = check_tree_full(o, t).astype(np.int64)
+        d_h, d_vel = dev(h), dev(vel)
+        rho, nngb, dr = o.otoo_sph_stage1(d_h, d_vel, G)
+        ref = t.sph_density(h, G, sums=False)
+        nt, _, npart = o.otoo_export_group_stats()
+        assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(npart, ref["n_parts"])
+        ng = t.n_groups(G)
+        sel = sample_groups(ng, npart.astype(np.int64), 2012, max_list=1 << 30)
+        idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
+        rs = t.sph_divrot(h, vel, G, groups=sel)
+        rg = rho.cpu().numpy()
+        assert (np.abs(rg[idx] - rs["rho"][idx]) / rs["rho"][idx]).max() <= TOL
+        got = dr.cpu().numpy().astype(np.float64)[idx]
+        want, tol = rs["divrot"][idx], 8 * U32 * rs["abs_sum"][idx]
+        assert np.all(np.abs(got[:, 0] - want[:, 0]) <= np.maximum(TOL * np.abs(want[:, 0]), tol))
+        d = np.linalg.norm(got[:, 1:] - want[:, 1:], axis=1)
+        assert np.all(d <= np.maximum(TOL * np.linalg.norm(want[:, 1:], axis=1), tol))
+        # stage 2 with viscosity, the oracle fed the GPU's own fp32 rho and P
+        P = o.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
+        Pg = P.cpu().numpy()
+        visc = np.zeros((n, 4), np.float32)
+        visc[:, 0] = np.sqrt((5.0 / 3.0) * Pg / rg)
+        visc[:, 1] = 0.5 + 0.5 * gen.uniform01(3, np.arange(n, dtype=np.uint64), 0)
+        visc[:, 2] = gen.uniform01(4, np.arange(n, dtype=np.uint64), 0)
+        out = o.otoo_sph_force_visc(d_h, rho, P, d_vel, dev(visc), G).cpu().numpy()
+        rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel, visc=visc, groups=sel)
+        vec_check(out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
+        tol = np.maximum(TOL * np.abs(rf["acc_dudt"][idx, 3]), 8 * U32 * rf["abs_sum"][idx, 1])
+        assert np.all(np.abs(out[idx, 3] - rf["acc_dudt"][idx, 3]) <= tol)
+        assert np.isfinite(out).all()
+    finally:
+        o.close()
