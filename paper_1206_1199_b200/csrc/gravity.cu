@@ -135,8 +135,6 @@ struct GravVisitor {
   }
   // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
   // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
-  // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
-  // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
   __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
     const float2 e2 = bc2(p.eps2);
 #pragma unroll
