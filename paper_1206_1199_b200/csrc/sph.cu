@@ -514,6 +514,9 @@ struct SphWalker {
   }
 };
 
+#ifndef OTOO_SPH_WS_WREG
+#define OTOO_SPH_WS_WREG 72     // registers of a walker thread (T <= 4; at 48 the SPH walker spilled 190-300 B); the evaluators get 160 - this
+#endif
 template <int T, int MODE>
 __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, T >= 8 ? 2 : 3) walk_sph_ws_kernel(const SphParams p) {
   typedef typename SphWalker<T, MODE>::Pair Pair;
@@ -530,14 +533,14 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, T >= 8 ? 2 : 3) walk_sph_w
   }
   __syncthreads();
   if (warp >= OTOO_WS_PAIRS) {
-    if (T >= 8) setmaxnreg_dec<80>(); else setmaxnreg_dec<48>();
+    if (T >= 8) setmaxnreg_dec<80>(); else setmaxnreg_dec<OTOO_SPH_WS_WREG>();
     Pair& sm = pairs[warp - OTOO_WS_PAIRS];
     SphWalker<T, MODE> w(p, sm, lane);
     float4* list = w.acquire();
     walk_driver(p.c, w, list, sm.stk, lane, (int64_t)blockIdx.x * OTOO_WS_PAIRS + (warp - OTOO_WS_PAIRS));
     w.finish();
   } else {
-    if (T >= 8) setmaxnreg_inc<176>(); else setmaxnreg_inc<112>();
+    if (T >= 8) setmaxnreg_inc<176>(); else setmaxnreg_inc<160 - OTOO_SPH_WS_WREG>();
     Pair& sm = pairs[warp];
     Eval v(p);
     v.msk = masks + warp * (Eval::W * T * 32);
