@@ -189,3 +189,36 @@ def test_fullsize_sph_stage1_and_viscosity(orc):
         assert np.isfinite(out).all()
     finally:
         o.close()
+
+
+def test_config2_accuracy_vs_theta(orc):
+    """BASELINE config 2: accuracy of the tree force against the O(N^2) direct sum (the oracle's fp64 definition) on a
+    seeded 4096-particle subsample of the 1 M Plummer sphere, theta in {0.4, 0.6, 0.8}.  The error of the method
+    (not of the arithmetic): it must fall with theta and stay at the level of a monopole tree code."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    cfg = gen.CONFIGS["C2"]
+    n, G = cfg["n"], cfg["group"]
+    pm = gen.make(cfg["kind"], n, 1206)
+    eps = float(np.float32(cfg["eps"]))
+    tg = np.sort(np.random.default_rng(4096).choice(n, size=4096, replace=False)).astype(np.int64)
+    ref = orc.direct_sum(pm, eps, tg)
+    an = np.linalg.norm(ref[:, :3], axis=1)
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        o.otoo_build_tree(dev(pm), cfg["n_crit"])
+        med, p99, inter = [], [], []
+        for theta in (0.4, 0.6, 0.8):
+            out = o.otoo_gravity(eps, float(np.float32(theta)), G).cpu().numpy().astype(np.float64)[tg]
+            e = np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / an
+            med.append(float(np.median(e))); p99.append(float(np.percentile(e, 99)))
+            inter.append(o.otoo_last_stats()["sum_interactions"])
+            pe = np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])
+            assert np.median(pe) < 1e-3
+        print("theta 0.4/0.6/0.8: median", med, "p99", p99, "interactions", inter)
+        assert med[0] < med[1] < med[2] and p99[0] < p99[1] < p99[2]
+        assert inter[0] > inter[1] > inter[2]
+        assert med[2] < 1e-2 and p99[2] < 5e-2 and med[0] < 2e-3
+    finally:
+        o.close()
