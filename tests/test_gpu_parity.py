@@ -441,3 +441,25 @@ def test_host_entry_point(otoo, orc):
     ref = orc.Tree(pm, 16).gravity(float(np.float32(0.01)), 0.5, 64)
     e, _ = acc_err(out, ref["acc_pot"], ref["abs_sum"])
     assert e.max() <= TOL
+
+
+def test_config1_against_direct_sum(otoo, orc):
+    """BASELINE config 1 (Plummer N = 16384, eps = 0.01, theta = 0.5, G = 64) against the O(N^2) direct sum: with
+    theta = 0 the lists hold every particle and the CUDA sums are the direct sum to fp32 accuracy; with theta = 0.5
+    the difference is the error of the monopole approximation."""
+    cfg = gen.CONFIGS["C1"]
+    n, G = cfg["n"], cfg["group"]
+    pm = gen.make(cfg["kind"], n, 1206)
+    eps = float(np.float32(cfg["eps"]))
+    ref = orc.direct_sum(pm, eps)
+    an = np.linalg.norm(ref[:, :3], axis=1)
+    otoo.otoo_build_tree(dev(pm), cfg["n_crit"])
+    out0 = otoo.otoo_gravity(eps, 0.0, G).cpu().numpy().astype(np.float64)
+    assert otoo.otoo_last_stats()["sum_interactions"] == n * n
+    e0 = np.linalg.norm(out0[:, :3] - ref[:, :3], axis=1) / an
+    assert np.percentile(e0, 99.9) <= TOL and e0.max() <= 1e-4
+    assert (np.abs(out0[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])).max() <= TOL
+    out = otoo.otoo_gravity(eps, float(np.float32(cfg["theta"])), G).cpu().numpy().astype(np.float64)
+    e = np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / an
+    assert 1e-6 < np.median(e) < 1e-3 and np.percentile(e, 99) < 1e-2
+    assert np.median(np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])) < 1e-3
