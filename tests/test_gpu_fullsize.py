@@ -222,3 +222,32 @@ def test_config2_accuracy_vs_theta(orc):
         assert med[2] < 1e-2 and p99[2] < 5e-2 and med[0] < 2e-3
     finally:
         o.close()
+
+
+def test_fullsize_adaptive_h(orc):
+    """BASELINE config 4: "smoothing length adaptive to ~50 neighbours" at full size.  Starting 30 % off the generator's
+    h, otoo_sph_adapt_h (R21) must bring (almost) every particle into 50 +- 3, and its counts must be the counts of a
+    fresh density pass with the final h.  (Bit-for-bit parity of the iteration with the oracle: small sizes in
+    test_gpu_parity.py.)"""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    cfg = gen.CONFIGS["C4"]
+    n, G = cfg["n"], cfg["group_sph"]
+    w = gen.wd_pair(n, 1206)
+    pm = w["pos_mass"]
+    h0 = (w["h"] * np.where(np.arange(n) % 2 == 0, 1.3, 0.7)).astype(np.float32)
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        o.otoo_build_tree(dev(pm), cfg["n_crit"])
+        d_h = dev(h0)
+        nn, it = o.otoo_sph_adapt_h(d_h, 50.0, 3.0, 40, G)
+        nn = nn.cpu().numpy()
+        assert 1 <= it <= 40
+        assert np.mean(np.abs(nn.astype(np.int64) - 50) <= 3) >= 0.995
+        _, nn2 = o.otoo_sph_density(d_h, G)
+        assert np.array_equal(nn, nn2.cpu().numpy())
+        hf = d_h.cpu().numpy()
+        assert np.isfinite(hf).all() and (hf > 0).all()
+    finally:
+        o.close()
