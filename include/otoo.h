@@ -99,7 +99,10 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
 
 /* PAPER II-C (Eq. 4, Eq. 5) SPH stage 1: density by direct summation during the walk (L99-L105;
  * R13-R16).  d_h: N floats, kernel SUPPORT radius (W = 0 for r >= h, L89), original order.
- * d_rho: N floats out.  d_nngb: N uint32 out (neighbours with r < h_i, self included) or NULL. */
+ * d_rho: N floats out.  d_nngb: N uint32 out (neighbours with r < h_i, self included) or NULL.
+ * Group counters and sum_interactions count the walk's candidate list (every particle of every opened leaf,
+ * L105); candidates farther from the group's box than any member's reach are not evaluated, which changes
+ * no neighbour decision ("walk-time cull"). */
 otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho,
                              uint32_t* d_nngb, void* stream);
 
