@@ -14,9 +14,9 @@ pytestmark = pytest.mark.gpu
 
 from workloads import generators as gen  # noqa: E402
 
-TOL = 1e-5
-U32 = 2.0 ** -24
-N_SAMPLE = 48
+from tests.parity_rule import TOL, U32, report   # noqa: E402  (the one statement of the rule, R12)
+
+N_SAMPLE = {"C2": 512, "C3": 256, "C4": 256, "C5": 256}     # seeded groups summed in fp64 per config (+ the two below)
 
 
 def dev(a):
@@ -34,22 +34,19 @@ def check_tree_full(o, t):
     return eo["perm"]
 
 
-def sample_groups(ng, lengths, seed, max_list):
-    """seeded sample of groups + the group with the longest list the oracle can sum in seconds"""
+def sample_groups(ng, lengths, seed, n_sample):
+    """seeded sample of groups + the group with the LONGEST list (in C3 it lists all 8.4 M particles and goes through
+    the task pool: many tasks, atomicAdd merges from many warps; the oracle sums its 128 targets in parallel) + the
+    ragged last group"""
     rng = np.random.default_rng(seed)
-    sel = set(rng.choice(ng, size=min(N_SAMPLE, ng), replace=False).tolist())
-    ok = np.where(lengths <= max_list)[0]
-    sel.add(int(ok[np.argmax(lengths[ok])]))
-    sel.add(ng - 1)                                   # the ragged last group
+    sel = set(rng.choice(ng, size=min(n_sample, ng), replace=False).tolist())
+    sel.add(int(np.argmax(lengths)))
+    sel.add(ng - 1)
     return np.array(sorted(sel), dtype=np.int64)
 
 
-def vec_check(got, want, abs_sum, pct):
-    d = np.linalg.norm(got[:, :3].astype(np.float64) - want[:, :3], axis=1)
-    an = np.linalg.norm(want[:, :3], axis=1)
-    tol = np.maximum(TOL * an, 8 * U32 * abs_sum)
-    assert np.all(d <= tol), float((d / np.maximum(tol, 1e-300)).max())
-    assert np.percentile(d / np.maximum(an, 1e-300), pct) <= TOL
+def vec_check(label, got, want, abs_sum, pct, floor_frac_max=1.0):
+    return report(label, got[:, :3], want[:, :3], abs_sum, pct=pct, floor_frac_max=floor_frac_max)
 
 
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5", "C2:hilbert", "C3:hilbert", "C2:exact", "C3:hilbert+exact"])
@@ -84,11 +81,11 @@ def test_fullsize_gravity(orc, name):
         # fp64 sums for a sample of groups
         ng = t.n_groups(G)
         lengths = nc.astype(np.int64) + npart
-        sel = sample_groups(ng, lengths, 1206, max_list=4_000_000)
+        sel = sample_groups(ng, lengths, 1206, N_SAMPLE[name])
         rs = t.gravity(eps, theta, G, groups=sel)
         assert np.array_equal(rs["n_tests"], nt[sel])
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
-        vec_check(out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9)
+        vec_check(f"fullsize_gravity[{name}:{order}]", out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9)
         pe = np.abs(out[idx, 3] - rs["acc_pot"][idx, 3]) / np.abs(rs["acc_pot"][idx, 3])
         assert pe.max() <= TOL, pe.max()
         assert np.isfinite(out).all()
@@ -120,7 +117,7 @@ def test_fullsize_sph(orc):
         assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(npart, ref["n_parts"])
         assert o.otoo_last_stats()["sum_interactions"] == ref["candidates"]
         ng = t.n_groups(G)
-        sel = sample_groups(ng, npart.astype(np.int64), 1199, max_list=1 << 30)
+        sel = sample_groups(ng, npart.astype(np.int64), 1199, N_SAMPLE["C4"])
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
         rs = t.sph_density(h, G, groups=sel)
         rg = rho.cpu().numpy()
@@ -133,9 +130,8 @@ def test_fullsize_sph(orc):
         vel2[:, :3] += (-0.3 * pm[:, :3]).astype(np.float32)          # a contraction: du/dt is not rounding noise
         out = o.otoo_sph_force(d_h, rho, P, G, vel=dev(vel2)).cpu().numpy()
         rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel2, groups=sel)
-        vec_check(out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
-        tol = np.maximum(TOL * np.abs(rf["acc_dudt"][idx, 3]), 8 * U32 * rf["abs_sum"][idx, 1])
-        assert np.all(np.abs(out[idx, 3] - rf["acc_dudt"][idx, 3]) <= tol)
+        vec_check("fullsize_sph:a_sph", out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
+        report("fullsize_sph:dudt", out[idx, 3], rf["acc_dudt"][idx, 3], rf["abs_sum"][idx, 1], pct=None)
     finally:
         o.close()
 
@@ -164,16 +160,15 @@ def test_fullsize_sph_stage1_and_viscosity(orc):
         nt, _, npart = o.otoo_export_group_stats()
         assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(npart, ref["n_parts"])
         ng = t.n_groups(G)
-        sel = sample_groups(ng, npart.astype(np.int64), 2012, max_list=1 << 30)
+        sel = sample_groups(ng, npart.astype(np.int64), 2012, N_SAMPLE["C4"])
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
         rs = t.sph_divrot(h, vel, G, groups=sel)
         rg = rho.cpu().numpy()
         assert (np.abs(rg[idx] - rs["rho"][idx]) / rs["rho"][idx]).max() <= TOL
         got = dr.cpu().numpy().astype(np.float64)[idx]
-        want, tol = rs["divrot"][idx], 8 * U32 * rs["abs_sum"][idx]
-        assert np.all(np.abs(got[:, 0] - want[:, 0]) <= np.maximum(TOL * np.abs(want[:, 0]), tol))
-        d = np.linalg.norm(got[:, 1:] - want[:, 1:], axis=1)
-        assert np.all(d <= np.maximum(TOL * np.linalg.norm(want[:, 1:], axis=1), tol))
+        want = rs["divrot"][idx]
+        report("fullsize_stage1:div_v", got[:, 0], want[:, 0], rs["abs_sum"][idx], pct=None)
+        report("fullsize_stage1:rot_v", got[:, 1:], want[:, 1:], rs["abs_sum"][idx], pct=None)
         # stage 2 with viscosity, the oracle fed the GPU's own fp32 rho and P
         P = o.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
         Pg = P.cpu().numpy()
@@ -183,9 +178,8 @@ def test_fullsize_sph_stage1_and_viscosity(orc):
         visc[:, 2] = gen.uniform01(4, np.arange(n, dtype=np.uint64), 0)
         out = o.otoo_sph_force_visc(d_h, rho, P, d_vel, dev(visc), G).cpu().numpy()
         rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel, visc=visc, groups=sel)
-        vec_check(out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
-        tol = np.maximum(TOL * np.abs(rf["acc_dudt"][idx, 3]), 8 * U32 * rf["abs_sum"][idx, 1])
-        assert np.all(np.abs(out[idx, 3] - rf["acc_dudt"][idx, 3]) <= tol)
+        vec_check("fullsize_sph_visc:a_sph", out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
+        report("fullsize_sph_visc:dudt", out[idx, 3], rf["acc_dudt"][idx, 3], rf["abs_sum"][idx, 1], pct=None)
         assert np.isfinite(out).all()
     finally:
         o.close()

@@ -141,13 +141,26 @@ def test_mass_com_and_two_particle_cell(orc):
     assert e2["s"][0] == pytest.approx(np.sqrt(0.5), rel=1e-15)
 
 
-def test_rb2_formula(orc):
-    pm = gen.plummer(1000, 9)
-    t = orc.Tree(pm, 8)
+def test_rb2_hand_built_tree(orc):
+    """R7 on a tree small enough to do by hand (l, s as defined at PAPER.md L63; none of the numbers below comes
+    from the oracle).  Three unit masses A = (0,0,0), B = (1,1,1), C = (1/8,1/8,1/8), n_crit = 1: root cube [0,1]^3.
+      root      l = 1,   centre (1/2,..),  CM = (3/8,..):   s = sqrt(3)/8,    r_b = 1/theta + s
+      octant 0  l = 1/2, centre (1/4,..),  CM = (1/16,..):  s = 3 sqrt(3)/16  (holds A and C)
+      octant 7  l = 1/2, centre (3/4,..),  CM = (1,1,1):    s = sqrt(3)/4     (holds B)
+    theta = 1/2:  r_b^2 = (2 + 0.21650635)^2 = 4.9129004, (1 + 0.32475953)^2 = 1.7549878, (1 + 0.43301270)^2 = 2.0535254;
+    the plain form r_b = l/theta (mac_kind 1) gives 4, 1, 1."""
+    pm = np.array([[0, 0, 0, 1.0], [1, 1, 1, 1.0], [0.125, 0.125, 0.125, 1.0]], np.float32)
+    t = orc.Tree(pm, 1)
     ex = t.export()
-    theta = 0.6
-    l = t.S / 2.0 ** ex["cells"]["level"].astype(np.float64)
-    want = ((l / theta + ex["s"]) ** 2).astype(np.float32)
-    assert np.array_equal(t.rb2(theta), want)
-    assert np.array_equal(t.rb2(theta, 1), ((l / theta) ** 2).astype(np.float32))
-    assert np.all(np.isinf(t.rb2(0.0)))
+    c = ex["cells"]
+    assert t.S == 1.0 and (c["level"][:3] == [0, 1, 1]).all() and (c["prefix"][:3] == [0, 0, 7]).all()
+    assert (c["count"][:3] == [3, 2, 1]).all()
+    assert ex["s"][:3] == pytest.approx([0.21650635, 0.32475953, 0.43301270], rel=2e-8)
+    assert t.rb2(0.5)[:3] == pytest.approx([4.9129004, 1.7549878, 2.0535254], rel=2e-7)
+    assert t.rb2(0.5, 1)[:3].tolist() == [4.0, 1.0, 1.0]
+    assert t.rb2(1.0)[:3] == pytest.approx([1.4798877, 0.6802283, 0.8705127], rel=2e-7)   # (l + s)^2: 1 + 2s + s^2 with s^2 = 3/64, 27/256, 3/16
+    assert np.all(np.isinf(t.rb2(0.0)))                                                    # theta = 0 opens everything
+    # the deeper cells are the single-child chain down to the level where A and C separate (R5: chains are kept)
+    assert t.depth == 3 and t.ncell == 6
+
+
