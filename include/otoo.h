@@ -61,6 +61,18 @@ typedef struct {
   uint64_t sum_steps;        /* walk steps (batches of <= 32 MAC tests) of the last walk */
   uint64_t sum_tasks;        /* units of work run: groups + task-pool tasks */
   uint64_t sum_flushes;      /* evaluations of a (full or final) shared-memory list */
+  /* Per-phase DEVICE times in ms (CUDA events on the call's stream; PAPER.md L195, L212 splits a step into TREE
+   * and KERNEL the same way).  ms_build[] of the last otoo_build_tree: [0] root cube (H1), [1] keys (H2),
+   * [2] key sort (H3), [3] gather (H4), [4] cells from the sorted keys (H5, includes the one host
+   * synchronisation), [5] bottom-up moments (H6), [6..7] unused (0); ms_build_total = their sum.
+   * Of the last walk call (gravity or SPH): ms_walk_prep = cell radii (r_b or Eq. 5), gathers and clears before
+   * the walk kernel; ms_walk_force = the fused walk + sum kernel alone (H7-H10 / H11 / H13); ms_total = the
+   * whole call.  0 where nothing has run. */
+  float ms_build[8], ms_build_total;
+  float ms_walk_prep, ms_walk_force, ms_total;
+  int32_t walk_only;         /* 1: the last walk ran with option "walk_only": counters valid, OUTPUTS MEANINGLESS */
+  int32_t error_flag;        /* != 0: the last walk dropped cells (private spill area full): outputs and counters
+                              * invalid; otoo_last_stats / otoo_export_group_stats return OTOO_ERR_CAPACITY */
 } otoo_stats_t;
 
 /* Lifecycle.  `device` is a CUDA ordinal; max_particles bounds N of every later build
@@ -68,7 +80,7 @@ typedef struct {
 otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles);
 void otoo_destroy(otoo_ctx* ctx);
 const char* otoo_last_error(const otoo_ctx* ctx);
-/* ABI version of this header (1). */
+/* ABI version of this header (2: otoo_stats_t carries per-phase times, walk_only and error_flag). */
 int otoo_version(void);
 
 /* PAPER III-B steps 1-4 + III-C, all on the device: root cube (L121,L127; R1), Morton keys
@@ -163,9 +175,19 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* host_out);
  * force kernel's roofline next to the nominal SMs x 128 x 2 x clock.  Synchronises. */
 otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* stream);
 
+/* Measurement aid: the microbenchmarks behind the ceilings DESIGN.md quotes for the force kernel (bench.py --probe).
+ * which = "ffma2": SM sub-partition cycles per FFMA2 warp instruction for the operand patterns of the sum loop;
+ * "sumloop": the product's own pair-sum loop on lists already in shared memory (no walk): interactions/s and
+ * cycles per (target pair, list entry).  Writes a JSON array as text into host_json (cap bytes; OTOO_ERR_CAPACITY
+ * if too small).  Uses the context's particle arrays as scratch: the tree is invalidated.  Synchronises. */
+otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_t cap, void* stream);
+
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).
+ * "walk_spill" = usable entries of that private area per warp (default and maximum 8192; test hook: with
+ * "task_pool" = 0 and a small value the area overflows, the walk drops cells and flags the launch --
+ * otoo_last_stats and otoo_export_group_stats then return OTOO_ERR_CAPACITY with error_flag = 1).
  * "key_order" = 0 (default): particles, groups and cells in Morton order (R3); 1: in Hilbert
  * order (the paper's own ordering; R20) -- same cells, other order: no group straddles an
  * octant boundary with a system-sized box, fewer interactions at the same theta.  Read by the next
@@ -193,6 +215,10 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value);
  * builds the tree, runs otoo_gravity, copies N x float4 back into h_acc_pot, synchronises. */
 otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit,
                               float eps, float theta, int group_size, float* h_acc_pot);
+/* The same for the paper's absolute-error MAC (otoo_build_tree + otoo_gravity_delta between the two copies). */
+otoo_status otoo_gravity_delta_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit,
+                                    float eps, float delta, float m_limit, int group_size,
+                                    float* h_acc_pot);
 
 #ifdef __cplusplus
 }

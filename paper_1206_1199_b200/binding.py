@@ -26,7 +26,7 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
+           "otoo_gravity_host", "otoo_gravity_delta_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_probe", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
 
 
 class TreeInfo(C.Structure):
@@ -38,7 +38,12 @@ class Stats(C.Structure):
     _fields_ = [("sum_tests", C.c_uint64), ("sum_interactions", C.c_uint64), ("sum_cells", C.c_uint64),
                 ("sum_parts", C.c_uint64), ("n_groups", C.c_int64), ("group_size", C.c_int32),
                 ("launches", C.c_int32), ("sum_steps", C.c_uint64), ("sum_tasks", C.c_uint64),
-                ("sum_flushes", C.c_uint64)]
+                ("sum_flushes", C.c_uint64), ("ms_build", C.c_float * 8), ("ms_build_total", C.c_float),
+                ("ms_walk_prep", C.c_float), ("ms_walk_force", C.c_float), ("ms_total", C.c_float),
+                ("walk_only", C.c_int32), ("error_flag", C.c_int32)]
+
+
+BUILD_PHASES = ["root_cube", "keys", "sort", "gather", "cells", "moments"]
 
 
 CELL_DTYPE = np.dtype([("prefix", "<u8"), ("first", "<u4"), ("count", "<u4"), ("child_first", "<u4"),
@@ -67,7 +72,9 @@ _lib.otoo_export_group_stats.argtypes = [_vp, _vp, _vp, _vp]
 _lib.otoo_last_stats.argtypes = [_vp, C.POINTER(Stats)]
 _lib.otoo_set_option.argtypes = [_vp, C.c_char_p, _i64]
 _lib.otoo_measure_fp32_peak.argtypes = [_vp, C.POINTER(C.c_double), _vp]
+_lib.otoo_probe.argtypes = [_vp, C.c_char_p, C.c_char_p, _i64, _vp]
 _lib.otoo_gravity_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _i32, _vp]
+_lib.otoo_gravity_delta_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _f, _i32, _vp]
 
 
 class OtooError(RuntimeError):
@@ -76,7 +83,9 @@ class OtooError(RuntimeError):
         self.status = status
 
 
-def _ptr(t, dtype=None, shape_last=None):
+def _ptr(t, dtype=None, shape_last=None, rows=None, device=None):
+    """data_ptr() of a contiguous CUDA tensor after the checks the C side cannot make: dtype, (N, k) shape, the row
+    count the kernels will read or write, and the device of the context."""
     if t is None:
         return None
     if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
@@ -85,13 +94,11 @@ def _ptr(t, dtype=None, shape_last=None):
         raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
     if shape_last is not None and (t.ndim != 2 or t.shape[1] != shape_last):
         raise TypeError(f"expected shape (N,{shape_last})")
+    if rows is not None and t.shape[0] != rows:
+        raise ValueError(f"expected {rows} rows, got {t.shape[0]}")
+    if device is not None and t.device.index != device:
+        raise ValueError(f"tensor on cuda:{t.device.index}, context on cuda:{device}")
     return t.data_ptr()
-
-
-def _stream(stream):
-    if stream is None:
-        return torch.cuda.current_stream().cuda_stream
-    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
 
 
 class Otoo:
@@ -123,40 +130,49 @@ class Otoo:
     def _dev(self):
         return torch.device("cuda", self.device)
 
+    def _stream(self, stream):
+        if stream is None:
+            return torch.cuda.current_stream(self.device).cuda_stream
+        return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+    def _p(self, t, dtype=None, shape_last=None):
+        """a per-particle argument: N rows on this context's device"""
+        return _ptr(t, dtype, shape_last, rows=self.N, device=self.device)
+
     # ---- the hot path
     def otoo_build_tree(self, pos_mass, n_crit=16, stream=None):
         n = 0 if pos_mass is None else pos_mass.shape[0]
-        self._check(_lib.otoo_build_tree(self._h, _ptr(pos_mass, torch.float32, 4) if n else None, n, int(n_crit),
-                                         _stream(stream)))
+        self._check(_lib.otoo_build_tree(self._h, _ptr(pos_mass, torch.float32, 4, device=self.device) if n else None, n, int(n_crit),
+                                         self._stream(stream)))
         self.N = n
 
     def otoo_gravity(self, eps, theta, group_size, out=None, stream=None):
         if out is None:
             out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
         self._check(_lib.otoo_gravity(self._h, float(eps), float(theta), int(group_size),
-                                      _ptr(out, torch.float32, 4), _stream(stream)))
+                                      self._p(out, torch.float32, 4), self._stream(stream)))
         return out
 
     def otoo_gravity_delta(self, eps, delta, m_limit, group_size, out=None, stream=None):
         if out is None:
             out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
         self._check(_lib.otoo_gravity_delta(self._h, float(eps), float(delta), float(m_limit), int(group_size),
-                                            _ptr(out, torch.float32, 4), _stream(stream)))
+                                            self._p(out, torch.float32, 4), self._stream(stream)))
         return out
 
     def otoo_sph_density(self, h, group_size, want_nngb=True, stream=None):
         rho = torch.empty(self.N, dtype=torch.float32, device=self._dev())
         nngb = torch.empty(self.N, dtype=torch.int32, device=self._dev()) if want_nngb else None
-        self._check(_lib.otoo_sph_density(self._h, _ptr(h, torch.float32), int(group_size), _ptr(rho),
-                                          _ptr(nngb), _stream(stream)))
+        self._check(_lib.otoo_sph_density(self._h, self._p(h, torch.float32), int(group_size), self._p(rho),
+                                          self._p(nngb), self._stream(stream)))
         return rho, nngb
 
     def otoo_sph_force_visc(self, h, rho, P, vel, visc, group_size, stream=None):
         """pressure force + artificial viscosity + du/dt; visc = (N,4) fp32 (c, alpha, Balsara f, -)"""
         out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
-        self._check(_lib.otoo_sph_force_visc(self._h, _ptr(h, torch.float32), _ptr(rho, torch.float32), _ptr(P, torch.float32),
-                                             _ptr(vel, torch.float32, 4), _ptr(visc, torch.float32, 4), int(group_size),
-                                             out.data_ptr(), _stream(stream)))
+        self._check(_lib.otoo_sph_force_visc(self._h, self._p(h, torch.float32), self._p(rho, torch.float32), self._p(P, torch.float32),
+                                             self._p(vel, torch.float32, 4), self._p(visc, torch.float32, 4), int(group_size),
+                                             out.dataself._p(), self._stream(stream)))
         return out
 
     def otoo_sph_stage1(self, h, vel, group_size, stream=None):
@@ -164,29 +180,29 @@ class Otoo:
         rho = torch.empty(self.N, dtype=torch.float32, device=self._dev())
         nngb = torch.empty(self.N, dtype=torch.int32, device=self._dev())
         dr = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
-        self._check(_lib.otoo_sph_stage1(self._h, _ptr(h, torch.float32), _ptr(vel, torch.float32, 4), int(group_size),
-                                         rho.data_ptr(), nngb.data_ptr(), dr.data_ptr(), _stream(stream)))
+        self._check(_lib.otoo_sph_stage1(self._h, self._p(h, torch.float32), self._p(vel, torch.float32, 4), int(group_size),
+                                         rho.dataself._p(), nngb.dataself._p(), dr.dataself._p(), self._stream(stream)))
         return rho, nngb, dr
 
     def otoo_sph_adapt_h(self, h, n_target, tol, max_iter, group_size, stream=None):
         """h (N floats on the device) is updated in place; returns (nngb of the final h, updates made)"""
         nngb = torch.empty(self.N, dtype=torch.int32, device=self._dev())
         it = C.c_int(0)
-        self._check(_lib.otoo_sph_adapt_h(self._h, _ptr(h, torch.float32), float(n_target), float(tol), int(max_iter),
-                                          int(group_size), nngb.data_ptr(), C.byref(it), _stream(stream)))
+        self._check(_lib.otoo_sph_adapt_h(self._h, self._p(h, torch.float32), float(n_target), float(tol), int(max_iter),
+                                          int(group_size), nngb.dataself._p(), C.byref(it), self._stream(stream)))
         return nngb, int(it.value)
 
     def otoo_sph_force(self, h, rho, P, group_size, vel=None, stream=None):
         out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
-        self._check(_lib.otoo_sph_force(self._h, _ptr(h, torch.float32), _ptr(rho, torch.float32),
-                                        _ptr(P, torch.float32), _ptr(vel, torch.float32, 4) if vel is not None else None,
-                                        int(group_size), _ptr(out), _stream(stream)))
+        self._check(_lib.otoo_sph_force(self._h, self._p(h, torch.float32), self._p(rho, torch.float32),
+                                        self._p(P, torch.float32), self._p(vel, torch.float32, 4) if vel is not None else None,
+                                        int(group_size), self._p(out), self._stream(stream)))
         return out
 
     def otoo_eos_ideal(self, rho, u, gamma=5.0 / 3.0, stream=None):
         P = torch.empty_like(rho)
         self._check(_lib.otoo_eos_ideal(self._h, _ptr(rho, torch.float32), _ptr(u, torch.float32), float(gamma),
-                                        rho.numel(), _ptr(P), _stream(stream)))
+                                        rho.numel(), _ptr(P), self._stream(stream)))
         return P
 
     def otoo_gravity_host(self, pos_mass: np.ndarray, n_crit, eps, theta, group_size, out: np.ndarray = None):
@@ -196,6 +212,16 @@ class Otoo:
             out = np.empty((n, 4), dtype=np.float32)
         self._check(_lib.otoo_gravity_host(self._h, pm.ctypes.data, n, int(n_crit), float(eps), float(theta),
                                            int(group_size), out.ctypes.data))
+        self.N = n
+        return out
+
+    def otoo_gravity_delta_host(self, pos_mass: np.ndarray, n_crit, eps, delta, m_limit, group_size, out: np.ndarray = None):
+        pm = np.ascontiguousarray(pos_mass, dtype=np.float32)
+        n = pm.shape[0]
+        if out is None:
+            out = np.empty((n, 4), dtype=np.float32)
+        self._check(_lib.otoo_gravity_delta_host(self._h, pm.ctypes.data, n, int(n_crit), float(eps), float(delta),
+                                                 float(m_limit), int(group_size), out.ctypes.data))
         self.N = n
         return out
 
@@ -237,12 +263,22 @@ class Otoo:
     def otoo_last_stats(self):
         s = Stats()
         self._check(_lib.otoo_last_stats(self._h, C.byref(s)))
-        return {k: getattr(s, k) for k, _ in Stats._fields_}
+        d = {k: getattr(s, k) for k, _ in Stats._fields_}
+        d["ms_build"] = dict(zip(BUILD_PHASES, [float(x) for x in s.ms_build]))
+        return d
 
     def otoo_measure_fp32_peak(self, stream=None) -> float:
         v = C.c_double(0.0)
-        self._check(_lib.otoo_measure_fp32_peak(self._h, C.byref(v), _stream(stream)))
+        self._check(_lib.otoo_measure_fp32_peak(self._h, C.byref(v), self._stream(stream)))
         return float(v.value)
+
+    def otoo_probe(self, which: str, stream=None):
+        """microbenchmark table of the library (list of dicts); invalidates the tree"""
+        import json
+        buf = C.create_string_buffer(1 << 16)
+        self._check(_lib.otoo_probe(self._h, which.encode(), buf, len(buf), self._stream(stream)))
+        self.N = 0
+        return json.loads(buf.value.decode())
 
     def otoo_set_option(self, name: str, value: int):
         self._check(_lib.otoo_set_option(self._h, name.encode(), int(value)))

@@ -50,6 +50,7 @@ otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups) {
   if (ctx->g_ntests) cudaFree(ctx->g_ntests);
   if (ctx->g_ncells) cudaFree(ctx->g_ncells);
   if (ctx->g_nparts) cudaFree(ctx->g_nparts);
+  ctx->g_ntests = ctx->g_ncells = ctx->g_nparts = nullptr;   // a failed allocation below must not leave freed pointers
   ctx->groupCap = 0;
   OTOO_TRY(dalloc(ctx, &ctx->g_ntests, ngroups));
   OTOO_TRY(dalloc(ctx, &ctx->g_ncells, ngroups));
@@ -60,6 +61,7 @@ otoo_status otoo_ensure_groups(otoo_ctx* ctx, int64_t ngroups) {
 otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps) {
   if (warps <= ctx->spill_warps) return OTOO_OK;
   if (ctx->walk_spill) cudaFree(ctx->walk_spill);
+  ctx->walk_spill = nullptr;
   ctx->spill_warps = 0;
   OTOO_TRY(dalloc(ctx, &ctx->walk_spill, (size_t)warps * OTOO_WALK_SPILL));
   ctx->spill_warps = warps;
@@ -68,7 +70,7 @@ otoo_status otoo_ensure_spill(otoo_ctx* ctx, int64_t warps) {
 
 extern "C" {
 
-int otoo_version(void) { return 1; }
+int otoo_version(void) { return 2; }
 
 otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
   if (!out) return OTOO_ERR_INVALID_ARG;
@@ -79,7 +81,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
   otoo_ctx* ctx = new (std::nothrow) otoo_ctx;
   if (!ctx) return OTOO_ERR_OOM;
   memset(ctx, 0, sizeof *ctx);
-  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->use_pool = 1; ctx->use_ws = 1; ctx->group_begin = 0; ctx->group_count = -1;
+  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->walk_spill_cap = OTOO_WALK_SPILL; ctx->use_pool = 1; ctx->use_ws = 1; ctx->group_begin = 0; ctx->group_count = -1;
   otoo_status s = OTOO_OK;
   auto body = [&]() -> otoo_status {
     OTOO_CUDA(ctx, cudaSetDevice(device));
@@ -100,6 +102,8 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, 8 * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
+    for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
+    for (auto& e : ctx->ev_walk) OTOO_CUDA(ctx, cudaEventCreate(&e));
     return OTOO_OK;
   };
   s = body();
@@ -120,6 +124,8 @@ void otoo_destroy(otoo_ctx* ctx) {
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);
+  for (auto& e : ctx->ev_build) if (e) cudaEventDestroy(e);
+  for (auto& e : ctx->ev_walk) if (e) cudaEventDestroy(e);
   delete ctx;
 }
 
@@ -293,7 +299,10 @@ otoo_status otoo_export_group_stats(otoo_ctx* ctx, uint32_t* d_ntests, uint32_t*
   if (d_ntests) OTOO_CUDA(ctx, cudaMemcpyAsync(d_ntests, ctx->g_ntests, b, cudaMemcpyDeviceToDevice, st));
   if (d_ncells) OTOO_CUDA(ctx, cudaMemcpyAsync(d_ncells, ctx->g_ncells, b, cudaMemcpyDeviceToDevice, st));
   if (d_nparts) OTOO_CUDA(ctx, cudaMemcpyAsync(d_nparts, ctx->g_nparts, b, cudaMemcpyDeviceToDevice, st));
+  unsigned long long flag = 0;
+  OTOO_CUDA(ctx, cudaMemcpyAsync(&flag, ctx->d_sums + 7, sizeof flag, cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaStreamSynchronize(st));
+  if (flag) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "the last walk overflowed its private spill area: results invalid");
   return OTOO_OK;
 }
 
@@ -307,9 +316,26 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
     OTOO_CUDA(ctx, cudaMemcpy(h, ctx->d_sums, sizeof h, cudaMemcpyDeviceToHost));
     o->sum_tests = h[0]; o->sum_interactions = h[1]; o->sum_cells = h[2]; o->sum_parts = h[3];
     o->sum_steps = h[4]; o->sum_tasks = h[5]; o->sum_flushes = h[6];
+    o->error_flag = (int32_t)h[7];
     o->n_groups = ctx->last_ngroups; o->group_size = ctx->last_group_size;
+    o->walk_only = ctx->last_walk_only;
   }
   o->launches = ctx->launches;
+  // per-phase device times; events of other streams than last_stream have completed too if the caller kept to
+  // one stream per context (the convention of otoo.h)
+  if (ctx->ev_build_valid) {
+    for (int p = 0; p < OTOO_BUILD_PHASES; p++)
+      if (cudaEventElapsedTime(&o->ms_build[p], ctx->ev_build[p], ctx->ev_build[p + 1]) != cudaSuccess) { o->ms_build[p] = 0.0f; cudaGetLastError(); }
+    for (int p = 0; p < OTOO_BUILD_PHASES; p++) o->ms_build_total += o->ms_build[p];
+  }
+  if (ctx->ev_walk_valid) {
+    float a = 0.0f, b = 0.0f;
+    if (cudaEventElapsedTime(&a, ctx->ev_walk[0], ctx->ev_walk[1]) == cudaSuccess &&
+        cudaEventElapsedTime(&b, ctx->ev_walk[1], ctx->ev_walk[2]) == cudaSuccess) {
+      o->ms_walk_prep = a; o->ms_walk_force = b; o->ms_total = a + b;
+    } else cudaGetLastError();
+  }
+  if (o->error_flag) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "the last walk overflowed its private spill area: results invalid");
   return OTOO_OK;
 }
 
@@ -324,6 +350,11 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   if (strcmp(name, "walk_stack") == 0) {
     if (value < 512 || value > OTOO_WALK_STACK_MAX) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "walk_stack out of range");
     ctx->walk_stack = (int)value;
+    return OTOO_OK;
+  }
+  if (strcmp(name, "walk_spill") == 0) {
+    if (value < 0 || value > OTOO_WALK_SPILL) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "walk_spill out of range");
+    ctx->walk_spill_cap = (int)value;
     return OTOO_OK;
   }
   if (strcmp(name, "task_pool") == 0) { ctx->use_pool = value != 0; return OTOO_OK; }
@@ -349,8 +380,8 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown option");
 }
 
-otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit, float eps, float theta,
-                              int group_size, float* h_acc_pot) {
+static otoo_status gravity_host_impl(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit, float eps, int mac, float p0,
+                                     float p1, int group_size, float* h_acc_pot) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
   if (N < 0 || !h_pos_mass || !h_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL host buffer or N < 0");
   if (N > ctx->maxN) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "N exceeds max_particles of otoo_create");
@@ -376,11 +407,22 @@ otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N,
   if (cudaMemcpyAsync(d_in, h_pos_mass, 16 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "H2D copy failed");
   if (s == OTOO_OK) s = otoo_build_tree(ctx, reinterpret_cast<const float*>(d_in), N, n_crit, st);
   int l1 = ctx->launches;
-  if (s == OTOO_OK) s = otoo_gravity(ctx, eps, theta, group_size, reinterpret_cast<float*>(d_out), st);
+  if (s == OTOO_OK)
+    s = mac == 0 ? otoo_gravity(ctx, eps, p0, group_size, reinterpret_cast<float*>(d_out), st)
+                 : otoo_gravity_delta(ctx, eps, p0, p1, group_size, reinterpret_cast<float*>(d_out), st);
   ctx->launches += l1;
   if (s == OTOO_OK && cudaMemcpyAsync(h_acc_pot, d_out, 16 * (size_t)N, cudaMemcpyDeviceToHost, st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "D2H copy failed");
   if (s == OTOO_OK && cudaStreamSynchronize(st) != cudaSuccess) s = otoo_fail(ctx, OTOO_ERR_CUDA, "synchronize failed");
   return s;
+}
+
+otoo_status otoo_gravity_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit, float eps, float theta,
+                              int group_size, float* h_acc_pot) {
+  return gravity_host_impl(ctx, h_pos_mass, N, n_crit, eps, 0, theta, 0.0f, group_size, h_acc_pot);
+}
+otoo_status otoo_gravity_delta_host(otoo_ctx* ctx, const float* h_pos_mass, int64_t N, int n_crit, float eps, float delta,
+                                    float m_limit, int group_size, float* h_acc_pot) {
+  return gravity_host_impl(ctx, h_pos_mass, N, n_crit, eps, 1, delta, m_limit, group_size, h_acc_pot);
 }
 
 }  // extern "C"

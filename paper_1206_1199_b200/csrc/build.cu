@@ -420,6 +420,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   const float4* pos = reinterpret_cast<const float4*>(d_pos_mass);
   unsigned* bbox = reinterpret_cast<unsigned*>(ctx->d_bbox);
   const unsigned nbN = (unsigned)cdiv(N, 256);
+  ctx->ev_build_valid = false;
+  OTOO_EV(ctx, ctx->ev_build[0], st);
   // H1
   OTOO_CUDA(ctx, cudaMemsetAsync(bbox, 0xFF, 12, st));      // min = 0xFFFFFFFF
   OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 12, st));  // max = 0
@@ -427,13 +429,17 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   int gb = ctx->sm_count * 4; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
   root_kernel<<<1, 1, 0, st>>>(bbox);
+  OTOO_EV(ctx, ctx->ev_build[1], st);
   // H2, H3, H4
   key_kernel<<<nbN, 256, 0, st>>>(pos, N, bbox, ctx->key[0], ctx->val[0], ctx->key_order);
   ctx->launches += 3;
+  OTOO_EV(ctx, ctx->ev_build[2], st);
   int res = 0;
   OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res));
   if (res != 0) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: sort result buffer");
+  OTOO_EV(ctx, ctx->ev_build[3], st);
   gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
+  OTOO_EV(ctx, ctx->ev_build[4], st);
   // H5a
   uint32_t* info = ctx->val[1];
   if (n_crit <= OTOO_SLOT_NCRIT_MAX) slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
@@ -459,6 +465,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
                                             ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
                                             ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);
   ctx->launches += 1;
+  OTOO_EV(ctx, ctx->ev_build[5], st);
   // H6 deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
                       bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order};
@@ -475,6 +482,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
     OTOO_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)moments_all_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
     ctx->launches += 1;
   }
+  OTOO_EV(ctx, ctx->ev_build[6], st);
+  ctx->ev_build_valid = true;
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 32, ctx->d_counters + 32, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->N = N; ctx->N_cell = ncell; ctx->n_crit = n_crit; ctx->depth = depth;

@@ -18,6 +18,7 @@
 // u32 words of sort scratch for n pairs: digit histograms + tickets (4096) + one u64 status word per tile and digit
 #define OTOO_SORT_SCRATCH(n) ((size_t)(((n) + OTOO_SORT_TILE - 1) / OTOO_SORT_TILE) * 512 + 4096)
 #define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
+#define OTOO_BUILD_PHASES 6          // root cube, keys, sort, gather, cells (topology), moments
 
 // Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).
 //   x = rb^2 bits (gravity MAC, R7), y = first child id (internal) or first sorted slot (leaf),
@@ -97,6 +98,7 @@ struct otoo_ctx {
   float lo[3], S;
   uint32_t level_off[OTOO_NLEV + 1];
   int walk_stack;        // option "walk_stack"
+  int walk_spill_cap;    // option "walk_spill" (test hook): usable private spill entries per warp
   int use_pool;          // option "task_pool"
   int64_t group_begin, group_count;   // options: the walks cover groups [begin, begin + count) only (count < 0: to the end)
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
@@ -107,7 +109,15 @@ struct otoo_ctx {
   int last_group_size;
   int64_t last_ngroups;
   int launches;          // kernels launched by the current/last API call
+  int last_walk_only;    // the last walk ran with option "walk_only" (its outputs are meaningless)
+
+  // ---- per-phase device times (the paper's TREE / KERNEL split): CUDA events
+  // recorded on the call's stream, read by otoo_last_stats (which synchronises)
+  cudaEvent_t ev_build[OTOO_BUILD_PHASES + 1];   // phase p = ev_build[p] .. ev_build[p + 1]
+  cudaEvent_t ev_walk[3];                        // call start, walk kernel start, walk kernel end
+  bool ev_build_valid, ev_walk_valid;
 };
+#define OTOO_EV(ctx, ev, st) OTOO_CUDA(ctx, cudaEventRecord((ev), (st)))
 
 #define OTOO_CUDA(ctx, call)                                                                   \
   do {                                                                                         \

@@ -1,10 +1,7 @@
 // gravity.cu -- theta-MAC radii (R7) and the fused group walk + softened Plummer sums
 // (PAPER.md III-D L159-L167, L43, L57; readings R7-R11).
-#include "walk_ws.cuh"
+#include "grav_eval.cuh"
 
-#ifndef OTOO_EVAL_UNR
-#define OTOO_EVAL_UNR 4
-#endif
 #ifndef OTOO_WS_MINB
 #define OTOO_WS_MINB 3
 #define OTOO_WS_EVAL_REGS 112
@@ -49,144 +46,6 @@ __global__ void __launch_bounds__(256) rb2_delta_kernel(const double* __restrict
   }
   reinterpret_cast<uint32_t*>(cell_b + c)[0] = __float_as_uint(rb2);
 }
-
-struct GravParams {
-  WalkCommon c;
-  float eps2;
-  float4* acc_pot;          // zeroed before the launch
-};
-
-constexpr float PAD_POS = 1.0e18f;  // zero-mass padding entries sit far away: contribute exactly 0
-
-// Gravity visitor: R10 sums.  13 FP32 lane-ops + 1 MUFU per interaction, issued two targets at a
-// time as FFMA2/FADD2/FMUL2; two-level summation (64-entry fp32 partial sums, then totals).
-__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
-__device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
-
-template <int T_, bool EPS0>
-struct GravVisitor {
-  static constexpr int T = T_, E = 1, LCAP = OTOO_LIST_CAP, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64, UNR = OTOO_EVAL_UNR;
-  const GravParams& p;
-  float pm[T];
-  float glo[3], ghi[3];
-  f32x2 PX[NP], PY[NP], PZ[NP];                       // two targets per aligned register pair (kept as b64)
-  float2 AX[NP], AY[NP], AZ[NP], PH[NP];
-  unsigned selfmask;
-  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_) {}
-
-  __device__ __forceinline__ void load_group(int64_t g0, int lane, float4* scratch) {
-    float px[T], py[T], pz[T];
-#pragma unroll
-    for (int t = 0; t < T; t++) {   // H7: lane holds slots g0 + t*32 + lane; out-of-range lanes mirror slot g0
-      int64_t s = g0 + t * 32 + lane;
-      float4 v = p.c.spos[s < p.c.N ? s : g0];
-      px[t] = v.x; py[t] = v.y; pz[t] = v.z; pm[t] = v.w;
-      if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
-      else {
-        glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
-        glo[1] = fminf(glo[1], v.y); ghi[1] = fmaxf(ghi[1], v.y);
-        glo[2] = fminf(glo[2], v.z); ghi[2] = fmaxf(ghi[2], v.z);
-      }
-    }
-#pragma unroll
-    for (int k = 0; k < 3; k++)
-#pragma unroll
-      for (int o = 16; o; o >>= 1) {
-        glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
-        ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
-      }
-#pragma unroll
-    for (int q = 0; q < NP; q++) {
-      const int t1 = (2 * q + 1 < T) ? 2 * q + 1 : 2 * q;
-      // Round trip through (idle) list memory: the pairs are born as 64-bit values in aligned register
-      // pairs.  Without it ptxas keeps the LDG.128 quads and re-pairs x/y/z with 6 MOVs per target pair
-      // and list entry inside the hot loop (measured: 25 % of all issued instructions).
-      const unsigned sa = (unsigned)__cvta_generic_to_shared(scratch) + (unsigned)(lane * NP * 3 + q * 3) * 8u;
-      asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(sa), "f"(px[2 * q]), "f"(px[t1]) : "memory");
-      asm volatile("st.shared.v2.f32 [%0+8], {%1,%2};" ::"r"(sa), "f"(py[2 * q]), "f"(py[t1]) : "memory");
-      asm volatile("st.shared.v2.f32 [%0+16], {%1,%2};" ::"r"(sa), "f"(pz[2 * q]), "f"(pz[t1]) : "memory");
-      asm volatile("ld.shared.b64 %0, [%1];" : "=l"(PX[q]) : "r"(sa) : "memory");
-      asm volatile("ld.shared.b64 %0, [%1+8];" : "=l"(PY[q]) : "r"(sa) : "memory");
-      asm volatile("ld.shared.b64 %0, [%1+16];" : "=l"(PZ[q]) : "r"(sa) : "memory");
-      AX[q] = AY[q] = AZ[q] = PH[q] = make_float2(0.0f, 0.0f);
-    }
-    selfmask = 0;
-  }
-  __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
-    A = __ldg(p.c.cell_cm + cell);
-    B = __ldg(p.c.cell_b + cell);
-    float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
-    return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
-  }
-  struct Entry { float4 a; };
-  __device__ __forceinline__ Entry get(uint32_t slot) const { Entry e; e.a = p.c.spos[slot]; return e; }
-  __device__ __forceinline__ void put(float4* dst, const Entry& e) const { *dst = e.a; }
-  __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
-  __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
-#pragma unroll
-    for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
-  }
-  static constexpr bool SUBMIT_LAST = false, CULL = false;
-  template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
-  __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
-    if (!p.c.walk_only) eval(list, n);
-    return list;
-  }
-  // 13 FP32 lane-ops + 1 MUFU per interaction, as 13 packed FFMA2/FADD2/FMUL2 + 2 MUFU per target pair
-  // (the list entry is a scalar broadcast operand); two-level summation: 64-entry partial sums, then totals.
-  __device__ __forceinline__ void eval(const float4* __restrict__ list, int n) {
-    const float2 e2 = bc2(p.eps2);
-#pragma unroll
-    for (int pb = 0; pb < NP; pb += PB) {
-      for (int j0 = 0; j0 < n; j0 += BLK) {
-        const int je = j0 + BLK < n ? j0 + BLK : n;
-        float2 cx[PB], cy[PB], cz[PB], cp[PB];
-#pragma unroll
-        for (int q = 0; q < PB; q++) cx[q] = cy[q] = cz[q] = cp[q] = make_float2(0.0f, 0.0f);
-#pragma unroll UNR
-        for (int j = j0; j < je; j++) {
-          const float4 s = list[j];
-#pragma unroll
-          for (int q = 0; q < PB; q++) {
-            const float2 dx = __fadd2_rn(bc2(s.x), neg2(as2(PX[pb + q])));
-            const float2 dy = __fadd2_rn(bc2(s.y), neg2(as2(PY[pb + q])));
-            const float2 dz = __fadd2_rn(bc2(s.z), neg2(as2(PZ[pb + q])));
-            const float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __ffma2_rn(dz, dz, e2)));
-            float2 ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
-            if (EPS0) { ri.x = r2.x > 0.0f ? ri.x : 0.0f; ri.y = r2.y > 0.0f ? ri.y : 0.0f; }  // r = 0 pairs contribute 0
-            const float2 mri = __fmul2_rn(bc2(s.w), ri);
-            const float2 mr3 = __fmul2_rn(mri, __fmul2_rn(ri, ri));
-            cp[q] = __fadd2_rn(cp[q], neg2(mri));
-            cx[q] = __ffma2_rn(mr3, dx, cx[q]);
-            cy[q] = __ffma2_rn(mr3, dy, cy[q]);
-            cz[q] = __ffma2_rn(mr3, dz, cz[q]);
-          }
-        }
-#pragma unroll
-        for (int q = 0; q < PB; q++) {
-          AX[pb + q] = __fadd2_rn(AX[pb + q], cx[q]); AY[pb + q] = __fadd2_rn(AY[pb + q], cy[q]);
-          AZ[pb + q] = __fadd2_rn(AZ[pb + q], cz[q]); PH[pb + q] = __fadd2_rn(PH[pb + q], cp[q]);
-        }
-      }
-    }
-  }
-  // H10: original order; the self term is removed from phi by whichever task saw it (R10)
-  __device__ __forceinline__ void store(int64_t g0, int lane) {
-    const float rie = EPS0 ? 0.0f : rsqrt_approx(p.eps2);
-#pragma unroll
-    for (int t = 0; t < T; t++) {
-      const int64_t s = g0 + t * 32 + lane;
-      const int q = t >> 1;
-      float4 o = (t & 1) ? make_float4(AX[q].y, AY[q].y, AZ[q].y, PH[q].y) : make_float4(AX[q].x, AY[q].x, AZ[q].x, PH[q].x);
-      if ((selfmask >> t) & 1u) o.w = __fmaf_rn(pm[t], rie, o.w);
-      if (s < p.c.N) {
-        float* dst = reinterpret_cast<float*>(p.acc_pot + p.c.perm[s]);
-        atomicAdd(dst + 0, o.x); atomicAdd(dst + 1, o.y); atomicAdd(dst + 2, o.z); atomicAdd(dst + 3, o.w);
-      }
-    }
-  }
-};
 
 template <int T, bool EPS0>
 __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(const GravParams p) {
@@ -406,6 +265,8 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   if (g_begin < 0 || ngroups < 0 || g_begin + ngroups > total_groups)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_begin / group_count outside the groups of this group_size");
   OTOO_TRY(otoo_ensure_groups(ctx, total_groups));
+  ctx->ev_walk_valid = false;
+  OTOO_EV(ctx, ctx->ev_walk[0], st);
   *smem = otoo_walk_smem_bytes();
   int per_sm = (int)((227 * 1024) / (*smem + 1024));
   if (per_sm < 1) per_sm = 1;
@@ -429,12 +290,12 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
-  c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack;
+  c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack; c->spill_cap = ctx->walk_spill_cap;
   c->use_pool = ctx->use_pool;
   c->walk_only = ctx->walk_only;
   c->dist_kind = 0;
   ctx->launches += 1;
-  ctx->last_group_size = G; ctx->last_ngroups = total_groups;
+  ctx->last_group_size = G; ctx->last_ngroups = total_groups; ctx->last_walk_only = ctx->walk_only;
   return OTOO_OK;
 }
 
@@ -457,6 +318,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   if (ctx->dist_kind && !ctx->use_ws)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance = 1 needs warp_specialized = 1");
   p.c.dist_kind = ctx->dist_kind;
+  OTOO_EV(ctx, ctx->ev_walk[1], st);
   if (ctx->use_ws) {
     switch (G) {
       case 32: OTOO_TRY(launch_walk_ws<1>(ctx, p, eps0, st)); break;
@@ -473,6 +335,8 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
     case 256: OTOO_TRY(launch_walk<8>(ctx, p, eps0, grid, smem, st)); break;
     default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
   }
+  OTOO_EV(ctx, ctx->ev_walk[2], st);
+  ctx->ev_walk_valid = true;
   ctx->launches += 2;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;

@@ -32,9 +32,13 @@ __global__ void __launch_bounds__(256) gather_vel_kernel(const float4* __restric
   if (s < n) svel[s] = vel[perm[s]];
 }
 // (div v, rot v) sums -> estimates: divide by the particle's density (R22)
-__global__ void __launch_bounds__(256) divrot_finish_kernel(const float* __restrict__ rho, int64_t n, float4* __restrict__ dr) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+// over the sorted slots [s0, s1) of the walked target groups only: with a group range (options group_begin /
+// group_count) the other targets keep their zeros (0/0 would poison the sum over the ranges)
+__global__ void __launch_bounds__(256) divrot_finish_kernel(const float* __restrict__ rho, const uint32_t* __restrict__ perm,
+                                                            int64_t s0, int64_t s1, float4* __restrict__ dr) {
+  const int64_t s = s0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= s1) return;
+  const uint32_t i = perm[s];
   const float r = rho[i];
   float4 v = dr[i];
   dr[i] = make_float4(__fdiv_rn(v.x, r), __fdiv_rn(v.y, r), __fdiv_rn(v.z, r), __fdiv_rn(v.w, r));
@@ -571,7 +575,10 @@ otoo_status launch_sph_ws2(otoo_ctx* ctx, const SphParams& p, cudaStream_t st) {
   if (occ < 1) occ = 1;
   int64_t grid = (int64_t)ctx->sm_count * occ;
   if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups > 0 ? p.c.ngroups : 1, OTOO_WS_PAIRS);
+  OTOO_EV(ctx, ctx->ev_walk[1], st);
   walk_sph_ws_kernel<T, MODE><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
+  OTOO_EV(ctx, ctx->ev_walk[2], st);
+  ctx->ev_walk_valid = true;
   return OTOO_OK;
 }
 template <int MODE>
@@ -595,7 +602,10 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_kernel<TT, MODE>, OTOO_WALK_WARPS * 32, smem));  \
   if (occ < 1) occ = 1;                                                                                                 \
   if (grid > ctx->sm_count * occ) grid = ctx->sm_count * occ;                                                          \
-  walk_sph_kernel<TT, MODE><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);
+  OTOO_EV(ctx, ctx->ev_walk[1], st);                                                                                    \
+  walk_sph_kernel<TT, MODE><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);                                               \
+  OTOO_EV(ctx, ctx->ev_walk[2], st);                                                                                    \
+  ctx->ev_walk_valid = true;
   switch (G) {
     case 32: OTOO_SPH_CASE(1) break;
     case 64: OTOO_SPH_CASE(2) break;
@@ -661,7 +671,11 @@ otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d
   if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(d_divrot, 0, 16 * (size_t)ctx->N, st));
   OTOO_TRY(launch_sph<3>(ctx, p, G, grid, smem, st));
-  divrot_finish_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_rho, ctx->N, reinterpret_cast<float4*>(d_divrot));
+  {
+    const int64_t s0 = (int64_t)p.c.g_begin * G, s1 = s0 + p.c.ngroups * G < ctx->N ? s0 + p.c.ngroups * G : ctx->N;
+    if (s1 > s0)
+      divrot_finish_kernel<<<(unsigned)cdiv(s1 - s0, 256), 256, 0, st>>>(d_rho, ctx->val[0], s0, s1, reinterpret_cast<float4*>(d_divrot));
+  }
   ctx->launches += 3;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;
@@ -699,12 +713,16 @@ otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_
 // ---------------------------------------------------------------- adaptive smoothing length (reading R21)
 namespace {
 // settle the particles whose count is within the tolerance, count the others
-__global__ void __launch_bounds__(256) adapt_check_kernel(const uint32_t* __restrict__ nngb, int64_t n, double n_target, double tol,
+// (both kernels run over the sorted slots [s0, s1) of the walked target groups: with a group range the other
+// particles' h is left alone)
+__global__ void __launch_bounds__(256) adapt_check_kernel(const uint32_t* __restrict__ nngb, const uint32_t* __restrict__ perm,
+                                                          int64_t s0, int64_t s1, double n_target, double tol,
                                                           const float* __restrict__ h, float* __restrict__ lo, float* __restrict__ hi,
                                                           uint32_t* __restrict__ bad) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t s = s0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   bool unsettled = false;
-  if (i < n) {
+  if (s < s1) {
+    const uint32_t i = perm[s];
     if (lo[i] != hi[i]) {                                           // lo == hi marks a settled particle
       if (!(fabs((double)nngb[i] - n_target) > tol)) lo[i] = hi[i] = h[i];
       else unsettled = true;
@@ -714,10 +732,13 @@ __global__ void __launch_bounds__(256) adapt_check_kernel(const uint32_t* __rest
   if ((threadIdx.x & 31) == 0 && m) atomicAdd(bad, (uint32_t)__popc(m));
 }
 // one update of the bracketed root search, same operations as the oracle
-__global__ void __launch_bounds__(256) adapt_update_kernel(const uint32_t* __restrict__ nngb, int64_t n, double n_target,
+__global__ void __launch_bounds__(256) adapt_update_kernel(const uint32_t* __restrict__ nngb, const uint32_t* __restrict__ perm,
+                                                           int64_t s0, int64_t s1, double n_target,
                                                            float* __restrict__ h, float* __restrict__ lo, float* __restrict__ hi) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n || lo[i] == hi[i]) return;
+  const int64_t s = s0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= s1) return;
+  const uint32_t i = perm[s];
+  if (lo[i] == hi[i]) return;
   const double ni = (double)nngb[i];
   float l = lo[i], u = hi[i];
   const float hc = h[i];
@@ -750,18 +771,24 @@ otoo_status otoo_sph_adapt_h_impl(otoo_ctx* ctx, float* d_h, float n_target, flo
   uint32_t* cnt = reinterpret_cast<uint32_t*>(lo + 3 * N);
   uint32_t* bad = ctx->d_counters + 48;
   const unsigned nb = (unsigned)cdiv(N, 256);
+  const int64_t total_groups = cdiv(N, G);
+  const int64_t gb = ctx->group_begin, gc = ctx->group_count < 0 ? total_groups - gb : ctx->group_count;
+  if (gb < 0 || gc < 0 || gb + gc > total_groups)
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_begin / group_count outside the groups of this group_size");
+  const int64_t s0 = gb * G, s1 = (gb + gc) * G < N ? (gb + gc) * G : N;
+  const unsigned nbr = (unsigned)cdiv(s1 > s0 ? s1 - s0 : 1, 256);
   adapt_init_kernel<<<nb, 256, 0, st>>>(N, lo, hi);
   int it = 0, launches = 1;
   for (;;) {
     OTOO_TRY(otoo_sph_density_impl(ctx, d_h, G, rho, cnt, st));
     launches += ctx->launches; ctx->launches = 0;
     OTOO_CUDA(ctx, cudaMemsetAsync(bad, 0, sizeof(uint32_t), st));
-    adapt_check_kernel<<<nb, 256, 0, st>>>(cnt, N, (double)n_target, (double)tol, d_h, lo, hi, bad);
+    adapt_check_kernel<<<nbr, 256, 0, st>>>(cnt, ctx->val[0], s0, s1, (double)n_target, (double)tol, d_h, lo, hi, bad);
     OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 48, bad, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
     OTOO_CUDA(ctx, cudaStreamSynchronize(st));
     launches += 1;
     if (ctx->h_counters[48] == 0 || it >= max_iter) break;
-    adapt_update_kernel<<<nb, 256, 0, st>>>(cnt, N, (double)n_target, d_h, lo, hi);
+    adapt_update_kernel<<<nbr, 256, 0, st>>>(cnt, ctx->val[0], s0, s1, (double)n_target, d_h, lo, hi);
     launches += 1;
     it++;
   }

@@ -69,6 +69,7 @@ struct WalkCommon {
   WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
   uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
   int stack_cap;
+  int spill_cap;                                                // usable entries of a warp's private spill area (<= OTOO_WALK_SPILL)
   int use_pool;                                                 // 0: never donate (test hook: private spill only)
   int walk_only;                                                // 1: lists are built and counted but not evaluated (measures the walk)
   int dist_kind;                                                // gravity: 0 group AABB distance (R8), 1 exact minimum over the members (R23)
@@ -256,8 +257,15 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
               pushed = true;
             } else {
               const int d = OTOO_TASK_CELLS;      // stack_cap >= 512, total <= 256
-              for (int i = lane; i < d; i += 32) gspill[gsp + i] = stk[i];
-              gsp += d;
+              if (gsp + d <= c.spill_cap) {
+                for (int i = lane; i < d; i += 32) gspill[gsp + i] = stk[i];
+                gsp += d;
+              } else if (lane == 0) {
+                // the private area is full too (cannot happen with the level-sorted stack bound of common.cuh;
+                // reachable only through the test hooks): the cells are dropped and the launch is flagged --
+                // otoo_last_stats / otoo_export_group_stats then return OTOO_ERR_CAPACITY
+                atomicExch(c.sums + 7, 1ull);
+              }
               __syncwarp();
               shift_down(d);
             }

@@ -458,3 +458,115 @@ def test_config1_against_direct_sum(otoo, orc):
     e = np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / an
     assert 1e-6 < np.median(e) < 1e-3 and np.percentile(e, 99) < 1e-2
     assert np.median(np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])) < 1e-3
+
+
+def test_stats_phase_times_and_walk_only_flag(otoo, orc):
+    """otoo_stats_t: per-phase device times of the last build and the last walk, and the record that a
+    walk ran with `walk_only` (its outputs must not be mistaken for a result)."""
+    pm = gen.plummer(200000, 3)
+    otoo.otoo_build_tree(dev(pm), 16)
+    otoo.otoo_gravity(0.01, 0.6, 128)
+    st = otoo.otoo_last_stats()
+    assert set(st["ms_build"]) == {"root_cube", "keys", "sort", "gather", "cells", "moments"}
+    assert all(v > 0 for v in st["ms_build"].values())
+    assert st["ms_build_total"] == pytest.approx(sum(st["ms_build"].values()), rel=1e-5)
+    assert st["ms_walk_force"] > 0 and st["ms_walk_prep"] > 0
+    assert st["ms_total"] == pytest.approx(st["ms_walk_prep"] + st["ms_walk_force"], rel=1e-5)
+    assert st["ms_walk_force"] > st["ms_walk_prep"]                   # the fused walk + sum kernel dominates the call
+    assert st["walk_only"] == 0 and st["error_flag"] == 0
+    inter = st["sum_interactions"]
+    otoo.otoo_set_option("walk_only", 1)
+    try:
+        otoo.otoo_gravity(0.01, 0.6, 128)
+        st2 = otoo.otoo_last_stats()
+        assert st2["walk_only"] == 1 and st2["sum_interactions"] == inter   # counters exact, outputs flagged
+    finally:
+        otoo.otoo_set_option("walk_only", 0)
+    otoo.otoo_gravity(0.01, 0.6, 128)
+    assert otoo.otoo_last_stats()["walk_only"] == 0
+
+
+def test_spill_overflow_is_reported(otoo, orc):
+    """Without the task pool and with a private spill area too small for theta = 0 on a deep tree the walk drops
+    cells: the launch is flagged and the introspection calls return OTOO_ERR_CAPACITY instead of wrong numbers."""
+    from paper_1206_1199_b200 import binding
+    pm = gen.plummer(30000, 77)
+    otoo.otoo_build_tree(dev(pm), 1)
+    try:
+        otoo.otoo_set_option("task_pool", 0)
+        otoo.otoo_set_option("walk_spill", 256)
+        otoo.otoo_gravity(0.01, 0.0, 32)
+        with pytest.raises(binding.OtooError) as e:
+            otoo.otoo_last_stats()
+        assert e.value.status == binding.OTOO_ERR_CAPACITY
+        with pytest.raises(binding.OtooError) as e:
+            otoo.otoo_export_group_stats()
+        assert e.value.status == binding.OTOO_ERR_CAPACITY
+        otoo.otoo_set_option("walk_spill", 8192)
+        otoo.otoo_gravity(0.01, 0.0, 32)
+        assert otoo.otoo_last_stats()["error_flag"] == 0 and otoo.otoo_last_stats()["sum_interactions"] == 30000 * 30000
+    finally:
+        otoo.otoo_set_option("task_pool", 1)
+        otoo.otoo_set_option("walk_spill", 8192)
+
+
+def test_delta_host_entry_point(otoo, orc):
+    pm = gen.plummer(10000, 5)
+    out = otoo.otoo_gravity_delta_host(pm, 16, 0.01, 0.01, 0.05, 64)
+    t = orc.Tree(pm, 16)
+    ref = t.gravity(float(np.float32(0.01)), 0.0, 64, rb2=t.rb2_delta(float(np.float32(0.01)), float(np.float32(0.05))))
+    e, _ = acc_err(out, ref["acc_pot"], ref["abs_sum"])
+    assert e.max() <= TOL
+    assert otoo.otoo_last_stats()["sum_interactions"] == ref["interactions"]
+
+
+def test_binding_rejects_short_arrays(otoo):
+    pm = gen.plummer(5000, 1)
+    otoo.otoo_build_tree(dev(pm), 16)
+    with pytest.raises(ValueError):
+        otoo.otoo_gravity(0.01, 0.5, 64, out=torch.empty((4999, 4), dtype=torch.float32, device="cuda"))
+    with pytest.raises(ValueError):
+        otoo.otoo_sph_density(torch.full((100,), 0.1, device="cuda"), 64)
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sph_target_sharding_ranges_add_up(otoo, orc, world):
+    """group_begin / group_count with the SPH entry points (PAPER III-E applied to stage 1 / stage 2): the ranges'
+    outputs are zero outside their targets (no 0/0 from the div/rot normalisation), add up to the single-call
+    result, and otoo_sph_adapt_h leaves the h of the other targets alone."""
+    from paper_1206_1199_b200 import sharded
+    n, G = 20000, 64
+    w = gen.wd_pair(n, 11)
+    pm, h = w["pos_mass"], w["h"]
+    vel = np.zeros((n, 4), np.float32)
+    vel[:, :3] = -0.4 * pm[:, :3] + 0.1 * np.sin(7 * pm[:, [1, 2, 0]])
+    t = check_tree(otoo, orc, pm, 16)
+    perm = t.export()["perm"].astype(np.int64)
+    d_h, d_v = dev(h), dev(vel)
+    rho_w, nn_w, dr_w = (x.cpu().numpy() for x in otoo.otoo_sph_stage1(d_h, d_v, G))
+    ng = t.n_groups(G)
+    h_adapt_whole = dev((h * np.float32(0.8)).astype(np.float32))
+    otoo.otoo_sph_adapt_h(h_adapt_whole, 50.0, 3.0, 30, G)
+    h_adapt_whole = h_adapt_whole.cpu().numpy()
+    rho_s, dr_s, nn_s = np.zeros(n), np.zeros((n, 4)), np.zeros(n, np.int64)
+    h_parts = (h * np.float32(0.8)).astype(np.float32)
+    try:
+        for b, c in sharded.group_ranges(ng, world):
+            otoo.otoo_set_option("group_begin", b)
+            otoo.otoo_set_option("group_count", c)
+            rho, nn, dr = (x.cpu().numpy() for x in otoo.otoo_sph_stage1(d_h, d_v, G))
+            mine = perm[b * G:min((b + c) * G, n)]
+            rest = np.setdiff1d(np.arange(n), mine)
+            assert np.isfinite(dr).all() and not dr[rest].any() and not rho[rest].any() and not nn[rest].any()
+            rho_s += rho; dr_s += dr; nn_s += nn
+            d_hp = dev(h_parts)
+            otoo.otoo_sph_adapt_h(d_hp, 50.0, 3.0, 30, G)
+            hp = d_hp.cpu().numpy()
+            assert np.array_equal(hp[rest], h_parts[rest])            # others untouched
+            assert np.array_equal(hp[mine].view(np.uint32), h_adapt_whole[mine].view(np.uint32))   # h_i depends on n_i(h_i) alone
+    finally:
+        otoo.otoo_set_option("group_begin", 0)
+        otoo.otoo_set_option("group_count", -1)
+    # (a group finished by several warps through the task pool adds its partial sums in another order)
+    assert np.array_equal(nn_s, nn_w) and np.allclose(rho_s, rho_w, rtol=2e-6)
+    assert np.allclose(dr_s, dr_w, rtol=1e-4, atol=1e-5 * np.abs(dr_w).max())
