@@ -231,11 +231,11 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
     torch.cuda.synchronize()
     if sampler is not None:
         sampler.start()
-    evs, kern_ms, prep_ms, phases = [], [], [], []
+    evs, kern_ms, prep_ms, phases, sm_mhz = [], [], [], [], []
     for _ in range(steps):
         evs.append(step())
         s = o.otoo_last_stats()      # synchronises: the kernel's own event pair and the build's phase events of THIS step
-        kern_ms.append(s["ms_walk_force"]); prep_ms.append(s["ms_walk_prep"]); phases.append(s["ms_build"])
+        kern_ms.append(s["ms_walk_force"]); prep_ms.append(s["ms_walk_prep"]); phases.append(s["ms_build"]); sm_mhz.append(s["walk_sm_mhz"])
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -246,7 +246,7 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
     ms_max, inter_all = replicas.aggregate(ms_step, float(inter), device="cuda")   # max over ranks, sum over ranks
     res = dict(cfg=cfg, n=n, G=G, inter=inter, inter_all=inter_all, ms_step=ms_max, value=inter_all / (ms_max * 1e-3),
                build_ms=float(t_build.mean()), call_ms=float(t_grav.mean()), kernel_ms=float(np.mean(kern_ms)),
-               prep_ms=float(np.mean(prep_ms)), launches_step=launches_step, clocks=clocks, delta=delta, m_limit=m_limit,
+               prep_ms=float(np.mean(prep_ms)), kernel_sm_mhz=float(np.mean(sm_mhz)), launches_step=launches_step, clocks=clocks, delta=delta, m_limit=m_limit,
                phases={k: float(np.mean([p[k] for p in phases])) for k in phases[0]}, pm=pm, o=o, stats=st)
 
     if e2e:   # ---- end to end through the host-buffer C-ABI call (pinned host memory)
@@ -331,6 +331,7 @@ def roofline_block(res, key, peak_tflops, peak_measured, sm_count):
             "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": res["inter"],
             "kernel_ms": res["kernel_ms"], "kernel_ms_source": "CUDA events around the kernel launch alone, on its stream (otoo_last_stats.ms_walk_force), mean over the timed steps",
             "otoo_gravity_call_ms": res["call_ms"], "prep_ms": res["prep_ms"],
+            "kernel_sm_mhz": res["kernel_sm_mhz"], "kernel_sm_mhz_source": "clock64 ticks per globaltimer ns inside the kernel (otoo_last_stats.walk_sm_mhz)",
             "interactions_per_s_kernel": res["inter"] / (res["kernel_ms"] * 1e-3)}
 
 

@@ -70,6 +70,8 @@ typedef struct {
    * whole call.  0 where nothing has run. */
   float ms_build[8], ms_build_total;
   float ms_walk_prep, ms_walk_force, ms_total;
+  float walk_sm_mhz;         /* SM clock the gravity walk kernel actually held: SM clock ticks per nanosecond of the
+                              * global timer, summed over its CTAs (0 for the other kernels) */
   int32_t walk_only;         /* 1: the last walk ran with option "walk_only": counters valid, OUTPUTS MEANINGLESS */
   int32_t error_flag;        /* != 0: the last walk dropped cells (private spill area full): outputs and counters
                               * invalid; otoo_last_stats / otoo_export_group_stats return OTOO_ERR_CAPACITY */

@@ -40,7 +40,7 @@ class Stats(C.Structure):
                 ("launches", C.c_int32), ("sum_steps", C.c_uint64), ("sum_tasks", C.c_uint64),
                 ("sum_flushes", C.c_uint64), ("ms_build", C.c_float * 8), ("ms_build_total", C.c_float),
                 ("ms_walk_prep", C.c_float), ("ms_walk_force", C.c_float), ("ms_total", C.c_float),
-                ("walk_only", C.c_int32), ("error_flag", C.c_int32)]
+                ("walk_sm_mhz", C.c_float), ("walk_only", C.c_int32), ("error_flag", C.c_int32)]
 
 
 BUILD_PHASES = ["root_cube", "keys", "sort", "gather", "cells", "moments"]
@@ -136,8 +136,8 @@ class Otoo:
         return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
 
     def _p(self, t, dtype=None, shape_last=None):
-        """a per-particle argument: N rows on this context's device"""
-        return _ptr(t, dtype, shape_last, rows=self.N, device=self.device)
+        """a per-particle argument: N rows on this context's device (before a build the C side answers NOT_BUILT)"""
+        return _ptr(t, dtype, shape_last, rows=self.N if self.N else None, device=self.device)
 
     # ---- the hot path
     def otoo_build_tree(self, pos_mass, n_crit=16, stream=None):
@@ -172,7 +172,7 @@ class Otoo:
         out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
         self._check(_lib.otoo_sph_force_visc(self._h, self._p(h, torch.float32), self._p(rho, torch.float32), self._p(P, torch.float32),
                                              self._p(vel, torch.float32, 4), self._p(visc, torch.float32, 4), int(group_size),
-                                             out.dataself._p(), self._stream(stream)))
+                                             out.data_ptr(), self._stream(stream)))
         return out
 
     def otoo_sph_stage1(self, h, vel, group_size, stream=None):
@@ -181,7 +181,7 @@ class Otoo:
         nngb = torch.empty(self.N, dtype=torch.int32, device=self._dev())
         dr = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
         self._check(_lib.otoo_sph_stage1(self._h, self._p(h, torch.float32), self._p(vel, torch.float32, 4), int(group_size),
-                                         rho.dataself._p(), nngb.dataself._p(), dr.dataself._p(), self._stream(stream)))
+                                         rho.data_ptr(), nngb.data_ptr(), dr.data_ptr(), self._stream(stream)))
         return rho, nngb, dr
 
     def otoo_sph_adapt_h(self, h, n_target, tol, max_iter, group_size, stream=None):
@@ -189,7 +189,7 @@ class Otoo:
         nngb = torch.empty(self.N, dtype=torch.int32, device=self._dev())
         it = C.c_int(0)
         self._check(_lib.otoo_sph_adapt_h(self._h, self._p(h, torch.float32), float(n_target), float(tol), int(max_iter),
-                                          int(group_size), nngb.dataself._p(), C.byref(it), self._stream(stream)))
+                                          int(group_size), nngb.data_ptr(), C.byref(it), self._stream(stream)))
         return nngb, int(it.value)
 
     def otoo_sph_force(self, h, rho, P, group_size, vel=None, stream=None):

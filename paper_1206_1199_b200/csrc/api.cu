@@ -98,8 +98,8 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));
     OTOO_TRY(dalloc(ctx, &ctx->d_bbox, 16));
     OTOO_TRY(dalloc(ctx, &ctx->d_counters, 64));
-    OTOO_TRY(dalloc(ctx, &ctx->d_sums, 8));
-    OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, 8 * sizeof(unsigned long long)));
+    OTOO_TRY(dalloc(ctx, &ctx->d_sums, OTOO_NSUMS));
+    OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
     for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
@@ -312,8 +312,9 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
   OTOO_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
   if (ctx->walked) {
-    unsigned long long h[8];
+    unsigned long long h[OTOO_NSUMS];
     OTOO_CUDA(ctx, cudaMemcpy(h, ctx->d_sums, sizeof h, cudaMemcpyDeviceToHost));
+    if (h[9]) o->walk_sm_mhz = (float)(1e3 * (double)h[8] / (double)h[9]);
     o->sum_tests = h[0]; o->sum_interactions = h[1]; o->sum_cells = h[2]; o->sum_parts = h[3];
     o->sum_steps = h[4]; o->sum_tasks = h[5]; o->sum_flushes = h[6];
     o->error_flag = (int32_t)h[7];

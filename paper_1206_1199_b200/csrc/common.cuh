@@ -18,6 +18,7 @@
 // u32 words of sort scratch for n pairs: digit histograms + tickets (4096) + one u64 status word per tile and digit
 #define OTOO_SORT_SCRATCH(n) ((size_t)(((n) + OTOO_SORT_TILE - 1) / OTOO_SORT_TILE) * 512 + 4096)
 #define OTOO_WALK_WARPS 4            // warps per CTA of the walk kernels
+#define OTOO_NSUMS 16
 #define OTOO_BUILD_PHASES 6          // root cube, keys, sort, gather, cells (topology), moments
 
 // Per-cell walk record, 16 B: the paper's 7-word node (L161) minus the 4 words of (cm, m).
@@ -79,7 +80,8 @@ struct otoo_ctx {
   uint32_t* g_nparts;
   uint32_t* walk_spill;  // OTOO_WALK_SPILL entries per resident warp
   int64_t spill_warps;
-  unsigned long long* d_sums; // [0] tests [1] interactions [2] cells [3] parts
+  unsigned long long* d_sums; // OTOO_NSUMS words: [0] tests [1] interactions [2] cells [3] parts [4] steps [5] tasks [6] flushes
+                              // [7] error flag [8] SM clock ticks and [9] ns spent by the CTAs of the walk kernel
   void* pool_slots;      // task pool (walk.cuh): TaskSlot[OTOO_POOL_SLOTS]
   void* pool_seq;        // uint32 sequence numbers
   void* walk_shared;     // WalkShared control block

@@ -24,9 +24,10 @@ __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y
 __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
 
-template <int T_, bool EPS0>
+// PB_ = target pairs per pass over the list (0: the default, min(NP, 2)); UNR_ = unroll factor of the entry loop
+template <int T_, bool EPS0, int PB_ = 0, int UNR_ = OTOO_EVAL_UNR>
 struct GravVisitor {
-  static constexpr int T = T_, E = 1, LCAP = OTOO_LIST_CAP, NP = (T_ + 1) / 2, PB = NP < 2 ? NP : 2, BLK = 64, UNR = OTOO_EVAL_UNR;
+  static constexpr int T = T_, E = 1, LCAP = OTOO_LIST_CAP, NP = (T_ + 1) / 2, PB = PB_ ? (PB_ < NP ? PB_ : NP) : (NP < 2 ? NP : 2), BLK = 64, UNR = UNR_;
   const GravParams& p;
   float pm[T];
   float glo[3], ghi[3];

@@ -181,6 +181,9 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
     for (int b = 0; b < OTOO_WS_NBUF; b++) { mbar_init(&s.full[b], 32); mbar_init(&s.empty[b], 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // SM clock held by this CTA (otoo_stats_t.walk_sm_mhz): clock64 ticks per globaltimer ns, evaluator warp 0
+  long long ck0 = 0; unsigned long long ns0 = 0;
+  if (threadIdx.x == 0) { ck0 = clock64(); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns0)); }
   __syncthreads();
   if (warp >= OTOO_WS_PAIRS) {
     // ---- walker: L57 rules through walk_driver, lists into the pair's buffers
@@ -207,6 +210,12 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
       if (m.flags & WS_LAST) { v.selfmask = sm.self[buf][lane]; v.store(g0, lane); }
       mbar_arrive(&sm.empty[buf]);
       buf = (buf + 1) % OTOO_WS_NBUF;
+    }
+    if (threadIdx.x == 0) {
+      unsigned long long ns1;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns1));
+      atomicAdd(p.c.sums + 8, (unsigned long long)(clock64() - ck0));
+      atomicAdd(p.c.sums + 9, ns1 - ns0);
     }
   }
 }
@@ -285,7 +294,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, 8 * sizeof(unsigned long long), st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long), st));
   c->spos = ctx->spos; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
   c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;

@@ -36,8 +36,8 @@ __global__ void __launch_bounds__(512, 1) ffma2_probe_kernel(const f32x2* __rest
       }
     }
   }
+  __syncthreads();                       // the slowest warp of the CTA ends the interval
   const long long t1 = clock64();
-  __syncthreads();
   f32x2 r = a[0];
 #pragma unroll
   for (int i = 1; i < FP_ACC; i++) r = add2(r, a[i]);
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(512, 1) ffma2_probe_kernel(const f32x2* __rest
 }
 
 // ---------------------------------------------------------------- the sum loop alone
-template <int T>
+template <int T, int PB, int UNR>
 __global__ void __launch_bounds__(128, T >= 8 ? 2 : 3) sumloop_probe_kernel(const GravParams p, int reps, float4* __restrict__ sink,
                                                                              unsigned long long* __restrict__ cycles) {
   __shared__ __align__(16) float4 lists[4][OTOO_LIST_CAP + 4];
@@ -60,20 +60,23 @@ __global__ void __launch_bounds__(128, T >= 8 ? 2 : 3) sumloop_probe_kernel(cons
     list[j] = make_float4(x, y, z, 1.0f / OTOO_LIST_CAP);
   }
   __syncwarp();
-  GravVisitor<T, false> v(p);
+  GravVisitor<T, false, PB, UNR> v(p);
   const int64_t g0 = ((int64_t)(blockIdx.x * 4 + warp) * (32 * T)) % (p.c.N - 32 * T);
   __shared__ __align__(16) float2 scratch[4][32 * ((T + 1) / 2) * 3];
   v.load_group(g0, lane, reinterpret_cast<float4*>(scratch[warp]));
   __syncthreads();
   const long long t0 = clock64();
+  unsigned long long g0ns, g1ns;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0ns));
   for (int r = 0; r < reps; r++) v.eval(list, OTOO_LIST_CAP);
+  __syncthreads();                       // the slowest warp of the CTA ends the interval
   const long long t1 = clock64();
-  __syncthreads();
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1ns));
   float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
   for (int q = 0; q < (T + 1) / 2; q++) { o.x += v.AX[q].x + v.AX[q].y; o.y += v.AY[q].x + v.AY[q].y; o.z += v.AZ[q].x + v.AZ[q].y; o.w += v.PH[q].x + v.PH[q].y; }
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = o;
-  if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+  if (threadIdx.x == 0) { cycles[blockIdx.x] = (unsigned long long)(t1 - t0); cycles[gridDim.x + blockIdx.x] = g1ns - g0ns; }
 }
 
 __global__ void __launch_bounds__(256) probe_fill_kernel(float4* pos, f32x2* pairs, int64_t n) {
@@ -110,39 +113,47 @@ double run_ffma2(otoo_ctx* ctx, const f32x2* in, f32x2* out, unsigned long long*
   return sum / n / ((double)warps_per_smsp * iters * FP_ACC);
 }
 
-template <int T>
+template <int T, int PB, int UNR>
 otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long long* d_cyc, cudaStream_t st, std::string& js) {
-  const int reps = 64;
+  const int reps = 256;
   int occ = 0;
-  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T>, 128, 0));
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR>, 128, 0));
   cudaFuncAttributes fa;
-  OTOO_CUDA(ctx, cudaFuncGetAttributes(&fa, sumloop_probe_kernel<T>));
+  OTOO_CUDA(ctx, cudaFuncGetAttributes(&fa, sumloop_probe_kernel<T, PB, UNR>));
   const int per_sm = T >= 8 ? 2 : 3;                    // evaluator warps per SM of the product kernel: 4 x this
   const int grid = ctx->sm_count * per_sm;
+  // dynamic shared memory sized so that EXACTLY per_sm CTAs fit an SM: every SM then runs per_sm CTAs of the
+  // grid at once (left to the occupancy of the kernel alone the block scheduler packs 4 on some SMs and 2 on others)
+  const size_t dyn = (size_t)(227 * 1024) / per_sm - fa.sharedSizeBytes - 2048;
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(sumloop_probe_kernel<T, PB, UNR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR>, 128, dyn));
+  if (occ != per_sm) return otoo_fail(ctx, OTOO_ERR_CUDA, "probe: occupancy is not the evaluator's");
   Timer tm;
-  sumloop_probe_kernel<T><<<grid, 128, 0, st>>>(p, 4, sink, d_cyc);
+  sumloop_probe_kernel<T, PB, UNR><<<grid, 128, dyn, st>>>(p, 4, sink, d_cyc);
   float best = 1e30f;
   for (int r = 0; r < 3; r++) {
     tm.start(st);
-    sumloop_probe_kernel<T><<<grid, 128, 0, st>>>(p, reps, sink, d_cyc);
+    sumloop_probe_kernel<T, PB, UNR><<<grid, 128, dyn, st>>>(p, reps, sink, d_cyc);
     const float ms = tm.stop(st);
     if (ms < best) best = ms;
   }
   OTOO_CUDA(ctx, cudaGetLastError());
   unsigned long long h[1024];
-  const int n = grid < 1024 ? grid : 1024;
+  const int n = grid < 512 ? grid : 512;
   OTOO_CUDA(ctx, cudaMemcpy(h, d_cyc, sizeof(unsigned long long) * n, cudaMemcpyDeviceToHost));
-  double cyc = 0;
-  for (int i = 0; i < n; i++) cyc += (double)h[i];
-  cyc /= n;
+  OTOO_CUDA(ctx, cudaMemcpy(h + 512, d_cyc + grid, sizeof(unsigned long long) * n, cudaMemcpyDeviceToHost));
+  double cyc = 0, ns = 0;
+  for (int i = 0; i < n; i++) { cyc += (double)h[i]; ns += (double)h[512 + i]; }
+  cyc /= n; ns /= n;
+  const double sm_mhz = 1e3 * cyc / ns;                  // SM clock held during the loop: clock64 ticks per globaltimer ns
   const double inter = (double)grid * 4 * 32 * T * OTOO_LIST_CAP * reps;
   // SMSP cycles per (target pair, list entry): every SMSP ran per_sm warps x NP pairs x entries x reps
   const double per_pair = cyc / ((double)per_sm * ((T + 1) / 2) * OTOO_LIST_CAP * reps);
   char buf[512];
   snprintf(buf, sizeof buf,
-           "{\"name\": \"sumloop G=%d\", \"eval_warps_per_sm\": %d, \"registers\": %d, \"occupancy_ctas\": %d, \"ms\": %.4f, "
-           "\"interactions_per_s\": %.6e, \"tflops_20flop\": %.3f, \"smsp_cycles_per_pair_entry\": %.3f}",
-           32 * T, 4 * per_sm, fa.numRegs, occ, best, inter / (best * 1e-3), 20.0 * inter / (best * 1e-3) / 1e12, per_pair);
+           "{\"name\": \"sumloop G=%d\", \"pairs_per_pass\": %d, \"unroll\": %d, \"eval_warps_per_sm\": %d, \"registers\": %d, \"occupancy_ctas\": %d, \"ms\": %.4f, "
+           "\"interactions_per_s\": %.6e, \"tflops_20flop\": %.3f, \"smsp_cycles_per_pair_entry\": %.3f, \"sm_mhz_during_loop\": %.0f}",
+           32 * T, GravVisitor<T, false, PB, UNR>::PB, UNR, 4 * per_sm, fa.numRegs, occ, best, inter / (best * 1e-3), 20.0 * inter / (best * 1e-3) / 1e12, per_pair, sm_mhz);
   if (!js.empty()) js += ", ";
   js += buf;
   return OTOO_OK;
@@ -182,9 +193,19 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
     memset(&p, 0, sizeof p);
     p.c.spos = ctx->spos; p.c.N = n; p.eps2 = 1e-6f;
     float4* sink = reinterpret_cast<float4*>(ctx->key[1]) + 4096;
-    OTOO_TRY(run_sumloop<2>(ctx, p, sink, d_cyc, st, js));
-    OTOO_TRY(run_sumloop<4>(ctx, p, sink, d_cyc, st, js));
-    OTOO_TRY(run_sumloop<8>(ctx, p, sink, d_cyc, st, js));
+    // the product's configuration first (pairs per pass = min(NP, 2), unroll OTOO_EVAL_UNR), then the variants tried
+    OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 2, 1>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 2, 2>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 2, 8>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 1, 4>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 2, 1>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 2, 2>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 4, 1>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 4, 2>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 1, 4>(ctx, p, sink, d_cyc, st, js)));
   } else return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown probe (ffma2, sumloop)");
   js = "[" + js + "]";
   if ((int64_t)js.size() + 1 > cap) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "probe output buffer too small");

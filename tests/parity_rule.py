@@ -8,8 +8,8 @@ magnitudes over the same list -- pinned against numpy brute force in tests/test_
 Reported (printed, and appended to gpurun_out/parity_report.jsonl when that directory exists): the un-floored
 maximum, p99.9 and median of |dx_i|/|x_i|; the maximum of |dx_i| over its bound; the fraction of particles whose
 bound is the 8 u A_i floor (A_i/|x_i| > 1e-5/(8u) = 21); and the same error under SURVEY's own floor,
-|dx_i| / max(|x_i|, 1e-2 x_rms).  `floor_frac_max` bounds the floor fraction: a test states how many particles
-it lets live on the floor."""
+|dx_i| / max(|x_i|, 1e-2 x_rms).  `floor_frac_max` bounds the floor fraction and `above_tol_frac_max` the fraction
+of particles whose plain relative error exceeds 1e-5: a test states how many particles it lets live on the floor."""
 import json
 import os
 
@@ -18,6 +18,12 @@ import numpy as np
 TOL = 1e-5
 U32 = 2.0 ** -24
 FLOOR_RATIO = TOL / (8 * U32)        # A_i / |x_i| above which the floor is the bound (= 20.97)
+# Measured on the B200 (profiles/r2_parity_audit.md): gravity has <= 0.4 % of the particles on the floor in every
+# test (0.00 % at C5), the SPH pressure force <= 2.2 %, and <= 2 particles per test exceed plain 1e-5.  The tests
+# assert these with a margin; a regression of the arithmetic shows up here before it reaches the bound.
+FLOOR_FRAC_MAX_GRAVITY = 0.01
+FLOOR_FRAC_MAX_SPH = 0.04
+ABOVE_TOL_FRAC_MAX = 5e-4            # fraction of particles whose plain relative error may exceed 1e-5 (they are held by 8 u A)
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -26,7 +32,7 @@ def _norm(a):
     return np.abs(a) if a.ndim == 1 else np.linalg.norm(a, axis=1)
 
 
-def report(label, got, want, abs_sum, pct=99.9, floor_frac_max=1.0, check=True):
+def report(label, got, want, abs_sum, pct=99.9, floor_frac_max=FLOOR_FRAC_MAX_SPH, above_tol_frac_max=ABOVE_TOL_FRAC_MAX, check=True):
     """got, want: (n,) or (n,k) arrays; abs_sum: (n,).  Returns the statistics; asserts the rule if check."""
     got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
     d = _norm(got - want)
@@ -57,6 +63,7 @@ def report(label, got, want, abs_sum, pct=99.9, floor_frac_max=1.0, check=True):
         if pct is not None:      # None: sums that cancel for most particles (div v, du/dt) are held by the bound alone
             assert float(np.percentile(rel, pct)) <= TOL, st
         assert st["floor_frac"] <= floor_frac_max, st
+        assert st["n_above_tol"] <= max(2, above_tol_frac_max * st["n"]), st
     return st
 
 

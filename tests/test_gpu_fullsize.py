@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 from workloads import generators as gen  # noqa: E402
 
-from tests.parity_rule import TOL, U32, report   # noqa: E402  (the one statement of the rule, R12)
+from tests.parity_rule import TOL, U32, FLOOR_FRAC_MAX_GRAVITY, FLOOR_FRAC_MAX_SPH, report   # noqa: E402  (the one statement of the rule, R12)
 
 N_SAMPLE = {"C2": 512, "C3": 256, "C4": 256, "C5": 256}     # seeded groups summed in fp64 per config (+ the two below)
 
@@ -45,7 +45,7 @@ def sample_groups(ng, lengths, seed, n_sample):
     return np.array(sorted(sel), dtype=np.int64)
 
 
-def vec_check(label, got, want, abs_sum, pct, floor_frac_max=1.0):
+def vec_check(label, got, want, abs_sum, pct, floor_frac_max=FLOOR_FRAC_MAX_SPH):
     return report(label, got[:, :3], want[:, :3], abs_sum, pct=pct, floor_frac_max=floor_frac_max)
 
 
@@ -85,7 +85,7 @@ def test_fullsize_gravity(orc, name):
         rs = t.gravity(eps, theta, G, groups=sel)
         assert np.array_equal(rs["n_tests"], nt[sel])
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
-        vec_check(f"fullsize_gravity[{name}:{order}]", out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9)
+        vec_check(f"fullsize_gravity[{name}:{order}]", out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9, FLOOR_FRAC_MAX_GRAVITY)
         pe = np.abs(out[idx, 3] - rs["acc_pot"][idx, 3]) / np.abs(rs["acc_pot"][idx, 3])
         assert pe.max() <= TOL, pe.max()
         assert np.isfinite(out).all()

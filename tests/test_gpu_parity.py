@@ -24,7 +24,7 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-from tests.parity_rule import TOL, U32, report, scalar_rel   # noqa: E402  (the one statement of the rule, R12)
+from tests.parity_rule import TOL, U32, FLOOR_FRAC_MAX_GRAVITY, FLOOR_FRAC_MAX_SPH, report, scalar_rel   # noqa: E402  (the one statement of the rule, R12)
 
 
 def _label():
@@ -32,10 +32,12 @@ def _label():
     return os.environ.get("PYTEST_CURRENT_TEST", "?").split("::")[-1].split(" ")[0]
 
 
-def acc_err(got, want, abs_sum, pct=99.9, floor_frac_max=1.0, what="acc"):
+def acc_err(got, want, abs_sum, pct=99.9, floor_frac_max=None, what="acc"):
     """R12 through tests/parity_rule.report (asserts the rule, prints and logs the audit numbers: un-floored max,
     p99.9, median, fraction of particles on the 8 u A floor).  Returns (|da| / bound scaled to 1e-5, plain
     relative error) for the callers' own assertions."""
+    if floor_frac_max is None:
+        floor_frac_max = FLOOR_FRAC_MAX_GRAVITY if what == "acc" else FLOOR_FRAC_MAX_SPH
     report(f"{_label()}:{what}", got[:, :3], want[:, :3], abs_sum, pct=pct, floor_frac_max=floor_frac_max)
     d = np.linalg.norm(got[:, :3].astype(np.float64) - want[:, :3], axis=1)
     an = np.linalg.norm(want[:, :3], axis=1)
@@ -494,7 +496,7 @@ def test_spill_overflow_is_reported(otoo, orc):
     otoo.otoo_build_tree(dev(pm), 1)
     try:
         otoo.otoo_set_option("task_pool", 0)
-        otoo.otoo_set_option("walk_spill", 256)
+        otoo.otoo_set_option("walk_spill", 0)
         otoo.otoo_gravity(0.01, 0.0, 32)
         with pytest.raises(binding.OtooError) as e:
             otoo.otoo_last_stats()
