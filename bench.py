@@ -355,9 +355,9 @@ def main():
                     help="delta: the paper's absolute-error MAC (otoo_gravity_delta) instead of BASELINE's theta criterion")
     ap.add_argument("--key-order", default="morton", choices=["morton", "hilbert"],
                     help="hilbert: the paper's ordering (L131) instead of BASELINE's Morton-contiguous groups")
-    ap.add_argument("--group-distance", default="box", choices=["box", "exact", "split"],
-                    help="exact: the paper's minimum over the members' distances (L163); split: minimum over the boxes of the "
-                         "group's pieces between its coarsest key boundaries; box: one bounding box per group")
+    ap.add_argument("--group-distance", default="split", choices=["box", "exact", "split"],
+                    help="split (default, R25): minimum over the boxes of the group's pieces between its coarsest key boundaries; "
+                         "box: one bounding box per group (R8); exact: the paper's minimum over the members' distances (L163)")
     ap.add_argument("--delta", type=float, default=None)
     ap.add_argument("--m-limit", type=float, default=None)
     ap.add_argument("--seed", type=int, default=1206)
@@ -400,7 +400,7 @@ def main():
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tflops = sm_count * SM_LANES * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
     cfg, n = res["cfg"], res["n"]
-    custom = args.theta is not None or args.n is not None or args.mac != "theta" or args.key_order != "morton" or args.group_distance != "box"
+    custom = args.theta is not None or args.n is not None or args.mac != "theta" or args.key_order != "morton" or args.group_distance != "split"
     key = args.workload if not custom else f"{args.workload}:custom"
     mac_txt = f"theta={cfg['theta']}" if args.mac == "theta" else f"Delta-MAC delta={res['delta']:g} m_limit={res['m_limit']:g}"
     line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,

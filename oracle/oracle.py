@@ -94,6 +94,7 @@ def lib():
         L.orc_dWdr.restype = dbl
         L.orc_dWdr.argtypes = [dbl, dbl]
         L.orc_set_dist_kind.argtypes = [vp, i32]
+        L.orc_set_split_pieces.argtypes = [vp, i32]
         L.orc_max_threads.restype = i32
         L.orc_set_threads.argtypes = [i32]
     return _lib
@@ -201,6 +202,9 @@ class Tree:
     def set_dist_kind(self, kind):
         """0: group AABB distance (R8); 1: exact minimum over the group's members (R23)"""
         lib().orc_set_dist_kind(self._h, int(kind))
+
+    def set_split_pieces(self, K):
+        lib().orc_set_split_pieces(self._h, int(K))
 
     def delta_cell_props(self):
         """(B2, b_max) per cell in fp64: PAPER.md Eq. 2 (bottom-up, reading R19) and L63."""

@@ -16,7 +16,9 @@ struct orc_tree {
   int64_t N;
   int n_crit;
   int key_order;  /* 0 Morton (R3), 1 Hilbert (R20) */
-  int dist_kind;  /* 0 group AABB distance (R8), 1 the paper's exact minimum over the members (L163; R23) */
+  int dist_kind;  /* 0 group AABB distance (R8), 1 the paper's exact minimum over the members (L163; R23),
+                     2 minimum over the AABBs of the group's pieces between its coarsest key boundaries (R25) */
+  int split_pieces; /* dist_kind 2: number of pieces K (8) */
   float lo[3], S;
   uint64_t* key;  /* sorted keys */
   uint32_t* perm; /* perm[s] = original index of sorted slot s */
@@ -212,6 +214,7 @@ orc_tree* orc_build(int64_t N, const float* pos_mass, int n_crit) { return orc_b
 orc_tree* orc_build_ord(int64_t N, const float* pos_mass, int n_crit, int key_order) {
   orc_tree* t = (orc_tree*)calloc(1, sizeof(orc_tree));
   t->N = N; t->n_crit = n_crit; t->key_order = key_order;
+  t->dist_kind = 2; t->split_pieces = 8;   /* R25 is the default group-cell distance of the gravity walks */
   /* R1 / L121,L127: cube enclosing all particles, anchored at the lo corner */
   float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
   for (int64_t i = 0; i < N; i++)
@@ -412,10 +415,53 @@ void orc_rb2_delta(const orc_tree* t, double delta, double m_limit, float* rb2) 
 }
 
 /* ---------------- R8: group AABB and group-cell distance (L163, Barnes 1990 form) ----------- */
-typedef struct { float lo[3], hi[3]; float hmax; const float* mem; int nmem; } gbox_t;   /* mem: the members' (x,y,z,m), set for dist_kind 1 */
+#define MAXPIECES 16
+typedef struct {
+  float lo[3], hi[3]; float hmax; const float* mem; int nmem;   /* mem: the members' (x,y,z,m), set for dist_kind 1 */
+  int npiece; float plo[MAXPIECES][3], phi[MAXPIECES][3];       /* dist_kind 2: tight boxes of the pieces */
+} gbox_t;
+static int key_cplev(uint64_t a, uint64_t b) {   /* number of leading octree levels two keys share, 0..21 */
+  int l = 0;
+  while (l < MAXLEV && ((a >> (3 * (MAXLEV - 1 - l))) & 7u) == ((b >> (3 * (MAXLEV - 1 - l))) & 7u)) l++;
+  return l;
+}
+/* Reading R25: the group [a, b) is cut at its K-1 coarsest key boundaries -- the slots s in (a, b) with
+ * the smallest number of octree levels shared by key[s-1] and key[s] (ties: the lowest slot first).  A Morton
+ * range that crosses the boundary of a coarse cell jumps across that cell (the curve is not continuous), so the
+ * bounding box of the whole group can be as large as the cell while each piece between two such boundaries is
+ * compact.  The group-cell distance is the minimum over the pieces of the box distance of R8. */
+static void split_pieces(const orc_tree* t, int64_t a, int64_t b, int K, gbox_t* g) {
+  int64_t cut[MAXPIECES]; int ncut = 0;
+  int n = (int)(b - a);
+  if (K > MAXPIECES) K = MAXPIECES;
+  unsigned char* taken = (unsigned char*)calloc(n > 0 ? n : 1, 1);
+  for (int k = 0; k < K - 1 && k < n - 1; k++) {          /* the k-th coarsest boundary */
+    int best = -1, bl = MAXLEV + 1;
+    for (int i = 1; i < n; i++) {
+      if (taken[i]) continue;
+      int l = key_cplev(t->key[a + i - 1], t->key[a + i]);
+      if (l < bl) { bl = l; best = i; }                   /* strict: ties keep the lowest slot */
+    }
+    taken[best] = 1;
+  }
+  for (int i = 1; i < n; i++) if (taken[i]) cut[ncut++] = a + i;   /* in slot order */
+  free(taken);
+  g->npiece = ncut + 1;
+  for (int p = 0; p <= ncut; p++) {
+    int64_t s0 = p == 0 ? a : cut[p - 1], s1 = p == ncut ? b : cut[p];
+    for (int k = 0; k < 3; k++) { g->plo[p][k] = t->spos[4 * s0 + k]; g->phi[p][k] = g->plo[p][k]; }
+    for (int64_t s = s0; s < s1; s++)
+      for (int k = 0; k < 3; k++) {
+        float v = t->spos[4 * s + k];
+        if (v < g->plo[p][k]) g->plo[p][k] = v;
+        if (v > g->phi[p][k]) g->phi[p][k] = v;
+      }
+  }
+}
 static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs /*sorted h or NULL*/) {
-  gbox_t g; g.hmax = 0.0f;
+  gbox_t g; g.hmax = 0.0f; g.npiece = 0;
   g.mem = (t->dist_kind == 1 && !hs) ? t->spos + 4 * a : NULL; g.nmem = (int)(b - a);   /* SPH walks (hs given): AABB only */
+  if (t->dist_kind == 2 && !hs) split_pieces(t, a, b, t->split_pieces, &g);
   for (int k = 0; k < 3; k++) { g.lo[k] = t->spos[4 * a + k]; g.hi[k] = g.lo[k]; }
   for (int64_t s = a; s < b; s++) {
     for (int k = 0; k < 3; k++) {
@@ -435,6 +481,20 @@ static float box_d2(const gbox_t* g, const float* cm) {
     for (int i = 0; i < g->nmem; i++) {
       float dx = g->mem[4 * i] - cm[0], dy = g->mem[4 * i + 1] - cm[1], dz = g->mem[4 * i + 2] - cm[2];
       float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+      if (d2 < best) best = d2;
+    }
+    return best;
+  }
+  if (g->npiece > 0) {   /* R25: minimum over the pieces' boxes of the R8 expression (the minimum of fp32 values is exact) */
+    float best = INFINITY;
+    for (int p = 0; p < g->npiece; p++) {
+      float e[3];
+      for (int k = 0; k < 3; k++) {
+        float a = g->plo[p][k] - cm[k], b = cm[k] - g->phi[p][k];
+        float m = a > b ? a : b;
+        e[k] = m > 0.0f ? m : 0.0f;
+      }
+      float d2 = fmaf(e[2], e[2], fmaf(e[1], e[1], e[0] * e[0]));
       if (d2 < best) best = d2;
     }
     return best;
@@ -907,6 +967,7 @@ uint64_t orc_sph_force(const orc_tree* t, const float* h, const double* rho, con
 }
 
 void orc_set_dist_kind(orc_tree* t, int kind) { t->dist_kind = kind; }
+void orc_set_split_pieces(orc_tree* t, int K) { t->split_pieces = K; }
 int orc_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -130,6 +130,7 @@ double orc_dWdr(double r, double h);
 /* group-cell distance of the gravity walks: 0 = from the group's AABB (R8, default), 1 = the paper's exact
  * minimum over the group's members (R23).  SPH walks always use the AABB. */
 void orc_set_dist_kind(orc_tree*, int kind);
+void orc_set_split_pieces(orc_tree*, int K);   /* dist_kind 2: pieces per group (8 = the reading R25; other values for the study in DESIGN.md only) */
 int orc_max_threads(void);
 void orc_set_threads(int n);
 #ifdef __cplusplus

@@ -81,7 +81,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
   otoo_ctx* ctx = new (std::nothrow) otoo_ctx;
   if (!ctx) return OTOO_ERR_OOM;
   memset(ctx, 0, sizeof *ctx);
-  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->walk_spill_cap = OTOO_WALK_SPILL; ctx->use_pool = 1; ctx->use_ws = 1; ctx->group_begin = 0; ctx->group_count = -1;
+  ctx->device = device; ctx->maxN = max_particles; ctx->walk_stack = OTOO_WALK_STACK_MAX; ctx->walk_spill_cap = OTOO_WALK_SPILL; ctx->use_pool = 1; ctx->use_ws = 1; ctx->dist_kind = 2; ctx->group_begin = 0; ctx->group_count = -1;
   otoo_status s = OTOO_OK;
   auto body = [&]() -> otoo_status {
     OTOO_CUDA(ctx, cudaSetDevice(device));
@@ -371,7 +371,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
   }
   if (strcmp(name, "group_count") == 0) { ctx->group_count = value < 0 ? -1 : value; return OTOO_OK; }
   if (strcmp(name, "group_distance") == 0) {
-    if (value != 0 && value != 1) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance must be 0 (AABB) or 1 (exact minimum)");
+    if (value < 0 || value > 2) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance must be 0 (one box), 1 (exact minimum) or 2 (pieces' boxes)");
     ctx->dist_kind = (int)value;
     return OTOO_OK;
   }

@@ -34,7 +34,8 @@ struct GravVisitor {
   f32x2 PX[NP], PY[NP], PZ[NP];                       // two targets per aligned register pair (kept as b64)
   float2 AX[NP], AY[NP], AZ[NP], PH[NP];
   unsigned selfmask;
-  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_) {}
+  float4* pbox;                                        // the pieces' boxes in shared memory (one-warp-does-both kernel, R25)
+  __device__ __forceinline__ GravVisitor(const GravParams& p_) : p(p_), pbox(nullptr) {}
 
   __device__ __forceinline__ void load_group(int64_t g0, int lane, float4* scratch) {
     float px[T], py[T], pz[T];
@@ -73,12 +74,23 @@ struct GravVisitor {
       AX[q] = AY[q] = AZ[q] = PH[q] = make_float2(0.0f, 0.0f);
     }
     selfmask = 0;
+    if (pbox && p.c.dist_kind == 2) {
+      // R25: members through the (idle) list memory, then the pieces' boxes
+      __syncwarp();
+#pragma unroll
+      for (int t = 0; t < T; t++) scratch[t * 32 + lane] = make_float4(px[t], py[t], pz[t], 0.0f);
+      __syncwarp();
+      const int64_t left = p.c.N - g0;
+      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, scratch, pbox);
+    }
   }
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
     A = __ldg(p.c.cell_cm + cell);
     B = __ldg(p.c.cell_b + cell);
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
-    return d2 > __uint_as_float(B.x) ? 1 : 2;   // strict: equality opens (R8)
+    if (d2 > __uint_as_float(B.x)) return 1;    // strict: equality opens (R8)
+    if (p.c.dist_kind != 2) return 2;
+    return pieces_d2(pbox, A.x, A.y, A.z) > __uint_as_float(B.x) ? 1 : 2;   // R25
   }
   struct Entry { float4 a; };
   __device__ __forceinline__ Entry get(uint32_t slot) const { Entry e; e.a = p.c.spos[slot]; return e; }

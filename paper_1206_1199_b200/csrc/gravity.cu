@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(cons
   uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
   GravVisitor<T, EPS0> v(p);
+  v.pbox = reinterpret_cast<float4*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (2 * OTOO_PIECES);
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
 
@@ -105,7 +106,11 @@ struct GravWalker {
     selfmask = 0; first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
     nmem = 32 * T;
     __syncwarp();
-    if (p.c.dist_kind) {
+    if (p.c.dist_kind == 2) {
+      const int64_t left = p.c.N - g0;
+      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, sm.mem, sm.pbox);
+    }
+    if (p.c.dist_kind == 1) {
       // tight boxes of 8 consecutive members (neighbours on the key curve): a box farther than r_b settles its
       // 8 members at once -- in fp32 too: rounding is monotone, so the box distance never exceeds a member's
       for (int b = lane; b < 4 * T; b += 32) {
@@ -128,6 +133,7 @@ struct GravWalker {
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
     if (d2 > rb2) return 1;                      // strict: equality opens (R8); the box distance bounds every member's from below
     if (!p.c.dist_kind) return 2;
+    if (p.c.dist_kind == 2) return pieces_d2(sm.pbox, A.x, A.y, A.z) > rb2 ? 1 : 2;   // R25 (>= the whole box's distance, in fp32 too)
     // PAPER L163 (R23): the actual minimum of the members' distances decides: accept iff every member is
     // farther than r_b.  d_i^2 = fma(dz,dz, fma(dy,dy, dx*dx)), d = fl32(x_i - cm), as the oracle computes it.
     for (int b = 0; b < 4 * T; b++) {
@@ -264,6 +270,7 @@ otoo_status launch_walk(otoo_ctx* ctx, const GravParams& p, bool eps0, int grid,
 size_t otoo_walk_smem_bytes() {
   return (size_t)OTOO_WALK_WARPS * (OTOO_LIST_STRIDE * sizeof(float4) + OTOO_WALK_STACK_MAX * sizeof(uint32_t));
 }
+static size_t grav_fused_smem_bytes() { return otoo_walk_smem_bytes() + (size_t)OTOO_WALK_WARPS * 2 * OTOO_PIECES * sizeof(float4); }
 
 // Common launch preparation of the walk kernels: persistent grid, task pool, zeroed counters.
 otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st) {
@@ -295,7 +302,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long), st));
-  c->spos = ctx->spos; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
+  c->spos = ctx->spos; c->keys = ctx->key[0]; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
   c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
@@ -312,6 +319,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   GravParams p;
   int grid; size_t smem;
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st));
+  smem = grav_fused_smem_bytes();                 // (the one-warp-does-both kernel: + the pieces' boxes)
   if (mac == 0) {
     rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b);
   } else {
@@ -324,7 +332,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);
   const bool eps0 = !(eps > 0.0f);
-  if (ctx->dist_kind && !ctx->use_ws)
+  if (ctx->dist_kind == 1 && !ctx->use_ws)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance = 1 needs warp_specialized = 1");
   p.c.dist_kind = ctx->dist_kind;
   OTOO_EV(ctx, ctx->ev_walk[1], st);

@@ -40,6 +40,84 @@ __device__ __forceinline__ float aabb_d2(const float glo[3], const float ghi[3],
   return __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
 }
 
+// ---- reading R25: the group's pieces between its OTOO_PIECES - 1 coarsest key boundaries, each with its tight box.
+// A Morton range that crosses the boundary of a coarse cell jumps across that cell, so the box of the whole group
+// can be as large as the cell (a few groups list the whole system) while the pieces are compact; the group-cell
+// distance is then the minimum over the pieces' box distances (same fp32 expression as R8 per piece).
+#define OTOO_PIECES 8
+__device__ __forceinline__ int key_cplev(uint64_t a, uint64_t b) {   // leading octree levels two keys share, 0..21
+  const uint64_t x = a ^ b;
+  return x == 0 ? OTOO_MAXLEV : 20 - (63 - __clzll((long long)x)) / 3;
+}
+__device__ __forceinline__ unsigned f2ord_(float f) { const unsigned u = __float_as_uint(f); return (u & 0x80000000u) ? ~u : (u | 0x80000000u); }
+__device__ __forceinline__ float ord2f_(unsigned u) { return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u); }
+// mem: the group's members in shared memory (slot g0 + i at mem[i], i < gcount); pbox[2p], pbox[2p+1] = (lo, hi) of
+// piece p; an unused piece gets (+inf, -inf): its distance is +inf and never the minimum.  Boundary i (between
+// members i-1 and i) has the key v = (shared levels << 16) | i; the OTOO_PIECES - 1 smallest keys are the cuts
+// (ties: the lowest slot), a member's piece is the number of cuts at or before it.
+template <int T>
+__device__ __forceinline__ void group_pieces(const uint64_t* __restrict__ keys, int64_t g0, int gcount, int lane,
+                                             const float4* mem, float4* pbox) {
+  uint32_t v[T];
+#pragma unroll
+  for (int t = 0; t < T; t++) {
+    const int i = t * 32 + lane;
+    v[t] = (i >= 1 && i < gcount) ? (((uint32_t)key_cplev(keys[g0 + i - 1], keys[g0 + i]) << 16) | (uint32_t)i) : 0xFFFFFFFFu;
+  }
+  uint32_t piece[T];
+#pragma unroll
+  for (int t = 0; t < T; t++) piece[t] = 0u;
+#pragma unroll 1
+  for (int k = 0; k < OTOO_PIECES - 1; k++) {
+    uint32_t m = v[0];
+#pragma unroll
+    for (int t = 1; t < T; t++) m = min(m, v[t]);
+    const uint32_t w = __reduce_min_sync(0xFFFFFFFFu, m);
+    if (w == 0xFFFFFFFFu) break;                      // fewer boundaries than cuts
+    const int ci = (int)(w & 0xFFFFu);
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      if (v[t] == w) v[t] = 0xFFFFFFFFu;
+      piece[t] += (t * 32 + lane >= ci) ? 1u : 0u;
+    }
+  }
+#pragma unroll 1
+  for (int p = 0; p < OTOO_PIECES; p++) {
+    unsigned lo[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu}, hi[3] = {0u, 0u, 0u};
+#pragma unroll
+    for (int t = 0; t < T; t++) {
+      const int i = t * 32 + lane;
+      if (i < gcount && piece[t] == (uint32_t)p) {
+        const float4 q = mem[i];
+        lo[0] = min(lo[0], f2ord_(q.x)); hi[0] = max(hi[0], f2ord_(q.x));
+        lo[1] = min(lo[1], f2ord_(q.y)); hi[1] = max(hi[1], f2ord_(q.y));
+        lo[2] = min(lo[2], f2ord_(q.z)); hi[2] = max(hi[2], f2ord_(q.z));
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; k++) { lo[k] = __reduce_min_sync(0xFFFFFFFFu, lo[k]); hi[k] = __reduce_max_sync(0xFFFFFFFFu, hi[k]); }
+    if (lane == 0) {
+      const bool any = lo[0] != 0xFFFFFFFFu || hi[0] != 0u;     // (a member at the ordered value 0xFFFFFFFF is a NaN: not a position)
+      pbox[2 * p] = any ? make_float4(ord2f_(lo[0]), ord2f_(lo[1]), ord2f_(lo[2]), 0.f) : make_float4(INFINITY, INFINITY, INFINITY, 0.f);
+      pbox[2 * p + 1] = any ? make_float4(ord2f_(hi[0]), ord2f_(hi[1]), ord2f_(hi[2]), 0.f) : make_float4(-INFINITY, -INFINITY, -INFINITY, 0.f);
+    }
+  }
+  __syncwarp();
+}
+// minimum over the pieces of the R8 box distance
+__device__ __forceinline__ float pieces_d2(const float4* pbox, float cx, float cy, float cz) {
+  float m = INFINITY;
+#pragma unroll
+  for (int p = 0; p < OTOO_PIECES; p++) {
+    const float4 lo = pbox[2 * p], hi = pbox[2 * p + 1];
+    const float ex = fmaxf(0.0f, fmaxf(__fsub_rn(lo.x, cx), __fsub_rn(cx, hi.x)));
+    const float ey = fmaxf(0.0f, fmaxf(__fsub_rn(lo.y, cy), __fsub_rn(cy, hi.y)));
+    const float ez = fmaxf(0.0f, fmaxf(__fsub_rn(lo.z, cz), __fsub_rn(cz, hi.z)));
+    m = fminf(m, __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex))));
+  }
+  return m;
+}
+
 __device__ __forceinline__ int warp_inclusive_scan(int x, int lane) {
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xFFFFFFFFu, x, o); if (lane >= o) x += y; }
@@ -62,6 +140,7 @@ struct WalkShared {                   // device-global control block, reset befo
 };
 struct WalkCommon {
   const float4* spos; const float4* cell_cm; const cellb_t* cell_b; const uint32_t* perm;
+  const uint64_t* keys;                                         // sorted keys (piece boundaries of R25)
   int64_t N, ngroups;                                           // ngroups: groups of THIS launch, starting at g_begin
   uint32_t g_begin;                                             // (target sharding over devices)
   uint32_t* g_ntests; uint32_t* g_ncells; uint32_t* g_nparts;   // zeroed before the launch
@@ -72,7 +151,8 @@ struct WalkCommon {
   int spill_cap;                                                // usable entries of a warp's private spill area (<= OTOO_WALK_SPILL)
   int use_pool;                                                 // 0: never donate (test hook: private spill only)
   int walk_only;                                                // 1: lists are built and counted but not evaluated (measures the walk)
-  int dist_kind;                                                // gravity: 0 group AABB distance (R8), 1 exact minimum over the members (R23)
+  int dist_kind;                                                // gravity: 0 one box per group (R8), 1 exact minimum over the members (R23),
+                                                                // 2 minimum over the boxes of the group's pieces (R25)
 };
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }

@@ -29,6 +29,7 @@ struct __align__(16) WsPair {
   float4 list[OTOO_WS_NBUF][OTOO_WS_LCAP + 4];   // +4 entries: consecutive buffers start on different banks
   float4 mem[NM];
   float4 sub[(NM + 7) / 8 * 2];                  // tight boxes of 8 consecutive members: (lo.xyz, -), (hi.xyz, -)
+  float4 pbox[2 * OTOO_PIECES];                  // tight boxes of the group's pieces (R25)
   float2 tgt[NT];
   uint32_t stk[OTOO_WALK_STACK_MAX];
   uint32_t self[OTOO_WS_NBUF][32];

@@ -49,11 +49,13 @@ def vec_check(label, got, want, abs_sum, pct, floor_frac_max=FLOOR_FRAC_MAX_SPH)
     return report(label, got[:, :3], want[:, :3], abs_sum, pct=pct, floor_frac_max=floor_frac_max)
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5", "C2:hilbert", "C3:hilbert", "C2:exact", "C3:hilbert+exact"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5", "C2:hilbert", "C3:hilbert", "C2:exact", "C3:hilbert+exact", "C2:box", "C3:box", "C5:box"])
 def test_fullsize_gravity(orc, name):
+    """default: group-cell distance from the boxes of the group's pieces (R25); :box = one box per group (R8: in C3 one
+    group then lists all 8.4 M particles and is summed here too); :exact = minimum over the members (R23)"""
     name, _, order = name.partition(":")
     key_order = 1 if "hilbert" in order else 0
-    dist_kind = 1 if "exact" in order else 0
+    dist_kind = 1 if "exact" in order else (0 if "box" in order else 2)
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from paper_1206_1199_b200 import binding

@@ -91,18 +91,22 @@ def test_tree_degenerate_inputs(otoo, orc):
                                                 ("uniform_cube", 50000, 128, 0.5, 0.001), ("plummer", 3000, 64, 0.0, 0.01),
                                                 ("plummer", 3000, 128, 0.5, 0.0), ("uniform_sphere", 2500, 256, 0.0, 0.0),
                                                 ("plummer", 40, 64, 0.5, 0.01)])
-@pytest.mark.parametrize("ws", [1, 0])
-def test_gravity_parity(otoo, orc, kind, n, G, theta, eps, ws):
-    """ws = 1: walker/evaluator warp pairs (default); ws = 0: the fused one-warp-does-both kernel."""
+@pytest.mark.parametrize("ws,dist", [(1, 2), (0, 2), (1, 0), (0, 0)])
+def test_gravity_parity(otoo, orc, kind, n, G, theta, eps, ws, dist):
+    """ws = 1: walker/evaluator warp pairs (default); ws = 0: the fused one-warp-does-both kernel.
+    dist = 2: group-cell distance from the boxes of the group's pieces (R25, default); 0: from one box (R8)."""
     pm = gen.make(kind, n, 1206)
     t = check_tree(otoo, orc, pm, 16)
     theta32, eps32 = float(np.float32(theta)), float(np.float32(eps))
+    t.set_dist_kind(dist)
     ref = t.gravity(eps32, theta32, G)
     otoo.otoo_set_option("warp_specialized", ws)
+    otoo.otoo_set_option("group_distance", dist)
     try:
         out = otoo.otoo_gravity(eps32, theta32, G).cpu().numpy()
     finally:
         otoo.otoo_set_option("warp_specialized", 1)
+        otoo.otoo_set_option("group_distance", 2)
     assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta32).view(np.uint32))
     nt, nc, npart = otoo.otoo_export_group_stats()
     assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
@@ -183,6 +187,7 @@ def test_exact_min_group_distance_parity(otoo, orc, kind, n, G, theta, key_order
     pm = gen.make(kind, n, 1206)
     t = check_tree(otoo, orc, pm, 16, key_order=key_order)
     theta32 = float(np.float32(theta))
+    t.set_dist_kind(0)
     aabb = t.gravity(0.01, theta32, G, forces=False)
     t.set_dist_kind(1)
     otoo.otoo_set_option("group_distance", 1)
@@ -207,7 +212,7 @@ def test_exact_min_group_distance_parity(otoo, orc, kind, n, G, theta, key_order
             otoo.otoo_gravity(0.01, theta32, G)
     finally:
         otoo.otoo_set_option("warp_specialized", 1)
-        otoo.otoo_set_option("group_distance", 0)
+        otoo.otoo_set_option("group_distance", 2)
 
 
 def test_walk_stack_spill(otoo, orc):

@@ -203,3 +203,89 @@ def test_exact_minimum_group_distance(orc):
     eb = np.linalg.norm(t2.gravity(0.01, float(theta), G)["acc_pot"][:, :3] - d[:, :3], axis=1).mean()
     ee = np.linalg.norm(t.gravity(0.01, float(theta), G)["acc_pot"][:, :3] - d[:, :3], axis=1).mean()
     assert eb <= ee <= 3 * eb
+
+
+def _np_cplev(a, b):
+    """leading octree levels two 63-bit keys share (0..21), by comparing octant digits from the top"""
+    l = 0
+    for lev in range(21):
+        sh = 3 * (20 - lev)
+        if ((int(a) >> sh) & 7) != ((int(b) >> sh) & 7):
+            break
+        l += 1
+    return l
+
+
+def _np_pieces(keys, a, b, K=8):
+    """reading R25 restated: cut [a, b) at its K-1 coarsest key boundaries (fewest shared levels; ties: lowest slot)"""
+    cand = sorted((( _np_cplev(keys[s - 1], keys[s]), s) for s in range(a + 1, b)))[:K - 1]
+    cuts = sorted(s for _, s in cand)
+    edges = [a] + cuts + [b]
+    return [(edges[i], edges[i + 1]) for i in range(len(edges) - 1)]
+
+
+def _np_box_d2(lo, hi, c):
+    """R8 in fp32: e = max(0, lo - c, c - hi); d2 = fma(ez, ez, fma(ey, ey, ex*ex)) (fma emulated in fp64: exact products)"""
+    e = np.maximum(np.float32(0), np.maximum((lo - c).astype(np.float32), (c - hi).astype(np.float32))).astype(np.float64)
+    t = np.float32(e[0] * e[0])
+    t = np.float32(e[1] * e[1] + np.float64(t))
+    return np.float32(e[2] * e[2] + np.float64(t))
+
+
+@pytest.mark.parametrize("kind,G,theta,key_order", [("plummer", 32, 0.7, 0), ("uniform_cube", 64, 0.5, 0), ("hernquist", 128, 0.6, 1)])
+def test_split_box_group_distance(orc, kind, G, theta, key_order):
+    """dist_kind = 2 (reading R25, the default): the group-cell distance is the minimum over the tight boxes of the
+    group's pieces between its 7 coarsest key boundaries.  Pins by brute force with the pieces recomputed here from
+    the exported keys: every accepted cell is farther than r_b from EVERY piece box, every cell whose parent was
+    opened has a parent within r_b of SOME piece, the lists tile the system, they are nested between the exact-minimum
+    lists (R23) and the one-box lists (R8), and theta = 0 is the direct sum."""
+    n, theta = 3000, np.float32(theta)
+    pm = gen.make(kind, n, 23)
+    t = orc.Tree(pm, 8, key_order=key_order)
+    e = t.export()
+    spos = pm[e["perm"]]
+    rb2 = t.rb2(float(theta))
+    t.set_dist_kind(0)
+    box = t.gravity(0.01, float(theta), G, forces=False)
+    t.set_dist_kind(1)
+    exact = t.gravity(0.01, float(theta), G, forces=False)
+    t.set_dist_kind(2)
+    sp = t.gravity(0.01, float(theta), G, forces=False)
+    Lb, Le, Ls = (x["n_cells"].astype(int) + x["n_parts"] for x in (box, exact, sp))
+    assert np.all(Le <= Ls) and np.all(Ls <= Lb) and sp["interactions"] < box["interactions"]
+    cm = e["com_m"][:, :3]
+    first, count, cf, cc = (e["cells"][k].astype(np.int64) for k in ("first", "count", "child_first", "child_count"))
+    parent = np.full(t.ncell, -1)
+    for c in range(t.ncell):
+        parent[cf[c]:cf[c] + cc[c]] = c
+    for g in range(0, t.n_groups(G), 7):
+        a, b = g * G, min((g + 1) * G, n)
+        pieces = _np_pieces(e["keys"], a, b)
+        assert len(pieces) == min(8, b - a) and pieces[0][0] == a and pieces[-1][1] == b
+        boxes = [(spos[s0:s1, :3].min(0), spos[s0:s1, :3].max(0)) for s0, s1 in pieces]
+        d2 = lambda c: min(_np_box_d2(lo, hi, cm[c]) for lo, hi in boxes)
+        cells, parts = t.group_lists_rb2(rb2, G, g, sp["n_cells"][g], sp["n_parts"][g])
+        cover = np.zeros(n, np.int32)
+        cover[parts] += 1
+        for c in cells:
+            cover[first[c]:first[c] + count[c]] += 1
+            assert d2(c) > rb2[c]                                   # accepted: outside r_b of every piece
+            assert not d2(parent[c]) > rb2[parent[c]]               # its parent was opened
+        assert np.all(cover == 1)
+    d = orc.direct_sum(pm, 0.01)
+    assert np.allclose(t.gravity(0.01, 0.0, G)["acc_pot"], d, rtol=1e-12, atol=1e-14)
+
+
+def test_split_box_removes_the_system_sized_lists(orc):
+    """What R25 is for: with one box per Morton group a few groups straddle the coarsest cell boundaries and list a
+    large part of the system; cut at their coarsest boundaries the same groups have lists like everybody else's."""
+    n, G = 200000, 128
+    pm = gen.plummer(n, 5)
+    t = orc.Tree(pm, 16)
+    t.set_dist_kind(0)
+    Lb = (lambda r: r["n_cells"].astype(int) + r["n_parts"])(t.gravity(0.004, 0.6, G, forces=False))
+    t.set_dist_kind(2)
+    Ls = (lambda r: r["n_cells"].astype(int) + r["n_parts"])(t.gravity(0.004, 0.6, G, forces=False))
+    assert Lb.max() > 20 * np.median(Lb)               # the pathology is there with one box
+    assert Ls.max() < 4 * np.median(Ls)                # and gone with the pieces
+    assert Ls.sum() < 0.8 * Lb.sum()
