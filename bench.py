@@ -240,6 +240,10 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
     if world > 1:
         dist.barrier()
     clocks = sampler.result() if sampler is not None else None
+    o.otoo_set_option("walk_profile", 1)          # one more step, outside the timed region, with the instrumented kernel
+    step()
+    s = o.otoo_last_stats()
+    o.otoo_set_option("walk_profile", 0)
     t_build = np.array([e[0].elapsed_time(e[1]) for e in evs])
     t_grav = np.array([e[1].elapsed_time(e[2]) for e in evs])
     ms_step = float((t_build + t_grav).mean())
@@ -247,7 +251,9 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
     res = dict(cfg=cfg, n=n, G=G, inter=inter, inter_all=inter_all, ms_step=ms_max, value=inter_all / (ms_max * 1e-3),
                build_ms=float(t_build.mean()), call_ms=float(t_grav.mean()), kernel_ms=float(np.mean(kern_ms)),
                prep_ms=float(np.mean(prep_ms)), kernel_sm_mhz=float(np.mean(sm_mhz)), launches_step=launches_step, clocks=clocks, delta=delta, m_limit=m_limit,
-               phases={k: float(np.mean([p[k] for p in phases])) for k in phases[0]}, pm=pm, o=o, stats=st)
+               phases={k: float(np.mean([p[k] for p in phases])) for k in phases[0]}, pm=pm, o=o, stats=st,
+               warp_time={k: float(s[k]) for k in ("eval_wait_frac", "walker_wait_frac", "walker_idle_frac")},
+               walk={k: int(st[k]) for k in ("sum_tests", "sum_steps", "sum_tasks", "sum_flushes", "n_groups")})
 
     if e2e:   # ---- end to end through the host-buffer C-ABI call (pinned host memory)
         h_in = torch.from_numpy(pm).pin_memory()
@@ -332,7 +338,8 @@ def roofline_block(res, key, peak_tflops, peak_measured, sm_count):
             "kernel_ms": res["kernel_ms"], "kernel_ms_source": "CUDA events around the kernel launch alone, on its stream (otoo_last_stats.ms_walk_force), mean over the timed steps",
             "otoo_gravity_call_ms": res["call_ms"], "prep_ms": res["prep_ms"],
             "kernel_sm_mhz": res["kernel_sm_mhz"], "kernel_sm_mhz_source": "clock64 ticks per globaltimer ns inside the kernel (otoo_last_stats.walk_sm_mhz)",
-            "interactions_per_s_kernel": res["inter"] / (res["kernel_ms"] * 1e-3)}
+            "interactions_per_s_kernel": res["inter"] / (res["kernel_ms"] * 1e-3),
+            "warp_time": res["warp_time"], "walk": res["walk"]}
 
 
 def build_block(res):

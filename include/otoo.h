@@ -72,6 +72,12 @@ typedef struct {
   float ms_walk_prep, ms_walk_force, ms_total;
   float walk_sm_mhz;         /* SM clock the gravity walk kernel actually held: SM clock ticks per nanosecond of the
                               * global timer, summed over its CTAs (0 for the other kernels) */
+  /* Where the warps of the warp-specialised gravity kernel spent their time (SM clock ticks, summed over warps):
+   * eval_wait_frac = evaluator warps waiting for a full list buffer; walker_wait_frac = walker warps waiting for a
+   * free buffer (they run ahead); walker_idle_frac = walker warps asleep waiting for a task-pool task (the tail of
+   * the kernel: 400 ns sleeps counted).  Filled only by a walk run with option "walk_profile" = 1 (the counting
+   * costs 3-4 % of the kernel, so it is a separate instantiation); 0 otherwise and for the other kernels. */
+  float eval_wait_frac, walker_wait_frac, walker_idle_frac;
   int32_t walk_only;         /* 1: the last walk ran with option "walk_only": counters valid, OUTPUTS MEANINGLESS */
   int32_t error_flag;        /* != 0: the last walk dropped cells (private spill area full): outputs and counters
                               * invalid; otoo_last_stats / otoo_export_group_stats return OTOO_ERR_CAPACITY */
@@ -199,15 +205,20 @@ otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_
  * the counters cover the range.  This is the paper's multi-device scheme (PAPER.md III-E, L179): every device
  * builds the same tree and takes a contiguous range of targets in key order; the ranges' outputs add up to
  * the whole.  A range outside the groups of a call: OTOO_ERR_INVALID_ARG.
- * "group_distance" = 0 (default): the gravity MAC compares r_b with the distance from the group's bounding box
- * (R8); 1: with the actual minimum of the members' distances, as the paper does (R23):
- * shorter lists (no system-sized boxes), costlier tests.  Gravity only; needs "warp_specialized" = 1.
+ * "group_distance" = 2 (default): the MAC compares r_b with the MINIMUM over the tight boxes of the group's pieces
+ * between its 7 coarsest key boundaries (R25: a Morton range that crosses a coarse cell boundary jumps
+ * across that cell; one box per group then spans the cell and a few groups list the whole system); the SPH walks
+ * apply their test per piece with the piece's own largest h (R26).  0: one bounding box per group (R8, R15).
+ * 1: the actual minimum of the members' distances, as the paper does (R23): shorter lists, costlier
+ * tests; gravity only (SPH walks: one box), needs "warp_specialized" = 1.
  * "warp_specialized" = 1 (default): otoo_gravity runs walker/evaluator warp pairs (walker warps build
  * the lists in shared memory, evaluator warps hold the targets and sum), 0: one warp does both in turn.
  * Same lists, same counters; sums differ in rounding order only.
  * "warp_specialized_sph" = 0 (default): the SPH kernels let one warp walk and sum in turn; 1: walker/evaluator
  * pairs as for gravity (SPH lists are short, the walkers become the bottleneck: faster only for
  * group_size >= 128).
+ * "walk_profile" = 1: otoo_gravity / otoo_gravity_delta run the instrumented form of the warp-specialised kernel that
+ * fills eval_wait_frac / walker_wait_frac / walker_idle_frac of otoo_stats_t (same results, 3-4 % slower); default 0.
  * "walk_only" = 1: the walks build and count their lists but skip the pair sums (outputs are
  * meaningless; counters exact) -- measures the walk's share of the fused kernel; default 0.
  * Unknown names: OTOO_ERR_INVALID_ARG. */

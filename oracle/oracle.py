@@ -200,7 +200,8 @@ class Tree:
         return out
 
     def set_dist_kind(self, kind):
-        """0: group AABB distance (R8); 1: exact minimum over the group's members (R23)"""
+        """2 (default): boxes of the group's pieces (R25; SPH: R26); 0: one box per group (R8, R15);
+        1: exact minimum over the group's members (R23; SPH walks then use one box)"""
         lib().orc_set_dist_kind(self._h, int(kind))
 
     def set_split_pieces(self, K):

@@ -419,6 +419,7 @@ void orc_rb2_delta(const orc_tree* t, double delta, double m_limit, float* rb2) 
 typedef struct {
   float lo[3], hi[3]; float hmax; const float* mem; int nmem;   /* mem: the members' (x,y,z,m), set for dist_kind 1 */
   int npiece; float plo[MAXPIECES][3], phi[MAXPIECES][3];       /* dist_kind 2: tight boxes of the pieces */
+  float phmax[MAXPIECES];                                       /* SPH: largest h of each piece */
 } gbox_t;
 static int key_cplev(uint64_t a, uint64_t b) {   /* number of leading octree levels two keys share, 0..21 */
   int l = 0;
@@ -430,7 +431,7 @@ static int key_cplev(uint64_t a, uint64_t b) {   /* number of leading octree lev
  * range that crosses the boundary of a coarse cell jumps across that cell (the curve is not continuous), so the
  * bounding box of the whole group can be as large as the cell while each piece between two such boundaries is
  * compact.  The group-cell distance is the minimum over the pieces of the box distance of R8. */
-static void split_pieces(const orc_tree* t, int64_t a, int64_t b, int K, gbox_t* g) {
+static void split_pieces(const orc_tree* t, int64_t a, int64_t b, int K, gbox_t* g, const float* hs) {
   int64_t cut[MAXPIECES]; int ncut = 0;
   int n = (int)(b - a);
   if (K > MAXPIECES) K = MAXPIECES;
@@ -450,18 +451,22 @@ static void split_pieces(const orc_tree* t, int64_t a, int64_t b, int K, gbox_t*
   for (int p = 0; p <= ncut; p++) {
     int64_t s0 = p == 0 ? a : cut[p - 1], s1 = p == ncut ? b : cut[p];
     for (int k = 0; k < 3; k++) { g->plo[p][k] = t->spos[4 * s0 + k]; g->phi[p][k] = g->plo[p][k]; }
-    for (int64_t s = s0; s < s1; s++)
+    g->phmax[p] = 0.0f;
+    for (int64_t s = s0; s < s1; s++) {
       for (int k = 0; k < 3; k++) {
         float v = t->spos[4 * s + k];
         if (v < g->plo[p][k]) g->plo[p][k] = v;
         if (v > g->phi[p][k]) g->phi[p][k] = v;
       }
+      if (hs && hs[s] > g->phmax[p]) g->phmax[p] = hs[s];
+    }
   }
 }
 static gbox_t group_box(const orc_tree* t, int64_t a, int64_t b, const float* hs /*sorted h or NULL*/) {
   gbox_t g; g.hmax = 0.0f; g.npiece = 0;
-  g.mem = (t->dist_kind == 1 && !hs) ? t->spos + 4 * a : NULL; g.nmem = (int)(b - a);   /* SPH walks (hs given): AABB only */
-  if (t->dist_kind == 2 && !hs) split_pieces(t, a, b, t->split_pieces, &g);
+  g.mem = (t->dist_kind == 1 && !hs) ? t->spos + 4 * a : NULL; g.nmem = (int)(b - a);   /* SPH walks (hs given) have no exact-minimum form: one box */
+  if (t->dist_kind == 2 && !hs) split_pieces(t, a, b, t->split_pieces, &g, NULL);
+  if (hs && t->dist_kind == 2) split_pieces(t, a, b, t->split_pieces, &g, hs);   /* SPH walks: R26 */
   for (int k = 0; k < 3; k++) { g.lo[k] = t->spos[4 * a + k]; g.hi[k] = g.lo[k]; }
   for (int64_t s = a; s < b; s++) {
     for (int k = 0; k < 3; k++) {
@@ -697,10 +702,29 @@ static void walk_sph(const orc_tree* t, const float* bmax, const float* rsph, co
                      int64_t id, lists_t* L) {
   const orc_cell* c = &t->cell[id];
   L->ntests++;
-  float d2 = box_d2(g, t->com_m + 4 * id);
-  float R = fmaxf(rsph[id], bmax[id] + g->hmax);
-  float R2 = R * R;
-  if (!(d2 <= R2)) return;
+  if (g->npiece > 0) {
+    /* R26: the cell is opened iff SOME piece p of the group has d_p^2 <= R_p^2, d_p = box distance of the piece (R8
+     * expression), R_p = max(r_SPH, b_max + h_max of the piece): the R15 test per piece */
+    int open = 0;
+    const float* cm = t->com_m + 4 * id;
+    for (int p = 0; p < g->npiece && !open; p++) {
+      float e[3];
+      for (int k = 0; k < 3; k++) {
+        float a = g->plo[p][k] - cm[k], b = cm[k] - g->phi[p][k];
+        float m = a > b ? a : b;
+        e[k] = m > 0.0f ? m : 0.0f;
+      }
+      float d2 = fmaf(e[2], e[2], fmaf(e[1], e[1], e[0] * e[0]));
+      float R = fmaxf(rsph[id], bmax[id] + g->phmax[p]);
+      if (d2 <= R * R) open = 1;
+    }
+    if (!open) return;
+  } else {
+    float d2 = box_d2(g, t->com_m + 4 * id);
+    float R = fmaxf(rsph[id], bmax[id] + g->hmax);
+    float R2 = R * R;
+    if (!(d2 <= R2)) return;
+  }
   if (c->child_count == 0) {
     for (uint32_t s = c->first; s < c->first + c->count; s++) push_u32(&L->parts, &L->np, &L->capp, s);
     return;

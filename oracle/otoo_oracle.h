@@ -127,8 +127,9 @@ uint64_t orc_sph_force_visc_sel(const orc_tree*, const float* h, const double* r
 double orc_W(double r, double h);
 double orc_dWdr(double r, double h);
 
-/* group-cell distance of the gravity walks: 0 = from the group's AABB (R8, default), 1 = the paper's exact
- * minimum over the group's members (R23).  SPH walks always use the AABB. */
+/* group-cell distance: 2 (default) = minimum over the tight boxes of the group's pieces between its 7 coarsest key
+ * boundaries (R25; the SPH walks apply their test per piece with the piece's own h_max, R26); 0 = from one box per
+ * group (R8 / R15); 1 = the paper's exact minimum over the group's members (R23; SPH walks: one box). */
 void orc_set_dist_kind(orc_tree*, int kind);
 void orc_set_split_pieces(orc_tree*, int K);   /* dist_kind 2: pieces per group (8 = the reading R25; other values for the study in DESIGN.md only) */
 int orc_max_threads(void);

@@ -63,7 +63,9 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_gravity_kernel(cons
 // ---------------------------------------------------------------- warp-specialised form (walk_ws.cuh)
 // Walker-side visitor: the MAC, the list entries and the self marks of GravVisitor without targets or
 // sums; submit() publishes the filled buffer to the pair's evaluator warp and returns the next one.
-template <int T_>
+// PROF: count the SM clock ticks spent waiting (option "walk_profile"; costs 3-4 % of the kernel, so it is a
+// separate instantiation and never the timed one)
+template <int T_, bool PROF = false>
 struct GravWalker {
   static constexpr int T = T_, E = 1, LCAP = OTOO_WS_LCAP, NP = (T_ + 1) / 2;
   static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
@@ -78,8 +80,12 @@ struct GravWalker {
   int lane_, nmem;
   __device__ __forceinline__ GravWalker(const GravParams& p_, Pair& sm_, int lane) : p(p_), sm(sm_), buf(0), eparity(~0u), first(0), lane_(lane) {}
 
+  long long wait_ticks = 0;                          // SM clock ticks spent waiting for a free buffer (otoo_stats_t.walker_wait_frac)
   __device__ __forceinline__ float4* acquire() {     // wait until the evaluator has released buffer `buf`
+    long long w0 = 0;
+    if (PROF) w0 = clock64();
     mbar_wait<500>(&sm.empty[buf], (eparity >> buf) & 1u);   // walkers run ahead: wait without stealing issue slots
+    if (PROF) wait_ticks += clock64() - w0;
     eparity ^= 1u << buf;
     return sm.list[buf];
   }
@@ -172,10 +178,17 @@ struct GravWalker {
   }
 };
 
-template <int T> struct WsRegs { static constexpr int MINB = OTOO_WS_MINB, EVAL = OTOO_WS_EVAL_REGS, WALK = OTOO_WS_WALK_REGS; };
-template <> struct WsRegs<8> { static constexpr int MINB = 2, EVAL = 176, WALK = 80; };
+#ifndef OTOO_EVAL_PB_T8
+#define OTOO_EVAL_PB_T8 0      // target pairs per pass over a list buffer for G = 256 (0: 2)
+#define OTOO_EVAL_UNR_T8 OTOO_EVAL_UNR
+#endif
+#ifndef OTOO_EVAL_UNR_T4
+#define OTOO_EVAL_UNR_T4 OTOO_EVAL_UNR
+#endif
+template <int T> struct WsRegs { static constexpr int MINB = OTOO_WS_MINB, EVAL = OTOO_WS_EVAL_REGS, WALK = OTOO_WS_WALK_REGS, PB = 0, UNR = T == 4 ? OTOO_EVAL_UNR_T4 : OTOO_EVAL_UNR; };
+template <> struct WsRegs<8> { static constexpr int MINB = 2, EVAL = 176, WALK = 80, PB = OTOO_EVAL_PB_T8, UNR = OTOO_EVAL_UNR_T8; };
 
-template <int T, bool EPS0>
+template <int T, bool EPS0, bool PROF>
 __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_gravity_ws_kernel(const GravParams p) {
   typedef typename GravWalker<T>::Pair Pair;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -195,18 +208,27 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
     // ---- walker: L57 rules through walk_driver, lists into the pair's buffers
     if (WsRegs<T>::WALK) setmaxnreg_dec<WsRegs<T>::WALK>();
     Pair& sm = pairs[warp - OTOO_WS_PAIRS];
-    GravWalker<T> w(p, sm, lane);
+    GravWalker<T, PROF> w(p, sm, lane);
+    long long wk0 = 0;
+    if (PROF) wk0 = clock64();
     float4* list = w.acquire();
     walk_driver(p.c, w, list, sm.stk, lane, (int64_t)blockIdx.x * OTOO_WS_PAIRS + (warp - OTOO_WS_PAIRS));
     w.finish();
+    if (PROF && lane == 0) { atomicAdd(p.c.sums + 11, (unsigned long long)w.wait_ticks); atomicAdd(p.c.sums + 13, (unsigned long long)(clock64() - wk0)); }
   } else {
     // ---- evaluator: targets and sums in registers, consumes the buffers in order
     if (WsRegs<T>::EVAL) setmaxnreg_inc<WsRegs<T>::EVAL>();
     Pair& sm = pairs[warp];
-    GravVisitor<T, EPS0> v(p);
+    GravVisitor<T, EPS0, WsRegs<T>::PB, WsRegs<T>::UNR> v(p);
     uint32_t buf = 0, fparity = 0;
+    long long ewait = 0;
+    long long ev0 = 0;
+    if (PROF) ev0 = clock64();
     for (;;) {
+      long long w0 = 0;
+      if (PROF) w0 = clock64();
       mbar_wait(&sm.full[buf], (fparity >> buf) & 1u);
+      if (PROF) ewait += clock64() - w0;
       fparity ^= 1u << buf;
       const WsMeta m = sm.meta[buf];
       if (m.flags & WS_EXIT) break;
@@ -217,6 +239,7 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
       mbar_arrive(&sm.empty[buf]);
       buf = (buf + 1) % OTOO_WS_NBUF;
     }
+    if (PROF && lane == 0) { atomicAdd(p.c.sums + 10, (unsigned long long)ewait); atomicAdd(p.c.sums + 12, (unsigned long long)(clock64() - ev0)); }
     if (threadIdx.x == 0) {
       unsigned long long ns1;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns1));
@@ -226,17 +249,21 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
   }
 }
 
-template <int T, bool EPS0>
-otoo_status launch_walk_ws2(otoo_ctx* ctx, const GravParams& p, cudaStream_t st) {
+template <int T, bool EPS0, bool PROF>
+otoo_status launch_walk_ws3(otoo_ctx* ctx, const GravParams& p, cudaStream_t st) {
   const size_t smem = OTOO_WS_PAIRS * sizeof(typename GravWalker<T>::Pair);
-  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_ws_kernel<T, EPS0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_gravity_ws_kernel<T, EPS0, PROF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int occ = 1;
-  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_gravity_ws_kernel<T, EPS0>, OTOO_WS_PAIRS * 64, smem));
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_gravity_ws_kernel<T, EPS0, PROF>, OTOO_WS_PAIRS * 64, smem));
   if (occ < 1) occ = 1;
   int64_t grid = (int64_t)ctx->sm_count * occ;                       // persistent: every CTA resident
   if (grid * OTOO_WS_PAIRS > p.c.ngroups) grid = cdiv(p.c.ngroups > 0 ? p.c.ngroups : 1, OTOO_WS_PAIRS);
-  walk_gravity_ws_kernel<T, EPS0><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
+  walk_gravity_ws_kernel<T, EPS0, PROF><<<(unsigned)grid, OTOO_WS_PAIRS * 64, smem, st>>>(p);
   return OTOO_OK;
+}
+template <int T, bool EPS0>
+otoo_status launch_walk_ws2(otoo_ctx* ctx, const GravParams& p, cudaStream_t st) {
+  return ctx->walk_profile ? launch_walk_ws3<T, EPS0, true>(ctx, p, st) : launch_walk_ws3<T, EPS0, false>(ctx, p, st);
 }
 template <int T>
 otoo_status launch_walk_ws(otoo_ctx* ctx, const GravParams& p, bool eps0, cudaStream_t st) {

@@ -108,6 +108,7 @@ struct SphParams {
   const float4* svel;   // sorted velocities (w: sound speed for the viscosity) or NULL
   const float4* svis;   // sorted (alpha, Balsara f, -, -) or NULL
   const float2* c_sph;  // (b_max, r_SPH) per cell
+  int pieces;                   // 1: MAC and cull per piece of the group (R26); 0: one box per group (R15)
   float* rho; uint32_t* nngb;   // density outputs (zeroed before the launch)
   float4* acc;                  // force output (zeroed before the launch)
 };
@@ -141,7 +142,8 @@ struct SphVisitor {
   f32x2 PX[(T + 1) / 2], PY[(T + 1) / 2], PZ[(T + 1) / 2], H2[(T + 1) / 2];   // pass 1: two targets per aligned register pair
   uint32_t cnt_ngb[T];
   float glo[3], ghi[3], hmax;
-  __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_) {}
+  float4* pbox;        // boxes (lo.xyz, h_max), (hi.xyz, -) of the group's pieces in shared memory (R26); set by the kernel
+  __device__ __forceinline__ SphVisitor(const SphParams& p_) : p(p_), pbox(nullptr) {}
 
   __device__ __forceinline__ void load_group(int64_t g0, int lane, float4* scratch) {
     hmax = 0.0f;
@@ -193,15 +195,34 @@ struct SphVisitor {
       }
     }
     if (scratch) __syncwarp();
+    if (scratch && pbox && p.pieces) {     // R26: members (x, y, z, h) through the idle list memory, then the pieces
+#pragma unroll
+      for (int t = 0; t < T; t++) scratch[t * 32 + lane] = make_float4(px[t], py[t], pz[t], ph[t]);
+      __syncwarp();
+      const int64_t left = p.c.N - g0;
+      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, scratch, pbox);
+    }
   }
-  // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105)
+  // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105).
+  // R26: the same test per piece of the group (its box, its own h_max); the whole-group test first: its distance
+  // is not above any piece's and its R not below (in fp32 too: every step is monotone), so it only rejects what
+  // every piece rejects.
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
     A = __ldg(p.c.cell_cm + cell);
     B = __ldg(p.c.cell_b + cell);
     float2 rr = __ldg(p.c_sph + cell);
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
     float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));
-    return d2 <= __fmul_rn(R, R) ? 2 : 0;
+    if (!(d2 <= __fmul_rn(R, R))) return 0;
+    if (!p.pieces) return 2;
+    bool open = false;
+#pragma unroll
+    for (int q = 0; q < OTOO_PIECES; q++) {
+      const float4 lo = pbox[2 * q], hi = pbox[2 * q + 1];
+      const float Rq = fmaxf(rr.y, __fadd_rn(rr.x, lo.w));
+      open = open || piece_d2(lo, hi, A.x, A.y, A.z) <= __fmul_rn(Rq, Rq);
+    }
+    return open ? 2 : 0;
   }
   struct Entry { float4 v[E]; };
   __device__ __forceinline__ Entry get(uint32_t s) const {
@@ -228,7 +249,21 @@ struct SphVisitor {
     const float bz = fmaxf(fmaxf(__fsub_rn(glo[2], a.z), __fsub_rn(a.z, ghi[2])), 0.0f);
     const float d2 = __fmaf_rn(bz, bz, __fmaf_rn(by, by, __fmul_rn(bx, bx)));
     const float hm2 = __fmul_rn(hmax, hmax);
-    return d2 < (GATHER ? hm2 : fmaxf(hm2, e.v[E >= 2 ? 1 : 0].z));
+    const float hj2 = GATHER ? 0.0f : e.v[E >= 2 ? 1 : 0].z;
+    if (!(d2 < fmaxf(hm2, hj2))) return false;
+    if (!p.pieces) return true;
+    // the same argument per piece: a member of piece q has r^2 >= the piece's box distance and a limit <= the
+    // piece's largest one
+    bool k = false;
+#pragma unroll
+    for (int q = 0; q < OTOO_PIECES; q++) {
+      const float4 lo = pbox[2 * q], hi = pbox[2 * q + 1];
+      const float ex = fmaxf(fmaxf(__fsub_rn(lo.x, a.x), __fsub_rn(a.x, hi.x)), 0.0f);
+      const float ey = fmaxf(fmaxf(__fsub_rn(lo.y, a.y), __fsub_rn(a.y, hi.y)), 0.0f);
+      const float ez = fmaxf(fmaxf(__fsub_rn(lo.z, a.z), __fsub_rn(a.z, hi.z)), 0.0f);
+      k = k || __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex))) < fmaxf(__fmul_rn(lo.w, lo.w), hj2);
+    }
+    return k;
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);   // far away, zero mass
@@ -413,6 +448,8 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const Sp
                   warp * OTOO_WALK_STACK_MAX;
   SphVisitor<T, MODE> v(p);
   v.msk = reinterpret_cast<uint32_t*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (SphVisitor<T, MODE>::W * T * 32);
+  v.pbox = reinterpret_cast<float4*>(smem_raw + otoo_walk_smem_bytes_dev() + (size_t)OTOO_WALK_WARPS * SphVisitor<T, MODE>::W * T * 32 * sizeof(uint32_t)) +
+           warp * (2 * OTOO_PIECES);
   v.lane_ = lane;
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
@@ -426,7 +463,7 @@ struct SphWalker {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
   static constexpr int LCAP = OTOO_WS_LCAP;
   static constexpr bool SUBMIT_LAST = true;
-  typedef WsPair<2> Pair;
+  typedef WsPair<2, 32 * T_> Pair;
   const SphParams& p;
   Pair& sm;
   float glo[3], ghi[3], hmax;
@@ -445,7 +482,9 @@ struct SphWalker {
       int64_t s = g0 + t * 32 + lane;
       s = s < p.c.N ? s : g0;
       float4 v = p.c.spos[s];
-      hmax = fmaxf(hmax, MODE == 0 ? p.hs[s] : p.aux[s].x);
+      const float hh = MODE == 0 ? p.hs[s] : p.aux[s].x;
+      hmax = fmaxf(hmax, hh);
+      if (p.pieces) sm.mem[t * 32 + lane] = make_float4(v.x, v.y, v.z, hh);
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
         glo[0] = fminf(glo[0], v.x); ghi[0] = fmaxf(ghi[0], v.x);
@@ -463,6 +502,11 @@ struct SphWalker {
       hmax = fmaxf(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, o));
     }
     first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+    if (p.pieces) {
+      __syncwarp();
+      const int64_t left = p.c.N - g0;
+      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, sm.mem, sm.pbox);
+    }
   }
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
     A = __ldg(p.c.cell_cm + cell);
@@ -470,7 +514,16 @@ struct SphWalker {
     float2 rr = __ldg(p.c_sph + cell);
     float d2 = aabb_d2(glo, ghi, A.x, A.y, A.z);
     float R = fmaxf(rr.y, __fadd_rn(rr.x, hmax));
-    return d2 <= __fmul_rn(R, R) ? 2 : 0;
+    if (!(d2 <= __fmul_rn(R, R))) return 0;
+    if (!p.pieces) return 2;
+    bool open = false;                            // R26, as SphVisitor::classify
+#pragma unroll
+    for (int q = 0; q < OTOO_PIECES; q++) {
+      const float4 lo = sm.pbox[2 * q], hi = sm.pbox[2 * q + 1];
+      const float Rq = fmaxf(rr.y, __fadd_rn(rr.x, lo.w));
+      open = open || piece_d2(lo, hi, A.x, A.y, A.z) <= __fmul_rn(Rq, Rq);
+    }
+    return open ? 2 : 0;
   }
   struct Entry { float4 v[E]; };
   __device__ __forceinline__ Entry get(uint32_t s) const {
@@ -496,7 +549,16 @@ struct SphWalker {
     const float bz = fmaxf(fmaxf(__fsub_rn(glo[2], a.z), __fsub_rn(a.z, ghi[2])), 0.0f);
     const float d2 = __fmaf_rn(bz, bz, __fmaf_rn(by, by, __fmul_rn(bx, bx)));
     const float hm2 = __fmul_rn(hmax, hmax);
-    return d2 < (MODE == 0 ? hm2 : fmaxf(hm2, e.v[E >= 2 ? 1 : 0].z));
+    const float hj2 = MODE == 0 ? 0.0f : e.v[E >= 2 ? 1 : 0].z;
+    if (!(d2 < fmaxf(hm2, hj2))) return false;
+    if (!p.pieces) return true;
+    bool k = false;                               // per piece, as SphVisitor::keep
+#pragma unroll
+    for (int q = 0; q < OTOO_PIECES; q++) {
+      const float4 lo = sm.pbox[2 * q], hi = sm.pbox[2 * q + 1];
+      k = k || piece_d2(lo, hi, a.x, a.y, a.z) < fmaxf(__fmul_rn(lo.w, lo.w), hj2);
+    }
+    return k;
   }
   __device__ __forceinline__ void pad(float4* dst) {
     dst[0] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);
@@ -597,7 +659,7 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
   int occ = 1;
   const size_t smem0 = smem;
 #define OTOO_SPH_CASE(TT)                                                                                              \
-  smem = smem0 + (size_t)OTOO_WALK_WARPS * SphVisitor<TT, MODE>::W * TT * 32 * sizeof(uint32_t);   /* + the mask words */   \
+  smem = smem0 + (size_t)OTOO_WALK_WARPS * (SphVisitor<TT, MODE>::W * TT * 32 * sizeof(uint32_t) + 2 * OTOO_PIECES * sizeof(float4));   /* + the mask words + the pieces' boxes */   \
   OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_kernel<TT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_kernel<TT, MODE>, OTOO_WALK_WARPS * 32, smem));  \
   if (occ < 1) occ = 1;                                                                                                 \
@@ -631,6 +693,7 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   ctx->launches += 3;
   p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->svis = nullptr; p->c_sph = ctx->c_sph;
   p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
+  p->pieces = ctx->dist_kind == 2;
   ctx->sph_radii_valid = true;
   return OTOO_OK;
 }

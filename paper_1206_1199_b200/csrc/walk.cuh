@@ -83,7 +83,7 @@ __device__ __forceinline__ void group_pieces(const uint64_t* __restrict__ keys, 
   }
 #pragma unroll 1
   for (int p = 0; p < OTOO_PIECES; p++) {
-    unsigned lo[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu}, hi[3] = {0u, 0u, 0u};
+    unsigned lo[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu}, hi[3] = {0u, 0u, 0u}, wmax = 0u;
 #pragma unroll
     for (int t = 0; t < T; t++) {
       const int i = t * 32 + lane;
@@ -92,17 +92,27 @@ __device__ __forceinline__ void group_pieces(const uint64_t* __restrict__ keys, 
         lo[0] = min(lo[0], f2ord_(q.x)); hi[0] = max(hi[0], f2ord_(q.x));
         lo[1] = min(lo[1], f2ord_(q.y)); hi[1] = max(hi[1], f2ord_(q.y));
         lo[2] = min(lo[2], f2ord_(q.z)); hi[2] = max(hi[2], f2ord_(q.z));
+        wmax = max(wmax, f2ord_(q.w));
       }
     }
 #pragma unroll
     for (int k = 0; k < 3; k++) { lo[k] = __reduce_min_sync(0xFFFFFFFFu, lo[k]); hi[k] = __reduce_max_sync(0xFFFFFFFFu, hi[k]); }
+    wmax = __reduce_max_sync(0xFFFFFFFFu, wmax);
     if (lane == 0) {
       const bool any = lo[0] != 0xFFFFFFFFu || hi[0] != 0u;     // (a member at the ordered value 0xFFFFFFFF is a NaN: not a position)
-      pbox[2 * p] = any ? make_float4(ord2f_(lo[0]), ord2f_(lo[1]), ord2f_(lo[2]), 0.f) : make_float4(INFINITY, INFINITY, INFINITY, 0.f);
+      // .w of the lo corner: the largest mem[].w of the piece (SPH walks stage h there: the piece's h_max, R26)
+      pbox[2 * p] = any ? make_float4(ord2f_(lo[0]), ord2f_(lo[1]), ord2f_(lo[2]), ord2f_(wmax)) : make_float4(INFINITY, INFINITY, INFINITY, 0.f);
       pbox[2 * p + 1] = any ? make_float4(ord2f_(hi[0]), ord2f_(hi[1]), ord2f_(hi[2]), 0.f) : make_float4(-INFINITY, -INFINITY, -INFINITY, 0.f);
     }
   }
   __syncwarp();
+}
+// R8 box distance of one piece
+__device__ __forceinline__ float piece_d2(const float4 lo, const float4 hi, float cx, float cy, float cz) {
+  const float ex = fmaxf(0.0f, fmaxf(__fsub_rn(lo.x, cx), __fsub_rn(cx, hi.x)));
+  const float ey = fmaxf(0.0f, fmaxf(__fsub_rn(lo.y, cy), __fsub_rn(cy, hi.y)));
+  const float ez = fmaxf(0.0f, fmaxf(__fsub_rn(lo.z, cz), __fsub_rn(cz, hi.z)));
+  return __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
 }
 // minimum over the pieces of the R8 box distance
 __device__ __forceinline__ float pieces_d2(const float4* pbox, float cx, float cy, float cz) {
@@ -181,6 +191,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;
   unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;
   unsigned long long tot_steps = 0, tot_tasks = 0, tot_flushes = 0;
+  uint32_t idle_polls = 0;          // 400 ns sleeps of this warp while it waited for a pool task
   bool main_done = false, have_ticket = false;
   uint32_t my_ticket = 0;
   float4* list = list0;
@@ -220,7 +231,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       }
       ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
       if (ok < 0) break;
-      if (ok == 0) { __nanosleep(400); continue; }
+      if (ok == 0) { __nanosleep(400); idle_polls++; continue; }
       take(my_ticket);
       have_ticket = false;
       got = true;
@@ -452,6 +463,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     atomicAdd(c.sums + 4, tot_steps); atomicAdd(c.sums + 5, tot_tasks);
     atomicAdd(c.sums + 6, tot_flushes);
   }
+  if (lane == 0 && idle_polls) atomicAdd(c.sums + 14, (unsigned long long)idle_polls);
 }
 
 // host side (gravity.cu)

@@ -235,18 +235,21 @@ def test_walk_stack_spill(otoo, orc):
         otoo.otoo_set_option("warp_specialized", 1)
 
 
-@pytest.mark.parametrize("ws", [1, 0])
+@pytest.mark.parametrize("ws,dist", [(0, 2), (1, 2), (0, 0), (1, 0)])
 @pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
-def test_sph_parity(otoo, orc, n, G, ws):
-    """ws = 0: one warp walks and sums in turn (default); ws = 1: walker/evaluator warp pairs."""
+def test_sph_parity(otoo, orc, n, G, ws, dist):
+    """ws = 0: one warp walks and sums in turn (default); ws = 1: walker/evaluator warp pairs.
+    dist = 2: the SPH MAC per piece of the group (R26, default); 0: one box per group (R15)."""
     otoo.otoo_set_option("warp_specialized_sph", ws)
+    otoo.otoo_set_option("group_distance", dist)
     try:
-        _sph_parity(otoo, orc, n, G)
+        _sph_parity(otoo, orc, n, G, dist)
     finally:
         otoo.otoo_set_option("warp_specialized_sph", 0)
+        otoo.otoo_set_option("group_distance", 2)
 
 
-def _sph_parity(otoo, orc, n, G):
+def _sph_parity(otoo, orc, n, G, dist=2):
     w = gen.wd_pair(n, 1206)
     pm, h, u = w["pos_mass"], w["h"], w["u"]
     # the generator's rigid rotation has (v_i - v_j).(x_i - x_j) = 0 for every pair (du/dt would be
@@ -255,6 +258,7 @@ def _sph_parity(otoo, orc, n, G):
     vel[:, :3] += -0.3 * pm[:, :3] + 0.05 * (gen.uniform01(99, np.arange(3 * n, dtype=np.uint64), 0).reshape(n, 3) - 0.5)
     vel = vel.astype(np.float32)
     t = check_tree(otoo, orc, pm, 16)
+    t.set_dist_kind(dist)
     ref = t.sph_density(h, G)
     rho, nngb = otoo.otoo_sph_density(dev(h), G)
     b, r = otoo.otoo_export_sph_radii()

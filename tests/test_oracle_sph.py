@@ -231,3 +231,34 @@ def test_artificial_viscosity(orc):
     assert a[0, 0] == pytest.approx(-1.0 * Pi * gw * (0 - 0.5) / r, rel=1e-12)     # pushed apart: a_0x < 0
     assert a[0, 0] < 0 and a[1, 0] == pytest.approx(-a[0, 0], rel=1e-12)
     assert a[0, 3] == pytest.approx(0.5 * Pi * gw * wdot / r, rel=1e-12) and a[0, 3] > 0
+
+
+def test_sph_walk_over_pieces_finds_the_same_neighbours(orc):
+    """Reading R26 (default): the SPH MAC of R15 applied per piece of the group (the piece's box, the piece's largest
+    h).  Fewer candidates, and -- Eq. 5's guarantee holds piece by piece -- exactly the same neighbours: counts equal,
+    density and forces equal to rounding (the candidate lists keep their tree order)."""
+    n, G = 6000, 64
+    w = gen.wd_pair(n, 21)
+    pm, h, u, vel = w["pos_mass"], w["h"], w["u"], w["vel"]
+    t = orc.Tree(pm, 16)
+    t.set_dist_kind(0)
+    a = t.sph_density(h, G)
+    t.set_dist_kind(2)
+    b = t.sph_density(h, G)
+    assert b["candidates"] < 0.8 * a["candidates"] and np.all(b["n_parts"] <= a["n_parts"])
+    assert np.array_equal(a["nngb"], b["nngb"]) and np.allclose(a["rho"], b["rho"], rtol=1e-14)
+    P = (2.0 / 3.0) * a["rho"] * u
+    t.set_dist_kind(0)
+    fa = t.sph_force(h, a["rho"], P, G, vel=vel)
+    t.set_dist_kind(2)
+    fb = t.sph_force(h, a["rho"], P, G, vel=vel)
+    assert np.allclose(fa["acc_dudt"], fb["acc_dudt"], rtol=1e-12, atol=1e-14 * np.abs(fa["acc_dudt"]).max())
+    # brute force: every true neighbour pair (r < max(h_i, h_j)) of every member is in its group's list
+    ex = t.export()
+    sp, sh = pm[ex["perm"]].astype(np.float64), h[ex["perm"]].astype(np.float64)
+    for g in range(0, t.n_groups(G), 5):
+        parts = t.sph_group_list(h, G, g, b["n_parts"][g])
+        mem = np.arange(g * G, min((g + 1) * G, n))
+        d = np.linalg.norm(sp[mem, None, :3] - sp[None, :, :3], axis=2)
+        need = (d < np.maximum(sh[mem, None], sh[None, :])).any(0)
+        assert np.isin(np.nonzero(need)[0], parts).all()
