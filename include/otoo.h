@@ -101,8 +101,10 @@ otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
 
 /* PAPER III-D: group walk (L57, L163; R7-R9) fused with the softened Plummer monopole/particle
  * sums (L43; R10).  eps >= 0 scalar softening; theta >= 0 opening angle (0 opens every cell =
- * direct sum); group_size in {32, 64, 128, 256} consecutive Morton-sorted targets share one
- * interaction list.  d_acc_pot: N x float4 (ax, ay, az, phi), original order. Asynchronous. */
+ * direct sum); group_size consecutive Morton-sorted targets share one interaction list: 32, 64, 128 or 256
+ * (a warp holds 1, 2, 4 or 8 targets per lane), or the paper's own vector lengths 4, 8, 16 (PAPER.md L163-L167,
+ * L183: n_vec = 4-8; run with one group per warp, the other lanes idle -- the regime of the paper's scaling
+ * laws, not a fast one).  d_acc_pot: N x float4 (ax, ay, az, phi), original order. Asynchronous. */
 otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, float* d_acc_pot,
                          void* stream);
 

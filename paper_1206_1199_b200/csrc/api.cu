@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) eos_ideal_kernel(const float* __restrict_
   if (i < n) P[i] = __fmul_rn(__fmul_rn(gm1, rho[i]), u[i]);
 }
 
-bool valid_group(int G) { return G == 32 || G == 64 || G == 128 || G == 256; }
+bool valid_group(int G) { return G == 4 || G == 8 || G == 16 || G == 32 || G == 64 || G == 128 || G == 256; }
 
 }  // namespace
 
@@ -146,7 +146,7 @@ otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
 otoo_status otoo_gravity(otoo_ctx* ctx, float eps, float theta, int group_size, float* d_acc_pot, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
   if (!(eps >= 0.0f) || !(theta >= 0.0f)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "eps >= 0 and theta >= 0 required");
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_acc_pot is NULL");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -159,7 +159,7 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
   if (!ctx) return OTOO_ERR_INVALID_ARG;
   if (!(eps >= 0.0f) || !(delta >= 0.0f) || !(m_limit > 0.0f))
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "eps >= 0, delta >= 0 and m_limit > 0 required");
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_acc_pot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_acc_pot is NULL");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -179,7 +179,7 @@ static otoo_status sph_scratch(otoo_ctx* ctx) {
 
 otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, float* d_rho, uint32_t* d_nngb, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_h || !d_rho) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_h and d_rho must not be NULL");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -191,7 +191,7 @@ otoo_status otoo_sph_density(otoo_ctx* ctx, const float* d_h, int group_size, fl
 otoo_status otoo_sph_stage1(otoo_ctx* ctx, const float* d_h, const float* d_vel, int group_size, float* d_rho, uint32_t* d_nngb,
                             float* d_divrot, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_h || !d_vel || !d_rho || !d_divrot) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_h, d_vel, d_rho, d_divrot must not be NULL");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -203,7 +203,7 @@ otoo_status otoo_sph_stage1(otoo_ctx* ctx, const float* d_h, const float* d_vel,
 otoo_status otoo_sph_adapt_h(otoo_ctx* ctx, float* d_h, float n_target, float tol, int max_iter, int group_size,
                              uint32_t* d_nngb, int* host_iters, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_h) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "d_h must not be NULL");
   if (!(n_target >= 1.0f) || !(tol >= 0.0f) || max_iter < 0)
@@ -217,7 +217,7 @@ otoo_status otoo_sph_adapt_h(otoo_ctx* ctx, float* d_h, float n_target, float to
 otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
                            int group_size, float* d_acc_sph, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_h || !d_rho || !d_P || !d_acc_sph) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL argument");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -229,7 +229,7 @@ otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, 
 otoo_status otoo_sph_force_visc(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
                                 const float* d_visc, int group_size, float* d_acc_sph, void* stream) {
   if (!ctx) return OTOO_ERR_INVALID_ARG;
-  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (!valid_group(group_size)) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
   if (!d_h || !d_rho || !d_P || !d_vel || !d_visc || !d_acc_sph) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "NULL argument");
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));

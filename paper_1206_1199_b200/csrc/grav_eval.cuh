@@ -42,7 +42,7 @@ struct GravVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) {   // H7: lane holds slots g0 + t*32 + lane; out-of-range lanes mirror slot g0
       int64_t s = g0 + t * 32 + lane;
-      float4 v = p.c.spos[s < p.c.N ? s : g0];
+      float4 v = p.c.spos[member_ok(p.c, g0, t * 32 + lane) ? s : g0];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z; pm[t] = v.w;
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
@@ -80,8 +80,7 @@ struct GravVisitor {
 #pragma unroll
       for (int t = 0; t < T; t++) scratch[t * 32 + lane] = make_float4(px[t], py[t], pz[t], 0.0f);
       __syncwarp();
-      const int64_t left = p.c.N - g0;
-      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, scratch, pbox);
+      group_pieces<T>(p.c.keys, g0, group_count(p.c, g0), lane, scratch, pbox);
     }
   }
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
@@ -98,7 +97,7 @@ struct GravVisitor {
   __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
   __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
 #pragma unroll
-    for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
+    for (int t = 0; t < T; t++) if (member_ok(p.c, g0, t * 32 + lane) && (uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
   static constexpr bool SUBMIT_LAST = false, CULL = false;
   template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
@@ -153,7 +152,7 @@ struct GravVisitor {
       const int q = t >> 1;
       float4 o = (t & 1) ? make_float4(AX[q].y, AY[q].y, AZ[q].y, PH[q].y) : make_float4(AX[q].x, AY[q].x, AZ[q].x, PH[q].x);
       if ((selfmask >> t) & 1u) o.w = __fmaf_rn(pm[t], rie, o.w);
-      if (s < p.c.N) {
+      if (member_ok(p.c, g0, t * 32 + lane)) {
         float* dst = reinterpret_cast<float*>(p.acc_pot + p.c.perm[s]);
         atomicAdd(dst + 0, o.x); atomicAdd(dst + 1, o.y); atomicAdd(dst + 2, o.z); atomicAdd(dst + 3, o.w);
       }

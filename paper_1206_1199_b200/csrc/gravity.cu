@@ -93,7 +93,7 @@ struct GravWalker {
 #pragma unroll
     for (int t = 0; t < T; t++) {   // H7: the group's tight AABB
       int64_t s = g0 + t * 32 + lane;
-      float4 v = p.c.spos[s < p.c.N ? s : g0];
+      float4 v = p.c.spos[member_ok(p.c, g0, t * 32 + lane) ? s : g0];
       if (p.c.dist_kind) sm.mem[t * 32 + lane] = v;      // out-of-range slots mirror slot g0: harmless duplicates
       if (t == 0) { glo[0] = ghi[0] = v.x; glo[1] = ghi[1] = v.y; glo[2] = ghi[2] = v.z; }
       else {
@@ -109,12 +109,11 @@ struct GravWalker {
         glo[k] = fminf(glo[k], __shfl_xor_sync(0xFFFFFFFFu, glo[k], o));
         ghi[k] = fmaxf(ghi[k], __shfl_xor_sync(0xFFFFFFFFu, ghi[k], o));
       }
-    selfmask = 0; first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+    selfmask = 0; first = WS_FIRST; group = (uint32_t)(g0 / p.c.gs);
     nmem = 32 * T;
     __syncwarp();
     if (p.c.dist_kind == 2) {
-      const int64_t left = p.c.N - g0;
-      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, sm.mem, sm.pbox);
+      group_pieces<T>(p.c.keys, g0, group_count(p.c, g0), lane, sm.mem, sm.pbox);
     }
     if (p.c.dist_kind == 1) {
       // tight boxes of 8 consecutive members (neighbours on the key curve): a box farther than r_b settles its
@@ -161,7 +160,7 @@ struct GravWalker {
   __device__ __forceinline__ void pad(float4* dst) { *dst = make_float4(PAD_POS, PAD_POS, PAD_POS, 0.0f); }
   __device__ __forceinline__ void mark_self(uint32_t f, uint32_t n, int64_t g0, int lane) {
 #pragma unroll
-    for (int t = 0; t < T; t++) if ((uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
+    for (int t = 0; t < T; t++) if (member_ok(p.c, g0, t * 32 + lane) && (uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
   __device__ __forceinline__ float4* submit(float4*, int n, bool last) {
     if (lane_ == 0) sm.meta[buf] = WsMeta{(uint32_t)n, first | (last ? WS_LAST : 0u), group, 0u};
@@ -232,7 +231,7 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, WsRegs<T>::MINB) walk_grav
       fparity ^= 1u << buf;
       const WsMeta m = sm.meta[buf];
       if (m.flags & WS_EXIT) break;
-      const int64_t g0 = (int64_t)m.group * (32 * T);
+      const int64_t g0 = (int64_t)m.group * p.c.gs;
       if (m.flags & WS_FIRST) { v.load_group(g0, lane, reinterpret_cast<float4*>(sm.tgt)); __syncwarp(); }
       if (!p.c.walk_only && m.count) v.eval(sm.list[buf], (int)m.count);
       if (m.flags & WS_LAST) { v.selfmask = sm.self[buf][lane]; v.store(g0, lane); }
@@ -330,7 +329,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long), st));
   c->spos = ctx->spos; c->keys = ctx->key[0]; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
-  c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin;
+  c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin; c->gs = G;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack; c->spill_cap = ctx->walk_spill_cap;
@@ -365,19 +364,19 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   OTOO_EV(ctx, ctx->ev_walk[1], st);
   if (ctx->use_ws) {
     switch (G) {
-      case 32: OTOO_TRY(launch_walk_ws<1>(ctx, p, eps0, st)); break;
+      case 4: case 8: case 16: case 32: OTOO_TRY(launch_walk_ws<1>(ctx, p, eps0, st)); break;
       case 64: OTOO_TRY(launch_walk_ws<2>(ctx, p, eps0, st)); break;
       case 128: OTOO_TRY(launch_walk_ws<4>(ctx, p, eps0, st)); break;
       case 256: OTOO_TRY(launch_walk_ws<8>(ctx, p, eps0, st)); break;
-      default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+      default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
     }
   } else
   switch (G) {
-    case 32: OTOO_TRY(launch_walk<1>(ctx, p, eps0, grid, smem, st)); break;
+    case 4: case 8: case 16: case 32: OTOO_TRY(launch_walk<1>(ctx, p, eps0, grid, smem, st)); break;
     case 64: OTOO_TRY(launch_walk<2>(ctx, p, eps0, grid, smem, st)); break;
     case 128: OTOO_TRY(launch_walk<4>(ctx, p, eps0, grid, smem, st)); break;
     case 256: OTOO_TRY(launch_walk<8>(ctx, p, eps0, grid, smem, st)); break;
-    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   }
   OTOO_EV(ctx, ctx->ev_walk[2], st);
   ctx->ev_walk_valid = true;

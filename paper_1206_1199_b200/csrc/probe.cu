@@ -191,7 +191,7 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
   } else if (strcmp(which, "sumloop") == 0) {
     GravParams p;
     memset(&p, 0, sizeof p);
-    p.c.spos = ctx->spos; p.c.N = n; p.eps2 = 1e-6f;
+    p.c.spos = ctx->spos; p.c.N = n; p.c.gs = 256; p.eps2 = 1e-6f;
     float4* sink = reinterpret_cast<float4*>(ctx->key[1]) + 4096;
     // the product's configuration first (pairs per pass = min(NP, 2), unroll OTOO_EVAL_UNR), then the variants tried
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));

@@ -150,7 +150,7 @@ struct SphVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) {
       int64_t s = g0 + t * 32 + lane;
-      s = s < p.c.N ? s : g0;
+      s = member_ok(p.c, g0, t * 32 + lane) ? s : g0;
       float4 v = p.c.spos[s];
       px[t] = v.x; py[t] = v.y; pz[t] = v.z;
       if (GATHER) { ph[t] = p.hs[s]; ppr[t] = 0.0f; }
@@ -199,8 +199,7 @@ struct SphVisitor {
 #pragma unroll
       for (int t = 0; t < T; t++) scratch[t * 32 + lane] = make_float4(px[t], py[t], pz[t], ph[t]);
       __syncwarp();
-      const int64_t left = p.c.N - g0;
-      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, scratch, pbox);
+      group_pieces<T>(p.c.keys, g0, group_count(p.c, g0), lane, scratch, pbox);
     }
   }
   // R15: open iff d^2 <= R^2, R = max(r_SPH, b_max + h_max,g); never "accept" (no p-c term, L105).
@@ -418,7 +417,7 @@ struct SphVisitor {
 #pragma unroll
     for (int t = 0; t < T; t++) {
       const int64_t s = g0 + t * 32 + lane;
-      if (s < p.c.N) {
+      if (member_ok(p.c, g0, t * 32 + lane)) {
         const uint32_t i = p.c.perm[s];
         if (GATHER) {
           float hi3 = hinv[t] * hinv[t] * hinv[t];
@@ -480,7 +479,7 @@ struct SphWalker {
 #pragma unroll
     for (int t = 0; t < T; t++) {
       int64_t s = g0 + t * 32 + lane;
-      s = s < p.c.N ? s : g0;
+      s = member_ok(p.c, g0, t * 32 + lane) ? s : g0;
       float4 v = p.c.spos[s];
       const float hh = MODE == 0 ? p.hs[s] : p.aux[s].x;
       hmax = fmaxf(hmax, hh);
@@ -501,11 +500,10 @@ struct SphWalker {
       }
       hmax = fmaxf(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, o));
     }
-    first = WS_FIRST; group = (uint32_t)(g0 / (32 * T));
+    first = WS_FIRST; group = (uint32_t)(g0 / p.c.gs);
     if (p.pieces) {
       __syncwarp();
-      const int64_t left = p.c.N - g0;
-      group_pieces<T>(p.c.keys, g0, (int)(left < 32 * T ? left : 32 * T), lane, sm.mem, sm.pbox);
+      group_pieces<T>(p.c.keys, g0, group_count(p.c, g0), lane, sm.mem, sm.pbox);
     }
   }
   __device__ __forceinline__ int classify(uint32_t cell, float4& A, cellb_t& B) {
@@ -617,7 +615,7 @@ __global__ void __launch_bounds__(OTOO_WS_PAIRS * 64, T >= 8 ? 2 : 3) walk_sph_w
       fparity ^= 1u << buf;
       const WsMeta m = sm.meta[buf];
       if (m.flags & WS_EXIT) break;
-      const int64_t g0 = (int64_t)m.group * (32 * T);
+      const int64_t g0 = (int64_t)m.group * p.c.gs;
       if (m.flags & WS_FIRST) v.load_group(g0, lane, nullptr);
       if (!p.c.walk_only && m.count) v.eval(sm.list[buf], (int)m.count);
       __syncwarp();
@@ -646,11 +644,11 @@ otoo_status launch_sph_ws2(otoo_ctx* ctx, const SphParams& p, cudaStream_t st) {
 template <int MODE>
 otoo_status launch_sph_ws(otoo_ctx* ctx, const SphParams& p, int G, cudaStream_t st) {
   switch (G) {
-    case 32: return launch_sph_ws2<1, MODE>(ctx, p, st);
+    case 4: case 8: case 16: case 32: return launch_sph_ws2<1, MODE>(ctx, p, st);
     case 64: return launch_sph_ws2<2, MODE>(ctx, p, st);
     case 128: return launch_sph_ws2<4, MODE>(ctx, p, st);
     case 256: return launch_sph_ws2<8, MODE>(ctx, p, st);
-    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   }
 }
 
@@ -669,19 +667,19 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
   OTOO_EV(ctx, ctx->ev_walk[2], st);                                                                                    \
   ctx->ev_walk_valid = true;
   switch (G) {
-    case 32: OTOO_SPH_CASE(1) break;
+    case 4: case 8: case 16: case 32: OTOO_SPH_CASE(1) break;
     case 64: OTOO_SPH_CASE(2) break;
     case 128: OTOO_SPH_CASE(4) break;
     case 256: OTOO_SPH_CASE(8) break;
-    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+    default: return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   }
 #undef OTOO_SPH_CASE
   return OTOO_OK;
 }
 
 otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, int* grid, size_t* smem, cudaStream_t st) {
-  if (G != 32 && G != 64 && G != 128 && G != 256)
-    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 32, 64, 128 or 256");
+  if (G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)
+    return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p->c, grid, smem, st));
   const unsigned nbN = (unsigned)cdiv(ctx->N, 256), nbC = (unsigned)cdiv(ctx->N_cell, 256);
   // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3)

@@ -157,6 +157,7 @@ struct WalkCommon {
   unsigned long long* sums;                                    // tests, interactions, cells, parts
   WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
   uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
+  int gs;                                                       // group size: 32 * T of the kernel, or 4 / 8 / 16 with T = 1 (the paper's n_vec, L163)
   int stack_cap;
   int spill_cap;                                                // usable entries of a warp's private spill area (<= OTOO_WALK_SPILL)
   int use_pool;                                                 // 0: never donate (test hook: private spill only)
@@ -164,6 +165,10 @@ struct WalkCommon {
   int dist_kind;                                                // gravity: 0 one box per group (R8), 1 exact minimum over the members (R23),
                                                                 // 2 minimum over the boxes of the group's pieces (R25)
 };
+
+// member idx (0 .. 32 T - 1) of the group starting at slot g0 exists
+__device__ __forceinline__ bool member_ok(const WalkCommon& c, int64_t g0, int idx) { return idx < c.gs && g0 + idx < c.N; }
+__device__ __forceinline__ int group_count(const WalkCommon& c, int64_t g0) { const int64_t left = c.N - g0; return (int)(left < c.gs ? left : c.gs); }
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
 
@@ -185,7 +190,7 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 //   void store(int64_t g0, int lane)               atomicAdd results to the outputs
 template <class V>
 __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list0, uint32_t* stk, int lane, int64_t gwarp) {
-  constexpr int G = 32 * V::T;
+  const int G = c.gs;                                // targets per group (<= 32 * V::T; below 32: the other lanes idle)
   constexpr int CAP = (V::LCAP / V::E) & ~3;         // list entries per buffer (multiple of the padding unit)
   constexpr int PADTO = 4;
   uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;

@@ -247,3 +247,53 @@ def test_fullsize_adaptive_h(orc):
         assert np.isfinite(hf).all() and (hf > 0).all()
     finally:
         o.close()
+
+
+def test_papers_vector_walk_scaling(orc):
+    """The paper's own regime on the GPU: uniform sphere N = 1 M, Hilbert order, absolute-error
+    MAC with m_limit = 0.05, exact-minimum group distance, n_vec = 4 and 8 targets per traversal (one group per warp).
+    Every group's counters equal the oracle's at n_vec = 4; the kernel time and the mean force error against the
+    O(N^2) sum follow the oracle's exponents (interactions ~ Delta^-0.45, error ~ Delta^0.5; the paper states -3/4 and
+    1/4, see tests/test_oracle_delta_mac.py::test_scaling_with_delta_at_the_papers_vector_length and DESIGN.md section 11);
+    the mean error does not depend on the vector length (L167)."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1206_1199_b200 import binding
+    n, eps, m_limit = 1 << 20, float(np.float32(0.002)), float(np.float32(0.05))
+    pm = gen.uniform_sphere(n, 1206)
+    tg = np.sort(np.random.default_rng(7).choice(n, size=1024, replace=False)).astype(np.int64)
+    ref = orc.direct_sum(pm, eps, tg)
+    deltas = [1e-2, 1e-3, 1e-4, 1e-5]
+    o = binding.Otoo(max_particles=n, device=0)
+    try:
+        o.otoo_set_option("key_order", 1)
+        o.otoo_set_option("group_distance", 1)
+        o.otoo_build_tree(dev(pm), 16)
+        t = orc.Tree(pm, 16, key_order=1)
+        t.set_dist_kind(1)
+        check_tree_full(o, t)
+        ms, err, inter = {}, {}, {}
+        for G in (4, 8, 32):
+            for d in deltas:
+                d32 = float(np.float32(d))
+                out = o.otoo_gravity_delta(eps, d32, m_limit, G).cpu().numpy().astype(np.float64)
+                st = o.otoo_last_stats()
+                ms[G, d], inter[G, d] = st["ms_walk_force"], st["sum_interactions"]
+                err[G, d] = np.linalg.norm(out[tg, :3] - ref[:, :3], axis=1).mean()
+                if G == 4 and d in (1e-2, 1e-4):
+                    r = t.gravity(eps, 0.0, G, forces=False, rb2=t.rb2_delta(d32, m_limit))
+                    nt, nc, npart = o.otoo_export_group_stats()
+                    assert np.array_equal(nt, r["n_tests"]) and np.array_equal(nc, r["n_cells"]) and np.array_equal(npart, r["n_parts"])
+                    assert inter[G, d] == r["interactions"]
+        lg = np.log10(deltas)
+        for G in (4, 8):
+            s_t = np.polyfit(lg, np.log10([ms[G, d] for d in deltas]), 1)[0]
+            s_i = np.polyfit(lg, np.log10([inter[G, d] for d in deltas]), 1)[0]
+            s_e = np.polyfit(lg, np.log10([err[G, d] for d in deltas]), 1)[0]
+            print(f"n_vec={G}: kernel ms {[round(ms[G, d], 2) for d in deltas]} slope {s_t:.3f}; interactions/particle "
+                  f"{[round(inter[G, d] / n) for d in deltas]} slope {s_i:.3f}; mean |da| {[float('%.3g' % err[G, d]) for d in deltas]} slope {s_e:.3f}")
+            assert -0.6 < s_i < -0.3 and -0.6 < s_t < -0.25 and 0.4 < s_e < 0.65, (s_i, s_t, s_e)
+        for d in deltas:
+            assert abs(err[8, d] / err[4, d] - 1) < 0.1 and 0.75 < err[32, d] / err[4, d] < 1.02
+    finally:
+        o.close()

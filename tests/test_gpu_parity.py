@@ -90,7 +90,8 @@ def test_tree_degenerate_inputs(otoo, orc):
                                                 ("plummer", 20000, 256, 0.8, 0.004), ("hernquist", 30000, 32, 0.4, 0.002),
                                                 ("uniform_cube", 50000, 128, 0.5, 0.001), ("plummer", 3000, 64, 0.0, 0.01),
                                                 ("plummer", 3000, 128, 0.5, 0.0), ("uniform_sphere", 2500, 256, 0.0, 0.0),
-                                                ("plummer", 40, 64, 0.5, 0.01)])
+                                                ("plummer", 40, 64, 0.5, 0.01), ("plummer", 6000 + 3, 4, 0.6, 0.01), ("hernquist", 9000 + 5, 8, 0.5, 0.002),
+                                                ("uniform_cube", 12000 + 7, 16, 0.5, 0.001)])
 @pytest.mark.parametrize("ws,dist", [(1, 2), (0, 2), (1, 0), (0, 0)])
 def test_gravity_parity(otoo, orc, kind, n, G, theta, eps, ws, dist):
     """ws = 1: walker/evaluator warp pairs (default); ws = 0: the fused one-warp-does-both kernel.
@@ -180,7 +181,8 @@ def test_hilbert_order_parity(otoo, orc, kind, n, n_crit, G):
 
 
 @pytest.mark.parametrize("kind,n,G,theta,key_order", [("plummer", 16384, 64, 0.5, 0), ("plummer", 20000 + 9, 128, 0.6, 0), ("hernquist", 30000, 32, 0.4, 1),
-                                                       ("uniform_cube", 40000, 256, 0.5, 0), ("plummer", 3000, 128, 0.0, 0)])
+                                                       ("uniform_cube", 40000, 256, 0.5, 0), ("plummer", 3000, 128, 0.0, 0),
+                                                       ("uniform_sphere", 8000 + 1, 4, 0.6, 1), ("plummer", 10000 + 3, 8, 0.5, 0)])
 def test_exact_min_group_distance_parity(otoo, orc, kind, n, G, theta, key_order):
     """group_distance = 1: the paper's vector walk (reading R23) -- the MAC compares r_b with the
     actual minimum of the members' distances.  Lists (counters) exact, sums within tolerance, for both MACs."""
@@ -236,7 +238,7 @@ def test_walk_stack_spill(otoo, orc):
 
 
 @pytest.mark.parametrize("ws,dist", [(0, 2), (1, 2), (0, 0), (1, 0)])
-@pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256)])
+@pytest.mark.parametrize("n,G", [(20000, 64), (20000 + 11, 32), (8000, 128), (6000, 256), (5000 + 3, 4), (6000 + 1, 16)])
 def test_sph_parity(otoo, orc, n, G, ws, dist):
     """ws = 0: one warp walks and sums in turn (default); ws = 1: walker/evaluator warp pairs.
     dist = 2: the SPH MAC per piece of the group (R26, default); 0: one box per group (R15)."""
@@ -427,7 +429,7 @@ def test_status_codes(otoo):
             fresh.otoo_gravity_delta(**bad)
         assert e.value.status == binding.OTOO_ERR_INVALID_ARG
     for bad in (dict(eps=-1.0, theta=0.5, group_size=64), dict(eps=0.01, theta=-0.5, group_size=64),
-                dict(eps=0.01, theta=0.5, group_size=48)):
+                dict(eps=0.01, theta=0.5, group_size=48), dict(eps=0.01, theta=0.5, group_size=2)):
         with pytest.raises(binding.OtooError) as e:
             fresh.otoo_gravity(**bad)
         assert e.value.status == binding.OTOO_ERR_INVALID_ARG

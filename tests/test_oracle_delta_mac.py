@@ -140,3 +140,39 @@ def test_delta_to_zero_is_direct_sum_and_error_falls(orc):
         inter.append(r["interactions"])
         assert d.max() <= 60 * delta          # loose: the bound is per accepted cell, errors add up over cells
     assert errs == sorted(errs, reverse=True) and inter == sorted(inter)     # L165-L167: cost up, error down
+
+
+def test_scaling_with_delta_at_the_papers_vector_length(orc):
+    """PAPER.md L165-L167 (Fig. 4-5, missing): "time ~ Delta^-3/4", "error ~ Delta^1/4", "the averaged error does not
+    depend on n_vec".  The paper's own configuration -- uniform sphere, n_vec = 4 and 8, exact-minimum group distance
+    (L163), Hilbert order, m_limit = 0.05 -- run by the oracle:
+      * the mean error is independent of the vector length (within 10 % between n_vec = 4 and 8; 32: up to 20 % lower): as stated;
+      * interactions per particle grow as Delta^-0.45 (local slope -0.33 ... -0.5 over Delta = 1e-1 ... 1e-6 at
+        N = 1e5 ... 1e6, cells and particles alike) and the mean error falls as Delta^0.5: NOT the paper's exponents.
+    r_b ~ (B2/Delta)^(1/4) with B2 ~ l^5 gives Delta^-3/4 cells per tree level, but the level at which r_b reaches
+    the system size moves with Delta (l_max ~ Delta^(1/5)) and m_limit opens the heavy cells regardless of Delta, so
+    the sum over levels is shallower.  The finding is recorded in DESIGN.md section 11; this test pins the measured
+    exponents so that a change of the MAC, of B2 or of the walk shows up."""
+    n, eps = 32768, 0.004
+    pm = gen.uniform_sphere(n, 1206)
+    ref = orc.direct_sum(pm, eps)
+    t = orc.Tree(pm, 16, key_order=1)
+    t.set_dist_kind(1)
+    deltas = [1e-2, 1e-3, 1e-4, 1e-5]
+    err, inter = {}, {}
+    for G in (4, 8, 32):
+        for d in deltas:
+            r = t.gravity(eps, 0.0, G, rb2=t.rb2_delta(float(np.float32(d)), float(np.float32(0.05))))
+            err[G, d] = np.linalg.norm(r["acc_pot"][:, :3] - ref[:, :3], axis=1).mean()
+            inter[G, d] = r["interactions"] / n
+    lg = np.log10(deltas)
+    for G in (4, 8):
+        si = np.polyfit(lg, np.log10([inter[G, d] for d in deltas]), 1)[0]
+        se = np.polyfit(lg, np.log10([err[G, d] for d in deltas]), 1)[0]
+        assert -0.6 < si < -0.3, si          # not -0.75
+        assert 0.4 < se < 0.65, se           # not +0.25
+    for d in deltas:
+        # n_vec = 4 vs 8 (the paper's range): within 10 %; a 32-wide vector shares longer lists and is a little MORE accurate
+        assert abs(err[8, d] / err[4, d] - 1) < 0.1 and 0.75 < err[32, d] / err[4, d] < 1.02, (d, err[4, d], err[8, d], err[32, d])
+    # larger vectors share longer lists (more interactions per particle) at the same error: the trade-off of L165
+    assert all(inter[4, d] < inter[8, d] < inter[32, d] for d in deltas)
