@@ -165,6 +165,11 @@ otoo_status otoo_sph_force(otoo_ctx* ctx, const float* d_h, const float* d_rho, 
 otoo_status otoo_eos_ideal(otoo_ctx* ctx, const float* d_rho, const float* d_u, float gamma,
                            int64_t N, float* d_P, void* stream);
 
+/* d_out[perm[s]] = d_sorted_rows[s] for N x float4 rows: results written in sorted order (option "output_sorted")
+ * back into the caller's particle order.  The multi-device scheme (PAPER.md III-E) gathers every device's
+ * contiguous range of sorted rows and calls this once.  Asynchronous. */
+otoo_status otoo_unsort(otoo_ctx* ctx, const float* d_sorted_rows, float* d_out, void* stream);
+
 /* Introspection for parity tests and the metric.  All synchronise the context's last stream. */
 otoo_status otoo_tree_info(otoo_ctx* ctx, otoo_tree_info_t* host_out);
 /* Any pointer may be NULL.  d_perm[s] = original index of sorted slot s (N); d_sorted_keys (N);
@@ -219,6 +224,10 @@ otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_
  * "warp_specialized_sph" = 0 (default): the SPH kernels let one warp walk and sum in turn; 1: walker/evaluator
  * pairs as for gravity (SPH lists are short, the walkers become the bottleneck: faster only for
  * group_size >= 128).
+ * "output_sorted" = 1: otoo_gravity / otoo_gravity_delta write row s of d_acc_pot for the target at SORTED slot s
+ * (otoo_export_tree's d_perm names its original index) instead of the caller's order; with a group range the rows
+ * [group_begin * group_size, ...) of the range are the only non-zero ones and are contiguous.  otoo_unsort brings
+ * rows back.  The SPH calls refuse it (OTOO_ERR_INVALID_ARG).  Default 0.
  * "walk_profile" = 1: otoo_gravity / otoo_gravity_delta run the instrumented form of the warp-specialised kernel that
  * fills eval_wait_frac / walker_wait_frac / walker_idle_frac of otoo_stats_t (same results, 3-4 % slower); default 0.
  * "walk_only" = 1: the walks build and count their lists but skip the pair sums (outputs are

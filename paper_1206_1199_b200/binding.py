@@ -26,7 +26,7 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host", "otoo_gravity_delta_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_probe", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
+           "otoo_gravity_host", "otoo_gravity_delta_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_probe", "otoo_unsort", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
 
 
 class TreeInfo(C.Structure):
@@ -73,6 +73,7 @@ _lib.otoo_export_group_stats.argtypes = [_vp, _vp, _vp, _vp]
 _lib.otoo_last_stats.argtypes = [_vp, C.POINTER(Stats)]
 _lib.otoo_set_option.argtypes = [_vp, C.c_char_p, _i64]
 _lib.otoo_measure_fp32_peak.argtypes = [_vp, C.POINTER(C.c_double), _vp]
+_lib.otoo_unsort.argtypes = [_vp, _vp, _vp, _vp]
 _lib.otoo_probe.argtypes = [_vp, C.c_char_p, C.c_char_p, _i64, _vp]
 _lib.otoo_gravity_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _i32, _vp]
 _lib.otoo_gravity_delta_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _f, _i32, _vp]
@@ -200,6 +201,13 @@ class Otoo:
                                         int(group_size), self._p(out), self._stream(stream)))
         return out
 
+    def otoo_unsort(self, sorted_rows, out=None, stream=None):
+        """rows (N,4) in sorted order -> the caller's particle order"""
+        if out is None:
+            out = torch.empty((self.N, 4), dtype=torch.float32, device=self._dev())
+        self._check(_lib.otoo_unsort(self._h, self._p(sorted_rows, torch.float32, 4), self._p(out, torch.float32, 4), self._stream(stream)))
+        return out
+
     def otoo_eos_ideal(self, rho, u, gamma=5.0 / 3.0, stream=None):
         P = torch.empty_like(rho)
         self._check(_lib.otoo_eos_ideal(self._h, _ptr(rho, torch.float32), _ptr(u, torch.float32), float(gamma),
@@ -254,11 +262,14 @@ class Otoo:
         self._check(_lib.otoo_export_sph_radii(self._h, b.data_ptr(), r.data_ptr()))
         return b.cpu().numpy(), r.cpu().numpy()
 
-    def otoo_export_group_stats(self):
+    def otoo_export_group_stats(self, on_device=False):
+        """(n_tests, n_cells, n_parts) per group of the last walk: numpy uint32 arrays, or int32 CUDA tensors"""
         st = self.otoo_last_stats()
         ng = st["n_groups"]
         a = [torch.empty(ng, dtype=torch.int32, device=self._dev()) for _ in range(3)]
         self._check(_lib.otoo_export_group_stats(self._h, a[0].data_ptr(), a[1].data_ptr(), a[2].data_ptr()))
+        if on_device:
+            return tuple(a)
         return tuple(x.cpu().numpy().view(np.uint32) for x in a)
 
     def otoo_last_stats(self):

@@ -35,6 +35,12 @@ __global__ void __launch_bounds__(256) export_sph_kernel(int64_t ncell, const fl
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c < ncell) { float2 v = in[c]; if (b) b[c] = v.x; if (r) r[c] = v.y; }
 }
+// out[perm[s]] = in[s]: rows in sorted order back into the caller's order (the inverse of the build's gather)
+__global__ void __launch_bounds__(256) unsort4_kernel(const float4* __restrict__ in, const uint32_t* __restrict__ perm, int64_t n,
+                                                      float4* __restrict__ out) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n) out[perm[s]] = in[s];
+}
 __global__ void __launch_bounds__(256) eos_ideal_kernel(const float* __restrict__ rho, const float* __restrict__ u, float gm1,
                                                         int64_t n, float* __restrict__ P) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -168,6 +174,7 @@ otoo_status otoo_gravity_delta(otoo_ctx* ctx, float eps, float delta, float m_li
 }
 
 static otoo_status sph_scratch(otoo_ctx* ctx) {
+  if (ctx->out_sorted) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "option output_sorted applies to the gravity calls only");
   if (!ctx->sorted_h) {
     OTOO_TRY(dalloc(ctx, &ctx->sorted_h, (size_t)ctx->maxN));
     OTOO_TRY(dalloc(ctx, &ctx->sorted_aux, (size_t)ctx->maxN));
@@ -246,6 +253,18 @@ otoo_status otoo_eos_ideal(otoo_ctx* ctx, const float* d_rho, const float* d_u, 
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
   eos_ideal_kernel<<<(unsigned)cdiv(N, 256), 256, 0, (cudaStream_t)stream>>>(d_rho, d_u, gamma - 1.0f, N, d_P);
   ctx->launches = 1;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  return OTOO_OK;
+}
+
+otoo_status otoo_unsort(otoo_ctx* ctx, const float* d_sorted_rows, float* d_out, void* stream) {
+  if (!ctx) return OTOO_ERR_INVALID_ARG;
+  if (!ctx->built) return otoo_fail(ctx, OTOO_ERR_NOT_BUILT, "otoo_build_tree has not succeeded");
+  if (!d_sorted_rows || !d_out || d_sorted_rows == d_out) return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "two distinct non-NULL buffers required");
+  OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
+  unsort4_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<const float4*>(d_sorted_rows), ctx->val[0],
+                                                                               ctx->N, reinterpret_cast<float4*>(d_out));
+  ctx->launches = 1; ctx->last_stream = (cudaStream_t)stream;
   OTOO_CUDA(ctx, cudaGetLastError());
   return OTOO_OK;
 }
@@ -377,6 +396,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     ctx->dist_kind = (int)value;
     return OTOO_OK;
   }
+  if (strcmp(name, "output_sorted") == 0) { ctx->out_sorted = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_profile") == 0) { ctx->walk_profile = value != 0; return OTOO_OK; }
   if (strcmp(name, "warp_specialized") == 0) { ctx->use_ws = value != 0; return OTOO_OK; }

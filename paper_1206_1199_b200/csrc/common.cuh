@@ -104,6 +104,7 @@ struct otoo_ctx {
   int use_pool;          // option "task_pool"
   int64_t group_begin, group_count;   // options: the walks cover groups [begin, begin + count) only (count < 0: to the end)
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
+  int out_sorted;        // option "output_sorted": otoo_gravity / otoo_gravity_delta write row s of the output for sorted slot s
   int walk_only;         // option "walk_only" (diagnostic)
   int walk_profile;      // option "walk_profile": the gravity walk kernel counts its warps' waiting time (slower)
   int dist_kind;         // option "group_distance": 0 AABB (R8), 1 exact minimum over the group's members (R23)

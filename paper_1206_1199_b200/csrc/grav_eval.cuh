@@ -153,7 +153,7 @@ struct GravVisitor {
       float4 o = (t & 1) ? make_float4(AX[q].y, AY[q].y, AZ[q].y, PH[q].y) : make_float4(AX[q].x, AY[q].x, AZ[q].x, PH[q].x);
       if ((selfmask >> t) & 1u) o.w = __fmaf_rn(pm[t], rie, o.w);
       if (member_ok(p.c, g0, t * 32 + lane)) {
-        float* dst = reinterpret_cast<float*>(p.acc_pot + p.c.perm[s]);
+        float* dst = reinterpret_cast<float*>(p.acc_pot + out_row(p.c, s));
         atomicAdd(dst + 0, o.x); atomicAdd(dst + 1, o.y); atomicAdd(dst + 2, o.z); atomicAdd(dst + 3, o.w);
       }
     }

@@ -329,7 +329,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long), st));
   c->spos = ctx->spos; c->keys = ctx->key[0]; c->cell_cm = ctx->cell_cm; c->cell_b = ctx->cell_b; c->perm = ctx->val[0];
-  c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin; c->gs = G;
+  c->N = ctx->N; c->ngroups = ngroups; c->g_begin = (uint32_t)g_begin; c->gs = G; c->out_sorted = 0;
   c->g_ntests = ctx->g_ntests; c->g_ncells = ctx->g_ncells; c->g_nparts = ctx->g_nparts;
   c->sums = ctx->d_sums; c->ws = (WalkShared*)ctx->walk_shared; c->slots = (TaskSlot*)ctx->pool_slots;
   c->seq = (uint32_t*)ctx->pool_seq; c->spill = ctx->walk_spill; c->stack_cap = ctx->walk_stack; c->spill_cap = ctx->walk_spill_cap;
@@ -361,6 +361,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   if (ctx->dist_kind == 1 && !ctx->use_ws)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_distance = 1 needs warp_specialized = 1");
   p.c.dist_kind = ctx->dist_kind;
+  p.c.out_sorted = ctx->out_sorted;
   OTOO_EV(ctx, ctx->ev_walk[1], st);
   if (ctx->use_ws) {
     switch (G) {

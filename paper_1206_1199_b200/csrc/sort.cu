@@ -22,6 +22,10 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 // + 12 B written per pair and pass), keys ranked in the tile and staged through shared memory so that the
 // global writes are runs of consecutive addresses.
 constexpr int OS_MAXPASS = 8;
+#ifndef OTOO_OS_LOOKBACK
+#define OTOO_OS_LOOKBACK 8
+#endif
+constexpr int OS_LOOKBACK = OTOO_OS_LOOKBACK;      // status words of preceding tiles a thread has in flight
 constexpr uint32_t OS_GHIST = 0;                       // u32 offsets into ctx->hist
 constexpr uint32_t OS_TICKET = OS_MAXPASS * 256;       // one tile ticket counter per pass
 constexpr uint32_t OS_STATUS = OS_TICKET + 256;        // u64 status words [tile][digit] from here (8 B aligned)
@@ -131,13 +135,13 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const uint6
     int64_t t = (int64_t)tile - 1;
     bool done = false;
     while (!done) {
-      unsigned long long w[8];
+      unsigned long long w[OS_LOOKBACK];
 #pragma unroll
-      for (int j = 0; j < 8; j++)
+      for (int j = 0; j < OS_LOOKBACK; j++)
         w[j] = t - j >= 0 ? *(status_v + (size_t)(t - j) * 256 + tid) : os_pack(epoch, 2u, 0u);
       int used = 0;
 #pragma unroll
-      for (int j = 0; j < 8; j++) {
+      for (int j = 0; j < OS_LOOKBACK; j++) {
         if (!done && used == j) {
           const uint32_t state = (uint32_t)(w[j] >> 32) & 3u;
           if ((uint32_t)(w[j] >> 34) == epoch && state != 0u) {

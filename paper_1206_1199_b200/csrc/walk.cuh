@@ -157,6 +157,7 @@ struct WalkCommon {
   unsigned long long* sums;                                    // tests, interactions, cells, parts
   WalkShared* ws; TaskSlot* slots; uint32_t* seq;               // seq[i] initialised to i
   uint32_t* spill;                                              // OTOO_WALK_SPILL per warp
+  int out_sorted;                                               // 1: results are written at the SORTED slot of a target instead of its original index
   int gs;                                                       // group size: 32 * T of the kernel, or 4 / 8 / 16 with T = 1 (the paper's n_vec, L163)
   int stack_cap;
   int spill_cap;                                                // usable entries of a warp's private spill area (<= OTOO_WALK_SPILL)
@@ -168,6 +169,8 @@ struct WalkCommon {
 
 // member idx (0 .. 32 T - 1) of the group starting at slot g0 exists
 __device__ __forceinline__ bool member_ok(const WalkCommon& c, int64_t g0, int idx) { return idx < c.gs && g0 + idx < c.N; }
+// row of the caller's output that belongs to sorted slot s
+__device__ __forceinline__ int64_t out_row(const WalkCommon& c, int64_t s) { return c.out_sorted ? s : (int64_t)c.perm[s]; }
 __device__ __forceinline__ int group_count(const WalkCommon& c, int64_t g0) { const int64_t left = c.N - g0; return (int)(left < c.gs ? left : c.gs); }
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }

@@ -583,3 +583,39 @@ def test_sph_target_sharding_ranges_add_up(otoo, orc, world):
     # (a group finished by several warps through the task pool adds its partial sums in another order)
     assert np.array_equal(nn_s, nn_w) and np.allclose(rho_s, rho_w, rtol=2e-6)
     assert np.allclose(dr_s, dr_w, rtol=1e-4, atol=1e-5 * np.abs(dr_w).max())
+
+
+def test_sorted_output_and_unsort(otoo, orc):
+    """option output_sorted + otoo_unsort (what sharded.ShardedGravity exchanges): a range's results are one contiguous
+    run of rows in sorted order, zero elsewhere; the runs of all ranges side by side, unsorted, are the plain result."""
+    from paper_1206_1199_b200 import sharded, binding
+    n, G = 30000 + 17, 128
+    pm = gen.plummer(n, 12)
+    t = check_tree(otoo, orc, pm, 16)
+    perm = t.export()["perm"].astype(np.int64)
+    whole = otoo.otoo_gravity(0.01, 0.5, G)
+    ng = t.n_groups(G)
+    rows = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    try:
+        otoo.otoo_set_option("output_sorted", 1)
+        srt = otoo.otoo_gravity(0.01, 0.5, G)
+        assert torch.allclose(srt, whole[torch.from_numpy(perm).cuda()], rtol=2e-6, atol=1e-6 * float(whole.abs().max()))
+        for b, c in sharded.group_ranges(ng, 3, np.linspace(1, 5, ng)):
+            otoo.otoo_set_option("group_begin", b)
+            otoo.otoo_set_option("group_count", c)
+            part = otoo.otoo_gravity(0.01, 0.5, G)
+            lo, hi = b * G, min((b + c) * G, n)
+            assert not part[:lo].any() and not part[hi:].any() and bool(part[lo:hi].any())
+            rows[lo:hi] = part[lo:hi]
+        with pytest.raises(binding.OtooError):                        # the SPH calls have no sorted-output form
+            otoo.otoo_sph_density(torch.full((n,), 0.1, device="cuda"), 64)
+    finally:
+        otoo.otoo_set_option("group_begin", 0)
+        otoo.otoo_set_option("group_count", -1)
+        otoo.otoo_set_option("output_sorted", 0)
+    back = otoo.otoo_unsort(rows)
+    assert torch.allclose(back, whole, rtol=2e-6, atol=1e-6 * float(whole.abs().max()))
+    sg = sharded.ShardedGravity(otoo)                                 # world 1: the same path end to end
+    one = sg.gravity(dev(pm), 16, 0.01, 0.5, G)
+    assert torch.allclose(one, whole, rtol=2e-6, atol=1e-6 * float(whole.abs().max()))
+    assert sg.cost is not None and sg.cost.shape[0] == ng and sg.cost.is_cuda

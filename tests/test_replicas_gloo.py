@@ -88,6 +88,7 @@ def test_group_ranges_partition_the_groups():
     by_count = [cost[b:b + c].sum() for b, c in sh.group_ranges(5000, 4)]
     assert max(shares) <= max(by_count) * 1.0001
     assert sh.group_ranges(6, 3, np.zeros(6)) == sh.group_ranges(6, 3)
+    assert sh.group_ranges(5000, 4, torch.from_numpy(cost)) == r                      # a tensor cost: same cuts
 
 
 def _shard_worker(rank, world, port, q):
@@ -97,12 +98,21 @@ def _shard_worker(rank, world, port, q):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     sh = _load_sharded()
     n_groups, G = 37, 4
-    full = torch.arange(n_groups * G * 4, dtype=torch.float32).reshape(-1, 4) + 1.0   # what one GPU would compute
+    n = n_groups * G - 1                                                               # ragged last group
+    full = torch.arange(n * 4, dtype=torch.float32).reshape(-1, 4) + 1.0              # what one GPU would compute (sorted order)
+    ok = True
+    for cost in (None, np.linspace(1.0, 9.0, n_groups)):                               # equal counts; unequal, cost-balanced ranges
+        ranges = sh.group_ranges(n_groups, world, cost)
+        b, c = ranges[rank]
+        rows = [(rb * G, min((rb + rc) * G, n)) for rb, rc in ranges]
+        local = torch.full_like(full, -7.0)                                            # rows of the other ranks: ignored garbage
+        local[rows[rank][0]:rows[rank][1]] = full[rows[rank][0]:rows[rank][1]]         # this rank's targets only
+        ok = ok and bool(torch.equal(sh.gather_ranges(local, rows), full))
+        lengths = torch.zeros(n_groups)
+        lengths[b:b + c] = torch.arange(b, b + c, dtype=torch.float32) + 1.0           # per-group cost, zero outside the range
+        ok = ok and bool(torch.equal(sh.combine(lengths), torch.arange(n_groups, dtype=torch.float32) + 1.0))
     b, c = sh.group_ranges(n_groups, world)[rank]
-    local = torch.zeros_like(full)
-    local[b * G:(b + c) * G] = full[b * G:(b + c) * G]                                # this rank's targets only
-    got = sh.combine(local)
-    q.put((rank, bool(torch.equal(got, full)), (b, c)))
+    q.put((rank, ok, (b, c)))
     dist.destroy_process_group()
 
 
