@@ -152,28 +152,46 @@ __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restr
                                                          uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
                                                          uint32_t* __restrict__ level_count) {
   __shared__ uint32_t lc[OTOO_NLEV];
-  __shared__ signed char cw[256 + OTOO_SLOT_NCRIT_MAX];
+  __shared__ signed char cwa[256 + OTOO_SLOT_NCRIT_MAX], cwb[256 + OTOO_SLOT_NCRIT_MAX];
   const int64_t s0 = (int64_t)blockIdx.x * 256;
+  const int m = 256 + n_crit;                       // window starts t = s0 - n_crit + i, i < m
   if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
-  for (int i = threadIdx.x; i < 256 + n_crit; i += 256) {
+  for (int i = threadIdx.x; i < m; i += 256) {
     const int64_t t = s0 - n_crit + i;
-    cw[i] = (t >= 0 && t <= n - n_crit - 1) ? (signed char)cplev(key[t], key[t + n_crit]) : (signed char)-1;
+    cwa[i] = (t >= 0 && t <= n - n_crit - 1) ? (signed char)cplev(key[t], key[t + n_crit]) : (signed char)-1;
   }
   __syncthreads();
+  // D(s) = max of the n_crit + 1 consecutive values cw[tid .. tid + n_crit]: doubling (m_k[i] = max of 2^k values from
+  // i) up to the largest power of two <= n_crit + 1, then two overlapping spans cover the window
+  const int w = n_crit + 1;
+  signed char *src = cwa, *dst = cwb;
+  int span = 1;
+  while (2 * span <= w) {
+    for (int i = threadIdx.x; i < m; i += 256) {
+      const signed char a = src[i], b = i + span < m ? src[i + span] : (signed char)-1;
+      dst[i] = a > b ? a : b;
+    }
+    __syncthreads();
+    signed char* tmp = src; src = dst; dst = tmp;
+    span *= 2;
+  }
   const int64_t s = s0 + threadIdx.x;
-  int lo = 1, LL = 0;   // empty level range for threads past the end
+  int lo = OTOO_NLEV, LL = -1;   // empty level range for threads past the end
   if (s < n) {
     const int cpl = (s == 0) ? -1 : cplev(key[s - 1], key[s]);
-    int D = -1;
-    for (int i = 0; i <= n_crit; i++) { const int c = cw[threadIdx.x + i]; D = c > D ? c : D; }
+    const signed char a = src[threadIdx.x], b = src[threadIdx.x + w - span];
+    const int D = a > b ? a : b;
     LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
     lo = cpl + 1;
     int nc = LL - cpl; if (nc < 0) nc = 0;
     slot_nc[s] = (uint32_t)nc;
     info[s] = (uint32_t)lo | ((uint32_t)LL << 8);
   }
-#pragma unroll
-  for (int l = 0; l < OTOO_NLEV; l++) {
+  // per-level counts, warp-aggregated: only the levels some lane of the warp starts a cell at (a few around the
+  // local leaf level, not all 22)
+  const bool has = lo <= LL;
+  const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
+  for (int l = wlo; l <= whi; l++) {
     const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
     if (b && (threadIdx.x & 31) == 0) atomicAdd(&lc[l], (uint32_t)__popc(b));
   }
@@ -322,12 +340,19 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, const Moment
 }
 // the whole bottom-up pass in ONE cooperative launch: every level deepest first, a grid-wide barrier
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
-__global__ void __launch_bounds__(256) moments_all_kernel(const LevelOff off, const int depth, const MomentArgs a) {
+// Levels 0 .. top are narrow (the top of the tree: 1, 8, 64, ... cells): one CTA finishes them with block barriers
+// instead of grid barriers.
+__global__ void __launch_bounds__(256) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
-  for (int l = depth; l >= 0; l--) {
+  for (int l = depth; l > top; l--) {
     for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) moments_cell(c, l, a);
-    if (l > 0) grid.sync();
+    grid.sync();
+  }
+  if (blockIdx.x != 0) return;
+  for (int l = top < depth ? top : depth; l >= 0; l--) {
+    for (uint32_t c = off.v[l] + threadIdx.x; c < off.v[l + 1]; c += blockDim.x) moments_cell(c, l, a);
+    __syncthreads();
   }
 }
 
@@ -477,8 +502,9 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
     uint32_t widest = 1;
     for (int l = 0; l <= depth; l++) if (off.v[l + 1] - off.v[l] > widest) widest = off.v[l + 1] - off.v[l];
     if (grid > cdiv(widest, 256)) grid = cdiv(widest, 256);
-    int depth_arg = depth;
-    void* args[] = {(void*)&off, (void*)&depth_arg, (void*)&ma};
+    int depth_arg = depth, top = -1;
+    while (top + 1 <= depth && off.v[top + 2] - off.v[top + 1] <= 256u) top++;       // levels 0 .. top hold <= 256 cells each (one per thread)
+    void* args[] = {(void*)&off, (void*)&depth_arg, (void*)&top, (void*)&ma};
     OTOO_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)moments_all_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
     ctx->launches += 1;
   }
