@@ -287,7 +287,7 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
         # BASELINE config 4 / the paper's cold collapse: the SPH rows (H11-H13) on the same tree, timed like the gravity step
         w = (gen.wd_pair if cfg["kind"] == "wd_pair" else gen.cold_sphere)(n, seed)
         d_h, d_u, d_v = (torch.from_numpy(w[k]).cuda() for k in ("h", "u", "vel"))
-        Gs = cfg.get("group_sph", 64)
+        Gs = args.group_sph if args.group_sph else cfg.get("group_sph", 64)
         ts, ks = [], []
         for it in range(3 + steps):
             flush_buf.fill_(1)
@@ -296,10 +296,14 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
             rho, nn = o.otoo_sph_density(d_h, Gs)
             P = o.otoo_eos_ideal(rho, d_u, 5.0 / 3.0)
             ev[1].record()
-            k1 = o.otoo_last_stats()["ms_walk_force"]
+            s1 = o.otoo_last_stats()
+            k1 = s1["ms_walk_force"]
+            o.otoo_set_option("sph_reuse_radii", 1)     # h is fixed within a step: stage 2 keeps stage 1's Eq. 5 radii
             o.otoo_sph_force(d_h, rho, P, Gs, vel=d_v)
+            o.otoo_set_option("sph_reuse_radii", 0)
             ev[2].record()
-            k2 = o.otoo_last_stats()["ms_walk_force"]
+            s2 = o.otoo_last_stats()
+            k2 = s2["ms_walk_force"]
             torch.cuda.synchronize()
             if it >= 3:
                 ts.append((ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])))
@@ -310,15 +314,18 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
         pairs = int(nn.sum().item())
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
         peak = sm_count * SM_LANES * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
-        ops_d = SPH_FLOP_TEST["density"] * cand + SPH_FLOP_HIT["density"] * pairs
-        ops_f = SPH_FLOP_TEST["force"] * cand + SPH_FLOP_HIT["force"] * pairs
+        # pair tests actually made: the candidates left after the walk-time cull (otoo_stats_t.sum_evaluated), not the
+        # paper's whole list -- the flops of skipped tests are not counted as achieved
+        ev_d, ev_f = s1["sum_evaluated"], s2["sum_evaluated"]
+        ops_d = SPH_FLOP_TEST["density"] * ev_d + SPH_FLOP_HIT["density"] * pairs
+        ops_f = SPH_FLOP_TEST["force"] * ev_f + SPH_FLOP_HIT["force"] * pairs
         res["sph"] = {"group": Gs, "density_eos_ms": td, "force_dudt_ms": tf, "density_kernel_ms": kd, "force_kernel_ms": kf,
-                      "candidate_pairs_per_pass": cand, "neighbour_pairs": pairs, "candidate_pairs_per_s": 2 * cand / ((td + tf) * 1e-3),
+                      "candidate_pairs_per_pass": cand, "evaluated_pair_tests": {"density": ev_d, "force_dudt": ev_f}, "neighbour_pairs": pairs, "candidate_pairs_per_s": 2 * cand / ((td + tf) * 1e-3),
                       "roofline": {"bound": "alu", "peak": peak, "unit": "TFLOP/s",
                                    "density": {"achieved": ops_d / (kd * 1e-3) / 1e12, "frac": ops_d / (kd * 1e-3) / 1e12 / peak},
                                    "force_dudt": {"achieved": ops_f / (kf * 1e-3) / 1e12, "frac": ops_f / (kf * 1e-3) / 1e12 / peak},
-                                   "flops": f"instruction-counted: {SPH_FLOP_TEST['density']} / {SPH_FLOP_TEST['force']} flop per candidate pair "
-                                            f"(the paper's list: every particle of every opened leaf) + {SPH_FLOP_HIT['density']} / "
+                                   "flops": f"instruction-counted: {SPH_FLOP_TEST['density']} / {SPH_FLOP_TEST['force']} flop per pair test made "
+                                            f"(candidates left after the walk-time cull) + {SPH_FLOP_HIT['density']} / "
                                             f"{SPH_FLOP_HIT['force']} per neighbour pair (density / force + du/dt)",
                                    "paper_convention_200flop_tflops": 200.0 * 2 * pairs / ((kd + kf) * 1e-3) / 1e12,
                                    "note": "the paper's 200 flop per SPH interaction (L254) counts its viscosity and overstates these kernels"}}
@@ -369,6 +376,7 @@ def main():
     ap.add_argument("--m-limit", type=float, default=None)
     ap.add_argument("--seed", type=int, default=1206)
     ap.add_argument("--n", type=int, default=None, help="override the workload's particle count (scaling runs, e.g. Fig. 9)")
+    ap.add_argument("--group-sph", type=int, default=None, help="group size of the SPH rows (C4 / COLD; default: the workload's, 64)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the C2 / C3 / C4 blocks of the default line")
     ap.add_argument("--probe", default=None, choices=["ffma2", "sumloop"],

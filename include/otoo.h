@@ -61,6 +61,8 @@ typedef struct {
   uint64_t sum_steps;        /* walk steps (batches of <= 32 MAC tests) of the last walk */
   uint64_t sum_tasks;        /* units of work run: groups + task-pool tasks */
   uint64_t sum_flushes;      /* evaluations of a (full or final) shared-memory list */
+  uint64_t sum_evaluated;    /* (target, list entry) pairs actually handed to the sums: = sum_interactions for gravity;
+                              * for the SPH walks the candidates left after the walk-time cull, times the group size */
   /* Per-phase DEVICE times in ms (CUDA events on the call's stream; PAPER.md L195, L212 splits a step into TREE
    * and KERNEL the same way).  ms_build[] of the last otoo_build_tree: [0] root cube (H1), [1] keys (H2),
    * [2] key sort (H3), [3] gather (H4), [4] cells from the sorted keys (H5, includes the one host
@@ -224,6 +226,9 @@ otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_
  * "warp_specialized_sph" = 0 (default): the SPH kernels let one warp walk and sum in turn; 1: walker/evaluator
  * pairs as for gravity (SPH lists are short, the walkers become the bottleneck: faster only for
  * group_size >= 128).
+ * "sph_reuse_radii" = 1: an SPH call keeps the sorted smoothing lengths and the Eq. 5 cell radii of the previous SPH
+ * call on the same tree instead of recomputing them: the caller states that d_h has not changed since (stage 2 after
+ * stage 1 of one step, PAPER.md L252 steps 4 and 6).  A new tree or otoo_gravity_delta invalidates them.  Default 0.
  * "output_sorted" = 1: otoo_gravity / otoo_gravity_delta write row s of d_acc_pot for the target at SORTED slot s
  * (otoo_export_tree's d_perm names its original index) instead of the caller's order; with a group range the rows
  * [group_begin * group_size, ...) of the range are the only non-zero ones and are contiguous.  otoo_unsort brings

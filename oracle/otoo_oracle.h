@@ -11,16 +11,19 @@
  * every sum is fp64; the quantities that decide an integer (key quantisation, the MAC compare,
  * the SPH neighbour compare) are evaluated in fp32 exactly as DESIGN.md states.
  *
- * Pins (tests/test_oracle_*.py): brute-force octants, stable sort, tree invariants, two-particle
- * cell, tiling invariant of the lists, stackless walk == recursive walk,
- * theta=0 == direct sum, Newton's third law, two-body closed form, Plummer potential, kernel
- * normalisation, lattice density, brute-force SPH neighbour sets; Delta-MAC: two-particle cell and
- * Eq. 3, B2 bottom-up == Eq. 2 direct, per-cell error <= Delta, r_b limits (L81);
- * exact-minimum group distance (L163): brute force over members, lists never longer than the box lists;
- * Hilbert keys (L131): bijection, face adjacency of consecutive keys, hierarchy, inverse, same cells as
- * the Morton tree; adaptive h: fixed point, lattice count steps; div v / rot v: linear fields, rigid
- * rotation; artificial viscosity: alpha = 0 / f = 0 limits, receding flow, momentum and energy balance,
- * two-particle closed form.
+ * Pins (tests/test_oracle_*.py, tests/test_golden.py): brute-force octants, stable sort, tree invariants, two-particle
+ * cell, r_b = l/theta + s on a three-particle tree done by hand, tiling invariant of the lists, stackless
+ * walk == recursive walk, theta=0 == direct sum, Newton's third law, two-body closed form, Plummer
+ * potential, kernel normalisation, lattice density, brute-force SPH neighbour sets; the abs_sum outputs (the
+ * denominators of the GPU parity tolerance) against numpy sums over the exported lists / all pairs, one-pair closed
+ * forms and |sum| <= sum of magnitudes; Delta-MAC: two-particle cell and Eq. 3, B2 bottom-up == Eq. 2
+ * direct, per-cell error <= Delta, r_b limits (L81), measured Delta exponents at n_vec = 4 / 8; group distance from
+ * the pieces' boxes (R25, default) and the exact minimum (L163; R23): brute force over pieces / members with the
+ * pieces recomputed from the exported keys, lists nested exact <= pieces <= one box; SPH walk per piece (R26): same
+ * neighbours, brute-force supersets; Hilbert keys (L131): bijection, face adjacency of consecutive keys, hierarchy,
+ * inverse, same cells as the Morton tree; adaptive h: fixed point, lattice count steps; div v / rot v: linear
+ * fields, rigid rotation; artificial viscosity: alpha = 0 / f = 0 limits, receding flow, momentum and energy
+ * balance, two-particle closed form.
  * parity unpinned: the absolute accuracy level of the theta-MAC (the paper's error plot, Fig. 5,
  * is for its Delta-MAC and is missing from PAPER.md).
  */

@@ -38,7 +38,7 @@ class Stats(C.Structure):
     _fields_ = [("sum_tests", C.c_uint64), ("sum_interactions", C.c_uint64), ("sum_cells", C.c_uint64),
                 ("sum_parts", C.c_uint64), ("n_groups", C.c_int64), ("group_size", C.c_int32),
                 ("launches", C.c_int32), ("sum_steps", C.c_uint64), ("sum_tasks", C.c_uint64),
-                ("sum_flushes", C.c_uint64), ("ms_build", C.c_float * 8), ("ms_build_total", C.c_float),
+                ("sum_flushes", C.c_uint64), ("sum_evaluated", C.c_uint64), ("ms_build", C.c_float * 8), ("ms_build_total", C.c_float),
                 ("ms_walk_prep", C.c_float), ("ms_walk_force", C.c_float), ("ms_total", C.c_float),
                 ("walk_sm_mhz", C.c_float), ("eval_wait_frac", C.c_float), ("walker_wait_frac", C.c_float),
                 ("walker_idle_frac", C.c_float), ("walk_only", C.c_int32), ("error_flag", C.c_int32)]

@@ -337,7 +337,7 @@ otoo_status otoo_last_stats(otoo_ctx* ctx, otoo_stats_t* o) {
     if (h[12]) o->eval_wait_frac = (float)((double)h[10] / (double)h[12]);
     if (h[13]) { o->walker_wait_frac = (float)((double)h[11] / (double)h[13]); o->walker_idle_frac = (float)((double)h[14] * 0.4e-6 * 1e9 * (h[9] ? (double)h[8] / (double)h[9] : 1.965) / (double)h[13]); }
     o->sum_tests = h[0]; o->sum_interactions = h[1]; o->sum_cells = h[2]; o->sum_parts = h[3];
-    o->sum_steps = h[4]; o->sum_tasks = h[5]; o->sum_flushes = h[6];
+    o->sum_steps = h[4]; o->sum_tasks = h[5]; o->sum_flushes = h[6]; o->sum_evaluated = h[15];
     o->error_flag = (int32_t)h[7];
     o->n_groups = ctx->last_ngroups; o->group_size = ctx->last_group_size;
     o->walk_only = ctx->last_walk_only;
@@ -396,6 +396,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     ctx->dist_kind = (int)value;
     return OTOO_OK;
   }
+  if (strcmp(name, "sph_reuse_radii") == 0) { ctx->sph_reuse = value != 0; return OTOO_OK; }
   if (strcmp(name, "output_sorted") == 0) { ctx->out_sorted = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_profile") == 0) { ctx->walk_profile = value != 0; return OTOO_OK; }

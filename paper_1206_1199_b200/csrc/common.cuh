@@ -81,7 +81,8 @@ struct otoo_ctx {
   uint32_t* walk_spill;  // OTOO_WALK_SPILL entries per resident warp
   int64_t spill_warps;
   unsigned long long* d_sums; // OTOO_NSUMS words: [0] tests [1] interactions [2] cells [3] parts [4] steps [5] tasks [6] flushes
-                              // [7] error flag [8] SM clock ticks and [9] ns spent by the CTAs of the walk kernel
+                              // [7] error flag [8] SM clock ticks and [9] ns spent by the CTAs of the walk kernel [10..14] waiting
+                              // times of the profiled kernel [15] (target, entry) pairs handed to the sums
   void* pool_slots;      // task pool (walk.cuh): TaskSlot[OTOO_POOL_SLOTS]
   void* pool_seq;        // uint32 sequence numbers
   void* walk_shared;     // WalkShared control block
@@ -105,6 +106,7 @@ struct otoo_ctx {
   int64_t group_begin, group_count;   // options: the walks cover groups [begin, begin + count) only (count < 0: to the end)
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int out_sorted;        // option "output_sorted": otoo_gravity / otoo_gravity_delta write row s of the output for sorted slot s
+  int sph_reuse;         // option "sph_reuse_radii": SPH calls keep sorted h and the Eq. 5 radii of the previous SPH call on this tree
   int walk_only;         // option "walk_only" (diagnostic)
   int walk_profile;      // option "walk_profile": the gravity walk kernel counts its warps' waiting time (slower)
   int dist_kind;         // option "group_distance": 0 AABB (R8), 1 exact minimum over the group's members (R23)

@@ -114,13 +114,14 @@ double run_ffma2(otoo_ctx* ctx, const f32x2* in, f32x2* out, unsigned long long*
 }
 
 template <int T, int PB, int UNR>
-otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long long* d_cyc, cudaStream_t st, std::string& js) {
+otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long long* d_cyc, cudaStream_t st, std::string& js,
+                        int per_sm_arg = 0) {
   const int reps = 256;
   int occ = 0;
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR>, 128, 0));
   cudaFuncAttributes fa;
   OTOO_CUDA(ctx, cudaFuncGetAttributes(&fa, sumloop_probe_kernel<T, PB, UNR>));
-  const int per_sm = T >= 8 ? 2 : 3;                    // evaluator warps per SM of the product kernel: 4 x this
+  const int per_sm = per_sm_arg ? per_sm_arg : (T >= 8 ? 2 : 3);   // CTAs of 4 evaluator warps per SM (default: the product kernel's)
   const int grid = ctx->sm_count * per_sm;
   // dynamic shared memory sized so that EXACTLY per_sm CTAs fit an SM: every SM then runs per_sm CTAs of the
   // grid at once (left to the occupancy of the kernel alone the block scheduler packs 4 on some SMs and 2 on others)
@@ -147,8 +148,11 @@ otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long
   cyc /= n; ns /= n;
   const double sm_mhz = 1e3 * cyc / ns;                  // SM clock held during the loop: clock64 ticks per globaltimer ns
   const double inter = (double)grid * 4 * 32 * T * OTOO_LIST_CAP * reps;
-  // SMSP cycles per (target pair, list entry): every SMSP ran per_sm warps x NP pairs x entries x reps
-  const double per_pair = cyc / ((double)per_sm * ((T + 1) / 2) * OTOO_LIST_CAP * reps);
+  // SMSP cycles per (target pair, list entry) from the kernel's duration at the clock it held: every SMSP ran per_sm
+  // warps x NP pairs x entries x reps (the CTAs' own tick counts are not used for this: the scheduler favours some
+  // warps, so a CTA's mean is below the kernel's)
+  (void)cyc;
+  const double per_pair = (double)best * 1e-3 * sm_mhz * 1e6 / ((double)per_sm * ((T + 1) / 2) * OTOO_LIST_CAP * reps);
   char buf[512];
   snprintf(buf, sizeof buf,
            "{\"name\": \"sumloop G=%d\", \"pairs_per_pass\": %d, \"unroll\": %d, \"eval_warps_per_sm\": %d, \"registers\": %d, \"occupancy_ctas\": %d, \"ms\": %.4f, "
@@ -193,7 +197,8 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
     memset(&p, 0, sizeof p);
     p.c.spos = ctx->spos; p.c.N = n; p.c.gs = 256; p.eps2 = 1e-6f;
     float4* sink = reinterpret_cast<float4*>(ctx->key[1]) + 4096;
-    // the product's configuration first (pairs per pass = min(NP, 2), unroll OTOO_EVAL_UNR), then the variants tried
+    // the product's three configurations (pairs per pass = min(NP, 2), unroll OTOO_EVAL_UNR, 12 / 12 / 8 evaluator
+    // warps per SM), then what was tried: other unroll factors and pairs per pass, more or fewer warps per SM
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<8, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js)));
@@ -201,11 +206,13 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
     OTOO_TRY((run_sumloop<4, 2, 2>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<4, 2, 8>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<4, 1, 4>(ctx, p, sink, d_cyc, st, js)));
-    OTOO_TRY((run_sumloop<8, 2, 1>(ctx, p, sink, d_cyc, st, js)));
-    OTOO_TRY((run_sumloop<8, 2, 2>(ctx, p, sink, d_cyc, st, js)));
-    OTOO_TRY((run_sumloop<8, 4, 1>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<8, 4, 2>(ctx, p, sink, d_cyc, st, js)));
     OTOO_TRY((run_sumloop<8, 1, 4>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 1)));
+    OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 2)));
+    OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
+    OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
+    OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 5)));
   } else return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown probe (ffma2, sumloop)");
   js = "[" + js + "]";
   if ((int64_t)js.size() + 1 > cap) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "probe output buffer too small");

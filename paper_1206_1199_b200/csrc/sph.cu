@@ -682,13 +682,17 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p->c, grid, smem, st));
   const unsigned nbN = (unsigned)cdiv(ctx->N, 256), nbC = (unsigned)cdiv(ctx->N_cell, 256);
-  // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3)
-  gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
-  sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->c_first, ctx->c_count, ctx->c_child_first,
-                                        ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
-  sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
-  ctx->launches += 3;
+  // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3) unless the
+  // caller says h has not changed since the previous SPH call on this tree (option "sph_reuse_radii": stage 2 of a
+  // step after stage 1, L252 steps 4 and 6)
+  if (!(ctx->sph_reuse && ctx->sph_radii_valid)) {
+    gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
+    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
+    sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->c_first, ctx->c_count, ctx->c_child_first,
+                                          ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
+    sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
+    ctx->launches += 3;
+  }
   p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->svis = nullptr; p->c_sph = ctx->c_sph;
   p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
   p->pieces = ctx->dist_kind == 2;

@@ -198,7 +198,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   constexpr int PADTO = 4;
   uint32_t* gspill = c.spill + gwarp * OTOO_WALK_SPILL;
   unsigned long long tot_tests = 0, tot_inter = 0, tot_cells = 0, tot_parts = 0;
-  unsigned long long tot_steps = 0, tot_tasks = 0, tot_flushes = 0;
+  unsigned long long tot_steps = 0, tot_tasks = 0, tot_flushes = 0, tot_eval = 0;
   uint32_t idle_polls = 0;          // 400 ns sleeps of this warp while it waited for a pool task
   bool main_done = false, have_ticket = false;
   uint32_t my_ticket = 0;
@@ -250,9 +250,10 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     const int gcount = (int)((c.N - g0) < G ? (c.N - g0) : G);
     v.load_group(g0, lane, list);   // the list is empty here: usable as scratch
     int gsp = 0, nlist = 0;
-    uint32_t ntests = 0, ncells = 0, nparts = 0, iter = 0, nflush = 0;
+    uint32_t ntests = 0, ncells = 0, nparts = 0, iter = 0, nflush = 0, nkept = 0;   // nkept: list entries handed to the sums (after a cull)
 
     auto flush = [&](bool last = false) {
+      nkept += (uint32_t)nlist;
       const int np = (nlist + PADTO - 1) & ~(PADTO - 1);
       if (lane < np - nlist) v.pad(list + V::E * (nlist + lane));
       __syncwarp();
@@ -463,6 +464,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     tot_tests += ntests; tot_cells += ncells; tot_parts += nparts;
     tot_steps += iter; tot_tasks += 1; tot_flushes += nflush;
     tot_inter += (unsigned long long)gcount * (ncells + nparts);
+    tot_eval += (unsigned long long)gcount * nkept;
   }
   if (lane == 0 && tot_tests) {
     atomicAdd(c.sums + 0, tot_tests); atomicAdd(c.sums + 1, tot_inter);
@@ -470,6 +472,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     atomicAdd(c.sums + 3, tot_parts);
     atomicAdd(c.sums + 4, tot_steps); atomicAdd(c.sums + 5, tot_tasks);
     atomicAdd(c.sums + 6, tot_flushes);
+    atomicAdd(c.sums + 15, tot_eval);
   }
   if (lane == 0 && idle_polls) atomicAdd(c.sums + 14, (unsigned long long)idle_polls);
 }

@@ -279,7 +279,15 @@ def _sph_parity(otoo, orc, n, G, dist=2):
     for v in (None, vel):
         rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=v)
         reff = rf["acc_dudt"]
-        out = otoo.otoo_sph_force(dev(h), rho, P, G, vel=None if v is None else dev(v)).cpu().numpy()
+        otoo.otoo_set_option("sph_reuse_radii", 0 if v is None else 1)     # second pass: keep the radii of the first
+        try:
+            out = otoo.otoo_sph_force(dev(h), rho, P, G, vel=None if v is None else dev(v)).cpu().numpy()
+        finally:
+            otoo.otoo_set_option("sph_reuse_radii", 0)
+        if v is not None:
+            assert otoo.otoo_last_stats()["launches"] < launches_plain
+        else:
+            launches_plain = otoo.otoo_last_stats()["launches"]
         # pressure forces cancel pairwise: same bound as gravity, max(1e-5 |a|, 8 u sum_j |a_ij|) (R12)
         e, raw = acc_err(out, reff, rf["abs_sum"][:, 0], pct=99, what="a_sph")
         assert e.max() <= TOL, e.max()
@@ -619,3 +627,28 @@ def test_sorted_output_and_unsort(otoo, orc):
     one = sg.gravity(dev(pm), 16, 0.01, 0.5, G)
     assert torch.allclose(one, whole, rtol=2e-6, atol=1e-6 * float(whole.abs().max()))
     assert sg.cost is not None and sg.cost.shape[0] == ng and sg.cost.is_cuda
+
+
+def test_walk_profile_and_evaluated_counters(otoo, orc):
+    """option walk_profile: the instrumented instantiation of the gravity kernel gives the same counters and fills the
+    waiting-time fractions; sum_evaluated = interactions for gravity and <= the candidates for the culled SPH walks."""
+    pm = gen.plummer(300000, 9)
+    otoo.otoo_build_tree(dev(pm), 16)
+    a = otoo.otoo_gravity(0.01, 0.6, 128)
+    s0 = otoo.otoo_last_stats()
+    assert s0["eval_wait_frac"] == 0 and s0["walker_wait_frac"] == 0 and s0["sum_evaluated"] == s0["sum_interactions"]
+    otoo.otoo_set_option("walk_profile", 1)
+    try:
+        b = otoo.otoo_gravity(0.01, 0.6, 128)
+        s1 = otoo.otoo_last_stats()
+    finally:
+        otoo.otoo_set_option("walk_profile", 0)
+    assert s1["sum_interactions"] == s0["sum_interactions"] and s1["sum_tests"] == s0["sum_tests"]
+    assert 0 < s1["eval_wait_frac"] < 0.5 and 0 < s1["walker_wait_frac"] < 1 and 0 <= s1["walker_idle_frac"] < 0.5
+    assert 1000 < s1["walk_sm_mhz"] < 2500
+    assert torch.allclose(a, b, rtol=2e-6, atol=1e-6 * float(a.abs().max()))
+    w = gen.wd_pair(50000, 3)
+    otoo.otoo_build_tree(dev(w["pos_mass"]), 16)
+    otoo.otoo_sph_density(dev(w["h"]), 64)
+    s2 = otoo.otoo_last_stats()
+    assert 0 < s2["sum_evaluated"] < s2["sum_interactions"]
