@@ -2,6 +2,9 @@
 // (PAPER.md III-D L159-L167, L43, L57; readings R7-R11).
 #include "grav_eval.cuh"
 
+#ifndef OTOO_WALKER_BACKOFF
+#define OTOO_WALKER_BACKOFF 500     // ns of __nanosleep between two polls of a walker waiting for a free list buffer
+#endif
 #ifndef OTOO_WS_MINB
 #define OTOO_WS_MINB 3
 #define OTOO_WS_EVAL_REGS 112
@@ -84,7 +87,7 @@ struct GravWalker {
   __device__ __forceinline__ float4* acquire() {     // wait until the evaluator has released buffer `buf`
     long long w0 = 0;
     if (PROF) w0 = clock64();
-    mbar_wait<500>(&sm.empty[buf], (eparity >> buf) & 1u);   // walkers run ahead: wait without stealing issue slots
+    mbar_wait<OTOO_WALKER_BACKOFF>(&sm.empty[buf], (eparity >> buf) & 1u);   // walkers run ahead: wait without stealing issue slots
     if (PROF) wait_ticks += clock64() - w0;
     eparity ^= 1u << buf;
     return sm.list[buf];
