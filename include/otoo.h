@@ -196,7 +196,8 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
  * which = "ffma2": SM sub-partition cycles per FFMA2 warp instruction for the operand patterns of the sum loop;
  * "sumloop": the product's own pair-sum loop on lists already in shared memory (no walk): interactions/s and
  * cycles per (target pair, list entry).  Writes a JSON array as text into host_json (cap bytes; OTOO_ERR_CAPACITY
- * if too small).  Uses the context's particle arrays as scratch: the tree is invalidated.  Synchronises. */
+ * if too small).  Uses the context's particle arrays as scratch (max_particles >= 262144, else OTOO_ERR_CAPACITY): the
+ * tree is invalidated.  Synchronises. */
 otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_t cap, void* stream);
 
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);

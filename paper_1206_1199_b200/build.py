@@ -9,7 +9,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = ["api.cu", "build.cu", "sort.cu", "gravity.cu", "sph.cu", "probe.cu"]
-HEADERS = ["common.cuh", "walk.cuh", "walk_ws.cuh", "grav_eval.cuh", os.path.join("..", "..", "include", "otoo.h")]
+HEADERS = ["common.cuh", "walk.cuh", "walk_ws.cuh", "grav_eval.cuh", "keys.cuh", os.path.join("..", "..", "include", "otoo.h")]
 LIB = os.path.join(HERE, "libotoo.so")
 
 

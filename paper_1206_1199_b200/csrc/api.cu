@@ -108,6 +108,8 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
+    OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_gbase, 256 * sizeof(uint32_t)));
+    OTOO_CUDA(ctx, cudaMemset(ctx->scan_tmp, 0, sizeof(uint32_t)));       // arrival counter of the scan
     for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
     for (auto& e : ctx->ev_walk) OTOO_CUDA(ctx, cudaEventCreate(&e));
     return OTOO_OK;
@@ -130,6 +132,7 @@ void otoo_destroy(otoo_ctx* ctx) {
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);
+  if (ctx->h_gbase) cudaFreeHost(ctx->h_gbase);
   for (auto& e : ctx->ev_build) if (e) cudaEventDestroy(e);
   for (auto& e : ctx->ev_walk) if (e) cudaEventDestroy(e);
   delete ctx;

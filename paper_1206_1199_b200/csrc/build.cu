@@ -6,6 +6,7 @@
 //   cpl(s) = common prefix levels of key[s-1], key[s] and D(s) = max over windows of n_crit+1
 //   consecutive slots containing s of their common prefix levels.
 #include "common.cuh"
+#include "keys.cuh"
 #include <cooperative_groups.h>
 namespace cg = cooperative_groups;
 
@@ -44,14 +45,18 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4* __restrict__ po
     for (int w = 1; w < 8; w++) v = threadIdx.x < 3 ? fminf(v, sh[w][threadIdx.x]) : fmaxf(v, sh[w][threadIdx.x]);
     if (threadIdx.x < 3) atomicMin(&bbox[threadIdx.x], f2ord(v)); else atomicMax(&bbox[threadIdx.x], f2ord(v));
   }
-}
-
-// root cube: floats at bbox[8..12] = lo.xyz, S, scale
-__global__ void root_kernel(unsigned* bbox) {
+  // the last block to arrive derives the root cube: floats at bbox[8..12] = lo.xyz, S, scale (bbox[6] counts arrivals)
+  __shared__ bool last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) last = atomicAdd(&bbox[6], 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last || threadIdx.x != 0) return;
+  __threadfence();
   float* out = reinterpret_cast<float*>(bbox) + 8;
   float S = 0.0f;
   for (int k = 0; k < 3; k++) {
-    float lo = ord2f(bbox[k]), hi = ord2f(bbox[3 + k]);
+    float lo = ord2f(__ldcg(&bbox[k])), hi = ord2f(__ldcg(&bbox[3 + k]));
     float d = __fsub_rn(hi, lo);
     if (d > S) S = d;
     out[k] = lo;
@@ -61,74 +66,6 @@ __global__ void root_kernel(unsigned* bbox) {
   out[4] = __fdiv_rn(2097152.0f, S);  // R2: IEEE division
 }
 
-__device__ __forceinline__ uint64_t dilate3(uint32_t v) {
-  uint64_t x = v & 0x1FFFFFu;
-  x = (x | x << 32) & 0x001F00000000FFFFull;
-  x = (x | x << 16) & 0x001F0000FF0000FFull;
-  x = (x | x << 8) & 0x100F00F00F00F00Full;
-  x = (x | x << 4) & 0x10C30C30C30C30C3ull;
-  x = (x | x << 2) & 0x1249249249249249ull;
-  return x;
-}
-__device__ __forceinline__ uint32_t compact3(uint64_t x) {
-  x &= 0x1249249249249249ull;
-  x = (x | x >> 2) & 0x10C30C30C30C30C3ull;
-  x = (x | x >> 4) & 0x100F00F00F00F00Full;
-  x = (x | x >> 8) & 0x001F0000FF0000FFull;
-  x = (x | x >> 16) & 0x001F00000000FFFFull;
-  x = (x | x >> 32) & 0x1FFFFFull;
-  return (uint32_t)x;
-}
-// Hilbert order (reading R20): Skilling's transpose form of the 3-D Hilbert curve on the 21-bit
-// quantised coordinates, x the most significant axis.  The key is the interleave of the transformed
-// coordinates, so its top 3l bits still name the level-l octree cell.
-__device__ __forceinline__ void hilbert_axes_to_transpose(uint32_t& x, uint32_t& y, uint32_t& z) {
-  uint32_t X[3] = {x, y, z};
-  for (uint32_t Q = 1u << (OTOO_MAXLEV - 1); Q > 1; Q >>= 1) {
-    const uint32_t P = Q - 1;
-#pragma unroll
-    for (int i = 0; i < 3; i++) {
-      if (X[i] & Q) X[0] ^= P;
-      else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
-    }
-  }
-  X[1] ^= X[0]; X[2] ^= X[1];
-  uint32_t t = 0;
-  for (uint32_t Q = 1u << (OTOO_MAXLEV - 1); Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
-  x = X[0] ^ t; y = X[1] ^ t; z = X[2] ^ t;
-}
-__device__ __forceinline__ void hilbert_transpose_to_axes(uint32_t& x, uint32_t& y, uint32_t& z) {
-  uint32_t X[3] = {x, y, z};
-  uint32_t t = X[2] >> 1;
-  X[2] ^= X[1]; X[1] ^= X[0]; X[0] ^= t;
-  for (uint32_t Q = 2; Q != (2u << (OTOO_MAXLEV - 1)); Q <<= 1) {
-    const uint32_t P = Q - 1;
-#pragma unroll
-    for (int i = 2; i >= 0; i--) {
-      if (X[i] & Q) X[0] ^= P;
-      else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
-    }
-  }
-  x = X[0]; y = X[1]; z = X[2];
-}
-__device__ __forceinline__ uint32_t quant(float x, float lo, float scale) {
-  float t = __fmul_rn(__fsub_rn(x, lo), scale);
-  return (t >= 2097151.0f) ? 2097151u : (t > 0.0f ? __float2uint_rz(t) : 0u);
-}
-// H2 (L129; R2, R3): 63-bit Morton key by bit dilation, x most significant in each octant.
-__global__ void __launch_bounds__(256) key_kernel(const float4* __restrict__ pos, int64_t n,
-                                                  const unsigned* __restrict__ bbox, uint64_t* __restrict__ key,
-                                                  uint32_t* __restrict__ id, int hilbert) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const float* r = reinterpret_cast<const float*>(bbox) + 8;
-  float scale = r[4];
-  float4 p = pos[i];
-  uint32_t qx = quant(p.x, r[0], scale), qy = quant(p.y, r[1], scale), qz = quant(p.z, r[2], scale);
-  if (hilbert) hilbert_axes_to_transpose(qx, qy, qz);
-  key[i] = (dilate3(qx) << 2) | (dilate3(qy) << 1) | dilate3(qz);
-  id[i] = (uint32_t)i;
-}
 // H4: positions into sorted order
 __global__ void __launch_bounds__(256) gather4_kernel(const float4* __restrict__ src, const uint32_t* __restrict__ perm,
                                                       int64_t n, float4* __restrict__ dst) {
@@ -449,18 +386,18 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_EV(ctx, ctx->ev_build[0], st);
   // H1
   OTOO_CUDA(ctx, cudaMemsetAsync(bbox, 0xFF, 12, st));      // min = 0xFFFFFFFF
-  OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 12, st));  // max = 0
+  OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 16, st));  // max = 0, arrival counter = 0
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 64 * sizeof(uint32_t), st));
   int gb = ctx->sm_count * 4; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
-  root_kernel<<<1, 1, 0, st>>>(bbox);
   OTOO_EV(ctx, ctx->ev_build[1], st);
   // H2, H3, H4
-  key_kernel<<<nbN, 256, 0, st>>>(pos, N, bbox, ctx->key[0], ctx->val[0], ctx->key_order);
-  ctx->launches += 3;
+  // keys and ids, and in the same read the eight digit histograms of the sort (otoo_keys_and_hist, sort.cu)
+  OTOO_TRY(otoo_keys_and_hist(ctx, d_pos_mass, N, st));
+  ctx->launches += 1;
   OTOO_EV(ctx, ctx->ev_build[2], st);
   int res = 0;
-  OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res));
+  OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res, nullptr, true));
   if (res != 0) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: sort result buffer");
   OTOO_EV(ctx, ctx->ev_build[3], st);
   gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
@@ -485,7 +422,9 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   // H5b, canonical order (level, first), H5c
   emit_cells_kernel<<<nbN, 256, 0, st>>>(ctx->slot_nc, info, N, ctx->tmp_key[0], ctx->tmp_val[0]);
   ctx->launches += 1;
-  OTOO_TRY(otoo_sort_pairs(ctx, ctx->tmp_key, ctx->tmp_val, ncell, 0, 8, st, &res));
+  // canonical order: one radix pass on the level; the digit offsets are the level offsets the host already has
+  for (int d = 0; d < 256; d++) ctx->h_gbase[d] = d <= OTOO_NLEV ? off.v[d] : off.v[OTOO_NLEV];
+  OTOO_TRY(otoo_sort_pairs(ctx, ctx->tmp_key, ctx->tmp_val, ncell, 0, 8, st, &res, ctx->h_gbase));
   cell_topology_kernel<<<nbC, 256, 0, st>>>(ctx->tmp_key[res], ctx->tmp_val[res], ncell, ctx->key[0], N, n_crit, off,
                                             ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
                                             ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);

@@ -72,6 +72,7 @@ struct otoo_ctx {
   // pinned host mirror
   uint32_t* h_counters;
   float* h_root;         // lo[3], S
+  uint32_t* h_gbase;     // 256 digit offsets of the cells-by-level pass (pinned)
 
   // ---- walk outputs
   int64_t groupCap;
@@ -149,7 +150,9 @@ static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // ---- internal entry points (one per .cu file)
 otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n,
-                            int first_bit, int end_bit, cudaStream_t st, int* result_buf);
+                            int first_bit, int end_bit, cudaStream_t st, int* result_buf, const uint32_t* host_offsets = nullptr,
+                            bool hist_done = false);
+otoo_status otoo_keys_and_hist(otoo_ctx* ctx, const float* d_pos_mass, int64_t n, cudaStream_t st);
 otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, uint32_t* total_out_dev,
                                     cudaStream_t st);
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st);

@@ -14,9 +14,17 @@
 namespace {
 
 // R7: r_b = l/theta + s in fp64, rb^2 rounded once to fp32.  theta = 0 -> +inf (open everything).
+// the first OTOO_POOL_SLOTS threads of the r_b kernels also reset the walk's control block and the pool's sequence
+// numbers (tickets restart from 0 every launch): was a kernel of its own
+struct WalkReset { WalkShared* ws; uint32_t* seq; int ngroups; };
+__device__ __forceinline__ void walk_reset(const WalkReset& r, int64_t i) {
+  if (i < OTOO_POOL_SLOTS) r.seq[i] = (uint32_t)i;
+  if (i == 0) { r.ws->queue = 0; r.ws->head = 0; r.ws->tail = 0; r.ws->outstanding = r.ngroups; }
+}
 __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_level, const double* __restrict__ c_s,
-                                                  int64_t ncell, float S, float theta, cellb_t* __restrict__ cell_b) {
+                                                  int64_t ncell, float S, float theta, cellb_t* __restrict__ cell_b, const WalkReset wr) {
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  walk_reset(wr, c);
   if (c >= ncell) return;
   float rb2;
   if (!(theta > 0.0f)) rb2 = INFINITY;
@@ -32,8 +40,9 @@ __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_
 // than m_limit: r_b = 2 S_root (L157); Delta = 0: open everything.  Same fp64 operation order as the oracle.
 __global__ void __launch_bounds__(256) rb2_delta_kernel(const double* __restrict__ c_B2, const double* __restrict__ c_MP,
                                                         const unsigned long long* __restrict__ bmax_bits, int64_t ncell,
-                                                        float S, float delta, float m_limit, cellb_t* __restrict__ cell_b) {
+                                                        float S, float delta, float m_limit, cellb_t* __restrict__ cell_b, const WalkReset wr) {
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  walk_reset(wr, c);
   if (c >= ncell) return;
   float rb2;
   if (!(delta > 0.0f)) rb2 = INFINITY;
@@ -302,7 +311,7 @@ size_t otoo_walk_smem_bytes() {
 static size_t grav_fused_smem_bytes() { return otoo_walk_smem_bytes() + (size_t)OTOO_WALK_WARPS * 2 * OTOO_PIECES * sizeof(float4); }
 
 // Common launch preparation of the walk kernels: persistent grid, task pool, zeroed counters.
-otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st) {
+otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st, bool reset) {
   const int64_t total_groups = cdiv(ctx->N, G);
   // target sharding (PAPER III-E, L179: every device holds the whole tree and walks a contiguous range of targets)
   const int64_t g_begin = ctx->group_begin;
@@ -326,7 +335,10 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->pool_seq, sizeof(uint32_t) * (size_t)OTOO_POOL_SLOTS));
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->walk_shared, sizeof(WalkShared)));
   }
-  walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq, (int)ngroups);
+  if (reset) {   // (the gravity calls do this inside their r_b kernel)
+    walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq, (int)ngroups);
+    ctx->launches += 1;
+  }
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_nparts, 0, 4 * (size_t)total_groups, st));
@@ -339,7 +351,6 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->use_pool = ctx->use_pool;
   c->walk_only = ctx->walk_only;
   c->dist_kind = 0;
-  ctx->launches += 1;
   ctx->last_group_size = G; ctx->last_ngroups = total_groups; ctx->last_walk_only = ctx->walk_only;
   return OTOO_OK;
 }
@@ -347,15 +358,16 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
 otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float p1, int G, float* d_acc_pot, cudaStream_t st) {
   GravParams p;
   int grid; size_t smem;
-  OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st));
+  OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st, false));
   smem = grav_fused_smem_bytes();                 // (the one-warp-does-both kernel: + the pieces' boxes)
+  const WalkReset wr{p.c.ws, p.c.seq, (int)p.c.ngroups};
+  const unsigned nbR = (unsigned)(cdiv(ctx->N_cell, 256) > OTOO_POOL_SLOTS / 256 ? cdiv(ctx->N_cell, 256) : OTOO_POOL_SLOTS / 256);
   if (mac == 0) {
-    rb2_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b);
+    rb2_kernel<<<nbR, 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b, wr);
   } else {
     OTOO_TRY(otoo_b2_impl(ctx, st));
     OTOO_TRY(otoo_bmax_impl(ctx, st));
-    rb2_delta_kernel<<<(unsigned)cdiv(ctx->N_cell, 256), 256, 0, st>>>(ctx->c_B2, ctx->c_MP, ctx->sph_acc, ctx->N_cell, ctx->S,
-                                                                         p0, p1, ctx->cell_b);
+    rb2_delta_kernel<<<nbR, 256, 0, st>>>(ctx->c_B2, ctx->c_MP, ctx->sph_acc, ctx->N_cell, ctx->S, p0, p1, ctx->cell_b, wr);
   }
   OTOO_CUDA(ctx, cudaMemsetAsync(d_acc_pot, 0, 16 * (size_t)ctx->N, st));
   p.eps2 = eps * eps;

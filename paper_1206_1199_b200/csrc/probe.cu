@@ -169,7 +169,9 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
   if (!ctx || !which || !host_json || cap < 64) return OTOO_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   OTOO_CUDA(ctx, cudaSetDevice(ctx->device));
-  if (ctx->maxN < (1 << 16)) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "otoo_probe needs max_particles >= 65536 of scratch");
+  // scratch inside the context's particle arrays: 64 Ki positions, and in key[1] (8 B per particle) the cycle counters
+  // followed by one float4 per probe thread (<= 5 CTAs x 128 threads per SM): 2 MB
+  if (ctx->maxN < (1 << 18)) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "otoo_probe needs max_particles >= 262144 of scratch");
   ctx->built = false; ctx->walked = false;               // the probes use the context's particle arrays as scratch
   const int64_t n = 1 << 16;
   f32x2* pairs = reinterpret_cast<f32x2*>(ctx->key[0]);

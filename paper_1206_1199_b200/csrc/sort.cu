@@ -3,6 +3,7 @@
 // The paper used a host parallel quicksort; here it is an 8-bit-digit stable LSD radix sort in the
 // one-sweep form (stable + ids initially ascending = ties broken by original index, reading R4).
 #include "common.cuh"
+#include "keys.cuh"
 
 namespace {
 
@@ -27,14 +28,14 @@ constexpr int OS_MAXPASS = 8;
 #endif
 constexpr int OS_LOOKBACK = OTOO_OS_LOOKBACK;      // status words of preceding tiles a thread has in flight
 constexpr uint32_t OS_GHIST = 0;                       // u32 offsets into ctx->hist
-constexpr uint32_t OS_TICKET = OS_MAXPASS * 256;       // one tile ticket counter per pass
+constexpr uint32_t OS_TICKET = OS_MAXPASS * 256;       // one tile ticket counter per pass; [OS_TICKET + 255] counts the histogram blocks
 constexpr uint32_t OS_STATUS = OS_TICKET + 256;        // u64 status words [tile][digit] from here (8 B aligned)
 constexpr size_t OS_SMEM = SORT_TILE * 12 + SORT_WARPS * 256 * 4 + 2 * 256 * 4 + 16;
 
 // all digit histograms of the key bits [first_bit, first_bit + 8 * npass) in one read of the keys
 __global__ void __launch_bounds__(SORT_THREADS) radix_hist_all_kernel(const uint64_t* __restrict__ keys, int64_t n,
                                                                       int first_bit, int npass,
-                                                                      uint32_t* __restrict__ ghist) {
+                                                                      uint32_t* __restrict__ ghist, uint32_t* __restrict__ done) {
   __shared__ uint32_t sh[OS_MAXPASS][256];
   const int tid = threadIdx.x;
   for (int p = 0; p < npass; p++) sh[p][tid] = 0;
@@ -45,22 +46,67 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_hist_all_kernel(const uint
   }
   __syncthreads();
   for (int p = 0; p < npass; p++) if (sh[p][tid]) atomicAdd(&ghist[p * 256 + tid], sh[p][tid]);
-}
-// counts -> exclusive digit offsets, one block per pass
-__global__ void __launch_bounds__(256) radix_hist_scan_kernel(uint32_t* __restrict__ ghist) {
-  __shared__ uint32_t sh[256];
-  uint32_t* h = ghist + blockIdx.x * 256;
-  const int tid = threadIdx.x;
-  const uint32_t c = h[tid];
-  sh[tid] = c;
+  // the last block to arrive turns the counts into exclusive digit offsets (was a kernel of its own)
+  __shared__ bool last;
+  __threadfence();
   __syncthreads();
-  for (int o = 1; o < 256; o <<= 1) {
-    uint32_t y = tid >= o ? sh[tid - o] : 0;
+  if (tid == 0) last = atomicAdd(done, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  for (int p = 0; p < npass; p++) {
+    const uint32_t c = __ldcg(&ghist[p * 256 + tid]);
+    sh[0][tid] = c;
     __syncthreads();
-    sh[tid] += y;
+    for (int o = 1; o < 256; o <<= 1) {
+      uint32_t y = tid >= o ? sh[0][tid - o] : 0;
+      __syncthreads();
+      sh[0][tid] += y;
+      __syncthreads();
+    }
+    ghist[p * 256 + tid] = sh[0][tid] - c;
     __syncthreads();
   }
-  h[tid] = sh[tid] - c;
+}
+
+// H2 fused with the histograms: keys and ids of all particles and, in the same pass over them, the eight digit
+// histograms of the 64-bit sort (one read of the positions instead of a key kernel plus a read of the keys)
+__global__ void __launch_bounds__(SORT_THREADS) key_hist_kernel(const float4* __restrict__ pos, int64_t n, const unsigned* __restrict__ bbox,
+                                                                uint64_t* __restrict__ key, uint32_t* __restrict__ id, int hilbert,
+                                                                uint32_t* __restrict__ ghist, uint32_t* __restrict__ done) {
+  __shared__ uint32_t sh[OS_MAXPASS][256];
+  const int tid = threadIdx.x;
+  for (int p = 0; p < OS_MAXPASS; p++) sh[p][tid] = 0;
+  __syncthreads();
+  const float* root = reinterpret_cast<const float*>(bbox) + 8;
+  for (int64_t i = (int64_t)blockIdx.x * SORT_THREADS + tid; i < n; i += (int64_t)gridDim.x * SORT_THREADS) {
+    const uint64_t k = particle_key(pos[i], root, hilbert);
+    key[i] = k;
+    id[i] = (uint32_t)i;
+    for (int p = 0; p < OS_MAXPASS; p++) atomicAdd(&sh[p][(unsigned)(k >> (8 * p)) & 0xFF], 1u);
+  }
+  __syncthreads();
+  for (int p = 0; p < OS_MAXPASS; p++) if (sh[p][tid]) atomicAdd(&ghist[p * 256 + tid], sh[p][tid]);
+  __shared__ bool last;
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) last = atomicAdd(done, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  for (int p = 0; p < OS_MAXPASS; p++) {           // counts -> exclusive digit offsets
+    const uint32_t c = __ldcg(&ghist[p * 256 + tid]);
+    sh[0][tid] = c;
+    __syncthreads();
+    for (int o = 1; o < 256; o <<= 1) {
+      uint32_t y = tid >= o ? sh[0][tid - o] : 0;
+      __syncthreads();
+      sh[0][tid] += y;
+      __syncthreads();
+    }
+    ghist[p * 256 + tid] = sh[0][tid] - c;
+    __syncthreads();
+  }
 }
 
 // status word: [63:34] epoch of the pass, [33:32] 1 = tile aggregate, 2 = inclusive prefix, [31:0] count
@@ -208,7 +254,7 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* t
 }
 
 __global__ void __launch_bounds__(SCAN_THREADS) scan_reduce_kernel(const uint32_t* __restrict__ data, int64_t n,
-                                                                   uint32_t* __restrict__ sums) {
+                                                                   uint32_t* sums, uint32_t* done, uint32_t* total_out) {
   int64_t base = (int64_t)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   uint32_t s = 0;
 #pragma unroll
@@ -216,15 +262,23 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_reduce_kernel(const uint32_
   uint32_t tot;
   block_exclusive_scan(s, &tot);
   if (threadIdx.x == 0) sums[blockIdx.x] = tot;
-}
-__global__ void __launch_bounds__(SCAN_THREADS) scan_sums_kernel(uint32_t* sums, int64_t nb, uint32_t* total_out) {
+  // the last block to arrive scans the block sums (was a kernel of its own)
+  __shared__ bool last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) last = atomicAdd(done, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  if (threadIdx.x == 0) *done = 0u;                  // ready for the next scan
+  const int64_t nb = gridDim.x;
   uint32_t carry = 0;
   for (int64_t c = 0; c < nb; c += SCAN_THREADS) {
     int64_t i = c + threadIdx.x;
-    uint32_t x = i < nb ? sums[i] : 0, tot;
-    uint32_t e = block_exclusive_scan(x, &tot);
+    uint32_t x = i < nb ? __ldcg(&sums[i]) : 0, t2;
+    uint32_t e = block_exclusive_scan(x, &t2);
     if (i < nb) sums[i] = e + carry;
-    carry += tot;
+    carry += t2;
   }
   if (threadIdx.x == 0 && total_out) *total_out = carry;
 }
@@ -249,18 +303,39 @@ otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, ui
     return OTOO_OK;
   }
   int64_t nb = cdiv(n, SCAN_TILE);
-  scan_reduce_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp);
-  scan_sums_kernel<<<1, SCAN_THREADS, 0, st>>>(ctx->scan_tmp, nb, total_out_dev);
-  scan_apply_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp);
-  ctx->launches += 3;
+  scan_reduce_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp + 1, ctx->scan_tmp, total_out_dev);   // scan_tmp[0]: arrival counter
+  scan_apply_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp + 1);
+  ctx->launches += 2;
+  OTOO_CUDA(ctx, cudaGetLastError());
+  return OTOO_OK;
+}
+
+// one epoch per radix pass tags the look-back status words; when they run out the words are cleared and the count restarts
+static otoo_status sort_epoch_check(otoo_ctx* ctx, int npass, cudaStream_t st) {
+  if (ctx->sort_epoch + (uint32_t)npass >= (1u << 30)) {
+    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t), st));
+    ctx->sort_epoch = 0;
+  }
+  return OTOO_OK;
+}
+
+// keys (R2, R3, R20) and ids of the particles into key[0] / val[0], and the digit offsets of the 8-pass sort that follows
+otoo_status otoo_keys_and_hist(otoo_ctx* ctx, const float* d_pos_mass, int64_t n, cudaStream_t st) {
+  OTOO_TRY(sort_epoch_check(ctx, OS_MAXPASS, st));
+  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
+  int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
+  key_hist_kernel<<<gh, SORT_THREADS, 0, st>>>(reinterpret_cast<const float4*>(d_pos_mass), n, reinterpret_cast<const unsigned*>(ctx->d_bbox),
+                                               ctx->key[0], ctx->val[0], ctx->key_order, ctx->hist + OS_GHIST, ctx->hist + OS_TICKET + 255);
   OTOO_CUDA(ctx, cudaGetLastError());
   return OTOO_OK;
 }
 
 // Sort n pairs on bits [first_bit, end_bit) in 8-bit digits (stable).  Input in buffer 0; *result_buf
 // tells which buffer holds the result.  Uses ctx->hist (digit histograms, tile tickets, look-back status).
+// host_offsets (may be NULL): the exclusive digit offsets of a ONE-pass sort when the caller knows the digit counts
+// already (the cells' levels): written from pinned host memory instead of a histogram kernel.
 otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n, int first_bit,
-                            int end_bit, cudaStream_t st, int* result_buf) {
+                            int end_bit, cudaStream_t st, int* result_buf, const uint32_t* host_offsets, bool hist_done) {
   int cur = 0;
   if (n > 0) {
     const int nb = (int)cdiv(n, SORT_TILE);
@@ -271,15 +346,17 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
       OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_SMEM));
       ctx->sort_attr_set = true;
     }
-    if (ctx->sort_epoch + (uint32_t)npass >= (1u << 30)) {      // epochs exhausted: clear the status words, restart
-      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t), st));
-      ctx->sort_epoch = 0;
+    if (!hist_done) OTOO_TRY(sort_epoch_check(ctx, npass, st));
+    if (hist_done) {       // otoo_keys_and_hist has cleared the scratch and left the digit offsets of all passes
+    } else if (host_offsets && npass == 1) {
+      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
+      OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->hist + OS_GHIST, host_offsets, 256 * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+    } else {
+      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
+      int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
+      radix_hist_all_kernel<<<gh, SORT_THREADS, 0, st>>>(key[0], n, first_bit, npass, ctx->hist + OS_GHIST, ctx->hist + OS_TICKET + 255);
+      ctx->launches += 1;
     }
-    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
-    int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
-    radix_hist_all_kernel<<<gh, SORT_THREADS, 0, st>>>(key[0], n, first_bit, npass, ctx->hist + OS_GHIST);
-    radix_hist_scan_kernel<<<npass, 256, 0, st>>>(ctx->hist + OS_GHIST);
-    ctx->launches += 2;
     unsigned long long* status = reinterpret_cast<unsigned long long*>(ctx->hist + OS_STATUS);
     for (int p = 0; p < npass; p++) {
       onesweep_pass_kernel<<<nb, SORT_THREADS, OS_SMEM, st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n,

@@ -478,4 +478,4 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
 }
 
 // host side (gravity.cu)
-otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st);
+otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, size_t* smem, cudaStream_t st, bool reset = true);
