@@ -11,7 +11,7 @@ cores on a bounded sample.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--theta 0.5] [--no-per-config]
     python bench.py --impl reference ...      # times the oracle (CPU) on the same workload
-    python bench.py --probe ffma2|sumloop     # the microbenchmarks behind DESIGN.md's ceilings
+    python bench.py --probe ffma2|sumloop|rank|sort   # the microbenchmarks behind DESIGN.md's ceilings
 """
 from __future__ import annotations
 
@@ -379,7 +379,7 @@ def main():
     ap.add_argument("--group-sph", type=int, default=None, help="group size of the SPH rows (C4 / COLD; default: the workload's, 64)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the C2 / C3 / C4 blocks of the default line")
-    ap.add_argument("--probe", default=None, choices=["ffma2", "sumloop"],
+    ap.add_argument("--probe", default=None, choices=["ffma2", "sumloop", "rank", "sort"],
                     help="run a microbenchmark of the library (otoo_probe) instead of the bench and print its table as JSON")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -396,7 +396,7 @@ def main():
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
     if args.probe:
-        o = binding.Otoo(max_particles=1 << 20, device=local)
+        o = binding.Otoo(max_particles=1 << (25 if args.probe == "sort" else 20), device=local)
         print(json.dumps({"probe": args.probe, "rows": o.otoo_probe(args.probe)}), flush=True)
         return
     if world > 1:

@@ -195,7 +195,10 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
 /* Measurement aid: the microbenchmarks behind the ceilings DESIGN.md quotes for the force kernel (bench.py --probe).
  * which = "ffma2": SM sub-partition cycles per FFMA2 warp instruction for the operand patterns of the sum loop;
  * "sumloop": the product's own pair-sum loop on lists already in shared memory (no walk): interactions/s and
- * cycles per (target pair, list entry).  Writes a JSON array as text into host_json (cap bytes; OTOO_ERR_CAPACITY
+ * cycles per (target pair, list entry); "rank": SM cycles per warp instruction of MATCH.ANY, ballot, shared-memory
+ * atomics and loads (the choices of the sort's ranking); "sort": otoo's eight-pass sort of (u64, u32) pairs beside
+ * cub::DeviceRadixSort::SortPairs on 1 M / 8 M / 32 M pairs (as far as max_particles allows; allocates and frees
+ * CUB's temporary storage).  Writes a JSON array as text into host_json (cap bytes; OTOO_ERR_CAPACITY
  * if too small).  Uses the context's particle arrays as scratch (max_particles >= 262144, else OTOO_ERR_CAPACITY): the
  * tree is invalidated.  Synchronises. */
 otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_t cap, void* stream);

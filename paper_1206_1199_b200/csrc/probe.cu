@@ -4,8 +4,14 @@
 //              consecutive instructions; pair + 32-bit broadcast register), by clock64() inside the kernel.
 //   "sumloop": the product's own pair-sum loop (GravVisitor::eval of grav_eval.cuh) on lists already resident in
 //              shared memory -- no walk, no hand-off: the evaluator's ceiling in interactions/s.
+//   "rank":    SM cycles per warp instruction of the primitives a radix ranking can be built from (MATCH.ANY on 8- and
+//              4-bit digits, ballot, shared-memory atomics, a random shared-memory load): why the sort's ranking ORs
+//              lane bits into shared memory instead of using match.any.
+//   "sort":    the product's eight-pass sort of (u64 key, u32 id) pairs (otoo_sort_pairs) beside the library's
+//              cub::DeviceRadixSort::SortPairs on the same pairs -- a reference point, CUB is not on the force path.
 // Measurement aids only: nothing here is on the force path.
 #include <string>
+#include <cub/device/device_radix_sort.cuh>
 #include "grav_eval.cuh"
 
 namespace {
@@ -88,6 +94,45 @@ __global__ void __launch_bounds__(256) probe_fill_kernel(float4* pos, f32x2* pai
   if (pairs) pairs[i] = pk2(1.0f + 1e-7f * (float)(h & 255u), 1.0f - 1e-7f * (float)((h >> 8) & 255u));
 }
 
+// ---------------------------------------------------------------- ranking primitives
+template <int MODE>
+__global__ void __launch_bounds__(512, 1) rank_probe_kernel(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int iters,
+                                                            unsigned long long* __restrict__ cycles) {
+  __shared__ uint32_t sm[16][256];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int i = tid; i < 16 * 256; i += blockDim.x) (&sm[0][0])[i] = 0;
+  uint32_t d[8];
+  for (int i = 0; i < 8; i++) d[i] = in[(size_t)tid * 8 + i] & 0xFFu;     // "random" 8-bit digits
+  uint32_t acc = 0;
+  __syncthreads();
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const uint32_t x = d[i];
+      if (MODE == 0) acc += __match_any_sync(0xFFFFFFFFu, x);
+      else if (MODE == 1) acc += __match_any_sync(0xFFFFFFFFu, x & 15u);
+      else if (MODE == 2) acc += __ballot_sync(0xFFFFFFFFu, x & 1u);
+      else if (MODE == 3) acc += atomicAdd(&sm[warp][x], 1u);
+      else if (MODE == 4) atomicOr(&sm[warp][x], 1u << lane);
+      else acc += sm[warp][x];
+      d[i] = (x * 5u + 1u) & 0xFFu;
+    }
+  }
+  __syncthreads();
+  const long long t1 = clock64();
+  out[(size_t)blockIdx.x * blockDim.x + tid] = acc + d[0] + sm[warp][lane];
+  if (tid == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+}
+
+__global__ void __launch_bounds__(256) sort_fill_kernel(uint64_t* k, uint32_t* v, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint64_t x = (uint64_t)i * 0x9E3779B97F4A7C15ull;      // SplitMix64 finaliser: 63 random key bits, ids ascending
+  x ^= x >> 30; x *= 0xBF58476D1CE4E5B9ull; x ^= x >> 27; x *= 0x94D049BB133111EBull; x ^= x >> 31;
+  k[i] = x >> 1; v[i] = (uint32_t)i;
+}
+
 struct Timer {
   cudaEvent_t e0, e1;
   Timer() { cudaEventCreate(&e0); cudaEventCreate(&e1); }
@@ -111,6 +156,20 @@ double run_ffma2(otoo_ctx* ctx, const f32x2* in, f32x2* out, unsigned long long*
   for (int i = 0; i < n; i++) sum += (double)h[i];
   // cycles per warp instruction and sub-partition: every SMSP issued warps_per_smsp x iters x FP_ACC FFMA2
   return sum / n / ((double)warps_per_smsp * iters * FP_ACC);
+}
+
+template <int MODE>
+double run_rank(otoo_ctx* ctx, const uint32_t* in, uint32_t* out, unsigned long long* d_cyc, int warps, cudaStream_t st) {
+  const int iters = 512, grid = ctx->sm_count;
+  rank_probe_kernel<MODE><<<grid, 32 * warps, 0, st>>>(in, out, 8, d_cyc);
+  rank_probe_kernel<MODE><<<grid, 32 * warps, 0, st>>>(in, out, iters, d_cyc);
+  unsigned long long h[256];
+  const int n = grid < 256 ? grid : 256;
+  cudaMemcpyAsync(h, d_cyc, sizeof(unsigned long long) * n, cudaMemcpyDeviceToHost, st);
+  cudaStreamSynchronize(st);
+  double sum = 0;
+  for (int i = 0; i < n; i++) sum += (double)h[i];
+  return sum / n / ((double)iters * 8 * warps);          // SM cycles per warp instruction (all warps of the SM share the unit)
 }
 
 template <int T, int PB, int UNR>
@@ -215,7 +274,53 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
     OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 5)));
-  } else return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown probe (ffma2, sumloop)");
+  } else if (strcmp(which, "rank") == 0) {
+    sort_fill_kernel<<<64, 256, 0, st>>>(ctx->key[0], ctx->val[0], 64 * 256);
+    const uint32_t* digits = reinterpret_cast<const uint32_t*>(ctx->key[0]);
+    uint32_t* out = reinterpret_cast<uint32_t*>(ctx->key[1]) + 4096;
+    const char* names[6] = {"MATCH.ANY, 8-bit digits", "MATCH.ANY, 4-bit digits", "VOTE (ballot)", "ATOMS.ADD with return, random digit",
+                            "ATOMS.OR without return, random digit", "LDS, random word"};
+    for (int w = 4; w <= 16; w += 12) {
+      const double c[6] = {run_rank<0>(ctx, digits, out, d_cyc, w, st), run_rank<1>(ctx, digits, out, d_cyc, w, st),
+                           run_rank<2>(ctx, digits, out, d_cyc, w, st), run_rank<3>(ctx, digits, out, d_cyc, w, st),
+                           run_rank<4>(ctx, digits, out, d_cyc, w, st), run_rank<5>(ctx, digits, out, d_cyc, w, st)};
+      for (int m = 0; m < 6; m++) {
+        char buf[256];
+        snprintf(buf, sizeof buf, "%s{\"name\": \"%s\", \"warps_per_sm\": %d, \"sm_cycles_per_warp_instruction\": %.2f}",
+                 js.empty() ? "" : ", ", names[m], w, c[m]);
+        js += buf;
+      }
+    }
+    OTOO_CUDA(ctx, cudaGetLastError());
+  } else if (strcmp(which, "sort") == 0) {
+    Timer tm;
+    for (int64_t ns = 1 << 20; ns <= ctx->maxN && ns <= (int64_t)1 << 25; ns <<= (ns == 1 << 20 ? 3 : 2)) {
+      size_t tb = 0;
+      OTOO_CUDA(ctx, cub::DeviceRadixSort::SortPairs(nullptr, tb, ctx->key[0], ctx->key[1], ctx->val[0], ctx->val[1], ns, 0, 63, st));
+      void* tmp = nullptr;
+      OTOO_CUDA(ctx, cudaMalloc(&tmp, tb));
+      float ours = 1e30f, lib = 1e30f;
+      for (int r = 0; r < 6; r++) {
+        sort_fill_kernel<<<(unsigned)cdiv(ns, 256), 256, 0, st>>>(ctx->key[0], ctx->val[0], ns);
+        int rb = 0;
+        tm.start(st);
+        const otoo_status s1 = otoo_sort_pairs(ctx, ctx->key, ctx->val, ns, 0, 63, st, &rb, nullptr, false);
+        const float a = tm.stop(st);
+        if (s1 != OTOO_OK) { cudaFree(tmp); return s1; }
+        sort_fill_kernel<<<(unsigned)cdiv(ns, 256), 256, 0, st>>>(ctx->key[0], ctx->val[0], ns);
+        tm.start(st);
+        cub::DeviceRadixSort::SortPairs(tmp, tb, ctx->key[0], ctx->key[1], ctx->val[0], ctx->val[1], ns, 0, 63, st);
+        const float b = tm.stop(st);
+        if (r >= 1) { if (a < ours) ours = a; if (b < lib) lib = b; }
+      }
+      cudaFree(tmp);
+      OTOO_CUDA(ctx, cudaGetLastError());
+      char buf[320];
+      snprintf(buf, sizeof buf, "%s{\"name\": \"sort of (u64 key, u32 id) pairs, key bits 0..62\", \"pairs\": %lld, \"otoo_sort_pairs_ms\": %.4f, "
+               "\"cub_DeviceRadixSort_SortPairs_ms\": %.4f, \"cub_temp_bytes\": %zu}", js.empty() ? "" : ", ", (long long)ns, ours, lib, tb);
+      js += buf;
+    }
+  } else return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "unknown probe (ffma2, sumloop, rank, sort)");
   js = "[" + js + "]";
   if ((int64_t)js.size() + 1 > cap) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "probe output buffer too small");
   memcpy(host_json, js.c_str(), js.size() + 1);

@@ -9,8 +9,6 @@ namespace {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_TILE = OTOO_SORT_TILE;             // pairs per CTA
-constexpr int SORT_ITEMS = SORT_TILE / SORT_THREADS;
-constexpr int SORT_WARPS = SORT_THREADS / 32;
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -30,7 +28,9 @@ constexpr int OS_LOOKBACK = OTOO_OS_LOOKBACK;      // status words of preceding 
 constexpr uint32_t OS_GHIST = 0;                       // u32 offsets into ctx->hist
 constexpr uint32_t OS_TICKET = OS_MAXPASS * 256;       // one tile ticket counter per pass; [OS_TICKET + 255] counts the histogram blocks
 constexpr uint32_t OS_STATUS = OS_TICKET + 256;        // u64 status words [tile][digit] from here (8 B aligned)
-constexpr size_t OS_SMEM = SORT_TILE * 12 + SORT_WARPS * 256 * 4 + 2 * 256 * 4 + 16;
+constexpr int OS_NMASK = 2;                            // peer-mask tables per warp: a lane's items alternate between them
+constexpr int64_t OS_SMALL_N = 4 << 20;                // up to here: CTAs of 512 threads (2 per SM); above: 256 threads (3 per SM)
+constexpr size_t os_smem(int threads) { return SORT_TILE * 12 + (size_t)(1 + OS_NMASK) * (threads / 32) * 256 * 4 + 256 * 4 + 16; }
 
 // all digit histograms of the key bits [first_bit, first_bit + 8 * npass) in one read of the keys
 __global__ void __launch_bounds__(SORT_THREADS) radix_hist_all_kernel(const uint64_t* __restrict__ keys, int64_t n,
@@ -114,109 +114,125 @@ __device__ __forceinline__ unsigned long long os_pack(uint32_t epoch, uint32_t s
   return ((unsigned long long)((epoch << 2) | state) << 32) | v;
 }
 
-__global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const uint64_t* __restrict__ kin,
-                                                                     const uint32_t* __restrict__ vin,
-                                                                     uint64_t* __restrict__ kout,
-                                                                     uint32_t* __restrict__ vout, int64_t n, int shift,
-                                                                     const uint32_t* __restrict__ gbase,
-                                                                     unsigned long long* status, uint32_t* ticket,
-                                                                     uint32_t epoch) {
-  extern __shared__ __align__(16) unsigned char os_smem[];
-  uint64_t* skey = reinterpret_cast<uint64_t*>(os_smem);
-  uint32_t* sval = reinterpret_cast<uint32_t*>(os_smem + SORT_TILE * 8);
-  uint32_t(*whist)[256] = reinterpret_cast<uint32_t(*)[256]>(os_smem + SORT_TILE * 12);
-  uint32_t* dstart = reinterpret_cast<uint32_t*>(os_smem + SORT_TILE * 12 + SORT_WARPS * 256 * 4);
-  uint32_t* goff = dstart + 256;
+// One pass: a CTA takes one tile of SORT_TILE pairs.  Ranking: the lanes that hold a lane's digit are found by ORing
+// lane bits into the digit's word of a per-warp mask table in shared memory -- MATCH.ANY on 8-bit digits costs
+// 60 SM cycles per warp instruction on this part, a shared-memory atomic 3.6 (otoo_probe "rank"; profiles/r2_probes.md),
+// and with MATCH the ADU pipe (66 % busy at two CTAs per SM) kept a third CTA per SM from helping.
+template <int OS_THREADS, int MINB>
+__global__ void __launch_bounds__(OS_THREADS, MINB) onesweep_pass_kernel(const uint64_t* __restrict__ kin,
+                                                                         const uint32_t* __restrict__ vin,
+                                                                         uint64_t* __restrict__ kout,
+                                                                         uint32_t* __restrict__ vout, int64_t n, int shift,
+                                                                         const uint32_t* __restrict__ gbase,
+                                                                         unsigned long long* status, uint32_t* ticket,
+                                                                         uint32_t epoch) {
+  constexpr int OS_WARPS = OS_THREADS / 32, OS_ITEMS = SORT_TILE / OS_THREADS;
+  extern __shared__ __align__(16) unsigned char os_raw[];
+  uint64_t* skey = reinterpret_cast<uint64_t*>(os_raw);
+  uint32_t* sval = reinterpret_cast<uint32_t*>(os_raw + SORT_TILE * 8);
+  uint32_t(*whist)[256] = reinterpret_cast<uint32_t(*)[256]>(os_raw + SORT_TILE * 12);
+  uint32_t(*wmask)[256] = whist + OS_WARPS;            // [OS_NMASK * OS_WARPS][256]
+  uint32_t* goff = reinterpret_cast<uint32_t*>(wmask + OS_NMASK * OS_WARPS);
   uint32_t* stile = goff + 256;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) *stile = atomicAdd(ticket, 1u);      // tiles are numbered in starting order: look-back cannot hang
-#pragma unroll
-  for (int w = 0; w < SORT_WARPS; w++) whist[w][tid] = 0;
+  for (int i = tid; i < (1 + OS_NMASK) * OS_WARPS * 256; i += OS_THREADS) (&whist[0][0])[i] = 0;
   __syncthreads();
   const uint32_t tile = *stile;
   const int64_t tbase = (int64_t)tile * SORT_TILE;
-  const int64_t base = tbase + warp * (32 * SORT_ITEMS);
-  uint64_t k[SORT_ITEMS];
-  uint32_t v[SORT_ITEMS];
-  uint32_t rk[SORT_ITEMS];  // rank among equal digits within the warp's chunk, in index order (stable)
+  const int64_t base = tbase + warp * (32 * OS_ITEMS);
+  uint64_t k[OS_ITEMS];
+  uint32_t v[OS_ITEMS];
+  uint32_t rk2[(OS_ITEMS + 1) / 2];  // rank among equal digits within the warp's chunk, in index order (stable); two 16-bit ranks per word
 #pragma unroll
-  for (int i = 0; i < SORT_ITEMS; i++) {
+  for (int i = 0; i < (OS_ITEMS + 1) / 2; i++) rk2[i] = 0;
+#pragma unroll
+  for (int i = 0; i < OS_ITEMS; i++) {
     int64_t idx = base + i * 32 + lane;
-    if (idx < n) { k[i] = kin[idx]; v[i] = vin[idx]; }
+    if (idx < n) { k[i] = kin[idx]; v[i] = vin[idx]; }   // (values loaded after the ranking instead: 2.46 -> 3.53 ms at 32 M pairs)
     else { k[i] = ~0ull; v[i] = 0; }
   }
+  const unsigned lt = lanemask_lt();
 #pragma unroll
-  for (int i = 0; i < SORT_ITEMS; i++) {
+  for (int i = 0; i < OS_ITEMS; i++) {
     const bool valid = base + i * 32 + lane < n;
-    const unsigned d = valid ? (unsigned)((k[i] >> shift) & 0xFF) : 0xFFFFFFFFu;
-    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-    const int leader = __ffs(peers) - 1;
-    uint32_t b = 0;
-    if (valid && lane == leader) { b = whist[warp][d]; whist[warp][d] = b + __popc(peers); }
-    b = __shfl_sync(0xFFFFFFFFu, b, leader);
-    rk[i] = b + __popc(peers & lanemask_lt());
+    const unsigned d = (unsigned)((k[i] >> shift) & 0xFF);
+    uint32_t* mask = &wmask[(i & 1) * OS_WARPS + warp][d];
+    if (valid) atomicOr(mask, 1u << lane);
     __syncwarp();
+    const unsigned peers = valid ? *mask : 0u;
+    const uint32_t b = valid ? whist[warp][d] : 0u;
+    __syncwarp();
+    // the lowest peer counts the digit and clears the mask word (two tables: the clear cannot meet the next item's
+    // OR, and the count is ordered before the next item's read by that item's first __syncwarp; one table and a
+    // third __syncwarp: 2 % slower)
+    if (valid && (peers & lt) == 0u) { whist[warp][d] = b + __popc(peers); *mask = 0u; }
+    rk2[i >> 1] |= (b + __popc(peers & lt)) << (16 * (i & 1));
   }
   __syncthreads();
-  // digit `tid`: exclusive prefix over the warps, tile count, look-back over the preceding tiles
-  uint32_t cnt = 0;
-#pragma unroll
-  for (int w = 0; w < SORT_WARPS; w++) { uint32_t c = whist[w][tid]; whist[w][tid] = cnt; cnt += c; }
+  // digit `tid`: tile count, look-back over the preceding tiles, start of the digit in the sorted tile
+  uint32_t cnt = 0, inc = 0;
   const volatile unsigned long long* status_v = status;
   volatile unsigned long long* st = status + (size_t)tile * 256 + tid;
-  *st = os_pack(epoch, tile == 0 ? 2u : 1u, cnt);
-  dstart[tid] = cnt;
-  __syncthreads();
-  for (int o = 1; o < 256; o <<= 1) {                 // inclusive scan of the tile's digit counts
-    uint32_t y = tid >= o ? dstart[tid - o] : 0;
-    __syncthreads();
-    dstart[tid] += y;
-    __syncthreads();
+  if (tid < 256) {
+#pragma unroll
+    for (int w = 0; w < OS_WARPS; w++) cnt += whist[w][tid];
+    *st = os_pack(epoch, tile == 0 ? 2u : 1u, cnt);
+    inc = cnt;                                         // exclusive scan of the tile's digit counts: warp shuffles + the warps' totals
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, inc, o); if (lane >= o) inc += y; }
+    if (lane == 31) goff[warp] = inc;
   }
-  const uint32_t my_start = dstart[tid] - cnt;
-  uint32_t excl = 0;
-  if (tile > 0) {
-    // look back over the preceding tiles, 8 status words in flight at a time (when all tiles of a small
-    // sort run in one wave the walk is long, and one L2 round trip per tile would dominate the pass)
-    int64_t t = (int64_t)tile - 1;
-    bool done = false;
-    while (!done) {
-      unsigned long long w[OS_LOOKBACK];
+  __syncthreads();
+  uint32_t my_start = inc - cnt, excl = 0;
+  if (tid < 256) {
 #pragma unroll
-      for (int j = 0; j < OS_LOOKBACK; j++)
-        w[j] = t - j >= 0 ? *(status_v + (size_t)(t - j) * 256 + tid) : os_pack(epoch, 2u, 0u);
-      int used = 0;
+    for (int w = 0; w < 7; w++) if (w < warp) my_start += goff[w];
+    uint32_t run = my_start;                          // whist[w][d] := position in the sorted tile of warp w's first key with digit d
 #pragma unroll
-      for (int j = 0; j < OS_LOOKBACK; j++) {
-        if (!done && used == j) {
-          const uint32_t state = (uint32_t)(w[j] >> 32) & 3u;
-          if ((uint32_t)(w[j] >> 34) == epoch && state != 0u) {
-            excl += (uint32_t)w[j];
-            used = j + 1;
-            done = state == 2u;
+    for (int w = 0; w < OS_WARPS; w++) { const uint32_t c = whist[w][tid]; whist[w][tid] = run; run += c; }
+    if (tile > 0) {
+      // look back over the preceding tiles, 8 status words in flight at a time (when all tiles of a small
+      // sort run in one wave the walk is long, and one L2 round trip per tile would dominate the pass)
+      int64_t t = (int64_t)tile - 1;
+      bool done = false;
+      while (!done) {
+        unsigned long long w[OS_LOOKBACK];
+#pragma unroll
+        for (int j = 0; j < OS_LOOKBACK; j++)
+          w[j] = t - j >= 0 ? *(status_v + (size_t)(t - j) * 256 + tid) : os_pack(epoch, 2u, 0u);
+        int used = 0;
+#pragma unroll
+        for (int j = 0; j < OS_LOOKBACK; j++) {
+          if (!done && used == j) {
+            const uint32_t state = (uint32_t)(w[j] >> 32) & 3u;
+            if ((uint32_t)(w[j] >> 34) == epoch && state != 0u) {
+              excl += (uint32_t)w[j];
+              used = j + 1;
+              done = state == 2u;
+            }
           }
         }
+        t -= used;
       }
-      t -= used;
+      *st = os_pack(epoch, 2u, excl + cnt);
     }
-    *st = os_pack(epoch, 2u, excl + cnt);
   }
   __syncthreads();
-  dstart[tid] = my_start;
-  goff[tid] = gbase[tid] + excl - my_start;           // global slot = goff[digit] + position in the sorted tile
+  if (tid < 256) goff[tid] = gbase[tid] + excl - my_start;   // global slot = goff[digit] + position in the sorted tile
   __syncthreads();
 #pragma unroll
-  for (int i = 0; i < SORT_ITEMS; i++) {
+  for (int i = 0; i < OS_ITEMS; i++) {
     if (base + i * 32 + lane < n) {
       const unsigned d = (unsigned)((k[i] >> shift) & 0xFF);
-      const uint32_t pos = dstart[d] + whist[warp][d] + rk[i];
+      const uint32_t pos = whist[warp][d] + ((rk2[i >> 1] >> (16 * (i & 1))) & 0xFFFFu);
       skey[pos] = k[i];
       sval[pos] = v[i];
     }
   }
   __syncthreads();
   const int cnt_tile = (int)((n - tbase) < SORT_TILE ? (n - tbase) : SORT_TILE);
-  for (int j = tid; j < cnt_tile; j += SORT_THREADS) {
+  for (int j = tid; j < cnt_tile; j += OS_THREADS) {
     const uint64_t key = skey[j];
     const uint32_t dst = goff[(unsigned)((key >> shift) & 0xFF)] + (uint32_t)j;
     kout[dst] = key;
@@ -343,7 +359,8 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
     if (npass > OS_MAXPASS || OTOO_SORT_SCRATCH(n) > ctx->hist_cap)
       return otoo_fail(ctx, OTOO_ERR_CAPACITY, "sort scratch too small");
     if (!ctx->sort_attr_set) {
-      OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_SMEM));
+      OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)os_smem(256)));
+      OTOO_CUDA(ctx, cudaFuncSetAttribute(onesweep_pass_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)os_smem(512)));
       ctx->sort_attr_set = true;
     }
     if (!hist_done) OTOO_TRY(sort_epoch_check(ctx, npass, st));
@@ -359,9 +376,13 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
     }
     unsigned long long* status = reinterpret_cast<unsigned long long*>(ctx->hist + OS_STATUS);
     for (int p = 0; p < npass; p++) {
-      onesweep_pass_kernel<<<nb, SORT_THREADS, OS_SMEM, st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n,
-                                                              first_bit + 8 * p, ctx->hist + OS_GHIST + p * 256, status,
-                                                              ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
+      // few tiles per SM: 2 CTAs of 16 warps hide more latency; many: 3 CTAs of 8 warps keep the shared-memory pipe busier
+      if (n <= OS_SMALL_N)
+        onesweep_pass_kernel<512, 2><<<nb, 512, os_smem(512), st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
+                                                                      ctx->hist + OS_GHIST + p * 256, status, ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
+      else
+        onesweep_pass_kernel<256, 3><<<nb, 256, os_smem(256), st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
+                                                                      ctx->hist + OS_GHIST + p * 256, status, ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
       ctx->launches += 1;
       cur ^= 1;
     }
