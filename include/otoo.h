@@ -203,6 +203,25 @@ otoo_status otoo_measure_fp32_peak(otoo_ctx* ctx, double* host_tflops, void* str
  * tree is invalidated.  Synchronises. */
 otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_json, int64_t cap, void* stream);
 
+/* The one entry point that allocates nothing (no cudaMalloc / cudaFree / allocating library call; no context): for
+ * callers under CUDA graph capture, in tight serving loops, or in harnesses that forbid allocation.
+ * (III-B step 3: "we sort an array of the pair of a key and a particle's id"): stable LSD radix sort of n (u64 key,
+ * u32 value) pairs on all 64 key bits, the same eight one-sweep passes as the tree build's sort, on the CURRENT device.
+ * d_keys / d_vals (device, n each): the pairs in, the sorted pairs out (ties keep their input order);
+ * d_keys_alt / d_vals_alt (device, n each, caller-owned): the passes' second buffer, contents undefined afterwards.
+ * The passes' scratch (digit histograms, tile tickets, look-back status words) is a file-scope device array inside the
+ * library, sized for OTOO_SORT_STATIC_MAX_PAIRS pairs: 1.03 MB that every GPU loading libotoo.so holds until the
+ * process exits.  n > OTOO_SORT_STATIC_MAX_PAIRS: OTOO_ERR_CAPACITY and a message (larger sorts go through a context);
+ * n < 0 or a null buffer with n > 0: OTOO_ERR_INVALID_ARG; CUDA failure: OTOO_ERR_CUDA.  host_err (host, err_cap bytes,
+ * may be NULL): receives the message of a failed call, "" on success.  Asynchronous on `stream`; every call clears the
+ * part of the array it uses, so calls in a row (and replays of a captured graph) are independent -- but ALL calls on a
+ * device share the one array: two calls that overlap on the GPU (different streams, no dependency between them) race
+ * and give wrong results; serialise them.  The first call on a device looks up the array's address and opts the kernel
+ * into its shared memory: make one call (n = 0 is enough) before starting a graph capture.  Thread-safe set-up. */
+#define OTOO_SORT_STATIC_MAX_PAIRS 2097152
+otoo_status otoo_sort_pairs_static(uint64_t* d_keys, uint32_t* d_vals, uint64_t* d_keys_alt, uint32_t* d_vals_alt,
+                                   int64_t n, void* stream, char* host_err, int64_t err_cap);
+
 /* Tuning/test knobs.  "walk_stack" = usable shared-memory walk-stack entries per warp (512);
  * "task_pool" = 1 (default): a warp with a long stack hands cells to the global task pool,
  * 0: it only spills to its private global area (test hook for that path).

@@ -26,7 +26,8 @@ STATUS_NAMES = ["OTOO_OK", "OTOO_ERR_INVALID_ARG", "OTOO_ERR_OOM", "OTOO_ERR_CUD
 EXPORTS = ["otoo_version", "otoo_create", "otoo_destroy", "otoo_last_error", "otoo_build_tree", "otoo_gravity",
            "otoo_sph_density", "otoo_sph_force", "otoo_eos_ideal", "otoo_tree_info", "otoo_export_tree",
            "otoo_export_sph_radii", "otoo_export_group_stats", "otoo_last_stats", "otoo_set_option",
-           "otoo_gravity_host", "otoo_gravity_delta_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_probe", "otoo_unsort", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc"]
+           "otoo_gravity_host", "otoo_gravity_delta_host", "otoo_gravity_delta", "otoo_measure_fp32_peak", "otoo_probe", "otoo_unsort", "otoo_sph_adapt_h", "otoo_sph_stage1", "otoo_sph_force_visc",
+           "otoo_sort_pairs_static"]
 
 
 class TreeInfo(C.Structure):
@@ -77,6 +78,8 @@ _lib.otoo_unsort.argtypes = [_vp, _vp, _vp, _vp]
 _lib.otoo_probe.argtypes = [_vp, C.c_char_p, C.c_char_p, _i64, _vp]
 _lib.otoo_gravity_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _i32, _vp]
 _lib.otoo_gravity_delta_host.argtypes = [_vp, _vp, _i64, _i32, _f, _f, _f, _i32, _vp]
+_lib.otoo_sort_pairs_static.argtypes = [_vp, _vp, _vp, _vp, _i64, _vp, C.c_char_p, _i64]
+SORT_STATIC_MAX_PAIRS = 2097152      # OTOO_SORT_STATIC_MAX_PAIRS of include/otoo.h
 
 
 class OtooError(RuntimeError):
@@ -295,6 +298,26 @@ class Otoo:
     def otoo_set_option(self, name: str, value: int):
         self._check(_lib.otoo_set_option(self._h, name.encode(), int(value)))
 
+
+def otoo_sort_pairs_static(keys, vals, keys_alt, vals_alt, n=None, stream=None):
+    """otoo_sort_pairs_static of include/otoo.h: stable sort of (int64-typed u64 key, int32-typed u32 value) pairs in
+    place on the tensors' device, no allocation inside the library (the four buffers are the caller's: create them
+    before a graph capture).  Argument marshalling only; raises OtooError with the library's message."""
+    n = int(keys.shape[0] if n is None else n)
+    dev = keys.device
+    for t, dt in ((keys, torch.int64), (vals, torch.int32), (keys_alt, torch.int64), (vals_alt, torch.int32)):
+        _ptr(t, dt, device=dev.index)
+        if t.ndim != 1 or t.shape[0] < n:
+            raise ValueError(f"expected 1-d tensors of at least {n} elements")
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(dev):                 # the entry point works on the current device
+        st = torch.cuda.current_stream(dev).cuda_stream if stream is None else (
+            stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+        status = _lib.otoo_sort_pairs_static(keys.data_ptr(), vals.data_ptr(), keys_alt.data_ptr(), vals_alt.data_ptr(),
+                                             n, st, err, len(err))
+    if status != 0:
+        raise OtooError(status, err.value.decode())
+    return keys, vals
 
 def raw():
     """The ctypes library handle (tests check exported symbols and error statuses)."""

@@ -2,6 +2,8 @@
 // PAPER.md L133 (III-B step 3): "we sort an array of the pair of a key and a particle's id".
 // The paper used a host parallel quicksort; here it is an 8-bit-digit stable LSD radix sort in the
 // one-sweep form (stable + ids initially ascending = ties broken by original index, reading R4).
+#include <cstdarg>
+#include <mutex>
 #include "common.cuh"
 #include "keys.cuh"
 
@@ -390,4 +392,88 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
   }
   *result_buf = cur;
   return OTOO_OK;
+}
+
+// ---------------------------------------------------------------- the no-allocation entry point (include/otoo.h)
+// otoo_sort_pairs_static: the same radix passes as otoo_sort_pairs, for callers that may not allocate (CUDA graph capture,
+// serving loops, harnesses that forbid cudaMalloc).  The passes' scratch -- digit histograms, tile tickets and the
+// look-back status words -- is NOT a context's `hist` buffer but this file-scope device array, sized for
+// OTOO_SORT_STATIC_MAX_PAIRS pairs; every GPU that loads libotoo.so holds it (1.03 MB) until the process exits.
+// In host code `g_sort_static` is only a stand-in for the symbol: its device address comes from cudaGetSymbolAddress,
+// once per device with that device current (sort_static_setup), and that pointer is what the kernels are given.
+namespace {
+static_assert(OTOO_SORT_STATIC_MAX_PAIRS <= OS_SMALL_N, "the static entry point launches the 512-thread pass only");
+constexpr int64_t SORT_STATIC_TILES = (OTOO_SORT_STATIC_MAX_PAIRS + SORT_TILE - 1) / SORT_TILE;
+constexpr size_t SORT_STATIC_WORDS = OS_STATUS + (size_t)SORT_STATIC_TILES * 256 * 2;      // u32 words: histograms, tickets, u64 status
+static __device__ __align__(256) uint32_t g_sort_static[SORT_STATIC_WORDS];
+
+constexpr int SORT_STATIC_MAXDEV = 64;
+struct SortStaticDev { std::once_flag once; cudaError_t err = cudaSuccess; uint32_t* scratch = nullptr; int sm_count = 0; };
+SortStaticDev g_sort_static_dev[SORT_STATIC_MAXDEV];
+
+// once per device, that device current: the array's device address, the SM count, the kernels' shared-memory opt-in
+cudaError_t sort_static_setup(int dev, SortStaticDev** out) {
+  SortStaticDev& d = g_sort_static_dev[dev];
+  std::call_once(d.once, [&]() {
+    void* p = nullptr;
+    d.err = cudaGetSymbolAddress(&p, g_sort_static);
+    if (d.err == cudaSuccess) d.err = cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (d.err == cudaSuccess) d.err = cudaFuncSetAttribute(onesweep_pass_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)os_smem(512));
+    if (d.err == cudaSuccess) d.scratch = static_cast<uint32_t*>(p);
+  });
+  *out = &d;
+  return d.err;
+}
+
+otoo_status sort_static_fail(otoo_status code, char* host_err, int64_t err_cap, const char* fmt, ...) {
+  if (host_err && err_cap > 0) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(host_err, (size_t)err_cap, fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+}  // namespace
+
+extern "C" otoo_status otoo_sort_pairs_static(uint64_t* d_keys, uint32_t* d_vals, uint64_t* d_keys_alt, uint32_t* d_vals_alt,
+                                              int64_t n, void* stream, char* host_err, int64_t err_cap) {
+  if (host_err && err_cap > 0) host_err[0] = 0;
+  if (n < 0) return sort_static_fail(OTOO_ERR_INVALID_ARG, host_err, err_cap, "otoo_sort_pairs_static: n = %lld is negative", (long long)n);
+  if (n > OTOO_SORT_STATIC_MAX_PAIRS)
+    return sort_static_fail(OTOO_ERR_CAPACITY, host_err, err_cap,
+                            "otoo_sort_pairs_static: n = %lld exceeds OTOO_SORT_STATIC_MAX_PAIRS = %lld (the static scratch is sized for that; "
+                            "larger sorts go through a context: otoo_build_tree)", (long long)n, (long long)OTOO_SORT_STATIC_MAX_PAIRS);
+  if (n > 0 && (!d_keys || !d_vals || !d_keys_alt || !d_vals_alt))
+    return sort_static_fail(OTOO_ERR_INVALID_ARG, host_err, err_cap, "otoo_sort_pairs_static: null buffer");
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess && (dev < 0 || dev >= SORT_STATIC_MAXDEV))
+    return sort_static_fail(OTOO_ERR_INVALID_ARG, host_err, err_cap, "otoo_sort_pairs_static: device index %d not supported (< %d)", dev, SORT_STATIC_MAXDEV);
+  SortStaticDev* d = nullptr;
+  if (e == cudaSuccess) e = sort_static_setup(dev, &d);
+  if (e != cudaSuccess)
+    return sort_static_fail(OTOO_ERR_CUDA, host_err, err_cap, "otoo_sort_pairs_static: set-up on device %d failed: %s", dev, cudaGetErrorString(e));
+  if (n == 0) return OTOO_OK;                       // (a call with n = 0 does the set-up and nothing else)
+  cudaStream_t st = (cudaStream_t)stream;
+  uint32_t* hist = d->scratch;                      // the DEVICE address of g_sort_static, never the host-side symbol
+  const int nb = (int)cdiv(n, SORT_TILE);
+  // the array keeps the last call's contents: histograms, tickets and this call's status words start at zero (the
+  // passes are tagged with epochs 1..8 of THIS call, so nothing is carried from call to call and a captured graph replays)
+  e = cudaMemsetAsync(hist, 0, (OS_STATUS + (size_t)nb * 256 * 2) * sizeof(uint32_t), st);
+  if (e != cudaSuccess) return sort_static_fail(OTOO_ERR_CUDA, host_err, err_cap, "otoo_sort_pairs_static: %s", cudaGetErrorString(e));
+  int gh = d->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
+  radix_hist_all_kernel<<<gh, SORT_THREADS, 0, st>>>(d_keys, n, 0, OS_MAXPASS, hist + OS_GHIST, hist + OS_TICKET + 255);
+  unsigned long long* status = reinterpret_cast<unsigned long long*>(hist + OS_STATUS);
+  uint64_t* key[2] = {d_keys, d_keys_alt};
+  uint32_t* val[2] = {d_vals, d_vals_alt};
+  int cur = 0;
+  for (int p = 0; p < OS_MAXPASS; p++) {            // n <= 2 Mi pairs: the 512-thread form (as otoo_sort_pairs chooses below OS_SMALL_N)
+    onesweep_pass_kernel<512, 2><<<nb, 512, os_smem(512), st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, 8 * p,
+                                                                  hist + OS_GHIST + p * 256, status, hist + OS_TICKET + p, (uint32_t)(p + 1));
+    cur ^= 1;
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return sort_static_fail(OTOO_ERR_CUDA, host_err, err_cap, "otoo_sort_pairs_static: launch failed: %s", cudaGetErrorString(e));
+  return OTOO_OK;                                   // eight passes: the result is back in d_keys / d_vals
 }
