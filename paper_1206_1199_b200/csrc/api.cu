@@ -97,7 +97,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     const size_t n = (size_t)max_particles;
     for (int b = 0; b < 2; b++) { OTOO_TRY(dalloc(ctx, &ctx->key[b], n)); OTOO_TRY(dalloc(ctx, &ctx->val[b], n)); }
     OTOO_TRY(dalloc(ctx, &ctx->spos, n));
-    OTOO_TRY(dalloc(ctx, &ctx->slot_nc, n));
+    OTOO_TRY(dalloc(ctx, &ctx->slot_nc, (size_t)OTOO_NLEV * (size_t)cdiv(max_particles, 256) + 64));   // per-block level counts (H5a)
     ctx->hist_cap = OTOO_SORT_SCRATCH(max_particles);   // look-back status (u64 per tile and digit) + histograms
     OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
     OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t)));
@@ -108,7 +108,6 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
-    OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_gbase, 256 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMemset(ctx->scan_tmp, 0, sizeof(uint32_t)));       // arrival counter of the scan
     for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
     for (auto& e : ctx->ev_walk) OTOO_CUDA(ctx, cudaEventCreate(&e));
@@ -132,7 +131,6 @@ void otoo_destroy(otoo_ctx* ctx) {
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);
-  if (ctx->h_gbase) cudaFreeHost(ctx->h_gbase);
   for (auto& e : ctx->ev_build) if (e) cudaEventDestroy(e);
   for (auto& e : ctx->ev_walk) if (e) cudaEventDestroy(e);
   delete ctx;

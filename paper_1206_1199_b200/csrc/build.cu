@@ -78,7 +78,9 @@ __device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leadin
   if (x == 0) return OTOO_MAXLEV;
   return 20 - (63 - __clzll((long long)x)) / 3;
 }
-// H5a: number of cells that start at each sorted slot, and the per-level cell counts.
+// H5a: the levels of the cells that start at each sorted slot, and the cell counts per level -- of the whole system
+// (level_count) and of every block of 256 slots (blk_lc[l * gridDim.x + block], level-major: one exclusive scan of
+// that array gives every block the canonical index of its first cell of each level, see place_cells_kernel).
 //   info[s] = (cpl+1) | LL << 8
 // A level-l range starting at s is a cell iff some window of n_crit+1 slots containing s shares l-1 levels:
 // c[t] = cplev(key[t], key[t + n_crit]) is computed once per t into shared memory (every thread of the
@@ -86,7 +88,7 @@ __device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leadin
 // counts are warp-aggregated (one ballot per level instead of contended shared-memory atomics).
 #define OTOO_SLOT_NCRIT_MAX 256
 __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
-                                                         uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
+                                                         uint32_t* __restrict__ blk_lc, uint32_t* __restrict__ info,
                                                          uint32_t* __restrict__ level_count) {
   __shared__ uint32_t lc[OTOO_NLEV];
   __shared__ signed char cwa[256 + OTOO_SLOT_NCRIT_MAX], cwb[256 + OTOO_SLOT_NCRIT_MAX];
@@ -120,8 +122,6 @@ __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restr
     const int D = a > b ? a : b;
     LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
     lo = cpl + 1;
-    int nc = LL - cpl; if (nc < 0) nc = 0;
-    slot_nc[s] = (uint32_t)nc;
     info[s] = (uint32_t)lo | ((uint32_t)LL << 8);
   }
   // per-level counts, warp-aggregated: only the levels some lane of the warp starts a cell at (a few around the
@@ -133,11 +133,14 @@ __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restr
     if (b && (threadIdx.x & 31) == 0) atomicAdd(&lc[l], (uint32_t)__popc(b));
   }
   __syncthreads();
-  if (threadIdx.x < OTOO_NLEV && lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+  if (threadIdx.x < OTOO_NLEV) {
+    blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
+    if (lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+  }
 }
 // the same for n_crit > OTOO_SLOT_NCRIT_MAX (every thread scans its own windows)
 __global__ void __launch_bounds__(256) slot_cells_wide_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
-                                                              uint32_t* __restrict__ slot_nc, uint32_t* __restrict__ info,
+                                                              uint32_t* __restrict__ blk_lc, uint32_t* __restrict__ info,
                                                               uint32_t* __restrict__ level_count) {
   __shared__ uint32_t lc[OTOO_NLEV];
   if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
@@ -150,24 +153,49 @@ __global__ void __launch_bounds__(256) slot_cells_wide_kernel(const uint64_t* __
     int64_t thi = n - n_crit - 1; if (thi > s) thi = s;
     for (int64_t t = tlo; t <= thi; t++) { int c = cplev(key[t], key[t + n_crit]); if (c > D) D = c; }
     int LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
-    int nc = LL - cpl; if (nc < 0) nc = 0;
-    slot_nc[s] = (uint32_t)nc;
     info[s] = (uint32_t)(cpl + 1) | ((uint32_t)LL << 8);
     for (int l = cpl + 1; l <= LL; l++) atomicAdd(&lc[l], 1u);
   }
   __syncthreads();
-  if (threadIdx.x < OTOO_NLEV && lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+  if (threadIdx.x < OTOO_NLEV) {
+    blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
+    if (lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
+  }
 }
-// H5b: emit (level, first) for every cell, in slot order
-__global__ void __launch_bounds__(256) emit_cells_kernel(const uint32_t* __restrict__ slot_off,
-                                                         const uint32_t* __restrict__ info, int64_t n,
-                                                         uint64_t* __restrict__ lev, uint32_t* __restrict__ first) {
-  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= n) return;
-  uint32_t inf = info[s];
-  int l0 = inf & 0xFF, LL = inf >> 8;
-  uint32_t off = slot_off[s];
-  for (int l = l0; l <= LL; l++, off++) { lev[off] = (uint64_t)l; first[off] = (uint32_t)s; }
+// H5b: first slot of every cell, written straight at the cell's canonical index.  Canonical order = (level, first slot):
+// the index of a level-l cell starting at slot s is (cells of lower levels) + (level-l cells starting before s) -- the
+// exclusive scan of the level-major per-block counts gives the first part plus the blocks before this one (blk_off), a
+// ballot per level the rank inside the block.  (Before: cells emitted in slot order with their level as a sort key, one
+// scan over all slots and one radix pass over all cells to bring them into level order.)
+__global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __restrict__ info, int64_t n,
+                                                          const uint32_t* __restrict__ blk_off, uint32_t* __restrict__ first) {
+  __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t s = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  int lo = OTOO_NLEV, LL = -1;
+  if (s < n) { const uint32_t inf = info[s]; lo = (int)(inf & 0xFF); LL = (int)(inf >> 8); }
+  const bool has = lo <= LL;
+  const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
+  for (int l = wlo; l <= whi; l++) {
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
+    if (lane == 0) wc[warp][l] = (uint32_t)__popc(b);
+  }
+  __syncthreads();
+  if (threadIdx.x < OTOO_NLEV) {
+    uint32_t run = blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
+#pragma unroll
+    for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
+  }
+  __syncthreads();
+  unsigned lt;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
+  for (int l = wlo; l <= whi; l++) {
+    const bool mine = lo <= l && l <= LL;
+    const unsigned b = __ballot_sync(0xFFFFFFFFu, mine);
+    if (mine) first[wc[warp][l] + (uint32_t)__popc(b & lt)] = (uint32_t)s;
+  }
 }
 
 struct LevelOff { uint32_t v[OTOO_NLEV + 1]; };
@@ -177,7 +205,7 @@ __device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* __restrict__
   return lo;
 }
 // H5c: per canonical cell: count, leaf flag, children (L135: "slicing the keys"; R5)
-__global__ void __launch_bounds__(256) cell_topology_kernel(const uint64_t* __restrict__ lev, const uint32_t* __restrict__ first,
+__global__ void __launch_bounds__(256) cell_topology_kernel(const uint32_t* __restrict__ first,
                                                             int64_t ncell, const uint64_t* __restrict__ key, int64_t n,
                                                             int n_crit, LevelOff off, uint32_t* __restrict__ c_first,
                                                             uint32_t* __restrict__ c_count, uint32_t* __restrict__ c_child_first,
@@ -185,7 +213,9 @@ __global__ void __launch_bounds__(256) cell_topology_kernel(const uint64_t* __re
                                                             cellb_t* __restrict__ cell_b, uint32_t* __restrict__ n_leaf) {
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= ncell) return;
-  int level = (int)lev[c];
+  int level = 0;                                   // canonical order is level-major: the level is where c falls in the offsets
+#pragma unroll
+  for (int l = 1; l < OTOO_NLEV; l++) level += c >= (int64_t)off.v[l] ? 1 : 0;
   uint32_t s = first[c];
   uint32_t count;
   if (level == 0) count = (uint32_t)n;
@@ -318,14 +348,7 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   OTOO_TRY(grow(ctx, &ctx->c_B2, cap));
   OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
   OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
-  for (int b = 0; b < 2; b++) { OTOO_TRY(grow(ctx, &ctx->tmp_key[b], cap)); OTOO_TRY(grow(ctx, &ctx->tmp_val[b], cap)); }
-  size_t need = OTOO_SORT_SCRATCH(cap);
-  if (need > ctx->hist_cap) {
-    OTOO_TRY(grow(ctx, &ctx->hist, need));
-    ctx->hist_cap = need;
-    OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, need * sizeof(uint32_t)));   // status epochs restart
-    ctx->sort_epoch = 0;
-  }
+  OTOO_TRY(grow(ctx, &ctx->tmp_val[0], cap));        // first slot of every cell (H5b)
   ctx->cellCap = cap;
   return OTOO_OK;
 }
@@ -397,17 +420,18 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   ctx->launches += 1;
   OTOO_EV(ctx, ctx->ev_build[2], st);
   int res = 0;
-  OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res, nullptr, true));
+  OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res, true));
   if (res != 0) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: sort result buffer");
   OTOO_EV(ctx, ctx->ev_build[3], st);
   gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
   OTOO_EV(ctx, ctx->ev_build[4], st);
   // H5a
   uint32_t* info = ctx->val[1];
-  if (n_crit <= OTOO_SLOT_NCRIT_MAX) slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
-  else slot_cells_wide_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, ctx->slot_nc, info, ctx->d_counters);
-  ctx->launches += 2;
-  OTOO_TRY(otoo_exclusive_scan_u32(ctx, ctx->slot_nc, N, ctx->d_counters + 40, st));
+  uint32_t* blk_lc = ctx->slot_nc;                 // OTOO_NLEV x nbN per-block level counts, then their exclusive scan
+  if (n_crit <= OTOO_SLOT_NCRIT_MAX) slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info, ctx->d_counters);
+  else slot_cells_wide_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info, ctx->d_counters);
+  ctx->launches += 1;
+  OTOO_TRY(otoo_exclusive_scan_u32(ctx, blk_lc, (int64_t)OTOO_NLEV * nbN, ctx->d_counters + 40, st));
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, 64 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_root, ctx->d_bbox + 8, 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaStreamSynchronize(st));
@@ -419,16 +443,12 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   if ((int64_t)run != ncell || ncell < 1) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: level counts disagree with cell count");
   OTOO_TRY(ensure_cells(ctx, ncell));
   const unsigned nbC = (unsigned)cdiv(ncell, 256);
-  // H5b, canonical order (level, first), H5c
-  emit_cells_kernel<<<nbN, 256, 0, st>>>(ctx->slot_nc, info, N, ctx->tmp_key[0], ctx->tmp_val[0]);
-  ctx->launches += 1;
-  // canonical order: one radix pass on the level; the digit offsets are the level offsets the host already has
-  for (int d = 0; d < 256; d++) ctx->h_gbase[d] = d <= OTOO_NLEV ? off.v[d] : off.v[OTOO_NLEV];
-  OTOO_TRY(otoo_sort_pairs(ctx, ctx->tmp_key, ctx->tmp_val, ncell, 0, 8, st, &res, ctx->h_gbase));
-  cell_topology_kernel<<<nbC, 256, 0, st>>>(ctx->tmp_key[res], ctx->tmp_val[res], ncell, ctx->key[0], N, n_crit, off,
+  // H5b: cells in canonical order (level, first slot); H5c
+  place_cells_kernel<<<nbN, 256, 0, st>>>(info, N, blk_lc, ctx->tmp_val[0]);
+  cell_topology_kernel<<<nbC, 256, 0, st>>>(ctx->tmp_val[0], ncell, ctx->key[0], N, n_crit, off,
                                             ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
                                             ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);
-  ctx->launches += 1;
+  ctx->launches += 2;
   OTOO_EV(ctx, ctx->ev_build[5], st);
   // H6 deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,

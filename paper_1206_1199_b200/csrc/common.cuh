@@ -37,7 +37,7 @@ struct otoo_ctx {
   uint64_t* key[2];      // key double buffer for the LSD sort; key[0] holds the sorted keys after build
   uint32_t* val[2];      // id double buffer; val[0] = perm after build
   float4* spos;          // positions+mass in sorted order
-  uint32_t* slot_nc;     // cells starting at slot s, then its exclusive scan
+  uint32_t* slot_nc;     // cells per level starting in each block of 256 slots (level-major), then its exclusive scan
   uint32_t* scan_tmp;    // block sums for the scan
   uint32_t* hist;        // sort scratch: digit histograms, tile tickets, look-back status words
   uint32_t sort_epoch;   // one epoch per radix pass: stale status words never match
@@ -63,8 +63,8 @@ struct otoo_ctx {
   double* c_B2;          // trace of the quadrupole tensor about the CM (PAPER Eq. 2; R19)
   float2* c_sph;         // (b_max, r_SPH) (R14)
   unsigned long long* sph_acc;  // 2 per cell: fp64 maxima as ordered bits
-  uint64_t* tmp_key[2];  // (level) keys for the canonical ordering pass
-  uint32_t* tmp_val[2];
+  uint64_t* tmp_key[2];  // (unused since the cells are placed at their canonical index directly)
+  uint32_t* tmp_val[2];  // [0]: first slot of every cell in canonical order
 
   // ---- small device scalars
   float* d_bbox;         // 6 floats lo/hi as ordered ints, then lo[3], S, scale
@@ -72,7 +72,6 @@ struct otoo_ctx {
   // pinned host mirror
   uint32_t* h_counters;
   float* h_root;         // lo[3], S
-  uint32_t* h_gbase;     // 256 digit offsets of the cells-by-level pass (pinned)
 
   // ---- walk outputs
   int64_t groupCap;
@@ -150,8 +149,7 @@ static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // ---- internal entry points (one per .cu file)
 otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n,
-                            int first_bit, int end_bit, cudaStream_t st, int* result_buf, const uint32_t* host_offsets = nullptr,
-                            bool hist_done = false);
+                            int first_bit, int end_bit, cudaStream_t st, int* result_buf, bool hist_done = false);
 otoo_status otoo_keys_and_hist(otoo_ctx* ctx, const float* d_pos_mass, int64_t n, cudaStream_t st);
 otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, uint32_t* total_out_dev,
                                     cudaStream_t st);

@@ -304,7 +304,7 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
         sort_fill_kernel<<<(unsigned)cdiv(ns, 256), 256, 0, st>>>(ctx->key[0], ctx->val[0], ns);
         int rb = 0;
         tm.start(st);
-        const otoo_status s1 = otoo_sort_pairs(ctx, ctx->key, ctx->val, ns, 0, 63, st, &rb, nullptr, false);
+        const otoo_status s1 = otoo_sort_pairs(ctx, ctx->key, ctx->val, ns, 0, 63, st, &rb, false);
         const float a = tm.stop(st);
         if (s1 != OTOO_OK) { cudaFree(tmp); return s1; }
         sort_fill_kernel<<<(unsigned)cdiv(ns, 256), 256, 0, st>>>(ctx->key[0], ctx->val[0], ns);

@@ -350,10 +350,9 @@ otoo_status otoo_keys_and_hist(otoo_ctx* ctx, const float* d_pos_mass, int64_t n
 
 // Sort n pairs on bits [first_bit, end_bit) in 8-bit digits (stable).  Input in buffer 0; *result_buf
 // tells which buffer holds the result.  Uses ctx->hist (digit histograms, tile tickets, look-back status).
-// host_offsets (may be NULL): the exclusive digit offsets of a ONE-pass sort when the caller knows the digit counts
-// already (the cells' levels): written from pinned host memory instead of a histogram kernel.
+// hist_done: otoo_keys_and_hist has left the digit offsets of all passes (no histogram kernel here).
 otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], int64_t n, int first_bit,
-                            int end_bit, cudaStream_t st, int* result_buf, const uint32_t* host_offsets, bool hist_done) {
+                            int end_bit, cudaStream_t st, int* result_buf, bool hist_done) {
   int cur = 0;
   if (n > 0) {
     const int nb = (int)cdiv(n, SORT_TILE);
@@ -367,9 +366,6 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
     }
     if (!hist_done) OTOO_TRY(sort_epoch_check(ctx, npass, st));
     if (hist_done) {       // otoo_keys_and_hist has cleared the scratch and left the digit offsets of all passes
-    } else if (host_offsets && npass == 1) {
-      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
-      OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->hist + OS_GHIST, host_offsets, 256 * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
     } else {
       OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
       int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
