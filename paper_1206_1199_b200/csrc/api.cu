@@ -97,7 +97,7 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     const size_t n = (size_t)max_particles;
     for (int b = 0; b < 2; b++) { OTOO_TRY(dalloc(ctx, &ctx->key[b], n)); OTOO_TRY(dalloc(ctx, &ctx->val[b], n)); }
     OTOO_TRY(dalloc(ctx, &ctx->spos, n));
-    OTOO_TRY(dalloc(ctx, &ctx->slot_nc, (size_t)OTOO_NLEV * (size_t)cdiv(max_particles, 256) + 64));   // per-block level counts (H5a)
+    OTOO_TRY(dalloc(ctx, &ctx->slot_nc, (size_t)(OTOO_NLEV + 1) * (size_t)cdiv(max_particles, 256) + 64));   // per-block level counts and leaf counts (H5a)
     ctx->hist_cap = OTOO_SORT_SCRATCH(max_particles);   // look-back status (u64 per tile and digit) + histograms
     OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
     OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t)));

@@ -87,14 +87,23 @@ __device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leadin
 // plain form recomputed its n_crit+1 windows from global memory: 480 GB/s at 32 M particles), the per-level
 // counts are warp-aggregated (one ballot per level instead of contended shared-memory atomics).
 #define OTOO_SLOT_NCRIT_MAX 256
+// H4 rides along: the block's 256 random 16-byte reads of the gather (HBM-latency-bound, 3.7 x its algorithmic bytes
+// for an unordered input) are issued first and stored last, so they are in flight while the block does its
+// issue-bound level arithmetic (as kernels of their own: 0.72 + 0.46 ms at 32 M particles).
 __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
                                                          uint32_t* __restrict__ blk_lc, uint32_t* __restrict__ info,
-                                                         uint32_t* __restrict__ level_count) {
-  __shared__ uint32_t lc[OTOO_NLEV];
+                                                         const float4* __restrict__ pos,
+                                                         const uint32_t* __restrict__ perm, float4* __restrict__ spos) {
+  __shared__ uint32_t lc[OTOO_NLEV + 1];
   __shared__ signed char cwa[256 + OTOO_SLOT_NCRIT_MAX], cwb[256 + OTOO_SLOT_NCRIT_MAX];
   const int64_t s0 = (int64_t)blockIdx.x * 256;
+  float4 pv = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  if (s0 + threadIdx.x < n) {
+    const float4* src = pos + perm[s0 + threadIdx.x];
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(pv.x), "=f"(pv.y), "=f"(pv.z), "=f"(pv.w) : "l"(src));
+  }
   const int m = 256 + n_crit;                       // window starts t = s0 - n_crit + i, i < m
-  if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
+  if (threadIdx.x <= OTOO_NLEV) lc[threadIdx.x] = 0;
   for (int i = threadIdx.x; i < m; i += 256) {
     const int64_t t = s0 - n_crit + i;
     cwa[i] = (t >= 0 && t <= n - n_crit - 1) ? (signed char)cplev(key[t], key[t + n_crit]) : (signed char)-1;
@@ -132,18 +141,19 @@ __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restr
     const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
     if (b && (threadIdx.x & 31) == 0) atomicAdd(&lc[l], (uint32_t)__popc(b));
   }
+  const unsigned hb = __ballot_sync(0xFFFFFFFFu, has);  // row OTOO_NLEV: slots that start cells = leaves (one per such slot)
+  if (hb && (threadIdx.x & 31) == 0) atomicAdd(&lc[OTOO_NLEV], (uint32_t)__popc(hb));
   __syncthreads();
-  if (threadIdx.x < OTOO_NLEV) {
-    blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
-    if (lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
-  }
+  // (no system-wide counters: the level totals and the leaf count are read off the scan of these rows; one global atomic
+  // per block and level on 22 addresses cost more than the rest of the kernel)
+  if (threadIdx.x <= OTOO_NLEV) blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
+  if (s < n) spos[s] = pv;                            // H4: the position in sorted order
 }
 // the same for n_crit > OTOO_SLOT_NCRIT_MAX (every thread scans its own windows)
 __global__ void __launch_bounds__(256) slot_cells_wide_kernel(const uint64_t* __restrict__ key, int64_t n, int n_crit,
-                                                              uint32_t* __restrict__ blk_lc, uint32_t* __restrict__ info,
-                                                              uint32_t* __restrict__ level_count) {
-  __shared__ uint32_t lc[OTOO_NLEV];
-  if (threadIdx.x < OTOO_NLEV) lc[threadIdx.x] = 0;
+                                                              uint32_t* __restrict__ blk_lc, uint32_t* __restrict__ info) {
+  __shared__ uint32_t lc[OTOO_NLEV + 1];
+  if (threadIdx.x <= OTOO_NLEV) lc[threadIdx.x] = 0;
   __syncthreads();
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s < n) {
@@ -155,27 +165,36 @@ __global__ void __launch_bounds__(256) slot_cells_wide_kernel(const uint64_t* __
     int LL = D + 1 > OTOO_MAXLEV ? OTOO_MAXLEV : D + 1;
     info[s] = (uint32_t)(cpl + 1) | ((uint32_t)LL << 8);
     for (int l = cpl + 1; l <= LL; l++) atomicAdd(&lc[l], 1u);
+    if (cpl + 1 <= LL) atomicAdd(&lc[OTOO_NLEV], 1u);
   }
   __syncthreads();
-  if (threadIdx.x < OTOO_NLEV) {
-    blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
-    if (lc[threadIdx.x]) atomicAdd(&level_count[threadIdx.x], lc[threadIdx.x]);
-  }
+  if (threadIdx.x <= OTOO_NLEV) blk_lc[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = lc[threadIdx.x];
 }
-// H5b: first slot of every cell, written straight at the cell's canonical index.  Canonical order = (level, first slot):
+// H5b: every cell written straight at its canonical index, leaves complete.  Canonical order = (level, first slot):
 // the index of a level-l cell starting at slot s is (cells of lower levels) + (level-l cells starting before s) -- the
 // exclusive scan of the level-major per-block counts gives the first part plus the blocks before this one (blk_off), a
-// ballot per level the rank inside the block.  (Before: cells emitted in slot order with their level as a sort key, one
-// scan over all slots and one radix pass over all cells to bring them into level order.)
-__global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __restrict__ info, int64_t n,
-                                                          const uint32_t* __restrict__ blk_off, uint32_t* __restrict__ first) {
+// ballot per level the rank inside the block.  Of the cells that start at slot s (levels lo .. LL) the one at LL is a
+// leaf, the others are internal and their first child is the cell one level down at the same slot (L135: "slicing the
+// keys"; R5).  A leaf ends at the next slot that starts a range of its level or a coarser one (lo <= LL): found in the
+// block's shared-memory window of lo values (a leaf holds <= n_crit slots unless it sits at level 21), by a search on
+// the key prefix beyond it.  Counts and child counts of the internal cells come bottom-up (moments_all_kernel).
+// (Before: a kernel of its own found every cell's count and children by binary searches on the keys and the first slots.)
+#define OTOO_PLACE_WIN 64
+struct CellOut {
+  uint32_t* c_first; uint32_t* c_count; uint32_t* c_child_first; uint8_t* c_level; uint8_t* c_child_count; cellb_t* cell_b;
+};
+__global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __restrict__ info, const uint64_t* __restrict__ key, int64_t n,
+                                                          const uint32_t* __restrict__ blk_off, const CellOut o) {
   __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
+  __shared__ uint8_t slo[256 + OTOO_PLACE_WIN];  // lo of the block's slots and of the OTOO_PLACE_WIN slots after them (0 past the end)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
-  __syncthreads();
-  const int64_t s = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  const int64_t s0 = (int64_t)blockIdx.x * 256, s = s0 + threadIdx.x;
   int lo = OTOO_NLEV, LL = -1;
   if (s < n) { const uint32_t inf = info[s]; lo = (int)(inf & 0xFF); LL = (int)(inf >> 8); }
+  slo[threadIdx.x] = (uint8_t)(s < n ? lo : 0);
+  if (threadIdx.x < OTOO_PLACE_WIN) slo[256 + threadIdx.x] = s + 256 < n ? (uint8_t)(info[s + 256] & 0xFF) : (uint8_t)0;
+  __syncthreads();
   const bool has = lo <= LL;
   const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
   for (int l = wlo; l <= whi; l++) {
@@ -189,77 +208,68 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
     for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
   }
   __syncthreads();
+  // the leaf's particle count
+  uint32_t count = 0;
+  if (has) {
+    if (LL == 0) count = (uint32_t)n;
+    else {
+      int j = threadIdx.x + 1;
+      while (j < 256 + OTOO_PLACE_WIN && (int)slo[j] > LL) j++;
+      if (j < 256 + OTOO_PLACE_WIN) count = (uint32_t)(j - threadIdx.x);
+      else {                                       // beyond the window: gallop, then bisect for the end of the prefix range
+        const int sh = 3 * (OTOO_MAXLEV - LL);
+        const uint64_t prefix = key[s] >> sh;
+        uint64_t step = 1, a = (uint64_t)s;        // key[a] has the prefix
+        while (s + step < (uint64_t)n && (key[s + step] >> sh) == prefix) { a = s + step; step <<= 1; }
+        uint64_t hi = s + step < (uint64_t)n ? s + step : (uint64_t)n;  // key[hi] lacks it (or hi == n)
+        while (a + 1 < hi) { const uint64_t mid = (a + hi) >> 1; if ((key[mid] >> sh) == prefix) a = mid; else hi = mid; }
+        count = (uint32_t)(hi - s);
+      }
+    }
+  }
   unsigned lt;
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
-  for (int l = wlo; l <= whi; l++) {
+  uint32_t below = 0;                              // canonical index of this slot's cell one level down
+  for (int l = whi; l >= wlo; l--) {
     const bool mine = lo <= l && l <= LL;
     const unsigned b = __ballot_sync(0xFFFFFFFFu, mine);
-    if (mine) first[wc[warp][l] + (uint32_t)__popc(b & lt)] = (uint32_t)s;
+    if (mine) {
+      const uint32_t c = wc[warp][l] + (uint32_t)__popc(b & lt);
+      o.c_first[c] = (uint32_t)s; o.c_level[c] = (uint8_t)l;
+      if (l == LL) {
+        o.c_count[c] = count; o.c_child_first[c] = 0u; o.c_child_count[c] = 0;
+        o.cell_b[c] = make_uint4(0u, (uint32_t)s, count, 1u | ((uint32_t)l << 8));
+      } else {
+        o.c_child_first[c] = below; o.c_child_count[c] = 0xFF;        // internal: count and children bottom-up
+      }
+      below = c;
+    }
   }
 }
 
 struct LevelOff { uint32_t v[OTOO_NLEV + 1]; };
 
-__device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* __restrict__ a, uint32_t lo, uint32_t hi, uint32_t x) {
-  while (lo < hi) { uint32_t mid = lo + ((hi - lo) >> 1); if (a[mid] < x) lo = mid + 1; else hi = mid; }
-  return lo;
-}
-// H5c: per canonical cell: count, leaf flag, children (L135: "slicing the keys"; R5)
-__global__ void __launch_bounds__(256) cell_topology_kernel(const uint32_t* __restrict__ first,
-                                                            int64_t ncell, const uint64_t* __restrict__ key, int64_t n,
-                                                            int n_crit, LevelOff off, uint32_t* __restrict__ c_first,
-                                                            uint32_t* __restrict__ c_count, uint32_t* __restrict__ c_child_first,
-                                                            uint8_t* __restrict__ c_level, uint8_t* __restrict__ c_child_count,
-                                                            cellb_t* __restrict__ cell_b, uint32_t* __restrict__ n_leaf) {
-  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncell) return;
-  int level = 0;                                   // canonical order is level-major: the level is where c falls in the offsets
-#pragma unroll
-  for (int l = 1; l < OTOO_NLEV; l++) level += c >= (int64_t)off.v[l] ? 1 : 0;
-  uint32_t s = first[c];
-  uint32_t count;
-  if (level == 0) count = (uint32_t)n;
-  else {
-    int sh = 3 * (OTOO_MAXLEV - level);
-    uint64_t prefix = key[s] >> sh;
-    // gallop then bisect for the end of the prefix range
-    uint64_t step = 1, lo = s;  // key[lo] has the prefix
-    while (s + step < (uint64_t)n && (key[s + step] >> sh) == prefix) { lo = s + step; step <<= 1; }
-    uint64_t hi = s + step < (uint64_t)n ? s + step : (uint64_t)n;  // key[hi] lacks it (or hi == n)
-    while (lo + 1 < hi) { uint64_t mid = (lo + hi) >> 1; if ((key[mid] >> sh) == prefix) lo = mid; else hi = mid; }
-    count = (uint32_t)(hi - s);
-  }
-  bool leaf = count <= (uint32_t)n_crit || level == OTOO_MAXLEV;
-  uint32_t cf = 0, cc = 0;
-  if (!leaf) {
-    uint32_t a = off.v[level + 1], b = off.v[level + 2];
-    cf = lower_bound_u32(first, a, b, s);
-    cc = lower_bound_u32(first, cf, b, s + count) - cf;
-  }
-  c_first[c] = s; c_count[c] = count; c_child_first[c] = cf;
-  c_level[c] = (uint8_t)level; c_child_count[c] = (uint8_t)cc;
-  cell_b[c] = leaf ? make_uint4(0u, s, count, 1u | ((uint32_t)level << 8))
-                   : make_uint4(0u, cf, cc, ((uint32_t)level << 8));
-  if (leaf) atomicAdd(n_leaf, 1u);
-}
-
 // H6 (L155; R6, R7): one level of the bottom-up pass; fp64, fixed summation order.
 struct MomentArgs {
-  const float4* spos; const uint64_t* key; const uint32_t* c_first; const uint32_t* c_count;
-  const uint32_t* c_child_first; const uint8_t* c_child_count; const unsigned* bbox;
+  const float4* spos; const uint64_t* key; const uint32_t* c_first; uint32_t* c_count;
+  const uint32_t* c_child_first; uint8_t* c_child_count; const unsigned* bbox;
   double* MP; double* cm64; float4* cell_cm; double* c_s; double* c_B2;
   int hilbert;
+  const uint32_t* info; cellb_t* cell_b;          // H5c for the internal cells (moments_all_kernel only)
 };
-__device__ __forceinline__ void moments_cell(uint32_t c, int level, const MomentArgs& a) {
+// level_end = canonical index one past the last cell of level + 1 (the children's level)
+__device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t level_end, const MomentArgs& a) {
   const float4* __restrict__ spos = a.spos; const uint64_t* __restrict__ key = a.key;
-  const uint32_t* __restrict__ c_first = a.c_first; const uint32_t* __restrict__ c_count = a.c_count;
-  const uint32_t* __restrict__ c_child_first = a.c_child_first; const uint8_t* __restrict__ c_child_count = a.c_child_count;
+  const uint32_t* __restrict__ c_first = a.c_first; uint32_t* c_count = a.c_count;
+  const uint32_t* __restrict__ c_child_first = a.c_child_first; uint8_t* c_child_count = a.c_child_count;
   const unsigned* __restrict__ bbox = a.bbox;
   double* MP = a.MP; double* cm64 = a.cm64; float4* cell_cm = a.cell_cm; double* c_s = a.c_s;
-  uint32_t first = c_first[c], count = c_count[c];
+  const uint32_t first = c_first[c];
+  uint32_t count;
   int nch = c_child_count[c];
   double M = 0.0, Px = 0.0, Py = 0.0, Pz = 0.0;
   if (nch == 0) {
+    count = c_count[c];
     for (uint32_t s0 = first; s0 < first + count; s0 += 8) {   // 8 loads in flight, sums in slot order (R6)
       float4 p[8];
       const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
@@ -275,11 +285,25 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, const Moment
       }
     }
   } else {
-    uint32_t ch = c_child_first[c];
+    // H5c for an internal cell: its children are the cell one level down at its own first slot and the cells after
+    // that one (canonical order = octant order) whose first slot starts a range of the children's level but not of
+    // this cell's (lo == level + 1: still inside this cell); its particles are theirs
+    const uint32_t ch = c_child_first[c];
+    uint32_t f[8];
+    unsigned sib = 1u;                                 // bit k: cell ch + k exists and does not start a new parent
+#pragma unroll
+    for (int k = 1; k < 8; k++) f[k] = ch + k < level_end ? c_first[ch + k] : 0xFFFFFFFFu;
+#pragma unroll
+    for (int k = 1; k < 8; k++) if (f[k] != 0xFFFFFFFFu && (int)(a.info[f[k]] & 0xFF) == level + 1) sib |= 1u << k;
+    nch = __ffs(~sib) - 1;                             // the run of siblings from ch
+    count = 0;
     for (int k = 0; k < nch; k++) {
       const double* q = MP + 4 * (size_t)(ch + k);
       M = __dadd_rn(M, q[0]); Px = __dadd_rn(Px, q[1]); Py = __dadd_rn(Py, q[2]); Pz = __dadd_rn(Pz, q[3]);
+      count += __ldcg(&c_count[ch + k]);
     }
+    c_count[c] = count; c_child_count[c] = (uint8_t)nch;
+    a.cell_b[c] = make_uint4(0u, ch, (uint32_t)nch, (uint32_t)level << 8);
   }
   double* o = MP + 4 * (size_t)c;
   o[0] = M; o[1] = Px; o[2] = Py; o[3] = Pz;
@@ -313,12 +337,12 @@ __global__ void __launch_bounds__(256) moments_all_kernel(const LevelOff off, co
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
   for (int l = depth; l > top; l--) {
-    for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) moments_cell(c, l, a);
+    for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) moments_cell(c, l, l < OTOO_MAXLEV ? off.v[l + 2] : off.v[l + 1], a);
     grid.sync();
   }
   if (blockIdx.x != 0) return;
   for (int l = top < depth ? top : depth; l >= 0; l--) {
-    for (uint32_t c = off.v[l] + threadIdx.x; c < off.v[l + 1]; c += blockDim.x) moments_cell(c, l, a);
+    for (uint32_t c = off.v[l] + threadIdx.x; c < off.v[l + 1]; c += blockDim.x) moments_cell(c, l, l < OTOO_MAXLEV ? off.v[l + 2] : off.v[l + 1], a);
     __syncthreads();
   }
 }
@@ -413,6 +437,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 64 * sizeof(uint32_t), st));
   int gb = ctx->sm_count * 4; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
+  ctx->launches += 1;
   OTOO_EV(ctx, ctx->ev_build[1], st);
   // H2, H3, H4
   // keys and ids, and in the same read the eight digit histograms of the sort (otoo_keys_and_hist, sort.cu)
@@ -423,36 +448,43 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_TRY(otoo_sort_pairs(ctx, ctx->key, ctx->val, N, 0, 64, st, &res, true));
   if (res != 0) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: sort result buffer");
   OTOO_EV(ctx, ctx->ev_build[3], st);
-  gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
-  OTOO_EV(ctx, ctx->ev_build[4], st);
-  // H5a
+  // H4 + H5a: positions into sorted order and, in the same kernel, the levels of the cells that start at each slot
   uint32_t* info = ctx->val[1];
   uint32_t* blk_lc = ctx->slot_nc;                 // OTOO_NLEV x nbN per-block level counts, then their exclusive scan
-  if (n_crit <= OTOO_SLOT_NCRIT_MAX) slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info, ctx->d_counters);
-  else slot_cells_wide_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info, ctx->d_counters);
+  if (n_crit <= OTOO_SLOT_NCRIT_MAX)
+    slot_cells_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info, pos, ctx->val[0], ctx->spos);
+  else {
+    gather4_kernel<<<nbN, 256, 0, st>>>(pos, ctx->val[0], N, ctx->spos);
+    slot_cells_wide_kernel<<<nbN, 256, 0, st>>>(ctx->key[0], N, n_crit, blk_lc, info);
+    ctx->launches += 1;
+  }
   ctx->launches += 1;
-  OTOO_TRY(otoo_exclusive_scan_u32(ctx, blk_lc, (int64_t)OTOO_NLEV * nbN, ctx->d_counters + 40, st));
-  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, 64 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  OTOO_EV(ctx, ctx->ev_build[4], st);
+  // one exclusive scan of the OTOO_NLEV + 1 rows: the canonical index of every block's first cell of each level, and at
+  // the start of row l the number of cells of the levels below l (row OTOO_NLEV starts at N_cell; the rest is the leaves)
+  OTOO_TRY(otoo_exclusive_scan_u32(ctx, blk_lc, (int64_t)(OTOO_NLEV + 1) * nbN, ctx->d_counters + 40, st));
+  OTOO_CUDA(ctx, cudaMemcpy2DAsync(ctx->h_counters, sizeof(uint32_t), blk_lc, (size_t)nbN * sizeof(uint32_t), sizeof(uint32_t), OTOO_NLEV + 1,
+                                   cudaMemcpyDeviceToHost, st));
+  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 40, ctx->d_counters + 40, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_root, ctx->d_bbox + 8, 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaStreamSynchronize(st));
-  int64_t ncell = ctx->h_counters[40];
   LevelOff off;
-  uint32_t run = 0; int depth = 0;
-  for (int l = 0; l < OTOO_NLEV; l++) { off.v[l] = run; run += ctx->h_counters[l]; if (ctx->h_counters[l]) depth = l; }
-  off.v[OTOO_NLEV] = run;
-  if ((int64_t)run != ncell || ncell < 1) return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: level counts disagree with cell count");
+  int depth = 0;
+  for (int l = 0; l <= OTOO_NLEV; l++) off.v[l] = ctx->h_counters[l];
+  for (int l = 0; l < OTOO_NLEV; l++) if (off.v[l + 1] > off.v[l]) depth = l;
+  const int64_t ncell = off.v[OTOO_NLEV];
+  if (ncell < 1 || (int64_t)ctx->h_counters[40] < ncell || off.v[0] != 0u)
+    return otoo_fail(ctx, OTOO_ERR_CUDA, "internal: level offsets disagree with the cell count");
+  ctx->h_counters[32] = ctx->h_counters[40] - (uint32_t)ncell;          // N_leaf (otoo_tree_info)
   OTOO_TRY(ensure_cells(ctx, ncell));
-  const unsigned nbC = (unsigned)cdiv(ncell, 256);
-  // H5b: cells in canonical order (level, first slot); H5c
-  place_cells_kernel<<<nbN, 256, 0, st>>>(info, N, blk_lc, ctx->tmp_val[0]);
-  cell_topology_kernel<<<nbC, 256, 0, st>>>(ctx->tmp_val[0], ncell, ctx->key[0], N, n_crit, off,
-                                            ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level,
-                                            ctx->c_child_count, ctx->cell_b, ctx->d_counters + 32);
-  ctx->launches += 2;
+  // H5b: cells in canonical order (level, first slot), leaves complete
+  const CellOut co{ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->cell_b};
+  place_cells_kernel<<<nbN, 256, 0, st>>>(info, ctx->key[0], N, blk_lc, co);
+  ctx->launches += 1;
   OTOO_EV(ctx, ctx->ev_build[5], st);
-  // H6 deepest level first
+  // H5c of the internal cells + H6, deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order};
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, info, ctx->cell_b};
   {
     int occ = 1;
     OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));
@@ -469,7 +501,6 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   }
   OTOO_EV(ctx, ctx->ev_build[6], st);
   ctx->ev_build_valid = true;
-  OTOO_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 32, ctx->d_counters + 32, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->N = N; ctx->N_cell = ncell; ctx->n_crit = n_crit; ctx->depth = depth;
   for (int k = 0; k < 3; k++) ctx->lo[k] = ctx->h_root[k];
@@ -486,7 +517,8 @@ otoo_status otoo_b2_impl(otoo_ctx* ctx, cudaStream_t st) {
   LevelOff off;
   for (int l = 0; l <= OTOO_NLEV; l++) off.v[l] = ctx->level_off[l];
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      reinterpret_cast<const unsigned*>(ctx->d_bbox), ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order_built};
+                      reinterpret_cast<const unsigned*>(ctx->d_bbox), ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order_built,
+                      nullptr, ctx->cell_b};
   int occ = 1;
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, b2_all_kernel, 256, 0));
   if (occ > 4) occ = 4;

@@ -7,6 +7,9 @@
 #ifndef OTOO_EVAL_UNR
 #define OTOO_EVAL_UNR 4
 #endif
+#ifndef OTOO_EVAL_ACC
+#define OTOO_EVAL_ACC 0
+#endif
 
 namespace {
 
@@ -25,7 +28,8 @@ __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
 
 // PB_ = target pairs per pass over the list (0: the default, min(NP, 2)); UNR_ = unroll factor of the entry loop
-template <int T_, bool EPS0, int PB_ = 0, int UNR_ = OTOO_EVAL_UNR>
+// ACC_ = form of the three accumulations c += (m/r^3) d: 0 packed FFMA2 (three distinct register pairs each), 1 six scalar FFMA
+template <int T_, bool EPS0, int PB_ = 0, int UNR_ = OTOO_EVAL_UNR, int ACC_ = OTOO_EVAL_ACC>
 struct GravVisitor {
   static constexpr int T = T_, E = 1, LCAP = OTOO_LIST_CAP, NP = (T_ + 1) / 2, PB = PB_ ? (PB_ < NP ? PB_ : NP) : (NP < 2 ? NP : 2), BLK = 64, UNR = UNR_;
   const GravParams& p;
@@ -130,9 +134,14 @@ struct GravVisitor {
             const float2 mri = __fmul2_rn(bc2(s.w), ri);
             const float2 mr3 = __fmul2_rn(mri, __fmul2_rn(ri, ri));
             cp[q] = __fadd2_rn(cp[q], neg2(mri));
-            cx[q] = __ffma2_rn(mr3, dx, cx[q]);
-            cy[q] = __ffma2_rn(mr3, dy, cy[q]);
-            cz[q] = __ffma2_rn(mr3, dz, cz[q]);
+            if (ACC_ == 0) {
+              cx[q] = __ffma2_rn(mr3, dx, cx[q]);
+              cy[q] = __ffma2_rn(mr3, dy, cy[q]);
+              cz[q] = __ffma2_rn(mr3, dz, cz[q]);
+            } else {
+              cx[q].x = __fmaf_rn(mr3.x, dx.x, cx[q].x); cy[q].x = __fmaf_rn(mr3.x, dy.x, cy[q].x); cz[q].x = __fmaf_rn(mr3.x, dz.x, cz[q].x);
+              cx[q].y = __fmaf_rn(mr3.y, dx.y, cx[q].y); cy[q].y = __fmaf_rn(mr3.y, dy.y, cy[q].y); cz[q].y = __fmaf_rn(mr3.y, dz.y, cz[q].y);
+            }
           }
         }
 #pragma unroll

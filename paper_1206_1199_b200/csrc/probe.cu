@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(512, 1) ffma2_probe_kernel(const f32x2* __rest
 }
 
 // ---------------------------------------------------------------- the sum loop alone
-template <int T, int PB, int UNR>
+template <int T, int PB, int UNR, int ACC>
 __global__ void __launch_bounds__(128, T >= 8 ? 2 : 3) sumloop_probe_kernel(const GravParams p, int reps, float4* __restrict__ sink,
                                                                              unsigned long long* __restrict__ cycles) {
   __shared__ __align__(16) float4 lists[4][OTOO_LIST_CAP + 4];
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(128, T >= 8 ? 2 : 3) sumloop_probe_kernel(cons
     list[j] = make_float4(x, y, z, 1.0f / OTOO_LIST_CAP);
   }
   __syncwarp();
-  GravVisitor<T, false, PB, UNR> v(p);
+  GravVisitor<T, false, PB, UNR, ACC> v(p);
   const int64_t g0 = ((int64_t)(blockIdx.x * 4 + warp) * (32 * T)) % (p.c.N - 32 * T);
   __shared__ __align__(16) float2 scratch[4][32 * ((T + 1) / 2) * 3];
   v.load_group(g0, lane, reinterpret_cast<float4*>(scratch[warp]));
@@ -172,28 +172,28 @@ double run_rank(otoo_ctx* ctx, const uint32_t* in, uint32_t* out, unsigned long 
   return sum / n / ((double)iters * 8 * warps);          // SM cycles per warp instruction (all warps of the SM share the unit)
 }
 
-template <int T, int PB, int UNR>
+template <int T, int PB, int UNR, int ACC = OTOO_EVAL_ACC>
 otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long long* d_cyc, cudaStream_t st, std::string& js,
                         int per_sm_arg = 0) {
   const int reps = 256;
   int occ = 0;
-  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR>, 128, 0));
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR, ACC>, 128, 0));
   cudaFuncAttributes fa;
-  OTOO_CUDA(ctx, cudaFuncGetAttributes(&fa, sumloop_probe_kernel<T, PB, UNR>));
+  OTOO_CUDA(ctx, cudaFuncGetAttributes(&fa, sumloop_probe_kernel<T, PB, UNR, ACC>));
   const int per_sm = per_sm_arg ? per_sm_arg : (T >= 8 ? 2 : 3);   // CTAs of 4 evaluator warps per SM (default: the product kernel's)
   const int grid = ctx->sm_count * per_sm;
   // dynamic shared memory sized so that EXACTLY per_sm CTAs fit an SM: every SM then runs per_sm CTAs of the
   // grid at once (left to the occupancy of the kernel alone the block scheduler packs 4 on some SMs and 2 on others)
   const size_t dyn = (size_t)(227 * 1024) / per_sm - fa.sharedSizeBytes - 2048;
-  OTOO_CUDA(ctx, cudaFuncSetAttribute(sumloop_probe_kernel<T, PB, UNR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR>, 128, dyn));
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(sumloop_probe_kernel<T, PB, UNR, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sumloop_probe_kernel<T, PB, UNR, ACC>, 128, dyn));
   if (occ != per_sm) return otoo_fail(ctx, OTOO_ERR_CUDA, "probe: occupancy is not the evaluator's");
   Timer tm;
-  sumloop_probe_kernel<T, PB, UNR><<<grid, 128, dyn, st>>>(p, 4, sink, d_cyc);
+  sumloop_probe_kernel<T, PB, UNR, ACC><<<grid, 128, dyn, st>>>(p, 4, sink, d_cyc);
   float best = 1e30f;
   for (int r = 0; r < 3; r++) {
     tm.start(st);
-    sumloop_probe_kernel<T, PB, UNR><<<grid, 128, dyn, st>>>(p, reps, sink, d_cyc);
+    sumloop_probe_kernel<T, PB, UNR, ACC><<<grid, 128, dyn, st>>>(p, reps, sink, d_cyc);
     const float ms = tm.stop(st);
     if (ms < best) best = ms;
   }
@@ -214,9 +214,9 @@ otoo_status run_sumloop(otoo_ctx* ctx, GravParams p, float4* sink, unsigned long
   const double per_pair = (double)best * 1e-3 * sm_mhz * 1e6 / ((double)per_sm * ((T + 1) / 2) * OTOO_LIST_CAP * reps);
   char buf[512];
   snprintf(buf, sizeof buf,
-           "{\"name\": \"sumloop G=%d\", \"pairs_per_pass\": %d, \"unroll\": %d, \"eval_warps_per_sm\": %d, \"registers\": %d, \"occupancy_ctas\": %d, \"ms\": %.4f, "
+           "{\"name\": \"sumloop G=%d\", \"accumulate\": \"%s\", \"pairs_per_pass\": %d, \"unroll\": %d, \"eval_warps_per_sm\": %d, \"registers\": %d, \"occupancy_ctas\": %d, \"ms\": %.4f, "
            "\"interactions_per_s\": %.6e, \"tflops_20flop\": %.3f, \"smsp_cycles_per_pair_entry\": %.3f, \"sm_mhz_during_loop\": %.0f}",
-           32 * T, GravVisitor<T, false, PB, UNR>::PB, UNR, 4 * per_sm, fa.numRegs, occ, best, inter / (best * 1e-3), 20.0 * inter / (best * 1e-3) / 1e12, per_pair, sm_mhz);
+           32 * T, ACC ? "scalar FFMA" : "FFMA2", GravVisitor<T, false, PB, UNR>::PB, UNR, 4 * per_sm, fa.numRegs, occ, best, inter / (best * 1e-3), 20.0 * inter / (best * 1e-3) / 1e12, per_pair, sm_mhz);
   if (!js.empty()) js += ", ";
   js += buf;
   return OTOO_OK;
@@ -274,6 +274,12 @@ extern "C" otoo_status otoo_probe(otoo_ctx* ctx, const char* which, char* host_j
     OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 4)));
     OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR>(ctx, p, sink, d_cyc, st, js, 5)));
+    // the other form of the accumulations (scalar FFMA <-> FFMA2) at the product's three configurations
+    OTOO_TRY((run_sumloop<2, 0, OTOO_EVAL_UNR, 1 - OTOO_EVAL_ACC>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 0, OTOO_EVAL_UNR, 1 - OTOO_EVAL_ACC>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 0, OTOO_EVAL_UNR, 1 - OTOO_EVAL_ACC>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<4, 2, 8, 1 - OTOO_EVAL_ACC>(ctx, p, sink, d_cyc, st, js)));
+    OTOO_TRY((run_sumloop<8, 4, 2, 1 - OTOO_EVAL_ACC>(ctx, p, sink, d_cyc, st, js)));
   } else if (strcmp(which, "rank") == 0) {
     sort_fill_kernel<<<64, 256, 0, st>>>(ctx->key[0], ctx->val[0], 64 * 256);
     const uint32_t* digits = reinterpret_cast<const uint32_t*>(ctx->key[0]);

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_hist_all_kernel(const uint
 // H2 fused with the histograms: keys and ids of all particles and, in the same pass over them, the eight digit
 // histograms of the 64-bit sort (one read of the positions instead of a key kernel plus a read of the keys)
 __global__ void __launch_bounds__(SORT_THREADS) key_hist_kernel(const float4* __restrict__ pos, int64_t n, const unsigned* __restrict__ bbox,
-                                                                uint64_t* __restrict__ key, uint32_t* __restrict__ id, int hilbert,
+                                                                uint64_t* __restrict__ key, int hilbert,
                                                                 uint32_t* __restrict__ ghist, uint32_t* __restrict__ done) {
   __shared__ uint32_t sh[OS_MAXPASS][256];
   const int tid = threadIdx.x;
@@ -83,8 +83,7 @@ __global__ void __launch_bounds__(SORT_THREADS) key_hist_kernel(const float4* __
   const float* root = reinterpret_cast<const float*>(bbox) + 8;
   for (int64_t i = (int64_t)blockIdx.x * SORT_THREADS + tid; i < n; i += (int64_t)gridDim.x * SORT_THREADS) {
     const uint64_t k = particle_key(pos[i], root, hilbert);
-    key[i] = k;
-    id[i] = (uint32_t)i;
+    key[i] = k;                                        // (the ids 0, 1, 2, ... are not written: the first sort pass makes them up)
     for (int p = 0; p < OS_MAXPASS; p++) atomicAdd(&sh[p][(unsigned)(k >> (8 * p)) & 0xFF], 1u);
   }
   __syncthreads();
@@ -151,7 +150,8 @@ __global__ void __launch_bounds__(OS_THREADS, MINB) onesweep_pass_kernel(const u
 #pragma unroll
   for (int i = 0; i < OS_ITEMS; i++) {
     int64_t idx = base + i * 32 + lane;
-    if (idx < n) { k[i] = kin[idx]; v[i] = vin[idx]; }   // (values loaded after the ranking instead: 2.46 -> 3.53 ms at 32 M pairs)
+    if (idx < n) { k[i] = kin[idx]; v[i] = vin ? vin[idx] : (uint32_t)idx; }   // vin == nullptr: the ids are still 0, 1, 2, ... (first pass of the build)
+                                                                               // (values loaded after the ranking instead: 2.46 -> 3.53 ms at 32 M pairs)
     else { k[i] = ~0ull; v[i] = 0; }
   }
   const unsigned lt = lanemask_lt();
@@ -337,13 +337,13 @@ static otoo_status sort_epoch_check(otoo_ctx* ctx, int npass, cudaStream_t st) {
   return OTOO_OK;
 }
 
-// keys (R2, R3, R20) and ids of the particles into key[0] / val[0], and the digit offsets of the 8-pass sort that follows
+// keys (R2, R3, R20) of the particles into key[0] (ids: see otoo_sort_pairs), and the digit offsets of the 8-pass sort that follows
 otoo_status otoo_keys_and_hist(otoo_ctx* ctx, const float* d_pos_mass, int64_t n, cudaStream_t st) {
   OTOO_TRY(sort_epoch_check(ctx, OS_MAXPASS, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->hist, 0, OS_STATUS * sizeof(uint32_t), st));   // histograms + tickets
   int gh = ctx->sm_count * 4; if (gh > (int)cdiv(n, SORT_THREADS)) gh = (int)cdiv(n, SORT_THREADS);
   key_hist_kernel<<<gh, SORT_THREADS, 0, st>>>(reinterpret_cast<const float4*>(d_pos_mass), n, reinterpret_cast<const unsigned*>(ctx->d_bbox),
-                                               ctx->key[0], ctx->val[0], ctx->key_order, ctx->hist + OS_GHIST, ctx->hist + OS_TICKET + 255);
+                                               ctx->key[0], ctx->key_order, ctx->hist + OS_GHIST, ctx->hist + OS_TICKET + 255);
   OTOO_CUDA(ctx, cudaGetLastError());
   return OTOO_OK;
 }
@@ -374,12 +374,13 @@ otoo_status otoo_sort_pairs(otoo_ctx* ctx, uint64_t* key[2], uint32_t* val[2], i
     }
     unsigned long long* status = reinterpret_cast<unsigned long long*>(ctx->hist + OS_STATUS);
     for (int p = 0; p < npass; p++) {
+      const uint32_t* vin = (p == 0 && hist_done) ? nullptr : val[cur];   // after otoo_keys_and_hist the ids are 0, 1, 2, ... and not stored
       // few tiles per SM: 2 CTAs of 16 warps hide more latency; many: 3 CTAs of 8 warps keep the shared-memory pipe busier
       if (n <= OS_SMALL_N)
-        onesweep_pass_kernel<512, 2><<<nb, 512, os_smem(512), st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
+        onesweep_pass_kernel<512, 2><<<nb, 512, os_smem(512), st>>>(key[cur], vin, key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
                                                                       ctx->hist + OS_GHIST + p * 256, status, ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
       else
-        onesweep_pass_kernel<256, 3><<<nb, 256, os_smem(256), st>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
+        onesweep_pass_kernel<256, 3><<<nb, 256, os_smem(256), st>>>(key[cur], vin, key[cur ^ 1], val[cur ^ 1], n, first_bit + 8 * p,
                                                                       ctx->hist + OS_GHIST + p * 256, status, ctx->hist + OS_TICKET + p, ++ctx->sort_epoch);
       ctx->launches += 1;
       cur ^= 1;
