@@ -28,11 +28,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     flags = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+    flags += os.environ.get("OTOO_NVCC_FLAGS", "").split()      # e.g. -DOTOO_EVAL_UNR=8 for an A/B library
     if verbose:
         flags += ["-Xptxas", "-v"]
 
+    hdr_time = max(os.path.getmtime(os.path.join(HERE, "csrc", h)) for h in HEADERS)
+
     def compile_one(f: str) -> str:          # one nvcc per translation unit, side by side (no device code crosses files)
         obj = os.path.join(objdir, f.replace(".cu", ".o"))
+        src_time = max(hdr_time, os.path.getmtime(os.path.join(HERE, "csrc", f)))
+        if not verbose and os.path.exists(obj) and os.path.getmtime(obj) > src_time:
+            return obj                       # (an object newer than its source and every header is kept)
         subprocess.run(["nvcc"] + flags + ["-c", os.path.join(HERE, "csrc", f), "-o", obj], check=True)
         return obj
 

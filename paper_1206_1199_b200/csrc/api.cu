@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(256) export_cells_kernel(int64_t ncell, const 
   if (c >= ncell) return;
   otoo_cell_t o;
   memset(&o, 0, sizeof o);
-  o.level = c_level[c]; o.first = c_first[c]; o.count = c_count[c];
+  o.level = c_level[c] & 0x1F; o.first = c_first[c]; o.count = c_count[c];
   o.child_first = c_child_first[c]; o.child_count = c_child_count[c];
   o.prefix = (o.level > 0 && o.count > 0) ? key[o.first] >> (3 * (OTOO_MAXLEV - o.level)) : 0ull;
   out[c] = o;

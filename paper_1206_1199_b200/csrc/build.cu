@@ -87,6 +87,9 @@ __device__ __forceinline__ int cplev(uint64_t a, uint64_t b) {  // common leadin
 // plain form recomputed its n_crit+1 windows from global memory: 480 GB/s at 32 M particles), the per-level
 // counts are warp-aggregated (one ballot per level instead of contended shared-memory atomics).
 #define OTOO_SLOT_NCRIT_MAX 256
+#ifndef OTOO_GATHER_L2HINT
+#define OTOO_GATHER_L2HINT ".L2::64B"        // a miss fetches 64 B instead of the default 128 B (gather + levels 0.86 -> 0.81 ms at 32 M)
+#endif
 // H4 rides along: the block's 256 random 16-byte reads of the gather (HBM-latency-bound, 3.7 x its algorithmic bytes
 // for an unordered input) are issued first and stored last, so they are in flight while the block does its
 // issue-bound level arithmetic (as kernels of their own: 0.72 + 0.46 ms at 32 M particles).
@@ -100,7 +103,7 @@ __global__ void __launch_bounds__(256) slot_cells_kernel(const uint64_t* __restr
   float4 pv = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   if (s0 + threadIdx.x < n) {
     const float4* src = pos + perm[s0 + threadIdx.x];
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(pv.x), "=f"(pv.y), "=f"(pv.z), "=f"(pv.w) : "l"(src));
+    asm volatile("ld.global.nc.L1::no_allocate" OTOO_GATHER_L2HINT ".v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(pv.x), "=f"(pv.y), "=f"(pv.z), "=f"(pv.w) : "l"(src));
   }
   const int m = 256 + n_crit;                       // window starts t = s0 - n_crit + i, i < m
   if (threadIdx.x <= OTOO_NLEV) lc[threadIdx.x] = 0;
@@ -197,9 +200,18 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
   __syncthreads();
   const bool has = lo <= LL;
   const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
+  // the leaf's particle count = distance to the next slot that starts a range of the leaf's level or a coarser one:
+  // per level a ballot over the warp's 32 slots and one over the 32 slots after them
+  const int lo_term = s < n ? lo : 0, lo_next = (int)slo[threadIdx.x + 32];      // (slots past the end end every range)
+  uint32_t count = 0;
   for (int l = wlo; l <= whi; l++) {
     const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, lo_term <= l), m2 = __ballot_sync(0xFFFFFFFFu, lo_next <= l);
     if (lane == 0) wc[warp][l] = (uint32_t)__popc(b);
+    if (l == LL) {
+      const unsigned long long mm = (((unsigned long long)m2 << 32) | m) >> (lane + 1);
+      count = mm ? (uint32_t)__ffsll((long long)mm) : 0u;           // 0: not within the next 63 - lane slots
+    }
   }
   __syncthreads();
   if (threadIdx.x < OTOO_NLEV) {
@@ -208,9 +220,7 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
     for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
   }
   __syncthreads();
-  // the leaf's particle count
-  uint32_t count = 0;
-  if (has) {
+  if (has && (count == 0u || LL == 0)) {
     if (LL == 0) count = (uint32_t)n;
     else {
       int j = threadIdx.x + 1;
@@ -235,12 +245,13 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
     const unsigned b = __ballot_sync(0xFFFFFFFFu, mine);
     if (mine) {
       const uint32_t c = wc[warp][l] + (uint32_t)__popc(b & lt);
-      o.c_first[c] = (uint32_t)s; o.c_level[c] = (uint8_t)l;
+      o.c_first[c] = (uint32_t)s;
+      o.c_level[c] = (uint8_t)(l | (l > lo ? 0x80 : 0));   // bit 7: the parent starts at this slot too = first of its siblings
       if (l == LL) {
         o.c_count[c] = count; o.c_child_first[c] = 0u; o.c_child_count[c] = 0;
         o.cell_b[c] = make_uint4(0u, (uint32_t)s, count, 1u | ((uint32_t)l << 8));
       } else {
-        o.c_child_first[c] = below; o.c_child_count[c] = 0xFF;        // internal: count and children bottom-up
+        o.c_child_first[c] = below;                                    // internal (>= 1): count and children bottom-up
       }
       below = c;
     }
@@ -255,7 +266,7 @@ struct MomentArgs {
   const uint32_t* c_child_first; uint8_t* c_child_count; const unsigned* bbox;
   double* MP; double* cm64; float4* cell_cm; double* c_s; double* c_B2;
   int hilbert;
-  const uint32_t* info; cellb_t* cell_b;          // H5c for the internal cells (moments_all_kernel only)
+  const uint8_t* c_level; cellb_t* cell_b;        // H5c for the internal cells (moments_all_kernel only)
 };
 // level_end = canonical index one past the last cell of level + 1 (the children's level)
 __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t level_end, const MomentArgs& a) {
@@ -264,17 +275,24 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
   const uint32_t* __restrict__ c_child_first = a.c_child_first; uint8_t* c_child_count = a.c_child_count;
   const unsigned* __restrict__ bbox = a.bbox;
   double* MP = a.MP; double* cm64 = a.cm64; float4* cell_cm = a.cell_cm; double* c_s = a.c_s;
-  const uint32_t first = c_first[c];
-  uint32_t count;
-  int nch = c_child_count[c];
+  const uint32_t first = c_first[c], ch = c_child_first[c];   // ch == 0: a leaf (the root's first child is cell 1)
+  uint32_t count = c_count[c];                                 // (of a leaf; an internal cell's is found below)
+  int nch = 0;
   double M = 0.0, Px = 0.0, Py = 0.0, Pz = 0.0;
-  if (nch == 0) {
-    count = c_count[c];
+  const float* r = reinterpret_cast<const float*>(bbox) + 8;
+  // integer cell coordinates = top `level` bits of the quantised coordinates (R2) of any particle of the cell
+  uint32_t qx = 0, qy = 0, qz = 0;
+  if (ch == 0u) {
     for (uint32_t s0 = first; s0 < first + count; s0 += 8) {   // 8 loads in flight, sums in slot order (R6)
       float4 p[8];
       const uint32_t nv = first + count - s0 < 8u ? first + count - s0 : 8u;
 #pragma unroll
       for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) p[j] = spos[s0 + j];
+      if (s0 == first && level > 0) {                          // from the first particle itself (no read of its key)
+        const float scale = r[4];
+        qx = quant(p[0].x, r[0], scale) >> (OTOO_MAXLEV - level); qy = quant(p[0].y, r[1], scale) >> (OTOO_MAXLEV - level);
+        qz = quant(p[0].z, r[2], scale) >> (OTOO_MAXLEV - level);
+      }
 #pragma unroll
       for (int j = 0; j < 8; j++) if ((uint32_t)j < nv) {
         double m = (double)p[j].w;
@@ -287,14 +305,10 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
   } else {
     // H5c for an internal cell: its children are the cell one level down at its own first slot and the cells after
     // that one (canonical order = octant order) whose first slot starts a range of the children's level but not of
-    // this cell's (lo == level + 1: still inside this cell); its particles are theirs
-    const uint32_t ch = c_child_first[c];
-    uint32_t f[8];
-    unsigned sib = 1u;                                 // bit k: cell ch + k exists and does not start a new parent
+    // this cell's (bit 7 of c_level clear: not the first child of another parent); its particles are theirs
+    unsigned sib = 1u;                                 // bit k: cell ch + k exists and is not the first child of the next parent
 #pragma unroll
-    for (int k = 1; k < 8; k++) f[k] = ch + k < level_end ? c_first[ch + k] : 0xFFFFFFFFu;
-#pragma unroll
-    for (int k = 1; k < 8; k++) if (f[k] != 0xFFFFFFFFu && (int)(a.info[f[k]] & 0xFF) == level + 1) sib |= 1u << k;
+    for (int k = 1; k < 8; k++) if (ch + k < level_end && !(a.c_level[ch + k] & 0x80)) sib |= 1u << k;
     nch = __ffs(~sib) - 1;                             // the run of siblings from ch
     count = 0;
     for (int k = 0; k < nch; k++) {
@@ -304,19 +318,16 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
     }
     c_count[c] = count; c_child_count[c] = (uint8_t)nch;
     a.cell_b[c] = make_uint4(0u, ch, (uint32_t)nch, (uint32_t)level << 8);
+    if (level > 0) {                                   // (internal cells are few: from the key of the first particle)
+      const uint64_t k0 = key[first];
+      qx = compact3(k0 >> 2); qy = compact3(k0 >> 1); qz = compact3(k0);
+      if (a.hilbert) hilbert_transpose_to_axes(qx, qy, qz);
+      qx >>= OTOO_MAXLEV - level; qy >>= OTOO_MAXLEV - level; qz >>= OTOO_MAXLEV - level;
+    }
   }
   double* o = MP + 4 * (size_t)c;
   o[0] = M; o[1] = Px; o[2] = Py; o[3] = Pz;
-  const float* r = reinterpret_cast<const float*>(bbox) + 8;
   double l = ldexp((double)r[3], -level);
-  // integer cell coordinates = top `level` bits of the quantised coordinates of any particle of the cell
-  uint32_t qx = 0, qy = 0, qz = 0;
-  if (count > 0 && level > 0) {
-    const uint64_t k0 = key[first];
-    qx = compact3(k0 >> 2); qy = compact3(k0 >> 1); qz = compact3(k0);
-    if (a.hilbert) hilbert_transpose_to_axes(qx, qy, qz);
-    qx >>= OTOO_MAXLEV - level; qy >>= OTOO_MAXLEV - level; qz >>= OTOO_MAXLEV - level;
-  }
   double g[3];
   g[0] = __dadd_rn((double)r[0], __dmul_rn((double)qx + 0.5, l));
   g[1] = __dadd_rn((double)r[1], __dmul_rn((double)qy + 0.5, l));
@@ -333,7 +344,10 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
 // Levels 0 .. top are narrow (the top of the tree: 1, 8, 64, ... cells): one CTA finishes them with block barriers
 // instead of grid barriers.
-__global__ void __launch_bounds__(256) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
+#ifndef OTOO_MOMENTS_MINB
+#define OTOO_MOMENTS_MINB 2
+#endif
+__global__ void __launch_bounds__(256, OTOO_MOMENTS_MINB) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
   for (int l = depth; l > top; l--) {
@@ -484,7 +498,7 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_EV(ctx, ctx->ev_build[5], st);
   // H5c of the internal cells + H6, deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, info, ctx->cell_b};
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, ctx->c_level, ctx->cell_b};
   {
     int occ = 1;
     OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));

@@ -55,7 +55,7 @@ struct otoo_ctx {
   uint32_t* c_first;
   uint32_t* c_count;
   uint32_t* c_child_first;
-  uint8_t* c_level;
+  uint8_t* c_level;      // level in bits 0..4; bit 7: the cell is the first child of its parent (build.cu, H5c)
   uint8_t* c_child_count;
   double* c_MP;          // 4 per cell: M, Px, Py, Pz (R6)
   double* c_cm64;        // 3 per cell: fp64 centre of mass (needed for Eq. 5)

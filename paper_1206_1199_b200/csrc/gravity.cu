@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_
   float rb2;
   if (!(theta > 0.0f)) rb2 = INFINITY;
   else {
-    double l = ldexp((double)S, -(int)c_level[c]);
+    double l = ldexp((double)S, -(int)(c_level[c] & 0x1F));   // (bit 7 of c_level: first-sibling flag of the build)
     double rb = __dadd_rn(__ddiv_rn(l, (double)theta), c_s[c]);
     rb2 = __double2float_rn(__dmul_rn(rb, rb));
   }
