@@ -267,6 +267,8 @@ struct MomentArgs {
   double* MP; double* cm64; float4* cell_cm; double* c_s; double* c_B2;
   int hilbert;
   const uint8_t* c_level; cellb_t* cell_b;        // H5c for the internal cells (moments_all_kernel only)
+  int do_rb2; float theta;                         // R7 for the theta of the last gravity call (moments_all_kernel only)
+  uint32_t* walk_ws; uint32_t* walk_seq;           // the walk's control block and pool sequence numbers to reset (or null)
 };
 // level_end = canonical index one past the last cell of level + 1 (the children's level)
 __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t level_end, const MomentArgs& a) {
@@ -338,7 +340,14 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
   cm64[3 * (size_t)c] = cx; cm64[3 * (size_t)c + 1] = cy; cm64[3 * (size_t)c + 2] = cz;
   cell_cm[c] = make_float4(__double2float_rn(cx), __double2float_rn(cy), __double2float_rn(cz), __double2float_rn(M));
   double dx = __dsub_rn(cx, g[0]), dy = __dsub_rn(cy, g[1]), dz = __dsub_rn(cz, g[2]);
-  c_s[c] = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+  const double sd = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+  c_s[c] = sd;
+  if (a.do_rb2) {
+    // R7, the operations of rb2_kernel (gravity.cu): r_b = l/theta + s in fp64, rb^2 rounded once to fp32
+    float rb2 = INFINITY;
+    if (a.theta > 0.0f) { const double rb = __dadd_rn(__ddiv_rn(l, (double)a.theta), sd); rb2 = __double2float_rn(__dmul_rn(rb, rb)); }
+    reinterpret_cast<uint32_t*>(a.cell_b + c)[0] = __float_as_uint(rb2);
+  }
 }
 // the whole bottom-up pass in ONE cooperative launch: every level deepest first, a grid-wide barrier
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
@@ -350,6 +359,10 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
 __global__ void __launch_bounds__(256, OTOO_MOMENTS_MINB) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+  if (a.walk_seq) {                                  // the next walk finds its control block and pool reset (was part of the r_b kernel)
+    for (uint32_t i = tid; i < OTOO_POOL_SLOTS; i += nthr) a.walk_seq[i] = i;
+    if (tid < 128) a.walk_ws[tid] = 0u;              // WalkShared: queue, head, tail, outstanding, one 128-byte line each
+  }
   for (int l = depth; l > top; l--) {
     for (uint32_t c = off.v[l] + tid; c < off.v[l + 1]; c += nthr) moments_cell(c, l, l < OTOO_MAXLEV ? off.v[l + 2] : off.v[l + 1], a);
     grid.sync();
@@ -440,6 +453,7 @@ __global__ void __launch_bounds__(256) b2_all_kernel(const LevelOff off, const i
 
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st) {
   ctx->built = false; ctx->walked = false; ctx->sph_radii_valid = false; ctx->b2_valid = false;
+  ctx->rb2_valid = false; ctx->walk_reset_valid = false;
   const float4* pos = reinterpret_cast<const float4*>(d_pos_mass);
   unsigned* bbox = reinterpret_cast<unsigned*>(ctx->d_bbox);
   const unsigned nbN = (unsigned)cdiv(N, 256);
@@ -498,7 +512,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   OTOO_EV(ctx, ctx->ev_build[5], st);
   // H5c of the internal cells + H6, deepest level first
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
-                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, ctx->c_level, ctx->cell_b};
+                      bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, ctx->c_level, ctx->cell_b,
+                      ctx->spec_theta_set ? 1 : 0, ctx->spec_theta, (uint32_t*)ctx->walk_shared, (uint32_t*)ctx->pool_seq};
   {
     int occ = 1;
     OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));
@@ -515,6 +530,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   }
   OTOO_EV(ctx, ctx->ev_build[6], st);
   ctx->ev_build_valid = true;
+  if (ctx->spec_theta_set) { ctx->rb2_valid = true; ctx->rb2_theta = ctx->spec_theta; }
+  ctx->walk_reset_valid = ctx->pool_seq != nullptr;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->N = N; ctx->N_cell = ncell; ctx->n_crit = n_crit; ctx->depth = depth;
   for (int k = 0; k < 3; k++) ctx->lo[k] = ctx->h_root[k];
@@ -532,7 +549,7 @@ otoo_status otoo_b2_impl(otoo_ctx* ctx, cudaStream_t st) {
   for (int l = 0; l <= OTOO_NLEV; l++) off.v[l] = ctx->level_off[l];
   const MomentArgs ma{ctx->spos, ctx->key[0], ctx->c_first, ctx->c_count, ctx->c_child_first, ctx->c_child_count,
                       reinterpret_cast<const unsigned*>(ctx->d_bbox), ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order_built,
-                      nullptr, ctx->cell_b};
+                      nullptr, ctx->cell_b, 0, 0.0f, nullptr, nullptr};
   int occ = 1;
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, b2_all_kernel, 256, 0));
   if (occ > 4) occ = 4;

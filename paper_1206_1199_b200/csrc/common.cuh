@@ -8,6 +8,7 @@
 
 #define OTOO_MAXLEV 21
 #define OTOO_NLEV 22                 // levels 0..21
+#define OTOO_POOL_SLOTS 16384         // task slots of the walk's pool (walk.cuh)
 #define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
 #define OTOO_LIST_CAP 256            // smem interaction-list float4 per warp (small: leaves the SM's L1 for the tree)
@@ -95,6 +96,12 @@ struct otoo_ctx {
   bool walked;
   bool sph_radii_valid;
   bool b2_valid;         // c_B2 computed for the current tree (on demand, by otoo_gravity_delta)
+  // theta of the last otoo_gravity call: the next build leaves rb^2 (R7) of it in cell_b.x from inside its bottom-up
+  // pass (l, s are in registers there), and resets the walk's control block and pool; a gravity call with the same
+  // theta then launches the walk kernel alone.  Another theta, the Delta-MAC or a second walk on the same tree run the
+  // r_b / reset kernels as before.
+  bool spec_theta_set, rb2_valid, walk_reset_valid;
+  float spec_theta, rb2_theta;
   int key_order_built;   // key order of the current tree
   int64_t N, N_cell, N_leaf;
   int n_crit, depth;

@@ -16,10 +16,10 @@ namespace {
 // R7: r_b = l/theta + s in fp64, rb^2 rounded once to fp32.  theta = 0 -> +inf (open everything).
 // the first OTOO_POOL_SLOTS threads of the r_b kernels also reset the walk's control block and the pool's sequence
 // numbers (tickets restart from 0 every launch): was a kernel of its own
-struct WalkReset { WalkShared* ws; uint32_t* seq; int ngroups; };
+struct WalkReset { WalkShared* ws; uint32_t* seq; };
 __device__ __forceinline__ void walk_reset(const WalkReset& r, int64_t i) {
   if (i < OTOO_POOL_SLOTS) r.seq[i] = (uint32_t)i;
-  if (i == 0) { r.ws->queue = 0; r.ws->head = 0; r.ws->tail = 0; r.ws->outstanding = r.ngroups; }
+  if (i == 0) { r.ws->queue = 0; r.ws->head = 0; r.ws->tail = 0; r.ws->outstanding = 0; }
 }
 __global__ void __launch_bounds__(256) rb2_kernel(const uint8_t* __restrict__ c_level, const double* __restrict__ c_s,
                                                   int64_t ncell, float S, float theta, cellb_t* __restrict__ cell_b, const WalkReset wr) {
@@ -282,10 +282,10 @@ otoo_status launch_walk_ws(otoo_ctx* ctx, const GravParams& p, bool eps0, cudaSt
 }
 
 // reset the control block and the pool's sequence numbers (tickets restart from 0 every launch)
-__global__ void __launch_bounds__(256) walk_init_kernel(WalkShared* ws, uint32_t* seq, int ngroups) {
+__global__ void __launch_bounds__(256) walk_init_kernel(WalkShared* ws, uint32_t* seq) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < OTOO_POOL_SLOTS) seq[i] = (uint32_t)i;
-  if (i == 0) { ws->queue = 0; ws->head = 0; ws->tail = 0; ws->outstanding = ngroups; }
+  if (i == 0) { ws->queue = 0; ws->head = 0; ws->tail = 0; ws->outstanding = 0; }
 }
 
 template <int T, bool EPS0>
@@ -335,9 +335,12 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->pool_seq, sizeof(uint32_t) * (size_t)OTOO_POOL_SLOTS));
     OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->walk_shared, sizeof(WalkShared)));
   }
-  if (reset) {   // (the gravity calls do this inside their r_b kernel)
-    walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq, (int)ngroups);
-    ctx->launches += 1;
+  if (reset) {   // (the gravity calls do this inside their r_b kernel, or find it done by the build)
+    if (!ctx->walk_reset_valid) {
+      walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>((WalkShared*)ctx->walk_shared, (uint32_t*)ctx->pool_seq);
+      ctx->launches += 1;
+    }
+    ctx->walk_reset_valid = false;                 // the walk that follows uses it up
   }
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ntests, 0, 4 * (size_t)total_groups, st));
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->g_ncells, 0, 4 * (size_t)total_groups, st));
@@ -360,15 +363,23 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   int grid; size_t smem;
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p.c, &grid, &smem, st, false));
   smem = grav_fused_smem_bytes();                 // (the one-warp-does-both kernel: + the pieces' boxes)
-  const WalkReset wr{p.c.ws, p.c.seq, (int)p.c.ngroups};
+  const WalkReset wr{p.c.ws, p.c.seq};
   const unsigned nbR = (unsigned)(cdiv(ctx->N_cell, 256) > OTOO_POOL_SLOTS / 256 ? cdiv(ctx->N_cell, 256) : OTOO_POOL_SLOTS / 256);
+  int prep_launches = 1;
   if (mac == 0) {
-    rb2_kernel<<<nbR, 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b, wr);
+    // the build has left rb^2 of the previous call's theta and a reset pool (build.cu): nothing to launch then
+    const bool have_rb2 = ctx->rb2_valid && memcmp(&ctx->rb2_theta, &p0, sizeof(float)) == 0;
+    if (!have_rb2) rb2_kernel<<<nbR, 256, 0, st>>>(ctx->c_level, ctx->c_s, ctx->N_cell, ctx->S, p0, ctx->cell_b, wr);
+    else if (!ctx->walk_reset_valid) walk_init_kernel<<<OTOO_POOL_SLOTS / 256, 256, 0, st>>>(p.c.ws, p.c.seq);
+    else prep_launches = 0;
+    ctx->rb2_valid = true; ctx->rb2_theta = p0; ctx->spec_theta = p0; ctx->spec_theta_set = true;
   } else {
     OTOO_TRY(otoo_b2_impl(ctx, st));
     OTOO_TRY(otoo_bmax_impl(ctx, st));
     rb2_delta_kernel<<<nbR, 256, 0, st>>>(ctx->c_B2, ctx->c_MP, ctx->sph_acc, ctx->N_cell, ctx->S, p0, p1, ctx->cell_b, wr);
+    ctx->rb2_valid = false;
   }
+  ctx->walk_reset_valid = false;                   // the walk below uses the reset up
   OTOO_CUDA(ctx, cudaMemsetAsync(d_acc_pot, 0, 16 * (size_t)ctx->N, st));
   p.eps2 = eps * eps;
   p.acc_pot = reinterpret_cast<float4*>(d_acc_pot);
@@ -396,7 +407,7 @@ otoo_status otoo_gravity_impl(otoo_ctx* ctx, float eps, int mac, float p0, float
   }
   OTOO_EV(ctx, ctx->ev_walk[2], st);
   ctx->ev_walk_valid = true;
-  ctx->launches += 2;
+  ctx->launches += prep_launches + 1;
   OTOO_CUDA(ctx, cudaGetLastError());
   ctx->walked = true;
   return OTOO_OK;

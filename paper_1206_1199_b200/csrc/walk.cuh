@@ -136,7 +136,6 @@ __device__ __forceinline__ int warp_inclusive_scan(int x, int lane) {
 
 // ---- global task pool (multi-producer multi-consumer ring of fixed-size tasks)
 #define OTOO_TASK_CELLS 256
-#define OTOO_POOL_SLOTS 16384
 #ifndef OTOO_MULTI_DONATE
 #define OTOO_MULTI_DONATE 4
 #endif
@@ -146,7 +145,7 @@ struct WalkShared {                   // device-global control block, reset befo
   uint32_t queue;  uint32_t pad0[31]; // next group of the main queue
   uint32_t head;   uint32_t pad1[31]; // consumer tickets: idle warps take one and wait on their slot
   uint32_t tail;   uint32_t pad2[31]; // producer tickets
-  int outstanding; uint32_t pad3[31]; // groups + tasks not yet finished
+  int outstanding; uint32_t pad3[31]; // tasks created - (groups + tasks finished): starts at 0, all done at -ngroups
 };
 struct WalkCommon {
   const float4* spos; const float4* cell_cm; const cellb_t* cell_b; const uint32_t* perm;
@@ -235,7 +234,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       int ok = 0;
       if (lane == 0) {
         if (ld_volatile(&c.seq[my_ticket % OTOO_POOL_SLOTS]) == my_ticket + 1u) ok = 1;
-        else if (*reinterpret_cast<volatile int*>(&c.ws->outstanding) <= 0) ok = -1;
+        else if (*reinterpret_cast<volatile int*>(&c.ws->outstanding) + (int)c.ngroups <= 0) ok = -1;
       }
       ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
       if (ok < 0) break;

@@ -507,6 +507,39 @@ def test_stats_phase_times_and_walk_only_flag(otoo, orc):
     assert otoo.otoo_last_stats()["walk_only"] == 0
 
 
+def test_build_leaves_rb2_and_reset_for_the_next_gravity_call(otoo, orc):
+    """A build after a gravity call leaves rb^2 of that call's theta (R7) and a reset walk pool from inside its bottom-up
+    pass: the next otoo_gravity with the same theta launches the walk kernel alone; another theta, or a second walk on
+    the same tree, runs the r_b / reset kernel as before.  All three paths against the oracle, bit for bit on rb^2 and
+    the counters."""
+    pm = gen.plummer(30000 + 11, 21)
+    t = orc.Tree(pm, 16)
+    th1, th2, eps = float(np.float32(0.55)), float(np.float32(0.75)), float(np.float32(0.01))
+
+    def check(theta, launches):
+        out = otoo.otoo_gravity(eps, theta, 128).cpu().numpy()
+        st = otoo.otoo_last_stats()
+        assert st["launches"] == launches, (st["launches"], launches)
+        ref = t.gravity(eps, theta, 128)
+        assert np.array_equal(otoo.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta).view(np.uint32))
+        nt, nc, npart = otoo.otoo_export_group_stats()
+        assert np.array_equal(nt, ref["n_tests"]) and np.array_equal(nc, ref["n_cells"]) and np.array_equal(npart, ref["n_parts"])
+        assert st["sum_interactions"] == ref["interactions"]
+        e, _ = acc_err(out, ref["acc_pot"], ref["abs_sum"])
+        assert e.max() <= TOL
+
+    otoo.otoo_build_tree(dev(pm), 16)
+    check(th2, 2)                       # (whatever the fixture's last theta was: not th2 on this tree yet)
+    otoo.otoo_build_tree(dev(pm), 16)
+    check(th2, 1)                       # rb^2 of th2 and the reset came with the build
+    check(th2, 2)                       # same tree, same theta: rb^2 stands, the pool needs its reset kernel
+    check(th1, 2)                       # another theta: the r_b kernel (with the reset inside)
+    otoo.otoo_build_tree(dev(pm), 16)
+    check(th1, 1)
+    otoo.otoo_build_tree(dev(pm), 16)
+    check(th2, 2)                       # the build guessed th1
+
+
 def test_spill_overflow_is_reported(otoo, orc):
     """Without the task pool and with a private spill area too small for theta = 0 on a deep tree the walk drops
     cells: the launch is flagged and the introspection calls return OTOO_ERR_CAPACITY instead of wrong numbers."""
