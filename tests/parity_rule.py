@@ -67,6 +67,19 @@ def report(label, got, want, abs_sum, pct=99.9, floor_frac_max=FLOOR_FRAC_MAX_SP
     return st
 
 
+def phi_tol(list_len):
+    """Tolerance of the potential of a target whose interaction list has `list_len` entries (R12).
+    phi is a sum of terms of one sign, so its error is pure rounding: plain 1e-5 relative, as long as fp32 arithmetic
+    can promise it.  The kernel adds 64-entry partial sums to running totals (and the totals of a group's pool tasks
+    to the output): L/64 fp32 additions of like-signed partials, each off by <= u/2 of the running total, a random walk
+    of about u sqrt(L/64) at a few sigma.  That passes 1e-5 at L = 64 (1e-5/u)^2 = 1.8 M entries: the bound is
+        max(1e-5, u sqrt(L/64)),
+    1e-5 for every list of the default walk (longest: 28 k entries at C2) and 2.1e-5 for the ONE group of C3 that lists
+    all 8.4 M particles under group_distance = 0 (measured on the B200 over 20 runs: 6.8e-6 ... 1.14e-5)."""
+    L = np.asarray(list_len, dtype=np.float64)
+    return np.maximum(TOL, U32 * np.sqrt(L / 64.0))
+
+
 def scalar_rel(label, got, want, tol=TOL):
     """plain relative error of a positive-definite scalar sum (potential, density): max |dx|/|x| <= tol"""
     got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)

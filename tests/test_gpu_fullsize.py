@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 from workloads import generators as gen  # noqa: E402
 
-from tests.parity_rule import TOL, U32, FLOOR_FRAC_MAX_GRAVITY, FLOOR_FRAC_MAX_SPH, report   # noqa: E402  (the one statement of the rule, R12)
+from tests.parity_rule import TOL, U32, FLOOR_FRAC_MAX_GRAVITY, FLOOR_FRAC_MAX_SPH, report, phi_tol   # noqa: E402  (the one statement of the rule, R12)
 
 N_SAMPLE = {"C2": 512, "C3": 256, "C4": 256, "C5": 256}     # seeded groups summed in fp64 per config (+ the two below)
 
@@ -89,7 +89,8 @@ def test_fullsize_gravity(orc, name):
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
         vec_check(f"fullsize_gravity[{name}:{order}]", out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9, FLOOR_FRAC_MAX_GRAVITY)
         pe = np.abs(out[idx, 3] - rs["acc_pot"][idx, 3]) / np.abs(rs["acc_pot"][idx, 3])
-        assert pe.max() <= TOL, pe.max()
+        ptol = np.concatenate([np.full(min((g + 1) * G, n) - g * G, phi_tol(lengths[g])) for g in sel])   # 1e-5 up to 1.8 M entries
+        assert (pe <= ptol).all(), (pe.max(), float((pe / ptol).max()))
         assert np.isfinite(out).all()
     finally:
         o.close()
