@@ -101,14 +101,15 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     ctx->hist_cap = OTOO_SORT_SCRATCH(max_particles);   // look-back status (u64 per tile and digit) + histograms
     OTOO_TRY(dalloc(ctx, &ctx->hist, ctx->hist_cap));
     OTOO_CUDA(ctx, cudaMemset(ctx->hist, 0, ctx->hist_cap * sizeof(uint32_t)));
-    OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, (size_t)cdiv(max_particles, 4096) + 1024));
+    ctx->scan_cap = (size_t)cdiv(max_particles, 4096) + 1024;
+    OTOO_TRY(dalloc(ctx, &ctx->scan_tmp, ctx->scan_cap));
     OTOO_TRY(dalloc(ctx, &ctx->d_bbox, 16));
     OTOO_TRY(dalloc(ctx, &ctx->d_counters, 64));
     OTOO_TRY(dalloc(ctx, &ctx->d_sums, OTOO_NSUMS));
     OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
-    OTOO_CUDA(ctx, cudaMemset(ctx->scan_tmp, 0, sizeof(uint32_t)));       // arrival counter of the scan
+    OTOO_CUDA(ctx, cudaMemset(ctx->scan_tmp, 0, ctx->scan_cap * sizeof(uint32_t)));   // tile ticket and status words of the scan
     for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
     for (auto& e : ctx->ev_walk) OTOO_CUDA(ctx, cudaEventCreate(&e));
     return OTOO_OK;

@@ -39,7 +39,9 @@ struct otoo_ctx {
   uint32_t* val[2];      // id double buffer; val[0] = perm after build
   float4* spos;          // positions+mass in sorted order
   uint32_t* slot_nc;     // cells per level starting in each block of 256 slots (level-major), then its exclusive scan
-  uint32_t* scan_tmp;    // block sums for the scan
+  uint32_t* scan_tmp;    // scan scratch: tile ticket, then one 64-bit look-back status word per tile of 4096 elements
+  size_t scan_cap;       // its size in words
+  uint32_t scan_epoch;   // one epoch per scan tags the status words: stale ones never match
   uint32_t* hist;        // sort scratch: digit histograms, tile tickets, look-back status words
   uint32_t sort_epoch;   // one epoch per radix pass: stale status words never match
   bool sort_attr_set;

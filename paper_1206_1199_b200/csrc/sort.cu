@@ -271,43 +271,53 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* t
   return r;
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) scan_reduce_kernel(const uint32_t* __restrict__ data, int64_t n,
-                                                                   uint32_t* sums, uint32_t* done, uint32_t* total_out) {
-  int64_t base = (int64_t)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
-  uint32_t s = 0;
-#pragma unroll
-  for (int i = 0; i < SCAN_ITEMS; i++) if (base + i < n) s += data[base + i];
-  uint32_t tot;
-  block_exclusive_scan(s, &tot);
-  if (threadIdx.x == 0) sums[blockIdx.x] = tot;
-  // the last block to arrive scans the block sums (was a kernel of its own)
-  __shared__ bool last;
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) last = atomicAdd(done, 1u) == gridDim.x - 1;
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  if (threadIdx.x == 0) *done = 0u;                  // ready for the next scan
-  const int64_t nb = gridDim.x;
-  uint32_t carry = 0;
-  for (int64_t c = 0; c < nb; c += SCAN_THREADS) {
-    int64_t i = c + threadIdx.x;
-    uint32_t x = i < nb ? __ldcg(&sums[i]) : 0, t2;
-    uint32_t e = block_exclusive_scan(x, &t2);
-    if (i < nb) sums[i] = e + carry;
-    carry += t2;
+// One kernel, one pass over the data: a tile of SCAN_TILE elements per block, the tile's exclusive offset by decoupled
+// look-back over the preceding tiles' status words (the sort's format: epoch | state | value; tiles numbered by a ticket
+// so that the wait cannot hang; nothing is cleared between scans).  Was a reduce kernel + an apply kernel.
+__global__ void __launch_bounds__(SCAN_THREADS) scan_onepass_kernel(uint32_t* __restrict__ data, int64_t n, unsigned long long* status,
+                                                                    uint32_t* ticket, uint32_t epoch, uint32_t* total_out) {
+  __shared__ uint32_t s_tile, s_excl;
+  if (threadIdx.x == 0) {
+    s_tile = atomicAdd(ticket, 1u);
+    if (s_tile == gridDim.x - 1) *ticket = 0u;            // the last ticket: ready for the next scan
   }
-  if (threadIdx.x == 0 && total_out) *total_out = carry;
-}
-__global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t* __restrict__ data, int64_t n,
-                                                                  const uint32_t* __restrict__ sums) {
-  int64_t base = (int64_t)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const int64_t base = (int64_t)tile * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   uint32_t x[SCAN_ITEMS], s = 0;
 #pragma unroll
   for (int i = 0; i < SCAN_ITEMS; i++) { x[i] = base + i < n ? data[base + i] : 0; s += x[i]; }
   uint32_t tot;
-  uint32_t run = block_exclusive_scan(s, &tot) + sums[blockIdx.x];
+  uint32_t run = block_exclusive_scan(s, &tot);
+  volatile unsigned long long* st = status;
+  if (threadIdx.x == 0) st[tile] = os_pack(epoch, tile == 0 ? 2u : 1u, tot);
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x;
+    uint32_t excl = 0;
+    int64_t t = (int64_t)tile - 1;
+    while (t >= 0) {                                      // 32 preceding tiles per round
+      const int64_t idx = t - lane;
+      const unsigned long long w = idx >= 0 ? st[idx] : os_pack(epoch, 2u, 0u);
+      const uint32_t state = (uint32_t)(w >> 32) & 3u;
+      const bool valid = (uint32_t)(w >> 34) == epoch && state != 0u;
+      const unsigned incl = __ballot_sync(0xFFFFFFFFu, valid && state == 2u), bad = __ballot_sync(0xFFFFFFFFu, !valid);
+      const int first_incl = incl ? __ffs(incl) - 1 : 32, first_bad = bad ? __ffs(bad) - 1 : 32;
+      if (first_bad < (first_incl < 32 ? first_incl + 1 : 32)) continue;          // a word of this range is not there yet
+      uint32_t c = lane <= first_incl ? (uint32_t)w : 0u;
+#pragma unroll
+      for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+      excl += c;
+      if (first_incl < 32) break;
+      t -= 32;
+    }
+    if (lane == 0) {
+      s_excl = excl;
+      if (tile > 0) st[tile] = os_pack(epoch, 2u, excl + tot);
+      if (tile == gridDim.x - 1 && total_out) *total_out = excl + tot;
+    }
+  }
+  __syncthreads();
+  run += s_excl;
 #pragma unroll
   for (int i = 0; i < SCAN_ITEMS; i++) { if (base + i < n) data[base + i] = run; run += x[i]; }
 }
@@ -320,10 +330,16 @@ otoo_status otoo_exclusive_scan_u32(otoo_ctx* ctx, uint32_t* data, int64_t n, ui
     if (total_out_dev) OTOO_CUDA(ctx, cudaMemsetAsync(total_out_dev, 0, 4, st));
     return OTOO_OK;
   }
-  int64_t nb = cdiv(n, SCAN_TILE);
-  scan_reduce_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp + 1, ctx->scan_tmp, total_out_dev);   // scan_tmp[0]: arrival counter
-  scan_apply_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, ctx->scan_tmp + 1);
-  ctx->launches += 2;
+  const int64_t nb = cdiv(n, SCAN_TILE);
+  if (2 + 2 * nb > ctx->scan_cap) return otoo_fail(ctx, OTOO_ERR_CAPACITY, "scan scratch too small");
+  if (ctx->scan_epoch + 1u >= (1u << 30)) {          // the epochs ran out: clear the status words and restart
+    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->scan_tmp, 0, ctx->scan_cap * sizeof(uint32_t), st));
+    ctx->scan_epoch = 0;
+  }
+  // scan_tmp: [0] tile ticket (left at 0 by every scan), [2..] one 64-bit status word per tile
+  scan_onepass_kernel<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, reinterpret_cast<unsigned long long*>(ctx->scan_tmp + 2), ctx->scan_tmp,
+                                                            ++ctx->scan_epoch, total_out_dev);
+  ctx->launches += 1;
   OTOO_CUDA(ctx, cudaGetLastError());
   return OTOO_OK;
 }
