@@ -109,6 +109,9 @@ otoo_status otoo_create(otoo_ctx** out, int device, int64_t max_particles) {
     OTOO_CUDA(ctx, cudaMemset(ctx->d_sums, 0, OTOO_NSUMS * sizeof(unsigned long long)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_counters, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMallocHost((void**)&ctx->h_root, 8 * sizeof(float)));
+    OTOO_CUDA(ctx, cudaMemset(ctx->d_bbox, 0xFF, 12));                      // bbox_kernel: minima as ordered uints ...
+    OTOO_CUDA(ctx, cudaMemset(reinterpret_cast<unsigned*>(ctx->d_bbox) + 3, 0, 16));   // ... maxima, arrival counter (kept so by the kernel)
+    OTOO_CUDA(ctx, cudaMemset(ctx->d_counters, 0, 64 * sizeof(uint32_t)));
     OTOO_CUDA(ctx, cudaMemset(ctx->scan_tmp, 0, ctx->scan_cap * sizeof(uint32_t)));   // tile ticket and status words of the scan
     for (auto& e : ctx->ev_build) OTOO_CUDA(ctx, cudaEventCreate(&e));
     for (auto& e : ctx->ev_walk) OTOO_CUDA(ctx, cudaEventCreate(&e));

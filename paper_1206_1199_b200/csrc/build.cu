@@ -64,6 +64,9 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float4* __restrict__ po
   if (!(S > 0.0f)) S = 1.0f;
   out[3] = S;
   out[4] = __fdiv_rn(2097152.0f, S);  // R2: IEEE division
+  // ready for the next build (was three memsets per build): min = 0xFFFFFFFF, max = 0, arrival counter = 0
+  for (int k = 0; k < 3; k++) { bbox[k] = 0xFFFFFFFFu; bbox[3 + k] = 0u; }
+  bbox[6] = 0u;
 }
 
 // H4: positions into sorted order
@@ -460,9 +463,8 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
   ctx->ev_build_valid = false;
   OTOO_EV(ctx, ctx->ev_build[0], st);
   // H1
-  OTOO_CUDA(ctx, cudaMemsetAsync(bbox, 0xFF, 12, st));      // min = 0xFFFFFFFF
-  OTOO_CUDA(ctx, cudaMemsetAsync(bbox + 3, 0x00, 16, st));  // max = 0, arrival counter = 0
-  OTOO_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 64 * sizeof(uint32_t), st));
+  // (the extrema and the arrival counter in d_bbox start from their initial values: set at otoo_create and put back by
+  // the last block of every bbox_kernel)
   int gb = ctx->sm_count * 4; if ((int64_t)gb > (int64_t)nbN) gb = (int)nbN;
   bbox_kernel<<<gb, 256, 0, st>>>(pos, N, bbox);
   ctx->launches += 1;

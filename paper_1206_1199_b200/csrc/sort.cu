@@ -81,10 +81,19 @@ __global__ void __launch_bounds__(SORT_THREADS) key_hist_kernel(const float4* __
   for (int p = 0; p < OS_MAXPASS; p++) sh[p][tid] = 0;
   __syncthreads();
   const float* root = reinterpret_cast<const float*>(bbox) + 8;
-  for (int64_t i = (int64_t)blockIdx.x * SORT_THREADS + tid; i < n; i += (int64_t)gridDim.x * SORT_THREADS) {
-    const uint64_t k = particle_key(pos[i], root, hilbert);
-    key[i] = k;                                        // (the ids 0, 1, 2, ... are not written: the first sort pass makes them up)
-    for (int p = 0; p < OS_MAXPASS; p++) atomicAdd(&sh[p][(unsigned)(k >> (8 * p)) & 0xFF], 1u);
+  constexpr int KH = 4;                                // positions in flight per thread (one: 0.26 ms at 32 M particles, latency-bound)
+  const int64_t stride = (int64_t)gridDim.x * SORT_THREADS;
+  for (int64_t i0 = (int64_t)blockIdx.x * SORT_THREADS + tid; i0 < n; i0 += KH * stride) {
+    float4 pv[KH];
+#pragma unroll
+    for (int j = 0; j < KH; j++) if (i0 + j * stride < n) pv[j] = pos[i0 + j * stride];
+#pragma unroll
+    for (int j = 0; j < KH; j++) if (i0 + j * stride < n) {
+      const uint64_t k = particle_key(pv[j], root, hilbert);
+      key[i0 + j * stride] = k;                        // (the ids 0, 1, 2, ... are not written: the first sort pass makes them up)
+#pragma unroll
+      for (int p = 0; p < OS_MAXPASS; p++) atomicAdd(&sh[p][(unsigned)(k >> (8 * p)) & 0xFF], 1u);
+    }
   }
   __syncthreads();
   for (int p = 0; p < OS_MAXPASS; p++) if (sh[p][tid]) atomicAdd(&ghist[p * 256 + tid], sh[p][tid]);
