@@ -65,8 +65,10 @@ typedef struct {
                               * for the SPH walks the candidates left after the walk-time cull, times the group size */
   /* Per-phase DEVICE times in ms (CUDA events on the call's stream; PAPER.md L195, L212 splits a step into TREE
    * and KERNEL the same way).  ms_build[] of the last otoo_build_tree: [0] root cube (H1), [1] keys (H2),
-   * [2] key sort (H3), [3] gather (H4), [4] cells from the sorted keys (H5, includes the one host
-   * synchronisation), [5] bottom-up moments (H6), [6..7] unused (0); ms_build_total = their sum.
+   * [2] key sort (H3), [3] gather fused with the levels of the cells that start at each slot (H4 + first part of
+   * H5), [4] cells from those levels (rest of H5: scan, placement; includes the one host synchronisation),
+   * [5] bottom-up pass (H6; also the internal cells' children and rb^2 of the last gravity call's theta),
+   * [6..7] unused (0); ms_build_total = their sum.
    * Of the last walk call (gravity or SPH): ms_walk_prep = cell radii (r_b or Eq. 5), gathers and clears before
    * the walk kernel; ms_walk_force = the fused walk + sum kernel alone (H7-H10 / H11 / H13); ms_total = the
    * whole call.  0 where nothing has run. */
