@@ -262,6 +262,9 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
 }
 
 struct LevelOff { uint32_t v[OTOO_NLEV + 1]; };
+#ifndef OTOO_MOMENTS_WIDE
+#define OTOO_MOMENTS_WIDE (4u << 20)      // cells in the widest level from which the bottom-up pass runs 4 CTAs per SM
+#endif
 
 // H6 (L155; R6, R7): one level of the bottom-up pass; fp64, fixed summation order.
 struct MomentArgs {
@@ -356,10 +359,11 @@ __device__ __forceinline__ void moments_cell(uint32_t c, int level, uint32_t lev
 // between levels (per-level launches of the sparse top and bottom levels were pure launch latency)
 // Levels 0 .. top are narrow (the top of the tree: 1, 8, 64, ... cells): one CTA finishes them with block barriers
 // instead of grid barriers.
-#ifndef OTOO_MOMENTS_MINB
-#define OTOO_MOMENTS_MINB 2
-#endif
-__global__ void __launch_bounds__(256, OTOO_MOMENTS_MINB) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
+// MINB = CTAs per SM the register count must allow: 2 (128 registers) up to a few million cells per level, 4 (64 registers)
+// beyond -- twice the loads in flight for the wide leaf levels (0.75 -> 0.69 ms at 32 M particles), but twice the blocks in
+// every grid barrier (10-30 % slower at 1-8 M particles)
+template <int MINB>
+__global__ void __launch_bounds__(256, MINB) moments_all_kernel(const LevelOff off, const int depth, const int top, const MomentArgs a) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
   if (a.walk_seq) {                                  // the next walk finds its control block and pool reset (was part of the r_b kernel)
@@ -517,17 +521,18 @@ otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, i
                       bbox, ctx->c_MP, ctx->c_cm64, ctx->cell_cm, ctx->c_s, ctx->c_B2, ctx->key_order, ctx->c_level, ctx->cell_b,
                       ctx->spec_theta_set ? 1 : 0, ctx->spec_theta, (uint32_t*)ctx->walk_shared, (uint32_t*)ctx->pool_seq};
   {
-    int occ = 1;
-    OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_all_kernel, 256, 0));
-    if (occ > 4) occ = 4;
-    int64_t grid = (int64_t)ctx->sm_count * (occ < 1 ? 1 : occ);
     uint32_t widest = 1;
     for (int l = 0; l <= depth; l++) if (off.v[l + 1] - off.v[l] > widest) widest = off.v[l + 1] - off.v[l];
+    const void* kern = widest >= OTOO_MOMENTS_WIDE ? (const void*)moments_all_kernel<4> : (const void*)moments_all_kernel<2>;
+    int occ = 1;
+    OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, 0));
+    if (occ > 4) occ = 4;
+    int64_t grid = (int64_t)ctx->sm_count * (occ < 1 ? 1 : occ);
     if (grid > cdiv(widest, 256)) grid = cdiv(widest, 256);
     int depth_arg = depth, top = -1;
     while (top + 1 <= depth && off.v[top + 2] - off.v[top + 1] <= 256u) top++;       // levels 0 .. top hold <= 256 cells each (one per thread)
     void* args[] = {(void*)&off, (void*)&depth_arg, (void*)&top, (void*)&ma};
-    OTOO_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)moments_all_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
+    OTOO_CUDA(ctx, cudaLaunchCooperativeKernel(kern, dim3((unsigned)grid), dim3(256), args, 0, st));
     ctx->launches += 1;
   }
   OTOO_EV(ctx, ctx->ev_build[6], st);

@@ -202,7 +202,11 @@ __global__ void __launch_bounds__(OS_THREADS, MINB) onesweep_pass_kernel(const u
     uint32_t run = my_start;                          // whist[w][d] := position in the sorted tile of warp w's first key with digit d
 #pragma unroll
     for (int w = 0; w < OS_WARPS; w++) { const uint32_t c = whist[w][tid]; whist[w][tid] = run; run += c; }
+#ifdef OTOO_OS_NOLOOKBACK          /* timing experiment only: wrong offsets, no chain over the tiles */
+    if (false) {
+#else
     if (tile > 0) {
+#endif
       // look back over the preceding tiles, 8 status words in flight at a time (when all tiles of a small
       // sort run in one wave the walk is long, and one L2 round trip per tile would dominate the pass)
       int64_t t = (int64_t)tile - 1;
