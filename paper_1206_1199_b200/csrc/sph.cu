@@ -439,7 +439,7 @@ struct SphVisitor {
 };
 
 template <int T, int MODE>
-__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) {
+__device__ __forceinline__ void walk_sph_body(const SphParams& p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_STRIDE;
@@ -451,6 +451,17 @@ __global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const Sp
            warp * (2 * OTOO_PIECES);
   v.lane_ = lane;
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
+}
+template <int T, int MODE>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) { walk_sph_body<T, MODE>(p); }
+// The density walk of groups up to 64 with 5 CTAs per SM (96 registers instead of 122-126): A/B at C4, G = 64: 2.13 -> 2.03 ms
+// (6 CTAs: 2.02).  The force kernels lose with 5 or 6 (force + du/dt 2.98 -> 3.22 / 3.32 ms) and keep ptxas' own choice.
+template <int T, int MODE>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32, 5) walk_sph_kernel_occ5(const SphParams p) { walk_sph_body<T, MODE>(p); }
+template <int T, int MODE>
+void (*sph_kernel_ptr())(const SphParams) {
+  if constexpr (MODE == 0 && T <= 2) return walk_sph_kernel_occ5<T, MODE>;
+  else return walk_sph_kernel<T, MODE>;
 }
 
 
@@ -656,14 +667,16 @@ template <int MODE>
 otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_t smem, cudaStream_t st) {
   int occ = 1;
   const size_t smem0 = smem;
+  void (*kern)(const SphParams) = nullptr;
 #define OTOO_SPH_CASE(TT)                                                                                              \
   smem = smem0 + (size_t)OTOO_WALK_WARPS * (SphVisitor<TT, MODE>::W * TT * 32 * sizeof(uint32_t) + 2 * OTOO_PIECES * sizeof(float4));   /* + the mask words + the pieces' boxes */   \
-  OTOO_CUDA(ctx, cudaFuncSetAttribute(walk_sph_kernel<TT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, walk_sph_kernel<TT, MODE>, OTOO_WALK_WARPS * 32, smem));  \
+  kern = sph_kernel_ptr<TT, MODE>();                                                                                  \
+  OTOO_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                   \
+  OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, OTOO_WALK_WARPS * 32, smem));                \
   if (occ < 1) occ = 1;                                                                                                 \
   if (grid > ctx->sm_count * occ) grid = ctx->sm_count * occ;                                                          \
   OTOO_EV(ctx, ctx->ev_walk[1], st);                                                                                    \
-  walk_sph_kernel<TT, MODE><<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);                                               \
+  kern<<<grid, OTOO_WALK_WARPS * 32, smem, st>>>(p);                                                                    \
   OTOO_EV(ctx, ctx->ev_walk[2], st);                                                                                    \
   ctx->ev_walk_valid = true;
   switch (G) {
