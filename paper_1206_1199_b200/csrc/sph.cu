@@ -44,51 +44,83 @@ __global__ void __launch_bounds__(256) divrot_finish_kernel(const float* __restr
   dr[i] = make_float4(__fdiv_rn(v.x, r), __fdiv_rn(v.y, r), __fdiv_rn(v.z, r), __fdiv_rn(v.w, r));
 }
 // ---- R14: b_max and r_SPH over ALL particles of every cell, from the fp64 centre of mass.
-// Each particle walks down its own root-to-leaf path; consecutive slots share cells, so a warp
-// first reduces runs of equal cell id with shuffles and only run heads touch memory.
+// A particle at sorted slot s lies in one cell of every level 0 .. LL(s) (LL of the build's per-slot record `info`: the
+// level of the slot's leaf), and that cell is the last level-l cell that starts at or before s.  Canonical cell indices
+// count exactly those starts (build.cu, place_cells_kernel), so the index comes from the build's scanned per-block level
+// counts (blk_off) plus a ballot -- no descent through the tree (the first form walked every particle from the root to its
+// leaf: five or more dependent loads per level, 0.30 ms for 2 M particles).  Consecutive slots share cells, so a warp first
+// reduces runs of equal cell id with shuffles and only run heads touch memory.
 __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict__ spos, const float* __restrict__ hs, int64_t n,
-                                                        const uint32_t* __restrict__ c_first, const uint32_t* __restrict__ c_count,
-                                                        const uint32_t* __restrict__ c_child_first,
-                                                        const uint8_t* __restrict__ c_child_count, const double* __restrict__ cm64,
-                                                        unsigned long long* __restrict__ acc /* 2 per cell */) {
-  const int lane = threadIdx.x & 31;
-  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+                                                        const uint32_t* __restrict__ info, const uint32_t* __restrict__ blk_off,
+                                                        const double* __restrict__ cm64,
+                                                        unsigned long long* acc /* 2 per cell */) {
+  __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = s < n;
-  float4 p = valid ? spos[s] : make_float4(0, 0, 0, 0);
-  double h = (valid && hs) ? (double)hs[s] : 0.0;     // hs == NULL: b_max only (the Delta-MAC of gravity)
-  uint32_t cell = valid ? 0u : 0xFFFFFFFFu;
-  while (__any_sync(0xFFFFFFFFu, cell != 0xFFFFFFFFu)) {
-    double b = 0.0, r = 0.0;
-    if (cell != 0xFFFFFFFFu) {
-      double dx = __dsub_rn((double)p.x, cm64[3 * (size_t)cell]), dy = __dsub_rn((double)p.y, cm64[3 * (size_t)cell + 1]),
-             dz = __dsub_rn((double)p.z, cm64[3 * (size_t)cell + 2]);
-      b = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
-      r = __dadd_rn(b, h);
-    }
-    // segmented max over runs of equal cell id (runs are contiguous in slot order)
+  int lo = OTOO_NLEV, LL = -1;
+  if (valid) { const uint32_t inf = info[s]; lo = (int)(inf & 0xFF); LL = (int)(inf >> 8); }
+  const float4 p = valid ? spos[s] : make_float4(0, 0, 0, 0);
+  const double h = (valid && hs) ? (double)hs[s] : 0.0;     // hs == NULL: b_max only (the Delta-MAC of gravity)
+  const bool has = lo <= LL;
+  const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
+  for (int l = wlo; l <= whi; l++) {
+    const unsigned st = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
+    if (lane == 0) wc[warp][l] = (uint32_t)__popc(st);
+  }
+  __syncthreads();
+  if (threadIdx.x < OTOO_NLEV) {
+    uint32_t run = blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
-      double ob = __shfl_down_sync(0xFFFFFFFFu, b, o), orr = __shfl_down_sync(0xFFFFFFFFu, r, o);
-      if (lane + o < 32 && oc == cell) { b = fmax(b, ob); r = fmax(r, orr); }
+    for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
+  }
+  __syncthreads();
+  unsigned le;
+  asm("mov.u32 %0, %%lanemask_le;" : "=r"(le));
+  const int amax = __reduce_max_sync(0xFFFFFFFFu, LL);        // deepest leaf among the warp's slots
+  constexpr int LB = 4;                                       // levels per batch: their centres of mass are fetched together
+  for (int l0 = 0; l0 <= amax; l0 += LB) {
+    uint32_t cells[LB];
+    double cx[LB], cy[LB], cz[LB];
+#pragma unroll
+    for (int j = 0; j < LB; j++) {
+      const int l = l0 + j;
+      const unsigned st = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
+      cells[j] = l <= LL ? wc[warp][l < OTOO_NLEV ? l : OTOO_NLEV - 1] + (uint32_t)__popc(st & le) - 1u : 0xFFFFFFFFu;
     }
-    uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
-    bool head = (lane == 0) || (pc != cell);
-    if (head && cell != 0xFFFFFFFFu) {
-      atomicMax(acc + 2 * (size_t)cell, (unsigned long long)__double_as_longlong(b));
-      atomicMax(acc + 2 * (size_t)cell + 1, (unsigned long long)__double_as_longlong(r));
+#pragma unroll
+    for (int j = 0; j < LB; j++) if (cells[j] != 0xFFFFFFFFu) {
+      cx[j] = cm64[3 * (size_t)cells[j]]; cy[j] = cm64[3 * (size_t)cells[j] + 1]; cz[j] = cm64[3 * (size_t)cells[j] + 2];
     }
-    // descend
-    if (cell != 0xFFFFFFFFu) {
-      int nch = c_child_count[cell];
-      if (nch == 0) cell = 0xFFFFFFFFu;
-      else {
-        uint32_t ch = c_child_first[cell], next = 0xFFFFFFFFu;
-        for (int k = 0; k < nch; k++) {
-          uint32_t f = c_first[ch + k];
-          if ((uint32_t)s - f < c_count[ch + k]) { next = ch + k; break; }
-        }
-        cell = next;
+#pragma unroll
+    for (int j = 0; j < LB; j++) {
+      if (l0 + j > amax) break;
+      const uint32_t cell = cells[j];
+      double b = 0.0, r = 0.0;
+      if (cell != 0xFFFFFFFFu) {
+        double dx = __dsub_rn((double)p.x, cx[j]), dy = __dsub_rn((double)p.y, cy[j]), dz = __dsub_rn((double)p.z, cz[j]);
+        b = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+        r = __dadd_rn(b, h);
+      }
+      // segmented max over runs of equal cell id (runs are contiguous in slot order)
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
+        double ob = __shfl_down_sync(0xFFFFFFFFu, b, o), orr = __shfl_down_sync(0xFFFFFFFFu, r, o);
+        if (lane + o < 32 && oc == cell) { b = fmax(b, ob); r = fmax(r, orr); }
+      }
+      uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
+      bool head = (lane == 0) || (pc != cell);
+      if (head && cell != 0xFFFFFFFFu) {
+        // a maximum only grows: a value not above what the cell already holds needs no atomic (the cells of the top
+        // levels take one atomic per warp otherwise: 65 000 on the root's two words for 2 M particles, and atomics on
+        // one address run one after the other -- the kernel took 0.30 ms whatever else it did)
+        const unsigned long long bb = (unsigned long long)__double_as_longlong(b), rr = (unsigned long long)__double_as_longlong(r);
+        const ulonglong2 cur = __ldcg(reinterpret_cast<const ulonglong2*>(acc + 2 * (size_t)cell));
+        if (bb > cur.x) atomicMax(acc + 2 * (size_t)cell, bb);
+        if (rr > cur.y) atomicMax(acc + 2 * (size_t)cell + 1, rr);
       }
     }
   }
@@ -701,8 +733,8 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   if (!(ctx->sph_reuse && ctx->sph_radii_valid)) {
     gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
     OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
-    sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->c_first, ctx->c_count, ctx->c_child_first,
-                                          ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
+    sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc);   // (val[1], slot_nc: the build's
+                                                                                                                                 // per-slot levels and scanned level counts)
     sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
     ctx->launches += 3;
   }
@@ -719,8 +751,7 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
 // ordered bits in sph_acc[2c].  The fp32 SPH radii are recomputed by every SPH call anyway.
 otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st) {
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
-  sph_radii_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->c_first, ctx->c_count,
-                                                                ctx->c_child_first, ctx->c_child_count, ctx->c_cm64, ctx->sph_acc);
+  sph_radii_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc);
   ctx->launches += 1;
   ctx->sph_radii_valid = false;
   return OTOO_OK;
