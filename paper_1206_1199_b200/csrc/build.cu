@@ -195,6 +195,8 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
   __shared__ uint8_t slo[256 + OTOO_PLACE_WIN];  // lo of the block's slots and of the OTOO_PLACE_WIN slots after them (0 past the end)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  // (fetched now, used after two block barriers: the load's latency was a fifth of the kernel's stall samples)
+  const uint32_t my_off = threadIdx.x < OTOO_NLEV ? blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x] : 0u;
   const int64_t s0 = (int64_t)blockIdx.x * 256, s = s0 + threadIdx.x;
   int lo = OTOO_NLEV, LL = -1;
   if (s < n) { const uint32_t inf = info[s]; lo = (int)(inf & 0xFF); LL = (int)(inf >> 8); }
@@ -218,7 +220,7 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
   }
   __syncthreads();
   if (threadIdx.x < OTOO_NLEV) {
-    uint32_t run = blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
+    uint32_t run = my_off;
 #pragma unroll
     for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
   }

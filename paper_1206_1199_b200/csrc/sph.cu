@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
   __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  const uint32_t my_off = threadIdx.x < OTOO_NLEV ? blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x] : 0u;   // (used after the next barrier)
   __syncthreads();
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = s < n;
@@ -72,7 +73,7 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
   }
   __syncthreads();
   if (threadIdx.x < OTOO_NLEV) {
-    uint32_t run = blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
+    uint32_t run = my_off;
 #pragma unroll
     for (int w = 0; w < 8; w++) { const uint32_t c = wc[w][threadIdx.x]; wc[w][threadIdx.x] = run; run += c; }
   }
