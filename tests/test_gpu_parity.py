@@ -72,6 +72,20 @@ def test_tree_parity(otoo, orc, kind, n, n_crit, seed):
     check_tree(otoo, orc, gen.make(kind, n, seed), n_crit)
 
 
+def test_tree_small_and_block_edge_sizes(otoo, orc):
+    """N around 1, a warp, a block of 256 slots and the 64-slot look-ahead window of place_cells_kernel, with leaves of
+    1 ... 100 particles: every cell tuple, key and moment against the oracle (leaves that straddle blocks and windows,
+    blocks whose last warp is ragged, trees that are a single leaf)."""
+    for n in (1, 2, 3, 5, 17, 31, 32, 33, 63, 64, 65, 255, 256, 257, 319, 320, 321, 511, 512, 513, 1000):
+        for n_crit in (1, 3, 16, 100):
+            pm = gen.plummer(n, 100 + n)
+            check_tree(otoo, orc, pm, n_crit)
+    pm = gen.uniform_cube(700, 5)
+    pm[250:330] = pm[250]                 # 80 coincident points across the first block boundary and beyond its window
+    check_tree(otoo, orc, pm, 4)
+    check_tree(otoo, orc, pm, 4, key_order=1)
+
+
 def test_tree_degenerate_inputs(otoo, orc):
     pm = np.zeros((300, 4), np.float32)
     pm[:, :3] = 2.5
