@@ -408,7 +408,6 @@ otoo_status ensure_cells(otoo_ctx* ctx, int64_t ncell) {
   OTOO_TRY(grow(ctx, &ctx->c_B2, cap));
   OTOO_TRY(grow(ctx, &ctx->c_sph, cap));
   OTOO_TRY(grow(ctx, &ctx->sph_acc, 2 * cap));
-  OTOO_TRY(grow(ctx, &ctx->tmp_val[0], cap));        // first slot of every cell (H5b)
   ctx->cellCap = cap;
   return OTOO_OK;
 }

@@ -67,7 +67,7 @@ struct otoo_ctx {
   float2* c_sph;         // (b_max, r_SPH) (R14)
   unsigned long long* sph_acc;  // 2 per cell: fp64 maxima as ordered bits
   uint64_t* tmp_key[2];  // (unused since the cells are placed at their canonical index directly)
-  uint32_t* tmp_val[2];  // [0]: first slot of every cell in canonical order
+  uint32_t* tmp_val[2];  // (unused since place_cells_kernel writes c_first directly)
 
   // ---- small device scalars
   float* d_bbox;         // 6 floats lo/hi as ordered ints, then lo[3], S, scale

@@ -50,10 +50,14 @@ __global__ void __launch_bounds__(256) divrot_finish_kernel(const float* __restr
 // counts (blk_off) plus a ballot -- no descent through the tree (the first form walked every particle from the root to its
 // leaf: five or more dependent loads per level, 0.30 ms for 2 M particles).  Consecutive slots share cells, so a warp first
 // reduces runs of equal cell id with shuffles and only run heads touch memory.
+// F32: the maxima are kept as fp32 rounded up (what the SPH walks read: rounding up is monotone, so the maximum of the
+// rounded values is the rounded maximum) in out32, by 32-bit atomics; else as fp64 bit patterns in acc (the Delta-MAC
+// needs b_max in fp64).
+template <bool F32>
 __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict__ spos, const float* __restrict__ hs, int64_t n,
                                                         const uint32_t* __restrict__ info, const uint32_t* __restrict__ blk_off,
                                                         const double* __restrict__ cm64,
-                                                        unsigned long long* acc /* 2 per cell */) {
+                                                        unsigned long long* acc /* 2 per cell */, uint32_t* out32 /* 2 per cell */) {
   __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
@@ -105,35 +109,42 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
         b = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
         r = __dadd_rn(b, h);
       }
-      // segmented max over runs of equal cell id (runs are contiguous in slot order)
+      // segmented max over runs of equal cell id (runs are contiguous in slot order); head = first lane of a run
+      const uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
+      const bool head = (lane == 0) || (pc != cell);
+      if (F32) {
+        // in the rounded-up fp32 domain from here (non-negative floats order as their bit patterns): one shuffle and
+        // an integer max per value and step instead of two shuffles and an fp64 compare-select
+        uint32_t bb = __float_as_uint(__double2float_ru(b)), rr = __float_as_uint(__double2float_ru(r));
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
-        double ob = __shfl_down_sync(0xFFFFFFFFu, b, o), orr = __shfl_down_sync(0xFFFFFFFFu, r, o);
-        if (lane + o < 32 && oc == cell) { b = fmax(b, ob); r = fmax(r, orr); }
-      }
-      uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
-      bool head = (lane == 0) || (pc != cell);
-      if (head && cell != 0xFFFFFFFFu) {
-        // a maximum only grows: a value not above what the cell already holds needs no atomic (the cells of the top
-        // levels take one atomic per warp otherwise: 65 000 on the root's two words for 2 M particles, and atomics on
-        // one address run one after the other -- the kernel took 0.30 ms whatever else it did)
-        const unsigned long long bb = (unsigned long long)__double_as_longlong(b), rr = (unsigned long long)__double_as_longlong(r);
-        const ulonglong2 cur = __ldcg(reinterpret_cast<const ulonglong2*>(acc + 2 * (size_t)cell));
-        if (bb > cur.x) atomicMax(acc + 2 * (size_t)cell, bb);
-        if (rr > cur.y) atomicMax(acc + 2 * (size_t)cell + 1, rr);
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
+          const uint32_t ob = __shfl_down_sync(0xFFFFFFFFu, bb, o), orr = __shfl_down_sync(0xFFFFFFFFu, rr, o);
+          if (lane + o < 32 && oc == cell) { bb = bb > ob ? bb : ob; rr = rr > orr ? rr : orr; }
+        }
+        if (head && cell != 0xFFFFFFFFu) {
+          // a maximum only grows: a value not above what the cell already holds needs no atomic (the cells of the top
+          // levels take one atomic per warp otherwise: 65 000 on the root's two words for 2 M particles, and atomics on
+          // one address run one after the other -- the kernel took 0.30 ms whatever else it did)
+          const uint2 cur = __ldcg(reinterpret_cast<const uint2*>(out32 + 2 * (size_t)cell));
+          if (bb > cur.x) atomicMax(out32 + 2 * (size_t)cell, bb);
+          if (rr > cur.y) atomicMax(out32 + 2 * (size_t)cell + 1, rr);
+        }
+      } else {          // the Delta-MAC's b_max alone, in fp64 (acc[2c]; acc[2c + 1] is not written)
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
+          const double ob = __shfl_down_sync(0xFFFFFFFFu, b, o);
+          if (lane + o < 32 && oc == cell) b = fmax(b, ob);
+        }
+        if (head && cell != 0xFFFFFFFFu) {
+          const unsigned long long bb = (unsigned long long)__double_as_longlong(b);
+          if (bb > __ldcg(acc + 2 * (size_t)cell)) atomicMax(acc + 2 * (size_t)cell, bb);
+        }
       }
     }
   }
 }
-__global__ void __launch_bounds__(256) sph_radii_finish_kernel(const unsigned long long* __restrict__ acc, int64_t ncell,
-                                                               float2* __restrict__ out) {
-  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncell) return;
-  double b = __longlong_as_double((long long)acc[2 * c]), r = __longlong_as_double((long long)acc[2 * c + 1]);
-  out[c] = make_float2(__double2float_ru(b), __double2float_ru(r));  // rounded up: supersets survive rounding
-}
-
 struct SphParams {
   WalkCommon c;
   const float* hs;      // h, sorted
@@ -727,17 +738,16 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   if (G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p->c, grid, smem, st));
-  const unsigned nbN = (unsigned)cdiv(ctx->N, 256), nbC = (unsigned)cdiv(ctx->N_cell, 256);
+  const unsigned nbN = (unsigned)cdiv(ctx->N, 256);
   // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3) unless the
   // caller says h has not changed since the previous SPH call on this tree (option "sph_reuse_radii": stage 2 of a
   // step after stage 1, L252 steps 4 and 6)
   if (!(ctx->sph_reuse && ctx->sph_radii_valid)) {
     gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
-    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
-    sph_radii_kernel<<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc);   // (val[1], slot_nc: the build's
-                                                                                                                                 // per-slot levels and scanned level counts)
-    sph_radii_finish_kernel<<<nbC, 256, 0, st>>>(ctx->sph_acc, ctx->N_cell, ctx->c_sph);
-    ctx->launches += 3;
+    OTOO_CUDA(ctx, cudaMemsetAsync(ctx->c_sph, 0, sizeof(float2) * ctx->N_cell, st));
+    sph_radii_kernel<true><<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, nullptr,   // (val[1], slot_nc: the build's
+                                                reinterpret_cast<uint32_t*>(ctx->c_sph));                                        // per-slot levels and scanned level counts)
+    ctx->launches += 2;
   }
   p->hs = ctx->sorted_h; p->aux = ctx->sorted_aux; p->svel = nullptr; p->svis = nullptr; p->c_sph = ctx->c_sph;
   p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
@@ -752,7 +762,7 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
 // ordered bits in sph_acc[2c].  The fp32 SPH radii are recomputed by every SPH call anyway.
 otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st) {
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
-  sph_radii_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc);
+  sph_radii_kernel<false><<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc, nullptr);
   ctx->launches += 1;
   ctx->sph_radii_valid = false;
   return OTOO_OK;
