@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(256) rb2_delta_kernel(const double* __restrict
     double rb;
     if (c_MP[4 * c] > (double)m_limit) rb = __dmul_rn(2.0, (double)S);
     else {
-      const double h = __dmul_rn(0.5, __longlong_as_double((long long)bmax_bits[2 * c]));
+      const double h = __dmul_rn(0.5, __dsqrt_rn(__longlong_as_double((long long)bmax_bits[2 * c])));   // bmax_bits: max |x - CM|^2
       const double q = __dsqrt_rn(__ddiv_rn(__dmul_rn(3.0, c_B2[c]), (double)delta));
       rb = __dadd_rn(h, __dsqrt_rn(__dadd_rn(__dmul_rn(h, h), q)));
     }

@@ -106,8 +106,10 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
       double b = 0.0, r = 0.0;
       if (cell != 0xFFFFFFFFu) {
         double dx = __dsub_rn((double)p.x, cx[j]), dy = __dsub_rn((double)p.y, cy[j]), dz = __dsub_rn((double)p.z, cz[j]);
-        b = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
-        r = __dadd_rn(b, h);
+        b = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        // fp64 form: the maximum of the SQUARED distances (the correctly rounded square root is monotone: the root of
+        // the maximum, taken once per cell by rb2_delta_kernel, is the maximum of the roots)
+        if (F32) { b = __dsqrt_rn(b); r = __dadd_rn(b, h); }
       }
       // segmented max over runs of equal cell id (runs are contiguous in slot order); head = first lane of a run
       const uint32_t pc = __shfl_up_sync(0xFFFFFFFFu, cell, 1);
@@ -130,7 +132,7 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
           if (bb > cur.x) atomicMax(out32 + 2 * (size_t)cell, bb);
           if (rr > cur.y) atomicMax(out32 + 2 * (size_t)cell + 1, rr);
         }
-      } else {          // the Delta-MAC's b_max alone, in fp64 (acc[2c]; acc[2c + 1] is not written)
+      } else {          // the Delta-MAC's b_max^2 alone, in fp64 (acc[2c]; acc[2c + 1] is not written)
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
           const uint32_t oc = __shfl_down_sync(0xFFFFFFFFu, cell, o);
@@ -758,8 +760,8 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
 
 }  // namespace
 
-// fp64 b_max (L63) of every cell for the absolute-error MAC: the Eq. 5 pass with h = 0; leaves the maxima as
-// ordered bits in sph_acc[2c].  The fp32 SPH radii are recomputed by every SPH call anyway.
+// fp64 b_max (L63) of every cell for the absolute-error MAC: the Eq. 5 pass with h = 0; leaves the maxima of the SQUARED
+// distances as ordered bits in sph_acc[2c] (b_max = their square root: rb2_delta_kernel).  The fp32 SPH radii are recomputed by every SPH call anyway.
 otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st) {
   OTOO_CUDA(ctx, cudaMemsetAsync(ctx->sph_acc, 0, 2 * sizeof(unsigned long long) * ctx->N_cell, st));
   sph_radii_kernel<false><<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(ctx->spos, nullptr, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, ctx->sph_acc, nullptr);
