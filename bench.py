@@ -293,14 +293,16 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
             flush_buf.fill_(1)
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
             ev[0].record()
+            o.otoo_set_option("sph_reuse_walk", 0 if args.no_sph_reuse_walk else 1)   # stage 1 records the leaves each group opens ...
             rho, nn = o.otoo_sph_density(d_h, Gs)
             P = o.otoo_eos_ideal(rho, d_u, 5.0 / 3.0)
             ev[1].record()
             s1 = o.otoo_last_stats()
             k1 = s1["ms_walk_force"]
             o.otoo_set_option("sph_reuse_radii", 1)     # h is fixed within a step: stage 2 keeps stage 1's Eq. 5 radii
-            o.otoo_sph_force(d_h, rho, P, Gs, vel=d_v)
+            o.otoo_sph_force(d_h, rho, P, Gs, vel=d_v)  # ... and stage 2 starts from them (same MAC, same radii: the same leaves)
             o.otoo_set_option("sph_reuse_radii", 0)
+            o.otoo_set_option("sph_reuse_walk", 0)
             ev[2].record()
             s2 = o.otoo_last_stats()
             k2 = s2["ms_walk_force"]
@@ -319,7 +321,8 @@ def measure(args, name, theta, seed, steps, warmup, local, world, n=None, e2e=Tr
         ev_d, ev_f = s1["sum_evaluated"], s2["sum_evaluated"]
         ops_d = SPH_FLOP_TEST["density"] * ev_d + SPH_FLOP_HIT["density"] * pairs
         ops_f = SPH_FLOP_TEST["force"] * ev_f + SPH_FLOP_HIT["force"] * pairs
-        res["sph"] = {"group": Gs, "density_eos_ms": td, "force_dudt_ms": tf, "density_kernel_ms": kd, "force_kernel_ms": kf,
+        res["sph"] = {"group": Gs, "stage2_walk": "full walk" if args.no_sph_reuse_walk else "replays the leaves stage 1 opened (option sph_reuse_walk)",
+                      "density_eos_ms": td, "force_dudt_ms": tf, "density_kernel_ms": kd, "force_kernel_ms": kf,
                       "candidate_pairs_per_pass": cand, "evaluated_pair_tests": {"density": ev_d, "force_dudt": ev_f}, "neighbour_pairs": pairs, "candidate_pairs_per_s": 2 * cand / ((td + tf) * 1e-3),
                       "roofline": {"bound": "alu", "peak": peak, "unit": "TFLOP/s",
                                    "density": {"achieved": ops_d / (kd * 1e-3) / 1e12, "frac": ops_d / (kd * 1e-3) / 1e12 / peak},
@@ -377,6 +380,7 @@ def main():
     ap.add_argument("--seed", type=int, default=1206)
     ap.add_argument("--n", type=int, default=None, help="override the workload's particle count (scaling runs, e.g. Fig. 9)")
     ap.add_argument("--group-sph", type=int, default=None, help="group size of the SPH rows (C4 / COLD; default: the workload's, 64)")
+    ap.add_argument("--no-sph-reuse-walk", action="store_true", help="SPH rows: stage 2 walks the tree again instead of starting from the leaves stage 1 opened")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the C2 / C3 / C4 blocks of the default line")
     ap.add_argument("--probe", default=None, choices=["ffma2", "sumloop", "rank", "sort"],

@@ -254,6 +254,13 @@ otoo_status otoo_sort_pairs_static(uint64_t* d_keys, uint32_t* d_vals, uint64_t*
  * "sph_reuse_radii" = 1: an SPH call keeps the sorted smoothing lengths and the Eq. 5 cell radii of the previous SPH
  * call on the same tree instead of recomputing them: the caller states that d_h has not changed since (stage 2 after
  * stage 1 of one step, PAPER.md L252 steps 4 and 6).  A new tree or otoo_gravity_delta invalidates them.  Default 0.
+ * "sph_reuse_walk" = 1 (with "sph_reuse_radii" = 1; default 0): otoo_sph_density / otoo_sph_stage1 record, per group, the leaves
+ * their walk opens (4 KB per group, allocated on first use), and an otoo_sph_force / otoo_sph_force_visc call that keeps
+ * the radii starts every group's walk from those leaves instead of the root: the SPH criterion (Eq. 5; R15, R26)
+ * is the same for both stages, so the same leaves open and the same particles are listed.  Same neighbours, same
+ * per-group counters (the tests of the internal cells are counted, not repeated); sums differ in rounding order only.
+ * Group sizes up to 64; a group that opened more than 1024 leaves or handed part of its walk to another warp, larger
+ * groups, another group_size / group range / group_distance than the recording call's: the full walk, as without it.
  * "output_sorted" = 1: otoo_gravity / otoo_gravity_delta write row s of d_acc_pot for the target at SORTED slot s
  * (otoo_export_tree's d_perm names its original index) instead of the caller's order; with a group range the rows
  * [group_begin * group_size, ...) of the range are the only non-zero ones and are contiguous.  otoo_unsort brings

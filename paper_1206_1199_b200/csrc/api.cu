@@ -131,7 +131,8 @@ void otoo_destroy(otoo_ctx* ctx) {
                   ctx->c_child_first, ctx->c_level, ctx->c_child_count, ctx->c_MP, ctx->c_cm64, ctx->c_s, ctx->c_B2, ctx->c_sph,
                   ctx->sph_acc, ctx->tmp_key[0], ctx->tmp_key[1], ctx->tmp_val[0], ctx->tmp_val[1], ctx->d_bbox,
                   ctx->d_counters, ctx->g_ntests, ctx->g_ncells, ctx->g_nparts, ctx->walk_spill, ctx->d_sums,
-                  ctx->pool_slots, ctx->pool_seq, ctx->walk_shared, ctx->stage_in, ctx->stage_out};
+                  ctx->pool_slots, ctx->pool_seq, ctx->walk_shared, ctx->stage_in, ctx->stage_out,
+                  ctx->rec_cells, ctx->rec_count, ctx->rec_ntests};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
   if (ctx->h_root) cudaFreeHost(ctx->h_root);
@@ -402,6 +403,7 @@ otoo_status otoo_set_option(otoo_ctx* ctx, const char* name, int64_t value) {
     return OTOO_OK;
   }
   if (strcmp(name, "sph_reuse_radii") == 0) { ctx->sph_reuse = value != 0; return OTOO_OK; }
+  if (strcmp(name, "sph_reuse_walk") == 0) { ctx->sph_reuse_walk = value != 0; return OTOO_OK; }
   if (strcmp(name, "output_sorted") == 0) { ctx->out_sorted = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_only") == 0) { ctx->walk_only = value != 0; return OTOO_OK; }
   if (strcmp(name, "walk_profile") == 0) { ctx->walk_profile = value != 0; return OTOO_OK; }

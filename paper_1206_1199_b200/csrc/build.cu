@@ -461,7 +461,7 @@ __global__ void __launch_bounds__(256) b2_all_kernel(const LevelOff off, const i
 
 otoo_status otoo_build_impl(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit, cudaStream_t st) {
   ctx->built = false; ctx->walked = false; ctx->sph_radii_valid = false; ctx->b2_valid = false;
-  ctx->rb2_valid = false; ctx->walk_reset_valid = false;
+  ctx->rb2_valid = false; ctx->walk_reset_valid = false; ctx->rec_valid = false;
   const float4* pos = reinterpret_cast<const float4*>(d_pos_mass);
   unsigned* bbox = reinterpret_cast<unsigned*>(ctx->d_bbox);
   const unsigned nbN = (unsigned)cdiv(N, 256);

@@ -8,6 +8,7 @@
 
 #define OTOO_MAXLEV 21
 #define OTOO_NLEV 22                 // levels 0..21
+#define OTOO_REC_CAP 1024             // recorded leaf ids per group (option sph_reuse_walk); a group that opens more walks again
 #define OTOO_POOL_SLOTS 16384         // task slots of the walk's pool (walk.cuh)
 #define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)
@@ -116,6 +117,11 @@ struct otoo_ctx {
   int key_order;         // option "key_order": 0 Morton (R3), 1 Hilbert (R20); read by the next build
   int out_sorted;        // option "output_sorted": otoo_gravity / otoo_gravity_delta write row s of the output for sorted slot s
   int sph_reuse;         // option "sph_reuse_radii": SPH calls keep sorted h and the Eq. 5 radii of the previous SPH call on this tree
+  int sph_reuse_walk;    // option "sph_reuse_walk": the density / stage-1 walk records the leaves every group opens, and a force
+                         // walk that keeps the radii (sph_reuse_radii) starts from them instead of the root (walk.cuh, REC)
+  uint32_t* rec_cells; uint32_t* rec_count; uint32_t* rec_ntests;   // OTOO_REC_CAP leaf ids per group; leaves and MAC tests per group
+  int64_t rec_groups_cap;
+  bool rec_valid; int rec_G, rec_pieces; int64_t rec_gb, rec_gc;     // what the record was taken with
   int walk_only;         // option "walk_only" (diagnostic)
   int walk_profile;      // option "walk_profile": the gravity walk kernel counts its warps' waiting time (slower)
   int dist_kind;         // option "group_distance": 0 AABB (R8), 1 exact minimum over the group's members (R23)

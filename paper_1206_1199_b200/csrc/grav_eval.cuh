@@ -104,6 +104,7 @@ struct GravVisitor {
     for (int t = 0; t < T; t++) if (member_ok(p.c, g0, t * 32 + lane) && (uint32_t)(g0 + t * 32 + lane) - f < n) selfmask |= 1u << t;
   }
   static constexpr bool SUBMIT_LAST = false, CULL = false;
+  static constexpr int REC = 0;
   template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
   __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
     if (!p.c.walk_only) eval(list, n);

@@ -82,6 +82,7 @@ struct GravWalker {
   static constexpr int T = T_, E = 1, LCAP = OTOO_WS_LCAP, NP = (T_ + 1) / 2;
   static constexpr bool SUBMIT_LAST = true;     // the evaluator needs the end-of-unit mark to store
   static constexpr bool CULL = false;
+  static constexpr int REC = 0;
   template <class En> __device__ __forceinline__ bool keep(const En&) const { return true; }
   typedef WsPair<32 * NP * 3, 32 * T_> Pair;
   const GravParams& p;
@@ -354,6 +355,7 @@ otoo_status otoo_walk_prepare(otoo_ctx* ctx, int G, WalkCommon* c, int* grid, si
   c->use_pool = ctx->use_pool;
   c->walk_only = ctx->walk_only;
   c->dist_kind = 0;
+  c->rec_mode = 0; c->rec_cap = 0; c->rec_cells = nullptr; c->rec_count = nullptr; c->rec_ntests = nullptr;
   ctx->last_group_size = G; ctx->last_ngroups = total_groups; ctx->last_walk_only = ctx->walk_only;
   return OTOO_OK;
 }

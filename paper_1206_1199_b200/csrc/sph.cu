@@ -174,7 +174,8 @@ struct SphParams {
 __device__ __forceinline__ f32x2 pk2v(float a, float b) { f32x2 r; asm volatile("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 __device__ __forceinline__ float2 as2(f32x2 v) { float2 r; upk2(v, r.x, r.y); return r; }
-template <int T_, int MODE>
+// REC_: 1 the walk records the leaves every whole group opens, 2 it starts from recorded leaves (walk.cuh; option sph_reuse_walk)
+template <int T_, int MODE, int REC_ = 0>
 struct SphVisitor {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 || MODE == 3 ? 2 : (MODE == 4 ? 4 : 3));
   static constexpr int LCAP = OTOO_LIST_CAP;
@@ -318,6 +319,7 @@ struct SphVisitor {
   }
   __device__ __forceinline__ void mark_self(uint32_t, uint32_t, int64_t, int) {}
   static constexpr bool SUBMIT_LAST = false;
+  static constexpr int REC = REC_;
   __device__ __forceinline__ float4* submit(float4* list, int n, bool) {
     if (!p.c.walk_only) eval(list, n);
     return list;
@@ -484,30 +486,38 @@ struct SphVisitor {
   }
 };
 
-template <int T, int MODE>
+template <int T, int MODE, int REC>
 __device__ __forceinline__ void walk_sph_body(const SphParams& p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float4* list = reinterpret_cast<float4*>(smem_raw) + warp * OTOO_LIST_STRIDE;
   uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
-  SphVisitor<T, MODE> v(p);
+  SphVisitor<T, MODE, REC> v(p);
   v.msk = reinterpret_cast<uint32_t*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (SphVisitor<T, MODE>::W * T * 32);
   v.pbox = reinterpret_cast<float4*>(smem_raw + otoo_walk_smem_bytes_dev() + (size_t)OTOO_WALK_WARPS * SphVisitor<T, MODE>::W * T * 32 * sizeof(uint32_t)) +
            warp * (2 * OTOO_PIECES);
   v.lane_ = lane;
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
 }
-template <int T, int MODE>
-__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) { walk_sph_body<T, MODE>(p); }
+template <int T, int MODE, int REC>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32) walk_sph_kernel(const SphParams p) { walk_sph_body<T, MODE, REC>(p); }
 // The density walk of groups up to 64 with 5 CTAs per SM (96 registers instead of 122-126): A/B at C4, G = 64: 2.13 -> 2.03 ms
 // (6 CTAs: 2.02).  The force kernels lose with 5 or 6 (force + du/dt 2.98 -> 3.22 / 3.32 ms) and keep ptxas' own choice.
+template <int T, int MODE, int REC>
+__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32, 5) walk_sph_kernel_occ5(const SphParams p) { walk_sph_body<T, MODE, REC>(p); }
+// rec = WalkCommon::rec_mode: the recording / replaying instantiations exist for groups up to 64 (T <= 2), recording for the
+// gather stages (density, stage 1), replaying for the force stages; anything else runs the plain walk (a group without a
+// record walks from the root in any case)
 template <int T, int MODE>
-__global__ void __launch_bounds__(OTOO_WALK_WARPS * 32, 5) walk_sph_kernel_occ5(const SphParams p) { walk_sph_body<T, MODE>(p); }
-template <int T, int MODE>
-void (*sph_kernel_ptr())(const SphParams) {
-  if constexpr (MODE == 0 && T <= 2) return walk_sph_kernel_occ5<T, MODE>;
-  else return walk_sph_kernel<T, MODE>;
+void (*sph_kernel_ptr(int rec))(const SphParams) {
+  constexpr bool GATHER = MODE == 0 || MODE == 3;
+  if constexpr (T <= 2) {
+    if (GATHER && rec == 1) { if constexpr (GATHER) { if constexpr (MODE == 0) return walk_sph_kernel_occ5<T, MODE, 1>; else return walk_sph_kernel<T, MODE, 1>; } }
+    if (!GATHER && rec == 2) { if constexpr (!GATHER) return walk_sph_kernel<T, MODE, 2>; }
+  }
+  if constexpr (MODE == 0 && T <= 2) return walk_sph_kernel_occ5<T, MODE, 0>;
+  else return walk_sph_kernel<T, MODE, 0>;
 }
 
 
@@ -519,6 +529,7 @@ struct SphWalker {
   static constexpr int T = T_, E = MODE == 0 ? 1 : (MODE == 1 ? 2 : 3);
   static constexpr int LCAP = OTOO_WS_LCAP;
   static constexpr bool SUBMIT_LAST = true;
+  static constexpr int REC = 0;
   typedef WsPair<2, 32 * T_> Pair;
   const SphParams& p;
   Pair& sm;
@@ -716,7 +727,7 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
   void (*kern)(const SphParams) = nullptr;
 #define OTOO_SPH_CASE(TT)                                                                                              \
   smem = smem0 + (size_t)OTOO_WALK_WARPS * (SphVisitor<TT, MODE>::W * TT * 32 * sizeof(uint32_t) + 2 * OTOO_PIECES * sizeof(float4));   /* + the mask words + the pieces' boxes */   \
-  kern = sph_kernel_ptr<TT, MODE>();                                                                                  \
+  kern = sph_kernel_ptr<TT, MODE>(p.c.rec_mode);                                                                      \
   OTOO_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                   \
   OTOO_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, OTOO_WALK_WARPS * 32, smem));                \
   if (occ < 1) occ = 1;                                                                                                 \
@@ -736,7 +747,8 @@ otoo_status launch_sph(otoo_ctx* ctx, const SphParams& p, int G, int grid, size_
   return OTOO_OK;
 }
 
-otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, int* grid, size_t* smem, cudaStream_t st) {
+// gather_stage: the density / stage-1 walks (they may record the opened leaves); the force walks may replay them
+otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, int* grid, size_t* smem, cudaStream_t st, bool gather_stage) {
   if (G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)
     return otoo_fail(ctx, OTOO_ERR_INVALID_ARG, "group_size must be 4, 8, 16, 32, 64, 128 or 256");
   OTOO_TRY(otoo_walk_prepare(ctx, G, &p->c, grid, smem, st));
@@ -744,7 +756,9 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   // Eq. 5 radii depend on h: recomputed per call ("update the cell properties for SPH", L248 step 3) unless the
   // caller says h has not changed since the previous SPH call on this tree (option "sph_reuse_radii": stage 2 of a
   // step after stage 1, L252 steps 4 and 6)
-  if (!(ctx->sph_reuse && ctx->sph_radii_valid)) {
+  const bool radii_kept = ctx->sph_reuse && ctx->sph_radii_valid;
+  if (!radii_kept) {
+    ctx->rec_valid = false;                          // other h: other radii, other opened leaves
     gather_h_kernel<<<nbN, 256, 0, st>>>(d_h, ctx->val[0], ctx->N, ctx->sorted_h);
     OTOO_CUDA(ctx, cudaMemsetAsync(ctx->c_sph, 0, sizeof(float2) * ctx->N_cell, st));
     sph_radii_kernel<true><<<nbN, 256, 0, st>>>(ctx->spos, ctx->sorted_h, ctx->N, ctx->val[1], ctx->slot_nc, ctx->c_cm64, nullptr,   // (val[1], slot_nc: the build's
@@ -755,6 +769,28 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   p->rho = nullptr; p->nngb = nullptr; p->acc = nullptr;
   p->pieces = ctx->dist_kind == 2;
   ctx->sph_radii_valid = true;
+  // option sph_reuse_walk: stage 2 of a step opens exactly the leaves stage 1 opened (same MAC, R15 / R26, same radii)
+  if (ctx->sph_reuse_walk && !ctx->use_ws_sph) {
+    const int64_t total_groups = cdiv(ctx->N, G);
+    if (gather_stage) {
+      if (total_groups > ctx->rec_groups_cap) {
+        ctx->rec_valid = false;
+        for (uint32_t** q : {&ctx->rec_cells, &ctx->rec_count, &ctx->rec_ntests}) { if (*q) cudaFree(*q); *q = nullptr; }
+        ctx->rec_groups_cap = 0;
+        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_cells, sizeof(uint32_t) * (size_t)total_groups * OTOO_REC_CAP));
+        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_count, sizeof(uint32_t) * (size_t)total_groups));
+        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_ntests, sizeof(uint32_t) * (size_t)total_groups));
+        ctx->rec_groups_cap = total_groups;
+      }
+      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->rec_count, 0xFF, sizeof(uint32_t) * (size_t)total_groups, st));   // nothing recorded yet
+      p->c.rec_mode = 1;
+      ctx->rec_valid = true; ctx->rec_G = G; ctx->rec_pieces = p->pieces; ctx->rec_gb = ctx->group_begin; ctx->rec_gc = ctx->group_count;
+    } else if (radii_kept && ctx->rec_valid && ctx->rec_G == G && ctx->rec_pieces == p->pieces && ctx->rec_gb == ctx->group_begin &&
+               ctx->rec_gc == ctx->group_count) {
+      p->c.rec_mode = 2;
+    }
+    p->c.rec_cap = OTOO_REC_CAP; p->c.rec_cells = ctx->rec_cells; p->c.rec_count = ctx->rec_count; p->c.rec_ntests = ctx->rec_ntests;
+  }
   return OTOO_OK;
 }
 
@@ -772,7 +808,7 @@ otoo_status otoo_bmax_impl(otoo_ctx* ctx, cudaStream_t st) {
 
 otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float* d_rho, uint32_t* d_nngb, cudaStream_t st) {
   SphParams p; int grid; size_t smem;
-  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st, true));
   p.rho = d_rho; p.nngb = d_nngb;
   OTOO_CUDA(ctx, cudaMemsetAsync(d_rho, 0, 4 * (size_t)ctx->N, st));
   if (d_nngb) OTOO_CUDA(ctx, cudaMemsetAsync(d_nngb, 0, 4 * (size_t)ctx->N, st));
@@ -786,7 +822,7 @@ otoo_status otoo_sph_density_impl(otoo_ctx* ctx, const float* d_h, int G, float*
 otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d_vel, int G, float* d_rho, uint32_t* d_nngb,
                                  float* d_divrot, cudaStream_t st) {
   SphParams p; int grid; size_t smem;
-  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st, true));
   gather_vel_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(reinterpret_cast<const float4*>(d_vel), ctx->val[0], ctx->N, ctx->sorted_vel);
   p.svel = ctx->sorted_vel; p.rho = d_rho; p.nngb = d_nngb; p.acc = reinterpret_cast<float4*>(d_divrot);
   OTOO_CUDA(ctx, cudaMemsetAsync(d_rho, 0, 4 * (size_t)ctx->N, st));
@@ -807,7 +843,7 @@ otoo_status otoo_sph_stage1_impl(otoo_ctx* ctx, const float* d_h, const float* d
 otoo_status otoo_sph_force_impl(otoo_ctx* ctx, const float* d_h, const float* d_rho, const float* d_P, const float* d_vel,
                                 const float* d_visc, int G, float* d_acc, cudaStream_t st) {
   SphParams p; int grid; size_t smem;
-  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st));
+  OTOO_TRY(sph_prepare(ctx, d_h, G, &p, &grid, &smem, st, false));
   gather_force_inputs_kernel<<<(unsigned)cdiv(ctx->N, 256), 256, 0, st>>>(d_h, d_rho, d_P, reinterpret_cast<const float4*>(d_vel),
                                                                           reinterpret_cast<const float4*>(d_visc), ctx->val[0],
                                                                           ctx->N, ctx->sorted_aux, ctx->sorted_vel, ctx->sorted_vis);

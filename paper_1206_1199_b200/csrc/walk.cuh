@@ -164,6 +164,11 @@ struct WalkCommon {
   int walk_only;                                                // 1: lists are built and counted but not evaluated (measures the walk)
   int dist_kind;                                                // gravity: 0 one box per group (R8), 1 exact minimum over the members (R23),
                                                                 // 2 minimum over the boxes of the group's pieces (R25)
+  // visitors with REC (the SPH walks): the leaves a group opens, recorded by one walk and replayed by the next one with
+  // the same MAC (option "sph_reuse_walk": stage 2 of an SPH step opens exactly the leaves of stage 1, R15 / R26)
+  int rec_mode;                                                 // 0 off, 1 record, 2 replay (host side: picks the kernel instantiation, V::REC)
+  int rec_cap;                                                  // leaf ids per group
+  uint32_t* rec_cells; uint32_t* rec_count; uint32_t* rec_ntests;   // [group][rec_cap]; per group: leaves (0xFFFFFFFF: none recorded), MAC tests of its walk
 };
 
 // member idx (0 .. 32 T - 1) of the group starting at slot g0 exists
@@ -190,6 +195,8 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 //   void pad(float4* dst)                          a null entry
 //   void mark_self(uint32_t first, uint32_t count, int64_t g0, int lane)
 //   void store(int64_t g0, int lane)               atomicAdd results to the outputs
+//   static constexpr int REC;   1: the walk records the leaves each whole group opens; 2: it starts from recorded leaves; 0: neither
+//                               (compile time: the bookkeeping costs the SPH kernels 5-7 % when it is only switched off at run time)
 template <class V>
 __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* list0, uint32_t* stk, int lane, int64_t gwarp) {
   const int G = c.gs;                                // targets per group (<= 32 * V::T; below 32: the other lanes idle)
@@ -206,7 +213,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
   for (;;) {
     // ---------------- acquire a unit of work
     uint32_t g = 0; int sp = 0;
-    bool got = false;
+    bool got = false, whole = false;                   // whole: the unit is a group from the main queue, not a pool task
     auto take = [&](uint32_t ticket) {   // copy task `ticket` (already published) to the shared stack
       const uint32_t slot = ticket % OTOO_POOL_SLOTS;
       __threadfence();
@@ -221,7 +228,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     if (!got && !main_done) {
       if (lane == 0) g = atomicAdd(&c.ws->queue, 1u);
       g = __shfl_sync(0xFFFFFFFFu, g, 0);
-      if ((int64_t)g < c.ngroups) { got = true; g += c.g_begin; if (lane == 0) stk[0] = 0u; sp = 1; }
+      if ((int64_t)g < c.ngroups) { got = true; whole = true; g += c.g_begin; if (lane == 0) stk[0] = 0u; sp = 1; }
       else main_done = true;
     }
     if (!got) {
@@ -250,6 +257,24 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     v.load_group(g0, lane, list);   // the list is empty here: usable as scratch
     int gsp = 0, nlist = 0;
     uint32_t ntests = 0, ncells = 0, nparts = 0, iter = 0, nflush = 0, nkept = 0;   // nkept: list entries handed to the sums (after a cull)
+    // recorded leaves (REC): a whole group records the leaves it opens unless part of its walk goes to the pool; a whole
+    // group with a record starts from those leaves (through the private spill area) instead of the root: the same MAC
+    // opens every one of them again, the tests of the internal cells are not repeated but counted (rec_ntests)
+    bool rec_on = false, rec_bad = false;
+    uint32_t nrec = 0, rec_extra = 0;
+    if constexpr (V::REC == 1) rec_on = whole;
+    if constexpr (V::REC == 2) {
+      if (whole) {
+        const uint32_t cnt = c.rec_count[g];
+        if (cnt != 0xFFFFFFFFu && (int)cnt <= c.spill_cap) {
+          const uint32_t* src = c.rec_cells + (size_t)g * c.rec_cap;
+          for (uint32_t i = lane; i < cnt; i += 32) gspill[i] = src[i];
+          __syncwarp();
+          gsp = (int)cnt; sp = 0;
+          rec_extra = c.rec_ntests[g] - cnt;
+        }
+      }
+    }
 
     auto flush = [&](bool last = false) {
       nkept += (uint32_t)nlist;
@@ -292,6 +317,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       if (!ts) return false;
       for (int i = lane; i < d; i += 32) __stcg(&ts->cells[i], stk[i]);
       pool_end(ts, d);
+      if constexpr (V::REC == 1) rec_bad = true;     // part of this group's walk is someone else's now
       return true;
     };
     // drop the d bottom entries of the shared stack (after they were donated or spilled)
@@ -354,6 +380,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
               for (int i = 0; i < nch; i++) __stcg(&ts->cells[o + i], B.y + (uint32_t)i);
               pool_end(ts, total);
               pushed = true;
+              if constexpr (V::REC == 1) rec_bad = true;
             } else {
               const int d = OTOO_TASK_CELLS;      // stack_cap >= 512, total <= 256
               if (gsp + d <= c.spill_cap) {
@@ -390,6 +417,14 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       }
       // opened leaves -> their particles (L57 rule 3)
       const unsigned lm = __ballot_sync(0xFFFFFFFFu, open_leaf);
+      if constexpr (V::REC == 1) {
+        if (rec_on && lm) {
+          const uint32_t nl = (uint32_t)__popc(lm);
+          if (nrec + nl <= (uint32_t)c.rec_cap) { if (open_leaf) c.rec_cells[(size_t)g * c.rec_cap + nrec + (uint32_t)__popc(lm & lanemask_lt_())] = cell; }
+          else rec_bad = true;
+          nrec += nl;
+        }
+      }
       if (lm) {
         const int cnt = open_leaf ? (int)B.z : 0;
         const int inc = warp_inclusive_scan(cnt, lane);
@@ -455,6 +490,10 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     }
     if (nlist || V::SUBMIT_LAST) flush(true);
     v.store(g0, lane);
+    if constexpr (V::REC == 2) ntests += rec_extra;
+    if constexpr (V::REC == 1) {
+      if (rec_on && lane == 0) { c.rec_count[g] = rec_bad ? 0xFFFFFFFFu : nrec; c.rec_ntests[g] = ntests; }
+    }
     if (lane == 0) {
       atomicAdd(c.g_ntests + g, ntests); atomicAdd(c.g_ncells + g, ncells); atomicAdd(c.g_nparts + g, nparts);
       __threadfence();

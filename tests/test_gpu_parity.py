@@ -312,6 +312,55 @@ def _sph_parity(otoo, orc, n, G, dist=2):
             assert np.all(out[:, 3] == 0)
 
 
+@pytest.mark.parametrize("pool", [1, 0])
+@pytest.mark.parametrize("n,G,dist", [(20000, 64, 2), (20000 + 11, 32, 2), (8000, 128, 0), (6000, 256, 2), (6000 + 1, 16, 2)])
+def test_sph_force_replays_the_leaves_of_the_density_walk(otoo, orc, n, G, dist, pool):
+    """Option sph_reuse_walk (with sph_reuse_radii): the density walk records the leaves every group opens, the force walk
+    starts from them instead of the root -- the same MAC (R15 / R26) opens them all again.  Against the oracle: per-group
+    tests and particles of the force walk exact (the tests of the internal cells are counted, not repeated), forces and
+    du/dt within the rule; against the plain force walk: the same counters, and fewer walk steps where every group could
+    record (pool = 0: no part of a group's walk is handed to another warp; with the pool a group that donated walks again)."""
+    w = gen.wd_pair(n, 77)
+    pm, h, u = w["pos_mass"], w["h"], w["u"]
+    vel = (w["vel"] - 0.3 * np.c_[pm[:, :3], np.zeros(n)]).astype(np.float32)
+    t = check_tree(otoo, orc, pm, 16)
+    t.set_dist_kind(dist)
+    otoo.otoo_set_option("group_distance", dist)
+    otoo.otoo_set_option("task_pool", pool)
+    try:
+        rho, _ = otoo.otoo_sph_density(dev(h), G)
+        P = otoo.otoo_eos_ideal(rho, dev(u), 5.0 / 3.0)
+        rg, Pg = rho.cpu().numpy(), P.cpu().numpy()
+        plain = otoo.otoo_sph_force(dev(h), rho, P, G, vel=dev(vel)).cpu().numpy()
+        st_plain = otoo.otoo_last_stats()
+        nt_plain, _, np_plain = otoo.otoo_export_group_stats()
+        otoo.otoo_set_option("sph_reuse_walk", 1)
+        otoo.otoo_set_option("sph_reuse_radii", 1)
+        rho2, _ = otoo.otoo_sph_density(dev(h), G)                       # records
+        assert float((rho2 - rho).abs().max()) <= 1e-6 * float(rho.abs().max())      # (pool tasks add in another order)
+        out = otoo.otoo_sph_force(dev(h), rho, P, G, vel=dev(vel)).cpu().numpy()   # replays
+        st = otoo.otoo_last_stats()
+        nt, _, npart = otoo.otoo_export_group_stats()
+    finally:
+        otoo.otoo_set_option("sph_reuse_walk", 0)
+        otoo.otoo_set_option("sph_reuse_radii", 0)
+        otoo.otoo_set_option("group_distance", 2)
+        otoo.otoo_set_option("task_pool", 1)
+    assert np.array_equal(nt, nt_plain) and np.array_equal(npart, np_plain)
+    assert st["sum_tests"] == st_plain["sum_tests"] and st["sum_interactions"] == st_plain["sum_interactions"]
+    if pool == 0 and G <= 64:                                           # (the replaying kernels exist for groups up to 64)
+        assert st["sum_steps"] < 0.9 * st_plain["sum_steps"]            # the internal levels were not walked again
+    if G > 64:
+        assert st["sum_steps"] == st_plain["sum_steps"] or pool == 1    # larger groups walk from the root as before
+    rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel)
+    rd = t.sph_density(h, G)                                            # (the oracle's walk is the same for both stages)
+    assert np.array_equal(nt, rd["n_tests"]) and np.array_equal(npart, rd["n_parts"])
+    e, raw = acc_err(out, rf["acc_dudt"], rf["abs_sum"][:, 0], pct=99, what="a_sph")
+    assert e.max() <= TOL, e.max()
+    report(f"{_label()}:dudt", out[:, 3], rf["acc_dudt"][:, 3], rf["abs_sum"][:, 1], pct=None)
+    assert np.abs(out - plain).max() <= 1e-4 * np.abs(plain).max()      # (another order of the same leaves)
+
+
 @pytest.mark.parametrize("kind,n,G,target,tol,h0", [("uniform_cube", 20000, 64, 40.0, 2.0, 0.03), ("wd", 16384 + 3, 32, 50.0, 3.0, None),
                                                       ("uniform_cube", 5000, 128, 32.0, 0.0, 0.2)])
 def test_adaptive_h_parity(otoo, orc, kind, n, G, target, tol, h0):
