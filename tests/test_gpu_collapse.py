@@ -32,6 +32,9 @@ def test_cold_collapse_energy_conservation():
         o.otoo_build_tree(x, 16)
         o.otoo_sph_adapt_h(h, 50.0, 4.0, 12, Gs)      # once: h then stays fixed (re-adapting h every step without
                                                       # grad-h terms triples the energy error of this short run)
+        # h fixed within a step: stage 2 keeps stage 1's Eq. 5 radii and starts from the leaves stage 1 opened
+        o.otoo_set_option("sph_reuse_radii", 1)
+        o.otoo_set_option("sph_reuse_walk", 1)
 
         def forces():
             o.otoo_build_tree(x, 16)
