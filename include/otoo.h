@@ -258,7 +258,7 @@ otoo_status otoo_sort_pairs_static(uint64_t* d_keys, uint32_t* d_vals, uint64_t*
  * their walk opens (4 KB per group, allocated on first use), and an otoo_sph_force / otoo_sph_force_visc call that keeps
  * the radii starts every group's walk from those leaves instead of the root: the SPH criterion (Eq. 5; R15, R26)
  * is the same for both stages, so the same leaves open and the same particles are listed.  Same neighbours, same
- * per-group counters (the tests of the internal cells are counted, not repeated); sums differ in rounding order only.
+ * per-group counters (the tests of the recording walk are counted, not repeated); sums differ in rounding order only.
  * Group sizes up to 64; a group that opened more than 1024 leaves or handed part of its walk to another warp, larger
  * groups, another group_size / group range / group_distance than the recording call's: the full walk, as without it.
  * "output_sorted" = 1: otoo_gravity / otoo_gravity_delta write row s of d_acc_pot for the target at SORTED slot s

@@ -260,7 +260,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
     // recorded leaves (REC): a whole group records the leaves it opens unless part of its walk goes to the pool; a whole
     // group with a record starts from those leaves (through the private spill area) instead of the root: the same MAC
     // opens every one of them again, the tests of the internal cells are not repeated but counted (rec_ntests)
-    bool rec_on = false, rec_bad = false;
+    bool rec_on = false, rec_bad = false, replaying = false;
     uint32_t nrec = 0, rec_extra = 0;
     if constexpr (V::REC == 1) rec_on = whole;
     if constexpr (V::REC == 2) {
@@ -272,6 +272,7 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
           __syncwarp();
           gsp = (int)cnt; sp = 0;
           rec_extra = c.rec_ntests[g] - cnt;
+          replaying = true;
         }
       }
     }
@@ -350,7 +351,14 @@ __device__ __forceinline__ void walk_driver(const WalkCommon& c, V& v, float4* l
       float4 A = make_float4(0.f, 0.f, 0.f, 0.f);
       cellb_t B = make_uint4(0u, 0u, 0u, 0u);
       int cls = 0;
-      if (have) cls = v.classify(cell, A, B);
+      if constexpr (V::REC == 2) {
+        // a recorded leaf passed this very test in the recording walk (same group geometry, same radii): it is opened
+        // without its centre of mass, its radii and the nine box tests; the test is counted all the same
+        if (replaying) { if (have) { B = __ldg(c.cell_b + cell); cls = 2; } }
+        else if (have) cls = v.classify(cell, A, B);
+      } else {
+        if (have) cls = v.classify(cell, A, B);
+      }
       ntests += (uint32_t)k;
       const bool leaf = (B.w & 1u) != 0u;
       const bool accept = cls == 1, open_leaf = cls == 2 && leaf, open_int = cls == 2 && !leaf;
