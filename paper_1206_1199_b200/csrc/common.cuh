@@ -9,6 +9,7 @@
 #define OTOO_MAXLEV 21
 #define OTOO_NLEV 22                 // levels 0..21
 #define OTOO_REC_CAP 1024             // recorded leaf ids per group (option sph_reuse_walk); a group that opens more walks again
+#define OTOO_REC_MAX_BYTES ((size_t)8 << 30)   // no records beyond this size (4 KB per group): the walks then run in full
 #define OTOO_POOL_SLOTS 16384         // task slots of the walk's pool (walk.cuh)
 #define OTOO_WALK_STACK_MAX 512      // smem walk-stack entries per warp
 #define OTOO_WALK_SPILL 8192         // global spill entries per warp (bound 8*32*21 = 5376)

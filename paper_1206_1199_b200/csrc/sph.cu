@@ -773,18 +773,28 @@ otoo_status sph_prepare(otoo_ctx* ctx, const float* d_h, int G, SphParams* p, in
   if (ctx->sph_reuse_walk && !ctx->use_ws_sph) {
     const int64_t total_groups = cdiv(ctx->N, G);
     if (gather_stage) {
-      if (total_groups > ctx->rec_groups_cap) {
+      bool have = total_groups <= ctx->rec_groups_cap;
+      // (the records are an optimisation: beyond OTOO_REC_MAX_BYTES -- tens of millions of small groups -- or if the
+      // allocation fails, the walks simply run in full)
+      if (!have && (size_t)total_groups * OTOO_REC_CAP * sizeof(uint32_t) <= OTOO_REC_MAX_BYTES) {
         ctx->rec_valid = false;
         for (uint32_t** q : {&ctx->rec_cells, &ctx->rec_count, &ctx->rec_ntests}) { if (*q) cudaFree(*q); *q = nullptr; }
         ctx->rec_groups_cap = 0;
-        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_cells, sizeof(uint32_t) * (size_t)total_groups * OTOO_REC_CAP));
-        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_count, sizeof(uint32_t) * (size_t)total_groups));
-        OTOO_CUDA(ctx, cudaMalloc((void**)&ctx->rec_ntests, sizeof(uint32_t) * (size_t)total_groups));
-        ctx->rec_groups_cap = total_groups;
+        if (cudaMalloc((void**)&ctx->rec_cells, sizeof(uint32_t) * (size_t)total_groups * OTOO_REC_CAP) == cudaSuccess &&
+            cudaMalloc((void**)&ctx->rec_count, sizeof(uint32_t) * (size_t)total_groups) == cudaSuccess &&
+            cudaMalloc((void**)&ctx->rec_ntests, sizeof(uint32_t) * (size_t)total_groups) == cudaSuccess) {
+          ctx->rec_groups_cap = total_groups;
+          have = true;
+        } else {
+          cudaGetLastError();
+          for (uint32_t** q : {&ctx->rec_cells, &ctx->rec_count, &ctx->rec_ntests}) { if (*q) cudaFree(*q); *q = nullptr; }
+        }
       }
-      OTOO_CUDA(ctx, cudaMemsetAsync(ctx->rec_count, 0xFF, sizeof(uint32_t) * (size_t)total_groups, st));   // nothing recorded yet
-      p->c.rec_mode = 1;
-      ctx->rec_valid = true; ctx->rec_G = G; ctx->rec_pieces = p->pieces; ctx->rec_gb = ctx->group_begin; ctx->rec_gc = ctx->group_count;
+      if (have) {
+        OTOO_CUDA(ctx, cudaMemsetAsync(ctx->rec_count, 0xFF, sizeof(uint32_t) * (size_t)total_groups, st));   // nothing recorded yet
+        p->c.rec_mode = 1;
+        ctx->rec_valid = true; ctx->rec_G = G; ctx->rec_pieces = p->pieces; ctx->rec_gb = ctx->group_begin; ctx->rec_gc = ctx->group_count;
+      } else ctx->rec_valid = false;
     } else if (radii_kept && ctx->rec_valid && ctx->rec_G == G && ctx->rec_pieces == p->pieces && ctx->rec_gb == ctx->group_begin &&
                ctx->rec_gc == ctx->group_count) {
       p->c.rec_mode = 2;
