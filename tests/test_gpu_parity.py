@@ -432,6 +432,21 @@ def test_sph_force_viscosity_parity(otoo, orc, n, G):
     out0 = otoo.otoo_sph_force_visc(dev(h), rho, P, dev(vel), dev(v0), G).cpu().numpy()
     plain = otoo.otoo_sph_force(dev(h), rho, P, G, vel=dev(vel)).cpu().numpy()
     assert np.allclose(out0, plain, rtol=1e-5, atol=1e-6 * np.abs(plain).max())
+    # the paper's step (L252 steps 4, 6) with option sph_reuse_walk: stage 1 records the opened leaves, the viscous force
+    # starts from them: the counters of the full walk, the same forces within the rule
+    nt_full, _, np_full = otoo.otoo_export_group_stats()
+    otoo.otoo_set_option("sph_reuse_walk", 1)
+    otoo.otoo_set_option("sph_reuse_radii", 1)
+    try:
+        otoo.otoo_sph_stage1(dev(h), dev(vel), G)
+        out_r = otoo.otoo_sph_force_visc(dev(h), rho, P, dev(vel), dev(visc), G).cpu().numpy()
+        nt_r, _, np_r = otoo.otoo_export_group_stats()
+    finally:
+        otoo.otoo_set_option("sph_reuse_walk", 0)
+        otoo.otoo_set_option("sph_reuse_radii", 0)
+    assert np.array_equal(nt_r, nt_full) and np.array_equal(np_r, np_full)
+    e, raw = acc_err(out_r, ref["acc_dudt"], ref["abs_sum"][:, 0], pct=99, what="a_sph_visc_replay")
+    assert e.max() <= TOL, e.max()
 
 
 @pytest.mark.parametrize("world,by_cost", [(3, False), (4, True)])
