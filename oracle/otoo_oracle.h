@@ -24,8 +24,10 @@
  * inverse, same cells as the Morton tree; adaptive h: fixed point, lattice count steps; div v / rot v: linear
  * fields, rigid rotation; artificial viscosity: alpha = 0 / f = 0 limits, receding flow, momentum and energy
  * balance, two-particle closed form.
- * parity unpinned: the absolute accuracy level of the theta-MAC (the paper's error plot, Fig. 5,
- * is for its Delta-MAC and is missing from PAPER.md).
+ * The absolute accuracy of the theta-MAC has no figure in PAPER.md (its error plot, Fig. 5, is for the Delta-MAC and is
+ * missing); it is pinned to the multipole remainder instead (test_theta_mac_error_is_bounded_by_the_multipole_remainder:
+ * every target outside r_b of every accepted cell, |a_exact - a_monopole| <= 3 M b^2 / (d - b)^4 per (target, cell) by
+ * brute force, the walk's force within the sum of these remainders of the O(N^2) sum, median error ~ theta^2.4).
  */
 #ifndef OTOO_ORACLE_H
 #define OTOO_ORACLE_H

@@ -105,6 +105,66 @@ def test_error_decreases_with_theta_and_lists_shrink(orc):
     assert inter[0] < inter[1] < inter[2] < inter[3]
 
 
+@pytest.mark.parametrize("dist", [0, 2])
+def test_theta_mac_error_is_bounded_by_the_multipole_remainder(orc, dist):
+    """The absolute accuracy of the theta-MAC (R7: accept iff the group's distance to the centre of mass exceeds
+    r_b = l/theta + s), pinned to what the mathematics fixes -- not to the oracle:
+    (1) geometry: every particle of a cell lies within (sqrt(3)/2) l + s of its centre of mass, every target farther than
+        r_b from it, so b/d < ((sqrt(3)/2) l + s) / (l/theta + s) < 1 for every (target, accepted cell), b = the cell's
+        largest particle distance from its centre of mass, by brute force;
+    (2) a monopole at the centre of mass has no dipole term: by Taylor's theorem with the third derivatives of 1/r
+        (largest multilinear value 6/r^4, radial) |a_exact - a_monopole| <= 3 M b^2 / (d - b)^4 per (target, cell);
+    (3) the oracle's force differs from the O(N^2) sum by no more than the sum of these remainders over its list;
+    (4) the median error grows as theta^2 ... theta^3 (quadrupole order) and stays below 0.005 theta^2.
+    Newtonian (eps = 0), so that (2) is the textbook bound."""
+    n, G, eps = 3000, 32, 0.0
+    pm = gen.plummer(n, 17)
+    t = orc.Tree(pm, 8)
+    t.set_dist_kind(dist)
+    ex = t.export()
+    xs = pm[ex["perm"].astype(np.int64), :3].astype(np.float64)          # positions in sorted order
+    ms = pm[ex["perm"].astype(np.int64), 3].astype(np.float64)
+    cm = ex["MP"][:, 1:4] / ex["MP"][:, :1]
+    M = ex["MP"][:, 0]
+    lvl = ex["cells"]["level"].astype(np.int64)
+    l = float(t.S) * 0.5 ** lvl
+    ref = np_direct(pm, eps)[ex["perm"].astype(np.int64)]                # direct sum, sorted order
+    med = {}
+    for theta in (0.2, 0.3, 0.45, 0.6, 0.9):
+        th = float(np.float32(theta))
+        r = t.gravity(eps, th, G)
+        a = r["acc_pot"][ex["perm"].astype(np.int64), :3]
+        err = np.linalg.norm(a - ref[:, :3], axis=1)
+        med[theta] = float(np.median(err / np.linalg.norm(ref[:, :3], axis=1)))
+        if theta not in (0.3, 0.6, 0.9):
+            continue
+        for g in range(0, t.n_groups(G), 9):
+            cells, parts = t.group_lists(th, G, g, r["n_cells"][g], r["n_parts"][g])
+            tg = np.arange(g * G, min((g + 1) * G, n))
+            bound = np.zeros(len(tg))
+            for c in cells.astype(np.int64):
+                f, k = int(ex["cells"]["first"][c]), int(ex["cells"]["count"][c])
+                dj = xs[f:f + k] - cm[c]
+                b = np.sqrt((dj ** 2).sum(1)).max()
+                rv = cm[c][None, :] - xs[tg]
+                d = np.sqrt((rv ** 2).sum(1))
+                rho = b / d
+                assert d.min() > (l[c] / th + ex["s"][c]) * (1 - 1e-6), (theta, g, c)          # every target outside r_b (R7, R8 / R25)
+                assert rho.max() <= ((np.sqrt(3) / 2) * l[c] + ex["s"][c]) / (l[c] / th + ex["s"][c]) * (1 + 1e-6), (theta, g, c)   # (1)
+                rem = 3.0 * M[c] * b * b / (d - b) ** 4
+                yv = xs[f:f + k][None, :, :] - xs[tg][:, None, :]
+                exact = (ms[f:f + k][None, :, None] * yv / ((yv ** 2).sum(-1) ** 1.5)[:, :, None]).sum(1)
+                mono = M[c] * rv / (d ** 3)[:, None]
+                assert (np.linalg.norm(exact - mono, axis=1) <= rem * (1 + 1e-9) + 1e-12).all(), (theta, g, c)                      # (2)
+                bound += rem
+            # (3); slack: the walk sees the centre of mass rounded to fp32 (R6)
+            assert (err[tg] <= bound + 1e-5 * np.linalg.norm(ref[tg, :3], axis=1)).all(), (theta, g)
+    ths = np.array(sorted(med))
+    slope = np.polyfit(np.log(ths), np.log([med[x] for x in ths]), 1)[0]
+    assert 2.0 < slope < 3.2, slope                                                                                                 # (4)
+    assert all(med[x] <= 0.005 * x * x for x in ths), med
+
+
 def test_plummer_potential_profile(orc):
     """Analytic Plummer potential phi(r) = -1/sqrt(r^2+1) (G=M=a=1), PAPER L193 workload."""
     n = 16384
