@@ -99,7 +99,10 @@ int otoo_version(void);
  * (L129; R2,R3), key sort (L133; R4), cells from the sorted keys (L135; R5), mass and centre of
  * mass bottom-up (L155; R6).  d_pos_mass: N x float4 (x,y,z,m), original order.  n_crit >= 1 is
  * the largest number of particles a leaf may hold (L41).  N = 0 is a no-op that leaves the
- * context "not built".  Synchronises `stream` once (to size the cell arrays). */
+ * context "not built".  Synchronises `stream` once (to size the cell arrays).
+ * A build that follows an otoo_gravity call also leaves the MAC radii r_b (R7) of that call's theta and a reset walk
+ * pool, from inside its bottom-up pass: the next otoo_gravity with the same theta launches its walk kernel alone
+ * (another theta, otoo_gravity_delta, or a second walk on the same tree compute / reset them as before; same results). */
 otoo_status otoo_build_tree(otoo_ctx* ctx, const float* d_pos_mass, int64_t N, int n_crit,
                             void* stream);
 
