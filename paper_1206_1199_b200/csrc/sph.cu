@@ -494,8 +494,8 @@ __device__ __forceinline__ void walk_sph_body(const SphParams& p) {
   uint32_t* stk = reinterpret_cast<uint32_t*>(smem_raw + OTOO_WALK_WARPS * OTOO_LIST_STRIDE * sizeof(float4)) +
                   warp * OTOO_WALK_STACK_MAX;
   SphVisitor<T, MODE, REC> v(p);
-  v.msk = reinterpret_cast<uint32_t*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (SphVisitor<T, MODE>::W * T * 32);
-  v.pbox = reinterpret_cast<float4*>(smem_raw + otoo_walk_smem_bytes_dev() + (size_t)OTOO_WALK_WARPS * SphVisitor<T, MODE>::W * T * 32 * sizeof(uint32_t)) +
+  v.msk = reinterpret_cast<uint32_t*>(smem_raw + otoo_walk_smem_bytes_dev()) + warp * (SphVisitor<T, MODE, REC>::W * T * 32);
+  v.pbox = reinterpret_cast<float4*>(smem_raw + otoo_walk_smem_bytes_dev() + (size_t)OTOO_WALK_WARPS * SphVisitor<T, MODE, REC>::W * T * 32 * sizeof(uint32_t)) +
            warp * (2 * OTOO_PIECES);
   v.lane_ = lane;
   walk_driver(p.c, v, list, stk, lane, (int64_t)blockIdx.x * OTOO_WALK_WARPS + warp);
