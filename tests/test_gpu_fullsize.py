@@ -135,6 +135,20 @@ def test_fullsize_sph(orc):
         rf = t.sph_force(h, rg.astype(np.float64), Pg.astype(np.float64), G, vel=vel2, groups=sel)
         vec_check("fullsize_sph:a_sph", out[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
         report("fullsize_sph:dudt", out[idx, 3], rf["acc_dudt"][idx, 3], rf["abs_sum"][idx, 1], pct=None)
+        steps_full = o.otoo_last_stats()["sum_steps"]
+        # the configuration bench.py times: stage 2 keeps stage 1's radii and starts from the leaves stage 1 opened
+        o.otoo_set_option("sph_reuse_radii", 1)
+        o.otoo_set_option("sph_reuse_walk", 1)
+        rho2, _ = o.otoo_sph_density(d_h, G)
+        out2 = o.otoo_sph_force(d_h, rho, P, G, vel=dev(vel2)).cpu().numpy()
+        st2 = o.otoo_last_stats()
+        nt2, _, npart2 = o.otoo_export_group_stats()
+        assert np.array_equal(nt2, ref["n_tests"]) and np.array_equal(npart2, ref["n_parts"])      # every group's counters
+        assert st2["sum_interactions"] == ref["candidates"]
+        assert st2["sum_steps"] < 0.75 * steps_full                                                # most groups did replay
+        vec_check("fullsize_sph:a_sph:replay", out2[idx], rf["acc_dudt"][idx], rf["abs_sum"][idx, 0], 99)
+        report("fullsize_sph:dudt:replay", out2[idx, 3], rf["acc_dudt"][idx, 3], rf["abs_sum"][idx, 1], pct=None)
+        assert float((rho2 - rho).abs().max()) <= 1e-6 * float(rho.abs().max())
     finally:
         o.close()
 
