@@ -88,6 +88,15 @@ def test_fullsize_gravity(orc, name):
         assert np.array_equal(rs["n_tests"], nt[sel])
         idx = np.concatenate([perm[g * G:min((g + 1) * G, n)] for g in sel])
         vec_check(f"fullsize_gravity[{name}:{order}]", out[idx], rs["acc_pot"][idx], rs["abs_sum"][idx], 99.9, FLOOR_FRAC_MAX_GRAVITY)
+        # the step bench.py times is a build AFTER a gravity call: r_b of that call's theta and the pool reset come with
+        # the build, the call launches the walk kernel alone -- same radii bit for bit, same counters of every group
+        o.otoo_build_tree(d_pm, cfg["n_crit"])
+        out_b = o.otoo_gravity(eps, theta, G).cpu().numpy()
+        assert o.otoo_last_stats()["launches"] == 1
+        assert np.array_equal(o.otoo_export_tree()["rb2"].view(np.uint32), t.rb2(theta).view(np.uint32))
+        nt_b, nc_b, np_b = o.otoo_export_group_stats()
+        assert np.array_equal(nt_b, nt) and np.array_equal(nc_b, nc) and np.array_equal(np_b, npart)
+        assert np.abs(out_b - out).max() <= 1e-4 * np.abs(out[:, :3]).max()      # (sums: the order of the atomics)
         pe = np.abs(out[idx, 3] - rs["acc_pot"][idx, 3]) / np.abs(rs["acc_pot"][idx, 3])
         ptol = np.concatenate([np.full(min((g + 1) * G, n) - g * G, phi_tol(lengths[g])) for g in sel])   # 1e-5 up to 1.8 M entries
         assert (pe <= ptol).all(), (pe.max(), float((pe / ptol).max()))
