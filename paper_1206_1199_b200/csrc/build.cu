@@ -192,22 +192,20 @@ struct CellOut {
 __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __restrict__ info, const uint64_t* __restrict__ key, int64_t n,
                                                           const uint32_t* __restrict__ blk_off, const CellOut o) {
   __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
-  __shared__ uint8_t slo[256 + OTOO_PLACE_WIN];  // lo of the block's slots and of the OTOO_PLACE_WIN slots after them (0 past the end)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  if (lane < OTOO_NLEV) wc[warp][lane] = 0;      // (each warp its own row: no block barrier before the ballots)
+  __syncwarp();
   // (fetched now, used after two block barriers: the load's latency was a fifth of the kernel's stall samples)
   const uint32_t my_off = threadIdx.x < OTOO_NLEV ? blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x] : 0u;
   const int64_t s0 = (int64_t)blockIdx.x * 256, s = s0 + threadIdx.x;
   int lo = OTOO_NLEV, LL = -1;
   if (s < n) { const uint32_t inf = info[s]; lo = (int)(inf & 0xFF); LL = (int)(inf >> 8); }
-  slo[threadIdx.x] = (uint8_t)(s < n ? lo : 0);
-  if (threadIdx.x < OTOO_PLACE_WIN) slo[256 + threadIdx.x] = s + 256 < n ? (uint8_t)(info[s + 256] & 0xFF) : (uint8_t)0;
-  __syncthreads();
+  const int lo_next = s + 32 < n ? (int)(info[s + 32] & 0xFF) : 0;      // lo of the slot 32 further on (0 past the end: ends every range)
   const bool has = lo <= LL;
   const int wlo = __reduce_min_sync(0xFFFFFFFFu, has ? lo : OTOO_NLEV), whi = __reduce_max_sync(0xFFFFFFFFu, has ? LL : -1);
   // the leaf's particle count = distance to the next slot that starts a range of the leaf's level or a coarser one:
   // per level a ballot over the warp's 32 slots and one over the 32 slots after them
-  const int lo_term = s < n ? lo : 0, lo_next = (int)slo[threadIdx.x + 32];      // (slots past the end end every range)
+  const int lo_term = s < n ? lo : 0;                                             // (slots past the end end every range)
   uint32_t count = 0;
   for (int l = wlo; l <= whi; l++) {
     const unsigned b = __ballot_sync(0xFFFFFFFFu, lo <= l && l <= LL);
@@ -228,9 +226,12 @@ __global__ void __launch_bounds__(256) place_cells_kernel(const uint32_t* __rest
   if (has && (count == 0u || LL == 0)) {
     if (LL == 0) count = (uint32_t)n;
     else {
-      int j = threadIdx.x + 1;
-      while (j < 256 + OTOO_PLACE_WIN && (int)slo[j] > LL) j++;
-      if (j < 256 + OTOO_PLACE_WIN) count = (uint32_t)(j - threadIdx.x);
+      // not within the 63 - lane slots the ballots cover (a leaf of more than 32 particles: n_crit > 32 or level 21):
+      // the next OTOO_PLACE_WIN slots one by one, then a search on the key prefix
+      int64_t j = s + 1;
+      const int64_t jend = s + OTOO_PLACE_WIN < n ? s + OTOO_PLACE_WIN : n;
+      while (j < jend && (int)(info[j] & 0xFF) > LL) j++;
+      if (j < jend || j == n) count = (uint32_t)(j - s);
       else {                                       // beyond the window: gallop, then bisect for the end of the prefix range
         const int sh = 3 * (OTOO_MAXLEV - LL);
         const uint64_t prefix = key[s] >> sh;
