@@ -60,9 +60,9 @@ __global__ void __launch_bounds__(256) sph_radii_kernel(const float4* __restrict
                                                         unsigned long long* acc /* 2 per cell */, uint32_t* out32 /* 2 per cell */) {
   __shared__ uint32_t wc[8][OTOO_NLEV];          // level-l cells the warp starts, then the canonical index of its first one
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (threadIdx.x < 8 * OTOO_NLEV) (&wc[0][0])[threadIdx.x] = 0;
+  if (lane < OTOO_NLEV) wc[warp][lane] = 0;      // (each warp its own row: no block barrier before the ballots)
+  __syncwarp();
   const uint32_t my_off = threadIdx.x < OTOO_NLEV ? blk_off[(size_t)threadIdx.x * gridDim.x + blockIdx.x] : 0u;   // (used after the next barrier)
-  __syncthreads();
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = s < n;
   int lo = OTOO_NLEV, LL = -1;
